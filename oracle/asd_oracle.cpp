@@ -1,0 +1,596 @@
+// ============================================================================
+// oracle/asd_oracle.cpp -- plain fp64 CPU oracle for the atomistic spin-dynamics
+// (ASD) window of arXiv 2502.02236 (Gija et al., multiscale HAMR model).
+//
+// THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke()
+// and bench.py's cpu_baseline / --impl reference legs may load it.  It shares no code,
+// header, table or constant generator with the CUDA library under
+// paper_2502_02236_b200/csrc/ and neither includes the other.
+//
+// What it computes, and where the definition comes from (P:<n> = /root/reference/PAPER.md
+// line n; S:<x> = SURVEY.md section 8(c) item x; D:<x> = DESIGN.md reading x):
+//   * stochastic LLG, Eq. (1), P:35          -> llg_rhs()          (LL form, S:O4)
+//   * thermal field sigma, P:38               -> sigma_T()          (Tesla units, S:O3)
+//   * exchange field Eq. (2), P:46-48         -> field_at()
+//   * uniaxial anisotropy Eq. (3), P:50-52    -> field_at()
+//   * stochastic Heun step                    -> orc_step_heun()    (S:O4, BASELINE north_star)
+//   * atomistic->macrocell transfer Eq. (6), P:64-66 -> orc_shift_window() outgoing part
+//   * macrocell->atomistic cone thermalisation, P:68 -> seed_site()  (S:S3 reading)
+//   * Philox4x32-10 (Salmon et al., SC'11, public definition) -> philox4x32_10()
+//
+// Everything is written in the paper's order and notation, one site at a time, with
+// explicit coordinate loops; no blocking, fusion or reordering.  OpenMP is used only
+// over sites inside one Jacobi stage (each site reads the OLD configuration), which does
+// not change any result.
+//
+// Units: B = mu_0 H in Tesla, energies in Joule, mu_s in J/T, gamma in rad s^-1 T^-1.
+//
+// Pins (tests/test_oracle_*.py): Philox vs ATen host engine; single-spin damped
+// precession closed form; Langevin function; monotone energy; brute-force energy
+// gradient; |S|=1; spin-wave dispersion (fixes exchange normalisation and the L1_0
+// shell geometry); simple-cubic T_C = 1.44 J/k_B;
+// shift index exactness; seeded-slab magnetisation magnitude (P:68 purpose clause).
+// "parity unpinned": bit-pattern outcomes / read-head scans -- not computed here.
+// ============================================================================
+#include <cmath>
+#include <cstdint>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+constexpr double kPi = 3.14159265358979323846264338327950288;
+constexpr double kBoltzmann = 1.380649e-23;  // J/K (SI exact)
+
+// ---------------------------------------------------------------------------
+// Philox4x32-10.  Public definition: Salmon, Moraes, Dror, Shaw, SC'11.
+// One round: (c0,c1,c2,c3) -> (hi(M1*c2)^c1^k0, lo(M1*c2), hi(M0*c0)^c3^k1, lo(M0*c0)),
+// M0 = 0xD2511F53, M1 = 0xCD9E8D57; key bumped by (0x9E3779B9, 0xBB67AE85) between rounds.
+// ---------------------------------------------------------------------------
+void philox4x32_10(const uint32_t key_in[2], const uint32_t ctr_in[4], uint32_t out[4]) {
+  uint32_t k0 = key_in[0], k1 = key_in[1];
+  uint32_t c0 = ctr_in[0], c1 = ctr_in[1], c2 = ctr_in[2], c3 = ctr_in[3];
+  for (int round = 0; round < 10; ++round) {
+    if (round > 0) {
+      k0 += 0x9E3779B9u;
+      k1 += 0xBB67AE85u;
+    }
+    const uint64_t p0 = (uint64_t)0xD2511F53u * (uint64_t)c0;
+    const uint64_t p1 = (uint64_t)0xCD9E8D57u * (uint64_t)c2;
+    const uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+    const uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+    const uint32_t n0 = hi1 ^ c1 ^ k0;
+    const uint32_t n1 = lo1;
+    const uint32_t n2 = hi0 ^ c3 ^ k1;
+    const uint32_t n3 = lo0;
+    c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// S:R1 keying.  key = (seed lo, seed hi); counter = (n lo, n hi, g lo, g hi | stream<<28).
+// n = step index before the step (thermal noise) or the pass number (shift seeding);
+// g = GLOBAL site id (gx*nz + k)*ny + j, so noise follows the atom, not the memory slot.
+void philox_block(uint64_t seed, uint64_t n, uint64_t g, uint32_t stream, uint32_t out[4]) {
+  const uint32_t key[2] = {(uint32_t)(seed & 0xFFFFFFFFull), (uint32_t)(seed >> 32)};
+  const uint32_t ctr[4] = {(uint32_t)(n & 0xFFFFFFFFull), (uint32_t)(n >> 32),
+                           (uint32_t)(g & 0xFFFFFFFFull), (uint32_t)(g >> 32) | (stream << 28)};
+  philox4x32_10(key, ctr, out);
+}
+
+// S:R2.  u = ((r >> 9) + 1/2) * 2^-23 in (0,1); exactly representable in fp32 and fp64.
+inline double uniform_from_u32(uint32_t r) { return ((double)(r >> 9) + 0.5) * (1.0 / 8388608.0); }
+
+// S:R3.  Box-Muller: xi_x = rho0 cos(2 pi u1), xi_y = rho0 sin(2 pi u1), rho0 = sqrt(-2 ln u0);
+// xi_z = rho2 cos(2 pi u3), rho2 = sqrt(-2 ln u2).  The fourth normal is discarded.
+void normals3(uint64_t seed, uint64_t step, uint64_t g, double xi[3]) {
+  uint32_t r[4];
+  philox_block(seed, step, g, 0u, r);
+  const double u0 = uniform_from_u32(r[0]), u1 = uniform_from_u32(r[1]);
+  const double u2 = uniform_from_u32(r[2]), u3 = uniform_from_u32(r[3]);
+  const double rho0 = std::sqrt(-2.0 * std::log(u0));
+  const double rho2 = std::sqrt(-2.0 * std::log(u2));
+  xi[0] = rho0 * std::cos(2.0 * kPi * u1);
+  xi[1] = rho0 * std::sin(2.0 * kPi * u1);
+  xi[2] = rho2 * std::cos(2.0 * kPi * u3);
+}
+
+// theta_max = root in [0, pi] of sin(theta)/theta = m  (S:S3: the distribution P:68 states --
+// polar angle uniform on [0, theta_max], free azimuth -- has <cos theta> = sin(theta_max)/theta_max,
+// so this root is what "reproduces the correct magnetization magnitude M").
+double theta_max_of_m(double m) {
+  if (m >= 1.0) return 0.0;
+  if (m <= 0.0) return kPi;
+  double lo = 0.0, hi = kPi;  // sin(x)/x decreases monotonically from 1 to 0 on [0, pi]
+  for (int it = 0; it < 200; ++it) {
+    const double mid = 0.5 * (lo + hi);
+    const double v = (mid == 0.0) ? 1.0 : std::sin(mid) / mid;
+    if (v > m) lo = mid; else hi = mid;
+  }
+  return 0.5 * (lo + hi);
+}
+
+struct Oracle {
+  int lattice = 0;               // 0 = simple cubic, 1 = L1_0 Fe sublattice (simple tetragonal axes)
+  int nx = 0, ny = 0, nz = 0;    // x along track, z film normal
+  int pbc[3] = {0, 0, 0};
+  double mu_s = 0, lambda = 0, gamma = 0, dt = 0;
+  double J[3] = {0, 0, 0};
+  int64_t track_nx = 0, x0 = 0;
+  std::vector<int32_t> grain_map;  // [track_nx * ny], -1 = vacant column
+  int n_grains = 0;
+  std::vector<double> ku;          // [n_grains]  J per atom
+  std::vector<double> axis;        // [n_grains*3]
+  int macro[3] = {1, 1, 1};
+  int ell_width = 0;               // > 0: general ELL override
+  std::vector<int32_t> ell_idx;    // [N * ell_width] site-major, -1 = none
+  std::vector<double> ell_J;       // [N * ell_width] Joule
+  uint64_t seed = 0;
+  int64_t step = 0, shift = 0, pass = 0;
+  double scale = 1.0;              // B_app = scale * B
+  int64_t N = 0;
+  std::vector<double> sx, sy, sz;  // spins (0 on vacant sites)
+  std::vector<double> T, Bx, By, Bz;
+  // track store (macrocells over the whole track)
+  int64_t ncx = 0, ncy = 0, ncz = 0;
+  std::vector<double> out_sum;     // [ncell*3]  sum of m_j (Eq. 6 with mu_S/V factored out)
+  std::vector<int64_t> out_cnt;    // [ncell]
+  std::vector<double> init_mean;   // [ncell*3]  what lies ahead of the window
+  int threads = 0;
+
+  int64_t site(int i, int k, int j) const { return ((int64_t)i * nz + k) * ny + j; }
+  int32_t grain_of(int i, int j) const { return grain_map[(size_t)((x0 + i) * ny + j)]; }
+  int64_t cell_of(int64_t gx, int j, int k) const {
+    return ((gx / macro[0]) * ncy + (j / macro[1])) * ncz + (k / macro[2]);
+  }
+};
+
+// sigma_i = sqrt(2 lambda k_B T_i / (gamma mu_s dt))  [Tesla]; P:38 with mu_0 absorbed (B = mu_0 H).
+inline double sigma_T(const Oracle& o, double T) {
+  return std::sqrt(2.0 * o.lambda * kBoltzmann * T / (o.gamma * o.mu_s * o.dt));
+}
+
+// Neighbour shells (S:O3).  SC: 6 nn, J[0].  L1_0 Fe sublattice in its own simple-tetragonal
+// axes: 4 in-plane nn J[0], 2 out-of-plane J[1], 4 in-plane nnn J[2] ("4 nearest + 6 next nearest",
+// z = 10; geometry fixed by A_L10 = 3J/2a, see the spin-wave pin).
+struct Offset { int dx, dy, dz, shell; };
+const Offset kOffsetsSC[6] = {{1,0,0,0},{-1,0,0,0},{0,1,0,0},{0,-1,0,0},{0,0,1,0},{0,0,-1,0}};
+const Offset kOffsetsL10[10] = {{1,0,0,0},{-1,0,0,0},{0,1,0,0},{0,-1,0,0},
+                                {0,0,1,1},{0,0,-1,1},
+                                {1,1,0,2},{1,-1,0,2},{-1,1,0,2},{-1,-1,0,2}};
+
+// Wrap or reject a coordinate.  Returns false when the neighbour does not exist (open boundary).
+inline bool wrap(int& c, int n, int periodic) {
+  if (c >= 0 && c < n) return true;
+  if (!periodic) return false;
+  c = (c % n + n) % n;
+  return true;
+}
+
+// Exchange sum  sum_j J_ij X_j  (Joule), Eq. (2) numerator, for site (i,k,j) in configuration X.
+// A bond is kept only if the neighbour exists, both ends are magnetic and in the same grain
+// (exchange-decoupled grains).
+void exchange_sum(const Oracle& o, const double* X0, const double* X1, const double* X2,
+                  int i, int k, int j, double e[3]) {
+  e[0] = e[1] = e[2] = 0.0;
+  const int64_t l = o.site(i, k, j);
+  if (o.ell_width > 0) {
+    for (int s = 0; s < o.ell_width; ++s) {
+      const int32_t n = o.ell_idx[(size_t)(l * o.ell_width + s)];
+      if (n < 0) continue;
+      const double Jij = o.ell_J[(size_t)(l * o.ell_width + s)];
+      e[0] += Jij * X0[n]; e[1] += Jij * X1[n]; e[2] += Jij * X2[n];
+    }
+    return;
+  }
+  const int32_t g = o.grain_of(i, j);
+  const Offset* offs = (o.lattice == 0) ? kOffsetsSC : kOffsetsL10;
+  const int noff = (o.lattice == 0) ? 6 : 10;
+  for (int s = 0; s < noff; ++s) {
+    int ii = i + offs[s].dx, jj = j + offs[s].dy, kk = k + offs[s].dz;
+    if (!wrap(ii, o.nx, o.pbc[0])) continue;
+    if (!wrap(jj, o.ny, o.pbc[1])) continue;
+    if (!wrap(kk, o.nz, o.pbc[2])) continue;
+    const int32_t gn = o.grain_of(ii, jj);
+    if (gn < 0 || gn != g) continue;
+    const int64_t n = o.site(ii, kk, jj);
+    const double Jij = o.J[offs[s].shell];
+    e[0] += Jij * X0[n]; e[1] += Jij * X1[n]; e[2] += Jij * X2[n];
+  }
+}
+
+// Effective field in Tesla at a magnetic site (S:O3):
+// B_i(X) = (1/mu_s) sum_j J_ij X_j + (2 k_u,g/mu_s)(X_i.e_g) e_g + s*B_app,i + sigma_i xi_i.
+void field_at(const Oracle& o, const double* X0, const double* X1, const double* X2,
+              int i, int k, int j, const double* xi /* may be null */, double B[3]) {
+  const int64_t l = o.site(i, k, j);
+  const int32_t g = o.grain_of(i, j);
+  double e[3];
+  exchange_sum(o, X0, X1, X2, i, k, j, e);
+  B[0] = e[0] / o.mu_s; B[1] = e[1] / o.mu_s; B[2] = e[2] / o.mu_s;        // Eq. (2)
+  const double ex = o.axis[3 * g], ey = o.axis[3 * g + 1], ez = o.axis[3 * g + 2];
+  const double d = X0[l] * ex + X1[l] * ey + X2[l] * ez;
+  const double ca = 2.0 * o.ku[g] / o.mu_s * d;                             // Eq. (3)
+  B[0] += ca * ex; B[1] += ca * ey; B[2] += ca * ez;
+  B[0] += o.scale * o.Bx[l]; B[1] += o.scale * o.By[l]; B[2] += o.scale * o.Bz[l];
+  if (xi) {
+    const double sg = sigma_T(o, o.T[l]);
+    B[0] += sg * xi[0]; B[1] += sg * xi[1]; B[2] += sg * xi[2];
+  }
+}
+
+// f(S,B) = -gamma/(1+lambda^2) [ S x B + lambda S x (S x B) ]  -- Eq. (1) solved for dm/dt
+// (cross Eq. (1) with m and use m.dm/dt = 0; S:O4).
+inline void llg_rhs(const Oracle& o, const double S[3], const double B[3], double f[3]) {
+  const double a0 = S[1] * B[2] - S[2] * B[1];
+  const double a1 = S[2] * B[0] - S[0] * B[2];
+  const double a2 = S[0] * B[1] - S[1] * B[0];
+  const double b0 = S[1] * a2 - S[2] * a1;
+  const double b1 = S[2] * a0 - S[0] * a2;
+  const double b2 = S[0] * a1 - S[1] * a0;
+  const double c = -o.gamma / (1.0 + o.lambda * o.lambda);
+  f[0] = c * (a0 + o.lambda * b0);
+  f[1] = c * (a1 + o.lambda * b1);
+  f[2] = c * (a2 + o.lambda * b2);
+}
+
+// Threads for the per-stage site loops: the caller's choice, else all cores for large lattices and one
+// for tiny ones (forking a team costs more than a few hundred sites of work).  Never changes a result.
+inline int thread_count(const Oracle& o) {
+#ifdef _OPENMP
+  if (o.threads > 0) return o.threads;
+  return o.N < 4096 ? 1 : omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+// One stochastic Heun step, Jacobi order (S:O4):
+// 1 draw xi_i; 2 k1 = f(S, B(S)); 3 S~ = (S + dt k1)/|.|; 4 k2 = f(S~, B(S~)) with the SAME xi_i;
+// 5 S <- (S + dt/2 (k1+k2))/|.|; 6 n <- n+1.  Vacant sites are skipped and stay 0.
+void heun_step(Oracle& o) {
+  const int64_t N = o.N;
+  std::vector<double> xi(3 * (size_t)N, 0.0), k1(3 * (size_t)N, 0.0);
+  std::vector<double> tx((size_t)N, 0.0), ty((size_t)N, 0.0), tz((size_t)N, 0.0);
+  const int nx = o.nx, ny = o.ny, nz = o.nz;
+  const int nt = thread_count(o);
+#pragma omp parallel for collapse(2) schedule(static) num_threads(nt)
+  for (int i = 0; i < nx; ++i)
+    for (int k = 0; k < nz; ++k)
+      for (int j = 0; j < ny; ++j) {
+        if (o.grain_of(i, j) < 0) continue;
+        const int64_t l = o.site(i, k, j);
+        const uint64_t g = (uint64_t)(((o.x0 + i) * nz + k) * ny + j);
+        normals3(o.seed, (uint64_t)o.step, g, &xi[3 * l]);
+        double B[3], f[3];
+        field_at(o, o.sx.data(), o.sy.data(), o.sz.data(), i, k, j, &xi[3 * l], B);
+        const double S[3] = {o.sx[l], o.sy[l], o.sz[l]};
+        llg_rhs(o, S, B, f);
+        k1[3 * l] = f[0]; k1[3 * l + 1] = f[1]; k1[3 * l + 2] = f[2];
+        const double p0 = S[0] + o.dt * f[0], p1 = S[1] + o.dt * f[1], p2 = S[2] + o.dt * f[2];
+        const double nrm = std::sqrt(p0 * p0 + p1 * p1 + p2 * p2);
+        tx[l] = p0 / nrm; ty[l] = p1 / nrm; tz[l] = p2 / nrm;
+      }
+  std::vector<double> n0((size_t)N, 0.0), n1((size_t)N, 0.0), n2((size_t)N, 0.0);
+#pragma omp parallel for collapse(2) schedule(static) num_threads(nt)
+  for (int i = 0; i < nx; ++i)
+    for (int k = 0; k < nz; ++k)
+      for (int j = 0; j < ny; ++j) {
+        if (o.grain_of(i, j) < 0) continue;
+        const int64_t l = o.site(i, k, j);
+        double B[3], f[3];
+        field_at(o, tx.data(), ty.data(), tz.data(), i, k, j, &xi[3 * l], B);
+        const double St[3] = {tx[l], ty[l], tz[l]};
+        llg_rhs(o, St, B, f);
+        const double q0 = o.sx[l] + 0.5 * o.dt * (k1[3 * l] + f[0]);
+        const double q1 = o.sy[l] + 0.5 * o.dt * (k1[3 * l + 1] + f[1]);
+        const double q2 = o.sz[l] + 0.5 * o.dt * (k1[3 * l + 2] + f[2]);
+        const double nrm = std::sqrt(q0 * q0 + q1 * q1 + q2 * q2);
+        n0[l] = q0 / nrm; n1[l] = q1 / nrm; n2[l] = q2 / nrm;
+      }
+  o.sx.swap(n0); o.sy.swap(n1); o.sz.swap(n2);
+  o.step += 1;
+}
+
+// Incoming-slab seeding for one magnetic site (S:S3).  v = track mean spin of the site's
+// macrocell, m = min(1,|v|), n^ = v/|v| (z^ if v = 0), theta = theta_max(m) u0, phi = 2 pi u1
+// (Philox stream 1, counter n := pass), S = sin(theta)cos(phi) e1 + sin(theta)sin(phi) e2 + cos(theta) n^,
+// e1 = normalise(n^ x x^) (n^ x y^ if |n^_x| > 0.9), e2 = n^ x e1.
+void seed_site(const Oracle& o, int64_t gx, int k, int j, double S[3]) {
+  const int64_t c = o.cell_of(gx, j, k);
+  const double v0 = o.init_mean[3 * c], v1 = o.init_mean[3 * c + 1], v2 = o.init_mean[3 * c + 2];
+  const double vn = std::sqrt(v0 * v0 + v1 * v1 + v2 * v2);
+  const double m = std::fmin(1.0, vn);
+  double n[3] = {0.0, 0.0, 1.0};
+  if (vn > 0.0) { n[0] = v0 / vn; n[1] = v1 / vn; n[2] = v2 / vn; }
+  double e1[3];
+  if (std::fabs(n[0]) > 0.9) {  // n x y^ = (-n_z, 0, n_x)
+    e1[0] = -n[2]; e1[1] = 0.0; e1[2] = n[0];
+  } else {                      // n x x^ = (0, n_z, -n_y)
+    e1[0] = 0.0; e1[1] = n[2]; e1[2] = -n[1];
+  }
+  const double e1n = std::sqrt(e1[0] * e1[0] + e1[1] * e1[1] + e1[2] * e1[2]);
+  e1[0] /= e1n; e1[1] /= e1n; e1[2] /= e1n;
+  const double e2[3] = {n[1] * e1[2] - n[2] * e1[1], n[2] * e1[0] - n[0] * e1[2],
+                        n[0] * e1[1] - n[1] * e1[0]};
+  uint32_t r[4];
+  const uint64_t g = (uint64_t)((gx * o.nz + k) * o.ny + j);
+  philox_block(o.seed, (uint64_t)o.pass, g, 1u, r);
+  const double theta = theta_max_of_m(m) * uniform_from_u32(r[0]);
+  const double phi = 2.0 * kPi * uniform_from_u32(r[1]);
+  const double st = std::sin(theta), ct = std::cos(theta), cp = std::cos(phi), sp = std::sin(phi);
+  for (int a = 0; a < 3; ++a) S[a] = st * cp * e1[a] + st * sp * e2[a] + ct * n[a];
+}
+
+}  // namespace
+
+// ============================================================================
+// C interface for ctypes (oracle/asd_oracle.py).  Its own description struct: nothing here is
+// shared with include/asd.h.
+// ============================================================================
+extern "C" {
+
+struct orc_desc {
+  int32_t lattice, nx, ny, nz;
+  int32_t pbc[3];
+  int32_t n_grains;
+  double mu_s, lambda, gamma, dt;
+  double J[3];
+  int64_t track_nx, x0;
+  const int32_t* grain_map;   // [track_nx*ny]
+  const double* grain_ku;     // [n_grains]
+  const double* grain_axis;   // [n_grains*3]
+  int32_t macro[3];
+  int32_t ell_width;
+  const int32_t* ell_idx;     // [N*ell_width] or null
+  const double* ell_J;        // [N*ell_width] or null
+  uint64_t seed;
+};
+
+void* orc_create(const orc_desc* d) {
+  if (!d || d->nx < 1 || d->ny < 1 || d->nz < 1) return nullptr;
+  for (int a = 0; a < 3; ++a) {
+    const int n = (a == 0) ? d->nx : (a == 1 ? d->ny : d->nz);
+    if (d->pbc[a] && n < 3) return nullptr;  // S:Q17
+  }
+  if (d->track_nx < d->x0 + d->nx || d->x0 < 0) return nullptr;
+  Oracle* o = new Oracle();
+  o->lattice = d->lattice; o->nx = d->nx; o->ny = d->ny; o->nz = d->nz;
+  for (int a = 0; a < 3; ++a) { o->pbc[a] = d->pbc[a]; o->J[a] = d->J[a]; o->macro[a] = d->macro[a] > 0 ? d->macro[a] : 1; }
+  o->mu_s = d->mu_s; o->lambda = d->lambda; o->gamma = d->gamma; o->dt = d->dt;
+  o->track_nx = d->track_nx; o->x0 = d->x0; o->n_grains = d->n_grains; o->seed = d->seed;
+  o->grain_map.assign(d->grain_map, d->grain_map + (size_t)(d->track_nx * d->ny));
+  o->ku.assign(d->grain_ku, d->grain_ku + d->n_grains);
+  o->axis.assign(d->grain_axis, d->grain_axis + 3 * (size_t)d->n_grains);
+  o->N = (int64_t)d->nx * d->ny * d->nz;
+  if (d->ell_width > 0 && d->ell_idx && d->ell_J) {
+    o->ell_width = d->ell_width;
+    o->ell_idx.assign(d->ell_idx, d->ell_idx + (size_t)(o->N * d->ell_width));
+    o->ell_J.assign(d->ell_J, d->ell_J + (size_t)(o->N * d->ell_width));
+  }
+  const size_t N = (size_t)o->N;
+  o->sx.assign(N, 0.0); o->sy.assign(N, 0.0); o->sz.assign(N, 0.0);
+  o->T.assign(N, 0.0); o->Bx.assign(N, 0.0); o->By.assign(N, 0.0); o->Bz.assign(N, 0.0);
+  o->ncx = (o->track_nx + o->macro[0] - 1) / o->macro[0];
+  o->ncy = (o->ny + o->macro[1] - 1) / o->macro[1];
+  o->ncz = (o->nz + o->macro[2] - 1) / o->macro[2];
+  const size_t nc = (size_t)(o->ncx * o->ncy * o->ncz);
+  o->out_sum.assign(3 * nc, 0.0); o->out_cnt.assign(nc, 0);
+  o->init_mean.assign(3 * nc, 0.0);
+  for (size_t c = 0; c < nc; ++c) o->init_mean[3 * c + 2] = 1.0;  // default track state +z, m0 = 1
+  return o;
+}
+
+void orc_destroy(void* h) { delete static_cast<Oracle*>(h); }
+
+void orc_set_threads(void* h, int n) {
+  static_cast<Oracle*>(h)->threads = n;   // 0 = automatic (see thread_count)
+}
+
+int orc_max_threads() {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+// fp32 inputs (the same arrays the GPU gets), widened without renormalising (S:O1); vacant -> 0.
+void orc_set_spins(void* h, const float* sx, const float* sy, const float* sz) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  for (int i = 0; i < o.nx; ++i)
+    for (int k = 0; k < o.nz; ++k)
+      for (int j = 0; j < o.ny; ++j) {
+        const int64_t l = o.site(i, k, j);
+        const bool mag = o.grain_of(i, j) >= 0;
+        o.sx[l] = mag ? (double)sx[l] : 0.0;
+        o.sy[l] = mag ? (double)sy[l] : 0.0;
+        o.sz[l] = mag ? (double)sz[l] : 0.0;
+      }
+}
+
+void orc_get_spins(void* h, double* sx, double* sy, double* sz) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  std::memcpy(sx, o.sx.data(), sizeof(double) * (size_t)o.N);
+  std::memcpy(sy, o.sy.data(), sizeof(double) * (size_t)o.N);
+  std::memcpy(sz, o.sz.data(), sizeof(double) * (size_t)o.N);
+}
+
+void orc_set_fields(void* h, const float* T, const float* Bx, const float* By, const float* Bz) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  for (int64_t l = 0; l < o.N; ++l) {
+    if (T) o.T[l] = (double)T[l];
+    if (Bx) o.Bx[l] = (double)Bx[l];
+    if (By) o.By[l] = (double)By[l];
+    if (Bz) o.Bz[l] = (double)Bz[l];
+  }
+}
+
+void orc_set_field_scale(void* h, float s) { static_cast<Oracle*>(h)->scale = (double)s; }
+
+void orc_step_heun(void* h, int64_t n) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  for (int64_t s = 0; s < n; ++s) heun_step(o);
+}
+
+// Deterministic field (no noise) or field with the noise of the current step counter, Tesla.
+void orc_field(void* h, int with_noise, double* bx, double* by, double* bz) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  for (int i = 0; i < o.nx; ++i)
+    for (int k = 0; k < o.nz; ++k)
+      for (int j = 0; j < o.ny; ++j) {
+        const int64_t l = o.site(i, k, j);
+        bx[l] = by[l] = bz[l] = 0.0;
+        if (o.grain_of(i, j) < 0) continue;
+        double xi[3], B[3];
+        if (with_noise) normals3(o.seed, (uint64_t)o.step, (uint64_t)(((o.x0 + i) * o.nz + k) * o.ny + j), xi);
+        field_at(o, o.sx.data(), o.sy.data(), o.sz.data(), i, k, j, with_noise ? xi : nullptr, B);
+        bx[l] = B[0]; by[l] = B[1]; bz[l] = B[2];
+      }
+}
+
+// E = -1/2 sum_i sum_{j in N(i)} J_ij S_i.S_j - sum_i k_u,g (S_i.e_g)^2 - mu_s sum_i s B_app,i.S_i
+// (each bond once; the convention under which Eq. (8) gives T_C = eps z J / 3 k_B; S:O3).
+double orc_energy(void* h) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  double E = 0.0;
+  for (int i = 0; i < o.nx; ++i)
+    for (int k = 0; k < o.nz; ++k)
+      for (int j = 0; j < o.ny; ++j) {
+        const int32_t g = o.grain_of(i, j);
+        if (g < 0) continue;
+        const int64_t l = o.site(i, k, j);
+        double e[3];
+        exchange_sum(o, o.sx.data(), o.sy.data(), o.sz.data(), i, k, j, e);
+        E -= 0.5 * (o.sx[l] * e[0] + o.sy[l] * e[1] + o.sz[l] * e[2]);
+        const double d = o.sx[l] * o.axis[3 * g] + o.sy[l] * o.axis[3 * g + 1] + o.sz[l] * o.axis[3 * g + 2];
+        E -= o.ku[g] * d * d;
+        E -= o.mu_s * o.scale * (o.Bx[l] * o.sx[l] + o.By[l] * o.sy[l] + o.Bz[l] * o.sz[l]);
+      }
+  return E;
+}
+
+// m = sum_{magnetic i} S_i / N_mag  (Eq. (6) with V = whole window; S:O6).
+void orc_magnetisation(void* h, double m[3], double* n_magnetic) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  double s0 = 0, s1 = 0, s2 = 0; int64_t cnt = 0;
+  for (int i = 0; i < o.nx; ++i)
+    for (int k = 0; k < o.nz; ++k)
+      for (int j = 0; j < o.ny; ++j) {
+        if (o.grain_of(i, j) < 0) continue;
+        const int64_t l = o.site(i, k, j);
+        s0 += o.sx[l]; s1 += o.sy[l]; s2 += o.sz[l]; ++cnt;
+      }
+  const double inv = cnt > 0 ? 1.0 / (double)cnt : 0.0;
+  m[0] = s0 * inv; m[1] = s1 * inv; m[2] = s2 * inv;
+  if (n_magnetic) *n_magnetic = (double)cnt;
+}
+
+void orc_grain_magnetisation(void* h, double* m /* [n_grains*3] */) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  std::vector<double> s(3 * (size_t)o.n_grains, 0.0); std::vector<int64_t> c((size_t)o.n_grains, 0);
+  for (int i = 0; i < o.nx; ++i)
+    for (int k = 0; k < o.nz; ++k)
+      for (int j = 0; j < o.ny; ++j) {
+        const int32_t g = o.grain_of(i, j);
+        if (g < 0) continue;
+        const int64_t l = o.site(i, k, j);
+        s[3 * g] += o.sx[l]; s[3 * g + 1] += o.sy[l]; s[3 * g + 2] += o.sz[l]; ++c[g];
+      }
+  for (int g = 0; g < o.n_grains; ++g)
+    for (int a = 0; a < 3; ++a) m[3 * g + a] = c[g] > 0 ? s[3 * g + a] / (double)c[g] : 0.0;
+}
+
+// Window shift by p planes (S:O5).
+int orc_shift_window(void* h, int32_t p) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  if (p < 1 || p > o.nx) return 1;
+  if (o.ell_width > 0) return 5;                       // general ELL cannot follow the window
+  if (o.x0 + p + o.nx > o.track_nx) return 1;          // grain map must cover the new window
+  const int nx = o.nx, ny = o.ny, nz = o.nz;
+  // S2 outgoing: planes i < p, magnetic sites only, ascending l.
+  for (int i = 0; i < p; ++i)
+    for (int k = 0; k < nz; ++k)
+      for (int j = 0; j < ny; ++j) {
+        if (o.grain_of(i, j) < 0) continue;
+        const int64_t l = o.site(i, k, j);
+        const int64_t c = o.cell_of(o.x0 + i, j, k);
+        o.out_sum[3 * c] += o.sx[l]; o.out_sum[3 * c + 1] += o.sy[l]; o.out_sum[3 * c + 2] += o.sz[l];
+        o.out_cnt[c] += 1;
+      }
+  // move: S(i,.,.) <- S(i+p,.,.) for i < nx-p
+  for (int i = 0; i + p < nx; ++i)
+    for (int k = 0; k < nz; ++k)
+      for (int j = 0; j < ny; ++j) {
+        const int64_t l = o.site(i, k, j), s = o.site(i + p, k, j);
+        o.sx[l] = o.sx[s]; o.sy[l] = o.sy[s]; o.sz[l] = o.sz[s];
+      }
+  // S3 incoming: planes i >= nx-p; new global plane gx = x0 + p + i.
+  for (int i = nx - p; i < nx; ++i)
+    for (int k = 0; k < nz; ++k)
+      for (int j = 0; j < ny; ++j) {
+        const int64_t l = o.site(i, k, j);
+        const int64_t gx = o.x0 + p + i;
+        if (o.grain_map[(size_t)(gx * ny + j)] < 0) { o.sx[l] = o.sy[l] = o.sz[l] = 0.0; continue; }
+        double S[3];
+        seed_site(o, gx, k, j, S);
+        o.sx[l] = S[0]; o.sy[l] = S[1]; o.sz[l] = S[2];
+      }
+  o.x0 += p; o.shift += 1;                              // S4: T and B are NOT moved
+  return 0;
+}
+
+void orc_track_set_init(void* h, const float* mean_spin /* [ncell*3] or null */, float m0) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  const size_t nc = (size_t)(o.ncx * o.ncy * o.ncz);
+  for (size_t c = 0; c < nc; ++c)
+    for (int a = 0; a < 3; ++a)
+      o.init_mean[3 * c + a] = mean_spin ? (double)mean_spin[3 * c + a] : (a == 2 ? (double)m0 : 0.0);
+}
+
+int64_t orc_track_ncell(void* h, int64_t dims[3]) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  if (dims) { dims[0] = o.ncx; dims[1] = o.ncy; dims[2] = o.ncz; }
+  return o.ncx * o.ncy * o.ncz;
+}
+
+// mean_spin[c] = out_sum[c] / out_cnt[c] (0 if empty), count[c] = out_cnt[c]; sums also returned.
+void orc_track_get(void* h, double* mean_spin, int64_t* count, double* sum) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  const size_t nc = (size_t)(o.ncx * o.ncy * o.ncz);
+  for (size_t c = 0; c < nc; ++c) {
+    if (count) count[c] = o.out_cnt[c];
+    for (int a = 0; a < 3; ++a) {
+      if (sum) sum[3 * c + a] = o.out_sum[3 * c + a];
+      if (mean_spin) mean_spin[3 * c + a] = o.out_cnt[c] > 0 ? o.out_sum[3 * c + a] / (double)o.out_cnt[c] : 0.0;
+    }
+  }
+}
+
+void orc_get_counters(void* h, int64_t* step, int64_t* shift, int64_t* x0, int64_t* pass) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  if (step) *step = o.step; if (shift) *shift = o.shift; if (x0) *x0 = o.x0; if (pass) *pass = o.pass;
+}
+
+void orc_set_counters(void* h, int64_t step, int64_t shift, int64_t pass) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  o.step = step; o.shift = shift; o.pass = pass;
+}
+
+// ---- building blocks exposed for the pins ----
+void orc_philox4x32_10(const uint32_t key[2], const uint32_t ctr[4], uint32_t out[4]) { philox4x32_10(key, ctr, out); }
+void orc_philox_block(uint64_t seed, uint64_t n, uint64_t g, uint32_t stream, uint32_t out[4]) { philox_block(seed, n, g, stream, out); }
+double orc_uniform(uint32_t r) { return uniform_from_u32(r); }
+void orc_normals3(uint64_t seed, uint64_t step, uint64_t g, double xi[3]) { normals3(seed, step, g, xi); }
+// Bulk version for moment tests: xi[3*count], sites g0..g0+count-1.
+void orc_normals3_bulk(uint64_t seed, uint64_t step, uint64_t g0, int64_t count, double* xi) {
+  for (int64_t a = 0; a < count; ++a) normals3(seed, step, g0 + (uint64_t)a, xi + 3 * a);
+}
+double orc_theta_max(double m) { return theta_max_of_m(m); }
+double orc_sigma(void* h, double T) { return sigma_T(*static_cast<Oracle*>(h), T); }
+
+}  // extern "C"

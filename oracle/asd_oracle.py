@@ -1,0 +1,300 @@
+"""ctypes wrapper around oracle/asd_oracle.cpp -- the fp64 CPU oracle.
+
+TEST INFRASTRUCTURE ONLY.  May be imported by tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs.  It never imports the CUDA package and the CUDA package
+never imports it.  All arithmetic lives in asd_oracle.cpp; this file only marshals arguments.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass, field
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "asd_oracle.cpp")
+_LIB = os.path.join(_HERE, "libasd_oracle.so")
+
+GAMMA_E = 1.76085963023e11   # rad s^-1 T^-1
+MU_B = 9.2740100783e-24      # J/T
+K_B = 1.380649e-23           # J/K
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with g++ (-O2, OpenMP).  Returns the path of the shared library."""
+    if (not force and os.path.exists(_LIB)
+            and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
+        return _LIB
+    cmd = ["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off",
+           "-o", _LIB, _SRC]
+    subprocess.run(cmd, check=True)
+    return _LIB
+
+
+class _Desc(C.Structure):
+    _fields_ = [
+        ("lattice", C.c_int32), ("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
+        ("pbc", C.c_int32 * 3),
+        ("n_grains", C.c_int32),
+        ("mu_s", C.c_double), ("lam", C.c_double), ("gamma", C.c_double), ("dt", C.c_double),
+        ("J", C.c_double * 3),
+        ("track_nx", C.c_int64), ("x0", C.c_int64),
+        ("grain_map", C.POINTER(C.c_int32)),
+        ("grain_ku", C.POINTER(C.c_double)),
+        ("grain_axis", C.POINTER(C.c_double)),
+        ("macro", C.c_int32 * 3),
+        ("ell_width", C.c_int32),
+        ("ell_idx", C.POINTER(C.c_int32)),
+        ("ell_J", C.POINTER(C.c_double)),
+        ("seed", C.c_uint64),
+    ]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(build())
+        L.orc_create.restype = C.c_void_p
+        L.orc_create.argtypes = [C.POINTER(_Desc)]
+        L.orc_destroy.argtypes = [C.c_void_p]
+        L.orc_set_threads.argtypes = [C.c_void_p, C.c_int]
+        L.orc_max_threads.restype = C.c_int
+        fp = C.POINTER(C.c_float)
+        dp = C.POINTER(C.c_double)
+        ip64 = C.POINTER(C.c_int64)
+        L.orc_set_spins.argtypes = [C.c_void_p, fp, fp, fp]
+        L.orc_get_spins.argtypes = [C.c_void_p, dp, dp, dp]
+        L.orc_set_fields.argtypes = [C.c_void_p, fp, fp, fp, fp]
+        L.orc_set_field_scale.argtypes = [C.c_void_p, C.c_float]
+        L.orc_step_heun.argtypes = [C.c_void_p, C.c_int64]
+        L.orc_field.argtypes = [C.c_void_p, C.c_int, dp, dp, dp]
+        L.orc_energy.restype = C.c_double
+        L.orc_energy.argtypes = [C.c_void_p]
+        L.orc_magnetisation.argtypes = [C.c_void_p, dp, dp]
+        L.orc_grain_magnetisation.argtypes = [C.c_void_p, dp]
+        L.orc_shift_window.restype = C.c_int
+        L.orc_shift_window.argtypes = [C.c_void_p, C.c_int32]
+        L.orc_track_set_init.argtypes = [C.c_void_p, fp, C.c_float]
+        L.orc_track_ncell.restype = C.c_int64
+        L.orc_track_ncell.argtypes = [C.c_void_p, ip64]
+        L.orc_track_get.argtypes = [C.c_void_p, dp, ip64, dp]
+        L.orc_get_counters.argtypes = [C.c_void_p, ip64, ip64, ip64, ip64]
+        L.orc_set_counters.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_int64]
+        u32p = C.POINTER(C.c_uint32)
+        L.orc_philox4x32_10.argtypes = [u32p, u32p, u32p]
+        L.orc_philox_block.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint32, u32p]
+        L.orc_uniform.restype = C.c_double
+        L.orc_uniform.argtypes = [C.c_uint32]
+        L.orc_normals3.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64, dp]
+        L.orc_normals3_bulk.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64, C.c_int64, dp]
+        L.orc_theta_max.restype = C.c_double
+        L.orc_theta_max.argtypes = [C.c_double]
+        L.orc_sigma.restype = C.c_double
+        L.orc_sigma.argtypes = [C.c_void_p, C.c_double]
+        _lib = L
+    return _lib
+
+
+def _f32(a):
+    return None if a is None else np.ascontiguousarray(a, dtype=np.float32)
+
+
+def _ptr(a, ct):
+    return None if a is None else a.ctypes.data_as(C.POINTER(ct))
+
+
+# ---- free functions (building blocks used by the pins) ----
+def philox4x32_10(key: Sequence[int], ctr: Sequence[int]) -> np.ndarray:
+    k = (C.c_uint32 * 2)(*[int(x) & 0xFFFFFFFF for x in key])
+    c = (C.c_uint32 * 4)(*[int(x) & 0xFFFFFFFF for x in ctr])
+    o = (C.c_uint32 * 4)()
+    lib().orc_philox4x32_10(k, c, o)
+    return np.array(list(o), dtype=np.uint32)
+
+
+def philox_block(seed: int, n: int, g: int, stream: int) -> np.ndarray:
+    o = (C.c_uint32 * 4)()
+    lib().orc_philox_block(C.c_uint64(seed), C.c_uint64(n), C.c_uint64(g), C.c_uint32(stream), o)
+    return np.array(list(o), dtype=np.uint32)
+
+
+def uniform(r: int) -> float:
+    return float(lib().orc_uniform(C.c_uint32(r)))
+
+
+def normals3(seed: int, step: int, g: int) -> np.ndarray:
+    o = np.zeros(3)
+    lib().orc_normals3(C.c_uint64(seed), C.c_uint64(step), C.c_uint64(g), _ptr(o, C.c_double))
+    return o
+
+
+def normals3_bulk(seed: int, step: int, g0: int, count: int) -> np.ndarray:
+    o = np.zeros((count, 3))
+    lib().orc_normals3_bulk(C.c_uint64(seed), C.c_uint64(step), C.c_uint64(g0), C.c_int64(count),
+                            _ptr(o, C.c_double))
+    return o
+
+
+def theta_max(m: float) -> float:
+    return float(lib().orc_theta_max(C.c_double(m)))
+
+
+def max_threads() -> int:
+    return int(lib().orc_max_threads())
+
+
+@dataclass
+class LatticeSpec:
+    """Plain description of a lattice; mirrors the quantities of SURVEY 8(b) but is the oracle's own."""
+    lattice: int                       # 0 = SC, 1 = L1_0 Fe sublattice
+    nx: int
+    ny: int
+    nz: int
+    pbc: Sequence[int] = (0, 0, 0)
+    mu_s: float = 3.23 * MU_B
+    lam: float = 0.1
+    gamma: float = GAMMA_E
+    dt: float = 1e-15
+    J: Sequence[float] = (6.71e-21, 0.0, 0.0)
+    track_nx: Optional[int] = None
+    x0: int = 0
+    grain_map: Optional[np.ndarray] = None     # [track_nx, ny] int32, -1 vacant
+    grain_ku: Optional[np.ndarray] = None      # [n_grains]
+    grain_axis: Optional[np.ndarray] = None    # [n_grains, 3]
+    macro: Sequence[int] = (7, 7, 7)
+    ell_idx: Optional[np.ndarray] = None       # [N, W] int32
+    ell_J: Optional[np.ndarray] = None         # [N, W] float
+    seed: int = 1
+
+
+class Oracle:
+    def __init__(self, spec: LatticeSpec):
+        L = lib()
+        self.spec = spec
+        track_nx = spec.track_nx if spec.track_nx is not None else spec.nx
+        gm = spec.grain_map
+        if gm is None:
+            gm = np.zeros((track_nx, spec.ny), dtype=np.int32)
+        self._gm = np.ascontiguousarray(gm, dtype=np.int32).reshape(track_nx, spec.ny)
+        ku = spec.grain_ku if spec.grain_ku is not None else np.zeros(1)
+        ax = spec.grain_axis if spec.grain_axis is not None else np.array([[0.0, 0.0, 1.0]])
+        self._ku = np.ascontiguousarray(ku, dtype=np.float64).reshape(-1)
+        self._ax = np.ascontiguousarray(ax, dtype=np.float64).reshape(-1, 3)
+        assert self._ax.shape[0] == self._ku.shape[0]
+        assert self._gm.max(initial=-1) < self._ku.shape[0]
+        d = _Desc()
+        d.lattice, d.nx, d.ny, d.nz = spec.lattice, spec.nx, spec.ny, spec.nz
+        d.pbc = (C.c_int32 * 3)(*[int(x) for x in spec.pbc])
+        d.n_grains = self._ku.shape[0]
+        d.mu_s, d.lam, d.gamma, d.dt = spec.mu_s, spec.lam, spec.gamma, spec.dt
+        d.J = (C.c_double * 3)(*[float(x) for x in spec.J])
+        d.track_nx, d.x0 = track_nx, spec.x0
+        d.grain_map = _ptr(self._gm, C.c_int32)
+        d.grain_ku = _ptr(self._ku, C.c_double)
+        d.grain_axis = _ptr(self._ax, C.c_double)
+        d.macro = (C.c_int32 * 3)(*[int(x) for x in spec.macro])
+        self.N = spec.nx * spec.ny * spec.nz
+        if spec.ell_idx is not None:
+            self._ei = np.ascontiguousarray(spec.ell_idx, dtype=np.int32).reshape(self.N, -1)
+            self._ej = np.ascontiguousarray(spec.ell_J, dtype=np.float64).reshape(self.N, -1)
+            d.ell_width = self._ei.shape[1]
+            d.ell_idx = _ptr(self._ei, C.c_int32)
+            d.ell_J = _ptr(self._ej, C.c_double)
+        else:
+            d.ell_width = 0
+        d.seed = spec.seed
+        self._h = L.orc_create(C.byref(d))
+        if not self._h:
+            raise ValueError("orc_create rejected the description")
+        self.n_grains = int(d.n_grains)
+
+    def __del__(self):
+        try:
+            if getattr(self, "_h", None):
+                lib().orc_destroy(self._h)
+                self._h = None
+        except Exception:
+            pass
+
+    def set_threads(self, n: int):
+        lib().orc_set_threads(self._h, int(n))
+
+    def set_spins(self, sx, sy, sz):
+        sx, sy, sz = _f32(sx).reshape(-1), _f32(sy).reshape(-1), _f32(sz).reshape(-1)
+        assert sx.size == self.N and sy.size == self.N and sz.size == self.N
+        lib().orc_set_spins(self._h, _ptr(sx, C.c_float), _ptr(sy, C.c_float), _ptr(sz, C.c_float))
+
+    def get_spins(self) -> np.ndarray:
+        """Returns [3, N] float64."""
+        o = np.zeros((3, self.N))
+        lib().orc_get_spins(self._h, _ptr(o[0], C.c_double), _ptr(o[1], C.c_double), _ptr(o[2], C.c_double))
+        return o
+
+    def set_fields(self, T=None, Bx=None, By=None, Bz=None):
+        arrs = [None if a is None else _f32(a).reshape(-1) for a in (T, Bx, By, Bz)]
+        for a in arrs:
+            assert a is None or a.size == self.N
+        lib().orc_set_fields(self._h, *[_ptr(a, C.c_float) for a in arrs])
+
+    def set_field_scale(self, s: float):
+        lib().orc_set_field_scale(self._h, C.c_float(s))
+
+    def step_heun(self, n: int = 1):
+        lib().orc_step_heun(self._h, C.c_int64(n))
+
+    def field(self, with_noise: bool = False) -> np.ndarray:
+        o = np.zeros((3, self.N))
+        lib().orc_field(self._h, int(with_noise), _ptr(o[0], C.c_double), _ptr(o[1], C.c_double),
+                        _ptr(o[2], C.c_double))
+        return o
+
+    def energy(self) -> float:
+        return float(lib().orc_energy(self._h))
+
+    def magnetisation(self):
+        m = np.zeros(3)
+        n = C.c_double(0)
+        lib().orc_magnetisation(self._h, _ptr(m, C.c_double), C.byref(n))
+        return m, n.value
+
+    def grain_magnetisation(self) -> np.ndarray:
+        m = np.zeros((self.n_grains, 3))
+        lib().orc_grain_magnetisation(self._h, _ptr(m, C.c_double))
+        return m
+
+    def shift_window(self, p: int) -> int:
+        return int(lib().orc_shift_window(self._h, C.c_int32(p)))
+
+    def track_dims(self):
+        d = (C.c_int64 * 3)()
+        lib().orc_track_ncell(self._h, d)
+        return tuple(int(x) for x in d)
+
+    def track_set_init(self, mean_spin=None, m0: float = 1.0):
+        a = None if mean_spin is None else _f32(mean_spin).reshape(-1)
+        lib().orc_track_set_init(self._h, _ptr(a, C.c_float), C.c_float(m0))
+
+    def track_get(self):
+        nc = int(np.prod(self.track_dims()))
+        mean = np.zeros((nc, 3))
+        cnt = np.zeros(nc, dtype=np.int64)
+        sm = np.zeros((nc, 3))
+        lib().orc_track_get(self._h, _ptr(mean, C.c_double), _ptr(cnt, C.c_int64), _ptr(sm, C.c_double))
+        return mean, cnt, sm
+
+    def counters(self):
+        a, b, c, d = C.c_int64(0), C.c_int64(0), C.c_int64(0), C.c_int64(0)
+        lib().orc_get_counters(self._h, C.byref(a), C.byref(b), C.byref(c), C.byref(d))
+        return {"step": a.value, "shift": b.value, "x0": c.value, "pass": d.value}
+
+    def set_counters(self, step: int, shift: int = 0, pass_: int = 0):
+        lib().orc_set_counters(self._h, C.c_int64(step), C.c_int64(shift), C.c_int64(pass_))
+
+    def sigma(self, T: float) -> float:
+        return float(lib().orc_sigma(self._h, C.c_double(T)))
