@@ -1,0 +1,170 @@
+/* ============================================================================
+ * asd.h -- C ABI of libasd: the atomistic spin-dynamics (ASD) window of the multiscale HAMR
+ * model of arXiv 2502.02236 (Gija et al.), as hand-written CUDA kernels for NVIDIA B200 (sm_100a).
+ *
+ * Citations: P:<n> = PAPER.md line n (with section / equation); S:<x> = SURVEY.md section 8 item x;
+ * D:<x> = DESIGN.md reading x.
+ *
+ * What the library computes
+ *   * stochastic Landau-Lifshitz-Gilbert equation on every atomic spin, Eq. (1) (sec. II)
+ *   * effective field B = mu_0 H in Tesla: exchange Eq. (2) + uniaxial anisotropy Eq. (3)
+ *      + external (write) field + thermal field, sigma = sqrt(2 lambda k_B T /
+ *     (gamma mu_s dt)) (P:38 with mu_0 absorbed)
+ *   * stochastic Heun integration (BASELINE.json north_star; D:Q1), noise from Philox4x32-10 keyed by
+ *     (seed; step, global site) generated in registers (D:R1-R3)
+ *   * moving-window shift: outgoing slab -> track macrocells by Eq. (6), incoming
+ *     slab <- cone sampling about the track magnetisation (D:S3)
+ *   * window / per-grain magnetisation (Eq. (6) with V = window or grain)
+ *
+ * Conventions
+ *   Site order   window-local l = (i*nz + k)*ny + j; x (i) along the track and slowest, z (k) film normal,
+ *                y (j) across the track and fastest.  All per-site arrays are [N], N = nx*ny*nz, fp32.
+ *   Global id    g = l + x0*ny*nz -- the Philox counter, so noise follows the atom, not the memory slot.
+ *   Units        Tesla, Joule, Kelvin, seconds; mu_s in J/T; gamma in rad s^-1 T^-1.
+ *   Pointers     "DEVICE" = CUDA device memory on the context's device; "HOST" = ordinary host memory
+ *                (pinned memory makes the *_host calls asynchronous; pageable memory makes them
+ *                synchronise).  The caller owns every buffer it passes.  The library copies what it
+ *                needs into the caller-provided workspace and never frees or keeps a caller pointer
+ *                except `d_workspace` (which must outlive the context).
+ *   Streams      every call enqueues on the `cuda_stream` given at create time and returns without
+ *                synchronising, except asd_magnetisation, asd_grain_magnetisation, asd_track_get,
+ *                asd_get_spins_host (they synchronise that stream).
+ *   Errors       every call returns asd_status.  Arguments are validated on the host -> ASD_EINVAL.
+ *                A CUDA failure is sticky: the context returns ASD_ECUDA until destroyed.
+ *                asd_last_error gives a static or context-owned message.  No exceptions, no abort().
+ *   Threads      a context is not thread-safe; distinct contexts are independent.
+ *   No fallback  there is no CPU path: without a CUDA device asd_create_lattice returns ASD_ECUDA.
+ * ========================================================================== */
+#ifndef ASD_H_
+#define ASD_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define ASD_API __attribute__((visibility("default")))
+#else
+#define ASD_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct asd_ctx asd_ctx; /* opaque; created by asd_create_lattice, freed by asd_destroy */
+
+typedef enum {
+  ASD_OK = 0,
+  ASD_EINVAL = 1,       /* bad argument (null, size, range)                                   */
+  ASD_ENOMEM = 2,       /* workspace too small                                                */
+  ASD_ECUDA = 3,        /* CUDA runtime / launch failure (sticky)                             */
+  ASD_ESTATE = 4,       /* call not valid in the current state (e.g. shift past the track end)*/
+  ASD_EUNSUPPORTED = 5  /* valid request the library does not implement                       */
+} asd_status;
+
+enum { ASD_SC = 0, ASD_L10_FE = 1 };
+
+/* Kernel variant for asd_step_heun.  AUTO picks the fastest supported. */
+enum { ASD_KERNEL_AUTO = 0, ASD_KERNEL_DIRECT = 1, ASD_KERNEL_TILED = 2 };
+
+/* Lattice description (S:8(b)).  Plain data; HOST pointers are read during asd_create_lattice only. */
+typedef struct {
+  int32_t lattice;      /* ASD_SC: simple cubic, 6 nearest neighbours, J[0]
+                           ASD_L10_FE: Fe sublattice of L1_0 FePt in its own simple-tetragonal axes,
+                           4 in-plane nn J[0] at (+-1,0,0),(0,+-1,0); 2 out-of-plane J[1] at (0,0,+-1);
+                           4 in-plane nnn J[2] at (+-1,+-1,0)  ("4 nearest + 6 next nearest") */
+  int32_t nx, ny, nz;   /* window size in sites                                                  */
+  int32_t pbc[3];       /* periodic flags (x,y,z); a periodic dimension needs n >= 3 (D:Q17);
+                           pbc[0] requires track_nx == nx and forbids asd_shift_window            */
+  double mu_s;          /* atomic moment, J/T                                                    */
+  double lambda;        /* Gilbert damping, >= 0                                                 */
+  double gamma;         /* gyromagnetic ratio, rad s^-1 T^-1; <= 0 selects 1.76085963023e11       */
+  double dt;            /* time step, s, > 0                                                     */
+  double J[3];          /* exchange energies per shell, Joule (see `lattice`)                    */
+  int64_t track_nx;     /* length of the grain map in planes, >= x0 + nx                         */
+  int64_t x0;           /* global plane index of window plane 0                                  */
+  const int32_t *grain_map; /* HOST [track_nx*ny], grain id of column (gx, j) at gx*ny + j; -1 = vacant
+                               (non-magnetic) column.  NULL = one grain (id 0) everywhere.
+                               Exchange bonds join only magnetic sites of the SAME grain.   */
+  int32_t n_grains;     /* >= 1, <= 65535                                                        */
+  const float *grain_ku;   /* HOST [n_grains] uniaxial anisotropy energy per atom K_1, Joule (Eq. 3); NULL = 0 */
+  const float *grain_axis; /* HOST [n_grains*3] unit easy axes e_A (|e| = 1 within 1e-4); NULL = z */
+  int32_t macro[3];     /* track macrocell edge in sites (mx,my,mz), each >= 1 (D:S1)            */
+  const int32_t *ell_idx;  /* optional general neighbour table, HOST [N*ell_width] site-major, entry =
+                              window-local neighbour site or -1; replaces the built-in shells      */
+  const float *ell_J;      /* HOST [N*ell_width] exchange energy of that pair, Joule              */
+  int32_t ell_width;    /* 0 = built-in shells; else 1..16                                       */
+  uint64_t seed;        /* Philox key                                                            */
+} asd_lattice_desc;
+
+/* Bytes of DEVICE workspace asd_create_lattice needs for this description (0 if desc is invalid).
+ * Callable without a GPU. */
+ASD_API size_t asd_workspace_bytes(const asd_lattice_desc *desc);
+
+/* Creates a context.  d_workspace: DEVICE, >= asd_workspace_bytes(desc) bytes, 256-byte aligned, owned by
+ * the caller and kept until asd_destroy.  cuda_stream: a cudaStream_t (NULL = default stream).
+ * Initial state: all spins +z on magnetic sites (0 on vacant), T = 0, B = 0, field scale 1, counters 0,
+ * track initial state +z with m0 = 1.  ASD_EINVAL / ASD_ENOMEM / ASD_ECUDA. */
+ASD_API asd_status asd_create_lattice(const asd_lattice_desc *desc, void *d_workspace, size_t bytes,
+                              void *cuda_stream, asd_ctx **out);
+ASD_API asd_status asd_destroy(asd_ctx *ctx);
+
+/* Spins, SoA fp32 [N] each.  set: values on vacant sites are ignored (stored as 0); values are NOT
+ * renormalised.  get: vacant sites read 0. */
+ASD_API asd_status asd_set_spins(asd_ctx *ctx, const float *sx, const float *sy, const float *sz);      /* DEVICE */
+ASD_API asd_status asd_get_spins(asd_ctx *ctx, float *sx, float *sy, float *sz);                        /* DEVICE */
+ASD_API asd_status asd_set_spins_host(asd_ctx *ctx, const float *sx, const float *sy, const float *sz); /* HOST */
+ASD_API asd_status asd_get_spins_host(asd_ctx *ctx, float *sx, float *sy, float *sz);       /* HOST; synchronises */
+
+/* Per-site temperature T [K] and applied field B [Tesla] in window-local order (the profiles
+ * are centred in the window and do not move with a shift).  NULL = keep the previous array.
+ * T < 0 is the caller's error (sigma becomes NaN); it is not scanned. */
+ASD_API asd_status asd_set_fields(asd_ctx *ctx, const float *T, const float *Bx, const float *By,
+                          const float *Bz);                                                     /* DEVICE */
+ASD_API asd_status asd_set_fields_host(asd_ctx *ctx, const float *T, const float *Bx, const float *By,
+                               const float *Bz);                                                /* HOST   */
+/* B_app = s * B : write-field polarity / ramp. */
+ASD_API asd_status asd_set_field_scale(asd_ctx *ctx, float s);
+
+/* n stochastic Heun steps (S:O4): per step one predictor and one corrector kernel, each fused
+ * field + update + renormalise with in-register Philox noise (same xi in both stages); step counter += n. */
+ASD_API asd_status asd_step_heun(asd_ctx *ctx, int64_t n);
+/* Selects the kernel variant (ASD_KERNEL_*); ASD_EUNSUPPORTED if the lattice cannot use it. */
+ASD_API asd_status asd_set_kernel(asd_ctx *ctx, int32_t variant);
+
+/* Window moves +x by p planes, 1 <= p <= nx (S:O5): outgoing planes -> macrocell sums and counts (Eq. 6);
+ * spins move by p planes; incoming planes seeded by cone sampling (D:S3); x0 += p; shift counter += 1.
+ * ASD_ESTATE if x0 + p + nx > track_nx; ASD_EUNSUPPORTED with a general ELL table or pbc[0]. */
+ASD_API asd_status asd_shift_window(asd_ctx *ctx, int32_t p_planes);
+
+/* m = sum over magnetic sites of S / N_mag (Eq. 6 with V = window), fp64; synchronises. */
+ASD_API asd_status asd_magnetisation(asd_ctx *ctx, double m[3], double *n_magnetic);
+/* Per-grain mean spin, HOST [n_grains*3] (0 for grains without sites in the window); synchronises. */
+ASD_API asd_status asd_grain_magnetisation(asd_ctx *ctx, double *m);
+
+/* Track store: macrocells (cx,cy,cz) = (floor(gx/mx), floor(j/my), floor(k/mz)), cell index
+ * c = (cx*ncy + cy)*ncz + cz over the whole track. */
+ASD_API asd_status asd_track_dims(const asd_ctx *ctx, int64_t dims[3]);
+/* What lies ahead of the window: mean spin per cell, HOST [ncell*3] (|v| <= 1 is the reduced
+ * magnetisation M/M_S^0); NULL = (0,0,m0) everywhere. */
+ASD_API asd_status asd_track_set_init(asd_ctx *ctx, const float *mean_spin, float m0);
+/* What the window has written: sum of spins and site count per cell (Eq. 6 with mu_S/V factored out).
+ * HOST sum [ncell*3] (fp64), count [ncell]; either may be NULL; synchronises. */
+ASD_API asd_status asd_track_get(asd_ctx *ctx, double *sum, int64_t *count);
+
+/* Counters for bit-exact checkpoint / resume (Philox is counter based: there is no RNG state). */
+ASD_API asd_status asd_get_counters(const asd_ctx *ctx, int64_t *step, int64_t *shift, int64_t *x0, int64_t *pass);
+ASD_API asd_status asd_set_counters(asd_ctx *ctx, int64_t step, int64_t shift, int64_t pass);
+
+/* Number of kernels this context has launched so far (bench.py's gpu_launches). */
+ASD_API int64_t asd_launch_count(const asd_ctx *ctx);
+
+/* Message of the last failure on this context (or a generic one for ctx == NULL); never NULL. */
+ASD_API const char *asd_last_error(const asd_ctx *ctx);
+/* Library version string, e.g. "asd-b200 0.1 (sm_100a)". */
+ASD_API const char *asd_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ASD_H_ */

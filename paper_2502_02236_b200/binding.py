@@ -1,0 +1,315 @@
+"""ctypes binding over libasd.so -- argument marshalling only (include/asd.h is the contract).
+
+Every method of `Context` has the name of the C call it wraps (minus the asd_ prefix) and does nothing but
+convert arguments: torch tensors -> device pointers, numpy arrays -> host pointers.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+from typing import Optional, Sequence
+
+import numpy as np
+
+ASD_SC, ASD_L10_FE = 0, 1
+KERNEL_AUTO, KERNEL_DIRECT, KERNEL_TILED = 0, 1, 2
+_STATUS = {0: "ASD_OK", 1: "ASD_EINVAL", 2: "ASD_ENOMEM", 3: "ASD_ECUDA", 4: "ASD_ESTATE", 5: "ASD_EUNSUPPORTED"}
+
+EXPORTED_SYMBOLS = [
+    "asd_workspace_bytes", "asd_create_lattice", "asd_destroy", "asd_set_spins", "asd_get_spins",
+    "asd_set_spins_host", "asd_get_spins_host", "asd_set_fields", "asd_set_fields_host", "asd_set_field_scale",
+    "asd_step_heun", "asd_set_kernel", "asd_shift_window", "asd_magnetisation", "asd_grain_magnetisation",
+    "asd_track_dims", "asd_track_set_init", "asd_track_get", "asd_get_counters", "asd_set_counters",
+    "asd_launch_count", "asd_last_error", "asd_version",
+]
+
+
+class AsdError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"{_STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+class _Desc(C.Structure):
+    _fields_ = [
+        ("lattice", C.c_int32), ("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
+        ("pbc", C.c_int32 * 3),
+        ("mu_s", C.c_double), ("lam", C.c_double), ("gamma", C.c_double), ("dt", C.c_double),
+        ("J", C.c_double * 3),
+        ("track_nx", C.c_int64), ("x0", C.c_int64),
+        ("grain_map", C.POINTER(C.c_int32)),
+        ("n_grains", C.c_int32),
+        ("grain_ku", C.POINTER(C.c_float)),
+        ("grain_axis", C.POINTER(C.c_float)),
+        ("macro", C.c_int32 * 3),
+        ("ell_idx", C.POINTER(C.c_int32)),
+        ("ell_J", C.POINTER(C.c_float)),
+        ("ell_width", C.c_int32),
+        ("seed", C.c_uint64),
+    ]
+
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_lib = None
+
+
+def lib_path() -> str:
+    return os.path.join(_HERE, "libasd.so")
+
+
+def load_library(build_if_missing: bool = True):
+    """Loads libasd.so (building it with nvcc if it is missing or stale).  Fails loudly: there is no fallback."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if build_if_missing:
+        from . import build as _build
+        try:
+            _build.build()
+        except Exception as e:  # stale sources without nvcc: use the existing library if there is one
+            if not os.path.exists(lib_path()):
+                raise RuntimeError(f"libasd.so is missing and cannot be built: {e}") from e
+    if not os.path.exists(lib_path()):
+        raise RuntimeError("libasd.so is missing: run `python -m paper_2502_02236_b200.build`")
+    L = C.CDLL(lib_path())
+    fp, dp, ip64 = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)
+    L.asd_workspace_bytes.restype = C.c_size_t
+    L.asd_workspace_bytes.argtypes = [C.POINTER(_Desc)]
+    L.asd_create_lattice.argtypes = [C.POINTER(_Desc), C.c_void_p, C.c_size_t, C.c_void_p, C.POINTER(C.c_void_p)]
+    L.asd_destroy.argtypes = [C.c_void_p]
+    for name in ("asd_set_spins", "asd_get_spins", "asd_set_spins_host", "asd_get_spins_host"):
+        getattr(L, name).argtypes = [C.c_void_p, fp, fp, fp]
+    for name in ("asd_set_fields", "asd_set_fields_host"):
+        getattr(L, name).argtypes = [C.c_void_p, fp, fp, fp, fp]
+    L.asd_set_field_scale.argtypes = [C.c_void_p, C.c_float]
+    L.asd_step_heun.argtypes = [C.c_void_p, C.c_int64]
+    L.asd_set_kernel.argtypes = [C.c_void_p, C.c_int32]
+    L.asd_shift_window.argtypes = [C.c_void_p, C.c_int32]
+    L.asd_magnetisation.argtypes = [C.c_void_p, dp, dp]
+    L.asd_grain_magnetisation.argtypes = [C.c_void_p, dp]
+    L.asd_track_dims.argtypes = [C.c_void_p, ip64]
+    L.asd_track_set_init.argtypes = [C.c_void_p, C.c_void_p, C.c_float]
+    L.asd_track_get.argtypes = [C.c_void_p, dp, ip64]
+    L.asd_get_counters.argtypes = [C.c_void_p, ip64, ip64, ip64, ip64]
+    L.asd_set_counters.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_int64]
+    L.asd_launch_count.restype = C.c_int64
+    L.asd_launch_count.argtypes = [C.c_void_p]
+    L.asd_last_error.restype = C.c_char_p
+    L.asd_last_error.argtypes = [C.c_void_p]
+    L.asd_version.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def version() -> str:
+    return load_library().asd_version().decode()
+
+
+@dataclass
+class LatticeDesc:
+    """Python mirror of asd_lattice_desc (include/asd.h)."""
+    lattice: int
+    nx: int
+    ny: int
+    nz: int
+    pbc: Sequence[int] = (0, 0, 0)
+    mu_s: float = 3.23 * 9.2740100783e-24
+    lam: float = 0.1
+    gamma: float = 0.0
+    dt: float = 1e-15
+    J: Sequence[float] = (6.71e-21, 0.0, 0.0)
+    track_nx: Optional[int] = None
+    x0: int = 0
+    grain_map: Optional[np.ndarray] = None
+    n_grains: int = 1
+    grain_ku: Optional[np.ndarray] = None
+    grain_axis: Optional[np.ndarray] = None
+    macro: Sequence[int] = (7, 7, 7)
+    ell_idx: Optional[np.ndarray] = None
+    ell_J: Optional[np.ndarray] = None
+    seed: int = 1
+
+    def to_c(self):
+        """Returns (struct, keepalive list)."""
+        d = _Desc()
+        keep = []
+        d.lattice, d.nx, d.ny, d.nz = int(self.lattice), int(self.nx), int(self.ny), int(self.nz)
+        d.pbc = (C.c_int32 * 3)(*[int(x) for x in self.pbc])
+        d.mu_s, d.lam, d.gamma, d.dt = float(self.mu_s), float(self.lam), float(self.gamma), float(self.dt)
+        d.J = (C.c_double * 3)(*[float(x) for x in self.J])
+        d.track_nx = int(self.track_nx if self.track_nx is not None else self.nx)
+        d.x0 = int(self.x0)
+
+        def host(a, dt, ct):
+            if a is None:
+                return None
+            arr = np.ascontiguousarray(a, dtype=dt)
+            keep.append(arr)
+            return arr.ctypes.data_as(C.POINTER(ct))
+        d.grain_map = host(self.grain_map, np.int32, C.c_int32)
+        d.n_grains = int(self.n_grains)
+        d.grain_ku = host(self.grain_ku, np.float32, C.c_float)
+        d.grain_axis = host(self.grain_axis, np.float32, C.c_float)
+        d.macro = (C.c_int32 * 3)(*[int(x) for x in self.macro])
+        d.ell_idx = host(self.ell_idx, np.int32, C.c_int32)
+        d.ell_J = host(self.ell_J, np.float32, C.c_float)
+        d.ell_width = 0 if self.ell_idx is None else int(np.asarray(self.ell_idx).reshape(self.nx * self.ny * self.nz, -1).shape[1])
+        d.seed = int(self.seed)
+        return d, keep
+
+
+def workspace_bytes(desc: LatticeDesc) -> int:
+    d, _keep = desc.to_c()
+    return int(load_library().asd_workspace_bytes(C.byref(d)))
+
+
+def _dev_ptr(t):
+    if t is None:
+        return None
+    import torch
+    assert isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()
+    return C.c_void_p(t.data_ptr())
+
+
+def _host_ptr(a, keep):
+    if a is None:
+        return None
+    import torch
+    if isinstance(a, torch.Tensor):
+        assert not a.is_cuda and a.dtype == torch.float32 and a.is_contiguous()
+        keep.append(a)
+        return C.c_void_p(a.data_ptr())
+    arr = np.ascontiguousarray(a, dtype=np.float32)
+    keep.append(arr)
+    return C.c_void_p(arr.ctypes.data)
+
+
+class Context:
+    """One asd_ctx plus its torch-allocated workspace.  Methods = the C calls."""
+
+    def __init__(self, desc: LatticeDesc, device: str = "cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("libasd needs a CUDA device: there is no CPU fallback")
+        self._L = load_library()
+        self.desc = desc
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        d, keep = desc.to_c()
+        nbytes = int(self._L.asd_workspace_bytes(C.byref(d)))
+        if nbytes == 0:
+            raise AsdError(1, self._L.asd_last_error(None).decode())
+        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        base = (self.workspace.data_ptr() + 255) // 256 * 256
+        self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        h = C.c_void_p()
+        st = self._L.asd_create_lattice(C.byref(d), C.c_void_p(base), C.c_size_t(nbytes),
+                                        C.c_void_p(self._stream.cuda_stream), C.byref(h))
+        if st != 0:
+            raise AsdError(st, self._L.asd_last_error(None).decode())
+        self._h = h
+        self.N = desc.nx * desc.ny * desc.nz
+        self.n_grains = desc.n_grains
+
+    def _ck(self, st):
+        if st != 0:
+            raise AsdError(st, self._L.asd_last_error(self._h).decode())
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            self._L.asd_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    # ---- spins / fields ----
+    def set_spins(self, sx, sy, sz):
+        self._ck(self._L.asd_set_spins(self._h, _dev_ptr(sx), _dev_ptr(sy), _dev_ptr(sz)))
+
+    def get_spins(self, sx, sy, sz):
+        self._ck(self._L.asd_get_spins(self._h, _dev_ptr(sx), _dev_ptr(sy), _dev_ptr(sz)))
+
+    def set_spins_host(self, sx, sy, sz):
+        keep = []
+        self._ck(self._L.asd_set_spins_host(self._h, _host_ptr(sx, keep), _host_ptr(sy, keep), _host_ptr(sz, keep)))
+        self._sync_if_unpinned(keep)
+
+    def get_spins_host(self) -> np.ndarray:
+        out = np.empty((3, self.N), dtype=np.float32)
+        self._ck(self._L.asd_get_spins_host(self._h, C.c_void_p(out[0].ctypes.data), C.c_void_p(out[1].ctypes.data),
+                                            C.c_void_p(out[2].ctypes.data)))
+        return out
+
+    def set_fields(self, T=None, Bx=None, By=None, Bz=None):
+        self._ck(self._L.asd_set_fields(self._h, _dev_ptr(T), _dev_ptr(Bx), _dev_ptr(By), _dev_ptr(Bz)))
+
+    def set_fields_host(self, T=None, Bx=None, By=None, Bz=None):
+        keep = []
+        self._ck(self._L.asd_set_fields_host(self._h, _host_ptr(T, keep), _host_ptr(Bx, keep), _host_ptr(By, keep),
+                                             _host_ptr(Bz, keep)))
+        self._sync_if_unpinned(keep)
+
+    def _sync_if_unpinned(self, keep):
+        import torch
+        if any(not (isinstance(a, torch.Tensor) and a.is_pinned()) for a in keep):
+            self._stream.synchronize()      # temporaries must outlive the asynchronous copy
+
+    def set_field_scale(self, s: float):
+        self._ck(self._L.asd_set_field_scale(self._h, C.c_float(s)))
+
+    # ---- dynamics ----
+    def step_heun(self, n: int = 1):
+        self._ck(self._L.asd_step_heun(self._h, C.c_int64(n)))
+
+    def set_kernel(self, variant: int):
+        self._ck(self._L.asd_set_kernel(self._h, C.c_int32(variant)))
+
+    def shift_window(self, p: int):
+        self._ck(self._L.asd_shift_window(self._h, C.c_int32(p)))
+
+    # ---- observables ----
+    def magnetisation(self):
+        m = np.zeros(3)
+        n = C.c_double(0)
+        self._ck(self._L.asd_magnetisation(self._h, m.ctypes.data_as(C.POINTER(C.c_double)), C.byref(n)))
+        return m, n.value
+
+    def grain_magnetisation(self) -> np.ndarray:
+        m = np.zeros((self.n_grains, 3))
+        self._ck(self._L.asd_grain_magnetisation(self._h, m.ctypes.data_as(C.POINTER(C.c_double))))
+        return m
+
+    # ---- track store ----
+    def track_dims(self):
+        d = (C.c_int64 * 3)()
+        self._ck(self._L.asd_track_dims(self._h, d))
+        return tuple(int(x) for x in d)
+
+    def track_set_init(self, mean_spin=None, m0: float = 1.0):
+        keep = []
+        self._ck(self._L.asd_track_set_init(self._h, _host_ptr(mean_spin, keep), C.c_float(m0)))
+
+    def track_get(self):
+        nc = int(np.prod(self.track_dims()))
+        s = np.zeros((nc, 3))
+        cnt = np.zeros(nc, dtype=np.int64)
+        self._ck(self._L.asd_track_get(self._h, s.ctypes.data_as(C.POINTER(C.c_double)),
+                                       cnt.ctypes.data_as(C.POINTER(C.c_int64))))
+        return s, cnt
+
+    # ---- counters ----
+    def counters(self):
+        a, b, c, d = C.c_int64(0), C.c_int64(0), C.c_int64(0), C.c_int64(0)
+        self._ck(self._L.asd_get_counters(self._h, C.byref(a), C.byref(b), C.byref(c), C.byref(d)))
+        return {"step": a.value, "shift": b.value, "x0": c.value, "pass": d.value}
+
+    def set_counters(self, step: int, shift: int = 0, pass_: int = 0):
+        self._ck(self._L.asd_set_counters(self._h, C.c_int64(step), C.c_int64(shift), C.c_int64(pass_)))
+
+    def launch_count(self) -> int:
+        return int(self._L.asd_launch_count(self._h))

@@ -1,0 +1,381 @@
+// asd_api.cu -- the C ABI of include/asd.h: argument validation, workspace layout, state, stream plumbing.
+// Every arithmetic step of the method runs in the kernels of asd_heun.cu / asd_shift.cu / asd_reduce.cu /
+// asd_setup.cu; this file only marshals.
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include "asd_internal.cuh"
+
+namespace asd {
+
+static const char* g_static_err = "no error";
+
+bool validate_desc(const asd_lattice_desc* d, const char** why) {
+  auto bad = [&](const char* m) { if (why) *why = m; return false; };
+  if (!d) return bad("desc is NULL");
+  if (d->lattice != ASD_SC && d->lattice != ASD_L10_FE) return bad("lattice must be ASD_SC or ASD_L10_FE");
+  if (d->nx < 1 || d->ny < 1 || d->nz < 1) return bad("nx, ny, nz must be >= 1");
+  if ((int64_t)d->nx * d->ny * d->nz > 2000000000LL) return bad("more than 2e9 sites");
+  const int n[3] = {d->nx, d->ny, d->nz};
+  for (int a = 0; a < 3; ++a) {
+    if (d->pbc[a] != 0 && d->pbc[a] != 1) return bad("pbc flags must be 0 or 1");
+    if (d->pbc[a] && n[a] < 3) return bad("a periodic dimension needs n >= 3");
+    if (d->macro[a] < 1) return bad("macro[] must be >= 1");
+    if (!std::isfinite(d->J[a])) return bad("J[] must be finite");
+  }
+  if (!(d->mu_s > 0.0) || !std::isfinite(d->mu_s)) return bad("mu_s must be > 0");
+  if (!(d->lambda >= 0.0) || !std::isfinite(d->lambda)) return bad("lambda must be >= 0");
+  if (!(d->dt > 0.0) || !std::isfinite(d->dt)) return bad("dt must be > 0");
+  if (!std::isfinite(d->gamma)) return bad("gamma must be finite");
+  if (d->x0 < 0 || d->track_nx < d->x0 + d->nx) return bad("track_nx must be >= x0 + nx and x0 >= 0");
+  if (d->pbc[0] && (d->track_nx != d->nx || d->x0 != 0)) return bad("pbc[0] requires track_nx == nx and x0 == 0");
+  if (d->track_nx * (int64_t)d->ny > 2000000000LL) return bad("grain map too large");
+  if (d->n_grains < 1 || d->n_grains > 65535) return bad("n_grains must be in 1..65535");
+  if (d->grain_map) {
+    const int64_t n = d->track_nx * d->ny;
+    for (int64_t t = 0; t < n; ++t)
+      if (d->grain_map[t] < -1 || d->grain_map[t] >= d->n_grains) return bad("grain id out of range");
+  }
+  if (d->grain_axis) {
+    for (int g = 0; g < d->n_grains; ++g) {
+      const double x = d->grain_axis[3 * g], y = d->grain_axis[3 * g + 1], z = d->grain_axis[3 * g + 2];
+      if (!(std::fabs(std::sqrt(x * x + y * y + z * z) - 1.0) <= 1e-4)) return bad("grain_axis must be unit vectors");
+    }
+  }
+  if (d->grain_ku)
+    for (int g = 0; g < d->n_grains; ++g)
+      if (!std::isfinite(d->grain_ku[g])) return bad("grain_ku must be finite");
+  if (d->ell_width < 0 || d->ell_width > 16) return bad("ell_width must be in 0..16");
+  if (d->ell_width > 0 && (!d->ell_idx || !d->ell_J)) return bad("ell_width > 0 needs ell_idx and ell_J");
+  return true;
+}
+
+bool compute_layout(const asd_lattice_desc& d, Layout& L) {
+  L.N = (int64_t)d.nx * d.ny * d.nz;
+  L.Npad = (int64_t)align_up((size_t)L.N, 64);
+  L.ncx = (d.track_nx + d.macro[0] - 1) / d.macro[0];
+  L.ncy = (d.ny + d.macro[1] - 1) / d.macro[1];
+  L.ncz = (d.nz + d.macro[2] - 1) / d.macro[2];
+  L.ncell = L.ncx * L.ncy * L.ncz;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { const size_t o = off; off = align_up(off + bytes, 256); return o; };
+  const size_t fN = sizeof(float) * (size_t)L.Npad;
+  for (int a = 0; a < 9; ++a) L.spins[a] = take(fN);
+  L.sigma = take(fN);
+  for (int a = 0; a < 3; ++a) L.B[a] = take(fN);
+  const size_t ncol = (size_t)(d.track_nx * d.ny);
+  L.col = take(sizeof(uint32_t) * ncol);
+  L.gmap = take(sizeof(int32_t) * ncol);
+  L.grain = take(sizeof(float4) * (size_t)d.n_grains);
+  const size_t ell = (size_t)d.ell_width * (size_t)L.N;
+  L.ell_idx = take(sizeof(int32_t) * ell * 2);   // slot-major table + staging for the site-major upload
+  L.ell_J = take(sizeof(float) * ell * 2);
+  L.init_mean = take(sizeof(float) * 3 * (size_t)L.ncell);
+  L.cell_frame = take(sizeof(float) * 12 * (size_t)L.ncell);
+  L.out_sum = take(sizeof(double) * 3 * (size_t)L.ncell);
+  L.out_cnt = take(sizeof(long long) * (size_t)L.ncell);
+  L.partials = take(sizeof(double) * 4 * kMaxPartialBlocks);
+  L.grain_acc = take(sizeof(long long) * 4 * (size_t)d.n_grains);
+  L.total = off;
+  return true;
+}
+
+asd_status fail_cuda(Ctx& c, cudaError_t e, const char* where) {
+  c.cuda_failed = true;
+  std::snprintf(c.err, sizeof(c.err), "CUDA error %d (%s) at %s", (int)e, cudaGetErrorString(e), where);
+  return ASD_ECUDA;
+}
+
+static asd_status fail(Ctx& c, asd_status s, const char* msg) {
+  std::snprintf(c.err, sizeof(c.err), "%s", msg);
+  return s;
+}
+
+}  // namespace asd
+
+using namespace asd;
+
+#define CTX_OR_RETURN(ctx)                                         \
+  if (!(ctx)) { g_static_err = "ctx is NULL"; return ASD_EINVAL; } \
+  Ctx& c = (ctx)->c;                                               \
+  if (c.cuda_failed) return ASD_ECUDA;
+
+extern "C" {
+
+size_t asd_workspace_bytes(const asd_lattice_desc* desc) {
+  const char* why = nullptr;
+  if (!validate_desc(desc, &why)) { g_static_err = why; return 0; }
+  Layout L;
+  compute_layout(*desc, L);
+  return L.total;
+}
+
+asd_status asd_create_lattice(const asd_lattice_desc* desc, void* d_workspace, size_t bytes, void* cuda_stream,
+                              asd_ctx** out) {
+  const char* why = nullptr;
+  if (!out) { g_static_err = "out is NULL"; return ASD_EINVAL; }
+  *out = nullptr;
+  if (!validate_desc(desc, &why)) { g_static_err = why; return ASD_EINVAL; }
+  if (!d_workspace || ((uintptr_t)d_workspace & 255u)) { g_static_err = "workspace NULL or not 256-byte aligned"; return ASD_EINVAL; }
+  Layout L;
+  compute_layout(*desc, L);
+  if (bytes < L.total) { g_static_err = "workspace too small"; return ASD_ENOMEM; }
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) { g_static_err = "no CUDA device (libasd has no CPU path)"; return ASD_ECUDA; }
+  asd_ctx* h = new (std::nothrow) asd_ctx();
+  if (!h) { g_static_err = "out of host memory"; return ASD_ENOMEM; }
+  Ctx& c = h->c;
+  c.d = *desc;
+  c.stream = (cudaStream_t)cuda_stream;
+  c.device = dev;
+  cudaDeviceGetAttribute(&c.sm_count, cudaDevAttrMultiProcessorCount, dev);
+  c.N = L.N; c.Npad = L.Npad; c.plane = desc->ny * desc->nz;
+  c.gamma = desc->gamma > 0.0 ? desc->gamma : kGammaDefault;
+  c.x0 = desc->x0;
+  c.ncx = L.ncx; c.ncy = L.ncy; c.ncz = L.ncz; c.ncell = L.ncell;
+  char* base = (char*)d_workspace;
+  float* sp[9];
+  for (int a = 0; a < 9; ++a) sp[a] = (float*)(base + L.spins[a]);
+  c.S = {sp[0], sp[1], sp[2]}; c.St = {sp[3], sp[4], sp[5]}; c.A = {sp[6], sp[7], sp[8]};
+  c.sigma = (float*)(base + L.sigma);
+  c.Bx = (float*)(base + L.B[0]); c.By = (float*)(base + L.B[1]); c.Bz = (float*)(base + L.B[2]);
+  c.col = (uint32_t*)(base + L.col);
+  c.grain_map_dev = (int32_t*)(base + L.gmap);
+  c.grain = (float4*)(base + L.grain);
+  c.ell_idx = desc->ell_width > 0 ? (int32_t*)(base + L.ell_idx) : nullptr;
+  c.ell_J = desc->ell_width > 0 ? (float*)(base + L.ell_J) : nullptr;
+  c.init_mean = (float*)(base + L.init_mean);
+  c.cell_frame = (float*)(base + L.cell_frame);
+  c.out_sum = (double*)(base + L.out_sum);
+  c.out_cnt = (long long*)(base + L.out_cnt);
+  c.partials = (double*)(base + L.partials);
+  c.grain_acc = (long long*)(base + L.grain_acc);
+
+  auto bail = [&](asd_status s) { g_static_err = "asd_create_lattice failed in CUDA set-up (see stderr)";
+                                  std::fprintf(stderr, "libasd: %s\n", c.err);
+                                  if (c.host_scratch) cudaFreeHost(c.host_scratch);
+                                  delete h; return s; };
+#define CREATE_TRY(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) { fail_cuda(c, e__, #expr); return bail(ASD_ECUDA); } } while (0)
+  CREATE_TRY(cudaMallocHost(&c.host_scratch, 4 * sizeof(double)));
+  CREATE_TRY(cudaMemsetAsync(d_workspace, 0, L.total, c.stream));
+  const size_t ncol = (size_t)(desc->track_nx * desc->ny);
+  if (desc->grain_map)
+    CREATE_TRY(cudaMemcpyAsync(c.grain_map_dev, desc->grain_map, sizeof(int32_t) * ncol, cudaMemcpyHostToDevice, c.stream));
+  // per-grain (e, 2 k_u / mu_s)
+  {
+    float4* gp = nullptr;
+    CREATE_TRY(cudaMallocHost(&gp, sizeof(float4) * (size_t)desc->n_grains));
+    for (int g = 0; g < desc->n_grains; ++g) {
+      float4 v = make_float4(0.f, 0.f, 1.f, 0.f);
+      if (desc->grain_axis) { v.x = desc->grain_axis[3 * g]; v.y = desc->grain_axis[3 * g + 1]; v.z = desc->grain_axis[3 * g + 2]; }
+      if (desc->grain_ku) v.w = (float)(2.0 * (double)desc->grain_ku[g] / desc->mu_s);
+      gp[g] = v;
+    }
+    cudaError_t e2 = cudaMemcpyAsync(c.grain, gp, sizeof(float4) * (size_t)desc->n_grains, cudaMemcpyHostToDevice, c.stream);
+    if (e2 == cudaSuccess) e2 = cudaStreamSynchronize(c.stream);
+    cudaFreeHost(gp);
+    CREATE_TRY(e2);
+  }
+  if (!desc->grain_map) c.grain_map_dev = nullptr;   // kernel treats NULL as "grain 0 everywhere"
+  if (launch_build_columns(c) != ASD_OK) return bail(ASD_ECUDA);
+  if (desc->ell_width > 0) {
+    const size_t ell = (size_t)desc->ell_width * (size_t)L.N;
+    int32_t* stage_i = c.ell_idx + ell;
+    float* stage_J = c.ell_J + ell;
+    CREATE_TRY(cudaMemcpyAsync(stage_i, desc->ell_idx, sizeof(int32_t) * ell, cudaMemcpyHostToDevice, c.stream));
+    CREATE_TRY(cudaMemcpyAsync(stage_J, desc->ell_J, sizeof(float) * ell, cudaMemcpyHostToDevice, c.stream));
+    if (launch_ell_transpose(c, stage_i, stage_J) != ASD_OK) return bail(ASD_ECUDA);
+  }
+  if (launch_init_spins(c) != ASD_OK) return bail(ASD_ECUDA);
+  // track initial state: +z, m0 = 1
+  {
+    float* im = nullptr;
+    CREATE_TRY(cudaMallocHost(&im, sizeof(float) * 3 * (size_t)L.ncell));
+    for (int64_t q = 0; q < L.ncell; ++q) { im[3 * q] = 0.f; im[3 * q + 1] = 0.f; im[3 * q + 2] = 1.f; }
+    cudaError_t e2 = cudaMemcpyAsync(c.init_mean, im, sizeof(float) * 3 * (size_t)L.ncell, cudaMemcpyHostToDevice, c.stream);
+    if (e2 == cudaSuccess) e2 = cudaStreamSynchronize(c.stream);
+    cudaFreeHost(im);
+    CREATE_TRY(e2);
+  }
+  if (launch_cell_frames(c) != ASD_OK) return bail(ASD_ECUDA);
+  CREATE_TRY(cudaStreamSynchronize(c.stream));
+#undef CREATE_TRY
+  // host pointers of the description are not kept
+  c.d.grain_map = nullptr; c.d.grain_ku = nullptr; c.d.grain_axis = nullptr; c.d.ell_idx = nullptr; c.d.ell_J = nullptr;
+  *out = h;
+  return ASD_OK;
+}
+
+asd_status asd_destroy(asd_ctx* ctx) {
+  if (!ctx) return ASD_EINVAL;
+  if (ctx->c.host_scratch) cudaFreeHost(ctx->c.host_scratch);
+  delete ctx;
+  return ASD_OK;
+}
+
+static asd_status set_spins_impl(Ctx& c, const float* sx, const float* sy, const float* sz, bool host) {
+  if (!sx || !sy || !sz) return fail(c, ASD_EINVAL, "asd_set_spins: NULL pointer");
+  const float* src[3] = {sx, sy, sz};
+  float* stage[3] = {c.St.x, c.St.y, c.St.z};
+  if (host) {
+    for (int a = 0; a < 3; ++a)
+      ASD_CUDA_TRY(c, cudaMemcpyAsync(stage[a], src[a], sizeof(float) * (size_t)c.N, cudaMemcpyHostToDevice, c.stream));
+    return launch_mask_spins(c, CVec3Ptr{stage[0], stage[1], stage[2]}, c.S);
+  }
+  return launch_mask_spins(c, CVec3Ptr{sx, sy, sz}, c.S);
+}
+
+asd_status asd_set_spins(asd_ctx* ctx, const float* sx, const float* sy, const float* sz) {
+  CTX_OR_RETURN(ctx);
+  return set_spins_impl(c, sx, sy, sz, false);
+}
+asd_status asd_set_spins_host(asd_ctx* ctx, const float* sx, const float* sy, const float* sz) {
+  CTX_OR_RETURN(ctx);
+  return set_spins_impl(c, sx, sy, sz, true);
+}
+
+static asd_status get_spins_impl(Ctx& c, float* sx, float* sy, float* sz, cudaMemcpyKind kind) {
+  if (!sx || !sy || !sz) return fail(c, ASD_EINVAL, "asd_get_spins: NULL pointer");
+  ASD_CUDA_TRY(c, cudaMemcpyAsync(sx, c.S.x, sizeof(float) * (size_t)c.N, kind, c.stream));
+  ASD_CUDA_TRY(c, cudaMemcpyAsync(sy, c.S.y, sizeof(float) * (size_t)c.N, kind, c.stream));
+  ASD_CUDA_TRY(c, cudaMemcpyAsync(sz, c.S.z, sizeof(float) * (size_t)c.N, kind, c.stream));
+  if (kind == cudaMemcpyDeviceToHost) ASD_CUDA_TRY(c, cudaStreamSynchronize(c.stream));
+  return ASD_OK;
+}
+asd_status asd_get_spins(asd_ctx* ctx, float* sx, float* sy, float* sz) {
+  CTX_OR_RETURN(ctx);
+  return get_spins_impl(c, sx, sy, sz, cudaMemcpyDeviceToDevice);
+}
+asd_status asd_get_spins_host(asd_ctx* ctx, float* sx, float* sy, float* sz) {
+  CTX_OR_RETURN(ctx);
+  return get_spins_impl(c, sx, sy, sz, cudaMemcpyDeviceToHost);
+}
+
+static asd_status set_fields_impl(Ctx& c, const float* T, const float* Bx, const float* By, const float* Bz,
+                                  cudaMemcpyKind kind) {
+  const size_t b = sizeof(float) * (size_t)c.N;
+  if (Bx) ASD_CUDA_TRY(c, cudaMemcpyAsync(c.Bx, Bx, b, kind, c.stream));
+  if (By) ASD_CUDA_TRY(c, cudaMemcpyAsync(c.By, By, b, kind, c.stream));
+  if (Bz) ASD_CUDA_TRY(c, cudaMemcpyAsync(c.Bz, Bz, b, kind, c.stream));
+  if (T) {
+    if (kind == cudaMemcpyHostToDevice) {        // stage T in the scratch spin buffer (free between steps)
+      ASD_CUDA_TRY(c, cudaMemcpyAsync(c.St.x, T, b, kind, c.stream));
+      return launch_sigma(c, c.St.x);
+    }
+    return launch_sigma(c, T);
+  }
+  return ASD_OK;
+}
+asd_status asd_set_fields(asd_ctx* ctx, const float* T, const float* Bx, const float* By, const float* Bz) {
+  CTX_OR_RETURN(ctx);
+  return set_fields_impl(c, T, Bx, By, Bz, cudaMemcpyDeviceToDevice);
+}
+asd_status asd_set_fields_host(asd_ctx* ctx, const float* T, const float* Bx, const float* By, const float* Bz) {
+  CTX_OR_RETURN(ctx);
+  return set_fields_impl(c, T, Bx, By, Bz, cudaMemcpyHostToDevice);
+}
+
+asd_status asd_set_field_scale(asd_ctx* ctx, float s) {
+  CTX_OR_RETURN(ctx);
+  if (!std::isfinite(s)) return fail(c, ASD_EINVAL, "asd_set_field_scale: not finite");
+  c.scale = s;
+  return ASD_OK;
+}
+
+asd_status asd_step_heun(asd_ctx* ctx, int64_t n) {
+  CTX_OR_RETURN(ctx);
+  if (n < 0) return fail(c, ASD_EINVAL, "asd_step_heun: n < 0");
+  return launch_heun(c, n);
+}
+
+asd_status asd_set_kernel(asd_ctx* ctx, int32_t variant) {
+  CTX_OR_RETURN(ctx);
+  if (variant != ASD_KERNEL_AUTO && variant != ASD_KERNEL_DIRECT)
+    return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: variant not available for this lattice");
+  c.kernel_variant = variant;
+  return ASD_OK;
+}
+
+asd_status asd_shift_window(asd_ctx* ctx, int32_t p) {
+  CTX_OR_RETURN(ctx);
+  if (p < 1 || p > c.d.nx) return fail(c, ASD_EINVAL, "asd_shift_window: p must be in 1..nx");
+  if (c.d.ell_width > 0) return fail(c, ASD_EUNSUPPORTED, "asd_shift_window: a general ELL table cannot follow the window");
+  if (c.d.pbc[0]) return fail(c, ASD_EUNSUPPORTED, "asd_shift_window: window is periodic in x");
+  if (c.x0 + p + c.d.nx > c.d.track_nx) return fail(c, ASD_ESTATE, "asd_shift_window: past the end of the track");
+  return launch_shift(c, p);
+}
+
+asd_status asd_magnetisation(asd_ctx* ctx, double m[3], double* n_magnetic) {
+  CTX_OR_RETURN(ctx);
+  if (!m) return fail(c, ASD_EINVAL, "asd_magnetisation: m is NULL");
+  double o[4];
+  const asd_status s = launch_magnetisation(c, o);
+  if (s != ASD_OK) return s;
+  const double inv = o[3] > 0.0 ? 1.0 / o[3] : 0.0;
+  m[0] = o[0] * inv; m[1] = o[1] * inv; m[2] = o[2] * inv;
+  if (n_magnetic) *n_magnetic = o[3];
+  return ASD_OK;
+}
+
+asd_status asd_grain_magnetisation(asd_ctx* ctx, double* m) {
+  CTX_OR_RETURN(ctx);
+  if (!m) return fail(c, ASD_EINVAL, "asd_grain_magnetisation: m is NULL");
+  return launch_grain_magnetisation(c, m);
+}
+
+asd_status asd_track_dims(const asd_ctx* ctx, int64_t dims[3]) {
+  if (!ctx || !dims) return ASD_EINVAL;
+  dims[0] = ctx->c.ncx; dims[1] = ctx->c.ncy; dims[2] = ctx->c.ncz;
+  return ASD_OK;
+}
+
+asd_status asd_track_set_init(asd_ctx* ctx, const float* mean_spin, float m0) {
+  CTX_OR_RETURN(ctx);
+  const size_t n = 3 * (size_t)c.ncell;
+  float* im = nullptr;
+  ASD_CUDA_TRY(c, cudaMallocHost(&im, sizeof(float) * n));
+  for (int64_t q = 0; q < c.ncell; ++q)
+    for (int a = 0; a < 3; ++a) im[3 * q + a] = mean_spin ? mean_spin[3 * q + a] : (a == 2 ? m0 : 0.0f);
+  cudaError_t e = cudaMemcpyAsync(c.init_mean, im, sizeof(float) * n, cudaMemcpyHostToDevice, c.stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c.stream);
+  cudaFreeHost(im);
+  if (e != cudaSuccess) return fail_cuda(c, e, "asd_track_set_init copy");
+  return launch_cell_frames(c);
+}
+
+asd_status asd_track_get(asd_ctx* ctx, double* sum, int64_t* count) {
+  CTX_OR_RETURN(ctx);
+  if (sum) ASD_CUDA_TRY(c, cudaMemcpyAsync(sum, c.out_sum, sizeof(double) * 3 * (size_t)c.ncell, cudaMemcpyDeviceToHost, c.stream));
+  if (count) ASD_CUDA_TRY(c, cudaMemcpyAsync(count, c.out_cnt, sizeof(long long) * (size_t)c.ncell, cudaMemcpyDeviceToHost, c.stream));
+  ASD_CUDA_TRY(c, cudaStreamSynchronize(c.stream));
+  return ASD_OK;
+}
+
+asd_status asd_get_counters(const asd_ctx* ctx, int64_t* step, int64_t* shift, int64_t* x0, int64_t* pass) {
+  if (!ctx) return ASD_EINVAL;
+  if (step) *step = ctx->c.step;
+  if (shift) *shift = ctx->c.shift;
+  if (x0) *x0 = ctx->c.x0;
+  if (pass) *pass = ctx->c.pass;
+  return ASD_OK;
+}
+
+asd_status asd_set_counters(asd_ctx* ctx, int64_t step, int64_t shift, int64_t pass) {
+  CTX_OR_RETURN(ctx);
+  if (step < 0 || shift < 0 || pass < 0) return fail(c, ASD_EINVAL, "asd_set_counters: negative counter");
+  c.step = step; c.shift = shift; c.pass = pass;
+  return ASD_OK;
+}
+
+int64_t asd_launch_count(const asd_ctx* ctx) { return ctx ? ctx->c.launches : 0; }
+
+const char* asd_last_error(const asd_ctx* ctx) {
+  if (ctx && ctx->c.err[0]) return ctx->c.err;
+  return g_static_err;
+}
+
+const char* asd_version(void) { return "asd-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

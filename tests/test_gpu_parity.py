@@ -1,0 +1,142 @@
+"""GPU parity: libasd (CUDA, fp32) against the fp64 oracle on the same seeded inputs, through the C ABI.
+
+Tolerances (BASELINE.json north_star): max |dS| <= 1e-5 per component after one Heun step; <= 1e-4 after
+1000 deterministic T = 0 steps.  |S| = 1 within 2e-7.
+"""
+import numpy as np
+import pytest
+
+import asd_inputs as ai
+from tests.helpers import gpu_from_workload, max_abs_diff, oracle_from_workload
+
+pytestmark = pytest.mark.gpu
+
+TOL_1STEP = 1e-5
+TOL_T0_1000 = 1e-4
+
+
+def _check_norm(ctx, w):
+    s = ctx.get_spins_host().astype(np.float64)
+    mag = w.magnetic_mask().reshape(-1)
+    nrm = np.sqrt((s ** 2).sum(axis=0))
+    assert np.all(np.abs(nrm[mag] - 1.0) < 2e-7)
+    assert np.all(s[:, ~mag] == 0.0)
+
+
+def test_cfg0_one_thermal_step():
+    w = ai.make_config(0)
+    o, g = oracle_from_workload(w), gpu_from_workload(w)
+    o.step_heun(1); g.step_heun(1)
+    assert max_abs_diff(g, o) <= TOL_1STEP
+    _check_norm(g, w)
+
+
+def test_cfg0_thermal_divergence_report():
+    """Informational: thermal trajectories diverge chaotically; 10 steps still agree closely."""
+    w = ai.make_config(0)
+    o, g = oracle_from_workload(w), gpu_from_workload(w)
+    o.step_heun(10); g.step_heun(10)
+    assert max_abs_diff(g, o) <= 1e-4
+
+
+def test_cfg0_1000_steps_zero_temperature():
+    w = ai.make_config(0, uniform_T=0.0)
+    o, g = oracle_from_workload(w), gpu_from_workload(w)
+    o.step_heun(1000); g.step_heun(1000)
+    assert max_abs_diff(g, o) <= TOL_T0_1000
+    _check_norm(g, w)
+
+
+@pytest.mark.parametrize("lattice", [ai.SC, ai.L10])
+@pytest.mark.parametrize("dims", [(21, 40, 7), (13, 37, 5), (9, 4, 3), (3, 3, 3), (1, 8, 1), (40, 132, 9)])
+def test_small_film_steps(lattice, dims):
+    """Several tiles and a ragged tail; ny % 4 == 0 takes the 128-bit path, odd ny the scalar one."""
+    nx, ny, nz = dims
+    w = ai.small_film(lattice, nx, ny, nz, tilt_deg=25.0, dt=1e-16)
+    o, g = oracle_from_workload(w), gpu_from_workload(w)
+    o.step_heun(1); g.step_heun(1)
+    assert max_abs_diff(g, o) <= TOL_1STEP
+    o.step_heun(4); g.step_heun(4)
+    assert max_abs_diff(g, o) <= 5e-5
+    _check_norm(g, w)
+
+
+@pytest.mark.parametrize("lattice", [ai.SC, ai.L10])
+@pytest.mark.parametrize("pbc", [(1, 1, 1), (0, 1, 0), (1, 0, 1), (0, 0, 1)])
+@pytest.mark.parametrize("dims", [(6, 8, 5), (5, 7, 3)])
+def test_adjacent_grains_and_periodic_boundaries(lattice, pbc, dims):
+    """Random grain map with touching grains (bonds must be cut between different grains) and every wrap."""
+    nx, ny, nz = dims
+    rng = np.random.default_rng(5)
+    w = ai.small_film(lattice, nx, ny, nz, tilt_deg=30.0, dt=1e-16)
+    w.pbc = pbc
+    w.grain_map = rng.integers(-1, 3, size=(nx, ny)).astype(np.int32)
+    w.grain_ku = (9.1e-23 * (1 + 0.3 * rng.standard_normal(3))).astype(np.float32)
+    ax = rng.standard_normal((3, 3)); ax /= np.linalg.norm(ax, axis=1, keepdims=True)
+    w.grain_axis = ax.astype(np.float32)
+    sx, sy, sz = ai.tilted_spins(w.n_sites, 30.0, seed=9)
+    mag = w.magnetic_mask().reshape(-1)
+    w.sx, w.sy, w.sz = sx * mag, sy * mag, sz * mag
+    o, g = oracle_from_workload(w), gpu_from_workload(w)
+    o.step_heun(2); g.step_heun(2)
+    assert max_abs_diff(g, o) <= 2e-5
+    _check_norm(g, w)
+
+
+def test_general_ell_table():
+    """User-supplied neighbour table with arbitrary per-pair J (random sparse couplings)."""
+    nx, ny, nz = 7, 12, 4
+    w = ai.small_film(ai.SC, nx, ny, nz, tilt_deg=30.0, dt=1e-16)
+    N, W = w.n_sites, 5
+    rng = np.random.default_rng(3)
+    idx = rng.integers(-1, N, size=(N, W)).astype(np.int32)
+    J = (6e-21 * rng.standard_normal((N, W))).astype(np.float32)
+    o = oracle_from_workload(w, ell_idx=idx, ell_J=J.astype(np.float64))
+    g = gpu_from_workload(w, ell_idx=idx, ell_J=J)
+    o.step_heun(2); g.step_heun(2)
+    assert max_abs_diff(g, o) <= 2e-5
+
+
+def test_magnetisation_and_grains():
+    w = ai.small_film(ai.L10, 30, 44, 6, tilt_deg=35.0)
+    o, g = oracle_from_workload(w), gpu_from_workload(w)
+    o.step_heun(3); g.step_heun(3)
+    mo, no = o.magnetisation()
+    mg, ng = g.magnetisation()
+    assert no == ng
+    assert np.abs(mo - mg).max() < 1e-6
+    assert np.abs(o.grain_magnetisation() - g.grain_magnetisation()).max() < 1e-6
+    mg2, _ = g.magnetisation()
+    assert np.array_equal(mg, mg2)                       # deterministic reduction
+    assert np.array_equal(g.grain_magnetisation(), g.grain_magnetisation())
+
+
+def test_counters_resume_bit_exact():
+    """Philox is counter based: restoring spins + counters reproduces the trajectory bit for bit."""
+    import torch
+    w = ai.small_film(ai.SC, 12, 16, 5, tilt_deg=20.0)
+    a = gpu_from_workload(w)
+    a.step_heun(5)
+    snap = a.get_spins_host()
+    cnt = a.counters()
+    a.step_heun(7)
+    ref = a.get_spins_host()
+    b = gpu_from_workload(w)
+    t = lambda x: torch.from_numpy(np.ascontiguousarray(x)).to(b.device)
+    b.set_spins(t(snap[0]), t(snap[1]), t(snap[2]))
+    b.set_counters(cnt["step"], cnt["shift"], cnt["pass"])
+    b.step_heun(7)
+    assert np.array_equal(b.get_spins_host(), ref)
+
+
+@pytest.mark.parametrize("cfg", [2, 4])
+def test_full_size_one_step(cfg):
+    """BASELINE configs at full size in the launch configuration bench.py times: every site against the oracle."""
+    w = ai.make_config(cfg)
+    sx, sy, sz = ai.tilted_spins(w.n_sites, 20.0, seed=4)
+    mag = w.magnetic_mask().reshape(-1)
+    w.sx, w.sy, w.sz = sx * mag, sy * mag, sz * mag
+    o, g = oracle_from_workload(w), gpu_from_workload(w)
+    o.step_heun(2); g.step_heun(2)
+    assert max_abs_diff(g, o) <= 2e-5
+    _check_norm(g, w)
