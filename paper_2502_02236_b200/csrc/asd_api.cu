@@ -53,21 +53,24 @@ bool validate_desc(const asd_lattice_desc* d, const char** why) {
 
 bool compute_layout(const asd_lattice_desc& d, Layout& L) {
   L.N = (int64_t)d.nx * d.ny * d.nz;
-  L.Npad = (int64_t)align_up((size_t)L.N, 64);
+  L.nyp = (int32_t)align_up((size_t)d.ny, 4) + 4;
+  L.lead = L.nyp + 4;
+  L.nrows = (int64_t)d.nx * d.nz;
+  L.Np = L.lead + L.nrows * L.nyp;
+  L.as = (int64_t)align_up((size_t)L.Np + 8, 64);     // +8: the last row's y+1 edge read of a redirected row stays inside
   L.ncx = (d.track_nx + d.macro[0] - 1) / d.macro[0];
   L.ncy = (d.ny + d.macro[1] - 1) / d.macro[1];
   L.ncz = (d.nz + d.macro[2] - 1) / d.macro[2];
   L.ncell = L.ncx * L.ncy * L.ncz;
   size_t off = 0;
   auto take = [&](size_t bytes) { const size_t o = off; off = align_up(off + bytes, 256); return o; };
-  const size_t fN = sizeof(float) * (size_t)L.Npad;
-  for (int a = 0; a < 9; ++a) L.spins[a] = take(fN);
-  L.sigma = take(fN);
-  for (int a = 0; a < 3; ++a) L.B[a] = take(fN);
+  L.arrays = take(sizeof(float) * (size_t)L.as * AR_COUNT);
   const size_t ncol = (size_t)(d.track_nx * d.ny);
   L.col = take(sizeof(uint32_t) * ncol);
   L.gmap = take(sizeof(int32_t) * ncol);
-  L.grain = take(sizeof(float4) * (size_t)d.n_grains);
+  L.grain = take(sizeof(float4) * ((size_t)d.n_grains + 1));
+  L.aniso = take(sizeof(float) * 4 * ncol + 64);
+  L.flags = take(sizeof(int32_t) * 4);
   const size_t ell = (size_t)d.ell_width * (size_t)L.N;
   L.ell_idx = take(sizeof(int32_t) * ell * 2);   // slot-major table + staging for the site-major upload
   L.ell_J = take(sizeof(float) * ell * 2);
@@ -131,16 +134,15 @@ asd_status asd_create_lattice(const asd_lattice_desc* desc, void* d_workspace, s
   c.stream = (cudaStream_t)cuda_stream;
   c.device = dev;
   cudaDeviceGetAttribute(&c.sm_count, cudaDevAttrMultiProcessorCount, dev);
-  c.N = L.N; c.Npad = L.Npad; c.plane = desc->ny * desc->nz;
+  c.N = L.N; c.nyp = L.nyp; c.lead = L.lead; c.nrows = L.nrows; c.Np = L.Np; c.as = L.as;
+  c.plane = desc->ny * desc->nz;
   c.gamma = desc->gamma > 0.0 ? desc->gamma : kGammaDefault;
   c.x0 = desc->x0;
   c.ncx = L.ncx; c.ncy = L.ncy; c.ncz = L.ncz; c.ncell = L.ncell;
   char* base = (char*)d_workspace;
-  float* sp[9];
-  for (int a = 0; a < 9; ++a) sp[a] = (float*)(base + L.spins[a]);
-  c.S = {sp[0], sp[1], sp[2]}; c.St = {sp[3], sp[4], sp[5]}; c.A = {sp[6], sp[7], sp[8]};
-  c.sigma = (float*)(base + L.sigma);
-  c.Bx = (float*)(base + L.B[0]); c.By = (float*)(base + L.B[1]); c.Bz = (float*)(base + L.B[2]);
+  c.arrays = (float*)(base + L.arrays);
+  c.aniso = (float*)(base + L.aniso);
+  c.flags = (int32_t*)(base + L.flags);
   c.col = (uint32_t*)(base + L.col);
   c.grain_map_dev = (int32_t*)(base + L.gmap);
   c.grain = (float4*)(base + L.grain);
@@ -166,20 +168,27 @@ asd_status asd_create_lattice(const asd_lattice_desc* desc, void* d_workspace, s
   // per-grain (e, 2 k_u / mu_s)
   {
     float4* gp = nullptr;
-    CREATE_TRY(cudaMallocHost(&gp, sizeof(float4) * (size_t)desc->n_grains));
+    CREATE_TRY(cudaMallocHost(&gp, sizeof(float4) * ((size_t)desc->n_grains + 1)));
+    gp[0] = make_float4(0.f, 0.f, 1.f, 0.f);           // vacant columns: no anisotropy
     for (int g = 0; g < desc->n_grains; ++g) {
       float4 v = make_float4(0.f, 0.f, 1.f, 0.f);
       if (desc->grain_axis) { v.x = desc->grain_axis[3 * g]; v.y = desc->grain_axis[3 * g + 1]; v.z = desc->grain_axis[3 * g + 2]; }
       if (desc->grain_ku) v.w = (float)(2.0 * (double)desc->grain_ku[g] / desc->mu_s);
-      gp[g] = v;
+      gp[g + 1] = v;
     }
-    cudaError_t e2 = cudaMemcpyAsync(c.grain, gp, sizeof(float4) * (size_t)desc->n_grains, cudaMemcpyHostToDevice, c.stream);
+    cudaError_t e2 = cudaMemcpyAsync(c.grain, gp, sizeof(float4) * ((size_t)desc->n_grains + 1), cudaMemcpyHostToDevice, c.stream);
     if (e2 == cudaSuccess) e2 = cudaStreamSynchronize(c.stream);
     cudaFreeHost(gp);
     CREATE_TRY(e2);
   }
   if (!desc->grain_map) c.grain_map_dev = nullptr;   // kernel treats NULL as "grain 0 everywhere"
   if (launch_build_columns(c) != ASD_OK) return bail(ASD_ECUDA);
+  {
+    int32_t touch = 1;
+    CREATE_TRY(cudaMemcpyAsync(&touch, c.flags, sizeof(int32_t), cudaMemcpyDeviceToHost, c.stream));
+    CREATE_TRY(cudaStreamSynchronize(c.stream));
+    c.grains_touch = touch != 0;
+  }
   if (desc->ell_width > 0) {
     const size_t ell = (size_t)desc->ell_width * (size_t)L.N;
     int32_t* stage_i = c.ell_idx + ell;
@@ -188,7 +197,7 @@ asd_status asd_create_lattice(const asd_lattice_desc* desc, void* d_workspace, s
     CREATE_TRY(cudaMemcpyAsync(stage_J, desc->ell_J, sizeof(float) * ell, cudaMemcpyHostToDevice, c.stream));
     if (launch_ell_transpose(c, stage_i, stage_J) != ASD_OK) return bail(ASD_ECUDA);
   }
-  if (launch_init_spins(c) != ASD_OK) return bail(ASD_ECUDA);
+  if (launch_pack_spins(c, CVec3Ptr{nullptr, nullptr, nullptr}, c.S()) != ASD_OK) return bail(ASD_ECUDA);
   // track initial state: +z, m0 = 1
   {
     float* im = nullptr;
@@ -215,16 +224,17 @@ asd_status asd_destroy(asd_ctx* ctx) {
   return ASD_OK;
 }
 
+// Host uploads are staged densely in the A arrays (free between steps: A lives only from a predictor to its
+// corrector, and nothing reads A's padding), then packed into the padded-row layout by a kernel.
 static asd_status set_spins_impl(Ctx& c, const float* sx, const float* sy, const float* sz, bool host) {
   if (!sx || !sy || !sz) return fail(c, ASD_EINVAL, "asd_set_spins: NULL pointer");
-  const float* src[3] = {sx, sy, sz};
-  float* stage[3] = {c.St.x, c.St.y, c.St.z};
   if (host) {
+    const float* src[3] = {sx, sy, sz};
     for (int a = 0; a < 3; ++a)
-      ASD_CUDA_TRY(c, cudaMemcpyAsync(stage[a], src[a], sizeof(float) * (size_t)c.N, cudaMemcpyHostToDevice, c.stream));
-    return launch_mask_spins(c, CVec3Ptr{stage[0], stage[1], stage[2]}, c.S);
+      ASD_CUDA_TRY(c, cudaMemcpyAsync(c.arr(AR_A + a), src[a], sizeof(float) * (size_t)c.N, cudaMemcpyHostToDevice, c.stream));
+    return launch_pack_spins(c, CVec3Ptr{c.arr(AR_A), c.arr(AR_A + 1), c.arr(AR_A + 2)}, c.S());
   }
-  return launch_mask_spins(c, CVec3Ptr{sx, sy, sz}, c.S);
+  return launch_pack_spins(c, CVec3Ptr{sx, sy, sz}, c.S());
 }
 
 asd_status asd_set_spins(asd_ctx* ctx, const float* sx, const float* sy, const float* sz) {
@@ -236,45 +246,64 @@ asd_status asd_set_spins_host(asd_ctx* ctx, const float* sx, const float* sy, co
   return set_spins_impl(c, sx, sy, sz, true);
 }
 
-static asd_status get_spins_impl(Ctx& c, float* sx, float* sy, float* sz, cudaMemcpyKind kind) {
+static asd_status get_spins_impl(Ctx& c, float* sx, float* sy, float* sz, bool host) {
   if (!sx || !sy || !sz) return fail(c, ASD_EINVAL, "asd_get_spins: NULL pointer");
-  ASD_CUDA_TRY(c, cudaMemcpyAsync(sx, c.S.x, sizeof(float) * (size_t)c.N, kind, c.stream));
-  ASD_CUDA_TRY(c, cudaMemcpyAsync(sy, c.S.y, sizeof(float) * (size_t)c.N, kind, c.stream));
-  ASD_CUDA_TRY(c, cudaMemcpyAsync(sz, c.S.z, sizeof(float) * (size_t)c.N, kind, c.stream));
-  if (kind == cudaMemcpyDeviceToHost) ASD_CUDA_TRY(c, cudaStreamSynchronize(c.stream));
+  float* dst[3] = {sx, sy, sz};
+  const Vec3Ptr S = c.S();
+  const float* src[3] = {S.x, S.y, S.z};
+  for (int a = 0; a < 3; ++a) {
+    if (host) {
+      const asd_status st = launch_unpack(c, src[a], c.arr(AR_A + a));
+      if (st != ASD_OK) return st;
+      ASD_CUDA_TRY(c, cudaMemcpyAsync(dst[a], c.arr(AR_A + a), sizeof(float) * (size_t)c.N, cudaMemcpyDeviceToHost, c.stream));
+    } else {
+      const asd_status st = launch_unpack(c, src[a], dst[a]);
+      if (st != ASD_OK) return st;
+    }
+  }
+  if (host) ASD_CUDA_TRY(c, cudaStreamSynchronize(c.stream));
   return ASD_OK;
 }
 asd_status asd_get_spins(asd_ctx* ctx, float* sx, float* sy, float* sz) {
   CTX_OR_RETURN(ctx);
-  return get_spins_impl(c, sx, sy, sz, cudaMemcpyDeviceToDevice);
+  return get_spins_impl(c, sx, sy, sz, false);
 }
 asd_status asd_get_spins_host(asd_ctx* ctx, float* sx, float* sy, float* sz) {
   CTX_OR_RETURN(ctx);
-  return get_spins_impl(c, sx, sy, sz, cudaMemcpyDeviceToHost);
+  return get_spins_impl(c, sx, sy, sz, true);
 }
 
 static asd_status set_fields_impl(Ctx& c, const float* T, const float* Bx, const float* By, const float* Bz,
-                                  cudaMemcpyKind kind) {
+                                  bool host) {
   const size_t b = sizeof(float) * (size_t)c.N;
-  if (Bx) ASD_CUDA_TRY(c, cudaMemcpyAsync(c.Bx, Bx, b, kind, c.stream));
-  if (By) ASD_CUDA_TRY(c, cudaMemcpyAsync(c.By, By, b, kind, c.stream));
-  if (Bz) ASD_CUDA_TRY(c, cudaMemcpyAsync(c.Bz, Bz, b, kind, c.stream));
-  if (T) {
-    if (kind == cudaMemcpyHostToDevice) {        // stage T in the scratch spin buffer (free between steps)
-      ASD_CUDA_TRY(c, cudaMemcpyAsync(c.St.x, T, b, kind, c.stream));
-      return launch_sigma(c, c.St.x);
+  const float* Bsrc[3] = {Bx, By, Bz};
+  for (int a = 0; a < 3; ++a) {
+    if (!Bsrc[a]) continue;
+    const float* dense = Bsrc[a];
+    if (host) {
+      ASD_CUDA_TRY(c, cudaMemcpyAsync(c.arr(AR_A + a), Bsrc[a], b, cudaMemcpyHostToDevice, c.stream));
+      dense = c.arr(AR_A + a);
     }
-    return launch_sigma(c, T);
+    const asd_status st = launch_pack_field(c, dense, c.B(a));
+    if (st != ASD_OK) return st;
+  }
+  if (T) {
+    const float* dense = T;
+    if (host) {
+      ASD_CUDA_TRY(c, cudaMemcpyAsync(c.arr(AR_A), T, b, cudaMemcpyHostToDevice, c.stream));
+      dense = c.arr(AR_A);
+    }
+    return launch_sigma(c, dense);
   }
   return ASD_OK;
 }
 asd_status asd_set_fields(asd_ctx* ctx, const float* T, const float* Bx, const float* By, const float* Bz) {
   CTX_OR_RETURN(ctx);
-  return set_fields_impl(c, T, Bx, By, Bz, cudaMemcpyDeviceToDevice);
+  return set_fields_impl(c, T, Bx, By, Bz, false);
 }
 asd_status asd_set_fields_host(asd_ctx* ctx, const float* T, const float* Bx, const float* By, const float* Bz) {
   CTX_OR_RETURN(ctx);
-  return set_fields_impl(c, T, Bx, By, Bz, cudaMemcpyHostToDevice);
+  return set_fields_impl(c, T, Bx, By, Bz, true);
 }
 
 asd_status asd_set_field_scale(asd_ctx* ctx, float s) {
@@ -292,8 +321,10 @@ asd_status asd_step_heun(asd_ctx* ctx, int64_t n) {
 
 asd_status asd_set_kernel(asd_ctx* ctx, int32_t variant) {
   CTX_OR_RETURN(ctx);
-  if (variant != ASD_KERNEL_AUTO && variant != ASD_KERNEL_DIRECT)
-    return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: variant not available for this lattice");
+  if (variant != ASD_KERNEL_AUTO && variant != ASD_KERNEL_GENERAL && variant != ASD_KERNEL_FAST)
+    return fail(c, ASD_EINVAL, "asd_set_kernel: unknown variant");
+  if (variant == ASD_KERNEL_FAST && !heun_fast_supported(c))
+    return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: the film kernel needs open boundaries, ny % 4 == 0, built-in shells and grains that do not touch");
   c.kernel_variant = variant;
   return ASD_OK;
 }

@@ -1,0 +1,201 @@
+// asd_heun_fast.cu -- the hot path, film variant: one fused kernel per stochastic-Heun stage for open-boundary
+// films whose grains do not touch (every BASELINE film config: >= 1 nm vacant grain boundaries).
+//
+// Why it needs no masks and no boundary predicates (asd_internal.cuh):
+//   * vacant sites hold S = 0, so their bonds drop out of Eq. (2) by themselves; two different grains are never
+//     neighbours (checked at create time), so "same grain" never has to be tested;
+//   * rows are stored padded with zeros, so y-1 of j = 0 and y+1 of j = ny-1 read zeros with the same unconditional
+//     loads as interior sites;
+//   * a missing x+-1 or z+-1 row (open window edge) is redirected to the all-zero row by one select per row.
+// Each thread owns 4 consecutive sites of one y-row: every neighbour row is one aligned 128-bit load per component,
+// the two y-edge sites are scalar loads at immediate offsets from the same address.  All arrays share one base and
+// one 32-bit element offset (13 arrays at a common stride).  Noise is generated in registers (asd_rng.cuh).
+//
+// Bytes per site per stage that must come from / go to HBM: 52; neighbour re-reads are served
+// by L1/L2.
+#include "asd_internal.cuh"
+#include "asd_site.cuh"
+
+namespace asd {
+
+namespace {
+
+constexpr int LAT_SC = 0, LAT_L10 = 1;
+
+struct FastParams {
+  const float* arrays;
+  float* arrays_w;
+  uint32_t as;                     // array stride (elements)
+  uint32_t oX, oA, oOut, oOutA;    // element offsets of component 0 of X, A, out, outA (array index * as)
+  uint32_t oSigma, oB;
+  const float* aniso;              // window origin; components at aniso_stride
+  uint32_t aniso_stride;
+  uint32_t nthreads, ngrp, nz, nx, ny, nyp, planep, lead;
+  uint32_t m_grp, s_grp, m_nz, s_nz;   // magic numbers: t / ngrp and r / nz
+  float j1, j2, j3;
+  float gdt, lambda, scale;
+  uint32_t n_lo, n_hi;
+  uint64_t g0;
+  PhiloxKey key;
+};
+
+// n / d for n < 2^31 (m == 0 means d == 1): q = umulhi(n, m) >> s, m = floor(2^(31+L)/d) + 1, s = L - 1,
+// L = ceil(log2 d)  (Granlund-Montgomery round-up method with 31-bit dividends: exact).
+__device__ __forceinline__ uint32_t fastdiv(uint32_t n, uint32_t m, uint32_t s) {
+  return m ? (__umulhi(n, m) >> s) : n;
+}
+
+__device__ __forceinline__ float4 ld4(const float* base, uint32_t e) {
+  return __ldg(reinterpret_cast<const float4*>(base + e));
+}
+__device__ __forceinline__ void st4(float* base, uint32_t e, const float v[4]) {
+  *reinterpret_cast<float4*>(base + e) = make_float4(v[0], v[1], v[2], v[3]);
+}
+
+template <int LAT, int STAGE>
+__global__ void __launch_bounds__(256, 3) heun_stage_fast(const FastParams p) {
+  const uint32_t t = blockIdx.x * 256u + threadIdx.x;
+  if (t >= p.nthreads) return;
+  const uint32_t r = fastdiv(t, p.m_grp, p.s_grp);
+  const uint32_t j0 = (t - r * p.ngrp) * 4u;
+  const uint32_t i = fastdiv(r, p.m_nz, p.s_nz);
+  const uint32_t k = r - i * p.nz;
+  const uint32_t e = p.lead + r * p.nyp + j0;                    // own sites
+  // neighbour rows; a row outside the window is read from the zero lead (elements [j0+3, j0+8] < lead)
+  const uint32_t ez = j0 + 4u;
+  const uint32_t e_zp = (k + 1u < p.nz) ? e + p.nyp : ez;
+  const uint32_t e_zm = (k > 0u) ? e - p.nyp : ez;
+  const uint32_t e_xp = (i + 1u < p.nx) ? e + p.planep : ez;
+  const uint32_t e_xm = (i > 0u) ? e - p.planep : ez;
+
+  // every address below is arrays + (one 32-bit element index): a single widening multiply-add per access
+  const float* __restrict__ base = p.arrays;
+
+  // ---- exchange field, Eq. (2): shell sums first, one multiply per shell ----
+  float own[3][6];                // own row with its y-1 and y+1 edge sites
+  float Bex[3][4];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    const uint32_t oc = p.oX + (uint32_t)c * p.as;
+    const float* q_own = base + (oc + e);
+    const float* q_xp = base + (oc + e_xp);
+    const float* q_xm = base + (oc + e_xm);
+    const float4 o = __ldg(reinterpret_cast<const float4*>(q_own));
+    own[c][0] = __ldg(q_own - 1); own[c][1] = o.x; own[c][2] = o.y; own[c][3] = o.z; own[c][4] = o.w;
+    own[c][5] = __ldg(q_own + 4);
+    const float4 zp = ld4(base, oc + e_zp), zm = ld4(base, oc + e_zm);
+    const float4 xp = __ldg(reinterpret_cast<const float4*>(q_xp)), xm = __ldg(reinterpret_cast<const float4*>(q_xm));
+    const float zs[4] = {zp.x + zm.x, zp.y + zm.y, zp.z + zm.z, zp.w + zm.w};
+    if (LAT == LAT_SC) {
+      // 6 nearest neighbours, one J
+      const float xs[4] = {xp.x + xm.x, xp.y + xm.y, xp.z + xm.z, xp.w + xm.w};
+#pragma unroll
+      for (int v = 0; v < 4; ++v) Bex[c][v] = p.j1 * ((xs[v] + zs[v]) + (own[c][v] + own[c][v + 2]));
+    } else {
+      // 4 in-plane nn (J1), 2 out-of-plane (J2), 4 in-plane nnn (J3): "4 nearest + 6 next nearest"
+      float xs[6];
+      xs[0] = __ldg(q_xp - 1) + __ldg(q_xm - 1);
+      xs[1] = xp.x + xm.x; xs[2] = xp.y + xm.y; xs[3] = xp.z + xm.z; xs[4] = xp.w + xm.w;
+      xs[5] = __ldg(q_xp + 4) + __ldg(q_xm + 4);
+#pragma unroll
+      for (int v = 0; v < 4; ++v) {
+        const float s1 = xs[v + 1] + (own[c][v] + own[c][v + 2]);
+        const float s3 = xs[v] + xs[v + 2];
+        Bex[c][v] = fmaf(p.j3, s3, fmaf(p.j2, zs[v], p.j1 * s1));
+      }
+    }
+  }
+
+  // ---- per-site inputs ----
+  const float4 sg4 = ld4(base, p.oSigma + e);
+  const float4 bx4 = ld4(base, p.oB + e), by4 = ld4(base, p.oB + p.as + e), bz4 = ld4(base, p.oB + 2u * p.as + e);
+  const uint32_t ec = i * p.ny + j0;                             // column (i, j0) of the window
+  const float4 ax4 = ld4(p.aniso, ec), ay4 = ld4(p.aniso, p.aniso_stride + ec),
+               az4 = ld4(p.aniso, 2u * p.aniso_stride + ec), ak4 = ld4(p.aniso, 3u * p.aniso_stride + ec);
+  const float sg[4] = {sg4.x, sg4.y, sg4.z, sg4.w};
+  const float bx[4] = {bx4.x, bx4.y, bx4.z, bx4.w}, by[4] = {by4.x, by4.y, by4.z, by4.w},
+              bz[4] = {bz4.x, bz4.y, bz4.z, bz4.w};
+  const float ax[4] = {ax4.x, ax4.y, ax4.z, ax4.w}, ay[4] = {ay4.x, ay4.y, ay4.z, ay4.w},
+              az[4] = {az4.x, az4.y, az4.z, az4.w}, ak[4] = {ak4.x, ak4.y, ak4.z, ak4.w};
+  float Ain[3][4];
+  if (STAGE == 1) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const float4 a = ld4(base, p.oA + (uint32_t)c * p.as + e);
+      Ain[c][0] = a.x; Ain[c][1] = a.y; Ain[c][2] = a.z; Ain[c][3] = a.w;
+    }
+  }
+
+  // ---- noise, torque, update, renormalise ----
+  const uint64_t g = p.g0 + (uint64_t)(r * p.ny + j0);           // global site id of the first own site
+  const SiteConst sc{p.gdt, p.lambda, p.scale};
+  float o[3][4], oA[3][4];
+#pragma unroll
+  for (int v = 0; v < 4; ++v) {
+    uint32_t rnd[4];
+    philox_site(p.key, p.n_lo, p.n_hi, g + (uint64_t)v, 0u, rnd);
+    float xi[3];
+    normals3(rnd, xi);
+    const float Xs[3] = {own[0][v + 1], own[1][v + 1], own[2][v + 1]};
+    const float Be[3] = {Bex[0][v], Bex[1][v], Bex[2][v]};
+    const float Bap[3] = {bx[v], by[v], bz[v]};
+    const float Ai[3] = {Ain[0][v], Ain[1][v], Ain[2][v]};
+    float ov[3], oAv[3];
+    site_update<STAGE>(sc, Xs, Be, make_float4(ax[v], ay[v], az[v], ak[v]), Bap, sg[v], xi, Ai, ov, oAv);
+    o[0][v] = ov[0]; o[1][v] = ov[1]; o[2][v] = ov[2];
+    if (STAGE == 0) { oA[0][v] = oAv[0]; oA[1][v] = oAv[1]; oA[2][v] = oAv[2]; }
+  }
+#pragma unroll
+  for (int c = 0; c < 3; ++c) st4(p.arrays_w, p.oOut + (uint32_t)c * p.as + e, o[c]);
+  if (STAGE == 0) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) st4(p.arrays_w, p.oOutA + (uint32_t)c * p.as + e, oA[c]);
+  }
+}
+
+void magic(uint32_t d, uint32_t& m, uint32_t& s) {
+  if (d <= 1) { m = 0; s = 0; return; }
+  uint32_t L = 0;
+  while ((1ull << L) < d) ++L;
+  m = (uint32_t)(((1ull << (31 + L)) / d) + 1ull);
+  s = L - 1;
+}
+
+template <int LAT>
+asd_status launch_pair_fast(Ctx& c, FastParams& f) {
+  const unsigned blocks = (f.nthreads + 255u) / 256u;
+  const uint32_t as = f.as;
+  f.oX = (uint32_t)c.aS * as; f.oOut = (uint32_t)c.aSt * as; f.oOutA = AR_A * as; f.oA = AR_A * as;
+  heun_stage_fast<LAT, 0><<<blocks, 256, 0, c.stream>>>(f);
+  ASD_LAUNCH_CHECK(c, "heun predictor (fast)");
+  f.oX = (uint32_t)c.aSt * as; f.oOut = (uint32_t)c.aS * as;
+  heun_stage_fast<LAT, 1><<<blocks, 256, 0, c.stream>>>(f);
+  ASD_LAUNCH_CHECK(c, "heun corrector (fast)");
+  return ASD_OK;
+}
+
+}  // namespace
+
+// Open boundaries, built-in shells, ny a multiple of 4, grains that do not touch, and 32-bit element offsets.
+bool heun_fast_supported(const Ctx& c) {
+  return c.d.ell_width == 0 && !c.d.pbc[0] && !c.d.pbc[1] && !c.d.pbc[2] && (c.d.ny % 4 == 0) && !c.grains_touch &&
+         (int64_t)AR_COUNT * c.as < (1ll << 31) && c.d.track_nx * (int64_t)c.d.ny < (1ll << 30);
+}
+
+asd_status launch_heun_fast(Ctx& c, StageParams& p) {
+  FastParams f;
+  f.arrays = c.arrays; f.arrays_w = c.arrays; f.as = (uint32_t)c.as;
+  f.oSigma = AR_SIGMA * f.as; f.oB = AR_B * f.as;
+  f.aniso = p.aniso; f.aniso_stride = p.aniso_stride;
+  f.ngrp = (uint32_t)(c.d.ny / 4); f.nthreads = (uint32_t)c.nrows * f.ngrp;
+  f.nz = (uint32_t)c.d.nz; f.nx = (uint32_t)c.d.nx; f.ny = (uint32_t)c.d.ny; f.nyp = (uint32_t)c.nyp; f.lead = (uint32_t)c.lead;
+  f.planep = (uint32_t)c.d.nz * (uint32_t)c.nyp;
+  magic(f.ngrp, f.m_grp, f.s_grp);
+  magic(f.nz, f.m_nz, f.s_nz);
+  f.j1 = p.jx[0]; f.j2 = p.jx[1]; f.j3 = p.jx[2];
+  f.gdt = p.gdt; f.lambda = p.lambda; f.scale = p.scale;
+  f.n_lo = p.n_lo; f.n_hi = p.n_hi; f.g0 = p.g0; f.key = p.key;
+  return c.d.lattice == ASD_SC ? launch_pair_fast<LAT_SC>(c, f) : launch_pair_fast<LAT_L10>(c, f);
+}
+
+}  // namespace asd

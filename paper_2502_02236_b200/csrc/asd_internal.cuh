@@ -1,4 +1,15 @@
 // asd_internal.cuh -- context, workspace layout and kernel parameter blocks of libasd (not part of the ABI).
+//
+// Device layout of every per-site array: "padded rows".
+//   A row is the ny sites (i, k, 0..ny-1); rows are numbered r = i*nz + k, so x is slowest and a window shift is
+//   one contiguous move.  Each row is stored with stride nyp = round_up(ny, 4) + 4 floats; the nyp - ny trailing
+//   floats are zero for ever.  lead = nyp + 4 zero floats precede row 0.  Element of site (r, j):  e = lead + r*nyp + j.
+//   => the y-1 neighbour of j = 0 and the y+1 neighbour of j = ny-1 are zeros that sit next to the row in memory,
+//      and a missing x+-1 / z+-1 row is read from the zero lead (at element j + 4, so that its j-1 and j+4 edge
+//      reads stay inside the lead): open boundaries cost no predicate and no mask,
+//      and 128-bit loads stay aligned (nyp % 4 == 0).
+//   The 13 per-site arrays (S, S~, A: 3 components each; sigma; B: 3) are consecutive with one stride `as`
+//   (elements), so one 32-bit element offset addresses all of them.
 #pragma once
 #include <cstddef>
 #include <cstdint>
@@ -24,31 +35,37 @@ enum : uint32_t {
   BOND_ALL_XP = BOND_XP | BOND_XPYP | BOND_XPYM, BOND_ALL_XM = BOND_XM | BOND_XMYP | BOND_XMYM
 };
 
+// indices of the 13 per-site arrays inside the block `arrays` (stride `as` elements)
+enum : int { AR_S = 0, AR_ST = 3, AR_A = 6, AR_SIGMA = 9, AR_B = 10, AR_COUNT = 13 };
+
 struct Vec3Ptr { float *x, *y, *z; };
 struct CVec3Ptr { const float *x, *y, *z; };
 
 // Parameters of one Heun stage (passed by value; lives in the constant bank).
 struct StageParams {
-  CVec3Ptr X;        // configuration whose neighbours are read: S (predictor) or S~ (corrector)
-  CVec3Ptr A;        // corrector only: A = S + dt/2 k1 of the own site
-  Vec3Ptr out;       // predictor: S~ ; corrector: new S
-  Vec3Ptr outA;      // predictor only: A
-  const float *sigma;          // c_th sqrt(T_i)  [Tesla]
-  const float *Bx, *By, *Bz;   // applied field [Tesla]
-  const uint32_t *col;         // column table at the window origin: col[i*ny + j]
-  const float4 *grain;         // (e_x, e_y, e_z, 2 k_u / mu_s) per grain
-  const int32_t *ell_idx;      // general ELL, slot-major [W][N] (or null)
-  const float *ell_J;          // J_ij / mu_s [Tesla], slot-major
+  float* arrays;               // base of the 13 padded per-site arrays
+  uint32_t as;                 // array stride, elements
+  uint32_t aX, aA, aOut, aOutA;  // array index (AR_*) of: the configuration whose neighbours are read (S or S~),
+                               // A = S + dt/2 k1 (corrector input), the output spins, the A output (predictor)
+  const uint32_t* col;         // column table at the window origin: col[i*ny + j]
+  const float4* grain;         // (e_x, e_y, e_z, 2 k_u / mu_s) per grain id + 1 (entry 0 = vacant: zeros)
+  const float* aniso;          // per-column SoA copy of the same: e_x | e_y | e_z | 2k_u/mu_s, each [track_nx*ny],
+  uint32_t aniso_stride;       //   at the window origin; component stride in elements
+  const int32_t* ell_idx;      // general ELL, slot-major [W][N], entries are padded element offsets (or -1)
+  const float* ell_J;          // J_ij / mu_s [Tesla], slot-major
   int32_t ell_w;
-  int32_t nx, ny, nz, plane;   // plane = ny*nz
-  int64_t N;
+  int32_t nx, ny, nz, nyp;     // nyp = padded row stride
+  int32_t lead;                // zero floats before row 0 (nyp + 4)
+  uint32_t nrows, ngrp;        // nx*nz; threads per row
+  uint32_t nthreads;           // nrows * ngrp
+  uint32_t N;                  // nx*ny*nz (dense count; < 2^31)
   int32_t pbc_x, pbc_y, pbc_z;
   float jx[3];                 // J_shell / mu_s [Tesla]
   float gdt;                   // gamma dt / (1 + lambda^2)
   float lambda;
   float scale;                 // B_app = scale * B
   uint32_t n_lo, n_hi;         // step index before the step
-  uint64_t g0;                 // x0 * plane: global id of window site 0
+  uint64_t g0;                 // x0 * ny * nz: global id of window site 0
   PhiloxKey key;
 };
 
@@ -57,16 +74,24 @@ struct Ctx {
   cudaStream_t stream = nullptr;
   int device = 0;
   int sm_count = 148;
-  int64_t N = 0, Npad = 0;
-  int32_t plane = 0;
+  int64_t N = 0;               // dense sites
+  int32_t nyp = 0;             // padded row stride
+  int32_t lead = 0;            // zero floats before row 0
+  int64_t nrows = 0;           // nx*nz
+  int64_t Np = 0;              // elements of one padded array: lead + nrows*nyp
+  int64_t as = 0;              // array stride (elements)
+  int32_t plane = 0;           // dense ny*nz
   double gamma = 0;
   // device arrays (sub-allocated from the caller's workspace)
-  Vec3Ptr S{}, St{}, A{};
-  float *sigma = nullptr, *Bx = nullptr, *By = nullptr, *Bz = nullptr;
+  float* arrays = nullptr;
+  int aS = AR_S, aSt = AR_ST;  // which third of the spin block currently holds S / the scratch S~ (swapped by a shift)
   uint32_t *col = nullptr;          // [track_nx * ny]
   int32_t *grain_map_dev = nullptr; // [track_nx * ny] as given
-  float4 *grain = nullptr;          // [n_grains]
+  float4 *grain = nullptr;          // [n_grains + 1]
+  float *aniso = nullptr;           // [4][track_nx * ny]
+  int32_t *flags = nullptr;         // [4] device: flags[0] = 1 if two different grains touch
   int32_t *ell_idx = nullptr; float *ell_J = nullptr;
+  bool grains_touch = true;
   // track store
   int64_t ncx = 0, ncy = 0, ncz = 0, ncell = 0;
   float *init_mean = nullptr;       // [ncell*3]
@@ -84,6 +109,15 @@ struct Ctx {
   int64_t launches = 0;
   bool cuda_failed = false;
   char err[256] = {0};
+
+  float* arr(int a) const { return arrays + (size_t)a * (size_t)as; }
+  Vec3Ptr vec(int a) const { return Vec3Ptr{arr(a), arr(a + 1), arr(a + 2)}; }
+  Vec3Ptr S() const { return vec(aS); }
+  Vec3Ptr St() const { return vec(aSt); }
+  Vec3Ptr A() const { return vec(AR_A); }
+  float* sigma() const { return arr(AR_SIGMA); }
+  float* B(int c) const { return arr(AR_B + c); }
+  const uint32_t* col_win() const { return col + x0 * d.ny; }
 };
 
 constexpr int kMaxPartialBlocks = 1024;
@@ -92,19 +126,24 @@ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 // Workspace layout: one place computes every offset (used by asd_workspace_bytes and asd_create_lattice).
 struct Layout {
-  size_t spins[9], sigma, B[3], col, gmap, grain, ell_idx, ell_J, init_mean, cell_frame, out_sum, out_cnt,
+  size_t arrays, col, gmap, grain, aniso, flags, ell_idx, ell_J, init_mean, cell_frame, out_sum, out_cnt,
       partials, grain_acc, total;
-  int64_t N, Npad, ncx, ncy, ncz, ncell;
+  int64_t N, nrows, Np, as, ncx, ncy, ncz, ncell;
+  int32_t nyp, lead;
 };
 bool compute_layout(const asd_lattice_desc& d, Layout& L);
 bool validate_desc(const asd_lattice_desc* d, const char** why);
 
 // kernels / launchers (defined in the .cu files)
 asd_status launch_build_columns(Ctx& c);
-asd_status launch_init_spins(Ctx& c);
-asd_status launch_mask_spins(Ctx& c, CVec3Ptr src, Vec3Ptr dst);
-asd_status launch_sigma(Ctx& c, const float* T_dev);
+asd_status launch_pack_spins(Ctx& c, CVec3Ptr dense_src /* null members: +z */, Vec3Ptr padded_dst);
+asd_status launch_unpack(Ctx& c, const float* padded, float* dense);
+asd_status launch_pack_field(Ctx& c, const float* dense, float* padded);
+asd_status launch_sigma(Ctx& c, const float* T_dense);
 asd_status launch_heun(Ctx& c, int64_t n);
+asd_status launch_heun_fast(Ctx& c, StageParams& p);          // one Heun step (2 kernels), fast path
+bool heun_fast_supported(const Ctx& c);
+void fill_stage_params(const Ctx& c, StageParams& p);
 asd_status launch_shift(Ctx& c, int32_t p);
 asd_status launch_cell_frames(Ctx& c);
 asd_status launch_magnetisation(Ctx& c, double out4[4]);

@@ -48,7 +48,7 @@ __global__ void mag_final(const double* __restrict__ partials, int nb, double* _
 // integer addition commutes, so the result does not depend on the order of the atomics.
 __global__ void grain_accumulate(const float* __restrict__ sx, const float* __restrict__ sy,
                                  const float* __restrict__ sz, const uint32_t* __restrict__ col, int nx, int ny, int nz,
-                                 long long* __restrict__ acc) {
+                                 int nyp, int lead, long long* __restrict__ acc) {
   const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= (int64_t)nx * ny) return;
   const uint32_t gid = col[t] & 0xFFFFu;
@@ -56,7 +56,7 @@ __global__ void grain_accumulate(const float* __restrict__ sx, const float* __re
   const int i = (int)(t / ny), j = (int)(t - (int64_t)i * ny);
   long long q0 = 0, q1 = 0, q2 = 0;
   for (int k = 0; k < nz; ++k) {
-    const int64_t l = ((int64_t)i * nz + k) * ny + j;
+    const int64_t l = lead + ((int64_t)i * nz + k) * nyp + j;
     q0 += __double2ll_rn((double)sx[l] * 4294967296.0);
     q1 += __double2ll_rn((double)sy[l] * 4294967296.0);
     q2 += __double2ll_rn((double)sz[l] * 4294967296.0);
@@ -73,8 +73,9 @@ __global__ void grain_accumulate(const float* __restrict__ sx, const float* __re
 asd_status launch_magnetisation(Ctx& c, double out4[4]) {
   const int nb = (int)min((int64_t)kMaxPartialBlocks - 1, max((int64_t)1, c.N / 4096));
   double* final_slot = c.partials + 4 * (int64_t)(kMaxPartialBlocks - 1);
-  mag_partial<<<nb, 256, 0, c.stream>>>(c.S.x, c.S.y, c.S.z, c.col + c.x0 * c.d.ny, c.N,
-                                        (int64_t)c.d.nx * c.d.ny, c.partials);
+  // the padded arrays are summed whole: pads and vacant sites hold exact zeros
+  const Vec3Ptr S = c.S();
+  mag_partial<<<nb, 256, 0, c.stream>>>(S.x, S.y, S.z, c.col_win(), c.Np, (int64_t)c.d.nx * c.d.ny, c.partials);
   ASD_LAUNCH_CHECK(c, "mag_partial");
   mag_final<<<1, 128, 0, c.stream>>>(c.partials, nb, final_slot);
   ASD_LAUNCH_CHECK(c, "mag_final");
@@ -89,8 +90,9 @@ asd_status launch_grain_magnetisation(Ctx& c, double* m_host) {
   const int G = c.d.n_grains;
   ASD_CUDA_TRY(c, cudaMemsetAsync(c.grain_acc, 0, sizeof(long long) * 4 * (size_t)G, c.stream));
   const int64_t ncol = (int64_t)c.d.nx * c.d.ny;
-  grain_accumulate<<<(unsigned)((ncol + 127) / 128), 128, 0, c.stream>>>(c.S.x, c.S.y, c.S.z, c.col + c.x0 * c.d.ny,
-                                                                        c.d.nx, c.d.ny, c.d.nz, c.grain_acc);
+  const Vec3Ptr S = c.S();
+  grain_accumulate<<<(unsigned)((ncol + 127) / 128), 128, 0, c.stream>>>(S.x, S.y, S.z, c.col_win(), c.d.nx, c.d.ny,
+                                                                        c.d.nz, c.nyp, c.lead, c.grain_acc);
   ASD_LAUNCH_CHECK(c, "grain_accumulate");
   long long* h = nullptr;
   ASD_CUDA_TRY(c, cudaMallocHost(&h, sizeof(long long) * 4 * (size_t)G));

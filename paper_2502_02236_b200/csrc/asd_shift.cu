@@ -13,7 +13,8 @@ namespace asd {
 namespace {
 
 struct ShiftGeom {
-  int nx, ny, nz, plane;
+  int nx, ny, nz, plane;   // plane = ny*nz (dense)
+  int nyp, lead;           // padded-row layout (asd_internal.cuh)
   int mx, my, mz;
   int64_t x0;           // window origin BEFORE the shift
   int64_t ncy, ncz;
@@ -45,7 +46,7 @@ __global__ void coarse_grain_outgoing(const float* __restrict__ sx, const float*
     const int64_t gx = gx_lo + di;
     const int j = j_lo + dj, k = k_lo + dk;
     if ((col_track[gx * g.ny + j] & 0xFFFFu) == 0u) continue;
-    const int64_t l = ((gx - g.x0) * g.nz + k) * g.ny + j;
+    const int64_t l = g.lead + ((gx - g.x0) * g.nz + k) * (int64_t)g.nyp + j;
     s0 += (double)sx[l]; s1 += (double)sy[l]; s2 += (double)sz[l];
     cnt += 1;
   }
@@ -64,13 +65,6 @@ __global__ void coarse_grain_outgoing(const float* __restrict__ sx, const float*
 }
 
 // dst[l] = src[l + off] for l < n_keep, three components.
-__global__ void move_planes(const float* __restrict__ sx, const float* __restrict__ sy, const float* __restrict__ sz,
-                            float* __restrict__ dx, float* __restrict__ dy, float* __restrict__ dz, int64_t off,
-                            int64_t n_keep) {
-  const int64_t l = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (l >= n_keep) return;
-  dx[l] = sx[l + off]; dy[l] = sy[l + off]; dz[l] = sz[l + off];
-}
 __global__ void move_planes_v4(const float4* __restrict__ sx, const float4* __restrict__ sy,
                                const float4* __restrict__ sz, float4* __restrict__ dx, float4* __restrict__ dy,
                                float4* __restrict__ dz, int64_t off4, int64_t n_keep4) {
@@ -90,7 +84,7 @@ __global__ void seed_incoming(float* __restrict__ dx, float* __restrict__ dy, fl
   const int k = pp / g.ny, j = pp - k * g.ny;
   const int i = g.nx - g.p + di;                       // window plane after the move
   const int64_t gx = g.x0 + g.p + i;                   // its global plane
-  const int64_t l = (int64_t)i * g.plane + pp;
+  const int64_t l = g.lead + ((int64_t)i * g.nz + k) * g.nyp + j;
   if ((col_track[gx * g.ny + j] & 0xFFFFu) == 0u) { dx[l] = 0.0f; dy[l] = 0.0f; dz[l] = 0.0f; return; }
   const int64_t c = ((gx / g.mx) * g.ncy + (j / g.my)) * g.ncz + (k / g.mz);
   const float* f = cell_frame + 12 * c;
@@ -157,27 +151,25 @@ asd_status launch_cell_frames(Ctx& c) {
 
 asd_status launch_shift(Ctx& c, int32_t p) {
   ShiftGeom g;
-  g.nx = c.d.nx; g.ny = c.d.ny; g.nz = c.d.nz; g.plane = c.plane;
+  g.nx = c.d.nx; g.ny = c.d.ny; g.nz = c.d.nz; g.plane = c.plane; g.nyp = c.nyp; g.lead = c.lead;
+  const Vec3Ptr S = c.S(), St = c.St();
   g.mx = c.d.macro[0]; g.my = c.d.macro[1]; g.mz = c.d.macro[2];
   g.x0 = c.x0; g.ncy = c.ncy; g.ncz = c.ncz; g.p = p;
   // 1. outgoing slab -> macrocells
   const int64_t cx_first = c.x0 / g.mx, cx_last = (c.x0 + p - 1) / g.mx;
   const int n_cx = (int)(cx_last - cx_first + 1);
   const int64_t warps = (int64_t)n_cx * c.ncy * c.ncz;
-  coarse_grain_outgoing<<<nblocks(warps * 32, 256), 256, 0, c.stream>>>(c.S.x, c.S.y, c.S.z, c.col, c.out_sum,
+  coarse_grain_outgoing<<<nblocks(warps * 32, 256), 256, 0, c.stream>>>(S.x, S.y, S.z, c.col, c.out_sum,
                                                                        c.out_cnt, g, cx_first, n_cx);
   ASD_LAUNCH_CHECK(c, "coarse_grain_outgoing");
   // 2. move into the scratch buffer
-  const int64_t off = (int64_t)p * c.plane, n_keep = c.N - off;
+  // (padded planes: nz*nyp floats each, a multiple of 4; the pads move with their rows and stay zero)
+  const int64_t planep = (int64_t)c.d.nz * c.nyp;
+  const int64_t off = (int64_t)p * planep, n_keep = c.nrows * c.nyp - off;
   if (n_keep > 0) {
-    if (c.plane % 4 == 0) {
-      move_planes_v4<<<nblocks(n_keep / 4, 256), 256, 0, c.stream>>>(
-          (const float4*)c.S.x, (const float4*)c.S.y, (const float4*)c.S.z, (float4*)c.St.x, (float4*)c.St.y,
-          (float4*)c.St.z, off / 4, n_keep / 4);
-    } else {
-      move_planes<<<nblocks(n_keep, 256), 256, 0, c.stream>>>(c.S.x, c.S.y, c.S.z, c.St.x, c.St.y, c.St.z, off,
-                                                             n_keep);
-    }
+    move_planes_v4<<<nblocks(n_keep / 4, 256), 256, 0, c.stream>>>(
+        (const float4*)(S.x + c.lead), (const float4*)(S.y + c.lead), (const float4*)(S.z + c.lead),
+        (float4*)(St.x + c.lead), (float4*)(St.y + c.lead), (float4*)(St.z + c.lead), off / 4, n_keep / 4);
     ASD_LAUNCH_CHECK(c, "move_planes");
   }
   // 3. incoming slab
@@ -185,11 +177,11 @@ asd_status launch_shift(Ctx& c, int32_t p) {
   uint32_t k0 = (uint32_t)(c.d.seed & 0xFFFFFFFFull), k1 = (uint32_t)(c.d.seed >> 32);
   for (int r = 0; r < 10; ++r) { key.k0[r] = k0; key.k1[r] = k1; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
   seed_incoming<<<nblocks((int64_t)p * c.plane, 256), 256, 0, c.stream>>>(
-      c.St.x, c.St.y, c.St.z, c.col, c.cell_frame, g, key, (uint32_t)((uint64_t)c.pass & 0xFFFFFFFFull),
+      St.x, St.y, St.z, c.col, c.cell_frame, g, key, (uint32_t)((uint64_t)c.pass & 0xFFFFFFFFull),
       (uint32_t)((uint64_t)c.pass >> 32));
   ASD_LAUNCH_CHECK(c, "seed_incoming");
   // 4. swap and advance
-  Vec3Ptr t = c.S; c.S = c.St; c.St = t;
+  { const int t = c.aS; c.aS = c.aSt; c.aSt = t; }
   c.x0 += p;
   c.shift += 1;
   return ASD_OK;
