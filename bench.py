@@ -113,6 +113,14 @@ def _workload(cfg: int, seed_offset: int = 0) -> ai.Workload:
     return w
 
 
+def _gpu_desc(asd, w: ai.Workload):
+    """Workload -> asd.LatticeDesc (argument marshalling; the product path never imports oracle/ or tests/)."""
+    return asd.LatticeDesc(lattice=w.lattice, nx=w.nx, ny=w.ny, nz=w.nz, pbc=w.pbc, mu_s=w.mu_s, lam=w.lam,
+                           gamma=w.gamma, dt=w.dt, J=w.J, track_nx=w.track_nx, x0=w.x0, grain_map=w.grain_map,
+                           n_grains=w.n_grains, grain_ku=w.grain_ku, grain_axis=w.grain_axis, macro=w.macro,
+                           seed=w.seed)
+
+
 def _drive(w: ai.Workload, heun_per_step: int):
     """Per bench step: (field scale, planes to shift after the step or 0).  DESIGN.md Q8 schedule."""
     bits = ai.nrz_bits(64, w.bit_seed)
@@ -133,7 +141,6 @@ def _drive(w: ai.Workload, heun_per_step: int):
 def run_ours(args):
     import torch
     import paper_2502_02236_b200 as asd
-    from tests.helpers import gpu_desc
 
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -153,7 +160,7 @@ def run_ours(args):
 
     w = _workload(args.config, seed_offset=rank)
     N = w.n_sites
-    ctx = asd.Context(gpu_desc(w), device=f"cuda:{local}")
+    ctx = asd.Context(_gpu_desc(asd, w), device=f"cuda:{local}")
     dev = ctx.device
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory()
     hT, hBx, hBy, hBz = pin(w.T), pin(w.Bx), pin(w.By), pin(w.Bz)
