@@ -113,6 +113,19 @@ def _workload(cfg: int, seed_offset: int = 0) -> ai.Workload:
     return w
 
 
+def reduce_over_ranks(ms_local: float, updates_local: float, dist=None, device="cpu"):
+    """Whole-job figures from per-rank ones: time = MAX over ranks, work = SUM over ranks (replicas, DESIGN.md
+    sec. 9).  `dist` is torch.distributed (any backend) or None for a single process."""
+    if dist is None:
+        return ms_local, updates_local
+    import torch
+    t = torch.tensor([ms_local], device=device, dtype=torch.float64)
+    u = torch.tensor([updates_local], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
 def _gpu_desc(asd, w: ai.Workload):
     """Workload -> asd.LatticeDesc (argument marshalling; the product path never imports oracle/ or tests/)."""
     return asd.LatticeDesc(lattice=w.lattice, nx=w.nx, ny=w.ny, nz=w.nz, pbc=w.pbc, mu_s=w.mu_s, lam=w.lam,
@@ -202,11 +215,7 @@ def run_ours(args):
     clocks = sampler.stop() if rank == 0 else None
     launches = ctx.launch_count() - l0
     heun_ms = sum(a.elapsed_time(b) for a, b in heun_events)
-    if dist is not None:
-        tt = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms = float(tt.item())
-    updates = float(args.steps) * hps * N * world
+    ms, updates = reduce_over_ranks(ms, float(args.steps) * hps * N, dist, dev)
     value = updates / (ms * 1e-3)
 
     # ---- e2e: the same steps through the C ABI with HOST buffers: H2D of the step's inputs, D2H of its result ----
@@ -229,11 +238,8 @@ def run_ours(args):
     barrier()
     e2e_ms = e0.elapsed_time(e1)
     wall_ms = (time.perf_counter() - w0) * 1e3
-    if dist is not None:
-        tt = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e_ms = float(tt.item())
-    e2e_value = float(e2e_steps) * hps * N * world / (e2e_ms * 1e-3)
+    e2e_ms, e2e_updates = reduce_over_ranks(e2e_ms, float(e2e_steps) * hps * N, dist, dev)
+    e2e_value = e2e_updates / (e2e_ms * 1e-3)
 
     if rank != 0:
         if dist is not None:
