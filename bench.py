@@ -175,6 +175,8 @@ def run_ours(args):
     N = w.n_sites
     ctx = asd.Context(_gpu_desc(asd, w), device=f"cuda:{local}")
     dev = ctx.device
+    if args.kernel != "auto":
+        ctx.set_kernel({"general": asd.KERNEL_GENERAL, "fast": asd.KERNEL_FAST, "tma": asd.KERNEL_TMA}[args.kernel])
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory()
     hT, hBx, hBy, hBz = pin(w.T), pin(w.Bx), pin(w.By), pin(w.Bz)
     ctx.set_spins_host(pin(w.sx), pin(w.sy), pin(w.sz))
@@ -346,6 +348,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=20)
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "general", "fast", "tma"],
+                    help="stage-kernel variant (asd_set_kernel); auto = the library's choice")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

@@ -65,7 +65,7 @@ typedef enum {
 enum { ASD_SC = 0, ASD_L10_FE = 1 };
 
 /* Kernel variant for asd_step_heun.  AUTO picks the fastest supported. */
-enum { ASD_KERNEL_AUTO = 0, ASD_KERNEL_GENERAL = 1, ASD_KERNEL_FAST = 2 };
+enum { ASD_KERNEL_AUTO = 0, ASD_KERNEL_GENERAL = 1, ASD_KERNEL_FAST = 2, ASD_KERNEL_TMA = 3 };
 
 /* Lattice description (S:8(b)).  Plain data; HOST pointers are read during asd_create_lattice only. */
 typedef struct {

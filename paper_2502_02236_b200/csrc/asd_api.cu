@@ -220,6 +220,7 @@ asd_status asd_create_lattice(const asd_lattice_desc* desc, void* d_workspace, s
 asd_status asd_destroy(asd_ctx* ctx) {
   if (!ctx) return ASD_EINVAL;
   if (ctx->c.host_scratch) cudaFreeHost(ctx->c.host_scratch);
+  asd::tma_plan_free(ctx->c);
   delete ctx;
   return ASD_OK;
 }
@@ -321,8 +322,11 @@ asd_status asd_step_heun(asd_ctx* ctx, int64_t n) {
 
 asd_status asd_set_kernel(asd_ctx* ctx, int32_t variant) {
   CTX_OR_RETURN(ctx);
-  if (variant != ASD_KERNEL_AUTO && variant != ASD_KERNEL_GENERAL && variant != ASD_KERNEL_FAST)
+  if (variant != ASD_KERNEL_AUTO && variant != ASD_KERNEL_GENERAL && variant != ASD_KERNEL_FAST &&
+      variant != ASD_KERNEL_TMA)
     return fail(c, ASD_EINVAL, "asd_set_kernel: unknown variant");
+  if (variant == ASD_KERNEL_TMA && (!heun_tma_supported(c) || !tma_plan(c)))
+    return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: the staged film kernel needs what the film kernel needs and a strip plan that fits in shared memory");
   if (variant == ASD_KERNEL_FAST && !heun_fast_supported(c))
     return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: the film kernel needs open boundaries, ny % 4 == 0, built-in shells and grains that do not touch");
   c.kernel_variant = variant;

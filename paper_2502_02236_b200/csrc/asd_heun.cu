@@ -263,11 +263,14 @@ asd_status launch_heun(Ctx& c, int64_t n) {
   const bool vec4 = (c.d.ny % 4 == 0);
   const bool fast = c.kernel_variant != ASD_KERNEL_GENERAL && heun_fast_supported(c);
   if (c.kernel_variant == ASD_KERNEL_FAST && !fast) return ASD_EUNSUPPORTED;
+  const bool staged = c.kernel_variant == ASD_KERNEL_TMA;
+  if (staged && !(heun_tma_supported(c) && tma_plan(c))) return ASD_EUNSUPPORTED;
   for (int64_t s = 0; s < n; ++s) {
     p.n_lo = (uint32_t)((uint64_t)c.step & 0xFFFFFFFFull);
     p.n_hi = (uint32_t)((uint64_t)c.step >> 32);
     asd_status st;
-    if (fast) st = launch_heun_fast(c, p);
+    if (staged) st = launch_heun_tma(c, p);
+    else if (fast) st = launch_heun_fast(c, p);
     else if (c.d.ell_width > 0) st = launch_pair<1, LAT_ELL>(c, p);
     else if (c.d.lattice == ASD_SC) st = vec4 ? launch_pair<4, LAT_SC>(c, p) : launch_pair<1, LAT_SC>(c, p);
     else st = vec4 ? launch_pair<4, LAT_L10>(c, p) : launch_pair<1, LAT_L10>(c, p);

@@ -69,6 +69,8 @@ struct StageParams {
   PhiloxKey key;
 };
 
+struct TmaPlan;             // asd_heun_tma.cu: tensor maps + strip / chunk plan of the staged film kernel
+
 struct Ctx {
   asd_lattice_desc d;          // host pointers inside are NOT valid after create
   cudaStream_t stream = nullptr;
@@ -106,6 +108,8 @@ struct Ctx {
   float scale = 1.0f;
   int64_t step = 0, shift = 0, pass = 0, x0 = 0;
   int32_t kernel_variant = ASD_KERNEL_AUTO;
+  TmaPlan* tma_plan = nullptr;      // built lazily by the first staged launch (host memory, freed by asd_destroy)
+  bool tma_plan_tried = false;
   int64_t launches = 0;
   bool cuda_failed = false;
   char err[256] = {0};
@@ -143,6 +147,10 @@ asd_status launch_sigma(Ctx& c, const float* T_dense);
 asd_status launch_heun(Ctx& c, int64_t n);
 asd_status launch_heun_fast(Ctx& c, StageParams& p);          // one Heun step (2 kernels), fast path
 bool heun_fast_supported(const Ctx& c);
+asd_status launch_heun_tma(Ctx& c, StageParams& p);           // one Heun step (2 kernels), TMA-staged film path
+bool heun_tma_supported(const Ctx& c);
+TmaPlan* tma_plan(Ctx& c);                                    // nullptr if the plan cannot be built
+void tma_plan_free(Ctx& c);
 void fill_stage_params(const Ctx& c, StageParams& p);
 asd_status launch_shift(Ctx& c, int32_t p);
 asd_status launch_cell_frames(Ctx& c);

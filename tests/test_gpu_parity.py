@@ -77,9 +77,11 @@ def test_adjacent_grains_and_periodic_boundaries(lattice, pbc, dims):
     sx, sy, sz = ai.tilted_spins(w.n_sites, 30.0, seed=9)
     mag = w.magnetic_mask().reshape(-1)
     w.sx, w.sy, w.sz = sx * mag, sy * mag, sz * mag
-    o, g = oracle_from_workload(w), gpu_from_workload(w)
-    o.step_heun(2); g.step_heun(2)
-    assert max_abs_diff(g, o) <= 2e-5
+    import paper_2502_02236_b200 as asd
+    o, g = _full_size_oracle(cfg, w), gpu_from_workload(w)
+    g.set_kernel({"fast": asd.KERNEL_FAST, "tma": asd.KERNEL_TMA}[kernel])
+    g.step_heun(2)
+    assert float(np.abs(g.get_spins_host().astype(np.float64) - o).max()) <= 2e-5
     _check_norm(g, w)
 
 
@@ -129,14 +131,46 @@ def test_counters_resume_bit_exact():
     assert np.array_equal(b.get_spins_host(), ref)
 
 
+_FULL = {}
+
+
+def _full_size_oracle(cfg, w):
+    """Oracle spins after 2 Heun steps of a full-size config (computed once per session, shared by the variants)."""
+    if cfg not in _FULL:
+        o = oracle_from_workload(w)
+        o.step_heun(2)
+        _FULL[cfg] = o.get_spins()
+    return _FULL[cfg]
+
+
+@pytest.mark.parametrize("lattice", [ai.SC, ai.L10])
+@pytest.mark.parametrize("dims", [(21, 40, 7), (9, 4, 3), (3, 8, 3), (1, 8, 1), (40, 132, 9), (70, 220, 27), (300, 24, 2)])
+def test_staged_tma_kernel(lattice, dims):
+    """The TMA-staged film kernel (asd_heun_tma.cu): several strips, chunks of 1..many planes, ragged last strip and
+    chunk, against the oracle and bit-for-bit against nothing else (its own arithmetic order)."""
+    import paper_2502_02236_b200 as asd
+    nx, ny, nz = dims
+    w = ai.small_film(lattice, nx, ny, nz, tilt_deg=25.0, dt=1e-16)
+    o, g = oracle_from_workload(w), gpu_from_workload(w)
+    g.set_kernel(asd.KERNEL_TMA)
+    o.step_heun(1); g.step_heun(1)
+    assert max_abs_diff(g, o) <= TOL_1STEP
+    o.step_heun(3); g.step_heun(3)
+    assert max_abs_diff(g, o) <= 5e-5
+    _check_norm(g, w)
+
+
 @pytest.mark.parametrize("cfg", [2, 4])
-def test_full_size_one_step(cfg):
+@pytest.mark.parametrize("kernel", ["fast", "tma"])
+def test_full_size_one_step(cfg, kernel):
     """BASELINE configs at full size in the launch configuration bench.py times: every site against the oracle."""
     w = ai.make_config(cfg)
     sx, sy, sz = ai.tilted_spins(w.n_sites, 20.0, seed=4)
     mag = w.magnetic_mask().reshape(-1)
     w.sx, w.sy, w.sz = sx * mag, sy * mag, sz * mag
-    o, g = oracle_from_workload(w), gpu_from_workload(w)
-    o.step_heun(2); g.step_heun(2)
-    assert max_abs_diff(g, o) <= 2e-5
+    import paper_2502_02236_b200 as asd
+    o, g = _full_size_oracle(cfg, w), gpu_from_workload(w)
+    g.set_kernel({"fast": asd.KERNEL_FAST, "tma": asd.KERNEL_TMA}[kernel])
+    g.step_heun(2)
+    assert float(np.abs(g.get_spins_host().astype(np.float64) - o).max()) <= 2e-5
     _check_norm(g, w)
