@@ -17,10 +17,10 @@ struct SiteConst {
 
 // q -> q/|q| (0 stays 0: vacant sites and padding hold exact zeros and must keep them).
 __device__ __forceinline__ void normalise3(float q0, float q1, float q2, float out[3]) {
-  const float n2 = fmaf(q0, q0, fmaf(q1, q1, q2 * q2));
+  // the floor keeps 1/|q| finite for q = 0 (0 * finite = 0); a real spin has |q| ~ 1
+  const float n2 = fmaxf(fmaf(q0, q0, fmaf(q1, q1, q2 * q2)), 1e-30f);
   float inv = mufu_rsqrt(n2);
   inv = inv * fmaf(-0.5f * n2, inv * inv, 1.5f);                  // one Newton step: |S| = 1 to ~1 ulp
-  inv = (n2 > 0.0f) ? inv : 0.0f;
   out[0] = q0 * inv; out[1] = q1 * inv; out[2] = q2 * inv;
 }
 

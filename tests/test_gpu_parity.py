@@ -77,11 +77,9 @@ def test_adjacent_grains_and_periodic_boundaries(lattice, pbc, dims):
     sx, sy, sz = ai.tilted_spins(w.n_sites, 30.0, seed=9)
     mag = w.magnetic_mask().reshape(-1)
     w.sx, w.sy, w.sz = sx * mag, sy * mag, sz * mag
-    import paper_2502_02236_b200 as asd
-    o, g = _full_size_oracle(cfg, w), gpu_from_workload(w)
-    g.set_kernel({"fast": asd.KERNEL_FAST, "tma": asd.KERNEL_TMA}[kernel])
-    g.step_heun(2)
-    assert float(np.abs(g.get_spins_host().astype(np.float64) - o).max()) <= 2e-5
+    o, g = oracle_from_workload(w), gpu_from_workload(w)
+    o.step_heun(2); g.step_heun(2)
+    assert max_abs_diff(g, o) <= 2e-5
     _check_norm(g, w)
 
 
