@@ -31,7 +31,7 @@ struct FastParams {
   const float* aniso;              // window origin; components at aniso_stride
   uint32_t aniso_stride;
   uint32_t nthreads, ngrp, nz, nx, ny, nyp, planep, lead;
-  uint32_t pf_elems;               // elements of one array spanned by the 1024 sites of one CTA (prefetch size)
+  uint32_t pf_elems;               // elements of one array spanned by the sites of one CTA (prefetch size)
   uint32_t m_grp, s_grp, m_nz, s_nz;   // magic numbers: t / ngrp and r / nz
   float j1, j2, j3;
   float gdt, lambda, scale;
@@ -53,18 +53,20 @@ __device__ __forceinline__ void st4(float* base, uint32_t e, const float v[4]) {
   *reinterpret_cast<float4*>(base + e) = make_float4(v[0], v[1], v[2], v[3]);
 }
 
-// Distance, in CTAs, of the L2 prefetch (see the kernel): a third of a wave of 148 SMs x 3 CTAs.  Measured on cfg4:
+// Distance, in units of 256 threads, of the L2 prefetch (see the kernel): a third of a wave of 148 SMs x 768 threads.  Measured on cfg4:
 // 64 .. 222 are equivalent (-6 % per stage), 444 gains nothing, 888 and more evict the lines before they are used.
 constexpr uint32_t kPrefetchAhead = 148;
 
-template <int LAT, int STAGE>
-__global__ void __launch_bounds__(256, 3) heun_stage_fast(const FastParams p) {
+// CTA shape: 128 threads x 5 CTAs per SM (96 registers per thread).  Measured on cfg4: 57.9 us per stage, against
+// 59.9 (256 x 3, 80 registers), 58.3 (128 x 4), 58.8 (128 x 6), 60.8 (256 x 2), 69.5 (512 x 1).
+template <int LAT, int STAGE, int NT = 128, int MINB = 5>
+__global__ void __launch_bounds__(NT, MINB) heun_stage_fast(const FastParams p) {
   // ---- L2 prefetch: one bulk-prefetch instruction per streamed array brings the sites of the CTA that will run
   // kPrefetchAhead blocks later from HBM into L2.  It holds no registers and nobody waits for it; when that CTA's
   // loads are issued they find their lines in L2 instead of paying the DRAM latency.
   {
     constexpr uint32_t kArr = (STAGE == 0) ? 7u : 10u;           // X(3), sigma, B(3) [, A(3)]
-    const uint32_t tb = (blockIdx.x + kPrefetchAhead) * 256u;
+    const uint32_t tb = (blockIdx.x + kPrefetchAhead * 256u / NT) * NT;
     if (threadIdx.x < kArr && tb < p.nthreads) {
       const uint32_t rb = fastdiv(tb, p.m_grp, p.s_grp);
       const uint32_t eb = p.lead + rb * p.nyp + (tb - rb * p.ngrp) * 4u;     // multiple of 4 elements: 16-byte aligned
@@ -77,7 +79,7 @@ __global__ void __launch_bounds__(256, 3) heun_stage_fast(const FastParams p) {
         asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p.arrays + (off + eb)), "r"(bytes) : "memory");
     }
   }
-  const uint32_t t = blockIdx.x * 256u + threadIdx.x;
+  const uint32_t t = blockIdx.x * NT + threadIdx.x;
   if (t >= p.nthreads) return;
   const uint32_t r = fastdiv(t, p.m_grp, p.s_grp);
   const uint32_t j0 = (t - r * p.ngrp) * 4u;
@@ -184,15 +186,16 @@ void magic(uint32_t d, uint32_t& m, uint32_t& s) {
   s = L - 1;
 }
 
-template <int LAT>
+template <int LAT, int NT = 128, int MINB = 5>
 asd_status launch_pair_fast(Ctx& c, FastParams& f) {
-  const unsigned blocks = (f.nthreads + 255u) / 256u;
+  const unsigned blocks = (f.nthreads + NT - 1u) / NT;
+  f.pf_elems = ((uint32_t)NT * 4u / f.ny + 2u) * f.nyp;
   const uint32_t as = f.as;
   f.oX = (uint32_t)c.aS * as; f.oOut = (uint32_t)c.aSt * as; f.oOutA = AR_A * as; f.oA = AR_A * as;
-  heun_stage_fast<LAT, 0><<<blocks, 256, 0, c.stream>>>(f);
+  heun_stage_fast<LAT, 0, NT, MINB><<<blocks, NT, 0, c.stream>>>(f);
   ASD_LAUNCH_CHECK(c, "heun predictor (fast)");
   f.oX = (uint32_t)c.aSt * as; f.oOut = (uint32_t)c.aS * as;
-  heun_stage_fast<LAT, 1><<<blocks, 256, 0, c.stream>>>(f);
+  heun_stage_fast<LAT, 1, NT, MINB><<<blocks, NT, 0, c.stream>>>(f);
   ASD_LAUNCH_CHECK(c, "heun corrector (fast)");
   return ASD_OK;
 }
@@ -213,7 +216,6 @@ asd_status launch_heun_fast(Ctx& c, StageParams& p) {
   f.ngrp = (uint32_t)(c.d.ny / 4); f.nthreads = (uint32_t)c.nrows * f.ngrp;
   f.nz = (uint32_t)c.d.nz; f.nx = (uint32_t)c.d.nx; f.ny = (uint32_t)c.d.ny; f.nyp = (uint32_t)c.nyp; f.lead = (uint32_t)c.lead;
   f.planep = (uint32_t)c.d.nz * (uint32_t)c.nyp;
-  f.pf_elems = (1024u / f.ny + 2u) * f.nyp;
   magic(f.ngrp, f.m_grp, f.s_grp);
   magic(f.nz, f.m_nz, f.s_nz);
   f.j1 = p.jx[0]; f.j2 = p.jx[1]; f.j3 = p.jx[2];
