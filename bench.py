@@ -262,7 +262,7 @@ def run_ours(args):
         "clocks": clocks, "gpu_launches": int(launches),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 16 * N, "d2h_bytes_per_step": 32,
                 "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps, "wall_ms_per_step": wall_ms / e2e_steps},
-        "roofline": {"bound": "hbm", "kernel": "heun_stage_direct (predictor+corrector, 52 B/site each)",
+        "roofline": {"bound": "hbm", "kernel": "heun_stage_fast (predictor+corrector, 52 B/site each)",
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "peak_source": peak_src, "avg_launch_us": avg_launch_s * 1e6,
                      "algorithmic_bytes_per_launch": alg_bytes, "traffic": _traffic(w.name)},
