@@ -67,6 +67,9 @@ enum { ASD_SC = 0, ASD_L10_FE = 1 };
 /* Kernel variant for asd_step_heun.  AUTO picks the fastest supported. */
 enum { ASD_KERNEL_AUTO = 0, ASD_KERNEL_GENERAL = 1, ASD_KERNEL_FAST = 2, ASD_KERNEL_TMA = 3 };
 
+/* CUDA-graph replay of asd_step_heun batches (launch-bound lattices).  AUTO: on for windows of <= 2^18 sites. */
+enum { ASD_GRAPH_AUTO = 0, ASD_GRAPH_OFF = 1, ASD_GRAPH_ON = 2 };
+
 /* Lattice description (S:8(b)).  Plain data; HOST pointers are read during asd_create_lattice only. */
 typedef struct {
   int32_t lattice;      /* ASD_SC: simple cubic, 6 nearest neighbours, J[0]
@@ -131,6 +134,8 @@ ASD_API asd_status asd_set_field_scale(asd_ctx *ctx, float s);
 ASD_API asd_status asd_step_heun(asd_ctx *ctx, int64_t n);
 /* Selects the kernel variant (ASD_KERNEL_*); ASD_EUNSUPPORTED if the lattice cannot use it. */
 ASD_API asd_status asd_set_kernel(asd_ctx *ctx, int32_t variant);
+/* Selects whether asd_step_heun(n >= 2) replays recorded CUDA graphs (ASD_GRAPH_*).  Results do not depend on it. */
+ASD_API asd_status asd_set_graph_mode(asd_ctx *ctx, int32_t mode);
 
 /* Window moves +x by p planes, 1 <= p <= nx (S:O5): outgoing planes -> macrocell sums and counts (Eq. 6);
  * spins move by p planes; incoming planes seeded by cone sampling (D:S3); x0 += p; shift counter += 1.

@@ -14,12 +14,13 @@ import numpy as np
 
 ASD_SC, ASD_L10_FE = 0, 1
 KERNEL_AUTO, KERNEL_GENERAL, KERNEL_FAST, KERNEL_TMA = 0, 1, 2, 3
+GRAPH_AUTO, GRAPH_OFF, GRAPH_ON = 0, 1, 2
 _STATUS = {0: "ASD_OK", 1: "ASD_EINVAL", 2: "ASD_ENOMEM", 3: "ASD_ECUDA", 4: "ASD_ESTATE", 5: "ASD_EUNSUPPORTED"}
 
 EXPORTED_SYMBOLS = [
     "asd_workspace_bytes", "asd_create_lattice", "asd_destroy", "asd_set_spins", "asd_get_spins",
     "asd_set_spins_host", "asd_get_spins_host", "asd_set_fields", "asd_set_fields_host", "asd_set_field_scale",
-    "asd_step_heun", "asd_set_kernel", "asd_shift_window", "asd_magnetisation", "asd_grain_magnetisation",
+    "asd_step_heun", "asd_set_kernel", "asd_set_graph_mode", "asd_shift_window", "asd_magnetisation", "asd_grain_magnetisation",
     "asd_track_dims", "asd_track_set_init", "asd_track_get", "asd_get_counters", "asd_set_counters",
     "asd_launch_count", "asd_last_error", "asd_version",
 ]
@@ -85,6 +86,7 @@ def load_library(build_if_missing: bool = True):
     L.asd_set_field_scale.argtypes = [C.c_void_p, C.c_float]
     L.asd_step_heun.argtypes = [C.c_void_p, C.c_int64]
     L.asd_set_kernel.argtypes = [C.c_void_p, C.c_int32]
+    L.asd_set_graph_mode.argtypes = [C.c_void_p, C.c_int32]
     L.asd_shift_window.argtypes = [C.c_void_p, C.c_int32]
     L.asd_magnetisation.argtypes = [C.c_void_p, dp, dp]
     L.asd_grain_magnetisation.argtypes = [C.c_void_p, dp]
@@ -268,6 +270,9 @@ class Context:
 
     def set_kernel(self, variant: int):
         self._ck(self._L.asd_set_kernel(self._h, C.c_int32(variant)))
+
+    def set_graph_mode(self, mode: int):
+        self._ck(self._L.asd_set_graph_mode(self._h, C.c_int32(mode)))
 
     def shift_window(self, p: int):
         self._ck(self._L.asd_shift_window(self._h, C.c_int32(p)))

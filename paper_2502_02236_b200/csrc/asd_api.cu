@@ -70,7 +70,7 @@ bool compute_layout(const asd_lattice_desc& d, Layout& L) {
   L.gmap = take(sizeof(int32_t) * ncol);
   L.grain = take(sizeof(float4) * ((size_t)d.n_grains + 1));
   L.aniso = take(sizeof(float) * 4 * ncol + 64);
-  L.flags = take(sizeof(int32_t) * 4);
+  L.flags = take(sizeof(int32_t) * 16);
   const size_t ell = (size_t)d.ell_width * (size_t)L.N;
   L.ell_idx = take(sizeof(int32_t) * ell * 2);   // slot-major table + staging for the site-major upload
   L.ell_J = take(sizeof(float) * ell * 2);
@@ -132,6 +132,7 @@ asd_status asd_create_lattice(const asd_lattice_desc* desc, void* d_workspace, s
   Ctx& c = h->c;
   c.d = *desc;
   c.stream = (cudaStream_t)cuda_stream;
+  c.launch_stream = c.stream;
   c.device = dev;
   cudaDeviceGetAttribute(&c.sm_count, cudaDevAttrMultiProcessorCount, dev);
   c.N = L.N; c.nyp = L.nyp; c.lead = L.lead; c.nrows = L.nrows; c.Np = L.Np; c.as = L.as;
@@ -221,6 +222,7 @@ asd_status asd_destroy(asd_ctx* ctx) {
   if (!ctx) return ASD_EINVAL;
   if (ctx->c.host_scratch) cudaFreeHost(ctx->c.host_scratch);
   asd::tma_plan_free(ctx->c);
+  asd::graphs_free(ctx->c);
   delete ctx;
   return ASD_OK;
 }
@@ -330,6 +332,15 @@ asd_status asd_set_kernel(asd_ctx* ctx, int32_t variant) {
   if (variant == ASD_KERNEL_FAST && !heun_fast_supported(c))
     return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: the film kernel needs open boundaries, ny % 4 == 0, built-in shells and grains that do not touch");
   c.kernel_variant = variant;
+  graphs_invalidate(c);
+  return ASD_OK;
+}
+
+asd_status asd_set_graph_mode(asd_ctx* ctx, int32_t mode) {
+  CTX_OR_RETURN(ctx);
+  if (mode != ASD_GRAPH_AUTO && mode != ASD_GRAPH_OFF && mode != ASD_GRAPH_ON)
+    return fail(c, ASD_EINVAL, "asd_set_graph_mode: unknown mode");
+  c.graph_mode = mode;
   return ASD_OK;
 }
 
@@ -339,6 +350,7 @@ asd_status asd_shift_window(asd_ctx* ctx, int32_t p) {
   if (c.d.ell_width > 0) return fail(c, ASD_EUNSUPPORTED, "asd_shift_window: a general ELL table cannot follow the window");
   if (c.d.pbc[0]) return fail(c, ASD_EUNSUPPORTED, "asd_shift_window: window is periodic in x");
   if (c.x0 + p + c.d.nx > c.d.track_nx) return fail(c, ASD_ESTATE, "asd_shift_window: past the end of the track");
+  graphs_invalidate(c);                        // window origin and buffer roles are frozen in recorded graphs
   return launch_shift(c, p);
 }
 

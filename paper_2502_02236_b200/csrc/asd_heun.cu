@@ -184,7 +184,9 @@ __global__ void __launch_bounds__(256) heun_stage_general(const StageParams p) {
       for (int c = 0; c < 3; ++c) VecIO<VEC>::ld(p.arrays + (size_t)(p.aA + c) * p.as + e0, Ain[c]);
     }
     const uint64_t g = p.g0 + (uint64_t)r * (uint64_t)p.ny + (uint64_t)j0;
-    const SiteConst sc{p.gdt, p.lambda, p.scale};
+    uint32_t n_lo = p.n_lo, n_hi = p.n_hi; float scale = p.scale;
+    resolve_dyn(p.dyn, n_lo, n_hi, scale);
+    const SiteConst sc{p.gdt, p.lambda, scale};
 #pragma unroll
     for (int v = 0; v < VEC; ++v) {
       const uint32_t gid = col[v] & 0xFFFFu;
@@ -194,7 +196,7 @@ __global__ void __launch_bounds__(256) heun_stage_general(const StageParams p) {
         continue;
       }
       uint32_t rnd[4];
-      philox_site(p.key, p.n_lo, p.n_hi, g + v, 0u, rnd);
+      philox_site(p.key, n_lo, n_hi, g + v, 0u, rnd);
       float xi[3];
       normals3(rnd, xi);
       const float4 gp = __ldg(p.grain + gid);
@@ -224,11 +226,11 @@ asd_status launch_pair(Ctx& c, StageParams& p) {
   const unsigned blocks = (p.nthreads + threads - 1) / threads;
   // predictor: X = S -> out = S~, outA = A
   p.aX = c.aS; p.aOut = c.aSt; p.aOutA = AR_A; p.aA = AR_A;
-  heun_stage_general<VEC, LAT, 0><<<blocks, threads, 0, c.stream>>>(p);
+  heun_stage_general<VEC, LAT, 0><<<blocks, threads, 0, c.launch_stream>>>(p);
   ASD_LAUNCH_CHECK(c, "heun predictor");
   // corrector: X = S~, A -> out = S
   p.aX = c.aSt; p.aOut = c.aS;
-  heun_stage_general<VEC, LAT, 1><<<blocks, threads, 0, c.stream>>>(p);
+  heun_stage_general<VEC, LAT, 1><<<blocks, threads, 0, c.launch_stream>>>(p);
   ASD_LAUNCH_CHECK(c, "heun corrector");
   return ASD_OK;
 }
@@ -257,17 +259,22 @@ void fill_stage_params(const Ctx& c, StageParams& p) {
   }
 }
 
-asd_status launch_heun(Ctx& c, int64_t n) {
+// n Heun steps as 2n plain launches on c.launch_stream.  dyn == nullptr: step indices come from c.step, which advances.
+// dyn != nullptr (graph capture): step s of the batch carries the offset s and reads the base from *dyn; c.step is
+// left to the caller.
+asd_status launch_heun_direct(Ctx& c, int64_t n, const DynState* dyn) {
   StageParams p;
   fill_stage_params(c, p);
+  p.dyn = dyn;
   const bool vec4 = (c.d.ny % 4 == 0);
   const bool fast = c.kernel_variant != ASD_KERNEL_GENERAL && heun_fast_supported(c);
   if (c.kernel_variant == ASD_KERNEL_FAST && !fast) return ASD_EUNSUPPORTED;
   const bool staged = c.kernel_variant == ASD_KERNEL_TMA;
   if (staged && !(heun_tma_supported(c) && tma_plan(c))) return ASD_EUNSUPPORTED;
   for (int64_t s = 0; s < n; ++s) {
-    p.n_lo = (uint32_t)((uint64_t)c.step & 0xFFFFFFFFull);
-    p.n_hi = (uint32_t)((uint64_t)c.step >> 32);
+    const uint64_t idx = dyn ? (uint64_t)s : (uint64_t)c.step;
+    p.n_lo = (uint32_t)(idx & 0xFFFFFFFFull);
+    p.n_hi = (uint32_t)(idx >> 32);
     asd_status st;
     if (staged) st = launch_heun_tma(c, p);
     else if (fast) st = launch_heun_fast(c, p);
@@ -275,7 +282,7 @@ asd_status launch_heun(Ctx& c, int64_t n) {
     else if (c.d.lattice == ASD_SC) st = vec4 ? launch_pair<4, LAT_SC>(c, p) : launch_pair<1, LAT_SC>(c, p);
     else st = vec4 ? launch_pair<4, LAT_L10>(c, p) : launch_pair<1, LAT_L10>(c, p);
     if (st != ASD_OK) return st;
-    c.step += 1;
+    if (!dyn) c.step += 1;
   }
   return ASD_OK;
 }

@@ -36,6 +36,7 @@ struct FastParams {
   float j1, j2, j3;
   float gdt, lambda, scale;
   uint32_t n_lo, n_hi;
+  const DynState* dyn;
   uint64_t g0;
   PhiloxKey key;
 };
@@ -153,12 +154,14 @@ __global__ void __launch_bounds__(NT, MINB) heun_stage_fast(const FastParams p) 
 
   // ---- noise, torque, update, renormalise ----
   const uint64_t g = p.g0 + (uint64_t)(r * p.ny + j0);           // global site id of the first own site
-  const SiteConst sc{p.gdt, p.lambda, p.scale};
+  uint32_t n_lo = p.n_lo, n_hi = p.n_hi; float scale = p.scale;
+  resolve_dyn(p.dyn, n_lo, n_hi, scale);
+  const SiteConst sc{p.gdt, p.lambda, scale};
   float o[3][4], oA[3][4];
 #pragma unroll
   for (int v = 0; v < 4; ++v) {
     uint32_t rnd[4];
-    philox_site(p.key, p.n_lo, p.n_hi, g + (uint64_t)v, 0u, rnd);
+    philox_site(p.key, n_lo, n_hi, g + (uint64_t)v, 0u, rnd);
     float xi[3];
     normals3(rnd, xi);
     const float Xs[3] = {own[0][v + 1], own[1][v + 1], own[2][v + 1]};
@@ -192,10 +195,10 @@ asd_status launch_pair_fast(Ctx& c, FastParams& f) {
   f.pf_elems = ((uint32_t)NT * 4u / f.ny + 2u) * f.nyp;
   const uint32_t as = f.as;
   f.oX = (uint32_t)c.aS * as; f.oOut = (uint32_t)c.aSt * as; f.oOutA = AR_A * as; f.oA = AR_A * as;
-  heun_stage_fast<LAT, 0, NT, MINB><<<blocks, NT, 0, c.stream>>>(f);
+  heun_stage_fast<LAT, 0, NT, MINB><<<blocks, NT, 0, c.launch_stream>>>(f);
   ASD_LAUNCH_CHECK(c, "heun predictor (fast)");
   f.oX = (uint32_t)c.aSt * as; f.oOut = (uint32_t)c.aS * as;
-  heun_stage_fast<LAT, 1, NT, MINB><<<blocks, NT, 0, c.stream>>>(f);
+  heun_stage_fast<LAT, 1, NT, MINB><<<blocks, NT, 0, c.launch_stream>>>(f);
   ASD_LAUNCH_CHECK(c, "heun corrector (fast)");
   return ASD_OK;
 }
@@ -220,7 +223,7 @@ asd_status launch_heun_fast(Ctx& c, StageParams& p) {
   magic(f.nz, f.m_nz, f.s_nz);
   f.j1 = p.jx[0]; f.j2 = p.jx[1]; f.j3 = p.jx[2];
   f.gdt = p.gdt; f.lambda = p.lambda; f.scale = p.scale;
-  f.n_lo = p.n_lo; f.n_hi = p.n_hi; f.g0 = p.g0; f.key = p.key;
+  f.n_lo = p.n_lo; f.n_hi = p.n_hi; f.dyn = p.dyn; f.g0 = p.g0; f.key = p.key;
   return c.d.lattice == ASD_SC ? launch_pair_fast<LAT_SC>(c, f) : launch_pair_fast<LAT_L10>(c, f);
 }
 

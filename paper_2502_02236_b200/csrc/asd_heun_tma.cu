@@ -46,6 +46,7 @@ struct TmaParams {
   float j1, j2, j3;
   float gdt, lambda, scale;
   uint32_t n_lo, n_hi;
+  const DynState* dyn;
   uint64_t g0;
   PhiloxKey key;
 };
@@ -175,7 +176,9 @@ heun_stage_tma(const __grid_constant__ CUtensorMap mapMain, const __grid_constan
   const uint32_t planep = (uint32_t)(p.nz * p.nyp);
   uint64_t gsite = p.g0 + (uint64_t)((uint32_t)(i_begin * p.nz + k) * (uint32_t)p.ny + (uint32_t)j);
   const uint32_t gplane = (uint32_t)(p.nz * p.ny);
-  const SiteConst sc{p.gdt, p.lambda, p.scale};
+  uint32_t n_lo = p.n_lo, n_hi = p.n_hi; float scale = p.scale;
+  resolve_dyn(p.dyn, n_lo, n_hi, scale);
+  const SiteConst sc{p.gdt, p.lambda, scale};
 
   mbar_wait(bar_full + 0u, 0u);
   mbar_wait(bar_full + 8u, 0u);
@@ -251,7 +254,7 @@ heun_stage_tma(const __grid_constant__ CUtensorMap mapMain, const __grid_constan
 #pragma unroll
       for (int v = 0; v < 4; ++v) {
         uint32_t rnd[4];
-        philox_site(p.key, p.n_lo, p.n_hi, gsite + (uint64_t)v, 0u, rnd);
+        philox_site(p.key, n_lo, n_hi, gsite + (uint64_t)v, 0u, rnd);
         float xi[3];
         normals3(rnd, xi);
         const float Xs[3] = {own[0][v + 1], own[1][v + 1], own[2][v + 1]};
@@ -463,16 +466,16 @@ asd_status launch_heun_tma(Ctx& c, StageParams& p) {
   f.main_pitch = pl->main_pitch; f.edge_pitch = pl->edge_pitch; f.an_pitch = pl->an_pitch;
   f.j1 = p.jx[0]; f.j2 = p.jx[1]; f.j3 = p.jx[2];
   f.gdt = p.gdt; f.lambda = p.lambda; f.scale = p.scale;
-  f.n_lo = p.n_lo; f.n_hi = p.n_hi; f.g0 = p.g0; f.key = p.key;
+  f.n_lo = p.n_lo; f.n_hi = p.n_hi; f.dyn = p.dyn; f.g0 = p.g0; f.key = p.key;
   const unsigned blocks = (unsigned)(pl->nstrips * pl->nchunks);
   const uint32_t as = f.as;
   // predictor: X = S -> S~, A
   f.aX = c.aS; f.oOut = (uint32_t)c.aSt * as; f.oOutA = AR_A * as; f.oA = AR_A * as;
-  pl->kern[0]<<<blocks, pl->threads, pl->smem_bytes, c.stream>>>(pl->mapMain, pl->mapEdge, pl->mapAn, f);
+  pl->kern[0]<<<blocks, pl->threads, pl->smem_bytes, c.launch_stream>>>(pl->mapMain, pl->mapEdge, pl->mapAn, f);
   ASD_LAUNCH_CHECK(c, "heun predictor (tma)");
   // corrector: X = S~, A -> S
   f.aX = c.aSt; f.oOut = (uint32_t)c.aS * as;
-  pl->kern[1]<<<blocks, pl->threads, pl->smem_bytes, c.stream>>>(pl->mapMain, pl->mapEdge, pl->mapAn, f);
+  pl->kern[1]<<<blocks, pl->threads, pl->smem_bytes, c.launch_stream>>>(pl->mapMain, pl->mapEdge, pl->mapAn, f);
   ASD_LAUNCH_CHECK(c, "heun corrector (tma)");
   return ASD_OK;
 }

@@ -41,6 +41,19 @@ enum : int { AR_S = 0, AR_ST = 3, AR_A = 6, AR_SIGMA = 9, AR_B = 10, AR_COUNT = 
 struct Vec3Ptr { float *x, *y, *z; };
 struct CVec3Ptr { const float *x, *y, *z; };
 
+// Device copy of the two values that change between replays of a captured CUDA graph: the step index and the
+// head-field scale.  A kernel launched with dyn != nullptr takes step = dyn step + its own n_lo (its offset inside
+// the graph) and the scale from here instead of from its (frozen) parameter block.
+struct DynState { uint32_t n_lo, n_hi; float scale; uint32_t pad; };
+#ifdef __CUDACC__
+__device__ __forceinline__ void resolve_dyn(const DynState* dyn, uint32_t& n_lo, uint32_t& n_hi, float& scale) {
+  if (dyn) {
+    const uint64_t n = (((uint64_t)dyn->n_hi << 32) | dyn->n_lo) + n_lo;
+    n_lo = (uint32_t)n; n_hi = (uint32_t)(n >> 32); scale = dyn->scale;
+  }
+}
+#endif
+
 // Parameters of one Heun stage (passed by value; lives in the constant bank).
 struct StageParams {
   float* arrays;               // base of the 13 padded per-site arrays
@@ -64,7 +77,8 @@ struct StageParams {
   float gdt;                   // gamma dt / (1 + lambda^2)
   float lambda;
   float scale;                 // B_app = scale * B
-  uint32_t n_lo, n_hi;         // step index before the step
+  uint32_t n_lo, n_hi;         // step index before the step (with dyn: offset of this step inside the graph)
+  const DynState* dyn;         // nullptr outside graph replays
   uint64_t g0;                 // x0 * ny * nz: global id of window site 0
   PhiloxKey key;
 };
@@ -74,6 +88,7 @@ struct TmaPlan;             // asd_heun_tma.cu: tensor maps + strip / chunk plan
 struct Ctx {
   asd_lattice_desc d;          // host pointers inside are NOT valid after create
   cudaStream_t stream = nullptr;
+  cudaStream_t launch_stream = nullptr;   // where the stage kernels go: `stream`, or the capture stream while a graph is recorded
   int device = 0;
   int sm_count = 148;
   int64_t N = 0;               // dense sites
@@ -91,7 +106,7 @@ struct Ctx {
   int32_t *grain_map_dev = nullptr; // [track_nx * ny] as given
   float4 *grain = nullptr;          // [n_grains + 1]
   float *aniso = nullptr;           // [4][track_nx * ny]
-  int32_t *flags = nullptr;         // [4] device: flags[0] = 1 if two different grains touch
+  int32_t *flags = nullptr;         // [16] device: flags[0] = 1 if two different grains touch; flags[4..7] = DynState
   int32_t *ell_idx = nullptr; float *ell_J = nullptr;
   bool grains_touch = true;
   // track store
@@ -108,6 +123,10 @@ struct Ctx {
   float scale = 1.0f;
   int64_t step = 0, shift = 0, pass = 0, x0 = 0;
   int32_t kernel_variant = ASD_KERNEL_AUTO;
+  // CUDA-graph replay of asd_step_heun(n) (asd_graph.cu)
+  int32_t graph_mode = ASD_GRAPH_AUTO;
+  cudaStream_t cap_stream = nullptr;   // internal stream the graphs are captured on (the caller's may be the legacy one)
+  struct GraphCache* graphs = nullptr;
   TmaPlan* tma_plan = nullptr;      // built lazily by the first staged launch (host memory, freed by asd_destroy)
   bool tma_plan_tried = false;
   int64_t launches = 0;
@@ -144,7 +163,11 @@ asd_status launch_pack_spins(Ctx& c, CVec3Ptr dense_src /* null members: +z */, 
 asd_status launch_unpack(Ctx& c, const float* padded, float* dense);
 asd_status launch_pack_field(Ctx& c, const float* dense, float* padded);
 asd_status launch_sigma(Ctx& c, const float* T_dense);
-asd_status launch_heun(Ctx& c, int64_t n);
+asd_status launch_heun(Ctx& c, int64_t n);                    // n Heun steps, through graphs when enabled
+asd_status launch_heun_direct(Ctx& c, int64_t n, const DynState* dyn);   // 2n plain launches on c.stream (or the capture stream)
+void graphs_invalidate(Ctx& c);                               // drop cached graphs (after a shift / a kernel change)
+void graphs_free(Ctx& c);
+DynState* dyn_state(const Ctx& c);
 asd_status launch_heun_fast(Ctx& c, StageParams& p);          // one Heun step (2 kernels), fast path
 bool heun_fast_supported(const Ctx& c);
 asd_status launch_heun_tma(Ctx& c, StageParams& p);           // one Heun step (2 kernels), TMA-staged film path
