@@ -141,6 +141,11 @@ struct Oracle {
   std::vector<int64_t> out_cnt;    // [ncell]
   std::vector<double> init_mean;   // [ncell*3]  what lies ahead of the window
   int threads = 0;
+  // demagnetising field (Eq. (6)-(7)); off unless orc_enable_demag was called
+  bool demag = false;
+  double cell_m[3] = {0, 0, 0};    // macrocell edge lengths, metres
+  int dcx = 0, dcy = 0, dcz = 0;   // macrocells that can overlap the window (x: worst alignment)
+  std::vector<double> demag_N;     // [(2dcx-1)(2dcy-1)(2dcz-1)][6]: Nxx Nyy Nzz Nxy Nxz Nyz at cell offsets
 
   int64_t site(int i, int k, int j) const { return ((int64_t)i * nz + k) * ny + j; }
   int32_t grain_of(int i, int j) const { return grain_map[(size_t)((x0 + i) * ny + j)]; }
@@ -203,10 +208,118 @@ void exchange_sum(const Oracle& o, const double* X0, const double* X1, const dou
   }
 }
 
+// ---- Demagnetising tensor of two equal cuboids (Newell, Williams and Dunlop, J. Geophys. Res. 98, 9551 (1993);
+// the paper's ref. [28]): N_ab(R) such that the cell-averaged field of a uniformly magnetised source cell at
+// offset R is H = -N M.  Written out as the 27-point second difference of the auxiliary functions f and g. ----
+double newell_f(double x, double y, double z) {
+  x = std::fabs(x); y = std::fabs(y); z = std::fabs(z);           // f is even in every argument
+  const double x2 = x * x, y2 = y * y, z2 = z * z, R = std::sqrt(x2 + y2 + z2);
+  if (R == 0.0) return 0.0;
+  double v = (2.0 * x2 - y2 - z2) * R / 6.0;
+  if (y > 0.0 && (x2 + z2) > 0.0) v += 0.5 * y * (z2 - x2) * std::asinh(y / std::sqrt(x2 + z2));
+  if (z > 0.0 && (x2 + y2) > 0.0) v += 0.5 * z * (y2 - x2) * std::asinh(z / std::sqrt(x2 + y2));
+  if (x > 0.0 && y > 0.0 && z > 0.0) v -= x * y * z * std::atan(y * z / (x * R));
+  return v;
+}
+double newell_g(double x, double y, double z) {
+  const double sgn = ((x < 0.0) != (y < 0.0)) ? -1.0 : 1.0;       // g is odd in x and in y, even in z
+  x = std::fabs(x); y = std::fabs(y); z = std::fabs(z);
+  const double x2 = x * x, y2 = y * y, z2 = z * z, R = std::sqrt(x2 + y2 + z2);
+  if (R == 0.0) return 0.0;
+  double v = -x * y * R / 3.0;
+  if (z > 0.0 && (x2 + y2) > 0.0) v += x * y * z * std::asinh(z / std::sqrt(x2 + y2));
+  if (x > 0.0 && (y2 + z2) > 0.0) v += y / 6.0 * (3.0 * z2 - y2) * std::asinh(x / std::sqrt(y2 + z2));
+  if (y > 0.0 && (x2 + z2) > 0.0) v += x / 6.0 * (3.0 * z2 - x2) * std::asinh(y / std::sqrt(x2 + z2));
+  if (z > 0.0) {
+    if (x > 0.0 && y > 0.0) v -= z * z2 / 6.0 * std::atan(x * y / (z * R));
+    if (y > 0.0 && x > 0.0) v -= 0.5 * z * y2 * std::atan(x * z / (y * R));
+    if (x > 0.0 && y > 0.0) v -= 0.5 * z * x2 * std::atan(y * z / (x * R));
+  }
+  return sgn * v;
+}
+// sum_{u,v,w in {-1,0,1}} w_u w_v w_w F(X + u dx, Y + v dy, Z + w dz), w = (1, -2, 1)
+template <class F>
+double second_difference(F fn, double X, double Y, double Z, double dx, double dy, double dz) {
+  static const double w[3] = {1.0, -2.0, 1.0};
+  double acc = 0.0;
+  for (int u = -1; u <= 1; ++u)
+    for (int v = -1; v <= 1; ++v)
+      for (int t = -1; t <= 1; ++t) acc += w[u + 1] * w[v + 1] * w[t + 1] * fn(X + u * dx, Y + v * dy, Z + t * dz);
+  return acc;
+}
+// out = (Nxx, Nyy, Nzz, Nxy, Nxz, Nyz) for cell size d and offset R.  Beyond kDemagNear cell diagonals the second
+// difference loses its digits to cancellation; there the cuboids are point dipoles to 1e-3 of an already tiny term:
+// N_ab = V/(4 pi R^3) (delta_ab - 3 R_a R_b / R^2)   (reading D2).
+constexpr double kDemagNear = 12.0;
+void newell_tensor(const double d[3], const double Rv[3], double out[6]) {
+  const double pi = 3.14159265358979323846;
+  const double X = Rv[0], Y = Rv[1], Z = Rv[2], V = d[0] * d[1] * d[2];
+  const double R2 = X * X + Y * Y + Z * Z, diag2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+  if (R2 > kDemagNear * kDemagNear * diag2) {
+    const double R = std::sqrt(R2), c = V / (4.0 * pi * R2 * R);
+    out[0] = c * (1.0 - 3.0 * X * X / R2); out[1] = c * (1.0 - 3.0 * Y * Y / R2); out[2] = c * (1.0 - 3.0 * Z * Z / R2);
+    out[3] = -3.0 * c * X * Y / R2; out[4] = -3.0 * c * X * Z / R2; out[5] = -3.0 * c * Y * Z / R2;
+    return;
+  }
+  const double k = -1.0 / (4.0 * pi * V);
+  out[0] = k * second_difference(newell_f, X, Y, Z, d[0], d[1], d[2]);
+  out[1] = k * second_difference(newell_f, Y, X, Z, d[1], d[0], d[2]);
+  out[2] = k * second_difference(newell_f, Z, Y, X, d[2], d[1], d[0]);
+  out[3] = k * second_difference(newell_g, X, Y, Z, d[0], d[1], d[2]);
+  out[4] = k * second_difference(newell_g, X, Z, Y, d[0], d[2], d[1]);
+  out[5] = k * second_difference(newell_g, Y, Z, X, d[1], d[2], d[0]);
+}
+
+// Demagnetising field of configuration X, Tesla, one 3-vector per window macrocell (S:8(f) item 1):
+//   M_c = (mu_s / V) sum_{j in c} X_j                       Eq. (6), V = full macrocell volume
+//   B_c = -mu_0 sum_c' N(r_c' - r_c) M_c'                    Eq. (7), open boundaries, the window's own cells only
+// Cells are the track macrocells (global alignment): window cell (a,b,c) is track cell (x0/mx + a, b, c).
+void demag_cells(const Oracle& o, const double* X0, const double* X1, const double* X2, std::vector<double>& Bd) {
+  const double mu0 = 4.0e-7 * 3.14159265358979323846;
+  const int mx = o.macro[0], my = o.macro[1], mz = o.macro[2];
+  const int64_t c0 = o.x0 / mx;
+  const int ncx = (int)((o.x0 + o.nx - 1) / mx - c0) + 1, ncy = o.dcy, ncz = o.dcz;
+  const double V = o.cell_m[0] * o.cell_m[1] * o.cell_m[2];
+  std::vector<double> M((size_t)ncx * ncy * ncz * 3, 0.0);
+  for (int i = 0; i < o.nx; ++i)
+    for (int k = 0; k < o.nz; ++k)
+      for (int j = 0; j < o.ny; ++j) {
+        const int64_t l = o.site(i, k, j);
+        const size_t c = ((size_t)((o.x0 + i) / mx - c0) * ncy + j / my) * ncz + k / mz;
+        M[3 * c] += X0[l]; M[3 * c + 1] += X1[l]; M[3 * c + 2] += X2[l];
+      }
+  for (double& v : M) v *= o.mu_s / V;
+  Bd.assign((size_t)o.dcx * ncy * ncz * 3, 0.0);
+  const int sy = 2 * o.dcy - 1, sz = 2 * o.dcz - 1;
+  for (int a = 0; a < ncx; ++a)
+    for (int b = 0; b < ncy; ++b)
+      for (int c = 0; c < ncz; ++c) {
+        double H[3] = {0, 0, 0};
+        for (int a2 = 0; a2 < ncx; ++a2)
+          for (int b2 = 0; b2 < ncy; ++b2)
+            for (int c2 = 0; c2 < ncz; ++c2) {
+              const size_t t = (((size_t)(a2 - a + o.dcx - 1) * sy + (b2 - b + o.dcy - 1)) * sz + (c2 - c + o.dcz - 1)) * 6;
+              const double* N = &o.demag_N[t];
+              const double* m = &M[3 * (((size_t)a2 * ncy + b2) * ncz + c2)];
+              H[0] -= N[0] * m[0] + N[3] * m[1] + N[4] * m[2];
+              H[1] -= N[3] * m[0] + N[1] * m[1] + N[5] * m[2];
+              H[2] -= N[4] * m[0] + N[5] * m[1] + N[2] * m[2];
+            }
+        const size_t q = 3 * (((size_t)a * ncy + b) * ncz + c);
+        Bd[q] = mu0 * H[0]; Bd[q + 1] = mu0 * H[1]; Bd[q + 2] = mu0 * H[2];
+      }
+}
+inline const double* demag_of_site(const Oracle& o, const std::vector<double>& Bd, int i, int k, int j) {
+  const int64_t c0 = o.x0 / o.macro[0];
+  const size_t c = ((size_t)((o.x0 + i) / o.macro[0] - c0) * o.dcy + j / o.macro[1]) * o.dcz + k / o.macro[2];
+  return &Bd[3 * c];
+}
+
 // Effective field in Tesla at a magnetic site (S:O3):
 // B_i(X) = (1/mu_s) sum_j J_ij X_j + (2 k_u,g/mu_s)(X_i.e_g) e_g + s*B_app,i + sigma_i xi_i.
 void field_at(const Oracle& o, const double* X0, const double* X1, const double* X2,
-              int i, int k, int j, const double* xi /* may be null */, double B[3]) {
+              int i, int k, int j, const double* xi /* may be null */, double B[3],
+              const double* Bd = nullptr /* demagnetising field of the site's macrocell, or null */) {
   const int64_t l = o.site(i, k, j);
   const int32_t g = o.grain_of(i, j);
   double e[3];
@@ -217,6 +330,7 @@ void field_at(const Oracle& o, const double* X0, const double* X1, const double*
   const double ca = 2.0 * o.ku[g] / o.mu_s * d;                             // Eq. (3)
   B[0] += ca * ex; B[1] += ca * ey; B[2] += ca * ez;
   B[0] += o.scale * o.Bx[l]; B[1] += o.scale * o.By[l]; B[2] += o.scale * o.Bz[l];
+  if (Bd) { B[0] += Bd[0]; B[1] += Bd[1]; B[2] += Bd[2]; }                   // Eq. (7)
   if (xi) {
     const double sg = sigma_T(o, o.T[l]);
     B[0] += sg * xi[0]; B[1] += sg * xi[1]; B[2] += sg * xi[2];
@@ -258,6 +372,8 @@ void heun_step(Oracle& o) {
   std::vector<double> tx((size_t)N, 0.0), ty((size_t)N, 0.0), tz((size_t)N, 0.0);
   const int nx = o.nx, ny = o.ny, nz = o.nz;
   const int nt = thread_count(o);
+  std::vector<double> Bd;                        // demagnetising field of the stage's configuration, per macrocell
+  if (o.demag) demag_cells(o, o.sx.data(), o.sy.data(), o.sz.data(), Bd);
 #pragma omp parallel for collapse(2) schedule(static) num_threads(nt)
   for (int i = 0; i < nx; ++i)
     for (int k = 0; k < nz; ++k)
@@ -267,7 +383,8 @@ void heun_step(Oracle& o) {
         const uint64_t g = (uint64_t)(((o.x0 + i) * nz + k) * ny + j);
         normals3(o.seed, (uint64_t)o.step, g, &xi[3 * l]);
         double B[3], f[3];
-        field_at(o, o.sx.data(), o.sy.data(), o.sz.data(), i, k, j, &xi[3 * l], B);
+        field_at(o, o.sx.data(), o.sy.data(), o.sz.data(), i, k, j, &xi[3 * l], B,
+                 o.demag ? demag_of_site(o, Bd, i, k, j) : nullptr);
         const double S[3] = {o.sx[l], o.sy[l], o.sz[l]};
         llg_rhs(o, S, B, f);
         k1[3 * l] = f[0]; k1[3 * l + 1] = f[1]; k1[3 * l + 2] = f[2];
@@ -276,6 +393,7 @@ void heun_step(Oracle& o) {
         tx[l] = p0 / nrm; ty[l] = p1 / nrm; tz[l] = p2 / nrm;
       }
   std::vector<double> n0((size_t)N, 0.0), n1((size_t)N, 0.0), n2((size_t)N, 0.0);
+  if (o.demag) demag_cells(o, tx.data(), ty.data(), tz.data(), Bd);     // B(S~) includes the demagnetising field of S~
 #pragma omp parallel for collapse(2) schedule(static) num_threads(nt)
   for (int i = 0; i < nx; ++i)
     for (int k = 0; k < nz; ++k)
@@ -283,7 +401,8 @@ void heun_step(Oracle& o) {
         if (o.grain_of(i, j) < 0) continue;
         const int64_t l = o.site(i, k, j);
         double B[3], f[3];
-        field_at(o, tx.data(), ty.data(), tz.data(), i, k, j, &xi[3 * l], B);
+        field_at(o, tx.data(), ty.data(), tz.data(), i, k, j, &xi[3 * l], B,
+                 o.demag ? demag_of_site(o, Bd, i, k, j) : nullptr);
         const double St[3] = {tx[l], ty[l], tz[l]};
         llg_rhs(o, St, B, f);
         const double q0 = o.sx[l] + 0.5 * o.dt * (k1[3 * l] + f[0]);
@@ -430,6 +549,33 @@ void orc_set_fields(void* h, const float* T, const float* Bx, const float* By, c
   }
 }
 
+// Switches the demagnetising field on: spacing = lattice constants (ax, ay, az) in metres; cell = macro * spacing.
+void orc_enable_demag(void* h, const double spacing[3]) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  for (int a = 0; a < 3; ++a) o.cell_m[a] = o.macro[a] * spacing[a];
+  o.dcx = (o.nx + o.macro[0] - 2) / o.macro[0] + 1;     // cells overlapped at the worst alignment of x0
+  o.dcy = (o.ny + o.macro[1] - 1) / o.macro[1];
+  o.dcz = (o.nz + o.macro[2] - 1) / o.macro[2];
+  const int sx = 2 * o.dcx - 1, sy = 2 * o.dcy - 1, sz = 2 * o.dcz - 1;
+  o.demag_N.assign((size_t)sx * sy * sz * 6, 0.0);
+  for (int a = 0; a < sx; ++a)
+    for (int b = 0; b < sy; ++b)
+      for (int c = 0; c < sz; ++c) {
+        const double R[3] = {(a - o.dcx + 1) * o.cell_m[0], (b - o.dcy + 1) * o.cell_m[1], (c - o.dcz + 1) * o.cell_m[2]};
+        newell_tensor(o.cell_m, R, &o.demag_N[(((size_t)a * sy + b) * sz + c) * 6]);
+      }
+  o.demag = true;
+}
+void orc_newell_tensor(const double cell[3], const double R[3], double out[6]) { newell_tensor(cell, R, out); }
+// Demagnetising field of the current spins per window macrocell, Tesla: out[dcx*dcy*dcz*3]; dims returned.
+void orc_demag_cells(void* h, double* out, int64_t dims[3]) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  std::vector<double> Bd;
+  demag_cells(o, o.sx.data(), o.sy.data(), o.sz.data(), Bd);
+  dims[0] = o.dcx; dims[1] = o.dcy; dims[2] = o.dcz;
+  if (out) for (size_t t = 0; t < Bd.size(); ++t) out[t] = Bd[t];
+}
+
 void orc_set_field_scale(void* h, float s) { static_cast<Oracle*>(h)->scale = (double)s; }
 
 void orc_step_heun(void* h, int64_t n) {
@@ -440,6 +586,8 @@ void orc_step_heun(void* h, int64_t n) {
 // Deterministic field (no noise) or field with the noise of the current step counter, Tesla.
 void orc_field(void* h, int with_noise, double* bx, double* by, double* bz) {
   Oracle& o = *static_cast<Oracle*>(h);
+  std::vector<double> Bd;
+  if (o.demag) demag_cells(o, o.sx.data(), o.sy.data(), o.sz.data(), Bd);
   for (int i = 0; i < o.nx; ++i)
     for (int k = 0; k < o.nz; ++k)
       for (int j = 0; j < o.ny; ++j) {
@@ -448,7 +596,8 @@ void orc_field(void* h, int with_noise, double* bx, double* by, double* bz) {
         if (o.grain_of(i, j) < 0) continue;
         double xi[3], B[3];
         if (with_noise) normals3(o.seed, (uint64_t)o.step, (uint64_t)(((o.x0 + i) * o.nz + k) * o.ny + j), xi);
-        field_at(o, o.sx.data(), o.sy.data(), o.sz.data(), i, k, j, with_noise ? xi : nullptr, B);
+        field_at(o, o.sx.data(), o.sy.data(), o.sz.data(), i, k, j, with_noise ? xi : nullptr, B,
+                 o.demag ? demag_of_site(o, Bd, i, k, j) : nullptr);
         bx[l] = B[0]; by[l] = B[1]; bz[l] = B[2];
       }
 }

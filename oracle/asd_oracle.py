@@ -97,6 +97,9 @@ def lib():
         L.orc_theta_max.argtypes = [C.c_double]
         L.orc_sigma.restype = C.c_double
         L.orc_sigma.argtypes = [C.c_void_p, C.c_double]
+        L.orc_enable_demag.argtypes = [C.c_void_p, dp]
+        L.orc_newell_tensor.argtypes = [dp, dp, dp]
+        L.orc_demag_cells.argtypes = [C.c_void_p, dp, ip64]
         _lib = L
     return _lib
 
@@ -139,6 +142,14 @@ def normals3_bulk(seed: int, step: int, g0: int, count: int) -> np.ndarray:
     lib().orc_normals3_bulk(C.c_uint64(seed), C.c_uint64(step), C.c_uint64(g0), C.c_int64(count),
                             _ptr(o, C.c_double))
     return o
+
+
+def newell_tensor(cell, R) -> np.ndarray:
+    """(Nxx, Nyy, Nzz, Nxy, Nxz, Nyz) of two equal cuboids `cell` (edge lengths) at centre offset R."""
+    c = np.ascontiguousarray(cell, dtype=np.float64); r = np.ascontiguousarray(R, dtype=np.float64)
+    out = np.zeros(6)
+    lib().orc_newell_tensor(_ptr(c, C.c_double), _ptr(r, C.c_double), _ptr(out, C.c_double))
+    return out
 
 
 def theta_max(m: float) -> float:
@@ -241,6 +252,19 @@ class Oracle:
         for a in arrs:
             assert a is None or a.size == self.N
         lib().orc_set_fields(self._h, *[_ptr(a, C.c_float) for a in arrs])
+
+    def enable_demag(self, spacing_m):
+        """Demagnetising field on (Eq. (6)-(7)); spacing_m = lattice constants (ax, ay, az) in metres."""
+        a = np.ascontiguousarray(spacing_m, dtype=np.float64)
+        lib().orc_enable_demag(self._h, _ptr(a, C.c_double))
+
+    def demag_cells(self) -> np.ndarray:
+        """Demagnetising field per window macrocell, Tesla: [dcx, dcy, dcz, 3]."""
+        dims = np.zeros(3, dtype=np.int64)
+        lib().orc_demag_cells(self._h, None, _ptr(dims, C.c_int64))
+        out = np.zeros((int(dims[0]), int(dims[1]), int(dims[2]), 3))
+        lib().orc_demag_cells(self._h, _ptr(out, C.c_double), _ptr(dims, C.c_int64))
+        return out
 
     def set_field_scale(self, s: float):
         lib().orc_set_field_scale(self._h, C.c_float(s))
