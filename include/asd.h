@@ -137,6 +137,19 @@ ASD_API asd_status asd_set_kernel(asd_ctx *ctx, int32_t variant);
 /* Selects whether asd_step_heun(n >= 2) replays recorded CUDA graphs (ASD_GRAPH_*).  Results do not depend on it. */
 ASD_API asd_status asd_set_graph_mode(asd_ctx *ctx, int32_t mode);
 
+/* ---- Demagnetising field of the window (Eq. (6)-(7)) ----------------------------------
+ * Once enabled, every Heun stage adds to the effective field of a site the field of its track macrocell,
+ *   B_c = -mu_0 sum_c' N(r_c' - r_c) M_c',  M_c = (mu_s / V) sum_{j in c} S_j   (V = macro[0..2] * spacing, full cell),
+ * N = demagnetising tensor of two equal cuboids (Newell et al., the paper's ref. [28]), summed over the macrocells that
+ * overlap the window (open boundaries).  Open-boundary lattices with the built-in shells; ASD_KERNEL_TMA and CUDA graphs
+ * are not used while it is on.  The caller owns the workspace (DEVICE, 256-byte aligned) for the life of the context.
+ * asd_demag_workspace_bytes needs the GPU (it sizes the cuFFT plans).  asd_demag_field computes the field of the current
+ * spins per macrocell into HOST cells[dims[0]*dims[1]*dims[2]*3] (x-cell slowest, component fastest; Tesla) and
+ * synchronises; cells == NULL returns dims only.  ASD_ESTATE if demag is not enabled. */
+ASD_API size_t asd_demag_workspace_bytes(asd_ctx *ctx);
+ASD_API asd_status asd_enable_demag(asd_ctx *ctx, const double spacing_m[3], void *d_workspace, size_t bytes);
+ASD_API asd_status asd_demag_field(asd_ctx *ctx, float *cells, int64_t dims[3]);
+
 /* Window moves +x by p planes, 1 <= p <= nx (S:O5): outgoing planes -> macrocell sums and counts (Eq. 6);
  * spins move by p planes; incoming planes seeded by cone sampling (D:S3); x0 += p; shift counter += 1.
  * ASD_ESTATE if x0 + p + nx > track_nx; ASD_EUNSUPPORTED with a general ELL table or pbc[0]. */

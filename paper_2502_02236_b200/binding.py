@@ -20,7 +20,8 @@ _STATUS = {0: "ASD_OK", 1: "ASD_EINVAL", 2: "ASD_ENOMEM", 3: "ASD_ECUDA", 4: "AS
 EXPORTED_SYMBOLS = [
     "asd_workspace_bytes", "asd_create_lattice", "asd_destroy", "asd_set_spins", "asd_get_spins",
     "asd_set_spins_host", "asd_get_spins_host", "asd_set_fields", "asd_set_fields_host", "asd_set_field_scale",
-    "asd_step_heun", "asd_set_kernel", "asd_set_graph_mode", "asd_shift_window", "asd_magnetisation", "asd_grain_magnetisation",
+    "asd_step_heun", "asd_set_kernel", "asd_set_graph_mode", "asd_demag_workspace_bytes", "asd_enable_demag",
+    "asd_demag_field", "asd_shift_window", "asd_magnetisation", "asd_grain_magnetisation",
     "asd_track_dims", "asd_track_set_init", "asd_track_get", "asd_get_counters", "asd_set_counters",
     "asd_launch_count", "asd_last_error", "asd_version",
 ]
@@ -87,6 +88,10 @@ def load_library(build_if_missing: bool = True):
     L.asd_step_heun.argtypes = [C.c_void_p, C.c_int64]
     L.asd_set_kernel.argtypes = [C.c_void_p, C.c_int32]
     L.asd_set_graph_mode.argtypes = [C.c_void_p, C.c_int32]
+    L.asd_demag_workspace_bytes.restype = C.c_size_t
+    L.asd_demag_workspace_bytes.argtypes = [C.c_void_p]
+    L.asd_enable_demag.argtypes = [C.c_void_p, dp, C.c_void_p, C.c_size_t]
+    L.asd_demag_field.argtypes = [C.c_void_p, fp, C.POINTER(C.c_int64)]
     L.asd_shift_window.argtypes = [C.c_void_p, C.c_int32]
     L.asd_magnetisation.argtypes = [C.c_void_p, dp, dp]
     L.asd_grain_magnetisation.argtypes = [C.c_void_p, dp]
@@ -270,6 +275,25 @@ class Context:
 
     def set_kernel(self, variant: int):
         self._ck(self._L.asd_set_kernel(self._h, C.c_int32(variant)))
+
+    def enable_demag(self, spacing_m):
+        """asd_enable_demag: spacing_m = lattice constants (ax, ay, az) in metres; allocates the demag workspace."""
+        import torch
+        nbytes = int(self._L.asd_demag_workspace_bytes(self._h))
+        if nbytes == 0:
+            raise AsdError("asd_demag_workspace_bytes failed (cuFFT plan)")
+        self._demag_ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        ptr = (self._demag_ws.data_ptr() + 255) & ~255
+        a = (C.c_double * 3)(*[float(x) for x in spacing_m])
+        self._ck(self._L.asd_enable_demag(self._h, a, C.c_void_p(ptr), C.c_size_t(nbytes)))
+
+    def demag_field(self) -> np.ndarray:
+        """asd_demag_field: demagnetising field of the current spins per macrocell, Tesla, [dcx, dcy, dcz, 3]."""
+        dims = (C.c_int64 * 3)()
+        self._ck(self._L.asd_demag_field(self._h, None, dims))
+        out = np.zeros((dims[0], dims[1], dims[2], 3), dtype=np.float32)
+        self._ck(self._L.asd_demag_field(self._h, out.ctypes.data_as(C.POINTER(C.c_float)), dims))
+        return out
 
     def set_graph_mode(self, mode: int):
         self._ck(self._L.asd_set_graph_mode(self._h, C.c_int32(mode)))

@@ -223,6 +223,7 @@ asd_status asd_destroy(asd_ctx* ctx) {
   if (ctx->c.host_scratch) cudaFreeHost(ctx->c.host_scratch);
   asd::tma_plan_free(ctx->c);
   asd::graphs_free(ctx->c);
+  asd::demag_free(ctx->c);
   delete ctx;
   return ASD_OK;
 }
@@ -342,6 +343,28 @@ asd_status asd_set_graph_mode(asd_ctx* ctx, int32_t mode) {
     return fail(c, ASD_EINVAL, "asd_set_graph_mode: unknown mode");
   c.graph_mode = mode;
   return ASD_OK;
+}
+
+size_t asd_demag_workspace_bytes(asd_ctx* ctx) {
+  if (!ctx) return 0;
+  return demag_workspace_bytes(ctx->c);
+}
+
+asd_status asd_enable_demag(asd_ctx* ctx, const double spacing_m[3], void* d_workspace, size_t bytes) {
+  CTX_OR_RETURN(ctx);
+  if (!spacing_m || !(spacing_m[0] > 0.0) || !(spacing_m[1] > 0.0) || !(spacing_m[2] > 0.0))
+    return fail(c, ASD_EINVAL, "asd_enable_demag: lattice constants must be > 0");
+  if (!d_workspace || ((uintptr_t)d_workspace & 255u)) return fail(c, ASD_EINVAL, "asd_enable_demag: workspace NULL or not 256-byte aligned");
+  if (c.d.ell_width > 0 || c.d.pbc[0] || c.d.pbc[1] || c.d.pbc[2])
+    return fail(c, ASD_EUNSUPPORTED, "asd_enable_demag: open-boundary lattices with built-in shells only");
+  return demag_enable(c, spacing_m, d_workspace, bytes);
+}
+
+asd_status asd_demag_field(asd_ctx* ctx, float* cells, int64_t dims[3]) {
+  CTX_OR_RETURN(ctx);
+  if (!dims) return fail(c, ASD_EINVAL, "asd_demag_field: dims is NULL");
+  if (!c.demag) return fail(c, ASD_ESTATE, "asd_demag_field: asd_enable_demag has not been called");
+  return demag_field_host(c, cells, dims);
 }
 
 asd_status asd_shift_window(asd_ctx* ctx, int32_t p) {

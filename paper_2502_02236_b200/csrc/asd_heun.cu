@@ -56,7 +56,7 @@ __device__ __forceinline__ void load_row(const float* X, uint32_t as, int64_t ba
   }
 }
 
-template <int VEC, int LAT, int STAGE>
+template <int VEC, int LAT, int STAGE, bool DEMAG>
 __global__ void __launch_bounds__(256) heun_stage_general(const StageParams p) {
   const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= p.nthreads) return;
@@ -201,7 +201,12 @@ __global__ void __launch_bounds__(256) heun_stage_general(const StageParams p) {
       normals3(rnd, xi);
       const float4 gp = __ldg(p.grain + gid);
       const float Xs[3] = {own.e[0][v + 1], own.e[1][v + 1], own.e[2][v + 1]};
-      const float Be[3] = {Bex[0][v], Bex[1][v], Bex[2][v]};
+      float Be[3] = {Bex[0][v], Bex[1][v], Bex[2][v]};
+      if (DEMAG) {                                   // Eq. (7): the field of the site's macrocell
+        float Bd[3];
+        demag_at(p, i, j0 + v, k, Bd);
+        Be[0] += Bd[0]; Be[1] += Bd[1]; Be[2] += Bd[2];
+      }
       const float Bap[3] = {Ba[0][v], Ba[1][v], Ba[2][v]};
       const float Ai[3] = {Ain[0][v], Ain[1][v], Ain[2][v]};
       float ov[3], oAv[3];
@@ -218,21 +223,28 @@ __global__ void __launch_bounds__(256) heun_stage_general(const StageParams p) {
   }
 }
 
-template <int VEC, int LAT>
-asd_status launch_pair(Ctx& c, StageParams& p) {
+template <int VEC, int LAT, bool DEMAG>
+asd_status launch_pair_d(Ctx& c, StageParams& p) {
   const int threads = 256;
   p.ngrp = (uint32_t)(c.d.ny / VEC);
   p.nthreads = p.nrows * p.ngrp;
   const unsigned blocks = (p.nthreads + threads - 1) / threads;
   // predictor: X = S -> out = S~, outA = A
   p.aX = c.aS; p.aOut = c.aSt; p.aOutA = AR_A; p.aA = AR_A;
-  heun_stage_general<VEC, LAT, 0><<<blocks, threads, 0, c.launch_stream>>>(p);
+  if (DEMAG) { const asd_status st = launch_demag(c, c.aS); if (st != ASD_OK) return st; }
+  heun_stage_general<VEC, LAT, 0, DEMAG><<<blocks, threads, 0, c.launch_stream>>>(p);
   ASD_LAUNCH_CHECK(c, "heun predictor");
   // corrector: X = S~, A -> out = S
   p.aX = c.aSt; p.aOut = c.aS;
-  heun_stage_general<VEC, LAT, 1><<<blocks, threads, 0, c.launch_stream>>>(p);
+  if (DEMAG) { const asd_status st = launch_demag(c, c.aSt); if (st != ASD_OK) return st; }
+  heun_stage_general<VEC, LAT, 1, DEMAG><<<blocks, threads, 0, c.launch_stream>>>(p);
   ASD_LAUNCH_CHECK(c, "heun corrector");
   return ASD_OK;
+}
+
+template <int VEC, int LAT>
+asd_status launch_pair(Ctx& c, StageParams& p) {
+  return p.demag_B ? launch_pair_d<VEC, LAT, true>(c, p) : launch_pair_d<VEC, LAT, false>(c, p);
 }
 
 }  // namespace
@@ -252,6 +264,7 @@ void fill_stage_params(const Ctx& c, StageParams& p) {
   p.lambda = (float)c.d.lambda;
   p.scale = c.scale;
   p.g0 = (uint64_t)c.x0 * (uint64_t)c.plane;
+  demag_fill_params(c, p);
   uint32_t k0 = (uint32_t)(c.d.seed & 0xFFFFFFFFull), k1 = (uint32_t)(c.d.seed >> 32);
   for (int r = 0; r < 10; ++r) {
     p.key.k0[r] = k0; p.key.k1[r] = k1;
@@ -271,6 +284,7 @@ asd_status launch_heun_direct(Ctx& c, int64_t n, const DynState* dyn) {
   if (c.kernel_variant == ASD_KERNEL_FAST && !fast) return ASD_EUNSUPPORTED;
   const bool staged = c.kernel_variant == ASD_KERNEL_TMA;
   if (staged && !(heun_tma_supported(c) && tma_plan(c))) return ASD_EUNSUPPORTED;
+  if (c.demag && (staged || c.d.ell_width > 0)) return ASD_EUNSUPPORTED;   // demag: film and general kernels only
   for (int64_t s = 0; s < n; ++s) {
     const uint64_t idx = dyn ? (uint64_t)s : (uint64_t)c.step;
     p.n_lo = (uint32_t)(idx & 0xFFFFFFFFull);

@@ -37,6 +37,9 @@ struct FastParams {
   float gdt, lambda, scale;
   uint32_t n_lo, n_hi;
   const DynState* dyn;
+  const float* demag_B;            // demagnetising field per macrocell (see StageParams); used by the DEMAG instances
+  uint32_t dm_comp, dm_sx, dm_sy;
+  int32_t dm_mx, dm_my, dm_mz, dm_x0, dm_c0;
   uint64_t g0;
   PhiloxKey key;
 };
@@ -60,7 +63,7 @@ constexpr uint32_t kPrefetchAhead = 148;
 
 // CTA shape: 128 threads x 5 CTAs per SM (96 registers per thread).  Measured on cfg4: 57.9 us per stage, against
 // 59.9 (256 x 3, 80 registers), 58.3 (128 x 4), 58.8 (128 x 6), 60.8 (256 x 2), 69.5 (512 x 1).
-template <int LAT, int STAGE, int NT = 128, int MINB = 5>
+template <int LAT, int STAGE, int NT = 128, int MINB = 5, bool DEMAG = false>
 __global__ void __launch_bounds__(NT, MINB) heun_stage_fast(const FastParams p) {
   // ---- L2 prefetch: one bulk-prefetch instruction per streamed array brings the sites of the CTA that will run
   // kPrefetchAhead blocks later from HBM into L2.  It holds no registers and nobody waits for it; when that CTA's
@@ -165,7 +168,12 @@ __global__ void __launch_bounds__(NT, MINB) heun_stage_fast(const FastParams p) 
     float xi[3];
     normals3(rnd, xi);
     const float Xs[3] = {own[0][v + 1], own[1][v + 1], own[2][v + 1]};
-    const float Be[3] = {Bex[0][v], Bex[1][v], Bex[2][v]};
+    float Be[3] = {Bex[0][v], Bex[1][v], Bex[2][v]};
+    if (DEMAG) {                                     // Eq. (7): the field of the site's macrocell
+      float Bd[3];
+      demag_at(p, (int)i, (int)(j0 + v), (int)k, Bd);
+      Be[0] += Bd[0]; Be[1] += Bd[1]; Be[2] += Bd[2];
+    }
     const float Bap[3] = {bx[v], by[v], bz[v]};
     const float Ai[3] = {Ain[0][v], Ain[1][v], Ain[2][v]};
     float ov[3], oAv[3];
@@ -189,16 +197,18 @@ void magic(uint32_t d, uint32_t& m, uint32_t& s) {
   s = L - 1;
 }
 
-template <int LAT, int NT = 128, int MINB = 5>
+template <int LAT, bool DEMAG, int NT = 128, int MINB = 5>
 asd_status launch_pair_fast(Ctx& c, FastParams& f) {
   const unsigned blocks = (f.nthreads + NT - 1u) / NT;
   f.pf_elems = ((uint32_t)NT * 4u / f.ny + 2u) * f.nyp;
   const uint32_t as = f.as;
   f.oX = (uint32_t)c.aS * as; f.oOut = (uint32_t)c.aSt * as; f.oOutA = AR_A * as; f.oA = AR_A * as;
-  heun_stage_fast<LAT, 0, NT, MINB><<<blocks, NT, 0, c.launch_stream>>>(f);
+  if (DEMAG) { const asd_status st = launch_demag(c, c.aS); if (st != ASD_OK) return st; }
+  heun_stage_fast<LAT, 0, NT, MINB, DEMAG><<<blocks, NT, 0, c.launch_stream>>>(f);
   ASD_LAUNCH_CHECK(c, "heun predictor (fast)");
   f.oX = (uint32_t)c.aSt * as; f.oOut = (uint32_t)c.aS * as;
-  heun_stage_fast<LAT, 1, NT, MINB><<<blocks, NT, 0, c.launch_stream>>>(f);
+  if (DEMAG) { const asd_status st = launch_demag(c, c.aSt); if (st != ASD_OK) return st; }
+  heun_stage_fast<LAT, 1, NT, MINB, DEMAG><<<blocks, NT, 0, c.launch_stream>>>(f);
   ASD_LAUNCH_CHECK(c, "heun corrector (fast)");
   return ASD_OK;
 }
@@ -224,7 +234,10 @@ asd_status launch_heun_fast(Ctx& c, StageParams& p) {
   f.j1 = p.jx[0]; f.j2 = p.jx[1]; f.j3 = p.jx[2];
   f.gdt = p.gdt; f.lambda = p.lambda; f.scale = p.scale;
   f.n_lo = p.n_lo; f.n_hi = p.n_hi; f.dyn = p.dyn; f.g0 = p.g0; f.key = p.key;
-  return c.d.lattice == ASD_SC ? launch_pair_fast<LAT_SC>(c, f) : launch_pair_fast<LAT_L10>(c, f);
+  f.demag_B = p.demag_B; f.dm_comp = p.dm_comp; f.dm_sx = p.dm_sx; f.dm_sy = p.dm_sy;
+  f.dm_mx = p.dm_mx; f.dm_my = p.dm_my; f.dm_mz = p.dm_mz; f.dm_x0 = p.dm_x0; f.dm_c0 = p.dm_c0;
+  if (p.demag_B) return c.d.lattice == ASD_SC ? launch_pair_fast<LAT_SC, true>(c, f) : launch_pair_fast<LAT_L10, true>(c, f);
+  return c.d.lattice == ASD_SC ? launch_pair_fast<LAT_SC, false>(c, f) : launch_pair_fast<LAT_L10, false>(c, f);
 }
 
 }  // namespace asd

@@ -79,10 +79,27 @@ struct StageParams {
   float scale;                 // B_app = scale * B
   uint32_t n_lo, n_hi;         // step index before the step (with dyn: offset of this step inside the graph)
   const DynState* dyn;         // nullptr outside graph replays
+  // demagnetising field per macrocell (asd_demag.cu); nullptr = off.  demag_B[comp*dm_comp + (ci*dm_sx + cj*dm_sy + ck)]
+  // with ci = (dm_x0 + i)/dm_mx - dm_c0, cj = j/dm_my, ck = k/dm_mz.
+  const float* demag_B;
+  uint32_t dm_comp, dm_sx, dm_sy;
+  int32_t dm_mx, dm_my, dm_mz, dm_x0, dm_c0;
   uint64_t g0;                 // x0 * ny * nz: global id of window site 0
   PhiloxKey key;
 };
 
+#ifdef __CUDACC__
+// Demagnetising field (Tesla) of the macrocell of window site (i, j, k); P = any parameter block with the dm_* members.
+template <class P>
+__device__ __forceinline__ void demag_at(const P& p, int i, int j, int k, float Bd[3]) {
+  const uint32_t q = (uint32_t)((p.dm_x0 + i) / p.dm_mx - p.dm_c0) * p.dm_sx + (uint32_t)(j / p.dm_my) * p.dm_sy +
+                     (uint32_t)(k / p.dm_mz);
+  Bd[0] = __ldg(p.demag_B + q); Bd[1] = __ldg(p.demag_B + (p.dm_comp + q)); Bd[2] = __ldg(p.demag_B + (2u * p.dm_comp + q));
+}
+#endif
+
+struct DemagPlan;           // asd_demag.cu: cuFFT plans, transformed tensor and buffers of the demagnetising field
+struct DemagPlan;           // asd_demag.cu: cuFFT plans, transformed tensor and buffers of the demagnetising field
 struct TmaPlan;             // asd_heun_tma.cu: tensor maps + strip / chunk plan of the staged film kernel
 
 struct Ctx {
@@ -127,6 +144,7 @@ struct Ctx {
   int32_t graph_mode = ASD_GRAPH_AUTO;
   cudaStream_t cap_stream = nullptr;   // internal stream the graphs are captured on (the caller's may be the legacy one)
   struct GraphCache* graphs = nullptr;
+  DemagPlan* demag = nullptr;       // non-null once asd_enable_demag succeeded
   TmaPlan* tma_plan = nullptr;      // built lazily by the first staged launch (host memory, freed by asd_destroy)
   bool tma_plan_tried = false;
   int64_t launches = 0;
@@ -168,6 +186,13 @@ asd_status launch_heun_direct(Ctx& c, int64_t n, const DynState* dyn);   // 2n p
 void graphs_invalidate(Ctx& c);                               // drop cached graphs (after a shift / a kernel change)
 void graphs_free(Ctx& c);
 DynState* dyn_state(const Ctx& c);
+// demagnetising field (asd_demag.cu)
+size_t demag_workspace_bytes(Ctx& c);
+asd_status demag_enable(Ctx& c, const double spacing[3], void* ws, size_t bytes);
+void demag_free(Ctx& c);
+asd_status launch_demag(Ctx& c, int aX);                      // field of the configuration in arrays aX..aX+2
+void demag_fill_params(const Ctx& c, StageParams& p);
+asd_status demag_field_host(Ctx& c, float* out, int64_t dims[3]);
 asd_status launch_heun_fast(Ctx& c, StageParams& p);          // one Heun step (2 kernels), fast path
 bool heun_fast_supported(const Ctx& c);
 asd_status launch_heun_tma(Ctx& c, StageParams& p);           // one Heun step (2 kernels), TMA-staged film path

@@ -1,0 +1,69 @@
+"""GPU parity of the demagnetising field (csrc/asd_demag.cu) against the oracle's Eq. (6)-(7) (pinned by P12):
+the per-macrocell field itself (FFT convolution vs the oracle's direct sum) and Heun steps with the field on, for both
+lattices, the film and the general kernel, a window whose origin is not aligned with the macrocells, and across a shift."""
+import numpy as np
+import pytest
+
+import asd_inputs as ai
+from tests.helpers import gpu_from_workload, max_abs_diff, oracle_from_workload
+
+pytestmark = pytest.mark.gpu
+
+
+def _film(lattice, nx, ny, nz, macro, x0, tilt, **kw):
+    """small_film whose window starts at global plane x0 (spins re-masked for the columns it then covers)."""
+    w = ai.small_film(lattice, nx, ny, nz, extra_track=8, macro=macro, **kw)
+    w.x0 = x0
+    sx, sy, sz = ai.tilted_spins(w.n_sites, tilt, seed=21)
+    mag = w.magnetic_mask().reshape(-1)
+    w.sx, w.sy, w.sz = (sx * mag).astype(np.float32), (sy * mag).astype(np.float32), (sz * mag).astype(np.float32)
+    return w
+
+
+def _pair(w):
+    sp = [a * 1e-9 for a in w.spacing_nm]
+    o, g = oracle_from_workload(w), gpu_from_workload(w)
+    o.enable_demag(sp); g.enable_demag(sp)
+    return o, g
+
+
+@pytest.mark.parametrize("lattice", [ai.SC, ai.L10])
+@pytest.mark.parametrize("dims,macro,x0", [((24, 28, 6), (3, 3, 3), 0), ((21, 40, 7), (4, 5, 2), 2), ((40, 132, 9), (7, 7, 5), 5)])
+def test_cell_field_matches_oracle(lattice, dims, macro, x0):
+    nx, ny, nz = dims
+    w = _film(lattice, nx, ny, nz, macro, x0, 35.0)
+    o, g = _pair(w)
+    Bo, Bg = o.demag_cells(), g.demag_field()
+    assert Bo.shape == Bg.shape
+    scale = np.abs(Bo).max()
+    assert scale > 1e-3                                            # Tesla: a real field, not zeros
+    assert np.abs(Bg - Bo).max() <= 2e-6 * max(scale, 1.0) + 1e-7  # fp32 FFT convolution vs fp64 direct sum
+
+
+@pytest.mark.parametrize("lattice", [ai.SC, ai.L10])
+@pytest.mark.parametrize("kernel", ["general", "fast"])
+def test_heun_steps_with_demag(lattice, kernel):
+    import paper_2502_02236_b200 as asd
+    w = _film(lattice, 24, 40, 6, (4, 5, 2), 1, 25.0, dt=1e-16)
+    o, g = _pair(w)
+    g.set_kernel({"general": asd.KERNEL_GENERAL, "fast": asd.KERNEL_FAST}[kernel])
+    o.step_heun(1); g.step_heun(1)
+    assert max_abs_diff(g, o) <= 1e-5
+    o.step_heun(3); g.step_heun(3)
+    assert max_abs_diff(g, o) <= 5e-5
+    o.shift_window(3); g.shift_window(3)                           # window origin moves: other cells, other alignment
+    assert np.abs(g.demag_field() - o.demag_cells()).max() <= 5e-6
+    o.step_heun(2); g.step_heun(2)
+    assert max_abs_diff(g, o) <= 1e-4
+
+
+def test_demag_changes_the_dynamics_and_tma_is_refused():
+    import paper_2502_02236_b200 as asd
+    w = ai.small_film(ai.SC, 24, 40, 6, tilt_deg=25.0, dt=1e-15)
+    a, b = gpu_from_workload(w), gpu_from_workload(w)
+    b.enable_demag([x * 1e-9 for x in w.spacing_nm])
+    a.step_heun(5); b.step_heun(5)
+    assert np.abs(a.get_spins_host() - b.get_spins_host()).max() > 1e-7
+    b.set_kernel(asd.KERNEL_TMA)
+    with pytest.raises(asd.AsdError):
+        b.step_heun(1)
