@@ -7,7 +7,7 @@
 // track macrocells that overlap the window (open boundaries; the frozen track's stray field is not included -- callers
 // add it through the per-site B arrays).  Each site then sees the field of its macrocell.
 //
-// Per stage, in stream order:  coarse_grain_cells (one warp per macrocell, shuffle reduction, deterministic)
+// Per stage, in stream order:  coarse_grain_cells (coalesced row sweeps, fixed summation order, deterministic)
 //   -> cuFFT R2C of the 3 zero-padded components -> multiply_tensor (6 real-even kernels, transformed once at set-up)
 //   -> cuFFT C2R -> the stage kernel adds demag_B[cell(site)] to its exchange field.
 // The FFT is the one library primitive on this path (like cuBLAS for a plain GEMM); everything around it is ours.
@@ -101,32 +101,56 @@ int nice_size(int n) {                       // smallest m >= n with only the fa
   }
 }
 
-// One warp per macrocell (a, b, c): sum of X over the cell's sites inside the window, times mu_s / V.
+// Eq. (6).  One CTA per (cell-x a, cell-z c) slab of macrocells.  Threads form a (row-lane, column-group) grid: thread
+// (rl, g) sums its VEC columns over every lanes-th of the slab's mx * mz rows (a row read is one coalesced sweep of ny
+// floats per component; the unrolled row loop keeps several rows in flight); the partial column sums meet in shared
+// memory, where thread b adds the row lanes and the my columns of macrocell (a, b, c) in a fixed order.  Deterministic.
+constexpr int kMaxRowLanes = 8;
+template <int VEC>
 __global__ void coarse_grain_cells(const float* __restrict__ X, uint32_t as, int nx, int ny, int nz, int nyp, int lead,
-                                   int mx, int my, int mz, long long x0, int dcx, int dcy, int dcz, int py, int pz,
-                                   size_t comp_stride, float mu_over_V, float* __restrict__ M) {
-  const int warp = (int)((blockIdx.x * (size_t)blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
-  if (warp >= dcx * dcy * dcz) return;
-  const int c = warp % dcz, b = (warp / dcz) % dcy, a = warp / (dcz * dcy);
-  const long long gx0 = (x0 / mx + a) * (long long)mx;          // first global plane of the cell
-  float s0 = 0.0f, s1 = 0.0f, s2 = 0.0f;
-  const int cell_sites = mx * my * mz;
-  for (int t = lane; t < cell_sites; t += 32) {
-    const int dj = t % my, dk = (t / my) % mz, di = t / (my * mz);
-    const long long i = gx0 + di - x0;
-    const int j = b * my + dj, k = c * mz + dk;
-    if (i >= 0 && i < nx && j < ny && k < nz) {
-      const size_t e = (size_t)lead + ((size_t)i * nz + k) * nyp + j;
-      s0 += X[e]; s1 += X[(size_t)as + e]; s2 += X[2 * (size_t)as + e];
-    }
-  }
+                                   int mx, int my, int mz, long long x0, int dcy, int dcz, int py, int pz,
+                                   size_t comp_stride, float mu_over_V, int lanes, float* __restrict__ M) {
+  extern __shared__ float col[];                                 // [lanes][3][ny]
+  const int a = blockIdx.x / dcz, c = blockIdx.x - a * dcz;
+  const int i0 = (int)((x0 / mx + a) * (long long)mx - x0);      // first window plane of the cell (may be < 0)
+  const int rows = mx * mz, groups = ny / VEC;
+  const int rl = threadIdx.x / groups, g = threadIdx.x - rl * groups;
+  if (rl < lanes) {
+    float s[3][VEC];
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    s0 += __shfl_xor_sync(0xffffffffu, s0, o); s1 += __shfl_xor_sync(0xffffffffu, s1, o); s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+    for (int comp = 0; comp < 3; ++comp)
+#pragma unroll
+      for (int v = 0; v < VEC; ++v) s[comp][v] = 0.0f;
+#pragma unroll 4
+    for (int r = rl; r < rows; r += lanes) {
+      const int i = i0 + r / mz, k = c * mz + r % mz;
+      if (i >= 0 && i < nx && k < nz) {
+        const size_t e = (size_t)lead + ((size_t)i * nz + k) * nyp + (size_t)g * VEC;
+#pragma unroll
+        for (int comp = 0; comp < 3; ++comp) {
+          if (VEC == 4) {
+            const float4 t = __ldg(reinterpret_cast<const float4*>(X + (size_t)comp * as + e));
+            s[comp][0] += t.x; s[comp][1 % VEC] += t.y; s[comp][2 % VEC] += t.z; s[comp][3 % VEC] += t.w;
+          } else {
+            s[comp][0] += __ldg(X + (size_t)comp * as + e);
+          }
+        }
+      }
+    }
+#pragma unroll
+    for (int comp = 0; comp < 3; ++comp)
+#pragma unroll
+      for (int v = 0; v < VEC; ++v) col[((size_t)rl * 3 + comp) * ny + g * VEC + v] = s[comp][v];
   }
-  if (lane == 0) {
+  __syncthreads();
+  for (int b = threadIdx.x; b < dcy; b += blockDim.x) {
+    float t[3] = {0.0f, 0.0f, 0.0f};
+    const int j1 = min((b + 1) * my, ny);
+    for (int j = b * my; j < j1; ++j)
+      for (int l = 0; l < lanes; ++l)
+        for (int comp = 0; comp < 3; ++comp) t[comp] += col[((size_t)l * 3 + comp) * ny + j];
     const size_t q = ((size_t)a * py + b) * pz + c;
-    M[q] = s0 * mu_over_V; M[comp_stride + q] = s1 * mu_over_V; M[2 * comp_stride + q] = s2 * mu_over_V;
+    M[q] = t[0] * mu_over_V; M[comp_stride + q] = t[1] * mu_over_V; M[2 * comp_stride + q] = t[2] * mu_over_V;
   }
 }
 
@@ -203,6 +227,7 @@ size_t demag_workspace_bytes(Ctx& c) {
 }
 
 asd_status demag_enable(Ctx& c, const double spacing[3], void* ws, size_t bytes) {
+  if ((c.d.ny % 4 == 0 ? c.d.ny / 4 : c.d.ny) > 1024 || (size_t)c.d.ny * 12 * kMaxRowLanes > 48 * 1024) { std::snprintf(c.err, sizeof(c.err), "asd_enable_demag: ny too large for the coarse-graining kernel"); return ASD_EUNSUPPORTED; }
   demag_free(c);
   DemagPlan* pl = new DemagPlan();
   plan_dims(c, *pl);
@@ -250,12 +275,24 @@ asd_status demag_enable(Ctx& c, const double spacing[3], void* ws, size_t bytes)
 // Demagnetising field of the configuration in array block aX (S or S~) into demag->B, on c.launch_stream.
 asd_status launch_demag(Ctx& c, int aX) {
   DemagPlan& pl = *c.demag;
-  const int ncell = pl.dcx * pl.dcy * pl.dcz;
   const size_t real = (size_t)pl.px * pl.py * pl.pz, cplx = (size_t)pl.px * pl.py * pl.pzc;
-  const unsigned blocks = (unsigned)((ncell * 32 + 255) / 256);
-  coarse_grain_cells<<<blocks, 256, 0, c.launch_stream>>>(c.arr(aX), (uint32_t)c.as, c.d.nx, c.d.ny, c.d.nz, c.nyp, c.lead,
-                                                          c.d.macro[0], c.d.macro[1], c.d.macro[2], (long long)c.x0, pl.dcx,
-                                                          pl.dcy, pl.dcz, pl.py, pl.pz, real, pl.mu_over_V, pl.M);
+  {
+    const int vec = (c.d.ny % 4 == 0) ? 4 : 1, groups = c.d.ny / vec;
+    int lanes = 1024 / groups;
+    if (lanes > kMaxRowLanes) lanes = kMaxRowLanes;
+    if (lanes < 1) lanes = 1;                                   // groups <= 1024 is checked at enable time
+    const int threads = (int)align_up((size_t)(groups * lanes), 32);
+    const size_t smem = (size_t)lanes * 3 * c.d.ny * sizeof(float);
+    const unsigned blocks = (unsigned)(pl.dcx * pl.dcz);
+    if (vec == 4)
+      coarse_grain_cells<4><<<blocks, threads, smem, c.launch_stream>>>(
+          c.arr(aX), (uint32_t)c.as, c.d.nx, c.d.ny, c.d.nz, c.nyp, c.lead, c.d.macro[0], c.d.macro[1], c.d.macro[2],
+          (long long)c.x0, pl.dcy, pl.dcz, pl.py, pl.pz, real, pl.mu_over_V, lanes, pl.M);
+    else
+      coarse_grain_cells<1><<<blocks, threads, smem, c.launch_stream>>>(
+          c.arr(aX), (uint32_t)c.as, c.d.nx, c.d.ny, c.d.nz, c.nyp, c.lead, c.d.macro[0], c.d.macro[1], c.d.macro[2],
+          (long long)c.x0, pl.dcy, pl.dcz, pl.py, pl.pz, real, pl.mu_over_V, lanes, pl.M);
+  }
   ASD_LAUNCH_CHECK(c, "coarse_grain_cells");
   cufftSetStream(pl.fwd, c.launch_stream); cufftSetStream(pl.inv, c.launch_stream);
   if (cufftExecR2C(pl.fwd, pl.M, pl.Mh) != CUFFT_SUCCESS) return fail_cuda(c, cudaErrorUnknown, "cufftExecR2C");
@@ -266,14 +303,16 @@ asd_status launch_demag(Ctx& c, int aX) {
 }
 
 void demag_fill_params(const Ctx& c, StageParams& p) {
-  p.demag_B = nullptr;
+  p.dm.B = nullptr;
   if (!c.demag) return;
   const DemagPlan& pl = *c.demag;
-  p.demag_B = pl.B;
-  p.dm_comp = (uint32_t)((size_t)pl.px * pl.py * pl.pz);
-  p.dm_sx = (uint32_t)(pl.py * pl.pz); p.dm_sy = (uint32_t)pl.pz;
-  p.dm_mx = c.d.macro[0]; p.dm_my = c.d.macro[1]; p.dm_mz = c.d.macro[2];
-  p.dm_x0 = (int32_t)c.x0; p.dm_c0 = (int32_t)(c.x0 / c.d.macro[0]);
+  p.dm.B = pl.B;
+  p.dm.comp_stride = (uint32_t)((size_t)pl.px * pl.py * pl.pz);
+  p.dm.sx = (uint32_t)(pl.py * pl.pz); p.dm.sy = (uint32_t)pl.pz;
+  magic_u31((uint32_t)c.d.macro[0], p.dm.mx_m, p.dm.mx_s);
+  magic_u31((uint32_t)c.d.macro[1], p.dm.my_m, p.dm.my_s);
+  magic_u31((uint32_t)c.d.macro[2], p.dm.mz_m, p.dm.mz_s);
+  p.dm.x0 = (uint32_t)c.x0; p.dm.c0 = (uint32_t)(c.x0 / c.d.macro[0]);
 }
 
 // Host copy of the cell field of the CURRENT spins (tests, diagnostics); synchronises.

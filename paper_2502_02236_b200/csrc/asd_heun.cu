@@ -204,7 +204,7 @@ __global__ void __launch_bounds__(256) heun_stage_general(const StageParams p) {
       float Be[3] = {Bex[0][v], Bex[1][v], Bex[2][v]};
       if (DEMAG) {                                   // Eq. (7): the field of the site's macrocell
         float Bd[3];
-        demag_at(p, i, j0 + v, k, Bd);
+        demag_at(p.dm, (uint32_t)i, (uint32_t)(j0 + v), (uint32_t)k, Bd);
         Be[0] += Bd[0]; Be[1] += Bd[1]; Be[2] += Bd[2];
       }
       const float Bap[3] = {Ba[0][v], Ba[1][v], Ba[2][v]};
@@ -244,7 +244,7 @@ asd_status launch_pair_d(Ctx& c, StageParams& p) {
 
 template <int VEC, int LAT>
 asd_status launch_pair(Ctx& c, StageParams& p) {
-  return p.demag_B ? launch_pair_d<VEC, LAT, true>(c, p) : launch_pair_d<VEC, LAT, false>(c, p);
+  return p.dm.B ? launch_pair_d<VEC, LAT, true>(c, p) : launch_pair_d<VEC, LAT, false>(c, p);
 }
 
 }  // namespace
@@ -280,7 +280,8 @@ asd_status launch_heun_direct(Ctx& c, int64_t n, const DynState* dyn) {
   fill_stage_params(c, p);
   p.dyn = dyn;
   const bool vec4 = (c.d.ny % 4 == 0);
-  const bool fast = c.kernel_variant != ASD_KERNEL_GENERAL && heun_fast_supported(c);
+  // with the demagnetising field on, the film kernel assumes its 4 sites span at most two macrocells (my >= 3)
+  const bool fast = c.kernel_variant != ASD_KERNEL_GENERAL && heun_fast_supported(c) && !(c.demag && c.d.macro[1] < 3);
   if (c.kernel_variant == ASD_KERNEL_FAST && !fast) return ASD_EUNSUPPORTED;
   const bool staged = c.kernel_variant == ASD_KERNEL_TMA;
   if (staged && !(heun_tma_supported(c) && tma_plan(c))) return ASD_EUNSUPPORTED;

@@ -37,9 +37,8 @@ struct FastParams {
   float gdt, lambda, scale;
   uint32_t n_lo, n_hi;
   const DynState* dyn;
-  const float* demag_B;            // demagnetising field per macrocell (see StageParams); used by the DEMAG instances
-  uint32_t dm_comp, dm_sx, dm_sy;
-  int32_t dm_mx, dm_my, dm_mz, dm_x0, dm_c0;
+  DemagGeom dm;                    // demagnetising field per macrocell; used by the DEMAG instances
+  uint32_t dm_my;                  // macrocell edge in y (sites)
   uint64_t g0;
   PhiloxKey key;
 };
@@ -160,6 +159,18 @@ __global__ void __launch_bounds__(NT, MINB) heun_stage_fast(const FastParams p) 
   uint32_t n_lo = p.n_lo, n_hi = p.n_hi; float scale = p.scale;
   resolve_dyn(p.dyn, n_lo, n_hi, scale);
   const SiteConst sc{p.gdt, p.lambda, scale};
+  // the 4 sites lie in at most two macrocells (any my >= 3; for my < 3 the kernel is not used with demag)
+  float Bd_lo[3] = {0.0f, 0.0f, 0.0f}, Bd_hi[3] = {0.0f, 0.0f, 0.0f};
+  uint32_t dm_split = 0u;                          // sites j < dm_split take Bd_lo
+  if (DEMAG) {
+    const uint32_t q_lo = demag_cell(p.dm, i, j0, k), q_hi = demag_cell(p.dm, i, j0 + 3u, k);
+    dm_split = (q_lo == q_hi) ? 0xFFFFFFFFu : (div_u31(j0 + 3u, p.dm.my_m, p.dm.my_s) * p.dm_my);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      Bd_lo[c] = __ldg(p.dm.B + ((uint32_t)c * p.dm.comp_stride + q_lo));
+      Bd_hi[c] = __ldg(p.dm.B + ((uint32_t)c * p.dm.comp_stride + q_hi));
+    }
+  }
   float o[3][4], oA[3][4];
 #pragma unroll
   for (int v = 0; v < 4; ++v) {
@@ -170,8 +181,7 @@ __global__ void __launch_bounds__(NT, MINB) heun_stage_fast(const FastParams p) 
     const float Xs[3] = {own[0][v + 1], own[1][v + 1], own[2][v + 1]};
     float Be[3] = {Bex[0][v], Bex[1][v], Bex[2][v]};
     if (DEMAG) {                                     // Eq. (7): the field of the site's macrocell
-      float Bd[3];
-      demag_at(p, (int)i, (int)(j0 + v), (int)k, Bd);
+      const float* Bd = (j0 + (uint32_t)v < dm_split) ? Bd_lo : Bd_hi;
       Be[0] += Bd[0]; Be[1] += Bd[1]; Be[2] += Bd[2];
     }
     const float Bap[3] = {bx[v], by[v], bz[v]};
@@ -189,13 +199,6 @@ __global__ void __launch_bounds__(NT, MINB) heun_stage_fast(const FastParams p) 
   }
 }
 
-void magic(uint32_t d, uint32_t& m, uint32_t& s) {
-  if (d <= 1) { m = 0; s = 0; return; }
-  uint32_t L = 0;
-  while ((1ull << L) < d) ++L;
-  m = (uint32_t)(((1ull << (31 + L)) / d) + 1ull);
-  s = L - 1;
-}
 
 template <int LAT, bool DEMAG, int NT = 128, int MINB = 5>
 asd_status launch_pair_fast(Ctx& c, FastParams& f) {
@@ -229,14 +232,13 @@ asd_status launch_heun_fast(Ctx& c, StageParams& p) {
   f.ngrp = (uint32_t)(c.d.ny / 4); f.nthreads = (uint32_t)c.nrows * f.ngrp;
   f.nz = (uint32_t)c.d.nz; f.nx = (uint32_t)c.d.nx; f.ny = (uint32_t)c.d.ny; f.nyp = (uint32_t)c.nyp; f.lead = (uint32_t)c.lead;
   f.planep = (uint32_t)c.d.nz * (uint32_t)c.nyp;
-  magic(f.ngrp, f.m_grp, f.s_grp);
-  magic(f.nz, f.m_nz, f.s_nz);
+  magic_u31(f.ngrp, f.m_grp, f.s_grp);
+  magic_u31(f.nz, f.m_nz, f.s_nz);
   f.j1 = p.jx[0]; f.j2 = p.jx[1]; f.j3 = p.jx[2];
   f.gdt = p.gdt; f.lambda = p.lambda; f.scale = p.scale;
   f.n_lo = p.n_lo; f.n_hi = p.n_hi; f.dyn = p.dyn; f.g0 = p.g0; f.key = p.key;
-  f.demag_B = p.demag_B; f.dm_comp = p.dm_comp; f.dm_sx = p.dm_sx; f.dm_sy = p.dm_sy;
-  f.dm_mx = p.dm_mx; f.dm_my = p.dm_my; f.dm_mz = p.dm_mz; f.dm_x0 = p.dm_x0; f.dm_c0 = p.dm_c0;
-  if (p.demag_B) return c.d.lattice == ASD_SC ? launch_pair_fast<LAT_SC, true>(c, f) : launch_pair_fast<LAT_L10, true>(c, f);
+  f.dm = p.dm; f.dm_my = (uint32_t)c.d.macro[1];
+  if (p.dm.B) return c.d.lattice == ASD_SC ? launch_pair_fast<LAT_SC, true>(c, f) : launch_pair_fast<LAT_L10, true>(c, f);
   return c.d.lattice == ASD_SC ? launch_pair_fast<LAT_SC, false>(c, f) : launch_pair_fast<LAT_L10, false>(c, f);
 }
 

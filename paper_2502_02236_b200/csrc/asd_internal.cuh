@@ -41,6 +41,38 @@ enum : int { AR_S = 0, AR_ST = 3, AR_A = 6, AR_SIGMA = 9, AR_B = 10, AR_COUNT = 
 struct Vec3Ptr { float *x, *y, *z; };
 struct CVec3Ptr { const float *x, *y, *z; };
 
+// n / d for n < 2^31 by multiply-high (m == 0 means d == 1): m = floor(2^(31+L)/d) + 1, s = L - 1, L = ceil(log2 d)
+// (Granlund-Montgomery round-up method with 31-bit dividends: exact).
+inline void magic_u31(uint32_t d, uint32_t& m, uint32_t& s) {
+  if (d <= 1) { m = 0; s = 0; return; }
+  uint32_t L = 0;
+  while ((1ull << L) < d) ++L;
+  m = (uint32_t)(((1ull << (31 + L)) / d) + 1ull);
+  s = L - 1;
+}
+
+// Where a stage kernel finds the demagnetising field of a site's macrocell (asd_demag.cu):
+//   B[comp * comp_stride + ci * sx + cj * sy + ck],  ci = (x0 + i) / mx - c0,  cj = j / my,  ck = k / mz
+// with the three divisions done by multiply-high (magic_u31).
+struct DemagGeom {
+  const float* B;              // nullptr = demag off
+  uint32_t comp_stride, sx, sy;
+  uint32_t mx_m, mx_s, my_m, my_s, mz_m, mz_s;
+  uint32_t x0, c0;
+};
+#ifdef __CUDACC__
+__device__ __forceinline__ uint32_t div_u31(uint32_t n, uint32_t m, uint32_t s) { return m ? (__umulhi(n, m) >> s) : n; }
+// offset of the macrocell of window site (i, j, k) inside one component of dm.B
+__device__ __forceinline__ uint32_t demag_cell(const DemagGeom& dm, uint32_t i, uint32_t j, uint32_t k) {
+  return (div_u31(dm.x0 + i, dm.mx_m, dm.mx_s) - dm.c0) * dm.sx + div_u31(j, dm.my_m, dm.my_s) * dm.sy +
+         div_u31(k, dm.mz_m, dm.mz_s);
+}
+__device__ __forceinline__ void demag_at(const DemagGeom& dm, uint32_t i, uint32_t j, uint32_t k, float Bd[3]) {
+  const uint32_t q = demag_cell(dm, i, j, k);
+  Bd[0] = __ldg(dm.B + q); Bd[1] = __ldg(dm.B + (dm.comp_stride + q)); Bd[2] = __ldg(dm.B + (2u * dm.comp_stride + q));
+}
+#endif
+
 // Device copy of the two values that change between replays of a captured CUDA graph: the step index and the
 // head-field scale.  A kernel launched with dyn != nullptr takes step = dyn step + its own n_lo (its offset inside
 // the graph) and the scale from here instead of from its (frozen) parameter block.
@@ -79,24 +111,11 @@ struct StageParams {
   float scale;                 // B_app = scale * B
   uint32_t n_lo, n_hi;         // step index before the step (with dyn: offset of this step inside the graph)
   const DynState* dyn;         // nullptr outside graph replays
-  // demagnetising field per macrocell (asd_demag.cu); nullptr = off.  demag_B[comp*dm_comp + (ci*dm_sx + cj*dm_sy + ck)]
-  // with ci = (dm_x0 + i)/dm_mx - dm_c0, cj = j/dm_my, ck = k/dm_mz.
-  const float* demag_B;
-  uint32_t dm_comp, dm_sx, dm_sy;
-  int32_t dm_mx, dm_my, dm_mz, dm_x0, dm_c0;
+  DemagGeom dm;                // demagnetising field per macrocell (asd_demag.cu); dm.B == nullptr: off
   uint64_t g0;                 // x0 * ny * nz: global id of window site 0
   PhiloxKey key;
 };
 
-#ifdef __CUDACC__
-// Demagnetising field (Tesla) of the macrocell of window site (i, j, k); P = any parameter block with the dm_* members.
-template <class P>
-__device__ __forceinline__ void demag_at(const P& p, int i, int j, int k, float Bd[3]) {
-  const uint32_t q = (uint32_t)((p.dm_x0 + i) / p.dm_mx - p.dm_c0) * p.dm_sx + (uint32_t)(j / p.dm_my) * p.dm_sy +
-                     (uint32_t)(k / p.dm_mz);
-  Bd[0] = __ldg(p.demag_B + q); Bd[1] = __ldg(p.demag_B + (p.dm_comp + q)); Bd[2] = __ldg(p.demag_B + (2u * p.dm_comp + q));
-}
-#endif
 
 struct DemagPlan;           // asd_demag.cu: cuFFT plans, transformed tensor and buffers of the demagnetising field
 struct DemagPlan;           // asd_demag.cu: cuFFT plans, transformed tensor and buffers of the demagnetising field
