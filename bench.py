@@ -177,6 +177,7 @@ def run_ours(args):
     dev = ctx.device
     if args.demag:
         ctx.enable_demag([a * 1e-9 for a in w.spacing_nm])
+        ctx.set_demag_every(args.demag_every)
     if args.kernel != "auto":
         ctx.set_kernel({"general": asd.KERNEL_GENERAL, "fast": asd.KERNEL_FAST, "tma": asd.KERNEL_TMA}[args.kernel])
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory()
@@ -259,7 +260,7 @@ def run_ours(args):
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": w.name, "sites": N, "heun_steps_per_step": hps, "shifts_in_timed_region": shifts,
-                   "shift_every_heun_steps": w.shift_every, "dt": w.dt, "parallelism": f"replicas x{world}", "demag": bool(args.demag),
+                   "shift_every_heun_steps": w.shift_every, "dt": w.dt, "parallelism": f"replicas x{world}", "demag": bool(args.demag), "demag_every": args.demag_every if args.demag else None,
                    "l2": "working set (13 fp32 arrays/site = %.0f MB) exceeds the 126 MB L2" % (13 * 4 * N / 1e6)},
         "clocks": clocks, "gpu_launches": int(launches),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 16 * N, "d2h_bytes_per_step": 32,
@@ -352,6 +353,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--demag", action="store_true",
                     help="switch the demagnetising field on (Eq. (6)-(7): coarse-graining + FFT convolution per stage)")
+    ap.add_argument("--demag-every", type=int, default=0,
+                    help="0: demag field recomputed in every Heun stage; P >= 1: every P-th step, held in between")
     ap.add_argument("--kernel", default="auto", choices=["auto", "general", "fast", "tma"],
                     help="stage-kernel variant (asd_set_kernel); auto = the library's choice")
     args = ap.parse_args()

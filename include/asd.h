@@ -149,6 +149,10 @@ ASD_API asd_status asd_set_graph_mode(asd_ctx *ctx, int32_t mode);
 ASD_API size_t asd_demag_workspace_bytes(asd_ctx *ctx);
 ASD_API asd_status asd_enable_demag(asd_ctx *ctx, const double spacing_m[3], void *d_workspace, size_t bytes);
 ASD_API asd_status asd_demag_field(asd_ctx *ctx, float *cells, int64_t dims[3]);
+/* every == 0 (default): the field is recomputed from the configuration of EVERY Heun stage (exact Heun on the full
+ * field).  every = P >= 1: it is recomputed from S at the predictor of every P-th Heun step (counted from the last
+ * enable / this call / window shift / asd_set_spins) and held for both stages in between (reading D3). */
+ASD_API asd_status asd_set_demag_every(asd_ctx *ctx, int32_t every);
 
 /* Window moves +x by p planes, 1 <= p <= nx (S:O5): outgoing planes -> macrocell sums and counts (Eq. 6);
  * spins move by p planes; incoming planes seeded by cone sampling (D:S3); x0 += p; shift counter += 1.

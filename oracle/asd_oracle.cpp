@@ -146,6 +146,9 @@ struct Oracle {
   double cell_m[3] = {0, 0, 0};    // macrocell edge lengths, metres
   int dcx = 0, dcy = 0, dcz = 0;   // macrocells that can overlap the window (x: worst alignment)
   std::vector<double> demag_N;     // [(2dcx-1)(2dcy-1)(2dcz-1)][6]: Nxx Nyy Nzz Nxy Nxz Nyz at cell offsets
+  int demag_every = 0;             // 0: recomputed in every stage; P >= 1: from S at every P-th step, held in between (D3)
+  int64_t demag_age = 0;           // steps since the held field was invalidated (enable, set_every, shift, set_spins)
+  std::vector<double> demag_hold;  // the held per-macrocell field
 
   int64_t site(int i, int k, int j) const { return ((int64_t)i * nz + k) * ny + j; }
   int32_t grain_of(int i, int j) const { return grain_map[(size_t)((x0 + i) * ny + j)]; }
@@ -373,7 +376,14 @@ void heun_step(Oracle& o) {
   const int nx = o.nx, ny = o.ny, nz = o.nz;
   const int nt = thread_count(o);
   std::vector<double> Bd;                        // demagnetising field of the stage's configuration, per macrocell
-  if (o.demag) demag_cells(o, o.sx.data(), o.sy.data(), o.sz.data(), Bd);
+  const bool held = o.demag && o.demag_every >= 1;
+  if (held) {
+    if (o.demag_age % o.demag_every == 0) demag_cells(o, o.sx.data(), o.sy.data(), o.sz.data(), o.demag_hold);
+    Bd = o.demag_hold;
+    o.demag_age += 1;
+  } else if (o.demag) {
+    demag_cells(o, o.sx.data(), o.sy.data(), o.sz.data(), Bd);
+  }
 #pragma omp parallel for collapse(2) schedule(static) num_threads(nt)
   for (int i = 0; i < nx; ++i)
     for (int k = 0; k < nz; ++k)
@@ -393,7 +403,7 @@ void heun_step(Oracle& o) {
         tx[l] = p0 / nrm; ty[l] = p1 / nrm; tz[l] = p2 / nrm;
       }
   std::vector<double> n0((size_t)N, 0.0), n1((size_t)N, 0.0), n2((size_t)N, 0.0);
-  if (o.demag) demag_cells(o, tx.data(), ty.data(), tz.data(), Bd);     // B(S~) includes the demagnetising field of S~
+  if (o.demag && !held) demag_cells(o, tx.data(), ty.data(), tz.data(), Bd);   // B(S~) includes the demagnetising field of S~
 #pragma omp parallel for collapse(2) schedule(static) num_threads(nt)
   for (int i = 0; i < nx; ++i)
     for (int k = 0; k < nz; ++k)
@@ -521,6 +531,7 @@ int orc_max_threads() {
 // fp32 inputs (the same arrays the GPU gets), widened without renormalising (S:O1); vacant -> 0.
 void orc_set_spins(void* h, const float* sx, const float* sy, const float* sz) {
   Oracle& o = *static_cast<Oracle*>(h);
+  o.demag_age = 0;
   for (int i = 0; i < o.nx; ++i)
     for (int k = 0; k < o.nz; ++k)
       for (int j = 0; j < o.ny; ++j) {
@@ -565,6 +576,11 @@ void orc_enable_demag(void* h, const double spacing[3]) {
         newell_tensor(o.cell_m, R, &o.demag_N[(((size_t)a * sy + b) * sz + c) * 6]);
       }
   o.demag = true;
+  o.demag_age = 0;
+}
+void orc_set_demag_every(void* h, int every) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  o.demag_every = every; o.demag_age = 0;
 }
 void orc_newell_tensor(const double cell[3], const double R[3], double out[6]) { newell_tensor(cell, R, out); }
 // Demagnetising field of the current spins per window macrocell, Tesla: out[dcx*dcy*dcz*3]; dims returned.
@@ -660,6 +676,7 @@ int orc_shift_window(void* h, int32_t p) {
   if (p < 1 || p > o.nx) return 1;
   if (o.ell_width > 0) return 5;                       // general ELL cannot follow the window
   if (o.x0 + p + o.nx > o.track_nx) return 1;          // grain map must cover the new window
+  o.demag_age = 0;                                     // a held demagnetising field belongs to the old window
   const int nx = o.nx, ny = o.ny, nz = o.nz;
   // S2 outgoing: planes i < p, magnetic sites only, ascending l.
   for (int i = 0; i < p; ++i)

@@ -98,6 +98,7 @@ def lib():
         L.orc_sigma.restype = C.c_double
         L.orc_sigma.argtypes = [C.c_void_p, C.c_double]
         L.orc_enable_demag.argtypes = [C.c_void_p, dp]
+        L.orc_set_demag_every.argtypes = [C.c_void_p, C.c_int]
         L.orc_newell_tensor.argtypes = [dp, dp, dp]
         L.orc_demag_cells.argtypes = [C.c_void_p, dp, ip64]
         _lib = L
@@ -257,6 +258,10 @@ class Oracle:
         """Demagnetising field on (Eq. (6)-(7)); spacing_m = lattice constants (ax, ay, az) in metres."""
         a = np.ascontiguousarray(spacing_m, dtype=np.float64)
         lib().orc_enable_demag(self._h, _ptr(a, C.c_double))
+
+    def set_demag_every(self, every: int):
+        """0: the field is recomputed in every Heun stage; P >= 1: from S at every P-th step, held in between."""
+        lib().orc_set_demag_every(self._h, C.c_int(every))
 
     def demag_cells(self) -> np.ndarray:
         """Demagnetising field per window macrocell, Tesla: [dcx, dcy, dcz, 3]."""

@@ -21,7 +21,7 @@ EXPORTED_SYMBOLS = [
     "asd_workspace_bytes", "asd_create_lattice", "asd_destroy", "asd_set_spins", "asd_get_spins",
     "asd_set_spins_host", "asd_get_spins_host", "asd_set_fields", "asd_set_fields_host", "asd_set_field_scale",
     "asd_step_heun", "asd_set_kernel", "asd_set_graph_mode", "asd_demag_workspace_bytes", "asd_enable_demag",
-    "asd_demag_field", "asd_shift_window", "asd_magnetisation", "asd_grain_magnetisation",
+    "asd_demag_field", "asd_set_demag_every", "asd_shift_window", "asd_magnetisation", "asd_grain_magnetisation",
     "asd_track_dims", "asd_track_set_init", "asd_track_get", "asd_get_counters", "asd_set_counters",
     "asd_launch_count", "asd_last_error", "asd_version",
 ]
@@ -92,6 +92,7 @@ def load_library(build_if_missing: bool = True):
     L.asd_demag_workspace_bytes.argtypes = [C.c_void_p]
     L.asd_enable_demag.argtypes = [C.c_void_p, dp, C.c_void_p, C.c_size_t]
     L.asd_demag_field.argtypes = [C.c_void_p, fp, C.POINTER(C.c_int64)]
+    L.asd_set_demag_every.argtypes = [C.c_void_p, C.c_int32]
     L.asd_shift_window.argtypes = [C.c_void_p, C.c_int32]
     L.asd_magnetisation.argtypes = [C.c_void_p, dp, dp]
     L.asd_grain_magnetisation.argtypes = [C.c_void_p, dp]
@@ -286,6 +287,9 @@ class Context:
         ptr = (self._demag_ws.data_ptr() + 255) & ~255
         a = (C.c_double * 3)(*[float(x) for x in spacing_m])
         self._ck(self._L.asd_enable_demag(self._h, a, C.c_void_p(ptr), C.c_size_t(nbytes)))
+
+    def set_demag_every(self, every: int):
+        self._ck(self._L.asd_set_demag_every(self._h, C.c_int32(every)))
 
     def demag_field(self) -> np.ndarray:
         """asd_demag_field: demagnetising field of the current spins per macrocell, Tesla, [dcx, dcy, dcz, 3]."""

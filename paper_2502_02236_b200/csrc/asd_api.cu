@@ -232,6 +232,7 @@ asd_status asd_destroy(asd_ctx* ctx) {
 // corrector, and nothing reads A's padding), then packed into the padded-row layout by a kernel.
 static asd_status set_spins_impl(Ctx& c, const float* sx, const float* sy, const float* sz, bool host) {
   if (!sx || !sy || !sz) return fail(c, ASD_EINVAL, "asd_set_spins: NULL pointer");
+  c.demag_age = 0;                             // a held demagnetising field belongs to the old spins
   if (host) {
     const float* src[3] = {sx, sy, sz};
     for (int a = 0; a < 3; ++a)
@@ -357,7 +358,16 @@ asd_status asd_enable_demag(asd_ctx* ctx, const double spacing_m[3], void* d_wor
   if (!d_workspace || ((uintptr_t)d_workspace & 255u)) return fail(c, ASD_EINVAL, "asd_enable_demag: workspace NULL or not 256-byte aligned");
   if (c.d.ell_width > 0 || c.d.pbc[0] || c.d.pbc[1] || c.d.pbc[2])
     return fail(c, ASD_EUNSUPPORTED, "asd_enable_demag: open-boundary lattices with built-in shells only");
+  c.demag_age = 0;
   return demag_enable(c, spacing_m, d_workspace, bytes);
+}
+
+asd_status asd_set_demag_every(asd_ctx* ctx, int32_t every) {
+  CTX_OR_RETURN(ctx);
+  if (every < 0) return fail(c, ASD_EINVAL, "asd_set_demag_every: every < 0");
+  c.demag_every = every;
+  c.demag_age = 0;
+  return ASD_OK;
 }
 
 asd_status asd_demag_field(asd_ctx* ctx, float* cells, int64_t dims[3]) {
@@ -374,6 +384,7 @@ asd_status asd_shift_window(asd_ctx* ctx, int32_t p) {
   if (c.d.pbc[0]) return fail(c, ASD_EUNSUPPORTED, "asd_shift_window: window is periodic in x");
   if (c.x0 + p + c.d.nx > c.d.track_nx) return fail(c, ASD_ESTATE, "asd_shift_window: past the end of the track");
   graphs_invalidate(c);                        // window origin and buffer roles are frozen in recorded graphs
+  c.demag_age = 0;                             // a held demagnetising field belongs to the old window position
   return launch_shift(c, p);
 }
 

@@ -231,12 +231,12 @@ asd_status launch_pair_d(Ctx& c, StageParams& p) {
   const unsigned blocks = (p.nthreads + threads - 1) / threads;
   // predictor: X = S -> out = S~, outA = A
   p.aX = c.aS; p.aOut = c.aSt; p.aOutA = AR_A; p.aA = AR_A;
-  if (DEMAG) { const asd_status st = launch_demag(c, c.aS); if (st != ASD_OK) return st; }
+  if (DEMAG && (c.demag_refresh & 1)) { const asd_status st = launch_demag(c, c.aS); if (st != ASD_OK) return st; }
   heun_stage_general<VEC, LAT, 0, DEMAG><<<blocks, threads, 0, c.launch_stream>>>(p);
   ASD_LAUNCH_CHECK(c, "heun predictor");
   // corrector: X = S~, A -> out = S
   p.aX = c.aSt; p.aOut = c.aS;
-  if (DEMAG) { const asd_status st = launch_demag(c, c.aSt); if (st != ASD_OK) return st; }
+  if (DEMAG && (c.demag_refresh & 2)) { const asd_status st = launch_demag(c, c.aSt); if (st != ASD_OK) return st; }
   heun_stage_general<VEC, LAT, 1, DEMAG><<<blocks, threads, 0, c.launch_stream>>>(p);
   ASD_LAUNCH_CHECK(c, "heun corrector");
   return ASD_OK;
@@ -290,6 +290,10 @@ asd_status launch_heun_direct(Ctx& c, int64_t n, const DynState* dyn) {
     const uint64_t idx = dyn ? (uint64_t)s : (uint64_t)c.step;
     p.n_lo = (uint32_t)(idx & 0xFFFFFFFFull);
     p.n_hi = (uint32_t)(idx >> 32);
+    if (c.demag) {
+      c.demag_refresh = c.demag_every <= 0 ? 3 : (c.demag_age % c.demag_every == 0 ? 1 : 0);
+      c.demag_age += 1;
+    }
     asd_status st;
     if (staged) st = launch_heun_tma(c, p);
     else if (fast) st = launch_heun_fast(c, p);

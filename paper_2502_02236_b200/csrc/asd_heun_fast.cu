@@ -206,11 +206,11 @@ asd_status launch_pair_fast(Ctx& c, FastParams& f) {
   f.pf_elems = ((uint32_t)NT * 4u / f.ny + 2u) * f.nyp;
   const uint32_t as = f.as;
   f.oX = (uint32_t)c.aS * as; f.oOut = (uint32_t)c.aSt * as; f.oOutA = AR_A * as; f.oA = AR_A * as;
-  if (DEMAG) { const asd_status st = launch_demag(c, c.aS); if (st != ASD_OK) return st; }
+  if (DEMAG && (c.demag_refresh & 1)) { const asd_status st = launch_demag(c, c.aS); if (st != ASD_OK) return st; }
   heun_stage_fast<LAT, 0, NT, MINB, DEMAG><<<blocks, NT, 0, c.launch_stream>>>(f);
   ASD_LAUNCH_CHECK(c, "heun predictor (fast)");
   f.oX = (uint32_t)c.aSt * as; f.oOut = (uint32_t)c.aS * as;
-  if (DEMAG) { const asd_status st = launch_demag(c, c.aSt); if (st != ASD_OK) return st; }
+  if (DEMAG && (c.demag_refresh & 2)) { const asd_status st = launch_demag(c, c.aSt); if (st != ASD_OK) return st; }
   heun_stage_fast<LAT, 1, NT, MINB, DEMAG><<<blocks, NT, 0, c.launch_stream>>>(f);
   ASD_LAUNCH_CHECK(c, "heun corrector (fast)");
   return ASD_OK;

@@ -164,6 +164,9 @@ struct Ctx {
   cudaStream_t cap_stream = nullptr;   // internal stream the graphs are captured on (the caller's may be the legacy one)
   struct GraphCache* graphs = nullptr;
   DemagPlan* demag = nullptr;       // non-null once asd_enable_demag succeeded
+  int32_t demag_every = 0;          // 0: field recomputed in every stage; P >= 1: from S at every P-th Heun step, held in between
+  int64_t demag_age = 0;            // Heun steps since the held field was last invalidated (enable, shift, set_spins)
+  int32_t demag_refresh = 3;        // this step: bit 0 = recompute before the predictor, bit 1 = before the corrector
   TmaPlan* tma_plan = nullptr;      // built lazily by the first staged launch (host memory, freed by asd_destroy)
   bool tma_plan_tried = false;
   int64_t launches = 0;

@@ -57,6 +57,24 @@ def test_heun_steps_with_demag(lattice, kernel):
     assert max_abs_diff(g, o) <= 1e-4
 
 
+@pytest.mark.parametrize("every", [1, 3])
+def test_held_field_update_period(every):
+    """asd_set_demag_every(P): field from S at every P-th step, held for both stages in between; a shift re-arms it."""
+    w = _film(ai.L10, 24, 40, 6, (4, 5, 2), 1, 25.0, dt=1e-16)
+    o, g = _pair(w)
+    o.set_demag_every(every); g.set_demag_every(every)
+    o.step_heun(4); g.step_heun(4)
+    assert max_abs_diff(g, o) <= 5e-5
+    o.shift_window(2); g.shift_window(2)
+    o.step_heun(2); g.step_heun(2)
+    assert max_abs_diff(g, o) <= 1e-4
+    # and it is a different scheme from the per-stage default (the corrector sees B_d(S), not B_d(S~))
+    o2, _g2 = _pair(w)
+    o2.step_heun(4)
+    o3, _g3 = _pair(w); o3.set_demag_every(every); o3.step_heun(4)
+    assert np.abs(o2.get_spins() - o3.get_spins()).max() > 0.0
+
+
 def test_demag_changes_the_dynamics_and_tma_is_refused():
     import paper_2502_02236_b200 as asd
     w = ai.small_film(ai.SC, 24, 40, 6, tilt_deg=25.0, dt=1e-15)
