@@ -79,3 +79,59 @@ def test_bulk_periodic_m_of_t():
     # paramagnetic 1/sqrt(N) remnant at 800 K (one 4096-spin system, slow fluctuations)
     assert np.abs(m_g - m_o)[:4].max() <= TOL_M
     assert m_g[4] < 0.12 and m_o[4] < 0.12 and abs(m_g[4] - m_o[4]) <= 0.04
+
+
+def test_thermal_divergence_report():
+    """Informational (SURVEY 8(c) acceptance, Q18): max |dS| between the fp32 path and the fp64 oracle after
+    1, 10, 100, 1000 thermal steps of cfg0 (300 K, same seed).  Rounding differences are amplified chaotically; only the
+    first decade is bounded here, the rest is printed for the record."""
+    w = ai.make_config(0)
+    o, g = oracle_from_workload(w), gpu_from_workload(w)
+    done, report = 0, {}
+    for n in (1, 10, 100, 1000):
+        o.step_heun(n - done); g.step_heun(n - done); done = n
+        report[n] = float(np.abs(g.get_spins_host().astype(np.float64) - o.get_spins()).max())
+    print("cfg0 thermal divergence, max |dS| after n steps:", {k: f"{v:.2e}" for k, v in report.items()})
+    assert report[1] <= 1e-5 and report[10] <= 1e-4
+    assert all(np.isfinite(v) and v <= 2.0 for v in report.values())
+
+
+def test_cfg1_full_size_temperature_sweep():
+    """BASELINE configs[1] at full size and full length on the GPU: 192x192x27 sites, T = 300 .. 900 K in 50 K steps,
+    2e4 Heun steps per temperature, state carried over; M(T) and per-grain T_C.  The oracle cannot follow at this size
+    (~3.5 h); its role is played by the shrunken-film comparison above.  Checked here: M(T) falls monotonically through
+    the transition; the fitted T_C lies between the 3 nm grains' 670 K (shrunken film above) and the bulk value at this
+    time step (745-766 K at dt = 1 fs, lambda = 1: pin P8's O(dt) bias of stochastic Heun), with the 3-D
+    Heisenberg exponent; the per-grain T_C scatter is small (k_u varies by 5 %, J does not).
+    Last run: T_C = 714.0 K, beta = 0.384, per-grain T_C 716.3 +- 7.5 K over 61 whole grains."""
+    w = ai.make_config(1, uniform_T=300.0)
+    temps = np.arange(300.0, 901.0, 50.0)
+    g = gpu_from_workload(w)
+    side = Side(g, w.n_sites, True)
+    wts = _weights(w)
+    per_grain = []
+    for T in temps:
+        side.set_uniform_T(float(T))
+        side.step(10000)
+        acc = []
+        for _ in range(20):
+            side.step(500)
+            acc.append(np.linalg.norm(side.grain_m(), axis=1))
+        per_grain.append(np.mean(acc, axis=0))
+    per_grain = np.array(per_grain)                                  # [temperature, grain]
+    big = wts >= 0.5 * np.median(wts[wts > 0])                       # whole grains (edge slivers excluded)
+    m = np.array([np.average(r[big], weights=wts[big]) for r in per_grain])
+    tc, beta = fit_tc(temps, m)
+    tcs = []
+    for gi in np.nonzero(big)[0]:
+        try:
+            tcs.append(fit_tc(temps, per_grain[:, gi])[0])
+        except Exception:
+            pass
+    tcs = np.array(tcs)
+    print("cfg1 full size: M(T)", np.round(m, 4), f"T_C {tc:.1f} K beta {beta:.3f}; per-grain T_C mean {tcs.mean():.1f} "
+          f"std {tcs.std():.1f} K over {len(tcs)} grains")
+    assert np.all(np.diff(m)[: np.argmax(m < 0.1)] < 0.0)
+    assert 670.0 < tc < 766.0 and 0.3 < beta < 0.45
+    assert m[0] > 0.75 and m[-1] < 0.1
+    assert tcs.std() < 40.0
