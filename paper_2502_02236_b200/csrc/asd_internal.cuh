@@ -32,7 +32,10 @@ constexpr double kGammaDefault = 1.76085963023e11; // rad s^-1 T^-1 (DESIGN.md Q
 enum : uint32_t {
   BOND_XP = 1u << 16, BOND_XM = 1u << 17, BOND_YP = 1u << 18, BOND_YM = 1u << 19,
   BOND_XPYP = 1u << 20, BOND_XPYM = 1u << 21, BOND_XMYP = 1u << 22, BOND_XMYM = 1u << 23,
-  BOND_ALL_XP = BOND_XP | BOND_XPYP | BOND_XPYM, BOND_ALL_XM = BOND_XM | BOND_XMYP | BOND_XMYM
+  BOND_ALL_XP = BOND_XP | BOND_XPYP | BOND_XPYM, BOND_ALL_XM = BOND_XM | BOND_XMYP | BOND_XMYM,
+  // bit 24: the 4-aligned group of columns (gx, 4q .. 4q+3) this column belongs to holds two DIFFERENT grains (the film
+  // kernel then gathers anisotropy parameters per site instead of once per group)
+  COL_GROUP_MIXED = 1u << 24
 };
 
 // indices of the 13 per-site arrays inside the block `arrays` (stride `as` elements)

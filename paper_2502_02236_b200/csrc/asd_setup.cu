@@ -24,7 +24,19 @@ __global__ void build_columns_kernel(const int32_t* __restrict__ gmap, uint32_t*
   const int32_t g = gmap ? gmap[t] : 0;
   const float4 gp = grain[g + 1];                 // entry 0 = vacant
   aniso[t] = gp.x; aniso[ncol + t] = gp.y; aniso[2 * ncol + t] = gp.z; aniso[3 * ncol + t] = gp.w;
-  if (g < 0) { col[t] = 0u; return; }
+  if (g < 0) {                                    // vacant column: id 0; the group flag still has to be right
+    uint32_t e0 = 0u;
+    const int j4 = j & ~3;
+    int32_t first = -1;
+    for (int q = j4; q < j4 + 4 && q < ny; ++q) {
+      const int32_t gq = gmap[gx * ny + q];
+      if (gq < 0) continue;
+      if (first < 0) first = gq;
+      else if (gq != first) e0 |= COL_GROUP_MIXED;
+    }
+    col[t] = e0;
+    return;
+  }
   uint32_t e = (uint32_t)(g + 1) & 0xFFFFu;
   const int dxs[8] = {1, -1, 0, 0, 1, 1, -1, -1};
   const int dys[8] = {0, 0, 1, -1, 1, -1, 1, -1};
@@ -38,6 +50,18 @@ __global__ void build_columns_kernel(const int32_t* __restrict__ gmap, uint32_t*
     const int32_t gn = gmap ? gmap[x * ny + y] : 0;
     if (gn == g) e |= 1u << (16 + b);
     else if (gn >= 0) touch = true;
+  }
+  {
+    const int j4 = j & ~3;
+    int32_t first = -1;
+    bool mixed = false;
+    for (int q = j4; q < j4 + 4 && q < ny; ++q) {
+      const int32_t gq = gmap ? gmap[gx * ny + q] : 0;
+      if (gq < 0) continue;
+      if (first < 0) first = gq;
+      else if (gq != first) mixed = true;
+    }
+    if (mixed) e |= COL_GROUP_MIXED;
   }
   col[t] = e;
   if (touch) atomicOr(flags, 1);
