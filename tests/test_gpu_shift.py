@@ -96,3 +96,20 @@ def test_shift_errors():
         g.shift_window(3)              # past the end of the track
     assert e.value.status == 4
     g.shift_window(2)
+
+
+def test_option_and_demag_errors():
+    """Error behaviour of the option calls (include/asd.h): bad arguments are ASD_EINVAL, demag queries before
+    asd_enable_demag are ASD_ESTATE, lattices the demag path does not cover are ASD_EUNSUPPORTED."""
+    import paper_2502_02236_b200 as asd
+    w = ai.small_film(ai.SC, 8, 8, 3)
+    g = gpu_from_workload(w)
+    for bad in (lambda: g.set_graph_mode(7), lambda: g.set_kernel(9), lambda: g.set_demag_every(-1),
+                lambda: g.demag_field(), lambda: g.enable_demag([0.3e-9, 0.0, 0.3e-9])):
+        with pytest.raises(asd.AsdError):
+            bad()
+    g.step_heun(2)                                        # the context is still usable after the refused calls
+    p = ai.make_config(0)                                 # periodic: no demag
+    gp = gpu_from_workload(p)
+    with pytest.raises(asd.AsdError):
+        gp.enable_demag([0.3e-9] * 3)
