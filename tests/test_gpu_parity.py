@@ -172,3 +172,46 @@ def test_full_size_one_step(cfg, kernel):
     g.step_heun(2)
     assert float(np.abs(g.get_spins_host().astype(np.float64) - o).max()) <= 2e-5
     _check_norm(g, w)
+
+
+def test_near_the_32bit_offset_limit():
+    """Maximum size of the film kernel (13 arrays x stride < 2^31 elements): a 147 M-site L1_0 window whose initial state
+    is periodic with period 8 in every direction must reproduce, plane for plane and bit for bit, a 24-plane window with
+    the same pattern (T = 0: no noise; identical local environments away from the x edges give identical arithmetic).
+    Checks every element offset of the large window without the oracle having to hold 147 M fp64 sites."""
+    import torch
+    import paper_2502_02236_b200 as asd
+    ny, nz = 256, 64
+    dev = torch.device("cuda", 0)
+    free, _ = torch.cuda.mem_get_info()
+    nx_big = 8960                                              # 146.8 M sites: 13 * stride = 1.99e9 < 2^31
+    if free < 12 * (1 << 30):
+        pytest.skip("needs 12 GB of free device memory")
+
+    def run(nx):
+        d = asd.LatticeDesc(lattice=ai.L10, nx=nx, ny=ny, nz=nz, J=(5.0e-21, 2.0e-21, 0.8e-21), dt=1e-15, lam=0.1,
+                            grain_ku=np.array([9.1e-23], dtype=np.float32),
+                            grain_axis=np.array([[0.0, 0.6, 0.8]], dtype=np.float32))
+        ctx = asd.Context(d)
+        ctx.set_kernel(asd.KERNEL_FAST)
+        i = torch.arange(nx, device=dev).view(nx, 1, 1) % 8
+        k = torch.arange(nz, device=dev).view(1, nz, 1) % 8
+        j = torch.arange(ny, device=dev).view(1, 1, ny) % 8
+        th = 0.3 + 0.05 * (i + 2 * k) + 0.02 * j                # polar angle pattern, period 8
+        ph = 0.7 * i + 0.4 * j + 0.9 * k
+        sx = (torch.sin(th) * torch.cos(ph)).float().reshape(-1).contiguous()
+        sy = (torch.sin(th) * torch.sin(ph)).float().reshape(-1).contiguous()
+        sz = torch.cos(th).float().reshape(-1).contiguous()
+        ctx.set_spins(sx, sy, sz)
+        N = nx * ny * nz
+        z = torch.zeros(N, device=dev)
+        ctx.set_fields(z, z, z, torch.full((N,), 0.5, device=dev))
+        ctx.step_heun(2)
+        ctx.get_spins(sx, sy, sz)
+        torch.cuda.synchronize()
+        return torch.stack([sx, sy, sz]).view(3, nx, nz * ny)
+
+    small = run(24)[:, 8:16].clone()                            # planes 8..15: two steps cannot see the x edges
+    big = run(nx_big)
+    for start in (8, 4480, nx_big - 16):                        # start % 8 == 0: same phase of the pattern
+        assert torch.equal(big[:, start:start + 8], small), start
