@@ -129,6 +129,21 @@ ASD_API asd_status asd_set_fields_host(asd_ctx *ctx, const float *T, const float
 /* B_app = s * B : write-field polarity / ramp. */
 ASD_API asd_status asd_set_field_scale(asd_ctx *ctx, float s);
 
+/* Double-buffered upload of host fields, for callers that change T / B every batch (the laser and the head move):
+ * the host-to-device copy of the NEXT batch's fields overlaps the Heun steps of the current one.
+ *   asd_set_staging        once: a caller-owned DEVICE buffer of asd_staging_bytes(ctx) bytes, 256-byte aligned.
+ *   asd_stage_fields_host  starts the copy of the given HOST arrays (pinned for a truly asynchronous copy; NULL = leave
+ *                          that field as it is) into the staging buffer on an internal stream and returns at once; the
+ *                          arrays must stay valid and unchanged until the next asd_commit_fields has been called and
+ *                          the stream has passed it.  It first waits (on the device) for the previous commit.
+ *   asd_commit_fields      makes the staged fields the current ones for every step enqueued after it (the context's
+ *                          stream waits for the copy, then repacks as asd_set_fields does).  Nothing staged: no-op.
+ * ASD_ESTATE before asd_set_staging. */
+ASD_API size_t asd_staging_bytes(const asd_ctx *ctx);
+ASD_API asd_status asd_set_staging(asd_ctx *ctx, void *d_staging, size_t bytes);
+ASD_API asd_status asd_stage_fields_host(asd_ctx *ctx, const float *T, const float *Bx, const float *By, const float *Bz);
+ASD_API asd_status asd_commit_fields(asd_ctx *ctx);
+
 /* n stochastic Heun steps (S:O4): per step one predictor and one corrector kernel, each fused
  * field + update + renormalise with in-register Philox noise (same xi in both stages); step counter += n. */
 ASD_API asd_status asd_step_heun(asd_ctx *ctx, int64_t n);

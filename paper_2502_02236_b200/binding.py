@@ -21,7 +21,8 @@ EXPORTED_SYMBOLS = [
     "asd_workspace_bytes", "asd_create_lattice", "asd_destroy", "asd_set_spins", "asd_get_spins",
     "asd_set_spins_host", "asd_get_spins_host", "asd_set_fields", "asd_set_fields_host", "asd_set_field_scale",
     "asd_step_heun", "asd_set_kernel", "asd_set_graph_mode", "asd_demag_workspace_bytes", "asd_enable_demag",
-    "asd_demag_field", "asd_set_demag_every", "asd_shift_window", "asd_magnetisation", "asd_grain_magnetisation",
+    "asd_demag_field", "asd_set_demag_every", "asd_staging_bytes", "asd_set_staging", "asd_stage_fields_host",
+    "asd_commit_fields", "asd_shift_window", "asd_magnetisation", "asd_grain_magnetisation",
     "asd_track_dims", "asd_track_set_init", "asd_track_get", "asd_get_counters", "asd_set_counters",
     "asd_launch_count", "asd_last_error", "asd_version",
 ]
@@ -85,6 +86,11 @@ def load_library(build_if_missing: bool = True):
     for name in ("asd_set_fields", "asd_set_fields_host"):
         getattr(L, name).argtypes = [C.c_void_p, fp, fp, fp, fp]
     L.asd_set_field_scale.argtypes = [C.c_void_p, C.c_float]
+    L.asd_staging_bytes.restype = C.c_size_t
+    L.asd_staging_bytes.argtypes = [C.c_void_p]
+    L.asd_set_staging.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t]
+    L.asd_stage_fields_host.argtypes = [C.c_void_p, fp, fp, fp, fp]
+    L.asd_commit_fields.argtypes = [C.c_void_p]
     L.asd_step_heun.argtypes = [C.c_void_p, C.c_int64]
     L.asd_set_kernel.argtypes = [C.c_void_p, C.c_int32]
     L.asd_set_graph_mode.argtypes = [C.c_void_p, C.c_int32]
@@ -261,6 +267,23 @@ class Context:
         self._ck(self._L.asd_set_fields_host(self._h, _host_ptr(T, keep), _host_ptr(Bx, keep), _host_ptr(By, keep),
                                              _host_ptr(Bz, keep)))
         self._sync_if_unpinned(keep)
+
+    def stage_fields_host(self, T=None, Bx=None, By=None, Bz=None):
+        """asd_stage_fields_host (allocates the staging buffer on first use).  Pass PINNED torch tensors and keep them
+        alive and unchanged until commit_fields() has been called and the stream has passed it."""
+        import torch
+        if getattr(self, "_staging", None) is None:
+            nbytes = int(self._L.asd_staging_bytes(self._h))
+            self._staging = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            ptr = (self._staging.data_ptr() + 255) & ~255
+            self._ck(self._L.asd_set_staging(self._h, C.c_void_p(ptr), C.c_size_t(nbytes)))
+        keep = []
+        self._ck(self._L.asd_stage_fields_host(self._h, _host_ptr(T, keep), _host_ptr(Bx, keep), _host_ptr(By, keep),
+                                               _host_ptr(Bz, keep)))
+        self._staged_keep = keep
+
+    def commit_fields(self):
+        self._ck(self._L.asd_commit_fields(self._h))
 
     def _sync_if_unpinned(self, keep):
         import torch

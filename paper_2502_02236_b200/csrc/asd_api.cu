@@ -223,6 +223,7 @@ asd_status asd_destroy(asd_ctx* ctx) {
   if (ctx->c.host_scratch) cudaFreeHost(ctx->c.host_scratch);
   asd::tma_plan_free(ctx->c);
   asd::graphs_free(ctx->c);
+  if (ctx->c.copy_stream) { cudaStreamDestroy(ctx->c.copy_stream); cudaEventDestroy(ctx->c.staged_ev); cudaEventDestroy(ctx->c.consumed_ev); }
   asd::demag_free(ctx->c);
   delete ctx;
   return ASD_OK;
@@ -309,6 +310,56 @@ asd_status asd_set_fields(asd_ctx* ctx, const float* T, const float* Bx, const f
 asd_status asd_set_fields_host(asd_ctx* ctx, const float* T, const float* Bx, const float* By, const float* Bz) {
   CTX_OR_RETURN(ctx);
   return set_fields_impl(c, T, Bx, By, Bz, true);
+}
+
+size_t asd_staging_bytes(const asd_ctx* ctx) {
+  if (!ctx) return 0;
+  return 4 * align_up(sizeof(float) * (size_t)ctx->c.N, 256);
+}
+
+asd_status asd_set_staging(asd_ctx* ctx, void* d_staging, size_t bytes) {
+  CTX_OR_RETURN(ctx);
+  if (!d_staging || ((uintptr_t)d_staging & 255u)) return fail(c, ASD_EINVAL, "asd_set_staging: NULL or not 256-byte aligned");
+  if (bytes < asd_staging_bytes(ctx)) return fail(c, ASD_ENOMEM, "asd_set_staging: buffer too small");
+  if (!c.copy_stream) {
+    ASD_CUDA_TRY(c, cudaStreamCreateWithFlags(&c.copy_stream, cudaStreamNonBlocking));
+    ASD_CUDA_TRY(c, cudaEventCreateWithFlags(&c.staged_ev, cudaEventDisableTiming));
+    ASD_CUDA_TRY(c, cudaEventCreateWithFlags(&c.consumed_ev, cudaEventDisableTiming));
+  }
+  c.staging = (float*)d_staging;
+  c.staged_mask = 0;
+  return ASD_OK;
+}
+
+asd_status asd_stage_fields_host(asd_ctx* ctx, const float* T, const float* Bx, const float* By, const float* Bz) {
+  CTX_OR_RETURN(ctx);
+  if (!c.staging) return fail(c, ASD_ESTATE, "asd_stage_fields_host: asd_set_staging has not been called");
+  const size_t b = sizeof(float) * (size_t)c.N, pitch = align_up(b, 256) / sizeof(float);
+  // the previous commit's pack kernels must have read the staging area before it is overwritten
+  ASD_CUDA_TRY(c, cudaStreamWaitEvent(c.copy_stream, c.consumed_ev, 0));
+  const float* src[4] = {T, Bx, By, Bz};
+  for (int a = 0; a < 4; ++a) {
+    if (!src[a]) continue;
+    ASD_CUDA_TRY(c, cudaMemcpyAsync(c.staging + (size_t)a * pitch, src[a], b, cudaMemcpyHostToDevice, c.copy_stream));
+    c.staged_mask |= 1u << a;
+  }
+  ASD_CUDA_TRY(c, cudaEventRecord(c.staged_ev, c.copy_stream));
+  return ASD_OK;
+}
+
+asd_status asd_commit_fields(asd_ctx* ctx) {
+  CTX_OR_RETURN(ctx);
+  if (!c.staging) return fail(c, ASD_ESTATE, "asd_commit_fields: asd_set_staging has not been called");
+  if (!c.staged_mask) return ASD_OK;
+  const size_t pitch = align_up(sizeof(float) * (size_t)c.N, 256) / sizeof(float);
+  ASD_CUDA_TRY(c, cudaStreamWaitEvent(c.stream, c.staged_ev, 0));
+  const float* st = c.staging;
+  const asd_status r = set_fields_impl(c, (c.staged_mask & 1u) ? st : nullptr, (c.staged_mask & 2u) ? st + pitch : nullptr,
+                                       (c.staged_mask & 4u) ? st + 2 * pitch : nullptr,
+                                       (c.staged_mask & 8u) ? st + 3 * pitch : nullptr, false);
+  c.staged_mask = 0;
+  ASD_CUDA_TRY(c, cudaEventRecord(c.consumed_ev, c.stream));
+  return r;
 }
 
 asd_status asd_set_field_scale(asd_ctx* ctx, float s) {

@@ -166,6 +166,11 @@ struct Ctx {
   int32_t graph_mode = ASD_GRAPH_AUTO;
   cudaStream_t cap_stream = nullptr;   // internal stream the graphs are captured on (the caller's may be the legacy one)
   struct GraphCache* graphs = nullptr;
+  // double-buffered field upload (asd_stage_fields_host / asd_commit_fields): caller-owned staging of 4 dense arrays
+  float* staging = nullptr;
+  cudaStream_t copy_stream = nullptr;   // the H2D copies run here, beside the stage kernels on `stream`
+  cudaEvent_t staged_ev = nullptr, consumed_ev = nullptr;
+  uint32_t staged_mask = 0;             // bit a: array a (T, Bx, By, Bz) was staged and awaits asd_commit_fields
   DemagPlan* demag = nullptr;       // non-null once asd_enable_demag succeeded
   int32_t demag_every = 0;          // 0: field recomputed in every stage; P >= 1: from S at every P-th Heun step, held in between
   int64_t demag_age = 0;            // Heun steps since the held field was last invalidated (enable, shift, set_spins)

@@ -113,3 +113,23 @@ def test_option_and_demag_errors():
     gp = gpu_from_workload(p)
     with pytest.raises(asd.AsdError):
         gp.enable_demag([0.3e-9] * 3)
+
+
+def test_staged_field_upload_equals_the_direct_one():
+    """asd_stage_fields_host + asd_commit_fields (double-buffered upload) must leave exactly the state asd_set_fields_host
+    does, including 'NULL = keep', a re-stage while steps are in flight, and a commit with nothing staged."""
+    import torch
+    w = ai.small_film(ai.L10, 16, 24, 5, tilt_deg=20.0)
+    a, b = gpu_from_workload(w), gpu_from_workload(w)
+    pin = lambda x: torch.from_numpy(np.ascontiguousarray(x, dtype=np.float32)).pin_memory()
+    rng = np.random.default_rng(1)
+    T2, Bz2 = pin(w.T * 1.3 + 5.0), pin(rng.standard_normal(w.n_sites))
+    T3, Bx3 = pin(w.T * 0.5), pin(rng.standard_normal(w.n_sites))
+    a.set_fields_host(T=T2, Bz=Bz2); a.step_heun(3)
+    a.set_fields_host(T=T3, Bx=Bx3); a.step_heun(2)
+
+    b.stage_fields_host(T=T2, Bz=Bz2); b.commit_fields(); b.step_heun(3)
+    b.stage_fields_host(T=T3, Bx=Bx3)                      # copied while the 3 steps above run
+    b.commit_fields(); b.commit_fields()                   # the second commit has nothing to do
+    b.step_heun(2)
+    assert np.array_equal(a.get_spins_host(), b.get_spins_host())
