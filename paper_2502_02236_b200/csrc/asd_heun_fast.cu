@@ -82,6 +82,9 @@ __global__ void __launch_bounds__(NT, MINB) heun_stage_fast(const FastParams p) 
         asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p.arrays + (off + eb)), "r"(bytes) : "memory");
     }
   }
+  // Programmatic dependent launch: this grid may be scheduled while the previous kernel of the stream drains; nothing
+  // above or below this line up to the wait touches memory that kernel writes (the prefetch only moves lines into L2).
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   const uint32_t t = blockIdx.x * NT + threadIdx.x;
   if (t >= p.nthreads) return;
   const uint32_t r = fastdiv(t, p.m_grp, p.s_grp);
@@ -98,6 +101,7 @@ __global__ void __launch_bounds__(NT, MINB) heun_stage_fast(const FastParams p) 
 
   // every address below is arrays + (one 32-bit element index): a single widening multiply-add per access
   const float* __restrict__ base = p.arrays;
+  asm volatile("griddepcontrol.wait;" ::: "memory");           // the previous kernel's stores are complete and visible
 
   // ---- exchange field, Eq. (2): shell sums first, one multiply per shell ----
   float own[3][6];                // own row with its y-1 and y+1 edge sites
@@ -211,6 +215,19 @@ __global__ void __launch_bounds__(NT, MINB) heun_stage_fast(const FastParams p) 
 }
 
 
+// Launch with programmatic stream serialization: the grid may start before its predecessor has finished and
+// synchronises with it at its own griddepcontrol.wait.
+inline void launch_pdl(void (*kern)(const FastParams), unsigned blocks, unsigned threads, cudaStream_t stream,
+                       const FastParams& f) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(blocks); cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = 0; cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  cudaLaunchKernelEx(&cfg, kern, f);
+}
+
 template <int LAT, bool DEMAG, int NT = 128, int MINB = 5>
 asd_status launch_pair_fast(Ctx& c, FastParams& f) {
   const unsigned blocks = (f.nthreads + NT - 1u) / NT;
@@ -218,11 +235,11 @@ asd_status launch_pair_fast(Ctx& c, FastParams& f) {
   const uint32_t as = f.as;
   f.oX = (uint32_t)c.aS * as; f.oOut = (uint32_t)c.aSt * as; f.oOutA = AR_A * as; f.oA = AR_A * as;
   if (DEMAG && (c.demag_refresh & 1)) { const asd_status st = launch_demag(c, c.aS); if (st != ASD_OK) return st; }
-  heun_stage_fast<LAT, 0, NT, MINB, DEMAG><<<blocks, NT, 0, c.launch_stream>>>(f);
+  launch_pdl(heun_stage_fast<LAT, 0, NT, MINB, DEMAG>, blocks, NT, c.launch_stream, f);
   ASD_LAUNCH_CHECK(c, "heun predictor (fast)");
   f.oX = (uint32_t)c.aSt * as; f.oOut = (uint32_t)c.aS * as;
   if (DEMAG && (c.demag_refresh & 2)) { const asd_status st = launch_demag(c, c.aSt); if (st != ASD_OK) return st; }
-  heun_stage_fast<LAT, 1, NT, MINB, DEMAG><<<blocks, NT, 0, c.launch_stream>>>(f);
+  launch_pdl(heun_stage_fast<LAT, 1, NT, MINB, DEMAG>, blocks, NT, c.launch_stream, f);
   ASD_LAUNCH_CHECK(c, "heun corrector (fast)");
   return ASD_OK;
 }
