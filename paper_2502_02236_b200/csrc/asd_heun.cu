@@ -58,6 +58,8 @@ __device__ __forceinline__ void load_row(const float* X, uint32_t as, int64_t ba
 
 template <int VEC, int LAT, int STAGE, bool DEMAG>
 __global__ void __launch_bounds__(256) heun_stage_general(const StageParams p) {
+  // programmatic dependent launch (see launch_pdl): only the read-only column table is touched before the wait
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= p.nthreads) return;
   const int r = (int)(t / p.ngrp);
@@ -75,6 +77,7 @@ __global__ void __launch_bounds__(256) heun_stage_general(const StageParams p) {
   bool any = false;
 #pragma unroll
   for (int v = 0; v < VEC; ++v) any |= (col[v] & 0xFFFFu) != 0u;
+  asm volatile("griddepcontrol.wait;" ::: "memory");             // the previous kernel's stores are complete and visible
   float o[3][VEC], oA[3][VEC];
   if (!any) {                                    // all vacant: keep the buffers zero there
 #pragma unroll
@@ -232,12 +235,12 @@ asd_status launch_pair_d(Ctx& c, StageParams& p) {
   // predictor: X = S -> out = S~, outA = A
   p.aX = c.aS; p.aOut = c.aSt; p.aOutA = AR_A; p.aA = AR_A;
   if (DEMAG && (c.demag_refresh & 1)) { const asd_status st = launch_demag(c, c.aS); if (st != ASD_OK) return st; }
-  heun_stage_general<VEC, LAT, 0, DEMAG><<<blocks, threads, 0, c.launch_stream>>>(p);
+  launch_pdl(heun_stage_general<VEC, LAT, 0, DEMAG>, blocks, threads, c.launch_stream, p, c.launch_stream == c.stream);
   ASD_LAUNCH_CHECK(c, "heun predictor");
   // corrector: X = S~, A -> out = S
   p.aX = c.aSt; p.aOut = c.aS;
   if (DEMAG && (c.demag_refresh & 2)) { const asd_status st = launch_demag(c, c.aSt); if (st != ASD_OK) return st; }
-  heun_stage_general<VEC, LAT, 1, DEMAG><<<blocks, threads, 0, c.launch_stream>>>(p);
+  launch_pdl(heun_stage_general<VEC, LAT, 1, DEMAG>, blocks, threads, c.launch_stream, p, c.launch_stream == c.stream);
   ASD_LAUNCH_CHECK(c, "heun corrector");
   return ASD_OK;
 }

@@ -215,19 +215,6 @@ __global__ void __launch_bounds__(NT, MINB) heun_stage_fast(const FastParams p) 
 }
 
 
-// Launch with programmatic stream serialization: the grid may start before its predecessor has finished and
-// synchronises with it at its own griddepcontrol.wait.
-inline void launch_pdl(void (*kern)(const FastParams), unsigned blocks, unsigned threads, cudaStream_t stream,
-                       const FastParams& f) {
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(blocks); cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = 0; cfg.stream = stream;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = attr; cfg.numAttrs = 1;
-  cudaLaunchKernelEx(&cfg, kern, f);
-}
-
 template <int LAT, bool DEMAG, int NT = 128, int MINB = 5>
 asd_status launch_pair_fast(Ctx& c, FastParams& f) {
   const unsigned blocks = (f.nthreads + NT - 1u) / NT;
@@ -235,11 +222,11 @@ asd_status launch_pair_fast(Ctx& c, FastParams& f) {
   const uint32_t as = f.as;
   f.oX = (uint32_t)c.aS * as; f.oOut = (uint32_t)c.aSt * as; f.oOutA = AR_A * as; f.oA = AR_A * as;
   if (DEMAG && (c.demag_refresh & 1)) { const asd_status st = launch_demag(c, c.aS); if (st != ASD_OK) return st; }
-  launch_pdl(heun_stage_fast<LAT, 0, NT, MINB, DEMAG>, blocks, NT, c.launch_stream, f);
+  launch_pdl(heun_stage_fast<LAT, 0, NT, MINB, DEMAG>, blocks, NT, c.launch_stream, f, c.launch_stream == c.stream);
   ASD_LAUNCH_CHECK(c, "heun predictor (fast)");
   f.oX = (uint32_t)c.aSt * as; f.oOut = (uint32_t)c.aS * as;
   if (DEMAG && (c.demag_refresh & 2)) { const asd_status st = launch_demag(c, c.aSt); if (st != ASD_OK) return st; }
-  launch_pdl(heun_stage_fast<LAT, 1, NT, MINB, DEMAG>, blocks, NT, c.launch_stream, f);
+  launch_pdl(heun_stage_fast<LAT, 1, NT, MINB, DEMAG>, blocks, NT, c.launch_stream, f, c.launch_stream == c.stream);
   ASD_LAUNCH_CHECK(c, "heun corrector (fast)");
   return ASD_OK;
 }

@@ -251,4 +251,22 @@ asd_status fail_cuda(Ctx& c, cudaError_t e, const char* where);
 
 }  // namespace asd
 
+#ifdef __CUDACC__
+namespace asd {
+// Launch with programmatic stream serialization (programmatic dependent launch): the grid may be scheduled before its
+// predecessor in the stream has finished and synchronises with it at its own griddepcontrol.wait.
+template <class Params>
+inline void launch_pdl(void (*kern)(const Params), unsigned blocks, unsigned threads, cudaStream_t stream, const Params& p,
+                       bool allow = true) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(blocks); cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = 0; cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = allow ? 1 : 0;             // recorded graphs keep plain edges (measured faster there)
+  cudaLaunchKernelEx(&cfg, kern, p);
+}
+}  // namespace asd
+#endif
+
 struct asd_ctx { asd::Ctx c; };
