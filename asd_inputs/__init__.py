@@ -11,6 +11,7 @@ the paper's own track realisation is not available.  The recipes are BASELINE.js
 with the readings Q7-Q13 of SURVEY.md section 8(c), restated in DESIGN.md section 4.
 """
 from .workloads import (  # noqa: F401
+    shell_ell_table,
     GAMMA_E, MU_B, K_B, SC, L10, Workload, voronoi_grain_map, laser_temperature, tilted_spins,
     make_config, small_film, ShiftSchedule, planes_for_shift, nrz_bits, field_scale_at,
 )

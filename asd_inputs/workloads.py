@@ -222,6 +222,34 @@ def small_film(lattice: int, nx: int, ny: int, nz: int, extra_track: int = 0, pi
     return w
 
 
+def shell_ell_table(w: "Workload"):
+    """The built-in neighbour shells of `w` written out as a general ELL table (window-local site indices, -1 = no
+    neighbour; exchange energy per pair in Joule): SC 6 nearest neighbours (J[0]); L1_0 4 in-plane nn (J[0]), 2
+    out-of-plane (J[1]), 4 in-plane diagonals (J[2]).  Open boundaries; a bond exists only between magnetic sites of the
+    SAME grain.  Pure indexing -- this is the data an external ELL user would hand to asd_create_lattice."""
+    nx, ny, nz = w.nx, w.ny, w.nz
+    if w.lattice == SC:
+        offs = [(1, 0, 0, 0), (-1, 0, 0, 0), (0, 1, 0, 0), (0, -1, 0, 0), (0, 0, 1, 0), (0, 0, -1, 0)]
+    else:
+        offs = [(1, 0, 0, 0), (-1, 0, 0, 0), (0, 1, 0, 0), (0, -1, 0, 0), (0, 0, 1, 1), (0, 0, -1, 1),
+                (1, 1, 0, 2), (1, -1, 0, 2), (-1, 1, 0, 2), (-1, -1, 0, 2)]
+    gm = np.asarray(w.grain_map)[w.x0:w.x0 + nx]                         # [nx, ny]
+    g3 = np.broadcast_to(gm[:, None, :], (nx, nz, ny))                   # site order (i, k, j)
+    i, k, j = np.meshgrid(np.arange(nx), np.arange(nz), np.arange(ny), indexing="ij")
+    idx = np.full((nx * ny * nz, len(offs)), -1, dtype=np.int32)
+    J = np.zeros((nx * ny * nz, len(offs)), dtype=np.float32)
+    for s, (dx, dy, dz, shell) in enumerate(offs):
+        i2, j2, k2 = i + dx, j + dy, k + dz
+        ok = (i2 >= 0) & (i2 < nx) & (j2 >= 0) & (j2 < ny) & (k2 >= 0) & (k2 < nz)
+        i2c, j2c, k2c = np.clip(i2, 0, nx - 1), np.clip(j2, 0, ny - 1), np.clip(k2, 0, nz - 1)
+        gn = gm[i2c, j2c]
+        ok &= (g3 >= 0) & (gn == g3)
+        n = (i2c * nz + k2c) * ny + j2c
+        idx[:, s] = np.where(ok, n, -1).reshape(-1)
+        J[:, s] = np.where(ok, w.J[shell], 0.0).reshape(-1)
+    return idx, J
+
+
 # ----------------------------------------------------------------------------------------------
 # Drive schedule (SURVEY 8(c) Q8, S1): integer planes per shift from a travel accumulator, a seeded
 # NRZ bit pattern, and the head-field scale s(t) ramped linearly over one bit period.

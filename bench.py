@@ -126,9 +126,10 @@ def reduce_over_ranks(ms_local: float, updates_local: float, dist=None, device="
     return float(t.item()), float(u.item())
 
 
-def _gpu_desc(asd, w: ai.Workload):
+def _gpu_desc(asd, w: ai.Workload, ell=None):
     """Workload -> asd.LatticeDesc (argument marshalling; the product path never imports oracle/ or tests/)."""
-    return asd.LatticeDesc(lattice=w.lattice, nx=w.nx, ny=w.ny, nz=w.nz, pbc=w.pbc, mu_s=w.mu_s, lam=w.lam,
+    extra = {} if ell is None else {"ell_idx": ell[0], "ell_J": ell[1]}
+    return asd.LatticeDesc(**extra, lattice=w.lattice, nx=w.nx, ny=w.ny, nz=w.nz, pbc=w.pbc, mu_s=w.mu_s, lam=w.lam,
                            gamma=w.gamma, dt=w.dt, J=w.J, track_nx=w.track_nx, x0=w.x0, grain_map=w.grain_map,
                            n_grains=w.n_grains, grain_ku=w.grain_ku, grain_axis=w.grain_axis, macro=w.macro,
                            seed=w.seed)
@@ -173,7 +174,14 @@ def run_ours(args):
 
     w = _workload(args.config, seed_offset=rank)
     N = w.n_sites
-    ctx = asd.Context(_gpu_desc(asd, w), device=f"cuda:{local}")
+    ell = None
+    if args.ell:
+        # the same exchange bonds handed over as a general ELL table (per-pair J); such a table cannot follow the
+        # window, so this variant runs without shifts
+        ell = ai.shell_ell_table(w)
+        w.shift_every = 0
+    ell_w = 0 if ell is None else int(ell[0].shape[1])
+    ctx = asd.Context(_gpu_desc(asd, w, ell), device=f"cuda:{local}")
     dev = ctx.device
     if args.demag:
         ctx.enable_demag([a * 1e-9 for a in w.spacing_nm])
@@ -258,19 +266,21 @@ def run_ours(args):
     peak, peak_src = _peaks()
     n_stage_launches = 2 * hps * len(heun_events)
     avg_launch_s = heun_ms * 1e-3 / n_stage_launches
-    alg_bytes = BYTES_PER_SITE_PER_STAGE * N
+    # a general ELL table adds its own compulsory bytes: int32 index + fp32 J per slot per site per stage
+    alg_bytes = (BYTES_PER_SITE_PER_STAGE + 8.0 * ell_w) * N
     achieved = alg_bytes / avg_launch_s / 1e9
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": w.name, "sites": N, "heun_steps_per_step": hps, "shifts_in_timed_region": shifts,
-                   "shift_every_heun_steps": w.shift_every, "dt": w.dt, "parallelism": f"replicas x{world}", "demag": bool(args.demag), "demag_every": args.demag_every if args.demag else None,
+                   "shift_every_heun_steps": w.shift_every, "dt": w.dt, "parallelism": f"replicas x{world}", "ell_width": ell_w, "demag": bool(args.demag), "demag_every": args.demag_every if args.demag else None,
                    "l2": "working set (13 fp32 arrays/site = %.0f MB) exceeds the 126 MB L2" % (13 * 4 * N / 1e6)},
         "clocks": clocks, "gpu_launches": int(launches),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 16 * N, "d2h_bytes_per_step": 32,
                 "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps, "wall_ms_per_step": wall_ms / e2e_steps},
-        "roofline": {"bound": "hbm", "kernel": "heun_stage_fast (predictor+corrector, 52 B/site each)",
+        "roofline": {"bound": "hbm", "kernel": ("heun_stage_general<ELL> (predictor+corrector, %d B/site each)" % (52 + 8 * ell_w)) if ell_w else
+                     "heun_stage_fast (predictor+corrector, 52 B/site each)",
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "peak_source": peak_src, "avg_launch_us": avg_launch_s * 1e6,
                      "algorithmic_bytes_per_launch": alg_bytes, "traffic": _traffic(w.name)},
@@ -356,6 +366,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=20)
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ell", action="store_true",
+                    help="hand the exchange bonds over as a general ELL neighbour table with per-pair J (no window shifts)")
     ap.add_argument("--demag", action="store_true",
                     help="switch the demagnetising field on (Eq. (6)-(7): coarse-graining + FFT convolution per stage)")
     ap.add_argument("--demag-every", type=int, default=0,

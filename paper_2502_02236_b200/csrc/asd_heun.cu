@@ -300,7 +300,8 @@ asd_status launch_heun_direct(Ctx& c, int64_t n, const DynState* dyn) {
     asd_status st;
     if (staged) st = launch_heun_tma(c, p);
     else if (fast) st = launch_heun_fast(c, p);
-    else if (c.d.ell_width > 0) st = launch_pair<1, LAT_ELL>(c, p);
+    else if (c.d.ell_width > 0) st = (c.kernel_variant != ASD_KERNEL_GENERAL && heun_ell_supported(c)) ? launch_heun_ell(c, p)
+                                                                                                     : launch_pair<1, LAT_ELL>(c, p);
     else if (c.d.lattice == ASD_SC) st = vec4 ? launch_pair<4, LAT_SC>(c, p) : launch_pair<1, LAT_SC>(c, p);
     else st = vec4 ? launch_pair<4, LAT_L10>(c, p) : launch_pair<1, LAT_L10>(c, p);
     if (st != ASD_OK) return st;

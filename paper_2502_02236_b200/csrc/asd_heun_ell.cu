@@ -1,0 +1,159 @@
+// asd_heun_ell.cu -- the hot path for a general ELL neighbour table with per-pair J (BASELINE north_star: "the L1_0 path
+// uses an ELL neighbour table with per-pair J"): one fused kernel per stochastic-Heun stage.
+//
+//   B_ex,i = sum_s (J_is / mu_s) X_{n(i,s)},   s = 0 .. W-1,   n(i,s) = -1: no neighbour in that slot
+//
+// The table is slot-major (idx int32[W][N], J/mu_s fp32[W][N], entries = padded element offsets), so with ONE site per
+// thread every table read is a coalesced 128-byte sweep per warp and every neighbour gather of adjacent sites lands on
+// adjacent (or the same few) cache lines.  All slots of a chunk are loaded before any is used (memory-level parallelism
+// without a dependent chain per slot); a missing neighbour is folded in branch-free (its J becomes 0, its index the site
+// itself).  The table, sigma, B (and A) are pure streams: a bulk L2 prefetch runs a third of a wave ahead exactly as in
+// the film kernel, and the kernels are launched with programmatic dependent launch.
+//
+// Bytes per site per stage that must come from / go to HBM: 52 + 8 W: 132 for the 10-neighbour L1_0
+// shells.  Boundaries, vacancies, grain decoupling and periodic wraps all live in the table; the kernel knows none of it.
+#include "asd_internal.cuh"
+#include "asd_site.cuh"
+
+namespace asd {
+
+namespace {
+
+constexpr int kEllThreads = 256;
+constexpr int kEllChunk = 5;                 // slots loaded together (W = 10: two chunks).  Measured on cfg4 (us per stage):
+                                             // 5 x 256 threads x 4 CTAs/SM 151.2; 10 x 256 x 4 153.3; 5 x 128 x 8 156.1; 5 x 256 x 6 156.4
+constexpr uint32_t kEllPrefetchAhead = 148;  // CTAs: a third of a wave, as in the film kernel
+
+struct EllParams {
+  const float* arrays;
+  float* arrays_w;
+  uint32_t as;
+  uint32_t oX, oA, oOut, oOutA, oSigma, oB;
+  const int32_t* idx;              // [W][N] padded element offsets, -1 = none
+  const float* Jt;                 // [W][N] J / mu_s, Tesla
+  int32_t W;
+  uint32_t N, ny, nyp, lead, nz;
+  uint32_t m_ny, s_ny, m_nz, s_nz; // multiply-high constants: l / ny and r / nz
+  const uint32_t* col;             // column table at the window origin (grain id + 1 in the low 16 bits)
+  const float4* grain;             // (e_x, e_y, e_z, 2 k_u/mu_s) per grain id + 1
+  float gdt, lambda, scale;
+  uint32_t n_lo, n_hi;
+  const DynState* dyn;
+  uint64_t g0;
+  PhiloxKey key;
+};
+
+template <int STAGE>
+__global__ void __launch_bounds__(kEllThreads, 4) heun_stage_ell(const EllParams p) {
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  // ---- L2 prefetch of the streams of the CTA that runs kEllPrefetchAhead blocks later: W index rows, W J rows ----
+  {
+    const uint32_t lb = (blockIdx.x + kEllPrefetchAhead) * (uint32_t)kEllThreads;
+    if (threadIdx.x < 2u * (uint32_t)p.W && lb < p.N) {
+      const uint32_t s = threadIdx.x >> 1;
+      const void* src = (threadIdx.x & 1u) ? (const void*)(p.Jt + (size_t)s * p.N + lb) : (const void*)(p.idx + (size_t)s * p.N + lb);
+      const uint32_t room = p.N - lb;
+      const uint32_t bytes = ((room < (uint32_t)kEllThreads ? room : (uint32_t)kEllThreads) * 4u) & ~15u;
+      if (bytes && (((uintptr_t)src) & 15u) == 0u)
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+    }
+  }
+  const uint32_t l = blockIdx.x * (uint32_t)kEllThreads + threadIdx.x;      // dense window-local site
+  if (l >= p.N) return;
+  const uint32_t r = div_u31(l, p.m_ny, p.s_ny);                            // row (i * nz + k)
+  const uint32_t j = l - r * p.ny;
+  const uint32_t i = div_u31(r, p.m_nz, p.s_nz);
+  const uint32_t e = p.lead + r * p.nyp + j;                                // padded element of the site
+  const float* __restrict__ base = p.arrays;
+  const uint32_t gid = __ldg(p.col + (i * p.ny + j)) & 0xFFFFu;             // read-only table: before the wait
+  const float4 gp = __ldg(p.grain + gid);
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+
+  // ---- own spin and streamed inputs ----
+  const float X0 = __ldg(base + (p.oX + e)), X1 = __ldg(base + (p.oX + p.as + e)), X2 = __ldg(base + (p.oX + 2u * p.as + e));
+  const float sg = __ldg(base + (p.oSigma + e));
+  const float Bap[3] = {__ldg(base + (p.oB + e)), __ldg(base + (p.oB + p.as + e)), __ldg(base + (p.oB + 2u * p.as + e))};
+  float Ai[3] = {0.0f, 0.0f, 0.0f};
+  if (STAGE == 1) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) Ai[c] = __ldg(base + (p.oA + (uint32_t)c * p.as + e));
+  }
+
+  // ---- exchange field: chunks of kEllChunk slots, table first, then the gathers, then the sums ----
+  float Be[3] = {0.0f, 0.0f, 0.0f};
+  for (int s0 = 0; s0 < p.W; s0 += kEllChunk) {
+    int32_t n[kEllChunk];
+    float Jt[kEllChunk];
+#pragma unroll
+    for (int u = 0; u < kEllChunk; ++u) {
+      const bool in = s0 + u < p.W;
+      const size_t q = (size_t)(in ? s0 + u : s0) * p.N + l;
+      n[u] = __ldg(p.idx + q);
+      Jt[u] = in ? __ldg(p.Jt + q) : 0.0f;
+    }
+    float nb[kEllChunk][3];
+#pragma unroll
+    for (int u = 0; u < kEllChunk; ++u) {
+      const bool ok = n[u] >= 0;
+      const uint32_t en = ok ? (uint32_t)n[u] : e;              // a missing neighbour reads the site itself, times J = 0
+      Jt[u] = ok ? Jt[u] : 0.0f;
+#pragma unroll
+      for (int c = 0; c < 3; ++c) nb[u][c] = __ldg(base + (p.oX + (uint32_t)c * p.as + en));
+    }
+#pragma unroll
+    for (int u = 0; u < kEllChunk; ++u)
+#pragma unroll
+      for (int c = 0; c < 3; ++c) Be[c] = fmaf(Jt[u], nb[u][c], Be[c]);
+  }
+
+  // ---- noise, torque, update, renormalise ----
+  uint32_t n_lo = p.n_lo, n_hi = p.n_hi; float scale = p.scale;
+  resolve_dyn(p.dyn, n_lo, n_hi, scale);
+  const SiteConst sc{p.gdt, p.lambda, scale};
+  uint32_t rnd[4];
+  philox_site(p.key, n_lo, n_hi, p.g0 + (uint64_t)l, 0u, rnd);
+  float xi[3];
+  normals3(rnd, xi);
+  const float Xs[3] = {X0, X1, X2};
+  float ov[3], oAv[3];
+  site_update<STAGE>(sc, Xs, Be, gp, Bap, sg, xi, Ai, ov, oAv);
+#pragma unroll
+  for (int c = 0; c < 3; ++c) p.arrays_w[p.oOut + (uint32_t)c * p.as + e] = ov[c];
+  if (STAGE == 0) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) p.arrays_w[p.oOutA + (uint32_t)c * p.as + e] = oAv[c];
+  }
+}
+
+}  // namespace
+
+// The dedicated ELL kernel needs 32-bit element offsets and dense site ids; everything else lives in the table.
+bool heun_ell_supported(const Ctx& c) {
+  return c.d.ell_width > 0 && (int64_t)AR_COUNT * c.as < (1ll << 31) && c.N < (1ll << 31) &&
+         c.d.track_nx * (int64_t)c.d.ny < (1ll << 30);
+}
+
+asd_status launch_heun_ell(Ctx& c, StageParams& p) {
+  EllParams f;
+  f.arrays = c.arrays; f.arrays_w = c.arrays; f.as = (uint32_t)c.as;
+  f.oSigma = AR_SIGMA * f.as; f.oB = AR_B * f.as;
+  f.idx = c.ell_idx; f.Jt = c.ell_J; f.W = c.d.ell_width;
+  f.N = (uint32_t)c.N; f.ny = (uint32_t)c.d.ny; f.nyp = (uint32_t)c.nyp; f.lead = (uint32_t)c.lead; f.nz = (uint32_t)c.d.nz;
+  magic_u31(f.ny, f.m_ny, f.s_ny);
+  magic_u31(f.nz, f.m_nz, f.s_nz);
+  f.col = p.col; f.grain = p.grain;
+  f.gdt = p.gdt; f.lambda = p.lambda; f.scale = p.scale;
+  f.n_lo = p.n_lo; f.n_hi = p.n_hi; f.dyn = p.dyn; f.g0 = p.g0; f.key = p.key;
+  const unsigned blocks = (unsigned)((c.N + kEllThreads - 1) / kEllThreads);
+  const uint32_t as = f.as;
+  const bool pdl = c.launch_stream == c.stream;
+  f.oX = (uint32_t)c.aS * as; f.oOut = (uint32_t)c.aSt * as; f.oOutA = AR_A * as; f.oA = AR_A * as;
+  launch_pdl(heun_stage_ell<0>, blocks, kEllThreads, c.launch_stream, f, pdl);
+  ASD_LAUNCH_CHECK(c, "heun predictor (ell)");
+  f.oX = (uint32_t)c.aSt * as; f.oOut = (uint32_t)c.aS * as;
+  launch_pdl(heun_stage_ell<1>, blocks, kEllThreads, c.launch_stream, f, pdl);
+  ASD_LAUNCH_CHECK(c, "heun corrector (ell)");
+  return ASD_OK;
+}
+
+}  // namespace asd

@@ -225,6 +225,8 @@ void demag_fill_params(const Ctx& c, StageParams& p);
 asd_status demag_field_host(Ctx& c, float* out, int64_t dims[3]);
 asd_status launch_heun_fast(Ctx& c, StageParams& p);          // one Heun step (2 kernels), fast path
 bool heun_fast_supported(const Ctx& c);
+asd_status launch_heun_ell(Ctx& c, StageParams& p);           // one Heun step (2 kernels), general ELL table
+bool heun_ell_supported(const Ctx& c);
 asd_status launch_heun_tma(Ctx& c, StageParams& p);           // one Heun step (2 kernels), TMA-staged film path
 bool heun_tma_supported(const Ctx& c);
 TmaPlan* tma_plan(Ctx& c);                                    // nullptr if the plan cannot be built

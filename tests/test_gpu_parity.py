@@ -83,6 +83,25 @@ def test_adjacent_grains_and_periodic_boundaries(lattice, pbc, dims):
     _check_norm(g, w)
 
 
+@pytest.mark.parametrize("kernel", ["auto", "general"])
+@pytest.mark.parametrize("lattice", [ai.SC, ai.L10])
+def test_shell_table_as_ell(lattice, kernel):
+    """The built-in shells handed over as an ELL table (asd_inputs.shell_ell_table): the dedicated ELL kernel
+    (asd_heun_ell.cu, what AUTO runs) and the general kernel against the oracle driven by the same table."""
+    import paper_2502_02236_b200 as asd
+    w = ai.small_film(lattice, 21, 38, 7, tilt_deg=25.0, dt=1e-16)
+    idx, J = ai.shell_ell_table(w)
+    o = oracle_from_workload(w, ell_idx=idx, ell_J=J.astype(np.float64))
+    g = gpu_from_workload(w, ell_idx=idx, ell_J=J)
+    if kernel == "general":
+        g.set_kernel(asd.KERNEL_GENERAL)
+    o.step_heun(1); g.step_heun(1)
+    assert max_abs_diff(g, o) <= TOL_1STEP
+    o.step_heun(4); g.step_heun(4)
+    assert max_abs_diff(g, o) <= 5e-5
+    _check_norm(g, w)
+
+
 def test_general_ell_table():
     """User-supplied neighbour table with arbitrary per-pair J (random sparse couplings)."""
     nx, ny, nz = 7, 12, 4
