@@ -6,12 +6,14 @@
 // The table is slot-major (idx int32[W][N], J/mu_s fp32[W][N], entries = padded element offsets), so with ONE site per
 // thread every table read is a coalesced 128-byte sweep per warp and every neighbour gather of adjacent sites lands on
 // adjacent (or the same few) cache lines.  All slots of a chunk are loaded before any is used (memory-level parallelism
-// without a dependent chain per slot); a missing neighbour is folded in branch-free (its J becomes 0, its index the site
-// itself).  The table, sigma, B (and A) are pure streams: a bulk L2 prefetch runs a third of a wave ahead exactly as in
+// without a dependent chain per slot); an empty slot is stored at set-up as (the site itself, J = 0), so the kernel has
+// neither a test nor a select per slot.  The table, sigma, B (and A) are pure streams: a bulk L2 prefetch runs a third of a wave ahead exactly as in
 // the film kernel, and the kernels are launched with programmatic dependent launch.
 //
 // Bytes per site per stage that must come from / go to HBM: 52 + 8 W: 132 for the 10-neighbour L1_0
 // shells.  Boundaries, vacancies, grain decoupling and periodic wraps all live in the table; the kernel knows none of it.
+#include <type_traits>
+
 #include "asd_internal.cuh"
 #include "asd_site.cuh"
 
@@ -43,13 +45,15 @@ struct EllParams {
   PhiloxKey key;
 };
 
-template <int STAGE>
+// WT = table width known at compile time (6: simple cubic, 10: the L1_0 shells), or 0 = read it from the parameters.
+template <int STAGE, int WT>
 __global__ void __launch_bounds__(kEllThreads, 4) heun_stage_ell(const EllParams p) {
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  const int W = WT > 0 ? WT : p.W;
   // ---- L2 prefetch of the streams of the CTA that runs kEllPrefetchAhead blocks later: W index rows, W J rows ----
   {
     const uint32_t lb = (blockIdx.x + kEllPrefetchAhead) * (uint32_t)kEllThreads;
-    if (threadIdx.x < 2u * (uint32_t)p.W && lb < p.N) {
+    if (threadIdx.x < 2u * (uint32_t)W && lb < p.N) {
       const uint32_t s = threadIdx.x >> 1;
       const void* src = (threadIdx.x & 1u) ? (const void*)(p.Jt + (size_t)s * p.N + lb) : (const void*)(p.idx + (size_t)s * p.N + lb);
       const uint32_t room = p.N - lb;
@@ -64,46 +68,54 @@ __global__ void __launch_bounds__(kEllThreads, 4) heun_stage_ell(const EllParams
   const uint32_t j = l - r * p.ny;
   const uint32_t i = div_u31(r, p.m_nz, p.s_nz);
   const uint32_t e = p.lead + r * p.nyp + j;                                // padded element of the site
-  const float* __restrict__ base = p.arrays;
   const uint32_t gid = __ldg(p.col + (i * p.ny + j)) & 0xFFFFu;             // read-only table: before the wait
   const float4 gp = __ldg(p.grain + gid);
   asm volatile("griddepcontrol.wait;" ::: "memory");
 
+  // component bases of the configuration read through the table, and the thread's place in each stream
+  const float* __restrict__ Xc0 = p.arrays + p.oX;
+  const float* __restrict__ Xc1 = Xc0 + p.as;
+  const float* __restrict__ Xc2 = Xc1 + p.as;
+  const float* __restrict__ own = p.arrays + e;
+
   // ---- own spin and streamed inputs ----
-  const float X0 = __ldg(base + (p.oX + e)), X1 = __ldg(base + (p.oX + p.as + e)), X2 = __ldg(base + (p.oX + 2u * p.as + e));
-  const float sg = __ldg(base + (p.oSigma + e));
-  const float Bap[3] = {__ldg(base + (p.oB + e)), __ldg(base + (p.oB + p.as + e)), __ldg(base + (p.oB + 2u * p.as + e))};
+  const float X0 = __ldg(Xc0 + e), X1 = __ldg(Xc1 + e), X2 = __ldg(Xc2 + e);
+  const float sg = __ldg(own + p.oSigma);
+  const float Bap[3] = {__ldg(own + p.oB), __ldg(own + (p.oB + p.as)), __ldg(own + (p.oB + 2u * p.as))};
   float Ai[3] = {0.0f, 0.0f, 0.0f};
   if (STAGE == 1) {
 #pragma unroll
-    for (int c = 0; c < 3; ++c) Ai[c] = __ldg(base + (p.oA + (uint32_t)c * p.as + e));
+    for (int c = 0; c < 3; ++c) Ai[c] = __ldg(own + (p.oA + (uint32_t)c * p.as));
   }
 
-  // ---- exchange field: chunks of kEllChunk slots, table first, then the gathers, then the sums ----
+  // ---- exchange field: chunks of kEllChunk slots, table first, then the gathers, then the sums.  Empty slots were
+  // stored at set-up as (the site itself, J = 0): no test, no select. ----
   float Be[3] = {0.0f, 0.0f, 0.0f};
-  for (int s0 = 0; s0 < p.W; s0 += kEllChunk) {
-    int32_t n[kEllChunk];
-    float Jt[kEllChunk];
+  const int32_t* __restrict__ pi = p.idx + l;
+  const float* __restrict__ pj = p.Jt + l;
+  auto chunk = [&](auto count) {
+    constexpr int C = decltype(count)::value;
+    uint32_t n[C];
+    float Jt[C];
 #pragma unroll
-    for (int u = 0; u < kEllChunk; ++u) {
-      const bool in = s0 + u < p.W;
-      const size_t q = (size_t)(in ? s0 + u : s0) * p.N + l;
-      n[u] = __ldg(p.idx + q);
-      Jt[u] = in ? __ldg(p.Jt + q) : 0.0f;
-    }
-    float nb[kEllChunk][3];
+    for (int u = 0; u < C; ++u) { n[u] = (uint32_t)__ldg(pi); Jt[u] = __ldg(pj); pi += p.N; pj += p.N; }
+    float nb[C][3];
 #pragma unroll
-    for (int u = 0; u < kEllChunk; ++u) {
-      const bool ok = n[u] >= 0;
-      const uint32_t en = ok ? (uint32_t)n[u] : e;              // a missing neighbour reads the site itself, times J = 0
-      Jt[u] = ok ? Jt[u] : 0.0f;
+    for (int u = 0; u < C; ++u) { nb[u][0] = __ldg(Xc0 + n[u]); nb[u][1] = __ldg(Xc1 + n[u]); nb[u][2] = __ldg(Xc2 + n[u]); }
 #pragma unroll
-      for (int c = 0; c < 3; ++c) nb[u][c] = __ldg(base + (p.oX + (uint32_t)c * p.as + en));
-    }
-#pragma unroll
-    for (int u = 0; u < kEllChunk; ++u)
+    for (int u = 0; u < C; ++u)
 #pragma unroll
       for (int c = 0; c < 3; ++c) Be[c] = fmaf(Jt[u], nb[u][c], Be[c]);
+  };
+  if (WT > 0) {
+#pragma unroll
+    for (int s0 = 0; s0 + kEllChunk <= WT; s0 += kEllChunk) chunk(std::integral_constant<int, kEllChunk>{});
+#pragma unroll
+    for (int s0 = WT - WT % kEllChunk; s0 < WT; ++s0) chunk(std::integral_constant<int, 1>{});
+  } else {
+    int s0 = 0;
+    for (; s0 + kEllChunk <= W; s0 += kEllChunk) chunk(std::integral_constant<int, kEllChunk>{});
+    for (; s0 < W; ++s0) chunk(std::integral_constant<int, 1>{});
   }
 
   // ---- noise, torque, update, renormalise ----
@@ -117,12 +129,24 @@ __global__ void __launch_bounds__(kEllThreads, 4) heun_stage_ell(const EllParams
   const float Xs[3] = {X0, X1, X2};
   float ov[3], oAv[3];
   site_update<STAGE>(sc, Xs, Be, gp, Bap, sg, xi, Ai, ov, oAv);
+  float* __restrict__ out = p.arrays_w + e;
 #pragma unroll
-  for (int c = 0; c < 3; ++c) p.arrays_w[p.oOut + (uint32_t)c * p.as + e] = ov[c];
+  for (int c = 0; c < 3; ++c) out[p.oOut + (uint32_t)c * p.as] = ov[c];
   if (STAGE == 0) {
 #pragma unroll
-    for (int c = 0; c < 3; ++c) p.arrays_w[p.oOutA + (uint32_t)c * p.as + e] = oAv[c];
+    for (int c = 0; c < 3; ++c) out[p.oOutA + (uint32_t)c * p.as] = oAv[c];
   }
+}
+
+template <int WT>
+void launch_ell_pair(Ctx& c, EllParams& f, unsigned blocks, bool pdl) {
+  const uint32_t as = f.as;
+  f.oX = (uint32_t)c.aS * as; f.oOut = (uint32_t)c.aSt * as; f.oOutA = AR_A * as; f.oA = AR_A * as;
+  launch_pdl(heun_stage_ell<0, WT>, blocks, kEllThreads, c.launch_stream, f, pdl);
+  c.launches += 1;
+  f.oX = (uint32_t)c.aSt * as; f.oOut = (uint32_t)c.aS * as;
+  launch_pdl(heun_stage_ell<1, WT>, blocks, kEllThreads, c.launch_stream, f, pdl);
+  c.launches += 1;
 }
 
 }  // namespace
@@ -145,14 +169,12 @@ asd_status launch_heun_ell(Ctx& c, StageParams& p) {
   f.gdt = p.gdt; f.lambda = p.lambda; f.scale = p.scale;
   f.n_lo = p.n_lo; f.n_hi = p.n_hi; f.dyn = p.dyn; f.g0 = p.g0; f.key = p.key;
   const unsigned blocks = (unsigned)((c.N + kEllThreads - 1) / kEllThreads);
-  const uint32_t as = f.as;
   const bool pdl = c.launch_stream == c.stream;
-  f.oX = (uint32_t)c.aS * as; f.oOut = (uint32_t)c.aSt * as; f.oOutA = AR_A * as; f.oA = AR_A * as;
-  launch_pdl(heun_stage_ell<0>, blocks, kEllThreads, c.launch_stream, f, pdl);
-  ASD_LAUNCH_CHECK(c, "heun predictor (ell)");
-  f.oX = (uint32_t)c.aSt * as; f.oOut = (uint32_t)c.aS * as;
-  launch_pdl(heun_stage_ell<1>, blocks, kEllThreads, c.launch_stream, f, pdl);
-  ASD_LAUNCH_CHECK(c, "heun corrector (ell)");
+  if (f.W == 10) launch_ell_pair<10>(c, f, blocks, pdl);
+  else if (f.W == 6) launch_ell_pair<6>(c, f, blocks, pdl);
+  else launch_ell_pair<0>(c, f, blocks, pdl);
+  const cudaError_t err = cudaGetLastError();
+  if (err != cudaSuccess) return fail_cuda(c, err, "heun stage (ell)");
   return ASD_OK;
 }
 

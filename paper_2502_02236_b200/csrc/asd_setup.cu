@@ -122,11 +122,14 @@ __global__ void ell_transpose_kernel(const int32_t* __restrict__ idx_in, const f
   const int64_t l = t / W;
   const int s = (int)(t - l * W);
   const int32_t n = idx_in[t];
-  int32_t e = -1;
-  if (n >= 0 && n < N) { const int32_t r = n / ny; e = lead + r * nyp + (n - r * ny); }
-  idx_out[(int64_t)s * N + l] = e;
+  // An empty slot is stored as "the site itself with J = 0": the stage kernels then need neither a test nor a select
+  // per slot (0 * S_i adds nothing; S_i is finite).
+  const bool has = n >= 0 && n < N;
+  const int64_t m = has ? (int64_t)n : l;
+  const int32_t r = (int32_t)(m / ny);
+  idx_out[(int64_t)s * N + l] = lead + r * nyp + (int32_t)(m - (int64_t)r * ny);
   // J/mu_s in Tesla; both factors are far outside fp32 range individually, so rescale first
-  J_out[(int64_t)s * N + l] = (J_in[t] * j_unit) * inv_mu_s_scaled;
+  J_out[(int64_t)s * N + l] = has ? (J_in[t] * j_unit) * inv_mu_s_scaled : 0.0f;
 }
 
 inline unsigned nblocks(int64_t n, int threads) { return (unsigned)((n + threads - 1) / threads); }
