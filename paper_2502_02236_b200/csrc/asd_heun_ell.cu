@@ -45,6 +45,14 @@ struct EllParams {
   PhiloxKey key;
 };
 
+// base + 4 * idx as ONE widening multiply-add (the compiler's default for pointer + zero-extended index is an LEA pair)
+template <class T>
+__device__ __forceinline__ const T* at32(const T* base, uint32_t idx) {
+  uint64_t a;
+  asm("mad.wide.u32 %0, %1, 4, %2;" : "=l"(a) : "r"(idx), "l"(base));
+  return reinterpret_cast<const T*>(a);
+}
+
 // WT = table width known at compile time (6: simple cubic, 10: the L1_0 shells), or 0 = read it from the parameters.
 template <int STAGE, int WT>
 __global__ void __launch_bounds__(kEllThreads, 4) heun_stage_ell(const EllParams p) {
@@ -91,17 +99,16 @@ __global__ void __launch_bounds__(kEllThreads, 4) heun_stage_ell(const EllParams
   // ---- exchange field: chunks of kEllChunk slots, table first, then the gathers, then the sums.  Empty slots were
   // stored at set-up as (the site itself, J = 0): no test, no select. ----
   float Be[3] = {0.0f, 0.0f, 0.0f};
-  const int32_t* __restrict__ pi = p.idx + l;
-  const float* __restrict__ pj = p.Jt + l;
+  uint32_t q = l;                                                // element offset of (slot, site) in the table: s * N + l
   auto chunk = [&](auto count) {
     constexpr int C = decltype(count)::value;
     uint32_t n[C];
     float Jt[C];
 #pragma unroll
-    for (int u = 0; u < C; ++u) { n[u] = (uint32_t)__ldg(pi); Jt[u] = __ldg(pj); pi += p.N; pj += p.N; }
+    for (int u = 0; u < C; ++u) { n[u] = (uint32_t)__ldg(at32(p.idx, q)); Jt[u] = __ldg(at32(p.Jt, q)); q += p.N; }
     float nb[C][3];
 #pragma unroll
-    for (int u = 0; u < C; ++u) { nb[u][0] = __ldg(Xc0 + n[u]); nb[u][1] = __ldg(Xc1 + n[u]); nb[u][2] = __ldg(Xc2 + n[u]); }
+    for (int u = 0; u < C; ++u) { nb[u][0] = __ldg(at32(Xc0, n[u])); nb[u][1] = __ldg(at32(Xc1, n[u])); nb[u][2] = __ldg(at32(Xc2, n[u])); }
 #pragma unroll
     for (int u = 0; u < C; ++u)
 #pragma unroll
@@ -153,7 +160,7 @@ void launch_ell_pair(Ctx& c, EllParams& f, unsigned blocks, bool pdl) {
 
 // The dedicated ELL kernel needs 32-bit element offsets and dense site ids; everything else lives in the table.
 bool heun_ell_supported(const Ctx& c) {
-  return c.d.ell_width > 0 && (int64_t)AR_COUNT * c.as < (1ll << 31) && c.N < (1ll << 31) &&
+  return c.d.ell_width > 0 && (int64_t)AR_COUNT * c.as < (1ll << 31) && c.N * (int64_t)c.d.ell_width < (1ll << 32) &&
          c.d.track_nx * (int64_t)c.d.ny < (1ll << 30);
 }
 
