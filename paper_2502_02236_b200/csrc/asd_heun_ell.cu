@@ -7,8 +7,8 @@
 // thread every table read is a coalesced 128-byte sweep per warp and every neighbour gather of adjacent sites lands on
 // adjacent (or the same few) cache lines.  All slots of a chunk are loaded before any is used (memory-level parallelism
 // without a dependent chain per slot); an empty slot is stored at set-up as (the site itself, J = 0), so the kernel has
-// neither a test nor a select per slot.  The table, sigma, B (and A) are pure streams: a bulk L2 prefetch runs a third of a wave ahead exactly as in
-// the film kernel, and the kernels are launched with programmatic dependent launch.
+// neither a test nor a select per slot.  The table is a pure stream: a bulk L2 prefetch runs a third of a wave ahead
+// exactly as in the film kernel, and the kernels are launched with programmatic dependent launch.
 //
 // Bytes per site per stage that must come from / go to HBM: 52 + 8 W: 132 for the 10-neighbour L1_0
 // shells.  Boundaries, vacancies, grain decoupling and periodic wraps all live in the table; the kernel knows none of it.
@@ -31,7 +31,7 @@ struct EllParams {
   float* arrays_w;
   uint32_t as;
   uint32_t oX, oA, oOut, oOutA, oSigma, oB;
-  const int32_t* idx;              // [W][N] padded element offsets, -1 = none
+  const int32_t* idx;              // [W][N] padded element offsets (an empty slot: the site itself, with J = 0)
   const float* Jt;                 // [W][N] J / mu_s, Tesla
   int32_t W;
   uint32_t N, ny, nyp, lead, nz;
