@@ -191,7 +191,8 @@ def run_ours(args):
         ctx.enable_demag([a * 1e-9 for a in w.spacing_nm])
         ctx.set_demag_every(args.demag_every)
     if args.kernel != "auto":
-        ctx.set_kernel({"general": asd.KERNEL_GENERAL, "fast": asd.KERNEL_FAST, "tma": asd.KERNEL_TMA}[args.kernel])
+        ctx.set_kernel({"general": asd.KERNEL_GENERAL, "fast": asd.KERNEL_FAST, "tma": asd.KERNEL_TMA,
+                        "fused": asd.KERNEL_FUSED}[args.kernel])
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory()
     hT, hBx, hBy, hBz = pin(w.T), pin(w.Bx), pin(w.By), pin(w.Bz)
     ctx.set_spins_host(pin(w.sx), pin(w.sy), pin(w.sz))
@@ -205,8 +206,9 @@ def run_ours(args):
         ctx.set_field_scale(s)
         if timed_heun is not None:
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            lc = ctx.launch_count()
             e0.record(); ctx.step_heun(hps); e1.record()
-            timed_heun.append((e0, e1))
+            timed_heun.append((e0, e1, ctx.launch_count() - lc))
         else:
             ctx.step_heun(hps)
         if p:
@@ -231,7 +233,7 @@ def run_ours(args):
     ms = t0.elapsed_time(t1)
     clocks = sampler.stop() if rank == 0 else None
     launches = ctx.launch_count() - l0
-    heun_ms = sum(a.elapsed_time(b) for a, b in heun_events)
+    heun_ms = sum(a.elapsed_time(b) for a, b, _ in heun_events)
     ms, updates = reduce_over_ranks(ms, float(args.steps) * hps * N, dist, dev)
     value = updates / (ms * 1e-3)
 
@@ -268,10 +270,11 @@ def run_ours(args):
             dist.destroy_process_group()
         return
     peak, peak_src = _peaks()
-    n_stage_launches = 2 * hps * len(heun_events)
+    n_stage_launches = sum(n for _, _, n in heun_events)
+    fused = n_stage_launches == hps * len(heun_events)       # one kernel per Heun step
     avg_launch_s = heun_ms * 1e-3 / n_stage_launches
     # a general ELL table adds its own compulsory bytes: int32 index + fp32 J per slot per site per stage
-    alg_bytes = (BYTES_PER_SITE_PER_STAGE + 8.0 * ell_w) * N
+    alg_bytes = (40.0 if fused else BYTES_PER_SITE_PER_STAGE + 8.0 * ell_w) * N
     achieved = alg_bytes / avg_launch_s / 1e9
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -284,7 +287,8 @@ def run_ours(args):
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 16 * N, "d2h_bytes_per_step": 32,
                 "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps, "wall_ms_per_step": wall_ms / e2e_steps},
         "roofline": {"bound": "hbm", "kernel": ("heun_stage_general<ELL> (predictor+corrector, %d B/site each)" % (52 + 8 * ell_w)) if ell_w else
-                     "heun_stage_fast (predictor+corrector, 52 B/site each)",
+                     ("heun_fused (one kernel per Heun step, 40 B/site)" if fused else
+                      "heun_stage_fast (predictor+corrector, 52 B/site each)"),
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "peak_source": peak_src, "avg_launch_us": avg_launch_s * 1e6,
                      "algorithmic_bytes_per_launch": alg_bytes, "traffic": _traffic(w.name)},
@@ -376,7 +380,7 @@ def main():
                     help="switch the demagnetising field on (Eq. (6)-(7): coarse-graining + FFT convolution per stage)")
     ap.add_argument("--demag-every", type=int, default=0,
                     help="0: demag field recomputed in every Heun stage; P >= 1: every P-th step, held in between")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "general", "fast", "tma"],
+    ap.add_argument("--kernel", default="auto", choices=["auto", "general", "fast", "tma", "fused"],
                     help="stage-kernel variant (asd_set_kernel); auto = the library's choice")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

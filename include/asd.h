@@ -64,8 +64,10 @@ typedef enum {
 
 enum { ASD_SC = 0, ASD_L10_FE = 1 };
 
-/* Kernel variant for asd_step_heun.  AUTO picks the fastest supported. */
-enum { ASD_KERNEL_AUTO = 0, ASD_KERNEL_GENERAL = 1, ASD_KERNEL_FAST = 2, ASD_KERNEL_TMA = 3 };
+/* Kernel variant for asd_step_heun.  AUTO picks the fastest supported.
+ * FUSED: one kernel per Heun step (predictor results stay in shared memory / registers); FAST, TMA, GENERAL: one
+ * kernel per stage. */
+enum { ASD_KERNEL_AUTO = 0, ASD_KERNEL_GENERAL = 1, ASD_KERNEL_FAST = 2, ASD_KERNEL_TMA = 3, ASD_KERNEL_FUSED = 4 };
 
 /* CUDA-graph replay of asd_step_heun batches (launch-bound lattices).  AUTO: on for windows of <= 2^18 sites. */
 enum { ASD_GRAPH_AUTO = 0, ASD_GRAPH_OFF = 1, ASD_GRAPH_ON = 2 };

@@ -222,6 +222,7 @@ asd_status asd_destroy(asd_ctx* ctx) {
   if (!ctx) return ASD_EINVAL;
   if (ctx->c.host_scratch) cudaFreeHost(ctx->c.host_scratch);
   asd::tma_plan_free(ctx->c);
+  asd::fused_plan_free(ctx->c);
   asd::graphs_free(ctx->c);
   if (ctx->c.copy_stream) { cudaStreamDestroy(ctx->c.copy_stream); cudaEventDestroy(ctx->c.staged_ev); cudaEventDestroy(ctx->c.consumed_ev); }
   asd::demag_free(ctx->c);
@@ -378,8 +379,10 @@ asd_status asd_step_heun(asd_ctx* ctx, int64_t n) {
 asd_status asd_set_kernel(asd_ctx* ctx, int32_t variant) {
   CTX_OR_RETURN(ctx);
   if (variant != ASD_KERNEL_AUTO && variant != ASD_KERNEL_GENERAL && variant != ASD_KERNEL_FAST &&
-      variant != ASD_KERNEL_TMA)
+      variant != ASD_KERNEL_TMA && variant != ASD_KERNEL_FUSED)
     return fail(c, ASD_EINVAL, "asd_set_kernel: unknown variant");
+  if (variant == ASD_KERNEL_FUSED && (!heun_fused_supported(c) || c.demag || !fused_plan(c)))
+    return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: the fused step needs what the film kernel needs, no demagnetising field, and a strip plan that fits in shared memory");
   if (variant == ASD_KERNEL_TMA && (!heun_tma_supported(c) || !tma_plan(c)))
     return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: the staged film kernel needs what the film kernel needs and a strip plan that fits in shared memory");
   if (variant == ASD_KERNEL_FAST && !heun_fast_supported(c))

@@ -82,7 +82,8 @@ void graphs_free(Ctx& c) {
 
 asd_status launch_heun(Ctx& c, int64_t n) {
   c.launch_stream = c.stream;
-  const bool use = !c.demag &&                  // the demag pipeline (cuFFT) is launched plainly
+  const bool use = !c.demag &&                  // the demag pipeline is launched plainly
+                   c.kernel_variant != ASD_KERNEL_FUSED &&   // the fused step swaps the spin buffers every step
                    (c.graph_mode == ASD_GRAPH_ON || (c.graph_mode == ASD_GRAPH_AUTO && c.N <= kAutoMaxSites));
   while (use && n >= 2) {
     const int64_t k = n < kBatch ? n : kBatch;

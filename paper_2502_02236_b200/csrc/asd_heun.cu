@@ -289,6 +289,12 @@ asd_status launch_heun_direct(Ctx& c, int64_t n, const DynState* dyn) {
   const bool staged = c.kernel_variant == ASD_KERNEL_TMA;
   if (staged && !(heun_tma_supported(c) && tma_plan(c))) return ASD_EUNSUPPORTED;
   if (c.demag && (staged || c.d.ell_width > 0)) return ASD_EUNSUPPORTED;   // demag: film and general kernels only
+  // one kernel per step: asked for, or AUTO on a film large enough to fill the machine with strip x chunk CTAs.
+  // Not inside a recorded graph (the spin buffers swap roles every step) and not with the demagnetising field.
+  const bool fused = !dyn && !c.demag && heun_fused_supported(c) &&
+                     (c.kernel_variant == ASD_KERNEL_FUSED || (c.kernel_variant == ASD_KERNEL_AUTO && heun_fused_preferred(c))) &&
+                     fused_plan(c);
+  if (c.kernel_variant == ASD_KERNEL_FUSED && !fused) return ASD_EUNSUPPORTED;
   for (int64_t s = 0; s < n; ++s) {
     const uint64_t idx = dyn ? (uint64_t)s : (uint64_t)c.step;
     p.n_lo = (uint32_t)(idx & 0xFFFFFFFFull);
@@ -298,7 +304,8 @@ asd_status launch_heun_direct(Ctx& c, int64_t n, const DynState* dyn) {
       c.demag_age += 1;
     }
     asd_status st;
-    if (staged) st = launch_heun_tma(c, p);
+    if (fused) st = launch_heun_fused(c, p);
+    else if (staged) st = launch_heun_tma(c, p);
     else if (fast) st = launch_heun_fast(c, p);
     else if (c.d.ell_width > 0) st = (c.kernel_variant != ASD_KERNEL_GENERAL && heun_ell_supported(c)) ? launch_heun_ell(c, p)
                                                                                                      : launch_pair<1, LAT_ELL>(c, p);

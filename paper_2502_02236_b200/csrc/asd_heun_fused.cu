@@ -1,0 +1,549 @@
+// asd_heun_fused.cu -- the hot path, fused variant: ONE kernel per stochastic-Heun step.
+//
+// The two-kernel step writes the predictor's S~ and A = S + dt/2 k1 to HBM and reads them back (104 B per site per
+// step).  Here the predictor's results never leave the SM: 40 B per site per step -- S in (12),
+// sigma and B in (16), S out (12) -- and the noise of a site (Philox4x32-10 + Box-Muller) is generated once per step
+// instead of once per stage.
+//
+// How.  Same lattices as the film kernel (open boundaries, built-in shells, ny % 4 == 0, grains that do not touch; a
+// missing or vacant neighbour is a stored or TMA-filled zero, so Eq. (2) needs no mask).  The window is cut into
+// y-strips of BY sites and x-chunks of CX planes; one CTA owns one (strip, chunk), holds the whole film thickness and
+// MARCHES along x.  Per march step m (predictor plane q, corrector plane q - 1):
+//   * S planes q-1, q, q+1 sit in a 4-slot shared-memory ring; plane q+2 is in flight.  One TMA box
+//     [3 components][nz + 2 rows][BY + 8 sites] per plane (cp.async.bulk.tensor.4d completing on an mbarrier); rows
+//     z = -1, nz, columns y < 0, >= ny and planes x < 0, >= nx are zero-filled by the TMA: the open boundary.
+//   * predictor of plane q from the S ring: the "main" threads own 4 consecutive y-sites of one z-row of the strip
+//     (same (row, group) for the whole march); the "halo" threads (one warp for nz <= 32) own the two sites of one z-row in the columns next to the
+//     strip, whose S~ the strip's corrector needs and which are RECOMPUTED here (the noise is a pure function of
+//     (seed, step, global site), so the neighbouring CTA computes the same values).  S~ goes to a second 4-slot ring
+//     in shared memory; A and the stage-independent part of the field, sigma xi + s B_app, stay in registers.
+//   * one CTA barrier; thread 0 then refills the S slot that has just been read for the last time.
+//   * corrector of plane q - 1 from S~ planes q-2, q-1, q; the new S goes to the OTHER spin buffer in HBM (the
+//     neighbouring chunk still needs the old values of its halo planes), and the buffers swap roles after the step.
+// A chunk recomputes the predictor of one plane before and one after itself (its x halo).
+// With four S~ slots one barrier per plane is enough: the predictor of step m+1 writes slot (m+1) % 4, which the
+// corrector of step m (slots m-2, m-1, m) does not read, and the predictor of step m+2 is behind the barrier of m+1.
+#include <cstdlib>
+
+#include "asd_internal.cuh"
+#include "asd_site.cuh"
+#include "asd_tma.cuh"
+
+namespace asd {
+
+namespace {
+
+constexpr int LAT_SC = 0, LAT_L10 = 1;
+constexpr int kRing = 4;
+
+struct FusedParams {
+  const float* arrays;
+  float* arrays_w;
+  uint32_t as;                     // array stride (elements)
+  int32_t aIn;                     // array index of component 0 of the input spins (TMA coordinate)
+  uint32_t oOut, oSigma, oB;       // element offsets (array index * as)
+  const uint32_t* col;             // column table at the window origin
+  const float4* grain;             // (e_x, e_y, e_z, 2 k_u/mu_s) per grain id + 1
+  int32_t nx, ny, nz, nyp, lead;
+  int32_t BY, G, nstrips, CX;      // strip width (sites), y-groups per strip row, strips, planes per chunk
+  int32_t n_main;                  // threads that own 4-site groups (a multiple of 32); the rest are halo threads
+  uint32_t slot_pitch;             // bytes of one ring slot (multiple of 128)
+  float j1, j2, j3;
+  float gdt, lambda, scale;
+  uint32_t n_lo, n_hi;
+  const DynState* dyn;
+  uint64_t g0;
+  PhiloxKey key;
+};
+
+__device__ __forceinline__ void cta_barrier() { asm volatile("bar.sync 0;" ::: "memory"); }
+
+// dt f(X, B) of Eq. (1) in LL form (asd_site.cuh)
+__device__ __forceinline__ void llg_dt_f(const SiteConst& p, const float X[3], float B0, float B1, float B2, float f[3]) {
+  const float a0 = X[1] * B2 - X[2] * B1, a1 = X[2] * B0 - X[0] * B2, a2 = X[0] * B1 - X[1] * B0;   // S x B
+  const float b0 = X[1] * a2 - X[2] * a1, b1 = X[2] * a0 - X[0] * a2, b2 = X[0] * a1 - X[1] * a0;   // S x (S x B)
+  f[0] = -p.gdt * fmaf(p.lambda, b0, a0);
+  f[1] = -p.gdt * fmaf(p.lambda, b1, a1);
+  f[2] = -p.gdt * fmaf(p.lambda, b2, a2);
+}
+
+// Exchange field of the 4 sites of a group from three ring slots (prev, cur, next = planes x-1, x, x+1); also returns
+// the group's own values X[c][0..3].  b = byte address of the group's own float4 in component 0 of slot `cur`.
+template <int LAT>
+__device__ __forceinline__ void exchange4(uint32_t prev, uint32_t cur, uint32_t next, uint32_t rowb, uint32_t compb,
+                                          float j1, float j2, float j3, float X[3][4], float Bex[3][4]) {
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    const uint32_t cb = (uint32_t)c * compb;
+    const float4 o = lds4(cur + cb);
+    const float oL = lds1(cur + cb - 4u), oR = lds1(cur + cb + 16u);
+    const float4 zp = lds4(cur + cb + rowb), zm = lds4(cur + cb - rowb);
+    const float4 xp = lds4(next + cb), xm = lds4(prev + cb);
+    const float own[6] = {oL, o.x, o.y, o.z, o.w, oR};
+    X[c][0] = o.x; X[c][1] = o.y; X[c][2] = o.z; X[c][3] = o.w;
+    const float zs[4] = {zp.x + zm.x, zp.y + zm.y, zp.z + zm.z, zp.w + zm.w};
+    if (LAT == LAT_SC) {
+      // 6 nearest neighbours, one J
+      const float xs[4] = {xp.x + xm.x, xp.y + xm.y, xp.z + xm.z, xp.w + xm.w};
+#pragma unroll
+      for (int v = 0; v < 4; ++v) Bex[c][v] = j1 * ((xs[v] + zs[v]) + (own[v] + own[v + 2]));
+    } else {
+      // 4 in-plane nn (J1), 2 out-of-plane (J2), 4 in-plane nnn (J3): "4 nearest + 6 next nearest"
+      float xs[6];
+      xs[0] = lds1(next + cb - 4u) + lds1(prev + cb - 4u);
+      xs[1] = xp.x + xm.x; xs[2] = xp.y + xm.y; xs[3] = xp.z + xm.z; xs[4] = xp.w + xm.w;
+      xs[5] = lds1(next + cb + 16u) + lds1(prev + cb + 16u);
+#pragma unroll
+      for (int v = 0; v < 4; ++v) {
+        const float s1 = xs[v + 1] + (own[v] + own[v + 2]);
+        const float s3 = xs[v] + xs[v + 2];
+        Bex[c][v] = fmaf(j3, s3, fmaf(j2, zs[v], j1 * s1));
+      }
+    }
+  }
+}
+
+template <int LAT, int NT, int MINB>
+__global__ void __launch_bounds__(NT, MINB) heun_fused(const __grid_constant__ CUtensorMap mapS, const FusedParams p) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const uint32_t sm0 = smem_u32(smem_raw);
+  const uint32_t bar_full = sm0;
+  const uint32_t sring = sm0 + 128u;
+  const uint32_t tring = sring + kRing * p.slot_pitch;
+
+  const int tid = (int)threadIdx.x;
+  const int strip = (int)blockIdx.x % p.nstrips, chunk = (int)blockIdx.x / p.nstrips;
+  const int j0 = strip * p.BY;
+  const int i0 = chunk * p.CX;
+  const int L = min(p.CX, p.nx - i0);                 // planes this CTA updates
+  const int W = p.BY + 8, R = p.nz + 2;
+  const uint32_t rowb = (uint32_t)(W * 4), compb = (uint32_t)(R * W * 4);
+  const uint32_t box_bytes = 3u * compb;
+
+  // S~ ring starts as zeros: the rows z = -1 and z = nz, and the columns of a ragged last strip, are never written.
+  for (uint32_t o = (uint32_t)tid * 16u; o < kRing * p.slot_pitch; o += (uint32_t)blockDim.x * 16u)
+    sts4(tring + o, 0.0f, 0.0f, 0.0f, 0.0f);
+  if (tid == 0) {
+    for (int s = 0; s < kRing; ++s) mbar_init(bar_full + 8u * s, 1u);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  // Programmatic dependent launch: everything above overlaps the tail of the previous step's grid; nothing below the
+  // wait runs before that grid has completed (it wrote the spins this one reads and read the buffer this one writes).
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  cta_barrier();
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+
+  // ring plane u (u = 0 is window plane i0 - 2) -> slot u % 4
+  auto issue = [&](int u) {
+    const uint32_t s = (uint32_t)(u & (kRing - 1));
+    const uint32_t bar = bar_full + 8u * s;
+    mbar_expect_tx(bar, box_bytes);
+    tma_load_4d(sring + s * p.slot_pitch, &mapS, bar, j0 - 4, -1, i0 - 2 + u, p.aIn);
+  };
+  if (tid == 0)
+    for (int u = 0; u < kRing; ++u) issue(u);          // L >= 1: planes u = 0 .. L+3 are all needed
+
+  uint32_t n_lo = p.n_lo, n_hi = p.n_hi; float scale = p.scale;
+  resolve_dyn(p.dyn, n_lo, n_hi, scale);
+  const SiteConst sc{p.gdt, p.lambda, scale};
+  const float* __restrict__ base = p.arrays;
+  const uint32_t planep = (uint32_t)(p.nz * p.nyp);
+
+  if (tid < p.n_main) {
+    // ================= main threads: 4 consecutive y-sites of one z-row, predictor and corrector =================
+    const int k = tid / p.G, g = tid - k * p.G;
+    const int j = j0 + 4 * g;
+    const bool active = (k < p.nz) && (j < p.ny);
+    const uint32_t own_b = (uint32_t)(((k + 1) * W + 4 + 4 * g) * 4);   // own float4 inside component 0 of a slot
+    // element of the group in predictor plane q = i0 - 1 (wraps below zero for q = -1; not dereferenced then)
+    uint32_t e = (uint32_t)(p.lead + ((i0 - 1) * p.nz + k) * p.nyp + j);
+    uint32_t ec = (uint32_t)((i0 - 1) * p.ny + j);                      // column (q, j) of the window
+    uint64_t gsite = p.g0 + (uint64_t)(int64_t)(((int64_t)(i0 - 1) * p.nz + k) * p.ny + j);
+    const uint32_t gplane = (uint32_t)(p.nz * p.ny);
+
+    // carried from the predictor of plane q to its corrector one march step later
+    float A[3][4], Bs[3][4];
+    uint32_t gid_c = 0u; bool mixed_c = false;
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+      for (int v = 0; v < 4; ++v) { A[c][v] = 0.0f; Bs[c][v] = 0.0f; }
+
+    mbar_wait(bar_full + 0u, 0u);
+    mbar_wait(bar_full + 8u, 0u);
+
+    for (int m = 0; m <= L + 1; ++m) {
+      const int q = i0 - 1 + m;
+      const bool qvalid = active && (q >= 0) && (q < p.nx);
+      // streaming inputs of the predictor plane: issued first, used after the wait
+      float4 sg4 = make_float4(0.f, 0.f, 0.f, 0.f), bx4 = sg4, by4 = sg4, bz4 = sg4;
+      uint4 cid4 = make_uint4(0u, 0u, 0u, 0u);
+      if (qvalid) {
+        sg4 = ldg_stream4(base + (p.oSigma + e));
+        bx4 = ldg_stream4(base + (p.oB + e));
+        by4 = ldg_stream4(base + (p.oB + p.as + e));
+        bz4 = ldg_stream4(base + (p.oB + 2u * p.as + e));
+        cid4 = __ldg(reinterpret_cast<const uint4*>(p.col + ec));
+      }
+      mbar_wait(bar_full + 8u * (uint32_t)((m + 2) & (kRing - 1)), (uint32_t)((m + 2) >> 2) & 1u);   // plane q + 1
+
+      float An[3][4], Bn[3][4];                        // this plane's A and sigma xi + s B_app
+      uint32_t gid_n = 0u; bool mixed_n = false;
+      const uint32_t tslot = tring + (uint32_t)(m & (kRing - 1)) * p.slot_pitch + own_b;
+      if (qvalid) {
+        // ---- noise: one Philox block per site per STEP ----
+        const float sg[4] = {sg4.x, sg4.y, sg4.z, sg4.w};
+        const float bx[4] = {bx4.x, bx4.y, bx4.z, bx4.w}, by[4] = {by4.x, by4.y, by4.z, by4.w},
+                    bz[4] = {bz4.x, bz4.y, bz4.z, bz4.w};
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+          uint32_t rnd[4];
+          philox_site(p.key, n_lo, n_hi, gsite + (uint64_t)v, 0u, rnd);
+          float xi[3];
+          normals3(rnd, xi);
+          Bn[0][v] = fmaf(sg[v], xi[0], scale * bx[v]);
+          Bn[1][v] = fmaf(sg[v], xi[1], scale * by[v]);
+          Bn[2][v] = fmaf(sg[v], xi[2], scale * bz[v]);
+        }
+        // ---- predictor: S~ = normalise(S + dt k1), A = S + dt/2 k1 ----
+        const uint32_t prev = sring + (uint32_t)(m & (kRing - 1)) * p.slot_pitch + own_b;
+        const uint32_t cur = sring + (uint32_t)((m + 1) & (kRing - 1)) * p.slot_pitch + own_b;
+        const uint32_t next = sring + (uint32_t)((m + 2) & (kRing - 1)) * p.slot_pitch + own_b;
+        float X[3][4], Bex[3][4];
+        exchange4<LAT>(prev, cur, next, rowb, compb, p.j1, p.j2, p.j3, X, Bex);
+        gid_n = max(max(cid4.x & 0xFFFFu, cid4.y & 0xFFFFu), max(cid4.z & 0xFFFFu, cid4.w & 0xFFFFu));
+        mixed_n = (cid4.x & COL_GROUP_MIXED) != 0u;
+        float4 gp4[4];
+        gp4[0] = gp4[1] = gp4[2] = gp4[3] = __ldg(p.grain + gid_n);
+        if (mixed_n) {
+          gp4[0] = __ldg(p.grain + (cid4.x & 0xFFFFu)); gp4[1] = __ldg(p.grain + (cid4.y & 0xFFFFu));
+          gp4[2] = __ldg(p.grain + (cid4.z & 0xFFFFu)); gp4[3] = __ldg(p.grain + (cid4.w & 0xFFFFu));
+        }
+        float St[3][4];
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+          const float Xs[3] = {X[0][v], X[1][v], X[2][v]};
+          const float4 gp = gp4[v];
+          const float ca = gp.w * fmaf(Xs[0], gp.x, fmaf(Xs[1], gp.y, Xs[2] * gp.z));     // Eq. (3)
+          float f[3];
+          llg_dt_f(sc, Xs, fmaf(ca, gp.x, Bex[0][v]) + Bn[0][v], fmaf(ca, gp.y, Bex[1][v]) + Bn[1][v],
+                   fmaf(ca, gp.z, Bex[2][v]) + Bn[2][v], f);
+          An[0][v] = fmaf(0.5f, f[0], Xs[0]); An[1][v] = fmaf(0.5f, f[1], Xs[1]); An[2][v] = fmaf(0.5f, f[2], Xs[2]);
+          float o[3];
+          normalise3(Xs[0] + f[0], Xs[1] + f[1], Xs[2] + f[2], o);
+          St[0][v] = o[0]; St[1][v] = o[1]; St[2][v] = o[2];
+        }
+#pragma unroll
+        for (int c = 0; c < 3; ++c) sts4(tslot + (uint32_t)c * compb, St[c][0], St[c][1], St[c][2], St[c][3]);
+      } else {
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+#pragma unroll
+          for (int v = 0; v < 4; ++v) { An[c][v] = 0.0f; Bn[c][v] = 0.0f; }
+        if (active) {                                  // a plane outside the window: S~ = 0 (open boundary in x)
+#pragma unroll
+          for (int c = 0; c < 3; ++c) sts4(tslot + (uint32_t)c * compb, 0.0f, 0.0f, 0.0f, 0.0f);
+        }
+      }
+      cta_barrier();                                   // S~ plane q is complete; S plane q - 1 has been read for the last time
+      if (tid == 0 && m + kRing <= L + 3) issue(m + kRing);
+
+      // ---- corrector of plane q - 1: S = normalise(A + dt/2 k2), k2 from S~ ----
+      if (active && m >= 2) {
+        const uint32_t prev = tring + (uint32_t)((m - 2) & (kRing - 1)) * p.slot_pitch + own_b;
+        const uint32_t cur = tring + (uint32_t)((m - 1) & (kRing - 1)) * p.slot_pitch + own_b;
+        const uint32_t next = tring + (uint32_t)(m & (kRing - 1)) * p.slot_pitch + own_b;
+        float X[3][4], Bex[3][4];
+        exchange4<LAT>(prev, cur, next, rowb, compb, p.j1, p.j2, p.j3, X, Bex);
+        float4 gp4[4];
+        gp4[0] = gp4[1] = gp4[2] = gp4[3] = __ldg(p.grain + gid_c);
+        if (mixed_c) {
+          const uint4 cc = __ldg(reinterpret_cast<const uint4*>(p.col + (ec - (uint32_t)p.ny)));
+          gp4[0] = __ldg(p.grain + (cc.x & 0xFFFFu)); gp4[1] = __ldg(p.grain + (cc.y & 0xFFFFu));
+          gp4[2] = __ldg(p.grain + (cc.z & 0xFFFFu)); gp4[3] = __ldg(p.grain + (cc.w & 0xFFFFu));
+        }
+        float So[3][4];
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+          const float Xs[3] = {X[0][v], X[1][v], X[2][v]};
+          const float4 gp = gp4[v];
+          const float ca = gp.w * fmaf(Xs[0], gp.x, fmaf(Xs[1], gp.y, Xs[2] * gp.z));
+          float f[3];
+          llg_dt_f(sc, Xs, fmaf(ca, gp.x, Bex[0][v]) + Bs[0][v], fmaf(ca, gp.y, Bex[1][v]) + Bs[1][v],
+                   fmaf(ca, gp.z, Bex[2][v]) + Bs[2][v], f);
+          float o[3];
+          normalise3(fmaf(0.5f, f[0], A[0][v]), fmaf(0.5f, f[1], A[1][v]), fmaf(0.5f, f[2], A[2][v]), o);
+          So[0][v] = o[0]; So[1][v] = o[1]; So[2][v] = o[2];
+        }
+        const uint32_t eo = e - planep;                // plane q - 1
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+          *reinterpret_cast<float4*>(p.arrays_w + (p.oOut + (uint32_t)c * p.as + eo)) =
+              make_float4(So[c][0], So[c][1], So[c][2], So[c][3]);
+      }
+#pragma unroll
+      for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int v = 0; v < 4; ++v) { A[c][v] = An[c][v]; Bs[c][v] = Bn[c][v]; }
+      gid_c = gid_n; mixed_c = mixed_n;
+      e += planep; ec += (uint32_t)p.ny; gsite += gplane;
+    }
+  } else {
+    // ================= halo threads: the two sites (y = j0 - 1, y = j0 + BY) of one z-row, predictor only =================
+    // Lanes of a warp read the same column of different rows (a bank-conflicted pattern), so each halo thread keeps
+    // the three columns around its sites for planes q-1, q in registers and loads only plane q+1's and the z
+    // neighbours of plane q per march step.
+    const int k = tid - p.n_main;
+    const bool row_ok = k < p.nz;
+    const int jh[2] = {j0 - 1, j0 + p.BY};
+    const bool act[2] = {row_ok && jh[0] >= 0, row_ok && jh[1] < p.ny};
+    const uint32_t own_b[2] = {(uint32_t)(((k + 1) * W + 3) * 4), (uint32_t)(((k + 1) * W + 4 + p.BY) * 4)};
+    uint32_t e = (uint32_t)(p.lead + ((i0 - 1) * p.nz + k) * p.nyp);          // + jh
+    uint32_t ec = (uint32_t)((i0 - 1) * p.ny);
+    uint64_t gsite = p.g0 + (uint64_t)(int64_t)(((int64_t)(i0 - 1) * p.nz + k) * p.ny);
+    const uint32_t gplane = (uint32_t)(p.nz * p.ny);
+
+    mbar_wait(bar_full + 0u, 0u);
+    mbar_wait(bar_full + 8u, 0u);
+    // window: rP = plane q-1, rC = plane q; [side][component][column y-1, y, y+1]
+    float rP[2][3][3], rC[2][3][3];
+#pragma unroll
+    for (int s = 0; s < 2; ++s)
+#pragma unroll
+      for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+          const uint32_t off = own_b[s] + (uint32_t)c * compb + (uint32_t)(4 * d) - 4u;
+          rP[s][c][d] = row_ok ? lds1(sring + off) : 0.0f;
+          rC[s][c][d] = row_ok ? lds1(sring + p.slot_pitch + off) : 0.0f;
+        }
+
+    for (int m = 0; m <= L + 1; ++m) {
+      const int q = i0 - 1 + m;
+      const bool qin = (q >= 0) && (q < p.nx);
+      float sg[2] = {0.f, 0.f}, bx[2] = {0.f, 0.f}, by[2] = {0.f, 0.f}, bz[2] = {0.f, 0.f};
+      uint32_t cid[2] = {0u, 0u};
+#pragma unroll
+      for (int s = 0; s < 2; ++s)
+        if (act[s] && qin) {
+          const uint32_t es = e + (uint32_t)jh[s];
+          sg[s] = ldg_stream1(base + (p.oSigma + es));
+          bx[s] = ldg_stream1(base + (p.oB + es));
+          by[s] = ldg_stream1(base + (p.oB + p.as + es));
+          bz[s] = ldg_stream1(base + (p.oB + 2u * p.as + es));
+          cid[s] = __ldg(p.col + (ec + (uint32_t)jh[s]));
+        }
+      mbar_wait(bar_full + 8u * (uint32_t)((m + 2) & (kRing - 1)), (uint32_t)((m + 2) >> 2) & 1u);
+      const uint32_t cur = sring + (uint32_t)((m + 1) & (kRing - 1)) * p.slot_pitch;
+      const uint32_t next = sring + (uint32_t)((m + 2) & (kRing - 1)) * p.slot_pitch;
+      const uint32_t tslot = tring + (uint32_t)(m & (kRing - 1)) * p.slot_pitch;
+      float rN[2][3][3];
+#pragma unroll
+      for (int s = 0; s < 2; ++s) {
+        float zs[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          const uint32_t off = own_b[s] + (uint32_t)c * compb;
+#pragma unroll
+          for (int d = 0; d < 3; ++d) rN[s][c][d] = row_ok ? lds1(next + off + (uint32_t)(4 * d) - 4u) : 0.0f;
+          zs[c] = row_ok ? lds1(cur + off + rowb) + lds1(cur + off - rowb) : 0.0f;
+        }
+        if (act[s] && qin) {
+          uint32_t rnd[4];
+          philox_site(p.key, n_lo, n_hi, gsite + (uint64_t)(int64_t)jh[s], 0u, rnd);
+          float xi[3];
+          normals3(rnd, xi);
+          float Xs[3], Bex[3];
+#pragma unroll
+          for (int c = 0; c < 3; ++c) {
+            Xs[c] = rC[s][c][1];
+            const float ys = rC[s][c][0] + rC[s][c][2];
+            const float xs = rN[s][c][1] + rP[s][c][1];
+            if (LAT == LAT_SC) {
+              Bex[c] = p.j1 * ((xs + zs[c]) + ys);
+            } else {
+              const float s3 = (rN[s][c][0] + rP[s][c][0]) + (rN[s][c][2] + rP[s][c][2]);
+              Bex[c] = fmaf(p.j3, s3, fmaf(p.j2, zs[c], p.j1 * (xs + ys)));
+            }
+          }
+          const float4 gp = __ldg(p.grain + (cid[s] & 0xFFFFu));
+          const float ca = gp.w * fmaf(Xs[0], gp.x, fmaf(Xs[1], gp.y, Xs[2] * gp.z));
+          float f[3];
+          llg_dt_f(sc, Xs, fmaf(ca, gp.x, Bex[0]) + fmaf(sg[s], xi[0], scale * bx[s]),
+                   fmaf(ca, gp.y, Bex[1]) + fmaf(sg[s], xi[1], scale * by[s]),
+                   fmaf(ca, gp.z, Bex[2]) + fmaf(sg[s], xi[2], scale * bz[s]), f);
+          float o[3];
+          normalise3(Xs[0] + f[0], Xs[1] + f[1], Xs[2] + f[2], o);
+#pragma unroll
+          for (int c = 0; c < 3; ++c) sts1(tslot + own_b[s] + (uint32_t)c * compb, o[c]);
+        } else if (act[s]) {
+#pragma unroll
+          for (int c = 0; c < 3; ++c) sts1(tslot + own_b[s] + (uint32_t)c * compb, 0.0f);
+        }
+      }
+      cta_barrier();
+#pragma unroll
+      for (int s = 0; s < 2; ++s)
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+#pragma unroll
+          for (int d = 0; d < 3; ++d) { rP[s][c][d] = rC[s][c][d]; rC[s][c][d] = rN[s][c][d]; }
+      e += planep; ec += (uint32_t)p.ny; gsite += gplane;
+    }
+  }
+}
+
+typedef void (*FusedKernel)(const CUtensorMap, const FusedParams);
+
+// Compiled CTA shapes (threads, CTAs per SM -> register budget): 256 x 2 -> 128 registers (4 warps per scheduler),
+// 512 x 1 -> 128.
+struct Shape { int nt, minb; };
+constexpr Shape kShapes[] = {{256, 2}, {512, 1}};
+constexpr int kNumShapes = 2;
+
+FusedKernel kernel_for(int lattice, int shape) {
+  if (lattice == ASD_SC) return shape == 0 ? heun_fused<LAT_SC, 256, 2> : heun_fused<LAT_SC, 512, 1>;
+  return shape == 0 ? heun_fused<LAT_L10, 256, 2> : heun_fused<LAT_L10, 512, 1>;
+}
+
+inline int round_up32(int v) { return (v + 31) / 32 * 32; }
+
+uint32_t plan_smem(int nz, int by, uint32_t& slot_pitch) {
+  slot_pitch = (uint32_t)align_up((size_t)3 * (nz + 2) * (by + 8) * 4, 128);
+  return 128u + 2u * kRing * slot_pitch;
+}
+
+}  // namespace
+
+struct FusedPlan {
+  CUtensorMap mapS;
+  FusedKernel kern = nullptr;
+  int32_t BY = 0, G = 0, nstrips = 0, CX = 0, nchunks = 0, threads = 0, n_main = 0, ctas_per_sm = 0;
+  uint32_t slot_pitch = 0, smem_bytes = 0;
+};
+
+bool heun_fused_supported(const Ctx& c) { return heun_fast_supported(c) && c.d.nz + 2 <= 256; }
+
+// ASD_KERNEL_AUTO takes the fused step for windows that stream from HBM and give every CTA a march of some length:
+// more than 2^21 sites and at least 64 planes.  Smaller films are L2-resident or launch-bound; there the two stage
+// kernels (or their graph replay) stay in charge.
+bool heun_fused_preferred(const Ctx& c) { return c.N > (1ll << 21) && c.d.nx >= 64; }
+
+namespace {
+
+bool build_plan(Ctx& c, FusedPlan& pl) {
+  if (!heun_fused_supported(c)) return false;
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (!enc) return false;
+  const int ny = c.d.ny, nz = c.d.nz, nx = c.d.nx;
+  int smem_sm = 0, smem_cta = 0;
+  cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, c.device);
+  cudaDeviceGetAttribute(&smem_cta, cudaDevAttrMaxSharedMemoryPerBlockOptin, c.device);
+
+  // Strip width: every multiple of 4 up to 64 sites; a plan is scored by the share of predictor work that is useful
+  // (ragged last strip, idle lanes of the last main warp, the recomputed halo columns), with a preference for
+  // 8 groups per row (a quarter-warp then reads one contiguous 128-byte row segment: conflict-free 128-bit loads)
+  // and for two resident CTAs per SM (one computes while the other waits at its barrier).
+  const char* force = std::getenv("ASD_FUSED_BY");          // tuning override (strip width in sites)
+  const int force_by = force ? std::atoi(force) : 0;
+  struct Cand { int by, shape, ctas; double score; } best{0, 0, 0, -1.0};
+  for (int by = 4; by <= 64; by += 4) {
+    if (force_by && by != force_by) continue;
+    if (by > ny && by != (ny + 3) / 4 * 4) continue;
+    const int ns = (ny + by - 1) / by, tasks = nz * (by / 4);
+    const int n_main = round_up32(tasks), n_halo = round_up32(nz);
+    uint32_t sp;
+    const uint32_t smem = plan_smem(nz, by, sp);
+    if ((int)smem > smem_cta) continue;
+    for (int sh = 0; sh < kNumShapes; ++sh) {
+      if (n_main + n_halo > kShapes[sh].nt) continue;
+      int ctas = smem_sm / (int)(smem + 1024);
+      if (ctas > kShapes[sh].minb) ctas = kShapes[sh].minb;
+      if (ctas < 1) continue;
+      const double useful = ((double)ny / (ns * by)) * ((double)tasks / n_main) * ((double)by / (by + 2.6));
+      const double score = useful * (by == 32 ? 1.0 : 0.92) * (ctas >= 2 ? 1.0 : 0.85);
+      if (score > best.score) best = Cand{by, sh, ctas, score};
+      break;                                                // smallest shape that holds the tasks
+    }
+  }
+  if (best.score < 0.0) return false;
+  pl.BY = best.by; pl.G = best.by / 4; pl.nstrips = (ny + best.by - 1) / best.by;
+  pl.n_main = round_up32(nz * pl.G);
+  pl.threads = pl.n_main + round_up32(nz);
+  pl.smem_bytes = plan_smem(nz, pl.BY, pl.slot_pitch);
+  pl.kern = kernel_for(c.d.lattice, best.shape);
+  int bps = 0;
+  if (cudaFuncSetAttribute((const void*)pl.kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes) != cudaSuccess ||
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, (const void*)pl.kern, pl.threads, pl.smem_bytes) != cudaSuccess ||
+      bps < 1) {
+    cudaGetLastError();
+    return false;
+  }
+  pl.ctas_per_sm = bps;
+  // one wave: as many x-chunks as there are CTA slots for each strip, but chunks of at least 4 planes (every chunk
+  // recomputes the predictor of 2 extra planes)
+  int nchunks = (c.sm_count * bps) / pl.nstrips;
+  if (nchunks > nx / 4) nchunks = nx / 4;
+  if (nchunks < 1) nchunks = 1;
+  const char* fc = std::getenv("ASD_FUSED_CHUNKS");         // tuning override
+  if (fc && std::atoi(fc) > 0) nchunks = std::min(std::atoi(fc), nx);
+  pl.CX = (nx + nchunks - 1) / nchunks;
+  pl.nchunks = (nx + pl.CX - 1) / pl.CX;
+
+  // The 13 per-site arrays as one 4-D tensor (y, z-row, x-plane, array); origin = site (0,0,0) of array 0.
+  const cuuint64_t dims[4] = {(cuuint64_t)ny, (cuuint64_t)nz, (cuuint64_t)nx, (cuuint64_t)AR_COUNT};
+  const cuuint64_t strides[3] = {(cuuint64_t)c.nyp * 4, (cuuint64_t)nz * c.nyp * 4, (cuuint64_t)c.as * 4};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  const cuuint32_t box[4] = {(cuuint32_t)(pl.BY + 8), (cuuint32_t)(nz + 2), 1u, 3u};
+  return enc(&pl.mapS, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void*)(c.arrays + c.lead), dims, strides, box, estr,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+}  // namespace
+
+FusedPlan* fused_plan(Ctx& c) {
+  if (!c.fused_plan_tried) {
+    c.fused_plan_tried = true;
+    FusedPlan* pl = new FusedPlan();
+    if (build_plan(c, *pl)) c.fused_plan = pl;
+    else delete pl;
+  }
+  return c.fused_plan;
+}
+
+void fused_plan_free(Ctx& c) {
+  delete c.fused_plan;
+  c.fused_plan = nullptr;
+}
+
+// One Heun step = one launch; the result lands in the scratch spin buffer, which then becomes S.
+asd_status launch_heun_fused(Ctx& c, StageParams& p) {
+  FusedPlan* pl = fused_plan(c);
+  if (!pl) return ASD_EUNSUPPORTED;
+  FusedParams f;
+  f.arrays = c.arrays; f.arrays_w = c.arrays; f.as = (uint32_t)c.as;
+  f.aIn = c.aS; f.oOut = (uint32_t)c.aSt * f.as;
+  f.oSigma = AR_SIGMA * f.as; f.oB = AR_B * f.as;
+  f.col = p.col; f.grain = p.grain;
+  f.nx = c.d.nx; f.ny = c.d.ny; f.nz = c.d.nz; f.nyp = c.nyp; f.lead = c.lead;
+  f.BY = pl->BY; f.G = pl->G; f.nstrips = pl->nstrips; f.CX = pl->CX; f.n_main = pl->n_main;
+  f.slot_pitch = pl->slot_pitch;
+  f.j1 = p.jx[0]; f.j2 = p.jx[1]; f.j3 = p.jx[2];
+  f.gdt = p.gdt; f.lambda = p.lambda; f.scale = p.scale;
+  f.n_lo = p.n_lo; f.n_hi = p.n_hi; f.dyn = p.dyn; f.g0 = p.g0; f.key = p.key;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)(pl->nstrips * pl->nchunks)); cfg.blockDim = dim3((unsigned)pl->threads);
+  cfg.dynamicSmemBytes = pl->smem_bytes; cfg.stream = c.launch_stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  cudaLaunchKernelEx(&cfg, pl->kern, pl->mapS, f);
+  ASD_LAUNCH_CHECK(c, "heun step (fused)");
+  const int t = c.aS; c.aS = c.aSt; c.aSt = t;
+  return ASD_OK;
+}
+
+}  // namespace asd

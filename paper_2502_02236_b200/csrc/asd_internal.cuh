@@ -120,9 +120,9 @@ struct StageParams {
 };
 
 
-struct DemagPlan;           // asd_demag.cu: cuFFT plans, transformed tensor and buffers of the demagnetising field
-struct DemagPlan;           // asd_demag.cu: cuFFT plans, transformed tensor and buffers of the demagnetising field
+struct DemagPlan;           // asd_demag.cu: plans, transformed tensor and buffers of the demagnetising field
 struct TmaPlan;             // asd_heun_tma.cu: tensor maps + strip / chunk plan of the staged film kernel
+struct FusedPlan;           // asd_heun_fused.cu: tensor map + strip / chunk plan of the one-kernel Heun step
 
 struct Ctx {
   asd_lattice_desc d;          // host pointers inside are NOT valid after create
@@ -177,6 +177,8 @@ struct Ctx {
   int32_t demag_refresh = 3;        // this step: bit 0 = recompute before the predictor, bit 1 = before the corrector
   TmaPlan* tma_plan = nullptr;      // built lazily by the first staged launch (host memory, freed by asd_destroy)
   bool tma_plan_tried = false;
+  FusedPlan* fused_plan = nullptr;  // likewise for the fused one-kernel step
+  bool fused_plan_tried = false;
   int64_t launches = 0;
   bool cuda_failed = false;
   char err[256] = {0};
@@ -231,6 +233,11 @@ asd_status launch_heun_tma(Ctx& c, StageParams& p);           // one Heun step (
 bool heun_tma_supported(const Ctx& c);
 TmaPlan* tma_plan(Ctx& c);                                    // nullptr if the plan cannot be built
 void tma_plan_free(Ctx& c);
+asd_status launch_heun_fused(Ctx& c, StageParams& p);         // one Heun step (1 kernel); swaps the roles of the spin buffers
+bool heun_fused_supported(const Ctx& c);
+bool heun_fused_preferred(const Ctx& c);                      // what ASD_KERNEL_AUTO asks
+FusedPlan* fused_plan(Ctx& c);
+void fused_plan_free(Ctx& c);
 void fill_stage_params(const Ctx& c, StageParams& p);
 asd_status launch_shift(Ctx& c, int32_t p);
 asd_status launch_cell_frames(Ctx& c);

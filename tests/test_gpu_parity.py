@@ -177,8 +177,40 @@ def test_staged_tma_kernel(lattice, dims):
     _check_norm(g, w)
 
 
+@pytest.mark.parametrize("lattice", [ai.SC, ai.L10])
+@pytest.mark.parametrize("dims", [(21, 40, 7), (9, 4, 3), (3, 8, 3), (1, 8, 1), (40, 132, 9), (70, 220, 27), (300, 24, 2),
+                                  (37, 100, 12)])
+def test_fused_kernel(lattice, dims):
+    """The one-kernel Heun step (asd_heun_fused.cu): several strips, chunks of 1..many planes, ragged last strip and
+    chunk, halo columns and halo planes recomputed per CTA; odd and even numbers of steps (the spin buffers swap)."""
+    import paper_2502_02236_b200 as asd
+    nx, ny, nz = dims
+    w = ai.small_film(lattice, nx, ny, nz, tilt_deg=25.0, dt=1e-16)
+    o, g = oracle_from_workload(w), gpu_from_workload(w)
+    g.set_kernel(asd.KERNEL_FUSED)
+    o.step_heun(1); g.step_heun(1)
+    assert max_abs_diff(g, o) <= TOL_1STEP
+    _check_norm(g, w)
+    o.step_heun(3); g.step_heun(3)
+    assert max_abs_diff(g, o) <= 5e-5
+    _check_norm(g, w)
+
+
+def test_fused_kernel_matches_two_kernel_step_closely():
+    """Fused and two-kernel steps compute the same Heun step in different association orders: they agree to a few ulp,
+    and the fused step is bit-reproducible from run to run."""
+    import paper_2502_02236_b200 as asd
+    w = ai.small_film(ai.L10, 45, 72, 11, tilt_deg=25.0, dt=1e-16)
+    a, b, c = gpu_from_workload(w), gpu_from_workload(w), gpu_from_workload(w)
+    a.set_kernel(asd.KERNEL_FAST); b.set_kernel(asd.KERNEL_FUSED); c.set_kernel(asd.KERNEL_FUSED)
+    a.step_heun(5); b.step_heun(5); c.step_heun(5)
+    sa, sb, sc = a.get_spins_host(), b.get_spins_host(), c.get_spins_host()
+    assert np.array_equal(sb, sc)
+    assert float(np.abs(sa - sb).max()) <= 2e-6
+
+
 @pytest.mark.parametrize("cfg", [2, 4])
-@pytest.mark.parametrize("kernel", ["fast", "tma"])
+@pytest.mark.parametrize("kernel", ["fast", "tma", "fused"])
 def test_full_size_one_step(cfg, kernel):
     """BASELINE configs at full size in the launch configuration bench.py times: every site against the oracle."""
     w = ai.make_config(cfg)
@@ -187,7 +219,7 @@ def test_full_size_one_step(cfg, kernel):
     w.sx, w.sy, w.sz = sx * mag, sy * mag, sz * mag
     import paper_2502_02236_b200 as asd
     o, g = _full_size_oracle(cfg, w), gpu_from_workload(w)
-    g.set_kernel({"fast": asd.KERNEL_FAST, "tma": asd.KERNEL_TMA}[kernel])
+    g.set_kernel({"fast": asd.KERNEL_FAST, "tma": asd.KERNEL_TMA, "fused": asd.KERNEL_FUSED}[kernel])
     g.step_heun(2)
     assert float(np.abs(g.get_spins_host().astype(np.float64) - o).max()) <= 2e-5
     _check_norm(g, w)
