@@ -34,7 +34,8 @@ namespace asd {
 namespace {
 
 constexpr int LAT_SC = 0, LAT_L10 = 1;
-constexpr int kRing = 4;
+constexpr int kRingS = 4;      // S planes q-1, q, q+1 and the one in flight
+constexpr int kRingT = 3;      // S~ planes q-2, q-1, q
 
 struct FusedParams {
   const float* arrays;
@@ -48,68 +49,65 @@ struct FusedParams {
   int32_t BY, G, nstrips, CX;      // strip width (sites), y-groups per strip row, strips, planes per chunk
   int32_t n_main;                  // threads that own 4-site groups (a multiple of 32); the rest are halo threads
   uint32_t slot_pitch;             // bytes of one ring slot (multiple of 128)
-  float j1, j2, j3;
-  float gdt, lambda, scale;
+  // Every field term is carried pre-multiplied by -gamma dt / (1 + lambda^2), so that dt f = S x B' + lambda S x (S x B')
+  // needs no further scaling: j*s = -gdt J_shell / mu_s, ngdt = -gdt (applied to sigma, B_app and 2 k_u / mu_s on load).
+  float j1s, j2s, j3s;
+  float ngdt, lambda, scale;
   uint32_t n_lo, n_hi;
   const DynState* dyn;
   uint64_t g0;
   PhiloxKey key;
 };
 
-__device__ __forceinline__ void cta_barrier() { asm volatile("bar.sync 0;" ::: "memory"); }
-
-// dt f(X, B) of Eq. (1) in LL form (asd_site.cuh)
-__device__ __forceinline__ void llg_dt_f(const SiteConst& p, const float X[3], float B0, float B1, float B2, float f[3]) {
-  const float a0 = X[1] * B2 - X[2] * B1, a1 = X[2] * B0 - X[0] * B2, a2 = X[0] * B1 - X[1] * B0;   // S x B
-  const float b0 = X[1] * a2 - X[2] * a1, b1 = X[2] * a0 - X[0] * a2, b2 = X[0] * a1 - X[1] * a0;   // S x (S x B)
-  f[0] = -p.gdt * fmaf(p.lambda, b0, a0);
-  f[1] = -p.gdt * fmaf(p.lambda, b1, a1);
-  f[2] = -p.gdt * fmaf(p.lambda, b2, a2);
+// dt f(X, B) of Eq. (1) in LL form (asd_site.cuh) from the pre-scaled field B' = -gdt B:  S x B' + lambda S x (S x B')
+__device__ __forceinline__ void llg_dt_f(float lambda, const float X[3], float B0, float B1, float B2, float f[3]) {
+  const float a0 = X[1] * B2 - X[2] * B1, a1 = X[2] * B0 - X[0] * B2, a2 = X[0] * B1 - X[1] * B0;   // S x B'
+  const float b0 = X[1] * a2 - X[2] * a1, b1 = X[2] * a0 - X[0] * a2, b2 = X[0] * a1 - X[1] * a0;   // S x (S x B')
+  f[0] = fmaf(lambda, b0, a0);
+  f[1] = fmaf(lambda, b1, a1);
+  f[2] = fmaf(lambda, b2, a2);
 }
 
-// Exchange field of the 4 sites of a group from three ring slots (prev, cur, next = planes x-1, x, x+1); also returns
-// the group's own values X[c][0..3].  b = byte address of the group's own float4 in component 0 of slot `cur`.
-template <int LAT>
-__device__ __forceinline__ void exchange4(uint32_t prev, uint32_t cur, uint32_t next, uint32_t rowb, uint32_t compb,
-                                          float j1, float j2, float j3, float X[3][4], float Bex[3][4]) {
+// Adds the anisotropy field, Eq. (3), pre-scaled by -gdt, to the exchange field of the 4 sites of a group.  gp = the
+// group's (e_x, e_y, e_z, 2 k_u/mu_s), gathered by the caller ahead of time by the group's grain id; a group that holds
+// two different grains (rare, flagged at set-up) gathers per site here.  A vacant site may borrow any parameters: its
+// spin is 0.
+__device__ __forceinline__ void add_aniso(const float4* grain, float4 gp, bool mixed, const uint32_t* colp, float ngdt,
+                                          const float X[3][4], float Bex[3][4]) {
+  uint4 cc = make_uint4(0u, 0u, 0u, 0u);
+  if (mixed) cc = __ldg(reinterpret_cast<const uint4*>(colp));
+  const uint32_t id[4] = {cc.x & 0xFFFFu, cc.y & 0xFFFFu, cc.z & 0xFFFFu, cc.w & 0xFFFFu};
 #pragma unroll
-  for (int c = 0; c < 3; ++c) {
-    const uint32_t cb = (uint32_t)c * compb;
-    const float4 o = lds4(cur + cb);
-    const float oL = lds1(cur + cb - 4u), oR = lds1(cur + cb + 16u);
-    const float4 zp = lds4(cur + cb + rowb), zm = lds4(cur + cb - rowb);
-    const float4 xp = lds4(next + cb), xm = lds4(prev + cb);
-    const float own[6] = {oL, o.x, o.y, o.z, o.w, oR};
-    X[c][0] = o.x; X[c][1] = o.y; X[c][2] = o.z; X[c][3] = o.w;
-    const float zs[4] = {zp.x + zm.x, zp.y + zm.y, zp.z + zm.z, zp.w + zm.w};
-    if (LAT == LAT_SC) {
-      // 6 nearest neighbours, one J
-      const float xs[4] = {xp.x + xm.x, xp.y + xm.y, xp.z + xm.z, xp.w + xm.w};
-#pragma unroll
-      for (int v = 0; v < 4; ++v) Bex[c][v] = j1 * ((xs[v] + zs[v]) + (own[v] + own[v + 2]));
-    } else {
-      // 4 in-plane nn (J1), 2 out-of-plane (J2), 4 in-plane nnn (J3): "4 nearest + 6 next nearest"
-      float xs[6];
-      xs[0] = lds1(next + cb - 4u) + lds1(prev + cb - 4u);
-      xs[1] = xp.x + xm.x; xs[2] = xp.y + xm.y; xs[3] = xp.z + xm.z; xs[4] = xp.w + xm.w;
-      xs[5] = lds1(next + cb + 16u) + lds1(prev + cb + 16u);
-#pragma unroll
-      for (int v = 0; v < 4; ++v) {
-        const float s1 = xs[v + 1] + (own[v] + own[v + 2]);
-        const float s3 = xs[v] + xs[v + 2];
-        Bex[c][v] = fmaf(j3, s3, fmaf(j2, zs[v], j1 * s1));
-      }
-    }
+  for (int v = 0; v < 4; ++v) {
+    float4 gv = gp;
+    if (mixed) gv = __ldg(grain + id[v]);
+    const float ca = (ngdt * gv.w) * fmaf(X[0][v], gv.x, fmaf(X[1][v], gv.y, X[2][v] * gv.z));
+    Bex[0][v] = fmaf(ca, gv.x, Bex[0][v]); Bex[1][v] = fmaf(ca, gv.y, Bex[1][v]); Bex[2][v] = fmaf(ca, gv.z, Bex[2][v]);
   }
+}
+// grain id of a group (the largest of its 4 columns' ids: vacant columns are 0) | bit 31: the group holds two grains
+__device__ __forceinline__ uint32_t pack_group(uint4 cid4) {
+  const uint32_t gid = max(max(cid4.x & 0xFFFFu, cid4.y & 0xFFFFu), max(cid4.z & 0xFFFFu, cid4.w & 0xFFFFu));
+  return gid | ((cid4.x & COL_GROUP_MIXED) ? 0x80000000u : 0u);
+}
+
+// Mbarrier with one arrival per warp: the split barrier of the march.
+__device__ __forceinline__ void warp_arrive(uint32_t bar) {
+  __syncwarp();
+  if ((threadIdx.x & 31u) == 0u) mbar_arrive(bar);
 }
 
 template <int LAT, int NT, int MINB>
-__global__ void __launch_bounds__(NT, MINB) heun_fused(const __grid_constant__ CUtensorMap mapS, const FusedParams p) {
+__global__ void __launch_bounds__(NT, MINB)
+heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUtensorMap mapF, const FusedParams p) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const uint32_t sm0 = smem_u32(smem_raw);
-  const uint32_t bar_full = sm0;
+  const uint32_t bar_full = sm0;                      // S plane landed (TMA transaction count)
+  const uint32_t bar_done = sm0 + 32u;                // S~ plane complete (one arrival per warp)
+  const uint32_t bar_fld = sm0 + 64u;                 // sigma / B plane landed
   const uint32_t sring = sm0 + 128u;
-  const uint32_t tring = sring + kRing * p.slot_pitch;
+  const uint32_t tring = sring + kRingS * p.slot_pitch;
+  const uint32_t fbox = tring + kRingT * p.slot_pitch;
 
   const int tid = (int)threadIdx.x;
   const int strip = (int)blockIdx.x % p.nstrips, chunk = (int)blockIdx.x / p.nstrips;
@@ -119,43 +117,55 @@ __global__ void __launch_bounds__(NT, MINB) heun_fused(const __grid_constant__ C
   const int W = p.BY + 8, R = p.nz + 2;
   const uint32_t rowb = (uint32_t)(W * 4), compb = (uint32_t)(R * W * 4);
   const uint32_t box_bytes = 3u * compb;
+  const uint32_t fcomp = (uint32_t)(p.nz * p.BY * 4), fbytes = 4u * fcomp;
 
   // S~ ring starts as zeros: the rows z = -1 and z = nz, and the columns of a ragged last strip, are never written.
-  for (uint32_t o = (uint32_t)tid * 16u; o < kRing * p.slot_pitch; o += (uint32_t)blockDim.x * 16u)
+  for (uint32_t o = (uint32_t)tid * 16u; o < kRingT * p.slot_pitch; o += (uint32_t)blockDim.x * 16u)
     sts4(tring + o, 0.0f, 0.0f, 0.0f, 0.0f);
   if (tid == 0) {
-    for (int s = 0; s < kRing; ++s) mbar_init(bar_full + 8u * s, 1u);
+    for (int s = 0; s < 4; ++s) { mbar_init(bar_full + 8u * s, 1u); mbar_init(bar_done + 8u * s, blockDim.x / 32u); }
+    mbar_init(bar_fld, 1u);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
   // Programmatic dependent launch: everything above overlaps the tail of the previous step's grid; nothing below the
   // wait runs before that grid has completed (it wrote the spins this one reads and read the buffer this one writes).
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-  cta_barrier();
+  asm volatile("bar.sync 0;" ::: "memory");
   asm volatile("griddepcontrol.wait;" ::: "memory");
 
-  // ring plane u (u = 0 is window plane i0 - 2) -> slot u % 4
-  auto issue = [&](int u) {
-    const uint32_t s = (uint32_t)(u & (kRing - 1));
-    const uint32_t bar = bar_full + 8u * s;
-    mbar_expect_tx(bar, box_bytes);
-    tma_load_4d(sring + s * p.slot_pitch, &mapS, bar, j0 - 4, -1, i0 - 2 + u, p.aIn);
+  // S ring plane u (u = 0 is window plane i0 - 2) -> slot u % 4;  field plane of march step m = window plane i0 - 1 + m
+  auto issue_S = [&](int u) {
+    const uint32_t s = (uint32_t)(u & (kRingS - 1));
+    mbar_expect_tx(bar_full + 8u * s, box_bytes);
+    tma_load_4d(sring + s * p.slot_pitch, &mapS, bar_full + 8u * s, j0 - 4, -1, i0 - 2 + u, p.aIn);
   };
-  if (tid == 0)
-    for (int u = 0; u < kRing; ++u) issue(u);          // L >= 1: planes u = 0 .. L+3 are all needed
+  auto issue_F = [&](int m) {
+    mbar_expect_tx(bar_fld, fbytes);
+    tma_load_4d(fbox, &mapF, bar_fld, j0, 0, i0 - 1 + m, AR_SIGMA);
+  };
+  if (tid == 0) {
+    for (int u = 0; u < kRingS; ++u) issue_S(u);       // L >= 1: planes u = 0 .. L+3 are all needed
+    issue_F(0);
+    for (int m = 1; m <= 3 && m <= L + 1; ++m) tma_prefetch_4d(&mapF, j0, 0, i0 - 1 + m, AR_SIGMA);
+  }
 
   uint32_t n_lo = p.n_lo, n_hi = p.n_hi; float scale = p.scale;
   resolve_dyn(p.dyn, n_lo, n_hi, scale);
-  const SiteConst sc{p.gdt, p.lambda, scale};
-  const float* __restrict__ base = p.arrays;
+  const float sscale = p.ngdt * scale;                // B'_app = sscale * B
+  const float lambda = p.lambda;
   const uint32_t planep = (uint32_t)(p.nz * p.nyp);
+  auto done_bar = [&](int m) { return bar_done + 8u * (uint32_t)(m & 3); };
+  auto phase = [](int m) { return (uint32_t)(m >> 2) & 1u; };
 
   if (tid < p.n_main) {
     // ================= main threads: 4 consecutive y-sites of one z-row, predictor and corrector =================
     const int k = tid / p.G, g = tid - k * p.G;
     const int j = j0 + 4 * g;
     const bool active = (k < p.nz) && (j < p.ny);
-    const uint32_t own_b = (uint32_t)(((k + 1) * W + 4 + 4 * g) * 4);   // own float4 inside component 0 of a slot
+    // own float4 inside component 0 of a slot (inactive threads read a valid dummy position and write nothing)
+    const uint32_t own_b = active ? (uint32_t)(((k + 1) * W + 4 + 4 * g) * 4) : (uint32_t)((W + 4) * 4);
+    const uint32_t fown = fbox + (active ? (uint32_t)((k * p.BY + 4 * g) * 4) : 0u);
     // element of the group in predictor plane q = i0 - 1 (wraps below zero for q = -1; not dereferenced then)
     uint32_t e = (uint32_t)(p.lead + ((i0 - 1) * p.nz + k) * p.nyp + j);
     uint32_t ec = (uint32_t)((i0 - 1) * p.ny + j);                      // column (q, j) of the window
@@ -164,148 +174,221 @@ __global__ void __launch_bounds__(NT, MINB) heun_fused(const __grid_constant__ C
 
     // carried from the predictor of plane q to its corrector one march step later
     float A[3][4], Bs[3][4];
-    uint32_t gid_c = 0u; bool mixed_c = false;
 #pragma unroll
     for (int c = 0; c < 3; ++c)
 #pragma unroll
       for (int v = 0; v < 4; ++v) { A[c][v] = 0.0f; Bs[c][v] = 0.0f; }
+    // packed grain id of the group in plane q (cgN: ready one march step ahead, so that the parameter gather does not
+    // wait for the column table) and in plane q - 1 (cgC)
+    uint32_t cgN = (active && i0 >= 1) ? pack_group(__ldg(reinterpret_cast<const uint4*>(p.col + ec))) : 0u, cgC = 0u;
+    // L1_0 only: the y-1 / y+4 edge columns of the group's row are 16-byte-strided scalar reads (4 shared-memory
+    // wavefronts each); every plane's pair is read once and kept while the plane is the x+1, own and x-1 plane.
+    float sP[3][2], sC[3][2];      // S edges of planes q-1, q
+    float tP[3][2], tC[3][2];      // S~ edges of planes q-2, q-1
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { sP[c][0] = sP[c][1] = sC[c][0] = sC[c][1] = tP[c][0] = tP[c][1] = tC[c][0] = tC[c][1] = 0.0f; }
 
-    mbar_wait(bar_full + 0u, 0u);
-    mbar_wait(bar_full + 8u, 0u);
+    mbar_wait_long(bar_full + 0u, 0u);
+    mbar_wait_long(bar_full + 8u, 0u);
+    if (LAT == LAT_L10) {
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        const uint32_t a0 = sring + own_b + (uint32_t)c * compb, a1 = a0 + p.slot_pitch;
+        sP[c][0] = lds1(a0 - 4u); sP[c][1] = lds1(a0 + 16u);
+        sC[c][0] = lds1(a1 - 4u); sC[c][1] = lds1(a1 + 16u);
+      }
+    }
+    uint32_t t3 = 0u;                                  // m % 3: S~ slot of plane q
 
     for (int m = 0; m <= L + 1; ++m) {
       const int q = i0 - 1 + m;
       const bool qvalid = active && (q >= 0) && (q < p.nx);
-      // streaming inputs of the predictor plane: issued first, used after the wait
-      float4 sg4 = make_float4(0.f, 0.f, 0.f, 0.f), bx4 = sg4, by4 = sg4, bz4 = sg4;
+      const uint32_t tN = tring + t3 * p.slot_pitch + own_b;                                   // S~ plane q
+      const uint32_t tCs = tring + (t3 == 0u ? 2u : t3 - 1u) * p.slot_pitch + own_b;           // q - 1
+      const uint32_t tPs = tring + (t3 == 2u ? 0u : t3 + 1u) * p.slot_pitch + own_b;           // q - 2
+      // issued first, used after the exchange sums: the group's anisotropy parameters, next plane's column entries
+      const float4 gpN = __ldg(p.grain + (cgN & 0xFFFFu));
       uint4 cid4 = make_uint4(0u, 0u, 0u, 0u);
-      if (qvalid) {
-        sg4 = ldg_stream4(base + (p.oSigma + e));
-        bx4 = ldg_stream4(base + (p.oB + e));
-        by4 = ldg_stream4(base + (p.oB + p.as + e));
-        bz4 = ldg_stream4(base + (p.oB + 2u * p.as + e));
-        cid4 = __ldg(reinterpret_cast<const uint4*>(p.col + ec));
-      }
-      mbar_wait(bar_full + 8u * (uint32_t)((m + 2) & (kRing - 1)), (uint32_t)((m + 2) >> 2) & 1u);   // plane q + 1
+      if (active && q + 1 >= 0 && q + 1 < p.nx) cid4 = __ldg(reinterpret_cast<const uint4*>(p.col + (ec + (uint32_t)p.ny)));
+      mbar_wait_long(bar_full + 8u * (uint32_t)((m + 2) & (kRingS - 1)), phase(m + 2));   // S plane q + 1
 
-      float An[3][4], Bn[3][4];                        // this plane's A and sigma xi + s B_app
-      uint32_t gid_n = 0u; bool mixed_n = false;
-      const uint32_t tslot = tring + (uint32_t)(m & (kRing - 1)) * p.slot_pitch + own_b;
-      if (qvalid) {
-        // ---- noise: one Philox block per site per STEP ----
-        const float sg[4] = {sg4.x, sg4.y, sg4.z, sg4.w};
-        const float bx[4] = {bx4.x, bx4.y, bx4.z, bx4.w}, by[4] = {by4.x, by4.y, by4.z, by4.w},
-                    bz[4] = {bz4.x, bz4.y, bz4.z, bz4.w};
-#pragma unroll
-        for (int v = 0; v < 4; ++v) {
-          uint32_t rnd[4];
-          philox_site(p.key, n_lo, n_hi, gsite + (uint64_t)v, 0u, rnd);
-          float xi[3];
-          normals3(rnd, xi);
-          Bn[0][v] = fmaf(sg[v], xi[0], scale * bx[v]);
-          Bn[1][v] = fmaf(sg[v], xi[1], scale * by[v]);
-          Bn[2][v] = fmaf(sg[v], xi[2], scale * bz[v]);
-        }
-        // ---- predictor: S~ = normalise(S + dt k1), A = S + dt/2 k1 ----
-        const uint32_t prev = sring + (uint32_t)(m & (kRing - 1)) * p.slot_pitch + own_b;
-        const uint32_t cur = sring + (uint32_t)((m + 1) & (kRing - 1)) * p.slot_pitch + own_b;
-        const uint32_t next = sring + (uint32_t)((m + 2) & (kRing - 1)) * p.slot_pitch + own_b;
+      // ---- predictor of plane q: S~ = normalise(S + dt k1), A = S + dt/2 k1 ----
+      float An[3][4], Bn[3][4];                        // this plane's A and -gdt (sigma xi + s B_app)
+      {
+        const uint32_t prev = sring + (uint32_t)(m & 3) * p.slot_pitch + own_b;
+        const uint32_t cur = sring + (uint32_t)((m + 1) & 3) * p.slot_pitch + own_b;
+        const uint32_t next = sring + (uint32_t)((m + 2) & 3) * p.slot_pitch + own_b;
         float X[3][4], Bex[3][4];
-        exchange4<LAT>(prev, cur, next, rowb, compb, p.j1, p.j2, p.j3, X, Bex);
-        gid_n = max(max(cid4.x & 0xFFFFu, cid4.y & 0xFFFFu), max(cid4.z & 0xFFFFu, cid4.w & 0xFFFFu));
-        mixed_n = (cid4.x & COL_GROUP_MIXED) != 0u;
-        float4 gp4[4];
-        gp4[0] = gp4[1] = gp4[2] = gp4[3] = __ldg(p.grain + gid_n);
-        if (mixed_n) {
-          gp4[0] = __ldg(p.grain + (cid4.x & 0xFFFFu)); gp4[1] = __ldg(p.grain + (cid4.y & 0xFFFFu));
-          gp4[2] = __ldg(p.grain + (cid4.z & 0xFFFFu)); gp4[3] = __ldg(p.grain + (cid4.w & 0xFFFFu));
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          const uint32_t cb = (uint32_t)c * compb;
+          const float4 o = lds4(cur + cb);
+          const float4 zp = lds4(cur + cb + rowb), zm = lds4(cur + cb - rowb);
+          const float4 xp = lds4(next + cb), xm = lds4(prev + cb);
+          X[c][0] = o.x; X[c][1] = o.y; X[c][2] = o.z; X[c][3] = o.w;
+          const float zs[4] = {zp.x + zm.x, zp.y + zm.y, zp.z + zm.z, zp.w + zm.w};
+          if (LAT == LAT_SC) {
+            // 6 nearest neighbours, one J
+            const float own[6] = {lds1(cur + cb - 4u), o.x, o.y, o.z, o.w, lds1(cur + cb + 16u)};
+            const float xs[4] = {xp.x + xm.x, xp.y + xm.y, xp.z + xm.z, xp.w + xm.w};
+#pragma unroll
+            for (int v = 0; v < 4; ++v) Bex[c][v] = p.j1s * ((xs[v] + zs[v]) + (own[v] + own[v + 2]));
+          } else {
+            // 4 in-plane nn (J1), 2 out-of-plane (J2), 4 in-plane nnn (J3): "4 nearest + 6 next nearest"
+            const float nL = lds1(next + cb - 4u), nR = lds1(next + cb + 16u);
+            const float own[6] = {sC[c][0], o.x, o.y, o.z, o.w, sC[c][1]};
+            const float xs[6] = {nL + sP[c][0], xp.x + xm.x, xp.y + xm.y, xp.z + xm.z, xp.w + xm.w, nR + sP[c][1]};
+#pragma unroll
+            for (int v = 0; v < 4; ++v) {
+              const float s1 = xs[v + 1] + (own[v] + own[v + 2]);
+              const float s3 = xs[v] + xs[v + 2];
+              Bex[c][v] = fmaf(p.j3s, s3, fmaf(p.j2s, zs[v], p.j1s * s1));
+            }
+            sP[c][0] = sC[c][0]; sP[c][1] = sC[c][1]; sC[c][0] = nL; sC[c][1] = nR;
+          }
+        }
+        add_aniso(p.grain, gpN, (cgN >> 31) != 0u, p.col + ec, p.ngdt, X, Bex);
+        // ---- noise: one Philox block per site per STEP; sigma and B of the plane come from the staged field box ----
+        mbar_wait_long(bar_fld, (uint32_t)m & 1u);
+        {
+          const float4 sg4 = lds4(fown), bx4 = lds4(fown + fcomp), by4 = lds4(fown + 2u * fcomp), bz4 = lds4(fown + 3u * fcomp);
+          const float sg[4] = {sg4.x, sg4.y, sg4.z, sg4.w};
+          const float bx[4] = {bx4.x, bx4.y, bx4.z, bx4.w}, by[4] = {by4.x, by4.y, by4.z, by4.w},
+                      bz[4] = {bz4.x, bz4.y, bz4.z, bz4.w};
+#pragma unroll
+          for (int v = 0; v < 4; ++v) {
+            uint32_t rnd[4];
+            philox_site(p.key, n_lo, n_hi, gsite + (uint64_t)v, 0u, rnd);
+            float xi[3];
+            normals3(rnd, xi);
+            const float sgs = p.ngdt * sg[v];
+            Bn[0][v] = fmaf(sgs, xi[0], sscale * bx[v]);
+            Bn[1][v] = fmaf(sgs, xi[1], sscale * by[v]);
+            Bn[2][v] = fmaf(sgs, xi[2], sscale * bz[v]);
+          }
         }
         float St[3][4];
 #pragma unroll
         for (int v = 0; v < 4; ++v) {
           const float Xs[3] = {X[0][v], X[1][v], X[2][v]};
-          const float4 gp = gp4[v];
-          const float ca = gp.w * fmaf(Xs[0], gp.x, fmaf(Xs[1], gp.y, Xs[2] * gp.z));     // Eq. (3)
           float f[3];
-          llg_dt_f(sc, Xs, fmaf(ca, gp.x, Bex[0][v]) + Bn[0][v], fmaf(ca, gp.y, Bex[1][v]) + Bn[1][v],
-                   fmaf(ca, gp.z, Bex[2][v]) + Bn[2][v], f);
+          llg_dt_f(lambda, Xs, Bex[0][v] + Bn[0][v], Bex[1][v] + Bn[1][v], Bex[2][v] + Bn[2][v], f);
           An[0][v] = fmaf(0.5f, f[0], Xs[0]); An[1][v] = fmaf(0.5f, f[1], Xs[1]); An[2][v] = fmaf(0.5f, f[2], Xs[2]);
           float o[3];
           normalise3(Xs[0] + f[0], Xs[1] + f[1], Xs[2] + f[2], o);
           St[0][v] = o[0]; St[1][v] = o[1]; St[2][v] = o[2];
         }
+        // a plane outside the window has S = 0 everywhere (TMA fill), hence S~ = 0: the open boundary in x
+        if (active) {
 #pragma unroll
-        for (int c = 0; c < 3; ++c) sts4(tslot + (uint32_t)c * compb, St[c][0], St[c][1], St[c][2], St[c][3]);
-      } else {
-#pragma unroll
-        for (int c = 0; c < 3; ++c)
-#pragma unroll
-          for (int v = 0; v < 4; ++v) { An[c][v] = 0.0f; Bn[c][v] = 0.0f; }
-        if (active) {                                  // a plane outside the window: S~ = 0 (open boundary in x)
-#pragma unroll
-          for (int c = 0; c < 3; ++c) sts4(tslot + (uint32_t)c * compb, 0.0f, 0.0f, 0.0f, 0.0f);
+          for (int c = 0; c < 3; ++c) sts4(tN + (uint32_t)c * compb, St[c][0], St[c][1], St[c][2], St[c][3]);
         }
       }
-      cta_barrier();                                   // S~ plane q is complete; S plane q - 1 has been read for the last time
-      if (tid == 0 && m + kRing <= L + 3) issue(m + kRing);
+      warp_arrive(done_bar(m));                        // this warp's share of S~ plane q is written
 
-      // ---- corrector of plane q - 1: S = normalise(A + dt/2 k2), k2 from S~ ----
-      if (active && m >= 2) {
-        const uint32_t prev = tring + (uint32_t)((m - 2) & (kRing - 1)) * p.slot_pitch + own_b;
-        const uint32_t cur = tring + (uint32_t)((m - 1) & (kRing - 1)) * p.slot_pitch + own_b;
-        const uint32_t next = tring + (uint32_t)(m & (kRing - 1)) * p.slot_pitch + own_b;
-        float X[3][4], Bex[3][4];
-        exchange4<LAT>(prev, cur, next, rowb, compb, p.j1, p.j2, p.j3, X, Bex);
-        float4 gp4[4];
-        gp4[0] = gp4[1] = gp4[2] = gp4[3] = __ldg(p.grain + gid_c);
-        if (mixed_c) {
-          const uint4 cc = __ldg(reinterpret_cast<const uint4*>(p.col + (ec - (uint32_t)p.ny)));
-          gp4[0] = __ldg(p.grain + (cc.x & 0xFFFFu)); gp4[1] = __ldg(p.grain + (cc.y & 0xFFFFu));
-          gp4[2] = __ldg(p.grain + (cc.z & 0xFFFFu)); gp4[3] = __ldg(p.grain + (cc.w & 0xFFFFu));
+      // ---- corrector of plane q - 1, first part: everything that does not need S~ plane q ----
+      const bool do_corr = active && (m >= 2);
+      const float4 gpC = __ldg(p.grain + (cgC & 0xFFFFu));
+      float X[3][4], Bp[3][4];
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        const uint32_t cb = (uint32_t)c * compb;
+        const float4 o = lds4(tCs + cb);
+        const float4 zp = lds4(tCs + cb + rowb), zm = lds4(tCs + cb - rowb);
+        const float4 xm = lds4(tPs + cb);
+        X[c][0] = o.x; X[c][1] = o.y; X[c][2] = o.z; X[c][3] = o.w;
+        const float zs[4] = {zp.x + zm.x, zp.y + zm.y, zp.z + zm.z, zp.w + zm.w};
+        if (LAT == LAT_SC) {
+          const float own[6] = {lds1(tCs + cb - 4u), o.x, o.y, o.z, o.w, lds1(tCs + cb + 16u)};
+          const float xmv[4] = {xm.x, xm.y, xm.z, xm.w};
+#pragma unroll
+          for (int v = 0; v < 4; ++v) Bp[c][v] = p.j1s * ((xmv[v] + zs[v]) + (own[v] + own[v + 2]));
+        } else {
+          const float own[6] = {tC[c][0], o.x, o.y, o.z, o.w, tC[c][1]};
+          const float xmv[6] = {tP[c][0], xm.x, xm.y, xm.z, xm.w, tP[c][1]};
+#pragma unroll
+          for (int v = 0; v < 4; ++v) {
+            const float s1 = xmv[v + 1] + (own[v] + own[v + 2]);
+            const float s3 = xmv[v] + xmv[v + 2];
+            Bp[c][v] = fmaf(p.j3s, s3, fmaf(p.j2s, zs[v], p.j1s * s1));
+          }
         }
+      }
+      add_aniso(p.grain, gpC, (cgC >> 31) != 0u, p.col + (ec - (uint32_t)p.ny), p.ngdt, X, Bp);
+#pragma unroll
+      for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int v = 0; v < 4; ++v) Bp[c][v] += Bs[c][v];
+
+      mbar_wait_long(done_bar(m), phase(m));           // S~ plane q complete; S plane q - 1 and the field box are free
+      if (tid == 0) {
+        if (m + kRingS <= L + 3) issue_S(m + kRingS);
+        if (m + 1 <= L + 1) issue_F(m + 1);
+        if (m + 4 <= L + 1) tma_prefetch_4d(&mapF, j0, 0, i0 - 1 + m + 4, AR_SIGMA);
+      }
+
+      // ---- second part: the x+1 plane, torque, update, store ----
+      {
         float So[3][4];
 #pragma unroll
-        for (int v = 0; v < 4; ++v) {
-          const float Xs[3] = {X[0][v], X[1][v], X[2][v]};
-          const float4 gp = gp4[v];
-          const float ca = gp.w * fmaf(Xs[0], gp.x, fmaf(Xs[1], gp.y, Xs[2] * gp.z));
-          float f[3];
-          llg_dt_f(sc, Xs, fmaf(ca, gp.x, Bex[0][v]) + Bs[0][v], fmaf(ca, gp.y, Bex[1][v]) + Bs[1][v],
-                   fmaf(ca, gp.z, Bex[2][v]) + Bs[2][v], f);
-          float o[3];
-          normalise3(fmaf(0.5f, f[0], A[0][v]), fmaf(0.5f, f[1], A[1][v]), fmaf(0.5f, f[2], A[2][v]), o);
-          So[0][v] = o[0]; So[1][v] = o[1]; So[2][v] = o[2];
-        }
-        const uint32_t eo = e - planep;                // plane q - 1
+        for (int c = 0; c < 3; ++c) {
+          const uint32_t cb = (uint32_t)c * compb;
+          const float4 xp = lds4(tN + cb);
+          if (LAT == LAT_SC) {
+            Bp[c][0] = fmaf(p.j1s, xp.x, Bp[c][0]); Bp[c][1] = fmaf(p.j1s, xp.y, Bp[c][1]);
+            Bp[c][2] = fmaf(p.j1s, xp.z, Bp[c][2]); Bp[c][3] = fmaf(p.j1s, xp.w, Bp[c][3]);
+          } else {
+            const float nL = lds1(tN + cb - 4u), nR = lds1(tN + cb + 16u);
+            const float xpv[6] = {nL, xp.x, xp.y, xp.z, xp.w, nR};
 #pragma unroll
-        for (int c = 0; c < 3; ++c)
-          *reinterpret_cast<float4*>(p.arrays_w + (p.oOut + (uint32_t)c * p.as + eo)) =
-              make_float4(So[c][0], So[c][1], So[c][2], So[c][3]);
+            for (int v = 0; v < 4; ++v) Bp[c][v] = fmaf(p.j1s, xpv[v + 1], fmaf(p.j3s, xpv[v] + xpv[v + 2], Bp[c][v]));
+            tP[c][0] = tC[c][0]; tP[c][1] = tC[c][1]; tC[c][0] = nL; tC[c][1] = nR;
+          }
+        }
+        if (do_corr) {
+#pragma unroll
+          for (int v = 0; v < 4; ++v) {
+            const float Xs[3] = {X[0][v], X[1][v], X[2][v]};
+            float f[3];
+            llg_dt_f(lambda, Xs, Bp[0][v], Bp[1][v], Bp[2][v], f);
+            float o[3];
+            normalise3(fmaf(0.5f, f[0], A[0][v]), fmaf(0.5f, f[1], A[1][v]), fmaf(0.5f, f[2], A[2][v]), o);
+            So[0][v] = o[0]; So[1][v] = o[1]; So[2][v] = o[2];
+          }
+          const uint32_t eo = e - planep;              // plane q - 1
+#pragma unroll
+          for (int c = 0; c < 3; ++c)
+            *reinterpret_cast<float4*>(p.arrays_w + (p.oOut + (uint32_t)c * p.as + eo)) =
+                make_float4(So[c][0], So[c][1], So[c][2], So[c][3]);
+        }
       }
 #pragma unroll
       for (int c = 0; c < 3; ++c)
 #pragma unroll
         for (int v = 0; v < 4; ++v) { A[c][v] = An[c][v]; Bs[c][v] = Bn[c][v]; }
-      gid_c = gid_n; mixed_c = mixed_n;
+      cgC = cgN; cgN = pack_group(cid4);
       e += planep; ec += (uint32_t)p.ny; gsite += gplane;
+      t3 = (t3 == 2u) ? 0u : t3 + 1u;
     }
   } else {
     // ================= halo threads: the two sites (y = j0 - 1, y = j0 + BY) of one z-row, predictor only =================
     // Lanes of a warp read the same column of different rows (a bank-conflicted pattern), so each halo thread keeps
     // the three columns around its sites for planes q-1, q in registers and loads only plane q+1's and the z
     // neighbours of plane q per march step.
+    const float* __restrict__ base = p.arrays;
     const int k = tid - p.n_main;
     const bool row_ok = k < p.nz;
     const int jh[2] = {j0 - 1, j0 + p.BY};
     const bool act[2] = {row_ok && jh[0] >= 0, row_ok && jh[1] < p.ny};
-    const uint32_t own_b[2] = {(uint32_t)(((k + 1) * W + 3) * 4), (uint32_t)(((k + 1) * W + 4 + p.BY) * 4)};
+    const int kk = row_ok ? k : 0;
+    const uint32_t own_b[2] = {(uint32_t)(((kk + 1) * W + 3) * 4), (uint32_t)(((kk + 1) * W + 4 + p.BY) * 4)};
     uint32_t e = (uint32_t)(p.lead + ((i0 - 1) * p.nz + k) * p.nyp);          // + jh
     uint32_t ec = (uint32_t)((i0 - 1) * p.ny);
     uint64_t gsite = p.g0 + (uint64_t)(int64_t)(((int64_t)(i0 - 1) * p.nz + k) * p.ny);
     const uint32_t gplane = (uint32_t)(p.nz * p.ny);
 
-    mbar_wait(bar_full + 0u, 0u);
-    mbar_wait(bar_full + 8u, 0u);
+    mbar_wait_long(bar_full + 0u, 0u);
+    mbar_wait_long(bar_full + 8u, 0u);
     // window: rP = plane q-1, rC = plane q; [side][component][column y-1, y, y+1]
     float rP[2][3][3], rC[2][3][3];
 #pragma unroll
@@ -315,9 +398,10 @@ __global__ void __launch_bounds__(NT, MINB) heun_fused(const __grid_constant__ C
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
           const uint32_t off = own_b[s] + (uint32_t)c * compb + (uint32_t)(4 * d) - 4u;
-          rP[s][c][d] = row_ok ? lds1(sring + off) : 0.0f;
-          rC[s][c][d] = row_ok ? lds1(sring + p.slot_pitch + off) : 0.0f;
+          rP[s][c][d] = lds1(sring + off);
+          rC[s][c][d] = lds1(sring + p.slot_pitch + off);
         }
+    uint32_t t3 = 0u;
 
     for (int m = 0; m <= L + 1; ++m) {
       const int q = i0 - 1 + m;
@@ -328,17 +412,17 @@ __global__ void __launch_bounds__(NT, MINB) heun_fused(const __grid_constant__ C
       for (int s = 0; s < 2; ++s)
         if (act[s] && qin) {
           const uint32_t es = e + (uint32_t)jh[s];
+          cid[s] = __ldg(p.col + (ec + (uint32_t)jh[s]));
           sg[s] = ldg_stream1(base + (p.oSigma + es));
           bx[s] = ldg_stream1(base + (p.oB + es));
           by[s] = ldg_stream1(base + (p.oB + p.as + es));
           bz[s] = ldg_stream1(base + (p.oB + 2u * p.as + es));
-          cid[s] = __ldg(p.col + (ec + (uint32_t)jh[s]));
         }
-      mbar_wait(bar_full + 8u * (uint32_t)((m + 2) & (kRing - 1)), (uint32_t)((m + 2) >> 2) & 1u);
-      const uint32_t cur = sring + (uint32_t)((m + 1) & (kRing - 1)) * p.slot_pitch;
-      const uint32_t next = sring + (uint32_t)((m + 2) & (kRing - 1)) * p.slot_pitch;
-      const uint32_t tslot = tring + (uint32_t)(m & (kRing - 1)) * p.slot_pitch;
+      mbar_wait_long(bar_full + 8u * (uint32_t)((m + 2) & (kRingS - 1)), phase(m + 2));
+      const uint32_t cur = sring + (uint32_t)((m + 1) & 3) * p.slot_pitch, next = sring + (uint32_t)((m + 2) & 3) * p.slot_pitch;
+      const uint32_t tslot = tring + t3 * p.slot_pitch;
       float rN[2][3][3];
+      float o[2][3];
 #pragma unroll
       for (int s = 0; s < 2; ++s) {
         float zs[3];
@@ -346,9 +430,10 @@ __global__ void __launch_bounds__(NT, MINB) heun_fused(const __grid_constant__ C
         for (int c = 0; c < 3; ++c) {
           const uint32_t off = own_b[s] + (uint32_t)c * compb;
 #pragma unroll
-          for (int d = 0; d < 3; ++d) rN[s][c][d] = row_ok ? lds1(next + off + (uint32_t)(4 * d) - 4u) : 0.0f;
-          zs[c] = row_ok ? lds1(cur + off + rowb) + lds1(cur + off - rowb) : 0.0f;
+          for (int d = 0; d < 3; ++d) rN[s][c][d] = lds1(next + off + (uint32_t)(4 * d) - 4u);
+          zs[c] = lds1(cur + off + rowb) + lds1(cur + off - rowb);
         }
+        o[s][0] = o[s][1] = o[s][2] = 0.0f;
         if (act[s] && qin) {
           uint32_t rnd[4];
           philox_site(p.key, n_lo, n_hi, gsite + (uint64_t)(int64_t)jh[s], 0u, rnd);
@@ -361,28 +446,36 @@ __global__ void __launch_bounds__(NT, MINB) heun_fused(const __grid_constant__ C
             const float ys = rC[s][c][0] + rC[s][c][2];
             const float xs = rN[s][c][1] + rP[s][c][1];
             if (LAT == LAT_SC) {
-              Bex[c] = p.j1 * ((xs + zs[c]) + ys);
+              Bex[c] = p.j1s * ((xs + zs[c]) + ys);
             } else {
               const float s3 = (rN[s][c][0] + rP[s][c][0]) + (rN[s][c][2] + rP[s][c][2]);
-              Bex[c] = fmaf(p.j3, s3, fmaf(p.j2, zs[c], p.j1 * (xs + ys)));
+              Bex[c] = fmaf(p.j3s, s3, fmaf(p.j2s, zs[c], p.j1s * (xs + ys)));
             }
           }
-          const float4 gp = __ldg(p.grain + (cid[s] & 0xFFFFu));
+          float4 gp = __ldg(p.grain + (cid[s] & 0xFFFFu));
+          gp.w *= p.ngdt;
           const float ca = gp.w * fmaf(Xs[0], gp.x, fmaf(Xs[1], gp.y, Xs[2] * gp.z));
+          const float sgs = p.ngdt * sg[s];
           float f[3];
-          llg_dt_f(sc, Xs, fmaf(ca, gp.x, Bex[0]) + fmaf(sg[s], xi[0], scale * bx[s]),
-                   fmaf(ca, gp.y, Bex[1]) + fmaf(sg[s], xi[1], scale * by[s]),
-                   fmaf(ca, gp.z, Bex[2]) + fmaf(sg[s], xi[2], scale * bz[s]), f);
-          float o[3];
-          normalise3(Xs[0] + f[0], Xs[1] + f[1], Xs[2] + f[2], o);
-#pragma unroll
-          for (int c = 0; c < 3; ++c) sts1(tslot + own_b[s] + (uint32_t)c * compb, o[c]);
-        } else if (act[s]) {
-#pragma unroll
-          for (int c = 0; c < 3; ++c) sts1(tslot + own_b[s] + (uint32_t)c * compb, 0.0f);
+          llg_dt_f(lambda, Xs, fmaf(ca, gp.x, Bex[0]) + fmaf(sgs, xi[0], sscale * bx[s]),
+                   fmaf(ca, gp.y, Bex[1]) + fmaf(sgs, xi[1], sscale * by[s]),
+                   fmaf(ca, gp.z, Bex[2]) + fmaf(sgs, xi[2], sscale * bz[s]), f);
+          normalise3(Xs[0] + f[0], Xs[1] + f[1], Xs[2] + f[2], o[s]);
         }
       }
-      cta_barrier();
+      // S~ slot m % 3 was last read by the correctors of march step m - 1 (as their x+1 plane) -- by the threads that own
+      // those sites -- and its halo columns by the edge reads of the same step; every warp has left that step's
+      // corrector once it has arrived for step... it arrives for step m only after its predictor, so wait for m - 1's
+      // completion AND use the fact that a main warp reads the halo columns of plane q - 3's slot no later than in
+      // step m - 2 (L1_0: as the x+1 plane's edges in step m - 3; SC: as the own plane's edges in step m - 2).
+      if (m >= 1) mbar_wait_long(done_bar(m - 1), phase(m - 1));
+#pragma unroll
+      for (int s = 0; s < 2; ++s)
+        if (act[s]) {
+#pragma unroll
+          for (int c = 0; c < 3; ++c) sts1(tslot + own_b[s] + (uint32_t)c * compb, o[s][c]);
+        }
+      warp_arrive(done_bar(m));
 #pragma unroll
       for (int s = 0; s < 2; ++s)
 #pragma unroll
@@ -390,11 +483,12 @@ __global__ void __launch_bounds__(NT, MINB) heun_fused(const __grid_constant__ C
 #pragma unroll
           for (int d = 0; d < 3; ++d) { rP[s][c][d] = rC[s][c][d]; rC[s][c][d] = rN[s][c][d]; }
       e += planep; ec += (uint32_t)p.ny; gsite += gplane;
+      t3 = (t3 == 2u) ? 0u : t3 + 1u;
     }
   }
 }
 
-typedef void (*FusedKernel)(const CUtensorMap, const FusedParams);
+typedef void (*FusedKernel)(const CUtensorMap, const CUtensorMap, const FusedParams);
 
 // Compiled CTA shapes (threads, CTAs per SM -> register budget): 256 x 2 -> 128 registers (4 warps per scheduler),
 // 512 x 1 -> 128.
@@ -411,13 +505,13 @@ inline int round_up32(int v) { return (v + 31) / 32 * 32; }
 
 uint32_t plan_smem(int nz, int by, uint32_t& slot_pitch) {
   slot_pitch = (uint32_t)align_up((size_t)3 * (nz + 2) * (by + 8) * 4, 128);
-  return 128u + 2u * kRing * slot_pitch;
+  return 128u + (kRingS + kRingT) * slot_pitch + (uint32_t)align_up((size_t)4 * nz * by * 4, 128);
 }
 
 }  // namespace
 
 struct FusedPlan {
-  CUtensorMap mapS;
+  CUtensorMap mapS, mapF;
   FusedKernel kern = nullptr;
   int32_t BY = 0, G = 0, nstrips = 0, CX = 0, nchunks = 0, threads = 0, n_main = 0, ctas_per_sm = 0;
   uint32_t slot_pitch = 0, smem_bytes = 0;
@@ -496,7 +590,11 @@ bool build_plan(Ctx& c, FusedPlan& pl) {
   const cuuint64_t strides[3] = {(cuuint64_t)c.nyp * 4, (cuuint64_t)nz * c.nyp * 4, (cuuint64_t)c.as * 4};
   const cuuint32_t estr[4] = {1, 1, 1, 1};
   const cuuint32_t box[4] = {(cuuint32_t)(pl.BY + 8), (cuuint32_t)(nz + 2), 1u, 3u};
+  const cuuint32_t boxF[4] = {(cuuint32_t)pl.BY, (cuuint32_t)nz, 1u, 4u};     // sigma, Bx, By, Bz of one strip plane
   return enc(&pl.mapS, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void*)(c.arrays + c.lead), dims, strides, box, estr,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS &&
+         enc(&pl.mapF, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void*)(c.arrays + c.lead), dims, strides, boxF, estr,
              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
@@ -530,8 +628,9 @@ asd_status launch_heun_fused(Ctx& c, StageParams& p) {
   f.nx = c.d.nx; f.ny = c.d.ny; f.nz = c.d.nz; f.nyp = c.nyp; f.lead = c.lead;
   f.BY = pl->BY; f.G = pl->G; f.nstrips = pl->nstrips; f.CX = pl->CX; f.n_main = pl->n_main;
   f.slot_pitch = pl->slot_pitch;
-  f.j1 = p.jx[0]; f.j2 = p.jx[1]; f.j3 = p.jx[2];
-  f.gdt = p.gdt; f.lambda = p.lambda; f.scale = p.scale;
+  f.ngdt = -p.gdt;
+  f.j1s = f.ngdt * p.jx[0]; f.j2s = f.ngdt * p.jx[1]; f.j3s = f.ngdt * p.jx[2];
+  f.lambda = p.lambda; f.scale = p.scale;
   f.n_lo = p.n_lo; f.n_hi = p.n_hi; f.dyn = p.dyn; f.g0 = p.g0; f.key = p.key;
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)(pl->nstrips * pl->nchunks)); cfg.blockDim = dim3((unsigned)pl->threads);
@@ -540,7 +639,7 @@ asd_status launch_heun_fused(Ctx& c, StageParams& p) {
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr; cfg.numAttrs = 1;
-  cudaLaunchKernelEx(&cfg, pl->kern, pl->mapS, f);
+  cudaLaunchKernelEx(&cfg, pl->kern, pl->mapS, pl->mapF, f);
   ASD_LAUNCH_CHECK(c, "heun step (fused)");
   const int t = c.aS; c.aS = c.aSt; c.aSt = t;
   return ASD_OK;
