@@ -70,64 +70,115 @@ __device__ __forceinline__ void llg_dt_f(float lambda, const float X[3], float B
 
 // Adds the anisotropy field, Eq. (3), pre-scaled by -gdt, to the exchange field of the 4 sites of a group.  gp = the
 // group's (e_x, e_y, e_z, 2 k_u/mu_s), gathered by the caller ahead of time by the group's grain id; a group that holds
-// two different grains (rare, flagged at set-up) gathers per site here.  A vacant site may borrow any parameters: its
-// spin is 0.
+// two different grains (rare, flagged at set-up; a branch of its own so that the common path carries no selects)
+// gathers per site here.  A vacant site may borrow any parameters: its spin is 0.
 __device__ __forceinline__ void add_aniso(const float4* grain, float4 gp, bool mixed, const uint32_t* colp, float ngdt,
                                           const float X[3][4], float Bex[3][4]) {
-  uint4 cc = make_uint4(0u, 0u, 0u, 0u);
-  if (mixed) cc = __ldg(reinterpret_cast<const uint4*>(colp));
-  const uint32_t id[4] = {cc.x & 0xFFFFu, cc.y & 0xFFFFu, cc.z & 0xFFFFu, cc.w & 0xFFFFu};
+  if (!mixed) {
+    const float kw = gp.w;                             // already pre-scaled by the halo warp
 #pragma unroll
-  for (int v = 0; v < 4; ++v) {
-    float4 gv = gp;
-    if (mixed) gv = __ldg(grain + id[v]);
-    const float ca = (ngdt * gv.w) * fmaf(X[0][v], gv.x, fmaf(X[1][v], gv.y, X[2][v] * gv.z));
-    Bex[0][v] = fmaf(ca, gv.x, Bex[0][v]); Bex[1][v] = fmaf(ca, gv.y, Bex[1][v]); Bex[2][v] = fmaf(ca, gv.z, Bex[2][v]);
+    for (int v = 0; v < 4; ++v) {
+      const float ca = kw * fmaf(X[0][v], gp.x, fmaf(X[1][v], gp.y, X[2][v] * gp.z));
+      Bex[0][v] = fmaf(ca, gp.x, Bex[0][v]); Bex[1][v] = fmaf(ca, gp.y, Bex[1][v]); Bex[2][v] = fmaf(ca, gp.z, Bex[2][v]);
+    }
+  } else {
+    const uint4 cc = __ldg(reinterpret_cast<const uint4*>(colp));
+    const uint32_t id[4] = {cc.x & 0xFFFFu, cc.y & 0xFFFFu, cc.z & 0xFFFFu, cc.w & 0xFFFFu};
+#pragma unroll
+    for (int v = 0; v < 4; ++v) {
+      const float4 gv = __ldg(grain + id[v]);
+      const float ca = (ngdt * gv.w) * fmaf(X[0][v], gv.x, fmaf(X[1][v], gv.y, X[2][v] * gv.z));
+      Bex[0][v] = fmaf(ca, gv.x, Bex[0][v]); Bex[1][v] = fmaf(ca, gv.y, Bex[1][v]); Bex[2][v] = fmaf(ca, gv.z, Bex[2][v]);
+    }
   }
 }
-// grain id of a group (the largest of its 4 columns' ids: vacant columns are 0) | bit 31: the group holds two grains
-__device__ __forceinline__ uint32_t pack_group(uint4 cid4) {
-  const uint32_t gid = max(max(cid4.x & 0xFFFFu, cid4.y & 0xFFFFu), max(cid4.z & 0xFFFFu, cid4.w & 0xFFFFu));
-  return gid | ((cid4.x & COL_GROUP_MIXED) ? 0x80000000u : 0u);
-}
-
-// Mbarrier with one arrival per warp: the split barrier of the march.
-__device__ __forceinline__ void warp_arrive(uint32_t bar) {
+// The split barrier of the march.  Waiters of an mbarrier are woken by EVERY arrival, so the warps first count
+// themselves on a shared-memory counter (acq_rel, so that each warp's S~ stores are visible to whoever comes last) and
+// only the last one arrives on the mbarrier (count 1): one wake-up per phase.
+__device__ __forceinline__ void warp_arrive(uint32_t cnt, uint32_t bar, uint32_t nwarps) {
   __syncwarp();
-  if ((threadIdx.x & 31u) == 0u) mbar_arrive(bar);
+  if ((threadIdx.x & 31u) == 0u) {
+    uint32_t old;
+    asm volatile("atom.acq_rel.cta.shared::cta.add.u32 %0, [%1], 1;" : "=r"(old) : "r"(cnt) : "memory");
+    if (old == nwarps - 1u) {
+      asm volatile("st.relaxed.cta.shared::cta.u32 [%0], %1;" ::"r"(cnt), "r"(0u) : "memory");
+      mbar_arrive(bar);
+    }
+  }
 }
 
-template <int LAT, int NT, int MINB>
+constexpr uint32_t kGpRing = 8;   // planes of per-group anisotropy parameters kept in shared memory
+
+// NZ_T / BY_T != 0: film thickness and strip width are compile-time constants (every shared-memory offset becomes an
+// immediate of its LDS / STS); 0: taken from the parameter block.
+template <int LAT, int NT, int MINB, int NZ_T, int BY_T>
 __global__ void __launch_bounds__(NT, MINB)
 heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUtensorMap mapF, const FusedParams p) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int NZ = NZ_T ? NZ_T : p.nz, BY = BY_T ? BY_T : p.BY, G = BY / 4;
+  const int W = BY + 8, R = NZ + 2;
+  const uint32_t rowb = (uint32_t)(W * 4), compb = (uint32_t)(R * W * 4);
+  const uint32_t box_bytes = 3u * compb;
+  const uint32_t slot_pitch = (NZ_T && BY_T) ? ((box_bytes + 127u) & ~127u) : p.slot_pitch;
+  const uint32_t fcomp = (uint32_t)(NZ * BY * 4), fbytes = 4u * fcomp;
+  const uint32_t gp_pitch = (uint32_t)((20 * G + 15) & ~15);   // per plane: float4 per group, then one flag word per group
   const uint32_t sm0 = smem_u32(smem_raw);
   const uint32_t bar_full = sm0;                      // S plane landed (TMA transaction count)
-  const uint32_t bar_done = sm0 + 32u;                // S~ plane complete (one arrival per warp)
+  const uint32_t bar_done = sm0 + 32u;                // S~ plane complete
   const uint32_t bar_fld = sm0 + 64u;                 // sigma / B plane landed
-  const uint32_t sring = sm0 + 128u;
-  const uint32_t tring = sring + kRingS * p.slot_pitch;
-  const uint32_t fbox = tring + kRingT * p.slot_pitch;
+  const uint32_t cnt_done = sm0 + 96u;                // warps that have finished their share of an S~ plane (4 counters)
+  const uint32_t gpring = sm0 + 128u;
+  const uint32_t sring = gpring + ((kGpRing * gp_pitch + 127u) & ~127u);
+  const uint32_t tring = sring + kRingS * slot_pitch;
+  const uint32_t fbox = tring + kRingT * slot_pitch;
 
   const int tid = (int)threadIdx.x;
   const int strip = (int)blockIdx.x % p.nstrips, chunk = (int)blockIdx.x / p.nstrips;
-  const int j0 = strip * p.BY;
+  const int j0 = strip * BY;
   const int i0 = chunk * p.CX;
   const int L = min(p.CX, p.nx - i0);                 // planes this CTA updates
-  const int W = p.BY + 8, R = p.nz + 2;
-  const uint32_t rowb = (uint32_t)(W * 4), compb = (uint32_t)(R * W * 4);
-  const uint32_t box_bytes = 3u * compb;
-  const uint32_t fcomp = (uint32_t)(p.nz * p.BY * 4), fbytes = 4u * fcomp;
+  const bool is_main = tid < p.n_main;
+
+  // Anisotropy parameters depend on the column only: for every plane the halo warp looks up, once per 4-site group of the
+  // strip, (e_x, e_y, e_z, 2 k_u/mu_s) by the group's grain id (the largest of its 4 columns' ids: vacant columns are 0 and
+  // may borrow a neighbour's parameters, their spins are 0) and a flag "this group holds two different grains" (set-up
+  // flagged it in the column table; such groups gather per site).  Planes i0 - 1 + mm, ring slot mm % 8.
+  auto fill_gp = [&](int mm, int lane) {
+    if (lane < G) {
+      const int plane = i0 - 1 + mm, jg = j0 + 4 * lane;
+      float4 gp = make_float4(0.f, 0.f, 1.f, 0.f);
+      uint32_t flag = 0u;
+      if (plane >= 0 && plane < p.nx && jg < p.ny) {
+        const uint4 cid4 = __ldg(reinterpret_cast<const uint4*>(p.col + ((uint32_t)plane * (uint32_t)p.ny + (uint32_t)jg)));
+        const uint32_t gid = max(max(cid4.x & 0xFFFFu, cid4.y & 0xFFFFu), max(cid4.z & 0xFFFFu, cid4.w & 0xFFFFu));
+        flag = (cid4.x & COL_GROUP_MIXED) ? 1u : 0u;
+        gp = __ldg(p.grain + gid);
+        gp.w *= p.ngdt;                               // pre-scaled like every field term
+      }
+      const uint32_t slot = gpring + ((uint32_t)mm & (kGpRing - 1u)) * gp_pitch;
+      sts4(slot + 16u * (uint32_t)lane, gp.x, gp.y, gp.z, gp.w);
+      sts1(slot + 16u * (uint32_t)G + 4u * (uint32_t)lane, __uint_as_float(flag));
+    }
+  };
 
   // S~ ring starts as zeros: the rows z = -1 and z = nz, and the columns of a ragged last strip, are never written.
-  for (uint32_t o = (uint32_t)tid * 16u; o < kRingT * p.slot_pitch; o += (uint32_t)blockDim.x * 16u)
+  for (uint32_t o = (uint32_t)tid * 16u; o < kRingT * slot_pitch; o += (uint32_t)blockDim.x * 16u)
     sts4(tring + o, 0.0f, 0.0f, 0.0f, 0.0f);
+  // ... and so does the parameter ring (the corrector of march step 0 reads the slot of a plane nobody fills; its result
+  // is discarded, but a stray "two grains" flag would send it to the column table)
+  for (uint32_t o = (uint32_t)tid * 16u; o < kGpRing * gp_pitch; o += (uint32_t)blockDim.x * 16u)
+    sts4(gpring + o, 0.0f, 0.0f, 0.0f, 0.0f);
+  asm volatile("bar.sync 0;" ::: "memory");
   if (tid == 0) {
-    for (int s = 0; s < 4; ++s) { mbar_init(bar_full + 8u * s, 1u); mbar_init(bar_done + 8u * s, blockDim.x / 32u); }
+    for (int s = 0; s < 4; ++s) {
+      mbar_init(bar_full + 8u * s, 1u); mbar_init(bar_done + 8u * s, 1u);
+      asm volatile("st.shared.u32 [%0], %1;" ::"r"(cnt_done + 4u * s), "r"(0u) : "memory");
+    }
     mbar_init(bar_fld, 1u);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
+  if (!is_main) { fill_gp(0, tid - p.n_main); fill_gp(1, tid - p.n_main); }    // static tables: no need to wait for the previous grid
   // Programmatic dependent launch: everything above overlaps the tail of the previous step's grid; nothing below the
   // wait runs before that grid has completed (it wrote the spins this one reads and read the buffer this one writes).
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
@@ -138,7 +189,7 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
   auto issue_S = [&](int u) {
     const uint32_t s = (uint32_t)(u & (kRingS - 1));
     mbar_expect_tx(bar_full + 8u * s, box_bytes);
-    tma_load_4d(sring + s * p.slot_pitch, &mapS, bar_full + 8u * s, j0 - 4, -1, i0 - 2 + u, p.aIn);
+    tma_load_4d(sring + s * slot_pitch, &mapS, bar_full + 8u * s, j0 - 4, -1, i0 - 2 + u, p.aIn);
   };
   auto issue_F = [&](int m) {
     mbar_expect_tx(bar_fld, fbytes);
@@ -154,23 +205,26 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
   resolve_dyn(p.dyn, n_lo, n_hi, scale);
   const float sscale = p.ngdt * scale;                // B'_app = sscale * B
   const float lambda = p.lambda;
-  const uint32_t planep = (uint32_t)(p.nz * p.nyp);
+  const uint32_t planep = (uint32_t)(NZ * p.nyp);
   auto done_bar = [&](int m) { return bar_done + 8u * (uint32_t)(m & 3); };
+  const uint32_t nwarps = blockDim.x / 32u;
+  auto arrive_done = [&](int m) { warp_arrive(cnt_done + 4u * (uint32_t)(m & 3), done_bar(m), nwarps); };
   auto phase = [](int m) { return (uint32_t)(m >> 2) & 1u; };
 
-  if (tid < p.n_main) {
+  if (is_main) {
     // ================= main threads: 4 consecutive y-sites of one z-row, predictor and corrector =================
-    const int k = tid / p.G, g = tid - k * p.G;
+    const int k = tid / G, g = tid - k * G;
     const int j = j0 + 4 * g;
-    const bool active = (k < p.nz) && (j < p.ny);
+    const bool active = (k < NZ) && (j < p.ny);
     // own float4 inside component 0 of a slot (inactive threads read a valid dummy position and write nothing)
     const uint32_t own_b = active ? (uint32_t)(((k + 1) * W + 4 + 4 * g) * 4) : (uint32_t)((W + 4) * 4);
-    const uint32_t fown = fbox + (active ? (uint32_t)((k * p.BY + 4 * g) * 4) : 0u);
+    const uint32_t fown = fbox + (active ? (uint32_t)((k * BY + 4 * g) * 4) : 0u);
+    const uint32_t gown = gpring + 16u * (uint32_t)g, gflag = gpring + 16u * (uint32_t)G + 4u * (uint32_t)g;
     // element of the group in predictor plane q = i0 - 1 (wraps below zero for q = -1; not dereferenced then)
-    uint32_t e = (uint32_t)(p.lead + ((i0 - 1) * p.nz + k) * p.nyp + j);
+    uint32_t e = (uint32_t)(p.lead + ((i0 - 1) * NZ + k) * p.nyp + j);
     uint32_t ec = (uint32_t)((i0 - 1) * p.ny + j);                      // column (q, j) of the window
-    uint64_t gsite = p.g0 + (uint64_t)(int64_t)(((int64_t)(i0 - 1) * p.nz + k) * p.ny + j);
-    const uint32_t gplane = (uint32_t)(p.nz * p.ny);
+    uint64_t gsite = p.g0 + (uint64_t)(int64_t)(((int64_t)(i0 - 1) * NZ + k) * p.ny + j);
+    const uint32_t gplane = (uint32_t)(NZ * p.ny);
 
     // carried from the predictor of plane q to its corrector one march step later
     float A[3][4], Bs[3][4];
@@ -178,9 +232,6 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
     for (int c = 0; c < 3; ++c)
 #pragma unroll
       for (int v = 0; v < 4; ++v) { A[c][v] = 0.0f; Bs[c][v] = 0.0f; }
-    // packed grain id of the group in plane q (cgN: ready one march step ahead, so that the parameter gather does not
-    // wait for the column table) and in plane q - 1 (cgC)
-    uint32_t cgN = (active && i0 >= 1) ? pack_group(__ldg(reinterpret_cast<const uint4*>(p.col + ec))) : 0u, cgC = 0u;
     // L1_0 only: the y-1 / y+4 edge columns of the group's row are 16-byte-strided scalar reads (4 shared-memory
     // wavefronts each); every plane's pair is read once and kept while the plane is the x+1, own and x-1 plane.
     float sP[3][2], sC[3][2];      // S edges of planes q-1, q
@@ -193,7 +244,7 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
     if (LAT == LAT_L10) {
 #pragma unroll
       for (int c = 0; c < 3; ++c) {
-        const uint32_t a0 = sring + own_b + (uint32_t)c * compb, a1 = a0 + p.slot_pitch;
+        const uint32_t a0 = sring + own_b + (uint32_t)c * compb, a1 = a0 + slot_pitch;
         sP[c][0] = lds1(a0 - 4u); sP[c][1] = lds1(a0 + 16u);
         sC[c][0] = lds1(a1 - 4u); sC[c][1] = lds1(a1 + 16u);
       }
@@ -201,23 +252,17 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
     uint32_t t3 = 0u;                                  // m % 3: S~ slot of plane q
 
     for (int m = 0; m <= L + 1; ++m) {
-      const int q = i0 - 1 + m;
-      const bool qvalid = active && (q >= 0) && (q < p.nx);
-      const uint32_t tN = tring + t3 * p.slot_pitch + own_b;                                   // S~ plane q
-      const uint32_t tCs = tring + (t3 == 0u ? 2u : t3 - 1u) * p.slot_pitch + own_b;           // q - 1
-      const uint32_t tPs = tring + (t3 == 2u ? 0u : t3 + 1u) * p.slot_pitch + own_b;           // q - 2
-      // issued first, used after the exchange sums: the group's anisotropy parameters, next plane's column entries
-      const float4 gpN = __ldg(p.grain + (cgN & 0xFFFFu));
-      uint4 cid4 = make_uint4(0u, 0u, 0u, 0u);
-      if (active && q + 1 >= 0 && q + 1 < p.nx) cid4 = __ldg(reinterpret_cast<const uint4*>(p.col + (ec + (uint32_t)p.ny)));
-      mbar_wait_long(bar_full + 8u * (uint32_t)((m + 2) & (kRingS - 1)), phase(m + 2));   // S plane q + 1
+      const uint32_t tN = tring + t3 * slot_pitch + own_b;                                   // S~ plane q
+      const uint32_t tCs = tring + (t3 == 0u ? 2u : t3 - 1u) * slot_pitch + own_b;           // q - 1
+      const uint32_t tPs = tring + (t3 == 2u ? 0u : t3 + 1u) * slot_pitch + own_b;           // q - 2
+      mbar_wait_long(bar_full + 8u * (uint32_t)((m + 2) & (kRingS - 1)), phase(m + 2));      // S plane q + 1
 
       // ---- predictor of plane q: S~ = normalise(S + dt k1), A = S + dt/2 k1 ----
       float An[3][4], Bn[3][4];                        // this plane's A and -gdt (sigma xi + s B_app)
       {
-        const uint32_t prev = sring + (uint32_t)(m & 3) * p.slot_pitch + own_b;
-        const uint32_t cur = sring + (uint32_t)((m + 1) & 3) * p.slot_pitch + own_b;
-        const uint32_t next = sring + (uint32_t)((m + 2) & 3) * p.slot_pitch + own_b;
+        const uint32_t prev = sring + (uint32_t)(m & 3) * slot_pitch + own_b;
+        const uint32_t cur = sring + (uint32_t)((m + 1) & 3) * slot_pitch + own_b;
+        const uint32_t next = sring + (uint32_t)((m + 2) & 3) * slot_pitch + own_b;
         float X[3][4], Bex[3][4];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
@@ -247,7 +292,10 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
             sP[c][0] = sC[c][0]; sP[c][1] = sC[c][1]; sC[c][0] = nL; sC[c][1] = nR;
           }
         }
-        add_aniso(p.grain, gpN, (cgN >> 31) != 0u, p.col + ec, p.ngdt, X, Bex);
+        {
+          const uint32_t gs = ((uint32_t)m & (kGpRing - 1u)) * gp_pitch;
+          add_aniso(p.grain, lds4(gown + gs), __float_as_uint(lds1(gflag + gs)) != 0u, p.col + ec, p.ngdt, X, Bex);
+        }
         // ---- noise: one Philox block per site per STEP; sigma and B of the plane come from the staged field box ----
         mbar_wait_long(bar_fld, (uint32_t)m & 1u);
         {
@@ -255,16 +303,17 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
           const float sg[4] = {sg4.x, sg4.y, sg4.z, sg4.w};
           const float bx[4] = {bx4.x, bx4.y, bx4.z, bx4.w}, by[4] = {by4.x, by4.y, by4.z, by4.w},
                       bz[4] = {bz4.x, bz4.y, bz4.z, bz4.w};
+          uint32_t rnd[4][4];
+          float xi[4][3];
+#pragma unroll
+          for (int v = 0; v < 4; ++v) philox_site(p.key, n_lo, n_hi, gsite + (uint64_t)v, 0u, rnd[v]);
+          normals3_multi<4>(rnd, xi);
 #pragma unroll
           for (int v = 0; v < 4; ++v) {
-            uint32_t rnd[4];
-            philox_site(p.key, n_lo, n_hi, gsite + (uint64_t)v, 0u, rnd);
-            float xi[3];
-            normals3(rnd, xi);
             const float sgs = p.ngdt * sg[v];
-            Bn[0][v] = fmaf(sgs, xi[0], sscale * bx[v]);
-            Bn[1][v] = fmaf(sgs, xi[1], sscale * by[v]);
-            Bn[2][v] = fmaf(sgs, xi[2], sscale * bz[v]);
+            Bn[0][v] = fmaf(sgs, xi[v][0], sscale * bx[v]);
+            Bn[1][v] = fmaf(sgs, xi[v][1], sscale * by[v]);
+            Bn[2][v] = fmaf(sgs, xi[v][2], sscale * bz[v]);
           }
         }
         float St[3][4];
@@ -284,11 +333,10 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
           for (int c = 0; c < 3; ++c) sts4(tN + (uint32_t)c * compb, St[c][0], St[c][1], St[c][2], St[c][3]);
         }
       }
-      warp_arrive(done_bar(m));                        // this warp's share of S~ plane q is written
+      arrive_done(m);                                  // this warp's share of S~ plane q is written
 
       // ---- corrector of plane q - 1, first part: everything that does not need S~ plane q ----
       const bool do_corr = active && (m >= 2);
-      const float4 gpC = __ldg(p.grain + (cgC & 0xFFFFu));
       float X[3][4], Bp[3][4];
 #pragma unroll
       for (int c = 0; c < 3; ++c) {
@@ -314,7 +362,10 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
           }
         }
       }
-      add_aniso(p.grain, gpC, (cgC >> 31) != 0u, p.col + (ec - (uint32_t)p.ny), p.ngdt, X, Bp);
+      {
+        const uint32_t gs = ((uint32_t)(m - 1) & (kGpRing - 1u)) * gp_pitch;
+        add_aniso(p.grain, lds4(gown + gs), __float_as_uint(lds1(gflag + gs)) != 0u, p.col + (ec - (uint32_t)p.ny), p.ngdt, X, Bp);
+      }
 #pragma unroll
       for (int c = 0; c < 3; ++c)
 #pragma unroll
@@ -366,26 +417,26 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
       for (int c = 0; c < 3; ++c)
 #pragma unroll
         for (int v = 0; v < 4; ++v) { A[c][v] = An[c][v]; Bs[c][v] = Bn[c][v]; }
-      cgC = cgN; cgN = pack_group(cid4);
       e += planep; ec += (uint32_t)p.ny; gsite += gplane;
       t3 = (t3 == 2u) ? 0u : t3 + 1u;
     }
   } else {
-    // ================= halo threads: the two sites (y = j0 - 1, y = j0 + BY) of one z-row, predictor only =================
+    // ================= halo warp(s): the two sites (y = j0 - 1, y = j0 + BY) of one z-row, predictor only; =================
+    // ================= and the per-group anisotropy parameters two planes ahead                              =================
     // Lanes of a warp read the same column of different rows (a bank-conflicted pattern), so each halo thread keeps
     // the three columns around its sites for planes q-1, q in registers and loads only plane q+1's and the z
     // neighbours of plane q per march step.
     const float* __restrict__ base = p.arrays;
     const int k = tid - p.n_main;
-    const bool row_ok = k < p.nz;
-    const int jh[2] = {j0 - 1, j0 + p.BY};
+    const bool row_ok = k < NZ;
+    const int jh[2] = {j0 - 1, j0 + BY};
     const bool act[2] = {row_ok && jh[0] >= 0, row_ok && jh[1] < p.ny};
     const int kk = row_ok ? k : 0;
-    const uint32_t own_b[2] = {(uint32_t)(((kk + 1) * W + 3) * 4), (uint32_t)(((kk + 1) * W + 4 + p.BY) * 4)};
-    uint32_t e = (uint32_t)(p.lead + ((i0 - 1) * p.nz + k) * p.nyp);          // + jh
+    const uint32_t own_b[2] = {(uint32_t)(((kk + 1) * W + 3) * 4), (uint32_t)(((kk + 1) * W + 4 + BY) * 4)};
+    uint32_t e = (uint32_t)(p.lead + ((i0 - 1) * NZ + k) * p.nyp);          // + jh
     uint32_t ec = (uint32_t)((i0 - 1) * p.ny);
-    uint64_t gsite = p.g0 + (uint64_t)(int64_t)(((int64_t)(i0 - 1) * p.nz + k) * p.ny);
-    const uint32_t gplane = (uint32_t)(p.nz * p.ny);
+    uint64_t gsite = p.g0 + (uint64_t)(int64_t)(((int64_t)(i0 - 1) * NZ + k) * p.ny);
+    const uint32_t gplane = (uint32_t)(NZ * p.ny);
 
     mbar_wait_long(bar_full + 0u, 0u);
     mbar_wait_long(bar_full + 8u, 0u);
@@ -399,7 +450,7 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
         for (int d = 0; d < 3; ++d) {
           const uint32_t off = own_b[s] + (uint32_t)c * compb + (uint32_t)(4 * d) - 4u;
           rP[s][c][d] = lds1(sring + off);
-          rC[s][c][d] = lds1(sring + p.slot_pitch + off);
+          rC[s][c][d] = lds1(sring + slot_pitch + off);
         }
     uint32_t t3 = 0u;
 
@@ -418,9 +469,11 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
           by[s] = ldg_stream1(base + (p.oB + p.as + es));
           bz[s] = ldg_stream1(base + (p.oB + 2u * p.as + es));
         }
+      // slot (m + 2) % 8 of the parameter ring was last read in march step m - 5
+      fill_gp(m + 2, k);
       mbar_wait_long(bar_full + 8u * (uint32_t)((m + 2) & (kRingS - 1)), phase(m + 2));
-      const uint32_t cur = sring + (uint32_t)((m + 1) & 3) * p.slot_pitch, next = sring + (uint32_t)((m + 2) & 3) * p.slot_pitch;
-      const uint32_t tslot = tring + t3 * p.slot_pitch;
+      const uint32_t cur = sring + (uint32_t)((m + 1) & 3) * slot_pitch, next = sring + (uint32_t)((m + 2) & 3) * slot_pitch;
+      const uint32_t tslot = tring + t3 * slot_pitch;
       float rN[2][3][3];
       float o[2][3];
 #pragma unroll
@@ -463,11 +516,9 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
           normalise3(Xs[0] + f[0], Xs[1] + f[1], Xs[2] + f[2], o[s]);
         }
       }
-      // S~ slot m % 3 was last read by the correctors of march step m - 1 (as their x+1 plane) -- by the threads that own
-      // those sites -- and its halo columns by the edge reads of the same step; every warp has left that step's
-      // corrector once it has arrived for step... it arrives for step m only after its predictor, so wait for m - 1's
-      // completion AND use the fact that a main warp reads the halo columns of plane q - 3's slot no later than in
-      // step m - 2 (L1_0: as the x+1 plane's edges in step m - 3; SC: as the own plane's edges in step m - 2).
+      // S~ slot m % 3 held plane q - 3.  Its halo columns were last read by main threads in march step m - 3 (L1_0: as
+      // the edges of their x+1 plane) or m - 2 (SC: as the edges of their own plane), i.e. before they arrived for
+      // step m - 1.
       if (m >= 1) mbar_wait_long(done_bar(m - 1), phase(m - 1));
 #pragma unroll
       for (int s = 0; s < 2; ++s)
@@ -475,7 +526,7 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
 #pragma unroll
           for (int c = 0; c < 3; ++c) sts1(tslot + own_b[s] + (uint32_t)c * compb, o[s][c]);
         }
-      warp_arrive(done_bar(m));
+      arrive_done(m);
 #pragma unroll
       for (int s = 0; s < 2; ++s)
 #pragma unroll
@@ -496,16 +547,21 @@ struct Shape { int nt, minb; };
 constexpr Shape kShapes[] = {{256, 2}, {512, 1}};
 constexpr int kNumShapes = 2;
 
-FusedKernel kernel_for(int lattice, int shape) {
-  if (lattice == ASD_SC) return shape == 0 ? heun_fused<LAT_SC, 256, 2> : heun_fused<LAT_SC, 512, 1>;
-  return shape == 0 ? heun_fused<LAT_L10, 256, 2> : heun_fused<LAT_L10, 512, 1>;
+// Film thickness 27 planes with 32-site strips (BASELINE configs 1, 3, 4) has its own instance with compile-time shared-
+// memory offsets; everything else takes the generic one.
+FusedKernel kernel_for(int lattice, int shape, int nz, int by) {
+  if (shape == 0 && nz == 27 && by == 32)
+    return lattice == ASD_SC ? heun_fused<LAT_SC, 256, 2, 27, 32> : heun_fused<LAT_L10, 256, 2, 27, 32>;
+  if (lattice == ASD_SC) return shape == 0 ? heun_fused<LAT_SC, 256, 2, 0, 0> : heun_fused<LAT_SC, 512, 1, 0, 0>;
+  return shape == 0 ? heun_fused<LAT_L10, 256, 2, 0, 0> : heun_fused<LAT_L10, 512, 1, 0, 0>;
 }
 
 inline int round_up32(int v) { return (v + 31) / 32 * 32; }
 
 uint32_t plan_smem(int nz, int by, uint32_t& slot_pitch) {
   slot_pitch = (uint32_t)align_up((size_t)3 * (nz + 2) * (by + 8) * 4, 128);
-  return 128u + (kRingS + kRingT) * slot_pitch + (uint32_t)align_up((size_t)4 * nz * by * 4, 128);
+  return 128u + (uint32_t)align_up((size_t)kGpRing * (size_t)((20 * (by / 4) + 15) & ~15), 128) + (kRingS + kRingT) * slot_pitch +
+         (uint32_t)align_up((size_t)4 * nz * by * 4, 128);
 }
 
 }  // namespace
@@ -566,7 +622,7 @@ bool build_plan(Ctx& c, FusedPlan& pl) {
   pl.n_main = round_up32(nz * pl.G);
   pl.threads = pl.n_main + round_up32(nz);
   pl.smem_bytes = plan_smem(nz, pl.BY, pl.slot_pitch);
-  pl.kern = kernel_for(c.d.lattice, best.shape);
+  pl.kern = kernel_for(c.d.lattice, best.shape, nz, pl.BY);
   int bps = 0;
   if (cudaFuncSetAttribute((const void*)pl.kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes) != cudaSuccess ||
       cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, (const void*)pl.kern, pl.threads, pl.smem_bytes) != cudaSuccess ||
