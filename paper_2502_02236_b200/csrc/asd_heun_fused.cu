@@ -92,19 +92,24 @@ __device__ __forceinline__ void add_aniso(const float4* grain, float4 gp, bool m
     }
   }
 }
-// The split barrier of the march.  Waiters of an mbarrier are woken by EVERY arrival, so the warps first count
-// themselves on a shared-memory counter (acq_rel, so that each warp's S~ stores are visible to whoever comes last) and
-// only the last one arrives on the mbarrier (count 1): one wake-up per phase.
-__device__ __forceinline__ void warp_arrive(uint32_t cnt, uint32_t bar, uint32_t nwarps) {
+// The split barrier of the march: one arrival per warp (release: the warp's shared-memory stores are visible to whoever
+// sees the phase complete), waited for later.
+__device__ __forceinline__ void warp_arrive(uint32_t bar) {
   __syncwarp();
+  if ((threadIdx.x & 31u) == 0u) mbar_arrive(bar);
+}
+// Counts the warp on a shared-memory counter; true (in lane 0 only) for the warp that comes last, which also resets it.
+// Relaxed: used where the warps only have to have CONSUMED something (their loads have returned: the values were used).
+__device__ __forceinline__ bool warp_count_last(uint32_t cnt, uint32_t nwarps) {
+  __syncwarp();
+  bool last = false;
   if ((threadIdx.x & 31u) == 0u) {
     uint32_t old;
-    asm volatile("atom.acq_rel.cta.shared::cta.add.u32 %0, [%1], 1;" : "=r"(old) : "r"(cnt) : "memory");
-    if (old == nwarps - 1u) {
-      asm volatile("st.relaxed.cta.shared::cta.u32 [%0], %1;" ::"r"(cnt), "r"(0u) : "memory");
-      mbar_arrive(bar);
-    }
+    asm volatile("atom.relaxed.cta.shared::cta.add.u32 %0, [%1], 1;" : "=r"(old) : "r"(cnt) : "memory");
+    last = (old == nwarps - 1u);
+    if (last) asm volatile("st.relaxed.cta.shared::cta.u32 [%0], %1;" ::"r"(cnt), "r"(0u) : "memory");
   }
+  return last;
 }
 
 constexpr uint32_t kGpRing = 8;   // planes of per-group anisotropy parameters kept in shared memory
@@ -121,12 +126,12 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
   const uint32_t box_bytes = 3u * compb;
   const uint32_t slot_pitch = (NZ_T && BY_T) ? ((box_bytes + 127u) & ~127u) : p.slot_pitch;
   const uint32_t fcomp = (uint32_t)(NZ * BY * 4), fbytes = 4u * fcomp;
-  const uint32_t gp_pitch = (uint32_t)((20 * G + 15) & ~15);   // per plane: float4 per group, then one flag word per group
+  const uint32_t gp_pitch = (uint32_t)((20 * G + 32 + 15) & ~15);   // per plane: float4 per group + 2 halo columns, then one flag word per group
   const uint32_t sm0 = smem_u32(smem_raw);
   const uint32_t bar_full = sm0;                      // S plane landed (TMA transaction count)
   const uint32_t bar_done = sm0 + 32u;                // S~ plane complete
   const uint32_t bar_fld = sm0 + 64u;                 // sigma / B plane landed
-  const uint32_t cnt_done = sm0 + 96u;                // warps that have finished their share of an S~ plane (4 counters)
+  const uint32_t cnt_fld = sm0 + 96u;                 // main warps that have consumed the current sigma / B plane
   const uint32_t gpring = sm0 + 128u;
   const uint32_t sring = gpring + ((kGpRing * gp_pitch + 127u) & ~127u);
   const uint32_t tring = sring + kRingS * slot_pitch;
@@ -142,22 +147,30 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
   // Anisotropy parameters depend on the column only: for every plane the halo warp looks up, once per 4-site group of the
   // strip, (e_x, e_y, e_z, 2 k_u/mu_s) by the group's grain id (the largest of its 4 columns' ids: vacant columns are 0 and
   // may borrow a neighbour's parameters, their spins are 0) and a flag "this group holds two different grains" (set-up
-  // flagged it in the column table; such groups gather per site).  Planes i0 - 1 + mm, ring slot mm % 8.
-  auto fill_gp = [&](int mm, int lane) {
-    if (lane < G) {
-      const int plane = i0 - 1 + mm, jg = j0 + 4 * lane;
-      float4 gp = make_float4(0.f, 0.f, 1.f, 0.f);
-      uint32_t flag = 0u;
-      if (plane >= 0 && plane < p.nx && jg < p.ny) {
-        const uint4 cid4 = __ldg(reinterpret_cast<const uint4*>(p.col + ((uint32_t)plane * (uint32_t)p.ny + (uint32_t)jg)));
-        const uint32_t gid = max(max(cid4.x & 0xFFFFu, cid4.y & 0xFFFFu), max(cid4.z & 0xFFFFu, cid4.w & 0xFFFFu));
-        flag = (cid4.x & COL_GROUP_MIXED) ? 1u : 0u;
-        gp = __ldg(p.grain + gid);
-        gp.w *= p.ngdt;                               // pre-scaled like every field term
-      }
+  // flagged it in the column table; such groups gather per site); lanes G and G + 1 do the same for the two halo columns.
+  // Planes i0 - 1 + mm, ring slot mm % 8.  The two dependent table reads of a plane are spread over two march steps
+  // (gp_lookup: column entries of plane mm -> packed id; gp_gather: id -> parameters; gp_store: parameters -> ring).
+  const int gl = tid - p.n_main;                        // lane of the parameter lookup (halo warp only)
+  const int gj = gl < G ? j0 + 4 * gl : (gl == G ? j0 - 1 : j0 + BY);
+  auto gp_lookup = [&](int mm) -> uint4 {               // raw column entries (a group's 4, or one halo column's)
+    const int plane = i0 - 1 + mm;
+    uint4 c4 = make_uint4(0u, 0u, 0u, 0u);
+    if (gl < 0 || gl >= G + 2 || plane < 0 || plane >= p.nx || gj < 0 || gj >= p.ny) return c4;
+    const uint32_t ci = (uint32_t)plane * (uint32_t)p.ny + (uint32_t)gj;
+    if (gl >= G) c4.x = __ldg(p.col + ci) & 0xFFFFu;
+    else c4 = __ldg(reinterpret_cast<const uint4*>(p.col + ci));
+    return c4;
+  };
+  auto gp_pack = [&](uint4 cid4) -> uint32_t {          // grain id | bit 31: two grains in the group
+    const uint32_t gid = max(max(cid4.x & 0xFFFFu, cid4.y & 0xFFFFu), max(cid4.z & 0xFFFFu, cid4.w & 0xFFFFu));
+    return gid | ((cid4.x & COL_GROUP_MIXED) ? 0x80000000u : 0u);
+  };
+  auto gp_gather = [&](uint32_t cg) -> float4 { return __ldg(p.grain + (cg & 0xFFFFu)); };
+  auto gp_store = [&](int mm, uint32_t cg, float4 gp) {
+    if (gl >= 0 && gl < G + 2) {
       const uint32_t slot = gpring + ((uint32_t)mm & (kGpRing - 1u)) * gp_pitch;
-      sts4(slot + 16u * (uint32_t)lane, gp.x, gp.y, gp.z, gp.w);
-      sts1(slot + 16u * (uint32_t)G + 4u * (uint32_t)lane, __uint_as_float(flag));
+      sts4(slot + 16u * (uint32_t)gl, gp.x, gp.y, gp.z, gp.w * p.ngdt);      // pre-scaled like every field term
+      if (gl < G) sts1(slot + 16u * (uint32_t)(G + 2) + 4u * (uint32_t)gl, __uint_as_float(cg >> 31));
     }
   };
 
@@ -171,14 +184,25 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
   asm volatile("bar.sync 0;" ::: "memory");
   if (tid == 0) {
     for (int s = 0; s < 4; ++s) {
-      mbar_init(bar_full + 8u * s, 1u); mbar_init(bar_done + 8u * s, 1u);
-      asm volatile("st.shared.u32 [%0], %1;" ::"r"(cnt_done + 4u * s), "r"(0u) : "memory");
+      mbar_init(bar_full + 8u * s, 1u); mbar_init(bar_done + 8u * s, blockDim.x / 32u);
     }
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(cnt_fld), "r"(0u) : "memory");
     mbar_init(bar_fld, 1u);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
-  if (!is_main) { fill_gp(0, tid - p.n_main); fill_gp(1, tid - p.n_main); }    // static tables: no need to wait for the previous grid
+  // planes 0 and 1 of the march directly, plane 2 gathered, plane 3 looked up (static tables: no need to wait for the
+  // previous grid)
+  uint4 cid_next = make_uint4(0u, 0u, 0u, 0u);
+  float4 gp_next = make_float4(0.f, 0.f, 1.f, 0.f);
+  uint32_t cg_gath = 0u;
+  if (!is_main) {
+    const uint32_t c0 = gp_pack(gp_lookup(0)), c1 = gp_pack(gp_lookup(1));
+    cg_gath = gp_pack(gp_lookup(2)); cid_next = gp_lookup(3);
+    const float4 g0 = gp_gather(c0), g1 = gp_gather(c1);
+    gp_next = gp_gather(cg_gath);
+    gp_store(0, c0, g0); gp_store(1, c1, g1);
+  }
   // Programmatic dependent launch: everything above overlaps the tail of the previous step's grid; nothing below the
   // wait runs before that grid has completed (it wrote the spins this one reads and read the buffer this one writes).
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
@@ -207,8 +231,7 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
   const float lambda = p.lambda;
   const uint32_t planep = (uint32_t)(NZ * p.nyp);
   auto done_bar = [&](int m) { return bar_done + 8u * (uint32_t)(m & 3); };
-  const uint32_t nwarps = blockDim.x / 32u;
-  auto arrive_done = [&](int m) { warp_arrive(cnt_done + 4u * (uint32_t)(m & 3), done_bar(m), nwarps); };
+  auto arrive_done = [&](int m) { warp_arrive(done_bar(m)); };
   auto phase = [](int m) { return (uint32_t)(m >> 2) & 1u; };
 
   if (is_main) {
@@ -219,7 +242,7 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
     // own float4 inside component 0 of a slot (inactive threads read a valid dummy position and write nothing)
     const uint32_t own_b = active ? (uint32_t)(((k + 1) * W + 4 + 4 * g) * 4) : (uint32_t)((W + 4) * 4);
     const uint32_t fown = fbox + (active ? (uint32_t)((k * BY + 4 * g) * 4) : 0u);
-    const uint32_t gown = gpring + 16u * (uint32_t)g, gflag = gpring + 16u * (uint32_t)G + 4u * (uint32_t)g;
+    const uint32_t gown = gpring + 16u * (uint32_t)g, gflag = gpring + 16u * (uint32_t)(G + 2) + 4u * (uint32_t)g;
     // element of the group in predictor plane q = i0 - 1 (wraps below zero for q = -1; not dereferenced then)
     uint32_t e = (uint32_t)(p.lead + ((i0 - 1) * NZ + k) * p.nyp + j);
     uint32_t ec = (uint32_t)((i0 - 1) * p.ny + j);                      // column (q, j) of the window
@@ -316,6 +339,12 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
             Bn[2][v] = fmaf(sgs, xi[v][2], sscale * bz[v]);
           }
         }
+        // the field box is refilled as soon as the last main warp has its values in registers (mid-predictor): the copy
+        // has the rest of the march step to land.  That warp issues it.
+        if (warp_count_last(cnt_fld, (uint32_t)p.n_main / 32u) && m + 1 <= L + 1) {
+          issue_F(m + 1);
+          if (m + 4 <= L + 1) tma_prefetch_4d(&mapF, j0, 0, i0 - 1 + m + 4, AR_SIGMA);
+        }
         float St[3][4];
 #pragma unroll
         for (int v = 0; v < 4; ++v) {
@@ -371,12 +400,8 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
 #pragma unroll
         for (int v = 0; v < 4; ++v) Bp[c][v] += Bs[c][v];
 
-      mbar_wait_long(done_bar(m), phase(m));           // S~ plane q complete; S plane q - 1 and the field box are free
-      if (tid == 0) {
-        if (m + kRingS <= L + 3) issue_S(m + kRingS);
-        if (m + 1 <= L + 1) issue_F(m + 1);
-        if (m + 4 <= L + 1) tma_prefetch_4d(&mapF, j0, 0, i0 - 1 + m + 4, AR_SIGMA);
-      }
+      mbar_wait_long(done_bar(m), phase(m));           // S~ plane q complete; S plane q - 1 is free
+      if (tid == 0 && m + kRingS <= L + 3) issue_S(m + kRingS);
 
       // ---- second part: the x+1 plane, torque, update, store ----
       {
@@ -458,19 +483,23 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
       const int q = i0 - 1 + m;
       const bool qin = (q >= 0) && (q < p.nx);
       float sg[2] = {0.f, 0.f}, bx[2] = {0.f, 0.f}, by[2] = {0.f, 0.f}, bz[2] = {0.f, 0.f};
-      uint32_t cid[2] = {0u, 0u};
 #pragma unroll
       for (int s = 0; s < 2; ++s)
         if (act[s] && qin) {
           const uint32_t es = e + (uint32_t)jh[s];
-          cid[s] = __ldg(p.col + (ec + (uint32_t)jh[s]));
           sg[s] = ldg_stream1(base + (p.oSigma + es));
           bx[s] = ldg_stream1(base + (p.oB + es));
           by[s] = ldg_stream1(base + (p.oB + p.as + es));
           bz[s] = ldg_stream1(base + (p.oB + 2u * p.as + es));
         }
-      // slot (m + 2) % 8 of the parameter ring was last read in march step m - 5
-      fill_gp(m + 2, k);
+      // parameter ring: plane m + 2 (gathered during the previous march step) goes to slot (m + 2) % 8, last read in
+      // march step m - 5; plane m + 3 is gathered, plane m + 4 looked up
+      asm volatile("" : "+r"(cid_next.x), "+r"(cid_next.y), "+r"(cid_next.z), "+r"(cid_next.w), "+f"(gp_next.x),
+                   "+f"(gp_next.y), "+f"(gp_next.z), "+f"(gp_next.w)::"memory");   // first use of last step's loads: here, not earlier
+      gp_store(m + 2, cg_gath, gp_next);
+      cg_gath = gp_pack(cid_next);
+      gp_next = gp_gather(cg_gath);
+      cid_next = gp_lookup(m + 4);
       mbar_wait_long(bar_full + 8u * (uint32_t)((m + 2) & (kRingS - 1)), phase(m + 2));
       const uint32_t cur = sring + (uint32_t)((m + 1) & 3) * slot_pitch, next = sring + (uint32_t)((m + 2) & 3) * slot_pitch;
       const uint32_t tslot = tring + t3 * slot_pitch;
@@ -505,8 +534,7 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
               Bex[c] = fmaf(p.j3s, s3, fmaf(p.j2s, zs[c], p.j1s * (xs + ys)));
             }
           }
-          float4 gp = __ldg(p.grain + (cid[s] & 0xFFFFu));
-          gp.w *= p.ngdt;
+          const float4 gp = lds4(gpring + ((uint32_t)m & (kGpRing - 1u)) * gp_pitch + 16u * (uint32_t)(G + s));
           const float ca = gp.w * fmaf(Xs[0], gp.x, fmaf(Xs[1], gp.y, Xs[2] * gp.z));
           const float sgs = p.ngdt * sg[s];
           float f[3];
@@ -560,7 +588,7 @@ inline int round_up32(int v) { return (v + 31) / 32 * 32; }
 
 uint32_t plan_smem(int nz, int by, uint32_t& slot_pitch) {
   slot_pitch = (uint32_t)align_up((size_t)3 * (nz + 2) * (by + 8) * 4, 128);
-  return 128u + (uint32_t)align_up((size_t)kGpRing * (size_t)((20 * (by / 4) + 15) & ~15), 128) + (kRingS + kRingT) * slot_pitch +
+  return 128u + (uint32_t)align_up((size_t)kGpRing * (size_t)((20 * (by / 4) + 32 + 15) & ~15), 128) + (kRingS + kRingT) * slot_pitch +
          (uint32_t)align_up((size_t)4 * nz * by * 4, 128);
 }
 

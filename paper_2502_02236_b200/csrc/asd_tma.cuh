@@ -36,8 +36,17 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     if (++spins > (1u << 24)) __trap();
   }
 }
-// The same with a suspend-time hint: the thread sleeps in hardware for up to ~`ticks` ns per attempt, so a long wait
-// costs a handful of issue slots instead of a busy loop.
+// Wait that backs off: a barrier that is not ready yet is polled every ~`ns` nanoseconds instead of in a busy loop (a
+// spinning warp takes issue slots from the warps it is waiting for).  Traps instead of hanging if the phase never comes.
+__device__ __forceinline__ void mbar_wait_sleep(uint32_t bar, uint32_t parity, uint32_t ns) {
+  if (mbar_try_wait(bar, parity)) return;
+  uint32_t spins = 0;
+  do {
+    asm volatile("nanosleep.u32 %0;" ::"r"(ns));
+    if (++spins > (1u << 22)) __trap();
+  } while (!mbar_try_wait(bar, parity));
+}
+// Wait with a suspend-time hint: the thread sleeps in hardware until the barrier's state changes or the hint expires.
 __device__ __forceinline__ void mbar_wait_long(uint32_t bar, uint32_t parity) {
   uint32_t spins = 0, ok;
   do {
@@ -47,7 +56,7 @@ __device__ __forceinline__ void mbar_wait_long(uint32_t bar, uint32_t parity) {
         "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n"
         "selp.u32 %0, 1, 0, p;\n"
         "}\n" : "=r"(ok) : "r"(bar), "r"(parity), "r"(1000000u) : "memory");
-    if (!ok && ++spins > (1u << 20)) __trap();
+    if (!ok && ++spins > (1u << 22)) __trap();
   } while (!ok);
 }
 __device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap* map, int c0, int c1, int c2, int c3) {
