@@ -191,18 +191,6 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
-  // planes 0 and 1 of the march directly, plane 2 gathered, plane 3 looked up (static tables: no need to wait for the
-  // previous grid)
-  uint4 cid_next = make_uint4(0u, 0u, 0u, 0u);
-  float4 gp_next = make_float4(0.f, 0.f, 1.f, 0.f);
-  uint32_t cg_gath = 0u;
-  if (!is_main) {
-    const uint32_t c0 = gp_pack(gp_lookup(0)), c1 = gp_pack(gp_lookup(1));
-    cg_gath = gp_pack(gp_lookup(2)); cid_next = gp_lookup(3);
-    const float4 g0 = gp_gather(c0), g1 = gp_gather(c1);
-    gp_next = gp_gather(cg_gath);
-    gp_store(0, c0, g0); gp_store(1, c1, g1);
-  }
   // Programmatic dependent launch: everything above overlaps the tail of the previous step's grid; nothing below the
   // wait runs before that grid has completed (it wrote the spins this one reads and read the buffer this one writes).
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
@@ -225,6 +213,19 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
     for (int m = 1; m <= 3 && m <= L + 1; ++m) tma_prefetch_4d(&mapF, j0, 0, i0 - 1 + m, AR_SIGMA);
   }
 
+  // Parameter ring: planes 0 and 1 of the march directly, plane 2 gathered, plane 3 looked up.  Done after the first
+  // TMA loads have been issued, so that these two dependent table reads overlap the flight of the first S planes; the
+  // main threads meet the halo warp at named barrier 1 before their first use.
+  uint4 cid_next = make_uint4(0u, 0u, 0u, 0u);
+  float4 gp_next = make_float4(0.f, 0.f, 1.f, 0.f);
+  uint32_t cg_gath = 0u;
+  if (!is_main) {
+    const uint32_t c0 = gp_pack(gp_lookup(0)), c1 = gp_pack(gp_lookup(1));
+    cg_gath = gp_pack(gp_lookup(2)); cid_next = gp_lookup(3);
+    const float4 g0 = gp_gather(c0), g1 = gp_gather(c1);
+    gp_next = gp_gather(cg_gath);
+    gp_store(0, c0, g0); gp_store(1, c1, g1);
+  }
   uint32_t n_lo = p.n_lo, n_hi = p.n_hi; float scale = p.scale;
   resolve_dyn(p.dyn, n_lo, n_hi, scale);
   const float sscale = p.ngdt * scale;                // B'_app = sscale * B
@@ -264,6 +265,7 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
 
     mbar_wait_long(bar_full + 0u, 0u);
     mbar_wait_long(bar_full + 8u, 0u);
+    asm volatile("bar.sync 1;" ::: "memory");          // the parameter ring's first planes are in place
     if (LAT == LAT_L10) {
 #pragma unroll
       for (int c = 0; c < 3; ++c) {
@@ -463,6 +465,7 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
     uint64_t gsite = p.g0 + (uint64_t)(int64_t)(((int64_t)(i0 - 1) * NZ + k) * p.ny);
     const uint32_t gplane = (uint32_t)(NZ * p.ny);
 
+    asm volatile("bar.sync 1;" ::: "memory");          // planes 0, 1 of the parameter ring are stored
     mbar_wait_long(bar_full + 0u, 0u);
     mbar_wait_long(bar_full + 8u, 0u);
     // window: rP = plane q-1, rC = plane q; [side][component][column y-1, y, y+1]
@@ -603,10 +606,15 @@ struct FusedPlan {
 
 bool heun_fused_supported(const Ctx& c) { return heun_fast_supported(c) && c.d.nz + 2 <= 256; }
 
-// ASD_KERNEL_AUTO takes the fused step for windows that stream from HBM and give every CTA a march of some length:
-// more than 2^21 sites and at least 64 planes.  Smaller films are L2-resident or launch-bound; there the two stage
-// kernels (or their graph replay) stay in charge.
-bool heun_fused_preferred(const Ctx& c) { return c.N > (1ll << 21) && c.d.nx >= 64; }
+// ASD_KERNEL_AUTO takes the fused step for windows that stream from HBM (more than 2^21 sites) and give every CTA a march
+// of at least 8 planes (a chunk recomputes the predictor of 2 extra planes).  Smaller films are L2-resident or launch-
+// bound; there the two stage kernels (or their graph replay) stay in charge.  Measured (B200, G updates/s, two-kernel ->
+// fused): cfg4 46.0 -> 55.3, cfg3 42.9 -> 46.6, cfg2 46.6 -> 32.3, cfg1 48.9 -> 41.3.
+bool heun_fused_preferred(Ctx& c) {
+  if (c.N <= (1ll << 21)) return false;
+  const FusedPlan* pl = fused_plan(c);
+  return pl && pl->CX >= 8;
+}
 
 namespace {
 

@@ -235,7 +235,7 @@ TmaPlan* tma_plan(Ctx& c);                                    // nullptr if the 
 void tma_plan_free(Ctx& c);
 asd_status launch_heun_fused(Ctx& c, StageParams& p);         // one Heun step (1 kernel); swaps the roles of the spin buffers
 bool heun_fused_supported(const Ctx& c);
-bool heun_fused_preferred(const Ctx& c);                      // what ASD_KERNEL_AUTO asks
+bool heun_fused_preferred(Ctx& c);                            // what ASD_KERNEL_AUTO asks (builds the plan)
 FusedPlan* fused_plan(Ctx& c);
 void fused_plan_free(Ctx& c);
 void fill_stage_params(const Ctx& c, StageParams& p);

@@ -46,6 +46,19 @@ __device__ __forceinline__ void mbar_wait_sleep(uint32_t bar, uint32_t parity, u
     if (++spins > (1u << 22)) __trap();
   } while (!mbar_try_wait(bar, parity));
 }
+// Busy poll (mbarrier.test_wait never suspends): the shortest wake-up latency, for waits that sit on the critical path.
+__device__ __forceinline__ void mbar_wait_spin(uint32_t bar, uint32_t parity) {
+  uint32_t spins = 0, ok;
+  do {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    if (!ok && ++spins > (1u << 26)) __trap();
+  } while (!ok);
+}
 // Wait with a suspend-time hint: the thread sleeps in hardware until the barrier's state changes or the hint expires.
 __device__ __forceinline__ void mbar_wait_long(uint32_t bar, uint32_t parity) {
   uint32_t spins = 0, ok;
