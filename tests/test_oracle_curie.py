@@ -4,12 +4,15 @@ T_C = eps z J / (3 k_B) with eps_SC = 0.72, z = 6  =>  T_C = 1.44 J / k_B   (PAP
 This is a whole-loop check: noise amplitude, exchange normalisation (Eq. (2)), the same-noise rule and
 the integrator all have to be right for the order-disorder transition to sit where the paper says.
 
-Two tiers (P8):
-  * always on (about 20 s): the transition is BRACKETED by 0.85 T_C and 1.15 T_C.  A thermal field wrong by a
-    factor sqrt(2) or sqrt(1 + lambda^2) in amplitude moves the apparent T_C by a factor 2 and fails this.
-  * opt-in (ASD_SLOW=1, about 10 min on 8 cores): T_C from a power-law fit, extrapolated linearly to dt -> 0
-    (stochastic Heun has an O(dt) bias of the stationary distribution: +6 % at dt = 1 fs, lambda = 1), within
-    3 % of 1.44 J/k_B.  Last recorded result: DESIGN.md sec. 3.
+Three checks (P8), all on the default path:
+  * the transition is BRACKETED by 0.85 T_C and 1.15 T_C (about 20 s).  A thermal field wrong by a factor sqrt(2) or
+    sqrt(1 + lambda^2) in amplitude moves the apparent T_C by a factor 2 and fails this.
+  * the quantitative value: tests/golden/p8_curie_record.json, written by tests/golden/gen_p8_curie.py (which calls only
+    oracle/; L = 24, two time steps, power-law fit, linear extrapolation to dt -> 0 -- stochastic Heun has an O(dt) bias of
+    the stationary distribution: +3.7 % at dt = 0.5 fs, lambda = 1) must be within 3 % of 1.44 J/k_B, and must have been
+    written by THIS oracle (SHA-256 of oracle/asd_oracle.cpp);
+  * the record is tied to the live oracle by replaying its first temperature point (same seed, same steps: the oracle
+    is deterministic, so m(575 K) must come out the same to rounding).
 """
 import os
 
@@ -52,20 +55,29 @@ def test_p8_transition_is_bracketed_by_the_paper_curie_temperature():
     assert above < 0.16, above
 
 
-@pytest.mark.skipif(os.environ.get("ASD_SLOW") != "1", reason="about 10 minutes; set ASD_SLOW=1")
-def test_p8_curie_temperature_extrapolated_to_zero_time_step():
-    from scipy.optimize import curve_fit
-    temps = np.arange(575.0, 751.0, 25.0)
-    tc = []
-    for dt, nsteps in ((5e-16, 8000), (2.5e-16, 16000)):
-        o, N = _bulk(24, dt)
-        m = np.array([_mean_m(o, N, T, nsteps // 2, nsteps // 2) for T in temps])
-        sel = m > 0.25
-        f = lambda T, Tc, b: np.clip(1.0 - T / Tc, 1e-12, None) ** b
-        p, _cov = curve_fit(f, temps[sel], m[sel], p0=(720.0, 0.36))
-        print("dt", dt, "m(T)", np.round(m, 4), "fit T_C, beta", p)
-        tc.append(p[0])
-    tc0 = 2.0 * tc[1] - tc[0]                      # linear extrapolation dt -> 0
-    print("T_C(dt->0) =", tc0, "paper", TC_PAPER)
-    assert tc[0] > tc[1] > 0.99 * TC_PAPER         # the O(dt) bias raises the apparent T_C
-    assert abs(tc0 / TC_PAPER - 1.0) < 0.03
+def _record():
+    import json
+    here = os.path.dirname(os.path.abspath(__file__))
+    return json.load(open(os.path.join(here, "golden", "p8_curie_record.json")))
+
+
+def test_p8_curie_temperature_extrapolated_to_zero_time_step_record():
+    import hashlib
+    rec = _record()
+    src = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "oracle", "asd_oracle.cpp")
+    assert rec["oracle_sha256"] == hashlib.sha256(open(src, "rb").read()).hexdigest(), \
+        "oracle/asd_oracle.cpp changed: re-run tests/golden/gen_p8_curie.py"
+    assert abs(rec["T_C_paper"] - TC_PAPER) < 1e-9 and rec["J"] == J and rec["L"] == 24
+    tc = [r["T_C_fit"] for r in rec["runs"]]
+    assert rec["runs"][0]["dt"] == 5e-16 and rec["runs"][1]["dt"] == 2.5e-16
+    assert tc[0] > tc[1] > 0.99 * TC_PAPER                       # the O(dt) bias raises the apparent T_C
+    assert abs(rec["T_C_dt0"] - (2.0 * tc[1] - tc[0])) < 1e-9    # linear extrapolation dt -> 0
+    assert abs(rec["T_C_dt0"] / TC_PAPER - 1.0) < 0.03, rec["T_C_dt0"]
+
+
+def test_p8_record_first_point_replayed_by_the_live_oracle():
+    rec = _record()
+    run = rec["runs"][0]
+    o, N = _bulk(rec["L"], run["dt"])
+    m = _mean_m(o, N, rec["temps_K"][0], run["steps_per_T"] // 2, run["steps_per_T"] // 2)
+    assert abs(m - run["m"][0]) < 1e-9, (m, run["m"][0])
