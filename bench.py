@@ -133,10 +133,7 @@ def reduce_over_ranks(ms_local: float, updates_local: float, dist=None, device="
 def _gpu_desc(asd, w: ai.Workload, ell=None):
     """Workload -> asd.LatticeDesc (argument marshalling; the product path never imports oracle/ or tests/)."""
     extra = {} if ell is None else {"ell_idx": ell[0], "ell_J": ell[1]}
-    return asd.LatticeDesc(**extra, lattice=w.lattice, nx=w.nx, ny=w.ny, nz=w.nz, pbc=w.pbc, mu_s=w.mu_s, lam=w.lam,
-                           gamma=w.gamma, dt=w.dt, J=w.J, track_nx=w.track_nx, x0=w.x0, grain_map=w.grain_map,
-                           n_grains=w.n_grains, grain_ku=w.grain_ku, grain_axis=w.grain_axis, macro=w.macro,
-                           seed=w.seed)
+    return asd.desc_from_workload(w, **extra)
 
 
 def _drive(w: ai.Workload, heun_per_step: int):
@@ -302,8 +299,8 @@ def run_ours(args):
 
 # ------------------------------------------------------------------------------------------------------------
 def _oracle_for(w: ai.Workload):
-    from tests.helpers import oracle_from_workload
-    return oracle_from_workload(w)
+    from oracle import asd_oracle as orc
+    return orc.from_workload(w)
 
 
 def _crop(w: ai.Workload, nx: int) -> ai.Workload:

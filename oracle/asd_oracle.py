@@ -327,3 +327,21 @@ class Oracle:
 
     def sigma(self, T: float) -> float:
         return float(lib().orc_sigma(self._h, C.c_double(T)))
+
+
+def spec_from_workload(w, **over) -> "LatticeSpec":
+    """asd_inputs.Workload -> LatticeSpec (argument marshalling only)."""
+    d = dict(lattice=w.lattice, nx=w.nx, ny=w.ny, nz=w.nz, pbc=w.pbc, mu_s=w.mu_s, lam=w.lam, gamma=w.gamma,
+             dt=w.dt, J=w.J, track_nx=w.track_nx, x0=w.x0, grain_map=w.grain_map,
+             grain_ku=np.asarray(w.grain_ku, dtype=np.float64), grain_axis=np.asarray(w.grain_axis, dtype=np.float64),
+             macro=w.macro, seed=w.seed)
+    d.update(over)
+    return LatticeSpec(**d)
+
+
+def from_workload(w, **over) -> "Oracle":
+    """An Oracle holding the workload's lattice, spins and fields."""
+    o = Oracle(spec_from_workload(w, **over))
+    o.set_spins(w.sx, w.sy, w.sz)
+    o.set_fields(w.T, w.Bx, w.By, w.Bz)
+    return o

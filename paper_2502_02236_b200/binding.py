@@ -305,7 +305,7 @@ class Context:
         import torch
         nbytes = int(self._L.asd_demag_workspace_bytes(self._h))
         if nbytes == 0:
-            raise AsdError("asd_demag_workspace_bytes failed (cuFFT plan)")
+            raise AsdError(5, "asd_demag_workspace_bytes failed")
         self._demag_ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
         ptr = (self._demag_ws.data_ptr() + 255) & ~255
         a = (C.c_double * 3)(*[float(x) for x in spacing_m])
@@ -369,3 +369,23 @@ class Context:
 
     def launch_count(self) -> int:
         return int(self._L.asd_launch_count(self._h))
+
+
+def desc_from_workload(w, **over) -> "LatticeDesc":
+    """asd_inputs.Workload -> LatticeDesc (argument marshalling only)."""
+    d = dict(lattice=w.lattice, nx=w.nx, ny=w.ny, nz=w.nz, pbc=w.pbc, mu_s=w.mu_s, lam=w.lam, gamma=w.gamma,
+             dt=w.dt, J=w.J, track_nx=w.track_nx, x0=w.x0, grain_map=w.grain_map, n_grains=w.n_grains,
+             grain_ku=w.grain_ku, grain_axis=w.grain_axis, macro=w.macro, seed=w.seed)
+    d.update(over)
+    return LatticeDesc(**d)
+
+
+def context_from_workload(w, device: str = "cuda:0", **over) -> "Context":
+    """A Context holding the workload's lattice, spins and fields (uploaded from host arrays)."""
+    import torch
+    ctx = Context(desc_from_workload(w, **over), device=device)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).to(ctx.device)
+    ctx.set_spins(t(w.sx), t(w.sy), t(w.sz))
+    ctx.set_fields(t(w.T), t(w.Bx), t(w.By), t(w.Bz))
+    torch.cuda.synchronize()
+    return ctx

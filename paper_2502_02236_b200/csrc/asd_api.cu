@@ -9,7 +9,8 @@
 
 namespace asd {
 
-static const char* g_static_err = "no error";
+// message of the last failure that has no context to carry it (create, NULL ctx); per thread, not process-wide
+static thread_local const char* g_static_err = "no error";
 
 bool validate_desc(const asd_lattice_desc* d, const char** why) {
   auto bad = [&](const char* m) { if (why) *why = m; return false; };
@@ -159,9 +160,11 @@ asd_status asd_create_lattice(const asd_lattice_desc* desc, void* d_workspace, s
   auto bail = [&](asd_status s) { g_static_err = "asd_create_lattice failed in CUDA set-up (see stderr)";
                                   std::fprintf(stderr, "libasd: %s\n", c.err);
                                   if (c.host_scratch) cudaFreeHost(c.host_scratch);
+                                  if (c.grain_scratch) cudaFreeHost(c.grain_scratch);
                                   delete h; return s; };
 #define CREATE_TRY(expr) do { cudaError_t e__ = (expr); if (e__ != cudaSuccess) { fail_cuda(c, e__, #expr); return bail(ASD_ECUDA); } } while (0)
   CREATE_TRY(cudaMallocHost(&c.host_scratch, 4 * sizeof(double)));
+  CREATE_TRY(cudaMallocHost(&c.grain_scratch, sizeof(long long) * 4 * (size_t)desc->n_grains));
   CREATE_TRY(cudaMemsetAsync(d_workspace, 0, L.total, c.stream));
   const size_t ncol = (size_t)(desc->track_nx * desc->ny);
   if (desc->grain_map)
@@ -221,6 +224,7 @@ asd_status asd_create_lattice(const asd_lattice_desc* desc, void* d_workspace, s
 asd_status asd_destroy(asd_ctx* ctx) {
   if (!ctx) return ASD_EINVAL;
   if (ctx->c.host_scratch) cudaFreeHost(ctx->c.host_scratch);
+  if (ctx->c.grain_scratch) cudaFreeHost(ctx->c.grain_scratch);
   asd::tma_plan_free(ctx->c);
   asd::fused_plan_free(ctx->c);
   asd::graphs_free(ctx->c);

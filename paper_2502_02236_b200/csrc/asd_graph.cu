@@ -8,6 +8,7 @@
 // buffer holds S, the kernel variant) changes only on a window shift or an asd_set_kernel call, and those drop the
 // cache.  Graphs are recorded on an internal stream (the caller's may be the legacy default stream, which cannot be
 // captured) and launched on the caller's.  Results are bit-identical to plain launches: same kernels, same order.
+#include <cstring>
 #include <vector>
 
 #include "asd_internal.cuh"
@@ -38,10 +39,17 @@ cudaGraphExec_t record(Ctx& c, int64_t n) {
     return nullptr;
   }
   const int64_t launches_before = c.launches;
+  const bool failed_before = c.cuda_failed;
+  char err_before[sizeof(c.err)];
+  std::memcpy(err_before, c.err, sizeof(c.err));
   c.launch_stream = c.cap_stream;
   const asd_status st = launch_heun_direct(c, n, dyn_state(c));
   c.launch_stream = c.stream;
   c.launches = launches_before;                // recording is not launching
+  if (st != ASD_OK) {                          // a launch refused during capture is not a sticky device error:
+    c.cuda_failed = failed_before;             // the caller falls back to plain launches
+    std::memcpy(c.err, err_before, sizeof(c.err));
+  }
   cudaGraph_t g = nullptr;
   const cudaError_t e = cudaStreamEndCapture(c.cap_stream, &g);
   if (st != ASD_OK || e != cudaSuccess || !g) {

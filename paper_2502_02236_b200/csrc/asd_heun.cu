@@ -109,12 +109,10 @@ __global__ void __launch_bounds__(256) heun_stage_general(const StageParams p) {
 #pragma unroll
         for (int v = 0; v < VEC; ++v) {
           const int64_t q = (int64_t)s * p.N + l0 + v;
-          const int32_t n = __ldg(p.ell_idx + q);
-          if (n >= 0) {
-            const float Jt = __ldg(p.ell_J + q);
+          const int32_t n = __ldg(p.ell_idx + q);          // an empty slot holds the site itself with J = 0
+          const float Jt = __ldg(p.ell_J + q);
 #pragma unroll
-            for (int c = 0; c < 3; ++c) Bex[c][v] = fmaf(Jt, __ldg(X + (size_t)c * p.as + n), Bex[c][v]);
-          }
+          for (int c = 0; c < 3; ++c) Bex[c][v] = fmaf(Jt, __ldg(X + (size_t)c * p.as + n), Bex[c][v]);
         }
       }
     } else {

@@ -99,7 +99,8 @@ struct StageParams {
   const float4* grain;         // (e_x, e_y, e_z, 2 k_u / mu_s) per grain id + 1 (entry 0 = vacant: zeros)
   const float* aniso;          // per-column SoA copy of the same: e_x | e_y | e_z | 2k_u/mu_s, each [track_nx*ny],
   uint32_t aniso_stride;       //   at the window origin; component stride in elements
-  const int32_t* ell_idx;      // general ELL, slot-major [W][N], entries are padded element offsets (or -1)
+  const int32_t* ell_idx;      // general ELL, slot-major [W][N]: padded element offset of the neighbour; an empty slot
+                               // holds the site itself with J = 0 (ell_transpose_kernel), never -1
   const float* ell_J;          // J_ij / mu_s [Tesla], slot-major
   int32_t ell_w;
   int32_t nx, ny, nz, nyp;     // nyp = padded row stride
@@ -158,6 +159,7 @@ struct Ctx {
   double *partials = nullptr;       // [kMaxPartialBlocks*4]
   long long *grain_acc = nullptr;   // [n_grains*4] fixed-point sums and counts
   double *host_scratch = nullptr;   // pinned, 4 doubles
+  long long *grain_scratch = nullptr;   // pinned, [n_grains*4]: asd_grain_magnetisation's device-to-host landing area
   // state
   float scale = 1.0f;
   int64_t step = 0, shift = 0, pass = 0, x0 = 0;

@@ -94,17 +94,14 @@ asd_status launch_grain_magnetisation(Ctx& c, double* m_host) {
   grain_accumulate<<<(unsigned)((ncol + 127) / 128), 128, 0, c.stream>>>(S.x, S.y, S.z, c.col_win(), c.d.nx, c.d.ny,
                                                                         c.d.nz, c.nyp, c.lead, c.grain_acc);
   ASD_LAUNCH_CHECK(c, "grain_accumulate");
-  long long* h = nullptr;
-  ASD_CUDA_TRY(c, cudaMallocHost(&h, sizeof(long long) * 4 * (size_t)G));
-  cudaError_t e = cudaMemcpyAsync(h, c.grain_acc, sizeof(long long) * 4 * (size_t)G, cudaMemcpyDeviceToHost, c.stream);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(c.stream);
-  if (e != cudaSuccess) { cudaFreeHost(h); return fail_cuda(c, e, "grain magnetisation copy"); }
+  long long* h = c.grain_scratch;                      // pinned, allocated once at create time
+  ASD_CUDA_TRY(c, cudaMemcpyAsync(h, c.grain_acc, sizeof(long long) * 4 * (size_t)G, cudaMemcpyDeviceToHost, c.stream));
+  ASD_CUDA_TRY(c, cudaStreamSynchronize(c.stream));
   for (int g = 0; g < G; ++g) {
     const double cnt = (double)h[4 * g + 3];
     for (int a = 0; a < 3; ++a)
       m_host[3 * g + a] = cnt > 0.0 ? ((double)h[4 * g + a] / 4294967296.0) / cnt : 0.0;
   }
-  cudaFreeHost(h);
   return ASD_OK;
 }
 

@@ -99,7 +99,8 @@ __global__ void pack_field_kernel(const float* __restrict__ src, float* __restri
   if (j < ny) {
     v = src[r * ny + j];
     // sigma_i = c_th sqrt(T_i), c_th = sqrt(2 lambda k_B / (gamma mu_s dt))  [Tesla]  (P:38 with mu_0 absorbed)
-    if (take_sqrt) v = scale * sqrtf(v);
+    // (T < 0 or NaN gives sigma = 0 instead of a NaN that would spread through the exchange field)
+    if (take_sqrt) v = scale * sqrtf(fmaxf(v, 0.0f));
   }
   dst[t + lead] = v;
 }
