@@ -48,18 +48,44 @@ def _oracle_curve(lattice):
 
 
 @pytest.mark.parametrize("lattice", [ai.SC, ai.L10])
-@pytest.mark.parametrize("kernel", ["general", "fast", "tma"])
+@pytest.mark.parametrize("kernel", ["general", "fast", "tma", "fused"])
 def test_film_m_of_t_and_curie_temperature(lattice, kernel):
     import paper_2502_02236_b200 as asd
     w = _film(lattice)
     temps = _temps(lattice)
     m_o = _oracle_curve(lattice)
     g = gpu_from_workload(w)
-    g.set_kernel({"general": asd.KERNEL_GENERAL, "fast": asd.KERNEL_FAST, "tma": asd.KERNEL_TMA}[kernel])
+    g.set_kernel({"general": asd.KERNEL_GENERAL, "fast": asd.KERNEL_FAST, "tma": asd.KERNEL_TMA,
+                  "fused": asd.KERNEL_FUSED}[kernel])
     m_g = sweep(Side(g, w.n_sites, True), temps, N_STEPS, grain_weights=_weights(w))
     tc_o, _ = fit_tc(temps, m_o)
     tc_g, _ = fit_tc(temps, m_g)
     print(f"lattice {lattice} kernel {kernel}: M_oracle {np.round(m_o, 4)} M_gpu {np.round(m_g, 4)} "
+          f"T_C oracle {tc_o:.1f} K gpu {tc_g:.1f} K")
+    assert np.abs(m_g - m_o).max() <= TOL_M
+    assert abs(tc_g / tc_o - 1.0) <= TOL_TC
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("kernel", ["fast", "fused"])
+def test_cfg1_structure_mid_size_m_of_t_and_curie_temperature(kernel):
+    """BASELINE configs[1]'s own structure -- 8 nm Voronoi grains, 1 nm vacant boundaries, 27 planes thick, lambda = 1,
+    dt = 1 fs, state carried from one temperature to the next -- on a 96 x 96 x 27 film (a quarter of cfg1's area, the
+    largest the oracle sweeps in about two minutes): M(T) within 0.02 and T_C within 2 % of the oracle."""
+    import paper_2502_02236_b200 as asd
+    w = ai.small_film(ai.SC, 96, 96, 27, pitch_nm=8.0, boundary_nm=1.0, lam=1.0, dt=1e-15, spot=False, uniform_T=300.0,
+                      bz=0.0)
+    temps = np.array([450.0, 550.0, 600.0, 650.0, 700.0, 800.0])
+    n_steps = 1500
+    if "cfg1mid" not in _ORACLE:
+        _ORACLE["cfg1mid"] = sweep(Side(oracle_from_workload(w), w.n_sites, False), temps, n_steps, grain_weights=_weights(w))
+    m_o = _ORACLE["cfg1mid"]
+    g = gpu_from_workload(w)
+    g.set_kernel({"fast": asd.KERNEL_FAST, "fused": asd.KERNEL_FUSED}[kernel])
+    m_g = sweep(Side(g, w.n_sites, True), temps, n_steps, grain_weights=_weights(w))
+    tc_o, _ = fit_tc(temps, m_o)
+    tc_g, _ = fit_tc(temps, m_g)
+    print(f"cfg1 structure 96x96x27, kernel {kernel}: M_oracle {np.round(m_o, 4)} M_gpu {np.round(m_g, 4)} "
           f"T_C oracle {tc_o:.1f} K gpu {tc_g:.1f} K")
     assert np.abs(m_g - m_o).max() <= TOL_M
     assert abs(tc_g / tc_o - 1.0) <= TOL_TC

@@ -151,13 +151,25 @@ def test_counters_resume_bit_exact():
 _FULL = {}
 
 
-def _full_size_oracle(cfg, w):
-    """Oracle spins after 2 Heun steps of a full-size config (computed once per session, shared by the variants)."""
-    if cfg not in _FULL:
-        o = oracle_from_workload(w)
-        o.step_heun(2)
-        _FULL[cfg] = o.get_spins()
-    return _FULL[cfg]
+def _full_size_workload(cfg):
+    w = ai.make_config(cfg)
+    sx, sy, sz = ai.tilted_spins(w.n_sites, 20.0, seed=4)
+    mag = w.magnetic_mask().reshape(-1)
+    w.sx, w.sy, w.sz = sx * mag, sy * mag, sz * mag
+    return w
+
+
+def _full_size_oracle(cfg, w, ell=None):
+    """Oracle spins after 1 and after 2 Heun steps of a full-size config (computed once per session, shared by the
+    kernel variants; the ELL run has its own entry: it exercises the oracle's table branch)."""
+    key = (cfg, ell is not None)
+    if key not in _FULL:
+        o = oracle_from_workload(w) if ell is None else oracle_from_workload(w, ell_idx=ell[0], ell_J=ell[1].astype(np.float64))
+        o.step_heun(1)
+        s1 = o.get_spins()
+        o.step_heun(1)
+        _FULL[key] = (s1, o.get_spins())
+    return _FULL[key]
 
 
 @pytest.mark.parametrize("lattice", [ai.SC, ai.L10])
@@ -209,19 +221,37 @@ def test_fused_kernel_matches_two_kernel_step_closely():
     assert float(np.abs(sa - sb).max()) <= 2e-6
 
 
-@pytest.mark.parametrize("cfg", [2, 4])
-@pytest.mark.parametrize("kernel", ["fast", "tma", "fused"])
+@pytest.mark.parametrize("cfg", [2, 3, 4])
+@pytest.mark.parametrize("kernel", ["fast", "tma", "fused", "auto"])
 def test_full_size_one_step(cfg, kernel):
-    """BASELINE configs at full size in the launch configuration bench.py times: every site against the oracle."""
-    w = ai.make_config(cfg)
-    sx, sy, sz = ai.tilted_spins(w.n_sites, 20.0, seed=4)
-    mag = w.magnetic_mask().reshape(-1)
-    w.sx, w.sy, w.sz = sx * mag, sy * mag, sz * mag
+    """BASELINE configs at full size in the launch configuration bench.py times: every site against the oracle, at
+    north_star's tolerance (1e-5 after ONE step), then a second step.  cfg3 = SC 400x200x27, cfg2 / cfg4 = L1_0."""
     import paper_2502_02236_b200 as asd
-    o, g = _full_size_oracle(cfg, w), gpu_from_workload(w)
-    g.set_kernel({"fast": asd.KERNEL_FAST, "tma": asd.KERNEL_TMA, "fused": asd.KERNEL_FUSED}[kernel])
-    g.step_heun(2)
-    assert float(np.abs(g.get_spins_host().astype(np.float64) - o).max()) <= 2e-5
+    w = _full_size_workload(cfg)
+    (o1, o2), g = _full_size_oracle(cfg, w), gpu_from_workload(w)
+    if kernel != "auto":
+        g.set_kernel({"fast": asd.KERNEL_FAST, "tma": asd.KERNEL_TMA, "fused": asd.KERNEL_FUSED}[kernel])
+    g.step_heun(1)
+    assert float(np.abs(g.get_spins_host().astype(np.float64) - o1).max()) <= TOL_1STEP
+    g.step_heun(1)
+    assert float(np.abs(g.get_spins_host().astype(np.float64) - o2).max()) <= 2e-5
+    _check_norm(g, w)
+
+
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_full_size_one_step_ell(cfg):
+    """The same windows handed over as a general ELL table with per-pair J (asd_inputs.shell_ell_table: W = 6 for SC,
+    W = 10 for L1_0) -- the configuration `bench.py --ell` times; every site against the oracle's ELL branch."""
+    w = _full_size_workload(cfg)
+    idx, J = ai.shell_ell_table(w)
+    (o1, o2) = _full_size_oracle(cfg, w, ell=(idx, J))
+    g = gpu_from_workload(w, ell_idx=idx, ell_J=J)
+    g.step_heun(1)
+    assert float(np.abs(g.get_spins_host().astype(np.float64) - o1).max()) <= TOL_1STEP
+    g.step_heun(1)
+    assert float(np.abs(g.get_spins_host().astype(np.float64) - o2).max()) <= 2e-5
+    # and the table says what the built-in shells say (the oracle's two branches, fp32-rounded J apart)
+    assert float(np.abs(o2 - _full_size_oracle(cfg, w)[1]).max()) <= 1e-6
     _check_norm(g, w)
 
 

@@ -73,6 +73,52 @@ def test_seeded_slab_matches_oracle_and_reproduces_m():
     assert np.all(tail[0] == 0) and np.all(tail[1] == 0)
 
 
+def test_full_size_cfg4_shift():
+    """asd_shift_window at BASELINE cfg4's size (881 x 220 x 27 L1_0, 220 x 27-site planes, macrocells (7, 7, 5)) with the
+    schedule's plane counts (p = 3 then 4) and a non-trivial track state: moved block, macrocell sums and counts bit
+    exact on integer-valued spins; seeded slabs against the oracle on real spins."""
+    w = _integer_valued(ai.make_config(4))
+    nx, ny, nz = w.nx, w.ny, w.nz
+    o, g = oracle_from_workload(w), gpu_from_workload(w)
+    for p in (3, 4):
+        before = g.get_spins_host()
+        assert o.shift_window(p) == 0
+        g.shift_window(p)
+        so, sg = o.get_spins(), g.get_spins_host()
+        nkeep = (nx - p) * ny * nz
+        assert np.array_equal(sg[:, :nkeep], before[:, p * ny * nz:])
+        assert np.array_equal(sg[:, :nkeep].astype(np.float64), so[:, :nkeep])
+        _, cnt_o, sum_o = o.track_get()
+        sum_g, cnt_g = g.track_get()
+        assert np.array_equal(cnt_o, cnt_g) and np.array_equal(sum_o, sum_g)
+        assert int(cnt_g.sum()) > 0
+    assert g.counters()["x0"] == o.counters()["x0"] == 7
+    # seeding: track state with random directions and magnitudes, real spins
+    w = ai.make_config(4)
+    sx, sy, sz = ai.tilted_spins(w.n_sites, 20.0, seed=4)
+    mag = w.magnetic_mask().reshape(-1)
+    w.sx, w.sy, w.sz = sx * mag, sy * mag, sz * mag
+    o, g = oracle_from_workload(w), gpu_from_workload(w)
+    ncx, ncy, ncz = g.track_dims()
+    rng = np.random.default_rng(8)
+    v = rng.standard_normal((ncx * ncy * ncz, 3))
+    v /= np.linalg.norm(v, axis=1, keepdims=True)
+    v *= rng.uniform(0.0, 1.0, size=(v.shape[0], 1))
+    v = v.astype(np.float32)
+    o.track_set_init(v); g.track_set_init(v)
+    for p in (3, 4):
+        assert o.shift_window(p) == 0
+        g.shift_window(p)
+        so, sg = o.get_spins(), g.get_spins_host().astype(np.float64)
+        assert np.abs(so - sg).max() < 3e-6
+        slab = sg[:, (nx - p) * ny * nz:]
+        n = np.sqrt((slab ** 2).sum(axis=0))
+        assert np.all((np.abs(n - 1.0) < 2e-6) | (n == 0.0))       # seeded spins are unit vectors, vacant sites 0
+    # one Heun step after the shifts: the window origin, the grain map and the Philox site ids moved along
+    o.step_heun(1); g.step_heun(1)
+    assert np.abs(o.get_spins() - g.get_spins_host()).max() <= 1e-5
+
+
 def test_heun_after_shift_uses_new_origin():
     """Noise follows the atom (global site id) and the grain map follows the window after a shift."""
     w = ai.small_film(ai.L10, 20, 24, 5, extra_track=12, tilt_deg=20.0, dt=1e-16)
