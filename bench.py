@@ -3,8 +3,8 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4] [--heun-per-step 50]
 
-A "step" is one pass of the whole hot path over one batch: `heun_per_step` stochastic Heun steps (2 fused kernels
-each) of the synthetic HAMR window, the head-field scale of the drive schedule, and asd_shift_window whenever the
+A "step" is one pass of the whole hot path over one batch: `heun_per_step` stochastic Heun steps (one fused kernel
+each on HBM-streaming films, a predictor and a corrector kernel otherwise) of the synthetic HAMR window, the head-field scale of the drive schedule, and asd_shift_window whenever the
 Heun-step counter crosses the shift cadence (every 5000 Heun steps, Q8).  Default workload: BASELINE
 configs[4], the 881x220x27 L1_0 window (5.23 M sites) -- the configuration the metric's roofline target is quoted on.
 
@@ -42,22 +42,6 @@ def _peaks():
     if os.path.exists(p):
         return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     return 6650.0, "fallback (B200_PROFILING.md)"
-
-
-def _traffic(workload: str):
-    """dram bytes per launch of the stage kernel from the committed ncu capture (profiles/traffic.csv), or None."""
-    p = os.path.join(ROOT, "profiles", "traffic.csv")
-    if not os.path.exists(p):
-        return None
-    vals = []
-    for line in open(p):
-        f = [x.strip() for x in line.split(",")]
-        if len(f) >= 3 and f[0] == workload and f[1].startswith("heun_stage"):
-            try:
-                vals.append(float(f[2]))
-            except ValueError:
-                pass
-    return float(np.mean(vals)) if vals else None
 
 
 class ClockSampler:
@@ -136,10 +120,12 @@ def _gpu_desc(asd, w: ai.Workload, ell=None):
     return asd.desc_from_workload(w, **extra)
 
 
-def _drive(w: ai.Workload, heun_per_step: int):
-    """Per bench step: (field scale, planes to shift after the step or 0).  DESIGN.md Q8 schedule."""
+def _drive(w: ai.Workload, heun_per_step: int, start_heun: int = 0):
+    """Per bench step: (field scale, planes to shift after the step or 0).  DESIGN.md Q8 schedule.  start_heun: where
+    on the schedule's step-index clock the run begins (bench.py starts shortly before a shift so that the window shift
+    falls inside the timed region whatever --steps is)."""
     bits = ai.nrz_bits(64, w.bit_seed)
-    state = {"heun": 0, "q": 0}
+    state = {"heun": start_heun, "q": (start_heun // w.shift_every) if w.shift_every else 0}
 
     def next_step():
         s = ai.field_scale_at(state["heun"], bits, w.bit_steps) if w.bit_steps else 1.0
@@ -152,7 +138,155 @@ def _drive(w: ai.Workload, heun_per_step: int):
     return next_step
 
 
-# ------------------------------------------------------------------------------------------------------------
+def _start_heun(w: ai.Workload, hps: int, warmup: int, steps: int) -> int:
+    """Schedule position at which the first warm-up step starts so that a shift closes the middle timed step."""
+    if not w.shift_every:
+        return 0
+    per = max(1, w.shift_every // hps)                      # bench steps per shift period
+    return (per - (warmup + max(1, (steps + 1) // 2)) % per) % per * hps
+
+
+# Algorithmic HBM bytes (DESIGN.md sec. 6).  Survey floors (SURVEY 8(d)): two-kernel step, k1 recomputed / structured.
+SURVEY_FLOOR_BYTES = {ai.SC: 92.0, ai.L10: 96.0}
+FUSED_BYTES_PER_SITE_STEP = 40.0
+# Plain-ALU roof (DESIGN.md sec. 6): one warp instruction per scheduler per clock.
+SM_COUNT, SCHEDULERS_PER_SM, LANES = 148, 4, 32
+# Arithmetic a fused Heun step needs per site, thread instructions (DESIGN.md sec. 6 derivation) by lattice
+ALG_INST_PER_SITE_STEP = {ai.SC: 196.0, ai.L10: 222.0}
+
+
+def _sm_max_hz():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return float(json.load(open(p)).get("sm_max_mhz", 1965.0)) * 1e6
+    return 1965e6
+
+
+def _captured(workload: str, kernel_prefix: str):
+    """(dram bytes per launch, executed warp instructions per launch) of a kernel from the committed ncu capture
+    (profiles/traffic.csv), or (None, None)."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(p):
+        return None, None
+    tr, wi = [], []
+    for line in open(p):
+        f = [x.strip() for x in line.split(",")]
+        if len(f) >= 3 and f[0] == workload and f[1].startswith(kernel_prefix):
+            try:
+                tr.append(float(f[2]))
+                if len(f) >= 4 and f[3]:
+                    wi.append(float(f[3]))
+            except ValueError:
+                pass
+    return (float(np.mean(tr)) if tr else None), (float(np.mean(wi)) if wi else None)
+
+
+class Run:
+    """One context on one workload: warm-up, device-timed bench steps (Heun batches + the schedule's shifts)."""
+
+    def __init__(self, asd, torch, w, device, hps, kernel="auto", ell=False, demag=False, demag_every=0):
+        self.asd, self.torch, self.w, self.hps = asd, torch, w, hps
+        self.N = w.n_sites
+        table = None
+        if ell:
+            # the same exchange bonds handed over as a general ELL table (per-pair J); such a table cannot follow the
+            # window, so this variant runs without shifts
+            table = ai.shell_ell_table(w)
+            w.shift_every = 0
+        self.ell_w = 0 if table is None else int(table[0].shape[1])
+        self.ctx = asd.Context(_gpu_desc(asd, w, table), device=device)
+        if demag:
+            self.ctx.enable_demag([a * 1e-9 for a in w.spacing_nm])
+            self.ctx.set_demag_every(demag_every)
+        if kernel != "auto":
+            self.ctx.set_kernel({"general": asd.KERNEL_GENERAL, "fast": asd.KERNEL_FAST, "tma": asd.KERNEL_TMA,
+                                 "fused": asd.KERNEL_FUSED}[kernel])
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory()
+        self.hT, self.hBx, self.hBy, self.hBz = pin(w.T), pin(w.Bx), pin(w.By), pin(w.Bz)
+        self.ctx.set_spins_host(pin(w.sx), pin(w.sy), pin(w.sz))
+        self.ctx.set_fields_host(self.hT, self.hBx, self.hBy, self.hBz)
+        torch.cuda.synchronize()
+        self.nxt = None
+
+    def start(self, warmup, steps):
+        self.nxt = _drive(self.w, self.hps, _start_heun(self.w, self.hps, warmup, steps))
+        for _ in range(warmup):
+            self.one_step()
+
+    def one_step(self, timed=None):
+        torch, ctx = self.torch, self.ctx
+        s, p = self.nxt()
+        ctx.set_field_scale(s)
+        if timed is not None:
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            lc = ctx.launch_count()
+            e0.record(); ctx.step_heun(self.hps); e1.record()
+            timed.append((e0, e1, ctx.launch_count() - lc))
+        else:
+            ctx.step_heun(self.hps)
+        if p:
+            ctx.shift_window(p)
+        return p
+
+    def timed(self, steps, barrier=None):
+        """-> dict(ms, shifts, launches, heun_ms, heun_launches): CUDA events around the whole region and each batch."""
+        torch = self.torch
+        sync = barrier or torch.cuda.synchronize
+        ev, shifts = [], 0
+        l0 = self.ctx.launch_count()
+        t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        sync()
+        t0.record()
+        for _ in range(steps):
+            shifts += 1 if self.one_step(ev) else 0
+        t1.record()
+        sync()
+        return {"ms": t0.elapsed_time(t1), "shifts": shifts, "launches": self.ctx.launch_count() - l0,
+                "heun_ms": sum(a.elapsed_time(b) for a, b, _ in ev), "heun_launches": sum(n for _, _, n in ev),
+                "steps": steps}
+
+    def roofline(self, t, peak, peak_src):
+        """The dominant kernel's roofline record from a timed() result."""
+        hps, N, w = self.hps, self.N, self.w
+        heun_steps = hps * t["steps"]
+        per_step = t["heun_launches"] / max(1, heun_steps)            # kernels per Heun step: 1 fused, 2 stage kernels
+        fused = per_step < 1.5 and self.ell_w == 0
+        avg_launch_s = t["heun_ms"] * 1e-3 / max(1, t["heun_launches"])
+        if fused:
+            name, alg = "heun_fused (one kernel per Heun step, 40 B/site)", FUSED_BYTES_PER_SITE_STEP * N
+            cap = "heun_fused"
+        elif self.ell_w:
+            name = "heun_stage_ell (predictor + corrector, %d B/site each)" % (52 + 8 * self.ell_w)
+            alg, cap = (BYTES_PER_SITE_PER_STAGE + 8.0 * self.ell_w) * N, "heun_stage_ell"
+        else:
+            name, alg = "stage kernels (predictor + corrector, 52 B/site each)", BYTES_PER_SITE_PER_STAGE * N
+            cap = "heun_stage_fast"
+        achieved = alg / avg_launch_s / 1e9
+        step_s = t["heun_ms"] * 1e-3 / max(1, heun_steps)
+        traffic, warp_inst = _captured(w.name, cap)
+        r = {"bound": "hbm", "kernel": name, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+             "peak_source": peak_src, "avg_launch_us": avg_launch_s * 1e6, "algorithmic_bytes_per_launch": alg,
+             "traffic": traffic,
+             # the same Heun steps accounted at SURVEY 8(d)'s two-kernel floor (92 B SC / 96 B L1_0 per site-step):
+             # comparable across kernel designs and rounds
+             "frac_survey_floor": SURVEY_FLOOR_BYTES[w.lattice] * N / step_s / 1e9 / peak if not self.ell_w else None,
+             # DRAM bytes the committed ncu capture counted for this kernel / this run's launch time
+             "frac_dram": (traffic / avg_launch_s / 1e9 / peak) if traffic else None}
+        if fused:
+            issue_peak = SM_COUNT * SCHEDULERS_PER_SM * LANES * _sm_max_hz()
+            alg_inst = ALG_INST_PER_SITE_STEP[w.lattice] * N
+            r["alu"] = {"bound": "alu", "unit": "thread-instructions/s", "peak": issue_peak,
+                        "peak_source": "148 SMs x 4 schedulers x 32 lanes x sm_max clock (one warp instruction per scheduler per clock)",
+                        "achieved": alg_inst / avg_launch_s, "frac": alg_inst / avg_launch_s / issue_peak,
+                        "algorithmic_thread_inst_per_site_step": ALG_INST_PER_SITE_STEP[w.lattice],
+                        "frac_executed": (warp_inst * LANES / avg_launch_s / issue_peak) if warp_inst else None}
+            r["note"] = ("the fused step moves 2.6x fewer bytes than the two-kernel step and is no longer HBM-bound: it is held "
+                         "by instruction issue / latency at 16 warps per SM (shared memory and registers are both full); "
+                         "frac = its own 40 B/site-step against the HBM peak, frac_survey_floor = the same steps at the "
+                         "two-kernel floor, alu.frac = arithmetic needed / issue peak")
+        return r
+
+
 def run_ours(args):
     import torch
     import paper_2502_02236_b200 as asd
@@ -173,69 +307,25 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    device = f"cuda:{local}"
     w = _workload(args.config, seed_offset=rank)
     N = w.n_sites
-    ell = None
-    if args.ell:
-        # the same exchange bonds handed over as a general ELL table (per-pair J); such a table cannot follow the
-        # window, so this variant runs without shifts
-        ell = ai.shell_ell_table(w)
-        w.shift_every = 0
-    ell_w = 0 if ell is None else int(ell[0].shape[1])
-    ctx = asd.Context(_gpu_desc(asd, w, ell), device=f"cuda:{local}")
-    dev = ctx.device
-    if args.demag:
-        ctx.enable_demag([a * 1e-9 for a in w.spacing_nm])
-        ctx.set_demag_every(args.demag_every)
-    if args.kernel != "auto":
-        ctx.set_kernel({"general": asd.KERNEL_GENERAL, "fast": asd.KERNEL_FAST, "tma": asd.KERNEL_TMA,
-                        "fused": asd.KERNEL_FUSED}[args.kernel])
-    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory()
-    hT, hBx, hBy, hBz = pin(w.T), pin(w.Bx), pin(w.By), pin(w.Bz)
-    ctx.set_spins_host(pin(w.sx), pin(w.sy), pin(w.sz))
-    ctx.set_fields_host(hT, hBx, hBy, hBz)
-    torch.cuda.synchronize()
     hps = args.heun_per_step
-    nxt = _drive(w, hps)
-
-    def one_step(timed_heun=None):
-        s, p = nxt()
-        ctx.set_field_scale(s)
-        if timed_heun is not None:
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            lc = ctx.launch_count()
-            e0.record(); ctx.step_heun(hps); e1.record()
-            timed_heun.append((e0, e1, ctx.launch_count() - lc))
-        else:
-            ctx.step_heun(hps)
-        if p:
-            ctx.shift_window(p)
-        return p
-
-    for _ in range(args.warmup):
-        one_step()
+    run = Run(asd, torch, w, device, hps, kernel=args.kernel, ell=args.ell, demag=args.demag, demag_every=args.demag_every)
+    ctx, dev = run.ctx, run.ctx.device
+    run.start(args.warmup, args.steps)
     barrier()
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-    l0 = ctx.launch_count()
-    heun_events, shifts = [], 0
-    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    t0.record()
-    for _ in range(args.steps):
-        shifts += 1 if one_step(heun_events) else 0
-    t1.record()
-    barrier()
-    ms = t0.elapsed_time(t1)
+    t = run.timed(args.steps, barrier)
     clocks = sampler.stop() if rank == 0 else None
-    launches = ctx.launch_count() - l0
-    heun_ms = sum(a.elapsed_time(b) for a, b, _ in heun_events)
-    ms, updates = reduce_over_ranks(ms, float(args.steps) * hps * N, dist, dev)
+    ms, updates = reduce_over_ranks(t["ms"], float(args.steps) * hps * N, dist, dev)
     value = updates / (ms * 1e-3)
 
     # ---- e2e: the same steps through the C ABI with HOST buffers: H2D of the step's inputs, D2H of its result ----
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    nxt = run.nxt
     barrier()
     w0 = time.perf_counter()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -243,7 +333,7 @@ def run_ours(args):
     msum = 0.0
     # double-buffered upload (asd_stage_fields_host / asd_commit_fields): the H2D copy of step n+1's fields runs on the
     # library's copy stream while step n's kernels run; every step still uploads its own 16 B/site and reads its result
-    ctx.stage_fields_host(hT, hBx, hBy, hBz)
+    ctx.stage_fields_host(run.hT, run.hBx, run.hBy, run.hBz)
     for it in range(e2e_steps):
         s, p = nxt()
         ctx.commit_fields()                              # wait for the staged copy, repack: fields of this step
@@ -252,7 +342,7 @@ def run_ours(args):
         if p:
             ctx.shift_window(p)
         if it + 1 < e2e_steps:
-            ctx.stage_fields_host(hT, hBx, hBy, hBz)     # pinned host -> device, 16 B/site, for the next step
+            ctx.stage_fields_host(run.hT, run.hBx, run.hBy, run.hBz)     # pinned host -> device, 16 B/site, for the next step
         m, _n = ctx.magnetisation()                      # device -> host, synchronises
         msum += float(m[2])
     e1.record()
@@ -267,34 +357,94 @@ def run_ours(args):
             dist.destroy_process_group()
         return
     peak, peak_src = _peaks()
-    n_stage_launches = sum(n for _, _, n in heun_events)
-    fused = n_stage_launches == hps * len(heun_events)       # one kernel per Heun step
-    avg_launch_s = heun_ms * 1e-3 / n_stage_launches
-    # a general ELL table adds its own compulsory bytes: int32 index + fp32 J per slot per site per stage
-    alg_bytes = (40.0 if fused else BYTES_PER_SITE_PER_STAGE + 8.0 * ell_w) * N
-    achieved = alg_bytes / avg_launch_s / 1e9
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": w.name, "sites": N, "heun_steps_per_step": hps, "shifts_in_timed_region": shifts,
-                   "shift_every_heun_steps": w.shift_every, "dt": w.dt, "parallelism": f"replicas x{world}", "ell_width": ell_w, "demag": bool(args.demag), "demag_every": args.demag_every if args.demag else None,
+        "config": {"workload": w.name, "sites": N, "heun_steps_per_step": hps, "shifts_in_timed_region": t["shifts"],
+                   "shift_every_heun_steps": w.shift_every, "dt": w.dt, "parallelism": f"replicas x{world}",
+                   "ell_width": run.ell_w, "demag": bool(args.demag), "demag_every": args.demag_every if args.demag else None,
+                   "kernel": args.kernel,
                    "l2": "working set (13 fp32 arrays/site = %.0f MB) exceeds the 126 MB L2" % (13 * 4 * N / 1e6)},
-        "clocks": clocks, "gpu_launches": int(launches),
+        "clocks": clocks, "gpu_launches": int(t["launches"]),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 16 * N, "d2h_bytes_per_step": 32,
-                "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps, "wall_ms_per_step": wall_ms / e2e_steps},
-        "roofline": {"bound": "hbm", "kernel": ("heun_stage_general<ELL> (predictor+corrector, %d B/site each)" % (52 + 8 * ell_w)) if ell_w else
-                     ("heun_fused (one kernel per Heun step, 40 B/site)" if fused else
-                      "heun_stage_fast (predictor+corrector, 52 B/site each)"),
-                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "peak_source": peak_src, "avg_launch_us": avg_launch_s * 1e6,
-                     "algorithmic_bytes_per_launch": alg_bytes, "traffic": _traffic(w.name)},
+                "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps, "wall_ms_per_step": wall_ms / e2e_steps,
+                "note": "per step: 16 B/site of fields up (pinned host, double-buffered), the window magnetisation (32 B) "
+                        "down; the spin state stays resident on the device and is not copied back"},
+        "roofline": run.roofline(t, peak, peak_src),
     }
+    if world == 1 and not args.no_sustained:
+        out["sustained"] = sustained(run, args.sustained_seconds, ms / args.steps, local, peak, peak_src)
+    if world == 1 and not args.no_secondary:
+        del run, ctx
+        torch.cuda.empty_cache()
+        out["secondary"] = secondary(asd, torch, device, args, peak, peak_src)
     if world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(args.config, budget_s=args.cpu_budget)
     print(json.dumps(out), flush=True)
     if dist is not None:
         dist.destroy_process_group()
+
+
+def sustained(run, seconds, ms_per_step, gpu_index, peak, peak_src):
+    """>= `seconds` of back-to-back bench steps (the regime BASELINE cfg4's 1e5 steps live in: the board reaches its power
+    cap), with its own clock record."""
+    steps = int(max(10, np.ceil(seconds * 1e3 / max(ms_per_step, 1e-3))))
+    sampler = ClockSampler(gpu_index)
+    sampler.start()
+    t = run.timed(steps)
+    clocks = sampler.stop()
+    r = run.roofline(t, peak, peak_src)
+    return {"value": float(steps) * run.hps * run.N / (t["ms"] * 1e-3), "unit": UNIT, "steps": steps,
+            "seconds": t["ms"] * 1e-3, "ms_per_step": t["ms"] / steps, "shifts_in_timed_region": t["shifts"],
+            "clocks": clocks, "avg_launch_us": r["avg_launch_us"], "frac": r["frac"],
+            "frac_survey_floor": r["frac_survey_floor"]}
+
+
+def secondary(asd, torch, device, args, peak, peak_src):
+    """Short runs of the other kernels / configs, each with its own roofline fraction (same timing rules, 6 timed steps of
+    20 Heun steps after 3 warm-up steps; working sets > L2 except where noted)."""
+    out = []
+    w4 = None
+
+    def one(label, cfg, **kw):
+        nonlocal w4
+        hps, steps, warm = kw.pop("hps", 20), kw.pop("steps", 6), 3
+        try:
+            if cfg == 4:
+                w4 = w4 or _workload(4)
+                import copy
+                w = copy.copy(w4)
+            else:
+                w = _workload(cfg)
+            run = Run(asd, torch, w, device, hps, **kw)
+            run.start(warm, steps)
+            t = run.timed(steps)
+            r = run.roofline(t, peak, peak_src)
+            heun_steps = hps * steps
+            rec = {"label": label, "workload": w.name, "sites": w.n_sites, "value": heun_steps * w.n_sites / (t["ms"] * 1e-3),
+                   "unit": UNIT, "us_per_heun_step": t["heun_ms"] * 1e3 / heun_steps, "kernel": r["kernel"],
+                   "avg_launch_us": r["avg_launch_us"], "frac": r["frac"], "frac_survey_floor": r["frac_survey_floor"],
+                   "shifts_in_timed_region": t["shifts"]}
+            if kw.get("demag"):
+                # the launches of a step include the demagnetising-field pipeline: no single-kernel fraction to quote
+                rec.update(kernel="stage kernels + demagnetising-field pipeline", avg_launch_us=None, frac=None)
+            elif w.n_sites < (1 << 18):
+                rec.update(frac=None, frac_survey_floor=None, note="launch-bound: no roofline fraction")
+            elif 13 * 4 * w.n_sites < 126e6:
+                rec["note"] = "working set fits the 126 MB L2: frac is not an HBM fraction"
+            out.append(rec)
+            del run
+            torch.cuda.empty_cache()
+        except Exception as e:                      # a secondary line must never cost the main one
+            out.append({"label": label, "error": str(e)[:200]})
+
+    one("cfg4, two-kernel film kernel (asd_set_kernel FAST)", 4, kernel="fast")
+    one("cfg4 as a general ELL table, W = 10, per-pair J (no shifts)", 4, ell=True)
+    one("cfg4 with the demagnetising field recomputed in every stage", 4, demag=True, demag_every=0)
+    one("cfg3 SC 400x200x27", 3)
+    one("cfg0 SC 16^3 periodic (launch-bound: us per Heun step is the figure)", 0, hps=1000, steps=3)
+    return out
 
 
 # ------------------------------------------------------------------------------------------------------------
@@ -315,15 +465,26 @@ def _crop(w: ai.Workload, nx: int) -> ai.Workload:
 
 
 def cpu_baseline(cfg: int, budget_s: float = 15.0):
-    """The oracle as it stands, on this host's cores, on a bounded sample: full lattice, as many Heun steps as fit."""
+    """The oracle as it stands, on this host's cores, on a bounded sample: the full lattice, as many Heun steps as fit
+    in the budget with all threads; then the same lattice on ONE thread for a third of the budget."""
     from oracle import asd_oracle as orc
     w = _workload(cfg)
     o = _oracle_for(w)
     t = time.perf_counter(); o.step_heun(1); t1 = time.perf_counter() - t
     n = int(max(1, min(200, budget_s / max(t1, 1e-3))))
     t = time.perf_counter(); o.step_heun(n); dt = time.perf_counter() - t
-    return {"value": n * w.n_sites / dt, "unit": UNIT, "cores": orc.max_threads(), "kind": "oracle",
-            "sample": f"{n} Heun steps of the full {w.name} lattice ({w.n_sites} sites), fp64, OpenMP"}
+    out = {"value": n * w.n_sites / dt, "unit": UNIT, "cores": orc.max_threads(), "kind": "oracle",
+           "sample": f"{n} Heun steps of the full {w.name} lattice ({w.n_sites} sites), fp64, OpenMP"}
+    # one thread: a crop of the first planes sized to ~budget/3 at the all-thread per-site rate x cores
+    per_site_1 = dt / (n * w.n_sites) * orc.max_threads()
+    nx1 = int(max(4, min(w.nx, (budget_s / 3.0) / (per_site_1 * w.ny * w.nz))))
+    w1 = _crop(w, nx1)
+    o1 = _oracle_for(w1)
+    o1.set_threads(1)
+    t = time.perf_counter(); o1.step_heun(1); d1 = time.perf_counter() - t
+    out["single_thread"] = {"value": w1.n_sites / d1, "unit": UNIT, "cores": 1,
+                            "sample": f"1 Heun step of the first {nx1} of {w.nx} planes ({w1.n_sites} sites), one thread"}
+    return out
 
 
 def run_reference(args):
@@ -371,6 +532,9 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=20)
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-sustained", action="store_true", help="skip the >= 2 s back-to-back sub-record")
+    ap.add_argument("--sustained-seconds", type=float, default=2.0)
+    ap.add_argument("--no-secondary", action="store_true", help="skip the short runs of the other kernels / configs")
     ap.add_argument("--ell", action="store_true",
                     help="hand the exchange bonds over as a general ELL neighbour table with per-pair J (no window shifts)")
     ap.add_argument("--demag", action="store_true",
