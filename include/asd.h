@@ -160,7 +160,10 @@ ASD_API asd_status asd_set_graph_mode(asd_ctx *ctx, int32_t mode);
  * N = demagnetising tensor of two equal cuboids (Newell et al., the paper's ref. [28]), summed over the macrocells that
  * overlap the window (open boundaries).  Open-boundary lattices with the built-in shells; ASD_KERNEL_TMA and CUDA graphs
  * are not used while it is on.  The caller owns the workspace (DEVICE, 256-byte aligned) for the life of the context.
- * asd_demag_workspace_bytes needs the GPU (it sizes the cuFFT plans).  asd_demag_field computes the field of the current
+ * The convolution is the library's own (direct sum over the film's macrocell layers, DFT across the film, shared-memory
+ * FFT along the track; no FFT library): ASD_EUNSUPPORTED if 3 * (layers of macrocells) fields of the padded track length
+ * do not fit in one CTA's shared memory (about 300 macrocell layers x cells along x / 256).
+ * asd_demag_workspace_bytes is pure host arithmetic.  asd_demag_field computes the field of the current
  * spins per macrocell into HOST cells[dims[0]*dims[1]*dims[2]*3] (x-cell slowest, component fastest; Tesla) and
  * synchronises; cells == NULL returns dims only.  ASD_ESTATE if demag is not enabled. */
 ASD_API size_t asd_demag_workspace_bytes(asd_ctx *ctx);

@@ -18,7 +18,7 @@ NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--shared", "-cudart", "static",
-         "-split-compile", "0", "-lcufft", "-Xlinker", "-rpath=/usr/local/cuda/lib64"]
+         "-split-compile", "0"]
 
 
 def sources():

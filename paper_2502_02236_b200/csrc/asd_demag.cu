@@ -7,14 +7,29 @@
 // track macrocells that overlap the window (open boundaries; the frozen track's stray field is not included -- callers
 // add it through the per-site B arrays).  Each site then sees the field of its macrocell.
 //
-// Per stage, in stream order:  coarse_grain_cells (coalesced row sweeps, fixed summation order, deterministic)
-//   -> cuFFT R2C of the 3 zero-padded components -> multiply_tensor (6 real-even kernels, transformed once at set-up)
-//   -> cuFFT C2R -> the stage kernel adds demag_B[cell(site)] to its exchange field.
-// The FFT is the one library primitive on this path (like cuBLAS for a plain GEMM); everything around it is ours.
-// The tensor itself is computed on the host in fp64 at enable time.
-#include <cufft.h>
-
+// The convolution is ours from end to end (no FFT library).  A film is a few macrocells thick, a few tens wide and a few
+// hundred long, so the three axes are treated differently:
+//   z (thickness, dcz cells):   summed DIRECTLY -- every pair of layers (c, c') has its own 2-D kernel K_ab(., ., c - c');
+//   y (width, dcy cells):       a plain DFT of length PY = 2^n >= 2 dcy - 1 (dcy real inputs -> PY/2 + 1 complex outputs:
+//                               a 32 x 33 matrix-vector product per row -- cheaper than an FFT's passes at this size);
+//   x (length, dcx cells):      a shared-memory radix-2 FFT of length PX = 2^n >= 2 dcx - 1.
+// Per evaluation, in stream order (3 launches):
+//   coarse_grain_ydft   Eq. (6) (coalesced row sweeps, fixed summation order, deterministic) and, in the same CTA, the
+//                       y-DFT of the row of cells it has just formed                  -> Y[ky][field][x-cell]
+//   demag_xconv         one CTA per (ky, output component): forward FFT along x of the 3 dcz input fields (decimation
+//                       in frequency, in place, output left in bit-reversed order), B^_a(c) = sum_b sum_c' K^_ab(c - c')
+//                       M^_b(c') with the transformed tensor stored in the SAME bit-reversed order (so no reordering
+//                       pass exists anywhere), inverse FFT (decimation in time: bit-reversed in, natural out)
+//                                                                                     -> Z[ky][field][x-cell]
+//   demag_yinv          inverse y-DFT (complex half-spectrum -> dcy real values)      -> B[comp][x-cell][y-cell][z-cell]
+// and the stage kernel adds B[cell(site)] to its exchange field.
+// The tensor is computed on the host in fp64 at enable time (Newell's closed form, point dipoles in the far field --
+// DESIGN.md reading D2) and transformed there with a small fp64 FFT.  N_xx, N_yy, N_zz, N_xy are even or odd in BOTH x
+// and y, so their (x, y) transforms are real; N_xz and N_yz are odd in exactly one of them: purely imaginary.  One float
+// per entry is stored either way.
+#include <algorithm>
 #include <cmath>
+#include <complex>
 #include <vector>
 
 #include "asd_internal.cuh"
@@ -23,15 +38,18 @@ namespace asd {
 
 struct DemagPlan {
   int dcx = 0, dcy = 0, dcz = 0;      // macrocells that can overlap the window (x: worst alignment of x0)
-  int px = 0, py = 0, pz = 0, pzc = 0; // padded transform size, and pz/2 + 1
+  int PX = 0, PY = 0, logPX = 0;      // transform lengths (powers of two), log2 PX
+  int NKY = 0, F = 0, NDZ = 0;        // PY/2 + 1 retained y-frequencies, 3 dcz fields, 2 dcz - 1 layer offsets
   double cell[3] = {0, 0, 0};
   float mu_over_V = 0.0f;
-  float* M = nullptr;                 // [3][px][py][pz]
-  cufftComplex* Mh = nullptr;         // [3][px][py][pzc]
-  cufftComplex* Kh = nullptr;         // [6][px][py][pzc], includes -mu_0 / (px py pz)
-  float* B = nullptr;                 // [3][px][py][pz]
-  cufftHandle fwd = 0, inv = 0;
-  bool plans = false;
+  float2* Y = nullptr;                // [NKY][F][dcx]      y-transformed cell magnetisation
+  float2* Z = nullptr;                // [NKY][F][dcx]      y-transformed cell field
+  float* Kh = nullptr;                // [6][NDZ][NKY][PX]  transformed tensor (x index bit-reversed), includes -mu_0/(PX PY)
+  float* B = nullptr;                 // [3][dcx][dcy][dcz] cell field, Tesla
+  float2* twx = nullptr;              // [PX/2] exp(-2 pi i n / PX)
+  float2* twy = nullptr;              // [PY]   exp(+2 pi i n / PY)
+  unsigned xconv_threads = 0;
+  size_t xconv_smem = 0;
 };
 
 namespace {
@@ -93,28 +111,79 @@ void cuboid_tensor(const double d[3], const double R[3], double N[6]) {
   }
 }
 
-int nice_size(int n) {                       // smallest m >= n with only the factors 2, 3, 5, 7
-  for (int m = n;; ++m) {
-    int q = m;
-    for (int f : {2, 3, 5, 7}) while (q % f == 0) q /= f;
-    if (q == 1) return m;
+
+int pow2_at_least(int n) { int p = 2; while (p < n) p <<= 1; return p; }
+
+// in-place iterative radix-2 FFT, fp64, forward (e^{-i...}); host, set-up only
+void host_fft(std::complex<double>* x, int n) {
+  for (int i = 1, j = 0; i < n; ++i) {
+    int bit = n >> 1;
+    for (; j & bit; bit >>= 1) j ^= bit;
+    j ^= bit;
+    if (i < j) std::swap(x[i], x[j]);
+  }
+  for (int len = 2; len <= n; len <<= 1) {
+    const double ang = -2.0 * kPi / len;
+    for (int i = 0; i < n; i += len)
+      for (int k = 0; k < len / 2; ++k) {
+        const std::complex<double> w(std::cos(ang * k), std::sin(ang * k));
+        const std::complex<double> u = x[i + k], v = x[i + k + len / 2] * w;
+        x[i + k] = u + v; x[i + k + len / 2] = u - v;
+      }
   }
 }
 
-// Eq. (6).  One CTA per (cell-x a, cell-z c) slab of macrocells.  Threads form a (row-lane, column-group) grid: thread
-// (rl, g) sums its VEC columns over every lanes-th of the slab's mx * mz rows (a row read is one coalesced sweep of ny
-// floats per component; the unrolled row loop keeps several rows in flight); the partial column sums meet in shared
-// memory, where thread b adds the row lanes and the my columns of macrocell (a, b, c) in a fixed order.  Deterministic.
+uint32_t bit_reverse(uint32_t v, int bits) {
+  uint32_t r = 0;
+  for (int b = 0; b < bits; ++b) r |= ((v >> b) & 1u) << (bits - 1 - b);
+  return r;
+}
+
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+__device__ __forceinline__ float2 cmul_conj(float2 a, float2 w) { return make_float2(a.x * w.x + a.y * w.y, a.y * w.x - a.x * w.y); }
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+
+// y-DFT of one row of dcy cell values per component (shared memory `cells` [3][dcy]) into Y[ky][comp dcz + c][a]:
+//   Y = sum_b M_comp(a, b, c) exp(-2 pi i ky b / PY),  ky = 0 .. PY/2.
+// Four threads share an output (every fourth b each, combined by shuffles in a fixed order); tws = exp(+i ...) table in
+// shared memory.  Called by all threads of the CTA (blockDim a multiple of 32).
+__device__ __forceinline__ void row_ydft(const float* cells, const float2* tws, int dcy, int dcz, int dcx, int PY, int NKY,
+                                         int a, int c, float2* __restrict__ Y) {
+  const int F = 3 * dcz, nout = 3 * NKY;
+  for (int o4 = threadIdx.x; o4 < ((4 * nout + 31) & ~31); o4 += blockDim.x) {
+    const int o = o4 >> 2, part = o4 & 3;
+    const int comp = o < nout ? o / NKY : 0, ky = o < nout ? o - comp * NKY : 0;
+    float re = 0.0f, im = 0.0f;
+    for (int b = part; b < dcy; b += 4) {
+      const float2 w = tws[(ky * b) & (PY - 1)];
+      const float m = cells[comp * dcy + b];
+      re = fmaf(m, w.x, re); im = fmaf(-m, w.y, im);
+    }
+    re += __shfl_xor_sync(0xFFFFFFFFu, re, 1); im += __shfl_xor_sync(0xFFFFFFFFu, im, 1);
+    re += __shfl_xor_sync(0xFFFFFFFFu, re, 2); im += __shfl_xor_sync(0xFFFFFFFFu, im, 2);
+    if (part == 0 && o < nout) Y[((size_t)ky * F + (size_t)(comp * dcz + c)) * dcx + a] = make_float2(re, im);
+  }
+}
+
+// Eq. (6) + the y-DFT.  One CTA per (cell-x a, cell-z c) slab of macrocells.  Threads form a (row-lane, column-group)
+// grid: thread (rl, g) sums its VEC columns over every lanes-th of the slab's mx * mz rows (a row read is one coalesced
+// sweep of ny floats per component; the unrolled row loop keeps several rows in flight); the partial column sums meet in
+// shared memory, where thread b adds the row lanes and the my columns of macrocell (a, b, c) in a fixed order.
+// Deterministic.  The dcy cell values of each component are then transformed along y (row_ydft).
 constexpr int kMaxRowLanes = 8;
 template <int VEC>
-__global__ void coarse_grain_cells(const float* __restrict__ X, uint32_t as, int nx, int ny, int nz, int nyp, int lead,
-                                   int mx, int my, int mz, long long x0, int dcy, int dcz, int py, int pz,
-                                   size_t comp_stride, float mu_over_V, int lanes, float* __restrict__ M) {
-  extern __shared__ float col[];                                 // [lanes][3][ny]
+__global__ void coarse_grain_ydft(const float* __restrict__ X, uint32_t as, int nx, int ny, int nz, int nyp, int lead,
+                                  int mx, int my, int mz, long long x0, int dcx, int dcy, int dcz, int PY, int NKY,
+                                  float mu_over_V, int lanes, const float2* __restrict__ twy, float2* __restrict__ Y) {
+  extern __shared__ __align__(16) float col[];                   // [lanes][3][ny] | cells [3][dcy] | tws [PY]
+  float* cells = col + (size_t)lanes * 3 * ny;
+  float2* tws = reinterpret_cast<float2*>(cells + ((3 * dcy + 1) & ~1));
   const int a = blockIdx.x / dcz, c = blockIdx.x - a * dcz;
   const int i0 = (int)((x0 / mx + a) * (long long)mx - x0);      // first window plane of the cell (may be < 0)
   const int rows = mx * mz, groups = ny / VEC;
   const int rl = threadIdx.x / groups, g = threadIdx.x - rl * groups;
+  for (int t = threadIdx.x; t < PY; t += blockDim.x) tws[t] = __ldg(twy + t);
   if (rl < lanes) {
     float s[3][VEC];
 #pragma unroll
@@ -149,66 +218,281 @@ __global__ void coarse_grain_cells(const float* __restrict__ X, uint32_t as, int
     for (int j = b * my; j < j1; ++j)
       for (int l = 0; l < lanes; ++l)
         for (int comp = 0; comp < 3; ++comp) t[comp] += col[((size_t)l * 3 + comp) * ny + j];
-    const size_t q = ((size_t)a * py + b) * pz + c;
-    M[q] = t[0] * mu_over_V; M[comp_stride + q] = t[1] * mu_over_V; M[2 * comp_stride + q] = t[2] * mu_over_V;
+    cells[b] = t[0] * mu_over_V; cells[dcy + b] = t[1] * mu_over_V; cells[2 * dcy + b] = t[2] * mu_over_V;
+  }
+  __syncthreads();
+  row_ydft(cells, tws, dcy, dcz, dcx, PY, NKY, a, c, Y);
+}
+
+// Which stored tensor component couples output component oc to input component b.  Storage order
+// (Nxx, Nyy, Nzz, Nxy, Nxz, Nyz); the (x, y) transforms of the last two are purely imaginary.
+__device__ __forceinline__ int tensor_comp(int oc, int b) {
+  return oc == b ? oc : (oc + b == 1 ? 3 : (oc + b == 2 ? 4 : 5));
+}
+
+// ---- shared-memory FFT along x ----
+// A field of PX complex points is stored with one pad element after every 8 (phys): the 8-point chunks that one thread
+// transforms in registers then start 72 bytes apart, which makes their 64-bit accesses bank-conflict-free, and the
+// wide-span stages (consecutive threads, consecutive points) lose next to nothing.
+__device__ __forceinline__ int phys(int n) { return n + (n >> 3); }
+
+// Decimation in frequency (forward, e^{-i}): stage of span h maps the pair (p, p + h), p mod 2h < h, to
+// (a + b, (a - b) w),  w = exp(-2 pi i (p mod h) / (2 h)) = tw[(p mod h) (PX / 2h)];  natural order in, bit-reversed out.
+// Decimation in time (inverse, e^{+i}): the same pairs, (a + b conj w, a - b conj w), spans ascending.
+__device__ __forceinline__ void dif_stage(float2* x, int f_count, int logPX, int sh, const float2* tw, int PXP) {
+  const int H = 1 << (logPX - 1), h = 1 << sh;
+  for (int t = threadIdx.x; t < f_count * H; t += blockDim.x) {
+    const int f = t >> (logPX - 1), u = t & (H - 1);
+    const int i = u & (h - 1), p = ((u >> sh) << (sh + 1)) + i;
+    float2* xf = x + f * PXP;
+    const float2 a = xf[phys(p)], b = xf[phys(p + h)];
+    xf[phys(p)] = cadd(a, b);
+    xf[phys(p + h)] = cmul(csub(a, b), tw[i << (logPX - 1 - sh)]);
+  }
+}
+__device__ __forceinline__ void dit_stage(float2* x, int f_count, int logPX, int sh, const float2* tw, int PXP) {
+  const int H = 1 << (logPX - 1), h = 1 << sh;
+  for (int t = threadIdx.x; t < f_count * H; t += blockDim.x) {
+    const int f = t >> (logPX - 1), u = t & (H - 1);
+    const int i = u & (h - 1), p = ((u >> sh) << (sh + 1)) + i;
+    float2* xf = x + f * PXP;
+    const float2 a = xf[phys(p)], b = cmul_conj(xf[phys(p + h)], tw[i << (logPX - 1 - sh)]);
+    xf[phys(p)] = cadd(a, b);
+    xf[phys(p + h)] = csub(a, b);
+  }
+}
+// Two stages at once (spans h = 2^sh and h/2), four points per work item in registers.
+__device__ __forceinline__ void dif_pair(float2* x, int f_count, int logPX, int sh, const float2* tw, int PXP) {
+  const int Q = 1 << (logPX - 2), h = 1 << sh, hh = h >> 1;
+  for (int t = threadIdx.x; t < f_count * Q; t += blockDim.x) {
+    const int f = t >> (logPX - 2), u = t & (Q - 1);
+    const int i = u & (hh - 1), p0 = ((u >> (sh - 1)) << (sh + 1)) + i;
+    float2* xf = x + f * PXP;
+    const int q0 = phys(p0), q1 = phys(p0 + hh), q2 = phys(p0 + h), q3 = phys(p0 + h + hh);
+    const float2 x0 = xf[q0], x1 = xf[q1], x2 = xf[q2], x3 = xf[q3];
+    const int ts = logPX - 1 - sh;                                // twiddle stride of span h
+    const float2 a0 = cadd(x0, x2), a2 = cmul(csub(x0, x2), tw[i << ts]);
+    const float2 a1 = cadd(x1, x3), a3 = cmul(csub(x1, x3), tw[(i + hh) << ts]);
+    const float2 w = tw[i << (ts + 1)];
+    xf[q0] = cadd(a0, a1); xf[q1] = cmul(csub(a0, a1), w);
+    xf[q2] = cadd(a2, a3); xf[q3] = cmul(csub(a2, a3), w);
+  }
+}
+// spans h = 2^sh and 2h
+__device__ __forceinline__ void dit_pair(float2* x, int f_count, int logPX, int sh, const float2* tw, int PXP) {
+  const int Q = 1 << (logPX - 2), h = 1 << sh;
+  for (int t = threadIdx.x; t < f_count * Q; t += blockDim.x) {
+    const int f = t >> (logPX - 2), u = t & (Q - 1);
+    const int i = u & (h - 1), p0 = ((u >> sh) << (sh + 2)) + i;
+    float2* xf = x + f * PXP;
+    const int q0 = phys(p0), q1 = phys(p0 + h), q2 = phys(p0 + 2 * h), q3 = phys(p0 + 3 * h);
+    const float2 x0 = xf[q0], x1 = xf[q1], x2 = xf[q2], x3 = xf[q3];
+    const int ts = logPX - 1 - sh;
+    const float2 w = tw[i << ts];
+    const float2 b1 = cmul_conj(x1, w), b3 = cmul_conj(x3, w);
+    const float2 a0 = cadd(x0, b1), a1 = csub(x0, b1), a2 = cadd(x2, b3), a3 = csub(x2, b3);
+    const float2 c2 = cmul_conj(a2, tw[i << (ts - 1)]), c3 = cmul_conj(a3, tw[(i + h) << (ts - 1)]);
+    xf[q0] = cadd(a0, c2); xf[q2] = csub(a0, c2);
+    xf[q1] = cadd(a1, c3); xf[q3] = csub(a1, c3);
+  }
+}
+// Spans 4, 2, 1 (forward) / 1, 2, 4 (inverse) of one aligned 8-point chunk, in registers.
+constexpr float kR = 0.70710678118654752440f;
+template <bool INV>
+__device__ __forceinline__ void chunk8(float2* x, int f_count, int logPX, int PXP) {
+  const int C = 1 << (logPX - 3);
+  for (int t = threadIdx.x; t < f_count * C; t += blockDim.x) {
+    const int f = t >> (logPX - 3), u = t & (C - 1);
+    float2* xc = x + f * PXP + 9 * u;                            // phys(8 u) = 9 u; the 8 points are contiguous
+    float2 v[8];
+#pragma unroll
+    for (int n = 0; n < 8; ++n) v[n] = xc[n];
+    // w8[i] = exp(-2 pi i i / 8)
+    const float2 w8[4] = {make_float2(1.f, 0.f), make_float2(kR, -kR), make_float2(0.f, -1.f), make_float2(-kR, -kR)};
+    if (!INV) {
+#pragma unroll
+      for (int i = 0; i < 4; ++i) { const float2 a = v[i], b = v[i + 4]; v[i] = cadd(a, b); v[i + 4] = cmul(csub(a, b), w8[i]); }
+#pragma unroll
+      for (int blk = 0; blk < 8; blk += 4)
+#pragma unroll
+        for (int i = 0; i < 2; ++i) { const float2 a = v[blk + i], b = v[blk + i + 2]; v[blk + i] = cadd(a, b); v[blk + i + 2] = cmul(csub(a, b), w8[2 * i]); }
+#pragma unroll
+      for (int blk = 0; blk < 8; blk += 2) { const float2 a = v[blk], b = v[blk + 1]; v[blk] = cadd(a, b); v[blk + 1] = csub(a, b); }
+    } else {
+#pragma unroll
+      for (int blk = 0; blk < 8; blk += 2) { const float2 a = v[blk], b = v[blk + 1]; v[blk] = cadd(a, b); v[blk + 1] = csub(a, b); }
+#pragma unroll
+      for (int blk = 0; blk < 8; blk += 4)
+#pragma unroll
+        for (int i = 0; i < 2; ++i) { const float2 a = v[blk + i], b = cmul_conj(v[blk + i + 2], w8[2 * i]); v[blk + i] = cadd(a, b); v[blk + i + 2] = csub(a, b); }
+#pragma unroll
+      for (int i = 0; i < 4; ++i) { const float2 a = v[i], b = cmul_conj(v[i + 4], w8[i]); v[i] = cadd(a, b); v[i + 4] = csub(a, b); }
+    }
+#pragma unroll
+    for (int n = 0; n < 8; ++n) xc[n] = v[n];
   }
 }
 
-// Bh_a = sum_b Kh_ab Mh_b  (Kh already carries -mu_0 and the 1/(px py pz) of the unnormalised inverse transform)
-__global__ void multiply_tensor(const cufftComplex* __restrict__ Kh, const cufftComplex* __restrict__ Mh,
-                                cufftComplex* __restrict__ Bh, size_t n) {
-  const size_t t = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
-  if (t >= n) return;
-  const cufftComplex m0 = Mh[t], m1 = Mh[n + t], m2 = Mh[2 * n + t];
-  const cufftComplex kxx = Kh[t], kyy = Kh[n + t], kzz = Kh[2 * n + t], kxy = Kh[3 * n + t], kxz = Kh[4 * n + t],
-                     kyz = Kh[5 * n + t];
-  auto mac = [](cufftComplex a, cufftComplex b, cufftComplex acc) {
-    acc.x += a.x * b.x - a.y * b.y; acc.y += a.x * b.y + a.y * b.x; return acc;
-  };
-  const cufftComplex z = make_cuFloatComplex(0.0f, 0.0f);
-  Bh[t] = mac(kxz, m2, mac(kxy, m1, mac(kxx, m0, z)));
-  Bh[n + t] = mac(kyz, m2, mac(kyy, m1, mac(kxy, m0, z)));
-  Bh[2 * n + t] = mac(kzz, m2, mac(kyz, m1, mac(kxz, m0, z)));
+// One CTA per (ky, output component oc): x-FFT of all F = 3 dcz input fields, the tensor product with the direct sum
+// over layers, inverse x-FFT of the dcz output fields of component oc.
+__global__ void __launch_bounds__(1024, 1)
+demag_xconv(const float2* __restrict__ Y, float2* __restrict__ Z, const float* __restrict__ Kh,
+            const float2* __restrict__ twx, int dcx, int dcz, int PX, int logPX, int NKY) {
+  extern __shared__ __align__(16) float2 xs[];                   // X[F][PXP] | O[dcz][PXP] | tw[PX/2] | Ks[3][NDZ][PX]
+  const int F = 3 * dcz, NDZ = 2 * dcz - 1, H = PX >> 1, PXP = PX + (PX >> 3);
+  float2* X = xs;
+  float2* O = X + (size_t)F * PXP;
+  float2* tw = O + (size_t)dcz * PXP;
+  float* Ks = reinterpret_cast<float*>(tw + H);
+  const int ky = blockIdx.x, oc = blockIdx.y;
+  const int tid = threadIdx.x, nt = blockDim.x;
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  // constants of the context (not written by the previous kernel): twiddles, and this CTA's slice of the transformed
+  // tensor -- 3 input components x NDZ layer offsets x PX points -- by asynchronous 16-byte copies that land while the
+  // forward transform runs
+  for (int t = tid; t < H; t += nt) tw[t] = __ldg(twx + t);
+  for (int t = tid; t < 3 * NDZ * (PX >> 2); t += nt) {
+    const int row = t / (PX >> 2), q = t - row * (PX >> 2);      // row = b NDZ + dzi
+    const int b = row / NDZ, dzi = row - b * NDZ;
+    const float* src = Kh + (((size_t)tensor_comp(oc, b) * NDZ + dzi) * NKY + ky) * PX + 4 * q;
+    const uint32_t dst = (uint32_t)__cvta_generic_to_shared(Ks + (size_t)row * PX + 4 * q);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+  }
+  asm volatile("cp.async.commit_group;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  __syncthreads();
+  // Load with the first forward stage folded in: the upper half of the padded input is zero (dcx <= PX/2), so that
+  // stage is X[p] = x[p], X[p + PX/2] = x[p] w^p.
+  for (int t = tid; t < F * H; t += nt) {
+    const int f = t >> (logPX - 1), p = t & (H - 1);
+    const float2 v = p < dcx ? Y[((size_t)ky * F + f) * dcx + p] : make_float2(0.0f, 0.0f);
+    X[f * PXP + phys(p)] = v;
+    X[f * PXP + phys(p + H)] = cmul(v, tw[p]);
+  }
+  __syncthreads();
+  if (logPX >= 4) {
+    int sh = logPX - 2;
+    while (sh >= 4) { dif_pair(X, F, logPX, sh, tw, PXP); sh -= 2; __syncthreads(); }
+    if (sh == 3) { dif_stage(X, F, logPX, 3, tw, PXP); __syncthreads(); }
+    chunk8<false>(X, F, logPX, PXP);
+  } else {
+    for (int sh = logPX - 2; sh >= 0; --sh) { dif_stage(X, F, logPX, sh, tw, PXP); __syncthreads(); }
+  }
+  asm volatile("cp.async.wait_all;" ::: "memory");
+  __syncthreads();
+  // X[f][p] now holds the spectrum at kx = bitrev(p); Ks is in the same order.  One work item per (output layer c, p).
+  for (int t = tid; t < dcz * PX; t += nt) {
+    const int c = t >> logPX, p = t & (PX - 1), pp = phys(p);
+    float2 acc = make_float2(0.0f, 0.0f);
+    for (int b = 0; b < 3; ++b) {
+      const bool imag = tensor_comp(oc, b) >= 4;
+      const float* kp = Ks + (size_t)(b * NDZ + c + dcz - 1) * PX + p;      // dz = c - c' -> dzi = c - c' + dcz - 1
+      const float2* xp = X + (size_t)(b * dcz) * PXP + pp;
+      float2 s = make_float2(0.0f, 0.0f);
+      for (int cp = 0; cp < dcz; ++cp) {
+        const float kap = kp[-cp * PX];
+        const float2 x = xp[cp * PXP];
+        s.x = fmaf(kap, x.x, s.x); s.y = fmaf(kap, x.y, s.y);
+      }
+      if (imag) { acc.x -= s.y; acc.y += s.x; } else { acc.x += s.x; acc.y += s.y; }
+    }
+    O[c * PXP + pp] = acc;
+  }
+  __syncthreads();
+  if (logPX >= 4) {
+    chunk8<true>(O, dcz, logPX, PXP);
+    __syncthreads();
+    int sh = 3;
+    while (sh + 1 <= logPX - 1) { dit_pair(O, dcz, logPX, sh, tw, PXP); sh += 2; __syncthreads(); }
+    if (sh == logPX - 1) { dit_stage(O, dcz, logPX, sh, tw, PXP); __syncthreads(); }
+  } else {
+    for (int sh = 0; sh < logPX; ++sh) { dit_stage(O, dcz, logPX, sh, tw, PXP); __syncthreads(); }
+  }
+  for (int t = tid; t < dcz * dcx; t += nt) {
+    const int c = t / dcx, a = t - c * dcx;
+    Z[((size_t)ky * F + (size_t)(oc * dcz + c)) * dcx + a] = O[c * PXP + phys(a)];
+  }
+}
+
+// Inverse y-DFT of the half spectrum: B_f(a, b) = Re sum_ky wgt_ky Z[ky][f][a] exp(+2 pi i ky b / PY), wgt = 1 for
+// ky = 0 and PY/2, 2 otherwise (Hermitian symmetry of a real field).  One CTA per (field f, 8 x-cells); one output per
+// thread and pass.
+constexpr int kYinvCols = 8;
+__global__ void demag_yinv(const float2* __restrict__ Z, const float2* __restrict__ twy, float* __restrict__ B,
+                           int dcx, int dcy, int dcz, int PY, int NKY) {
+  extern __shared__ __align__(16) float2 zs[];                   // [NKY][8] | tws[PY]
+  float2* tws = zs + NKY * kYinvCols;
+  const int F = 3 * dcz, f = blockIdx.y, a0 = blockIdx.x * kYinvCols;
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  for (int t = threadIdx.x; t < PY; t += blockDim.x) tws[t] = __ldg(twy + t);
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  for (int t = threadIdx.x; t < NKY * kYinvCols; t += blockDim.x) {
+    const int ky = t / kYinvCols, da = t - ky * kYinvCols;
+    float2 v = make_float2(0.0f, 0.0f);
+    if (a0 + da < dcx) v = Z[((size_t)ky * F + f) * dcx + a0 + da];
+    const float wgt = (ky == 0 || ky == NKY - 1) ? 1.0f : 2.0f;
+    zs[t] = make_float2(wgt * v.x, wgt * v.y);
+  }
+  __syncthreads();
+  const int comp = f / dcz, c = f - comp * dcz;
+  for (int t = threadIdx.x; t < dcy * kYinvCols; t += blockDim.x) {
+    const int b = t / kYinvCols, da = t - b * kYinvCols;
+    if (a0 + da >= dcx) continue;
+    float acc0 = 0.0f, acc1 = 0.0f;
+    int ky = 0;
+    for (; ky + 1 < NKY; ky += 2) {
+      const float2 w0 = tws[(ky * b) & (PY - 1)], w1 = tws[((ky + 1) * b) & (PY - 1)];
+      const float2 z0 = zs[ky * kYinvCols + da], z1 = zs[(ky + 1) * kYinvCols + da];
+      acc0 = fmaf(z0.x, w0.x, fmaf(-z0.y, w0.y, acc0));
+      acc1 = fmaf(z1.x, w1.x, fmaf(-z1.y, w1.y, acc1));
+    }
+    if (ky < NKY) {
+      const float2 w0 = tws[(ky * b) & (PY - 1)];
+      const float2 z0 = zs[ky * kYinvCols + da];
+      acc0 = fmaf(z0.x, w0.x, fmaf(-z0.y, w0.y, acc0));
+    }
+    B[(((size_t)comp * dcx + (a0 + da)) * dcy + b) * dcz + c] = acc0 + acc1;
+  }
 }
 
 void plan_dims(const Ctx& c, DemagPlan& pl) {
   pl.dcx = (c.d.nx + c.d.macro[0] - 2) / c.d.macro[0] + 1;
   pl.dcy = (c.d.ny + c.d.macro[1] - 1) / c.d.macro[1];
   pl.dcz = (c.d.nz + c.d.macro[2] - 1) / c.d.macro[2];
-  pl.px = nice_size(2 * pl.dcx - 1); pl.py = nice_size(2 * pl.dcy - 1); pl.pz = nice_size(2 * pl.dcz - 1);
-  if (pl.pz & 1) pl.pz = nice_size(pl.pz + 1);                 // even last dimension: aligned rows for R2C / C2R
-  pl.pzc = pl.pz / 2 + 1;
+  pl.PX = std::max(4, pow2_at_least(2 * pl.dcx - 1)); pl.PY = pow2_at_least(2 * pl.dcy - 1);   // PX >= 4: 16-byte rows of the tensor slice
+  pl.logPX = 0;
+  while ((1 << pl.logPX) < pl.PX) ++pl.logPX;
+  pl.NKY = pl.PY / 2 + 1; pl.F = 3 * pl.dcz; pl.NDZ = 2 * pl.dcz - 1;
+  const size_t PXP = (size_t)pl.PX + pl.PX / 8;
+  pl.xconv_smem = ((size_t)(pl.F + pl.dcz) * PXP + pl.PX / 2) * sizeof(float2) + (size_t)3 * pl.NDZ * pl.PX * sizeof(float);
+  // one 8-point chunk per thread in the register stage (two 4-point items in the paired stages)
+  const size_t chunks = (size_t)pl.F * std::max(pl.PX / 8, 1);
+  pl.xconv_threads = (unsigned)std::min<size_t>(1024, std::max<size_t>(128, (chunks + 31) / 32 * 32));
+}
+
+size_t cg_smem_bytes(int lanes, int ny, const DemagPlan& pl) {
+  return ((size_t)lanes * 3 * ny + ((3 * (size_t)pl.dcy + 1) & ~(size_t)1)) * sizeof(float) + (size_t)pl.PY * sizeof(float2);
 }
 
 struct Carve {
-  size_t M, Mh, Kh, B, work, total;
+  size_t Y, Z, Kh, B, twx, twy, total;
 };
-bool make_plans(DemagPlan& pl, size_t work[2]) {
-  int n[3] = {pl.px, pl.py, pl.pz};
-  if (cufftCreate(&pl.fwd) != CUFFT_SUCCESS || cufftCreate(&pl.inv) != CUFFT_SUCCESS) return false;
-  cufftSetAutoAllocation(pl.fwd, 0); cufftSetAutoAllocation(pl.inv, 0);
-  if (cufftMakePlanMany(pl.fwd, 3, n, nullptr, 1, 0, nullptr, 1, 0, CUFFT_R2C, 3, &work[0]) != CUFFT_SUCCESS) return false;
-  if (cufftMakePlanMany(pl.inv, 3, n, nullptr, 1, 0, nullptr, 1, 0, CUFFT_C2R, 3, &work[1]) != CUFFT_SUCCESS) return false;
-  pl.plans = true;
-  return true;
-}
-void carve(const DemagPlan& pl, const size_t work[2], Carve& cv) {
-  const size_t real = (size_t)pl.px * pl.py * pl.pz, cplx = (size_t)pl.px * pl.py * pl.pzc;
+void carve(const DemagPlan& pl, Carve& cv) {
+  const size_t spec = (size_t)pl.NKY * pl.F * pl.dcx;
   size_t off = 0;
   auto take = [&](size_t bytes) { const size_t o = off; off = align_up(off + bytes, 256); return o; };
-  cv.M = take(3 * real * sizeof(float));
-  cv.Mh = take(3 * cplx * sizeof(cufftComplex));
-  cv.Kh = take(6 * cplx * sizeof(cufftComplex));
-  cv.B = take(3 * real * sizeof(float));
-  cv.work = take(work[0] > work[1] ? work[0] : work[1]);
+  cv.Y = take(spec * sizeof(float2));
+  cv.Z = take(spec * sizeof(float2));
+  cv.Kh = take((size_t)6 * pl.NDZ * pl.NKY * pl.PX * sizeof(float));
+  cv.B = take((size_t)3 * pl.dcx * pl.dcy * pl.dcz * sizeof(float));
+  cv.twx = take((size_t)(pl.PX / 2) * sizeof(float2));
+  cv.twy = take((size_t)pl.PY * sizeof(float2));
   cv.total = off;
 }
 
 }  // namespace
 
 void demag_free(Ctx& c) {
-  if (!c.demag) return;
-  if (c.demag->plans) { cufftDestroy(c.demag->fwd); cufftDestroy(c.demag->inv); }
   delete c.demag;
   c.demag = nullptr;
 }
@@ -216,89 +500,122 @@ void demag_free(Ctx& c) {
 size_t demag_workspace_bytes(Ctx& c) {
   DemagPlan pl;
   plan_dims(c, pl);
-  size_t work[2] = {0, 0};
-  const bool ok = make_plans(pl, work);
-  if (pl.fwd) cufftDestroy(pl.fwd);
-  if (pl.inv) cufftDestroy(pl.inv);
-  if (!ok) return 0;
   Carve cv;
-  carve(pl, work, cv);
+  carve(pl, cv);
   return cv.total;
 }
 
 asd_status demag_enable(Ctx& c, const double spacing[3], void* ws, size_t bytes) {
-  if ((c.d.ny % 4 == 0 ? c.d.ny / 4 : c.d.ny) > 1024 || (size_t)c.d.ny * 12 * kMaxRowLanes > 48 * 1024) { std::snprintf(c.err, sizeof(c.err), "asd_enable_demag: ny too large for the coarse-graining kernel"); return ASD_EUNSUPPORTED; }
+  if ((c.d.ny % 4 == 0 ? c.d.ny / 4 : c.d.ny) > 1024) { std::snprintf(c.err, sizeof(c.err), "asd_enable_demag: ny too large for the coarse-graining kernel"); return ASD_EUNSUPPORTED; }
   demag_free(c);
   DemagPlan* pl = new DemagPlan();
   plan_dims(c, *pl);
-  size_t work[2] = {0, 0};
-  if (!make_plans(*pl, work)) { c.demag = pl; demag_free(c); std::snprintf(c.err, sizeof(c.err), "cuFFT plan creation failed"); return ASD_ECUDA; }
+  int smem_cta = 0;
+  cudaDeviceGetAttribute(&smem_cta, cudaDevAttrMaxSharedMemoryPerBlockOptin, c.device);
+  const size_t cg_smem = cg_smem_bytes(kMaxRowLanes, c.d.ny, *pl);
+  if (pl->xconv_smem > (size_t)smem_cta || cg_smem > (size_t)smem_cta) {
+    delete pl;
+    std::snprintf(c.err, sizeof(c.err), "asd_enable_demag: window too long / thick for the shared-memory transform (3 dcz fields x PX points must fit in %d bytes)", smem_cta);
+    return ASD_EUNSUPPORTED;
+  }
   Carve cv;
-  carve(*pl, work, cv);
+  carve(*pl, cv);
+  if (bytes < cv.total) { delete pl; std::snprintf(c.err, sizeof(c.err), "demag workspace too small"); return ASD_ENOMEM; }
   c.demag = pl;
-  if (bytes < cv.total) { demag_free(c); std::snprintf(c.err, sizeof(c.err), "demag workspace too small"); return ASD_ENOMEM; }
   char* base = (char*)ws;
-  pl->M = (float*)(base + cv.M); pl->Mh = (cufftComplex*)(base + cv.Mh); pl->Kh = (cufftComplex*)(base + cv.Kh);
-  pl->B = (float*)(base + cv.B);
-  cufftSetWorkArea(pl->fwd, base + cv.work); cufftSetWorkArea(pl->inv, base + cv.work);
+  pl->Y = (float2*)(base + cv.Y); pl->Z = (float2*)(base + cv.Z); pl->Kh = (float*)(base + cv.Kh);
+  pl->B = (float*)(base + cv.B); pl->twx = (float2*)(base + cv.twx); pl->twy = (float2*)(base + cv.twy);
   for (int a = 0; a < 3; ++a) pl->cell[a] = c.d.macro[a] * spacing[a];
   pl->mu_over_V = (float)(c.d.mu_s / (pl->cell[0] * pl->cell[1] * pl->cell[2]));
+  ASD_CUDA_TRY(c, cudaFuncSetAttribute((const void*)demag_xconv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->xconv_smem));
+  ASD_CUDA_TRY(c, cudaFuncSetAttribute((const void*)coarse_grain_ydft<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cg_smem));
+  ASD_CUDA_TRY(c, cudaFuncSetAttribute((const void*)coarse_grain_ydft<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cg_smem));
 
-  // the six tensor components on the padded, wrapped grid (fp64 on the host), scaled by -mu_0 / (px py pz)
-  const size_t real = (size_t)pl->px * pl->py * pl->pz, cplx = (size_t)pl->px * pl->py * pl->pzc;
-  const double scale = -4.0e-7 * kPi / (double)real;
-  std::vector<float> K(6 * real, 0.0f);
-  for (int a = -(pl->dcx - 1); a <= pl->dcx - 1; ++a)
-    for (int b = -(pl->dcy - 1); b <= pl->dcy - 1; ++b)
-      for (int g = -(pl->dcz - 1); g <= pl->dcz - 1; ++g) {
+  // The six tensor components for every cell offset (fp64, host), one (x, y) plane per layer offset dz: wrapped onto the
+  // PX x PY grid, transformed, scaled by -mu_0 / (PX PY) (both inverse transforms are unnormalised), reduced to the real
+  // or imaginary part that survives, and stored with the x index bit-reversed (the order demag_xconv's forward transform
+  // leaves its spectra in).
+  const int PX = pl->PX, PY = pl->PY, NKY = pl->NKY, NDZ = pl->NDZ;
+  const double scale = -4.0e-7 * kPi / ((double)PX * PY);
+  std::vector<float> Kh((size_t)6 * NDZ * NKY * PX, 0.0f);
+  std::vector<std::complex<double>> plane((size_t)6 * PX * PY), line((size_t)std::max(PX, PY));
+  std::vector<uint32_t> rev(PX);
+  for (int p = 0; p < PX; ++p) rev[p] = bit_reverse((uint32_t)p, pl->logPX);
+  for (int dzi = 0; dzi < NDZ; ++dzi) {
+    const int g = dzi - (pl->dcz - 1);
+    std::fill(plane.begin(), plane.end(), std::complex<double>(0.0, 0.0));
+    for (int a = -(pl->dcx - 1); a <= pl->dcx - 1; ++a)
+      for (int b = -(pl->dcy - 1); b <= pl->dcy - 1; ++b) {
         const double R[3] = {a * pl->cell[0], b * pl->cell[1], g * pl->cell[2]};
         double N[6];
         cuboid_tensor(pl->cell, R, N);
-        const size_t q = ((size_t)((a + pl->px) % pl->px) * pl->py + (size_t)((b + pl->py) % pl->py)) * pl->pz +
-                         (size_t)((g + pl->pz) % pl->pz);
-        for (int comp = 0; comp < 6; ++comp) K[comp * real + q] = (float)(N[comp] * scale);
+        const size_t q = (size_t)((a + PX) % PX) * PY + (size_t)((b + PY) % PY);
+        for (int comp = 0; comp < 6; ++comp) plane[(size_t)comp * PX * PY + q] = N[comp] * scale;
       }
-  // transform them once: stage the real kernels in M / B (3 at a time), R2C into Kh
-  ASD_CUDA_TRY(c, cudaMemsetAsync(pl->M, 0, 3 * real * sizeof(float), c.stream));
-  cufftSetStream(pl->fwd, c.stream);
-  for (int half = 0; half < 2; ++half) {
-    ASD_CUDA_TRY(c, cudaMemcpyAsync(pl->B, K.data() + (size_t)half * 3 * real, 3 * real * sizeof(float),
-                                    cudaMemcpyHostToDevice, c.stream));
-    if (cufftExecR2C(pl->fwd, pl->B, pl->Kh + (size_t)half * 3 * cplx) != CUFFT_SUCCESS) return fail_cuda(c, cudaErrorUnknown, "cufftExecR2C (tensor)");
-    ASD_CUDA_TRY(c, cudaStreamSynchronize(c.stream));        // K is host memory about to go out of scope
+    for (int comp = 0; comp < 6; ++comp) {
+      std::complex<double>* P = plane.data() + (size_t)comp * PX * PY;
+      for (int x = 0; x < PX; ++x) host_fft(P + (size_t)x * PY, PY);
+      for (int y = 0; y < NKY; ++y) {
+        for (int x = 0; x < PX; ++x) line[x] = P[(size_t)x * PY + y];
+        host_fft(line.data(), PX);
+        float* dst = Kh.data() + (((size_t)comp * NDZ + dzi) * NKY + y) * PX;
+        for (int p = 0; p < PX; ++p) dst[p] = (float)(comp >= 4 ? line[rev[p]].imag() : line[rev[p]].real());
+      }
+    }
   }
-  ASD_CUDA_TRY(c, cudaMemsetAsync(pl->B, 0, 3 * real * sizeof(float), c.stream));
+  std::vector<float2> twx(PX / 2), twy(PY);
+  for (int n = 0; n < PX / 2; ++n) twx[n] = make_float2((float)std::cos(-2.0 * kPi * n / PX), (float)std::sin(-2.0 * kPi * n / PX));
+  for (int n = 0; n < PY; ++n) twy[n] = make_float2((float)std::cos(2.0 * kPi * n / PY), (float)std::sin(2.0 * kPi * n / PY));
+  ASD_CUDA_TRY(c, cudaMemcpyAsync(pl->Kh, Kh.data(), Kh.size() * sizeof(float), cudaMemcpyHostToDevice, c.stream));
+  ASD_CUDA_TRY(c, cudaMemcpyAsync(pl->twx, twx.data(), twx.size() * sizeof(float2), cudaMemcpyHostToDevice, c.stream));
+  ASD_CUDA_TRY(c, cudaMemcpyAsync(pl->twy, twy.data(), twy.size() * sizeof(float2), cudaMemcpyHostToDevice, c.stream));
+  ASD_CUDA_TRY(c, cudaMemsetAsync(pl->B, 0, (size_t)3 * pl->dcx * pl->dcy * pl->dcz * sizeof(float), c.stream));
+  ASD_CUDA_TRY(c, cudaStreamSynchronize(c.stream));             // the host vectors are about to go out of scope
   graphs_invalidate(c);
   return ASD_OK;
 }
 
+namespace {
+template <typename... Args>
+void launch_chain(void (*kern)(Args...), dim3 grid, unsigned threads, size_t smem, cudaStream_t stream, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  cudaLaunchKernelEx(&cfg, kern, args...);
+}
+}  // namespace
+
 // Demagnetising field of the configuration in array block aX (S or S~) into demag->B, on c.launch_stream.
 asd_status launch_demag(Ctx& c, int aX) {
   DemagPlan& pl = *c.demag;
-  const size_t real = (size_t)pl.px * pl.py * pl.pz, cplx = (size_t)pl.px * pl.py * pl.pzc;
   {
     const int vec = (c.d.ny % 4 == 0) ? 4 : 1, groups = c.d.ny / vec;
     int lanes = 1024 / groups;
     if (lanes > kMaxRowLanes) lanes = kMaxRowLanes;
     if (lanes < 1) lanes = 1;                                   // groups <= 1024 is checked at enable time
     const int threads = (int)align_up((size_t)(groups * lanes), 32);
-    const size_t smem = (size_t)lanes * 3 * c.d.ny * sizeof(float);
+    const size_t smem = cg_smem_bytes(lanes, c.d.ny, pl);
     const unsigned blocks = (unsigned)(pl.dcx * pl.dcz);
     if (vec == 4)
-      coarse_grain_cells<4><<<blocks, threads, smem, c.launch_stream>>>(
+      coarse_grain_ydft<4><<<blocks, threads, smem, c.launch_stream>>>(
           c.arr(aX), (uint32_t)c.as, c.d.nx, c.d.ny, c.d.nz, c.nyp, c.lead, c.d.macro[0], c.d.macro[1], c.d.macro[2],
-          (long long)c.x0, pl.dcy, pl.dcz, pl.py, pl.pz, real, pl.mu_over_V, lanes, pl.M);
+          (long long)c.x0, pl.dcx, pl.dcy, pl.dcz, pl.PY, pl.NKY, pl.mu_over_V, lanes, pl.twy, pl.Y);
     else
-      coarse_grain_cells<1><<<blocks, threads, smem, c.launch_stream>>>(
+      coarse_grain_ydft<1><<<blocks, threads, smem, c.launch_stream>>>(
           c.arr(aX), (uint32_t)c.as, c.d.nx, c.d.ny, c.d.nz, c.nyp, c.lead, c.d.macro[0], c.d.macro[1], c.d.macro[2],
-          (long long)c.x0, pl.dcy, pl.dcz, pl.py, pl.pz, real, pl.mu_over_V, lanes, pl.M);
+          (long long)c.x0, pl.dcx, pl.dcy, pl.dcz, pl.PY, pl.NKY, pl.mu_over_V, lanes, pl.twy, pl.Y);
   }
-  ASD_LAUNCH_CHECK(c, "coarse_grain_cells");
-  cufftSetStream(pl.fwd, c.launch_stream); cufftSetStream(pl.inv, c.launch_stream);
-  if (cufftExecR2C(pl.fwd, pl.M, pl.Mh) != CUFFT_SUCCESS) return fail_cuda(c, cudaErrorUnknown, "cufftExecR2C");
-  multiply_tensor<<<(unsigned)((cplx + 255) / 256), 256, 0, c.launch_stream>>>(pl.Kh, pl.Mh, pl.Mh, cplx);
-  ASD_LAUNCH_CHECK(c, "multiply_tensor");
-  if (cufftExecC2R(pl.inv, pl.Mh, pl.B) != CUFFT_SUCCESS) return fail_cuda(c, cudaErrorUnknown, "cufftExecC2R");
+  ASD_LAUNCH_CHECK(c, "coarse_grain_ydft");
+  launch_chain(demag_xconv, dim3((unsigned)pl.NKY, 3u), pl.xconv_threads, pl.xconv_smem, c.launch_stream,
+               (const float2*)pl.Y, pl.Z, (const float*)pl.Kh, (const float2*)pl.twx, pl.dcx, pl.dcz, pl.PX, pl.logPX, pl.NKY);
+  ASD_LAUNCH_CHECK(c, "demag_xconv");
+  launch_chain(demag_yinv, dim3((unsigned)((pl.dcx + kYinvCols - 1) / kYinvCols), (unsigned)pl.F), 256u,
+               ((size_t)pl.NKY * kYinvCols + pl.PY) * sizeof(float2), c.launch_stream,
+               (const float2*)pl.Z, (const float2*)pl.twy, pl.B, pl.dcx, pl.dcy, pl.dcz, pl.PY, pl.NKY);
+  ASD_LAUNCH_CHECK(c, "demag_yinv");
   return ASD_OK;
 }
 
@@ -307,8 +624,8 @@ void demag_fill_params(const Ctx& c, StageParams& p) {
   if (!c.demag) return;
   const DemagPlan& pl = *c.demag;
   p.dm.B = pl.B;
-  p.dm.comp_stride = (uint32_t)((size_t)pl.px * pl.py * pl.pz);
-  p.dm.sx = (uint32_t)(pl.py * pl.pz); p.dm.sy = (uint32_t)pl.pz;
+  p.dm.comp_stride = (uint32_t)((size_t)pl.dcx * pl.dcy * pl.dcz);
+  p.dm.sx = (uint32_t)(pl.dcy * pl.dcz); p.dm.sy = (uint32_t)pl.dcz;
   magic_u31((uint32_t)c.d.macro[0], p.dm.mx_m, p.dm.mx_s);
   magic_u31((uint32_t)c.d.macro[1], p.dm.my_m, p.dm.my_s);
   magic_u31((uint32_t)c.d.macro[2], p.dm.mz_m, p.dm.mz_s);
@@ -323,9 +640,9 @@ asd_status demag_field_host(Ctx& c, float* out, int64_t dims[3]) {
   c.launch_stream = c.stream;
   const asd_status st = launch_demag(c, c.aS);
   if (st != ASD_OK) return st;
-  const size_t real = (size_t)pl.px * pl.py * pl.pz;
-  std::vector<float> h(3 * real);
-  ASD_CUDA_TRY(c, cudaMemcpyAsync(h.data(), pl.B, 3 * real * sizeof(float), cudaMemcpyDeviceToHost, c.stream));
+  const size_t cells = (size_t)pl.dcx * pl.dcy * pl.dcz;
+  std::vector<float> h(3 * cells);
+  ASD_CUDA_TRY(c, cudaMemcpyAsync(h.data(), pl.B, 3 * cells * sizeof(float), cudaMemcpyDeviceToHost, c.stream));
   ASD_CUDA_TRY(c, cudaStreamSynchronize(c.stream));
   // cells of the spare x-slot that do not overlap the window at this alignment hold no site: reported as 0
   const int ncx = (int)((c.x0 + c.d.nx - 1) / c.d.macro[0] - c.x0 / c.d.macro[0]) + 1;
@@ -334,7 +651,7 @@ asd_status demag_field_host(Ctx& c, float* out, int64_t dims[3]) {
       for (int g = 0; g < pl.dcz; ++g)
         for (int comp = 0; comp < 3; ++comp)
           out[(((size_t)a * pl.dcy + b) * pl.dcz + g) * 3 + comp] =
-              a < ncx ? h[comp * real + ((size_t)a * pl.py + b) * pl.pz + g] : 0.0f;
+              a < ncx ? h[comp * cells + ((size_t)a * pl.dcy + b) * pl.dcz + g] : 0.0f;
   return ASD_OK;
 }
 
