@@ -15,3 +15,4 @@ from .workloads import (  # noqa: F401
     GAMMA_E, MU_B, K_B, SC, L10, Workload, voronoi_grain_map, laser_temperature, tilted_spins,
     make_config, small_film, ShiftSchedule, planes_for_shift, nrz_bits, field_scale_at,
 )
+from .two_track import TwoTrack, two_track_film, drive_pass, read_tracks  # noqa: F401

@@ -17,6 +17,8 @@
 //   * atomistic->macrocell transfer Eq. (6), P:64-66 -> orc_shift_window() outgoing part
 //   * macrocell->atomistic cone thermalisation, P:68 -> seed_site()  (S:S3 reading)
 //   * Philox4x32-10 (Salmon et al., SC'11, public definition) -> philox4x32_10()
+//   * passes over the track (two parallel tracks) -> orc_track_end_pass(), orc_track_begin_pass();
+//     Gaussian-footprint read-back standing in for the TMR head -> orc_track_read_scan()  (S:8(f) item 4)
 //
 // Everything is written in the paper's order and notation, one site at a time, with
 // explicit coordinate loops; no blocking, fusion or reordering.  OpenMP is used only
@@ -455,6 +457,18 @@ void seed_site(const Oracle& o, int64_t gx, int k, int j, double S[3]) {
   for (int a = 0; a < 3; ++a) S[a] = st * cp * e1[a] + st * sp * e2[a] + ct * n[a];
 }
 
+// Window plane i becomes global plane gx of the track: vacant columns 0, magnetic sites seeded (S3).
+void seed_plane(Oracle& o, int i, int64_t gx) {
+  for (int k = 0; k < o.nz; ++k)
+    for (int j = 0; j < o.ny; ++j) {
+      const int64_t l = o.site(i, k, j);
+      if (o.grain_map[(size_t)(gx * o.ny + j)] < 0) { o.sx[l] = o.sy[l] = o.sz[l] = 0.0; continue; }
+      double S[3];
+      seed_site(o, gx, k, j, S);
+      o.sx[l] = S[0]; o.sy[l] = S[1]; o.sz[l] = S[2];
+    }
+}
+
 }  // namespace
 
 // ============================================================================
@@ -696,18 +710,79 @@ int orc_shift_window(void* h, int32_t p) {
         o.sx[l] = o.sx[s]; o.sy[l] = o.sy[s]; o.sz[l] = o.sz[s];
       }
   // S3 incoming: planes i >= nx-p; new global plane gx = x0 + p + i.
-  for (int i = nx - p; i < nx; ++i)
-    for (int k = 0; k < nz; ++k)
-      for (int j = 0; j < ny; ++j) {
-        const int64_t l = o.site(i, k, j);
-        const int64_t gx = o.x0 + p + i;
-        if (o.grain_map[(size_t)(gx * ny + j)] < 0) { o.sx[l] = o.sy[l] = o.sz[l] = 0.0; continue; }
-        double S[3];
-        seed_site(o, gx, k, j, S);
-        o.sx[l] = S[0]; o.sy[l] = S[1]; o.sz[l] = S[2];
-      }
+  for (int i = nx - p; i < nx; ++i) seed_plane(o, i, o.x0 + p + i);
   o.x0 += p; o.shift += 1;                              // S4: T and B are NOT moved
   return 0;
+}
+
+// ---- Passes over the track (S:8(f) item 4; sec. III / Fig. 4: "The two tracks were written sequentially ...
+// The written bit pattern was then used as the starting state for a second pass through the track shifting algorithm").
+// Readings T1-T3 of DESIGN.md sec. 13.
+//
+// T1 end of a pass: the planes still inside the window are transferred to the track by Eq. (6) exactly as outgoing
+//    planes are (S2), and every macrocell the pass has written (count > 0) becomes what lies ahead of the next pass:
+//    init_mean[c] = out_sum[c] / out_cnt[c]  (mean spin = M / M_S^0 of the cell).  Cells never written keep their value.
+//    The written store is kept (orc_track_get / orc_track_read_scan read it).
+int orc_track_end_pass(void* h) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  if (o.ell_width > 0) return 5;
+  for (int i = 0; i < o.nx; ++i)
+    for (int k = 0; k < o.nz; ++k)
+      for (int j = 0; j < o.ny; ++j) {
+        if (o.grain_of(i, j) < 0) continue;
+        const int64_t l = o.site(i, k, j);
+        const int64_t c = o.cell_of(o.x0 + i, j, k);
+        o.out_sum[3 * c] += o.sx[l]; o.out_sum[3 * c + 1] += o.sy[l]; o.out_sum[3 * c + 2] += o.sz[l];
+        o.out_cnt[c] += 1;
+      }
+  const size_t nc = (size_t)(o.ncx * o.ncy * o.ncz);
+  for (size_t c = 0; c < nc; ++c) {
+    if (o.out_cnt[c] == 0) continue;
+    for (int a = 0; a < 3; ++a) o.init_mean[3 * c + a] = o.out_sum[3 * c + a] / (double)o.out_cnt[c];
+  }
+  return 0;
+}
+
+// T2 start of the next pass: the written store is cleared, pass += 1, the window returns to global plane x0_new and
+//    ALL its planes are generated from the track by the cone thermalisation of P:68 (S3), Philox counter n := pass.
+//    The step and shift counters run on.
+int orc_track_begin_pass(void* h, int64_t x0_new) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  if (o.ell_width > 0) return 5;
+  if (x0_new < 0 || x0_new + o.nx > o.track_nx) return 1;
+  const size_t nc = (size_t)(o.ncx * o.ncy * o.ncz);
+  for (size_t c = 0; c < nc; ++c) { o.out_cnt[c] = 0; o.out_sum[3 * c] = o.out_sum[3 * c + 1] = o.out_sum[3 * c + 2] = 0.0; }
+  o.pass += 1;
+  o.x0 = x0_new;
+  o.demag_age = 0;
+  for (int i = 0; i < o.nx; ++i) seed_plane(o, i, o.x0 + i);
+  return 0;
+}
+
+// T3 read-back figure of merit, standing in for the TMR read head of P:114 (which needs a solver that is not part of
+//    the method): the mean S_z per magnetic site under a Gaussian reader footprint, from the WRITTEN store,
+//      R(x_r) = sum_c w_c sum_z[c] / sum_c w_c cnt[c],   w_c = exp(-(x_c - x_r)^2 / (2 sx^2) - (y_c - y_r)^2 / (2 sy^2)),
+//    (x_c, y_c) = nominal centre of macrocell c in site units ((cx + 1/2) mx, (cy + 1/2) my), all layers cz summed;
+//    x_r = x_first + n x_step, n = 0..count-1.  0 where the footprint holds no written site.
+void orc_track_read_scan(void* h, double y_r, double sigma_x, double sigma_y, double x_first, double x_step,
+                         int64_t count, double* out) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  for (int64_t n = 0; n < count; ++n) {
+    const double x_r = x_first + (double)n * x_step;
+    double num = 0.0, den = 0.0;
+    for (int64_t cx = 0; cx < o.ncx; ++cx)
+      for (int64_t cy = 0; cy < o.ncy; ++cy) {
+        const double xc = ((double)cx + 0.5) * o.macro[0], yc = ((double)cy + 0.5) * o.macro[1];
+        const double w = std::exp(-(xc - x_r) * (xc - x_r) / (2.0 * sigma_x * sigma_x)
+                                  - (yc - y_r) * (yc - y_r) / (2.0 * sigma_y * sigma_y));
+        for (int64_t cz = 0; cz < o.ncz; ++cz) {
+          const size_t c = (size_t)((cx * o.ncy + cy) * o.ncz + cz);
+          num += w * o.out_sum[3 * c + 2];
+          den += w * (double)o.out_cnt[c];
+        }
+      }
+    out[n] = den > 0.0 ? num / den : 0.0;
+  }
 }
 
 void orc_track_set_init(void* h, const float* mean_spin /* [ncell*3] or null */, float m0) {

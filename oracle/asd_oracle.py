@@ -84,6 +84,12 @@ def lib():
         L.orc_track_ncell.restype = C.c_int64
         L.orc_track_ncell.argtypes = [C.c_void_p, ip64]
         L.orc_track_get.argtypes = [C.c_void_p, dp, ip64, dp]
+        L.orc_track_end_pass.restype = C.c_int
+        L.orc_track_end_pass.argtypes = [C.c_void_p]
+        L.orc_track_begin_pass.restype = C.c_int
+        L.orc_track_begin_pass.argtypes = [C.c_void_p, C.c_int64]
+        L.orc_track_read_scan.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double,
+                                          C.c_int64, dp]
         L.orc_get_counters.argtypes = [C.c_void_p, ip64, ip64, ip64, ip64]
         L.orc_set_counters.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_int64]
         u32p = C.POINTER(C.c_uint32)
@@ -316,6 +322,22 @@ class Oracle:
         sm = np.zeros((nc, 3))
         lib().orc_track_get(self._h, _ptr(mean, C.c_double), _ptr(cnt, C.c_int64), _ptr(sm, C.c_double))
         return mean, cnt, sm
+
+    def track_end_pass(self) -> int:
+        """Window -> track by Eq. (6); what the pass wrote becomes what lies ahead of the next one (reading T1)."""
+        return int(lib().orc_track_end_pass(self._h))
+
+    def track_begin_pass(self, x0_new: int = 0) -> int:
+        """Written store cleared, pass += 1, window back at plane x0_new and regenerated from the track (reading T2)."""
+        return int(lib().orc_track_begin_pass(self._h, C.c_int64(x0_new)))
+
+    def track_read_scan(self, y_r: float, sigma_x: float, sigma_y: float, x_first: float, x_step: float,
+                        count: int) -> np.ndarray:
+        """Mean S_z per written magnetic site under a Gaussian reader footprint, at `count` positions (reading T3)."""
+        out = np.zeros(int(count))
+        lib().orc_track_read_scan(self._h, C.c_double(y_r), C.c_double(sigma_x), C.c_double(sigma_y),
+                                  C.c_double(x_first), C.c_double(x_step), C.c_int64(count), _ptr(out, C.c_double))
+        return out
 
     def counters(self):
         a, b, c, d = C.c_int64(0), C.c_int64(0), C.c_int64(0), C.c_int64(0)
