@@ -194,6 +194,29 @@ ASD_API asd_status asd_track_set_init(asd_ctx *ctx, const float *mean_spin, floa
  * HOST sum [ncell*3] (fp64), count [ncell]; either may be NULL; synchronises. */
 ASD_API asd_status asd_track_get(asd_ctx *ctx, double *sum, int64_t *count);
 
+/* ---- Passes over the track: writing parallel tracks one after the other (sec. III / Fig. 4: "The written
+ * bit pattern was then used as the starting state for a second pass through the track shifting algorithm"; DESIGN.md
+ * sec. 13, readings T1-T3) -----------------------------------------------------------------------------------------------
+ * asd_track_end_pass    the nx planes still inside the window are transferred to the track by Eq. (6) exactly
+ *                       as outgoing planes are; then every macrocell the pass has written (count > 0) becomes what lies
+ *                       ahead of the next pass: init mean spin = sum / count (cells never written keep theirs).  The
+ *                       written store stays readable (asd_track_get, asd_track_read_scan).  Asynchronous.
+ * asd_track_begin_pass  the written store is cleared, pass counter += 1, the window returns to global plane x0_new
+ *                       (0 <= x0_new <= track_nx - nx) and ALL its planes are generated from the track by the cone
+ *                       sampling of P:68 (D:S3) with Philox counter n := pass; step and shift counters run on.  T and B
+ *                       are not touched.  Asynchronous.  ASD_EUNSUPPORTED with a general ELL table or pbc[0].
+ * asd_track_read_scan   read-back figure of merit standing in for the TMR read head of P:114: the mean S_z per magnetic
+ *                       site of the WRITTEN store under a Gaussian reader footprint,
+ *                         R(x_r) = sum_c w_c sum_z[c] / sum_c w_c count[c],
+ *                         w_c = exp(-(x_c - x_r)^2 / (2 sigma_x^2) - (y_c - y_r)^2 / (2 sigma_y^2)),
+ *                       (x_c, y_c) = ((cx + 1/2) mx, (cy + 1/2) my) the nominal centre of macrocell c in site units (x in
+ *                       global planes), all layers cz summed; x_r = x_first + n x_step, n = 0 .. count-1; 0 where the
+ *                       footprint holds no written site.  out: HOST [count] fp64; deterministic; synchronises. */
+ASD_API asd_status asd_track_end_pass(asd_ctx *ctx);
+ASD_API asd_status asd_track_begin_pass(asd_ctx *ctx, int64_t x0_new);
+ASD_API asd_status asd_track_read_scan(asd_ctx *ctx, double y_r, double sigma_x, double sigma_y, double x_first,
+                                       double x_step, int64_t count, double *out);
+
 /* Counters for bit-exact checkpoint / resume (Philox is counter based: there is no RNG state). */
 ASD_API asd_status asd_get_counters(const asd_ctx *ctx, int64_t *step, int64_t *shift, int64_t *x0, int64_t *pass);
 ASD_API asd_status asd_set_counters(asd_ctx *ctx, int64_t step, int64_t shift, int64_t pass);

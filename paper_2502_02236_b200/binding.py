@@ -23,7 +23,8 @@ EXPORTED_SYMBOLS = [
     "asd_step_heun", "asd_set_kernel", "asd_set_graph_mode", "asd_demag_workspace_bytes", "asd_enable_demag",
     "asd_demag_field", "asd_set_demag_every", "asd_staging_bytes", "asd_set_staging", "asd_stage_fields_host",
     "asd_commit_fields", "asd_shift_window", "asd_magnetisation", "asd_grain_magnetisation",
-    "asd_track_dims", "asd_track_set_init", "asd_track_get", "asd_get_counters", "asd_set_counters",
+    "asd_track_dims", "asd_track_set_init", "asd_track_get",
+    "asd_track_end_pass", "asd_track_begin_pass", "asd_track_read_scan", "asd_get_counters", "asd_set_counters",
     "asd_launch_count", "asd_last_error", "asd_version",
 ]
 
@@ -105,6 +106,10 @@ def load_library(build_if_missing: bool = True):
     L.asd_track_dims.argtypes = [C.c_void_p, ip64]
     L.asd_track_set_init.argtypes = [C.c_void_p, C.c_void_p, C.c_float]
     L.asd_track_get.argtypes = [C.c_void_p, dp, ip64]
+    L.asd_track_end_pass.argtypes = [C.c_void_p]
+    L.asd_track_begin_pass.argtypes = [C.c_void_p, C.c_int64]
+    L.asd_track_read_scan.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double,
+                                      C.c_int64, dp]
     L.asd_get_counters.argtypes = [C.c_void_p, ip64, ip64, ip64, ip64]
     L.asd_set_counters.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_int64]
     L.asd_launch_count.restype = C.c_int64
@@ -357,6 +362,20 @@ class Context:
         self._ck(self._L.asd_track_get(self._h, s.ctypes.data_as(C.POINTER(C.c_double)),
                                        cnt.ctypes.data_as(C.POINTER(C.c_int64))))
         return s, cnt
+
+    def track_end_pass(self):
+        self._ck(self._L.asd_track_end_pass(self._h))
+
+    def track_begin_pass(self, x0_new: int = 0):
+        self._ck(self._L.asd_track_begin_pass(self._h, C.c_int64(x0_new)))
+
+    def track_read_scan(self, y_r: float, sigma_x: float, sigma_y: float, x_first: float, x_step: float,
+                        count: int) -> np.ndarray:
+        out = np.zeros(int(count))
+        self._ck(self._L.asd_track_read_scan(self._h, C.c_double(y_r), C.c_double(sigma_x), C.c_double(sigma_y),
+                                             C.c_double(x_first), C.c_double(x_step), C.c_int64(count),
+                                             out.ctypes.data_as(C.POINTER(C.c_double))))
+        return out
 
     # ---- counters ----
     def counters(self):

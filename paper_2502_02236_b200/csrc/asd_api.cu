@@ -492,6 +492,32 @@ asd_status asd_track_get(asd_ctx* ctx, double* sum, int64_t* count) {
   return ASD_OK;
 }
 
+asd_status asd_track_end_pass(asd_ctx* ctx) {
+  CTX_OR_RETURN(ctx);
+  if (c.d.ell_width > 0) return fail(c, ASD_EUNSUPPORTED, "asd_track_end_pass: a general ELL table has no track");
+  return launch_track_end_pass(c);
+}
+
+asd_status asd_track_begin_pass(asd_ctx* ctx, int64_t x0_new) {
+  CTX_OR_RETURN(ctx);
+  if (c.d.ell_width > 0) return fail(c, ASD_EUNSUPPORTED, "asd_track_begin_pass: a general ELL table cannot follow the window");
+  if (c.d.pbc[0]) return fail(c, ASD_EUNSUPPORTED, "asd_track_begin_pass: window is periodic in x");
+  if (x0_new < 0 || x0_new + c.d.nx > c.d.track_nx) return fail(c, ASD_EINVAL, "asd_track_begin_pass: window must lie inside the track");
+  graphs_invalidate(c);
+  c.demag_age = 0;
+  return launch_track_begin_pass(c, x0_new);
+}
+
+asd_status asd_track_read_scan(asd_ctx* ctx, double y_r, double sigma_x, double sigma_y, double x_first, double x_step,
+                               int64_t count, double* out) {
+  CTX_OR_RETURN(ctx);
+  if (!out || count < 1) return fail(c, ASD_EINVAL, "asd_track_read_scan: out is NULL or count < 1");
+  if (!(sigma_x > 0.0) || !(sigma_y > 0.0) || !std::isfinite(sigma_x) || !std::isfinite(sigma_y) || !std::isfinite(y_r) ||
+      !std::isfinite(x_first) || !std::isfinite(x_step))
+    return fail(c, ASD_EINVAL, "asd_track_read_scan: footprint widths must be > 0 and positions finite");
+  return launch_track_read_scan(c, y_r, sigma_x, sigma_y, x_first, x_step, count, out);
+}
+
 asd_status asd_get_counters(const asd_ctx* ctx, int64_t* step, int64_t* shift, int64_t* x0, int64_t* pass) {
   if (!ctx) return ASD_EINVAL;
   if (step) *step = ctx->c.step;

@@ -139,9 +139,121 @@ __global__ void cell_frames_kernel(const float* __restrict__ init_mean, float* _
   f[10] = 0.0f; f[11] = 0.0f;
 }
 
+// End of a pass (reading T1): what the pass has written becomes what lies ahead of the next one.
+__global__ void track_commit_kernel(const double* __restrict__ out_sum, const long long* __restrict__ out_cnt,
+                                    float* __restrict__ init_mean, int64_t ncell) {
+  const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= ncell) return;
+  const long long n = out_cnt[c];
+  if (n == 0) return;                                   // never written: keeps its value
+  const double inv = 1.0 / (double)n;
+  init_mean[3 * c] = (float)(out_sum[3 * c] * inv);
+  init_mean[3 * c + 1] = (float)(out_sum[3 * c + 1] * inv);
+  init_mean[3 * c + 2] = (float)(out_sum[3 * c + 2] * inv);
+}
+
+// Read-back scan (reading T3): one CTA per reader position; thread t takes the (cx, cy) cell columns t, t + 256, ...
+// in ascending order and the partial sums meet in a fixed tree, so the result does not depend on scheduling.
+constexpr int kScanThreads = 256;
+__global__ void __launch_bounds__(kScanThreads)
+track_read_scan_kernel(const double* __restrict__ out_sum, const long long* __restrict__ out_cnt, int64_t ncx,
+                       int64_t ncy, int64_t ncz, int mx, int my, double y_r, double inv2sx, double inv2sy,
+                       double x_first, double x_step, double* __restrict__ out) {
+  __shared__ double s_num[kScanThreads], s_den[kScanThreads];
+  const double x_r = x_first + (double)blockIdx.x * x_step;
+  double num = 0.0, den = 0.0;
+  for (int64_t q = threadIdx.x; q < ncx * ncy; q += kScanThreads) {
+    const int64_t cx = q / ncy, cy = q - cx * ncy;
+    const double dx = ((double)cx + 0.5) * mx - x_r, dy = ((double)cy + 0.5) * my - y_r;
+    const double w = exp(-dx * dx * inv2sx - dy * dy * inv2sy);
+    if (w == 0.0) continue;
+    for (int64_t cz = 0; cz < ncz; ++cz) {
+      const int64_t c = q * ncz + cz;
+      num += w * out_sum[3 * c + 2];
+      den += w * (double)out_cnt[c];
+    }
+  }
+  s_num[threadIdx.x] = num; s_den[threadIdx.x] = den;
+  __syncthreads();
+  for (int off = kScanThreads / 2; off > 0; off >>= 1) {
+    if ((int)threadIdx.x < off) { s_num[threadIdx.x] += s_num[threadIdx.x + off]; s_den[threadIdx.x] += s_den[threadIdx.x + off]; }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) out[blockIdx.x] = s_den[0] > 0.0 ? s_num[0] / s_den[0] : 0.0;
+}
+
 inline unsigned nblocks(int64_t n, int threads) { return (unsigned)((n + threads - 1) / threads); }
 
+ShiftGeom shift_geom(const Ctx& c, int p) {
+  ShiftGeom g;
+  g.nx = c.d.nx; g.ny = c.d.ny; g.nz = c.d.nz; g.plane = c.plane; g.nyp = c.nyp; g.lead = c.lead;
+  g.mx = c.d.macro[0]; g.my = c.d.macro[1]; g.mz = c.d.macro[2];
+  g.x0 = c.x0; g.ncy = c.ncy; g.ncz = c.ncz; g.p = p;
+  return g;
+}
+
+PhiloxKey expand_key(uint64_t seed) {
+  PhiloxKey key;
+  uint32_t k0 = (uint32_t)(seed & 0xFFFFFFFFull), k1 = (uint32_t)(seed >> 32);
+  for (int r = 0; r < 10; ++r) { key.k0[r] = k0; key.k1[r] = k1; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
+  return key;
+}
+
+// Eq. (6) over window planes [0, p): the macrocells they touch accumulate the spins and the site counts.
+asd_status launch_coarse_grain(Ctx& c, const ShiftGeom& g) {
+  const Vec3Ptr S = c.S();
+  const int64_t cx_first = c.x0 / g.mx, cx_last = (c.x0 + g.p - 1) / g.mx;
+  const int n_cx = (int)(cx_last - cx_first + 1);
+  const int64_t warps = (int64_t)n_cx * c.ncy * c.ncz;
+  coarse_grain_outgoing<<<nblocks(warps * 32, 256), 256, 0, c.stream>>>(S.x, S.y, S.z, c.col, c.out_sum,
+                                                                       c.out_cnt, g, cx_first, n_cx);
+  ASD_LAUNCH_CHECK(c, "coarse_grain_outgoing");
+  return ASD_OK;
+}
+
 }  // namespace
+
+// asd_track_end_pass: all nx planes of the window -> track (Eq. (6)); written cells -> init_mean; frames rebuilt.
+asd_status launch_track_end_pass(Ctx& c) {
+  const asd_status st = launch_coarse_grain(c, shift_geom(c, c.d.nx));
+  if (st != ASD_OK) return st;
+  track_commit_kernel<<<nblocks(c.ncell, 128), 128, 0, c.stream>>>(c.out_sum, c.out_cnt, c.init_mean, c.ncell);
+  ASD_LAUNCH_CHECK(c, "track_commit");
+  return launch_cell_frames(c);
+}
+
+// asd_track_begin_pass: written store cleared; pass += 1; window at x0_new; every plane seeded from the track.
+asd_status launch_track_begin_pass(Ctx& c, int64_t x0_new) {
+  ASD_CUDA_TRY(c, cudaMemsetAsync(c.out_sum, 0, sizeof(double) * 3 * (size_t)c.ncell, c.stream));
+  ASD_CUDA_TRY(c, cudaMemsetAsync(c.out_cnt, 0, sizeof(long long) * (size_t)c.ncell, c.stream));
+  c.pass += 1;
+  c.x0 = x0_new;
+  ShiftGeom g = shift_geom(c, c.d.nx);
+  g.x0 = x0_new - c.d.nx;                               // seed_incoming's planes nx-p .. nx-1 "after a shift by p" = all of them
+  const Vec3Ptr S = c.S();
+  seed_incoming<<<nblocks((int64_t)c.d.nx * c.plane, 256), 256, 0, c.stream>>>(
+      S.x, S.y, S.z, c.col, c.cell_frame, g, expand_key(c.d.seed), (uint32_t)((uint64_t)c.pass & 0xFFFFFFFFull),
+      (uint32_t)((uint64_t)c.pass >> 32));
+  ASD_LAUNCH_CHECK(c, "seed_incoming(all planes)");
+  return ASD_OK;
+}
+
+// asd_track_read_scan: `count` reader positions into HOST out; synchronises.  The device results land in the
+// reduction scratch (4 * kMaxPartialBlocks doubles), so long scans go in chunks.
+asd_status launch_track_read_scan(Ctx& c, double y_r, double sigma_x, double sigma_y, double x_first, double x_step,
+                                  int64_t count, double* out_host) {
+  const int64_t chunk = 4 * (int64_t)kMaxPartialBlocks;
+  for (int64_t done = 0; done < count; done += chunk) {
+    const int64_t n = count - done < chunk ? count - done : chunk;
+    track_read_scan_kernel<<<(unsigned)n, kScanThreads, 0, c.stream>>>(
+        c.out_sum, c.out_cnt, c.ncx, c.ncy, c.ncz, c.d.macro[0], c.d.macro[1], y_r, 0.5 / (sigma_x * sigma_x),
+        0.5 / (sigma_y * sigma_y), x_first + (double)done * x_step, x_step, c.partials);
+    ASD_LAUNCH_CHECK(c, "track_read_scan");
+    ASD_CUDA_TRY(c, cudaMemcpyAsync(out_host + done, c.partials, sizeof(double) * (size_t)n, cudaMemcpyDeviceToHost, c.stream));
+    ASD_CUDA_TRY(c, cudaStreamSynchronize(c.stream));
+  }
+  return ASD_OK;
+}
 
 asd_status launch_cell_frames(Ctx& c) {
   cell_frames_kernel<<<nblocks(c.ncell, 128), 128, 0, c.stream>>>(c.init_mean, c.cell_frame, c.ncell);
@@ -150,18 +262,10 @@ asd_status launch_cell_frames(Ctx& c) {
 }
 
 asd_status launch_shift(Ctx& c, int32_t p) {
-  ShiftGeom g;
-  g.nx = c.d.nx; g.ny = c.d.ny; g.nz = c.d.nz; g.plane = c.plane; g.nyp = c.nyp; g.lead = c.lead;
+  const ShiftGeom g = shift_geom(c, p);
   const Vec3Ptr S = c.S(), St = c.St();
-  g.mx = c.d.macro[0]; g.my = c.d.macro[1]; g.mz = c.d.macro[2];
-  g.x0 = c.x0; g.ncy = c.ncy; g.ncz = c.ncz; g.p = p;
   // 1. outgoing slab -> macrocells
-  const int64_t cx_first = c.x0 / g.mx, cx_last = (c.x0 + p - 1) / g.mx;
-  const int n_cx = (int)(cx_last - cx_first + 1);
-  const int64_t warps = (int64_t)n_cx * c.ncy * c.ncz;
-  coarse_grain_outgoing<<<nblocks(warps * 32, 256), 256, 0, c.stream>>>(S.x, S.y, S.z, c.col, c.out_sum,
-                                                                       c.out_cnt, g, cx_first, n_cx);
-  ASD_LAUNCH_CHECK(c, "coarse_grain_outgoing");
+  { const asd_status st = launch_coarse_grain(c, g); if (st != ASD_OK) return st; }
   // 2. move into the scratch buffer
   // (padded planes: nz*nyp floats each, a multiple of 4; the pads move with their rows and stay zero)
   const int64_t planep = (int64_t)c.d.nz * c.nyp;
@@ -173,9 +277,7 @@ asd_status launch_shift(Ctx& c, int32_t p) {
     ASD_LAUNCH_CHECK(c, "move_planes");
   }
   // 3. incoming slab
-  PhiloxKey key;
-  uint32_t k0 = (uint32_t)(c.d.seed & 0xFFFFFFFFull), k1 = (uint32_t)(c.d.seed >> 32);
-  for (int r = 0; r < 10; ++r) { key.k0[r] = k0; key.k1[r] = k1; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
+  const PhiloxKey key = expand_key(c.d.seed);
   seed_incoming<<<nblocks((int64_t)p * c.plane, 256), 256, 0, c.stream>>>(
       St.x, St.y, St.z, c.col, c.cell_frame, g, key, (uint32_t)((uint64_t)c.pass & 0xFFFFFFFFull),
       (uint32_t)((uint64_t)c.pass >> 32));
