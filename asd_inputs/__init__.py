@@ -16,3 +16,5 @@ from .workloads import (  # noqa: F401
     make_config, small_film, ShiftSchedule, planes_for_shift, nrz_bits, field_scale_at,
 )
 from .two_track import TwoTrack, two_track_film, drive_pass, read_tracks  # noqa: F401
+from . import multiscale  # noqa: F401
+from .multiscale import Multiscale, multiscale_film, apply_multiscale, cell_grain_map  # noqa: F401

@@ -1,0 +1,153 @@
+"""Inputs for the multiscale window (Fig. 1): a central
+atomistic mesh with a micromagnetic LLG mesh either side, all moving along the granular track together.
+
+Input generation only -- no method arithmetic.  The micromagnetic cells ARE the track macrocells (DESIGN.md sec. 14,
+reading M1); their material parameters are the continuum limits of the atomistic ones (Eq. (9)-(10)):
+
+    M_S^0 = mu_s / V_atom                         one moment per lattice cell of the (Fe sub)lattice
+    K_0,g = k_u,g / V_atom                        per grain
+    A_0,a = sum_j J_j r_j,a^2 / (4 V_atom)        per axis a; simple cubic: J / 2a along every axis (Eq. (9)); with one J on
+                                                  all ten L1_0 neighbours: 3J / 2a in the plane (Eq. (10))
+    T_C,g ~ Normal(T_C, 5 %)                      per grain ("a normal distribution with standard deviation about T_C ...
+                                                  of 0.05 x T_C")
+
+A cell column (cx, cy) of the track belongs to the grain that owns most of its magnetic columns, and is empty when fewer
+than half of its columns are magnetic.
+"""
+from __future__ import annotations
+
+import math
+from dataclasses import dataclass
+from typing import List, Optional, Sequence, Tuple
+
+import numpy as np
+
+from . import workloads as wl
+
+
+@dataclass
+class Multiscale:
+    w: wl.Workload                 # the atomistic mesh (w.x0 = cells of the trailing mesh * mx)
+    mcx: Tuple[int, int]           # cells along x of the trailing / leading micromagnetic mesh
+    every: int                     # Heun steps per RK4 step (dt_mm = every * dt; 20 fs against 10 / 5 fs)
+    Ms0: float                     # A/m
+    A0: Tuple[float, float, float] # J/m along x, y, z
+    K0: np.ndarray                 # [G] J/m^3
+    Tc: np.ndarray                 # [G] K
+    cell_grain: np.ndarray         # [ncx, ncy] int32, -1 = empty cell column
+    T_mesh: List[np.ndarray]       # [2] per cell [mcx, ncy, ncz], K
+    B_mesh: List[np.ndarray]       # [2] per cell [mcx, ncy, ncz, 3], Tesla
+    spacing_m: Tuple[float, float, float]
+
+    def track_cells(self) -> Tuple[int, int, int]:
+        m = self.w.macro
+        return (-(-self.w.track_nx // m[0]), -(-self.w.ny // m[1]), -(-self.w.nz // m[2]))
+
+
+def cell_grain_map(grain_map: np.ndarray, macro: Sequence[int]) -> np.ndarray:
+    """[ncx, ncy] majority grain of every track cell column; -1 when fewer than half of its columns are magnetic."""
+    track_nx, ny = grain_map.shape
+    mx, my = int(macro[0]), int(macro[1])
+    ncx, ncy = -(-track_nx // mx), -(-ny // my)
+    out = -np.ones((ncx, ncy), dtype=np.int32)
+    for cx in range(ncx):
+        for cy in range(ncy):
+            blk = grain_map[cx * mx:(cx + 1) * mx, cy * my:(cy + 1) * my].reshape(-1)
+            mag = blk[blk >= 0]
+            if 2 * mag.size >= blk.size and mag.size > 0:
+                ids, cnt = np.unique(mag, return_counts=True)
+                out[cx, cy] = ids[np.argmax(cnt)]
+    return out
+
+
+def continuum_parameters(lattice: int, J: Sequence[float], spacing_nm: Sequence[float], mu_s: float, ku: np.ndarray):
+    """(M_S^0, (A_x, A_y, A_z), K_0[G]) of the lattice's long-wavelength limit."""
+    a = [s * 1e-9 for s in spacing_nm]
+    V = a[0] * a[1] * a[2]
+    if lattice == wl.SC:
+        offs = [((1, 0, 0), 0), ((-1, 0, 0), 0), ((0, 1, 0), 0), ((0, -1, 0), 0), ((0, 0, 1), 0), ((0, 0, -1), 0)]
+    else:
+        offs = [((1, 0, 0), 0), ((-1, 0, 0), 0), ((0, 1, 0), 0), ((0, -1, 0), 0), ((0, 0, 1), 1), ((0, 0, -1), 1),
+                ((1, 1, 0), 2), ((1, -1, 0), 2), ((-1, 1, 0), 2), ((-1, -1, 0), 2)]
+    A = [sum(J[sh] * (d[ax] * a[ax]) ** 2 for d, sh in offs) / (4.0 * V) for ax in range(3)]
+    return mu_s / V, tuple(A), np.asarray(ku, dtype=np.float64) / V
+
+
+def multiscale_film(lattice: int = wl.SC, atom_cells: int = 48, mesh_cells: Tuple[int, int] = (48, 48),
+                    width_nm: float = 60.0, nz: int = 27, extra_cells: int = 12, every: int = 20,
+                    macro: Optional[Sequence[int]] = None, pitch_nm: float = 8.0, boundary_nm: float = 1.0,
+                    fwhm_nm: float = 60.0, t_peak: float = 800.0, t_ambient: float = 300.0, bz: float = 0.8,
+                    tc_mean: Optional[float] = None, tc_rel_sigma: float = 0.05, lam: float = 0.1, dt: float = 1e-15,
+                    grain_seed: int = 2, seed: int = 1, tilt_deg: float = 0.0) -> Multiscale:
+    """[trailing mesh | atomistic mesh | leading mesh] over a granular track.  Defaults follow the paper's split of a
+    window into three equal parts ("a 100 nm long atomistic simulation region and two 100 nm long micromagnetic
+    simulation regions") on the cfg3 lattice; the parity tests shrink every length."""
+    spacing = wl.A_SC if lattice == wl.SC else wl.A_L10
+    J = wl.J_SC if lattice == wl.SC else wl.J_L10
+    if macro is None:
+        macro = (7, 7, 7) if lattice == wl.SC else (7, 7, 5)
+    mx, my, mz = (int(v) for v in macro)
+    nx = atom_cells * mx
+    ny = int(round(width_nm / spacing[1] / 4.0)) * 4
+    x0 = mesh_cells[0] * mx
+    track_nx = x0 + nx + (mesh_cells[1] + extra_cells) * mx
+    gm, ku, axis = wl.voronoi_grain_map(track_nx, ny, spacing[0], spacing[1], pitch_nm=pitch_nm,
+                                        boundary_nm=boundary_nm, seed=grain_seed)
+    G = ku.shape[0]
+    mu_s = 3.23 * wl.MU_B
+    Ms0, A0, K0 = continuum_parameters(lattice, J, spacing, mu_s, ku)
+    if tc_mean is None:
+        # Eq. (8) with the paper's mean-field correction factors: T_C = eps z J / 3 k_B for a single J;
+        # per-shell J: z J -> sum_j J_j
+        eps = 0.72 if lattice == wl.SC else 0.78
+        zJ = 6 * J[0] if lattice == wl.SC else 4 * J[0] + 2 * J[1] + 4 * J[2]
+        tc_mean = eps * zJ / (3.0 * wl.K_B)
+    rng = np.random.default_rng(grain_seed + 1000)
+    Tc = tc_mean * (1.0 + tc_rel_sigma * rng.standard_normal(G))
+    # profiles centred on the window [trailing mesh | atoms | leading mesh]; the spot sits on the atomistic mesh
+    xc_nm = (x0 + 0.5 * nx) * spacing[0]
+    yc_nm = 0.5 * ny * spacing[1]
+
+    def temperature(x_nm, y_nm):
+        r2 = (x_nm - xc_nm) ** 2 + (y_nm - yc_nm) ** 2
+        return t_ambient + (t_peak - t_ambient) * np.exp(-4.0 * math.log(2.0) * r2 / fwhm_nm ** 2)
+    xs = (x0 + np.arange(nx) + 0.5) * spacing[0]
+    ys = (np.arange(ny) + 0.5) * spacing[1]
+    T2 = temperature(xs[:, None], ys[None, :])
+    N = nx * ny * nz
+    T = np.broadcast_to(T2[:, None, :], (nx, nz, ny)).astype(np.float32).reshape(-1).copy()
+    mag = np.broadcast_to((gm[x0:x0 + nx, :] >= 0)[:, None, :], (nx, nz, ny)).reshape(-1)
+    z = np.zeros(N, dtype=np.float32)
+    w = wl.Workload(name=f"multiscale_{'sc' if lattice == wl.SC else 'l10'}_{mesh_cells[0]}c+{nx}x{ny}x{nz}+{mesh_cells[1]}c",
+                    lattice=lattice, nx=nx, ny=ny, nz=nz, pbc=(0, 0, 0), mu_s=mu_s, lam=lam, gamma=wl.GAMMA_E, dt=dt,
+                    J=J, spacing_nm=spacing, track_nx=track_nx, x0=x0, grain_map=gm, grain_ku=ku, grain_axis=axis,
+                    macro=(mx, my, mz), seed=seed, T=T, Bx=z.copy(), By=z.copy(), Bz=np.full(N, bz, dtype=np.float32),
+                    sx=z.copy(), sy=z.copy(), sz=mag.astype(np.float32), steps=0, shift_every=0, bit_steps=0,
+                    notes="multiscale window: micromagnetic | atomistic | micromagnetic (Fig. 1)")
+    if tilt_deg > 0.0:
+        sx, sy, sz = wl.tilted_spins(N, tilt_deg, seed=seed + 100)
+        w.sx, w.sy, w.sz = (sx * mag).astype(np.float32), (sy * mag).astype(np.float32), (sz * mag).astype(np.float32)
+    ncy, ncz = -(-ny // my), -(-nz // mz)
+    cyc = (np.arange(ncy) + 0.5) * my * spacing[1]
+    T_mesh, B_mesh = [], []
+    for side, c0 in ((0, 0), (1, (x0 + nx) // mx)):
+        cxc = (c0 + np.arange(mesh_cells[side]) + 0.5) * mx * spacing[0]
+        Tm = temperature(cxc[:, None], cyc[None, :])
+        T_mesh.append(np.broadcast_to(Tm[:, :, None], (mesh_cells[side], ncy, ncz)).copy())
+        Bm = np.zeros((mesh_cells[side], ncy, ncz, 3))
+        Bm[..., 2] = bz
+        B_mesh.append(Bm)
+    return Multiscale(w=w, mcx=(int(mesh_cells[0]), int(mesh_cells[1])), every=every, Ms0=Ms0, A0=A0, K0=K0, Tc=Tc,
+                      cell_grain=cell_grain_map(gm, (mx, my, mz)), T_mesh=T_mesh, B_mesh=B_mesh,
+                      spacing_m=tuple(s * 1e-9 for s in spacing))
+
+
+def apply_multiscale(sim, ms: Multiscale):
+    """Switches the micromagnetic meshes on in `sim` (the oracle or the CUDA context: same method names) and hands them
+    their temperature and field profiles."""
+    st = sim.mm_enable(ms.mcx, ms.every, ms.Ms0, ms.A0, ms.K0, ms.Tc, ms.cell_grain, ms.spacing_m)
+    if st not in (None, 0):
+        raise ValueError(f"mm_enable rejected the description (status {st})")
+    for side in (0, 1):
+        B = ms.B_mesh[side]
+        sim.mm_set_fields(side, ms.T_mesh[side], B[..., 0], B[..., 1], B[..., 2])

@@ -33,6 +33,8 @@ class TwoTrack:
     batch: int                         # Heun steps per asd_step_heun call (field scale constant inside a batch)
     reader_sigma: Tuple[float, float]  # Gaussian reader footprint (along, across the track), in sites
     spot_plane: float                  # window plane under the centre of the laser spot
+    write_offset: float = 0.0          # planes between the spot centre and the trailing edge of the region above T_C,
+                                       # where the grains freeze: the head polarity follows the bit under THAT point
 
     @property
     def n_periods(self) -> int:
@@ -46,12 +48,20 @@ class TwoTrack:
 
     def bit_at_plane(self, p: int, gx: float) -> float:
         """Polarity the head writes while the spot centre is over global plane gx."""
-        b = min(max(int(gx // self.bit_planes), 0), len(self.bits[p]) - 1)
+        b = min(max(int((gx - self.write_offset) // self.bit_planes), 0), len(self.bits[p]) - 1)
         return float(self.bits[p][b])
 
     def bit_centres(self) -> np.ndarray:
         """Global plane coordinate of every bit centre."""
         return (np.arange(len(self.bits[0])) + 0.5) * self.bit_planes
+
+    def written_bits(self, periods: Optional[int] = None) -> np.ndarray:
+        """Indices of the bits whose whole length the freezing point has swept in a pass of `periods` shift periods."""
+        periods = self.n_periods if periods is None else periods
+        travel = sum(wl.planes_for_shift(q, self.w.spacing_nm[0]) for q in range(1, periods + 1))
+        lo, hi = self.spot_plane - self.write_offset, self.spot_plane - self.write_offset + travel
+        b = np.arange(len(self.bits[0]))
+        return b[(b * self.bit_planes >= lo) & ((b + 1) * self.bit_planes <= hi)]
 
 
 def two_track_film(lattice: int = wl.SC, length_nm: float = 120.0, width_nm: float = 80.0, nz: int = 27,
@@ -94,7 +104,7 @@ def two_track_film(lattice: int = wl.SC, length_nm: float = 120.0, width_nm: flo
     sigma = (0.5 * bit_nm / 2.355 / spacing[0], bit_width_nm / 2.355 / spacing[1])
     return TwoTrack(w=w, T_pass=T_pass, bits=bits, track_y=(yc_nm[0] / spacing[1], yc_nm[1] / spacing[1]),
                     bit_planes=bit_planes, shift_every=shift_every, batch=batch, reader_sigma=sigma,
-                    spot_plane=0.5 * nx)
+                    spot_plane=0.5 * nx, write_offset=0.5 * bit_width_nm / spacing[0])
 
 
 def drive_pass(sim, tt: TwoTrack, p: int, set_temperature: Callable, periods: Optional[int] = None,

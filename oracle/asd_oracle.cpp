@@ -17,6 +17,9 @@
 //   * atomistic->macrocell transfer Eq. (6), P:64-66 -> orc_shift_window() outgoing part
 //   * macrocell->atomistic cone thermalisation, P:68 -> seed_site()  (S:S3 reading)
 //   * Philox4x32-10 (Salmon et al., SC'11, public definition) -> philox4x32_10()
+//   * multiscale window: micromagnetic LLG meshes either side of the atomistic mesh, Eq. (4)-(5), temperature scalings
+//     m_e(T), A = A0 m_e^2, K = K0 m_e^3, alpha = lambda (1 - T/3T_C), RK4, two-way exchange coupling
+//     across the mesh boundaries, transfers on a shift (Fig. 1) -> the "Multiscale window" section (S:8(f) item 3)
 //   * passes over the track (two parallel tracks) -> orc_track_end_pass(), orc_track_begin_pass();
 //     Gaussian-footprint read-back standing in for the TMR head -> orc_track_read_scan()  (S:8(f) item 4)
 //
@@ -151,6 +154,23 @@ struct Oracle {
   int demag_every = 0;             // 0: recomputed in every stage; P >= 1: from S at every P-th step, held in between (D3)
   int64_t demag_age = 0;           // steps since the held field was invalidated (enable, set_every, shift, set_spins)
   std::vector<double> demag_hold;  // the held per-macrocell field
+  // multiscale window (S:8(f) item 3): micromagnetic LLG meshes either side of the atomistic
+  // mesh; off unless orc_mm_enable was called.  Mesh cells ARE track macrocells; side 0 = trailing (lower x), 1 = leading.
+  bool mm = false;
+  struct MicroMesh {
+    int mcx = 0;                          // cells along x
+    std::vector<double> m;                // [mcx*ncy*ncz*3] unit magnetisation direction; 0 for an empty cell
+    std::vector<double> T, Bx, By, Bz;    // per cell, window-fixed profiles
+    std::vector<double> me, alpha;        // m_e(T) and alpha(T) per cell
+  } mesh[2];
+  double mm_Ms0 = 0, mm_A0[3] = {0, 0, 0};  // M_S^0 [A/m]; A_0 [J/m] along x, y, z (one value three times = the paper's scalar A)
+  std::vector<double> mm_K0, mm_Tc;       // per grain: K_0 [J/m^3], T_C [K]
+  std::vector<int32_t> mm_grain;          // [ncx*ncy] grain id of a track cell column (cx, cy), -1 = empty
+  double mm_cell[3] = {0, 0, 0};          // cell edge lengths, metres
+  int mm_every = 1;                       // Heun steps per RK4 step: dt_mm = mm_every * dt
+  int64_t mm_age = 0;                     // Heun steps since the last (re)start of the exchange cadence
+  std::vector<double> mm_ghost[2];        // [ncy*ncz*3] direction of the mesh cells that touch the atomistic mesh (held)
+  std::vector<double> mm_avg[2];          // [ncy*ncz*3] direction of the average atomistic spin in the stencil cell (held)
 
   int64_t site(int i, int k, int j) const { return ((int64_t)i * nz + k) * ny + j; }
   int32_t grain_of(int i, int j) const { return grain_map[(size_t)((x0 + i) * ny + j)]; }
@@ -202,6 +222,18 @@ void exchange_sum(const Oracle& o, const double* X0, const double* X1, const dou
   const int noff = (o.lattice == 0) ? 6 : 10;
   for (int s = 0; s < noff; ++s) {
     int ii = i + offs[s].dx, jj = j + offs[s].dy, kk = k + offs[s].dz;
+    if (o.mm && (ii == -1 || ii == o.nx)) {
+      // Across the mesh boundary: "For the contribution from the micromagnetic region the respective
+      // magnetization direction is used directly" -- the neighbour spin of Eq. (2) is the direction m of the
+      // micromagnetic cell that holds the neighbour position (as captured at the last exchange, reading M9).
+      if (jj < 0 || jj >= o.ny || kk < 0 || kk >= o.nz) continue;
+      const int32_t gn = o.grain_map[(size_t)((o.x0 + ii) * o.ny + jj)];
+      if (gn < 0 || gn != g) continue;                        // exchange-decoupled grains
+      const double* mg = &o.mm_ghost[ii < 0 ? 0 : 1][3 * ((size_t)(jj / o.macro[1]) * o.ncz + kk / o.macro[2])];
+      const double Jij = o.J[offs[s].shell];
+      e[0] += Jij * mg[0]; e[1] += Jij * mg[1]; e[2] += Jij * mg[2];
+      continue;
+    }
     if (!wrap(ii, o.nx, o.pbc[0])) continue;
     if (!wrap(jj, o.ny, o.pbc[1])) continue;
     if (!wrap(kk, o.nz, o.pbc[2])) continue;
@@ -371,8 +403,10 @@ inline int thread_count(const Oracle& o) {
 // One stochastic Heun step, Jacobi order (S:O4):
 // 1 draw xi_i; 2 k1 = f(S, B(S)); 3 S~ = (S + dt k1)/|.|; 4 k2 = f(S~, B(S~)) with the SAME xi_i;
 // 5 S <- (S + dt/2 (k1+k2))/|.|; 6 n <- n+1.  Vacant sites are skipped and stay 0.
+void mm_before_heun_step(Oracle& o);
 void heun_step(Oracle& o) {
   const int64_t N = o.N;
+  mm_before_heun_step(o);
   std::vector<double> xi(3 * (size_t)N, 0.0), k1(3 * (size_t)N, 0.0);
   std::vector<double> tx((size_t)N, 0.0), ty((size_t)N, 0.0), tz((size_t)N, 0.0);
   const int nx = o.nx, ny = o.ny, nz = o.nz;
@@ -431,9 +465,14 @@ void heun_step(Oracle& o) {
 // macrocell, m = min(1,|v|), n^ = v/|v| (z^ if v = 0), theta = theta_max(m) u0, phi = 2 pi u1
 // (Philox stream 1, counter n := pass), S = sin(theta)cos(phi) e1 + sin(theta)sin(phi) e2 + cos(theta) n^,
 // e1 = normalise(n^ x x^) (n^ x y^ if |n^_x| > 0.9), e2 = n^ x e1.
+void seed_site_about(const Oracle& o, int64_t gx, int k, int j, const double v[3], double S[3]);
 void seed_site(const Oracle& o, int64_t gx, int k, int j, double S[3]) {
   const int64_t c = o.cell_of(gx, j, k);
-  const double v0 = o.init_mean[3 * c], v1 = o.init_mean[3 * c + 1], v2 = o.init_mean[3 * c + 2];
+  seed_site_about(o, gx, k, j, &o.init_mean[3 * c], S);
+}
+// v = M / M_S^0 of the cell the site is generated from (track cell, or micromagnetic cell: m_e(T) m)
+void seed_site_about(const Oracle& o, int64_t gx, int k, int j, const double v[3], double S[3]) {
+  const double v0 = v[0], v1 = v[1], v2 = v[2];
   const double vn = std::sqrt(v0 * v0 + v1 * v1 + v2 * v2);
   const double m = std::fmin(1.0, vn);
   double n[3] = {0.0, 0.0, 1.0};
@@ -455,6 +494,287 @@ void seed_site(const Oracle& o, int64_t gx, int k, int j, double S[3]) {
   const double phi = 2.0 * kPi * uniform_from_u32(r[1]);
   const double st = std::sin(theta), ct = std::cos(theta), cp = std::cos(phi), sp = std::sin(phi);
   for (int a = 0; a < 3; ++a) S[a] = st * cp * e1[a] + st * sp * e2[a] + ct * n[a];
+}
+
+// ============================================================================================================
+// Multiscale window: micromagnetic LLG meshes (S:8(f) item 3).  Readings M1-M10 of DESIGN.md sec. 14.
+// ============================================================================================================
+// Langevin function B(x) = coth(x) - 1/x, with its series where the difference cancels.
+double langevin(double x) {
+  if (std::fabs(x) < 1e-3) return x / 3.0 - x * x * x / 45.0 + 2.0 * x * x * x * x * x / 945.0;
+  return 1.0 / std::tanh(x) - 1.0 / x;
+}
+// Equilibrium magnetisation scaling m_e(T) = B[m_e 3 T_C / T + mu_S B_ext / (k_B T)]  (B_ext = mu_0 H_ext, Tesla):
+// the largest root in [0, 1].  g(m) = B(beta m + h) - m is concave on m > 0 with g(1) < 0, so that root is unique
+// whenever g is positive just above 0 (h > 0, or h = 0 and T < T_C); otherwise m_e = 0.
+double m_e_of(double T, double Tc, double mu_s_Bext) {
+  if (!(T > 0.0)) return 1.0;
+  const double beta = 3.0 * Tc / T, h = mu_s_Bext / (kBoltzmann * T);
+  double lo = (h > 0.0) ? 0.0 : 1e-9, hi = 1.0;
+  if (!(langevin(beta * lo + h) - lo > 0.0)) return 0.0;
+  for (int it = 0; it < 200; ++it) {
+    const double mid = 0.5 * (lo + hi);
+    if (langevin(beta * mid + h) - mid > 0.0) lo = mid; else hi = mid;
+  }
+  return 0.5 * (lo + hi);
+}
+
+inline int64_t mm_cx0(const Oracle& o, int side) {              // global x index of the mesh's first cell column
+  return side == 0 ? o.x0 / o.macro[0] - o.mesh[0].mcx : (o.x0 + o.nx) / o.macro[0];
+}
+inline size_t mm_idx(const Oracle& o, int a, int b, int c) { return ((size_t)a * o.ncy + b) * o.ncz + c; }
+inline int32_t mm_grain_of(const Oracle& o, int64_t cx, int b) {
+  if (cx < 0 || cx >= o.ncx || b < 0 || b >= o.ncy) return -1;
+  return o.mm_grain[(size_t)(cx * o.ncy + b)];
+}
+// direction of the frozen track in cell (cx, b, c): what the window has written there, else what lies ahead
+bool track_direction(const Oracle& o, int64_t cx, int b, int c, double n[3]) {
+  const size_t t = (size_t)((cx * o.ncy + b) * o.ncz + c);
+  const double* v = o.out_cnt[t] > 0 ? &o.out_sum[3 * t] : &o.init_mean[3 * t];
+  const double vn = std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+  if (!(vn > 0.0)) return false;
+  n[0] = v[0] / vn; n[1] = v[1] / vn; n[2] = v[2] / vn;
+  return true;
+}
+
+// M2, M3: per-cell m_e(T) and alpha(T) = lambda (1 - T / 3 T_C) (held at its T = T_C value above T_C)
+void mm_refresh_params(Oracle& o) {
+  for (int side = 0; side < 2; ++side) {
+    Oracle::MicroMesh& M = o.mesh[side];
+    const int64_t cx0 = mm_cx0(o, side);
+    for (int a = 0; a < M.mcx; ++a)
+      for (int b = 0; b < o.ncy; ++b)
+        for (int c = 0; c < o.ncz; ++c) {
+          const size_t q = mm_idx(o, a, b, c);
+          const int32_t g = mm_grain_of(o, cx0 + a, b);
+          if (g < 0) { M.me[q] = 0.0; M.alpha[q] = 0.0; continue; }
+          const double Bext = std::fabs(o.scale) * std::sqrt(M.Bx[q] * M.Bx[q] + M.By[q] * M.By[q] + M.Bz[q] * M.Bz[q]);
+          M.me[q] = m_e_of(M.T[q], o.mm_Tc[g], o.mu_s * Bext);
+          M.alpha[q] = o.lambda * (1.0 - std::fmin(M.T[q], o.mm_Tc[g]) / (3.0 * o.mm_Tc[g]));
+        }
+  }
+}
+
+// M9: the two-way exchange of boundary data.  mm_avg = direction of the average atomistic spin in the stencil cell next
+// to each mesh; mm_ghost = direction of the mesh cells next to the atomistic mesh.
+void mm_exchange(Oracle& o) {
+  const int mx = o.macro[0], my = o.macro[1], mz = o.macro[2];
+  for (int side = 0; side < 2; ++side) {
+    const int i_lo = side == 0 ? 0 : o.nx - mx;
+    for (int b = 0; b < o.ncy; ++b)
+      for (int c = 0; c < o.ncz; ++c) {
+        double s0 = 0, s1 = 0, s2 = 0;
+        for (int i = i_lo; i < i_lo + mx; ++i)
+          for (int k = c * mz; k < std::min((c + 1) * mz, o.nz); ++k)
+            for (int j = b * my; j < std::min((b + 1) * my, o.ny); ++j) {
+              if (o.grain_of(i, j) < 0) continue;
+              const int64_t l = o.site(i, k, j);
+              s0 += o.sx[l]; s1 += o.sy[l]; s2 += o.sz[l];
+            }
+        const double n = std::sqrt(s0 * s0 + s1 * s1 + s2 * s2);
+        double* av = &o.mm_avg[side][3 * ((size_t)b * o.ncz + c)];
+        av[0] = n > 0.0 ? s0 / n : 0.0; av[1] = n > 0.0 ? s1 / n : 0.0; av[2] = n > 0.0 ? s2 / n : 0.0;
+        const Oracle::MicroMesh& M = o.mesh[side];
+        const size_t q = mm_idx(o, side == 0 ? M.mcx - 1 : 0, b, c);
+        double* gh = &o.mm_ghost[side][3 * ((size_t)b * o.ncz + c)];
+        gh[0] = M.m[3 * q]; gh[1] = M.m[3 * q + 1]; gh[2] = M.m[3 * q + 2];
+      }
+  }
+}
+
+// Effective field of mesh cell (a, b, c), Tesla, for mesh configuration X (M4-M6):
+//   B = (2 A(T) / M_S(T)) lap(m) + (2 K(T) / M_S(T)) (m.e) e + s B_app         Eq. (4), (5) in Tesla
+//   A(T) = A_0 m_e^2, K(T) = K_0 m_e^3, M_S(T) = M_S^0 m_e  =>  2 A_0 m_e / M_S^0  and  2 K_0 m_e^2 / M_S^0
+//   lap(m) by the 6-neighbour stencil: sum over existing neighbours n of the same grain of (m_n - m) / d_n^2.
+// A neighbour beyond the mesh is the stencil cell of the atomistic mesh (its average spin direction) on one
+// side and the frozen track cell on the other ("the ends of the simulation window are exchange coupled to the track").
+void mm_field(const Oracle& o, int side, const std::vector<double>& X, int a, int b, int c, double B[3]) {
+  const Oracle::MicroMesh& M = o.mesh[side];
+  const size_t q = mm_idx(o, a, b, c);
+  const int64_t cx0 = mm_cx0(o, side);
+  const int32_t g = mm_grain_of(o, cx0 + a, b);
+  B[0] = B[1] = B[2] = 0.0;
+  if (g < 0 || !(M.me[q] > 0.0)) return;
+  const double m[3] = {X[3 * q], X[3 * q + 1], X[3 * q + 2]};
+  auto add = [&](const double* n, int axis) {
+    const double pref = 2.0 * o.mm_A0[axis] * M.me[q] / o.mm_Ms0, d = o.mm_cell[axis];
+    for (int t = 0; t < 3; ++t) B[t] += pref * (n[t] - m[t]) / (d * d);
+  };
+  // x neighbours
+  for (int dir = -1; dir <= 1; dir += 2) {
+    const int a2 = a + dir;
+    if (mm_grain_of(o, cx0 + a2, b) != g) continue;
+    if (a2 >= 0 && a2 < M.mcx) { add(&X[3 * mm_idx(o, a2, b, c)], 0); continue; }
+    const bool towards_atoms = (side == 0) == (dir > 0);
+    if (towards_atoms) {
+      const double* av = &o.mm_avg[side][3 * ((size_t)b * o.ncz + c)];
+      if (av[0] != 0.0 || av[1] != 0.0 || av[2] != 0.0) add(av, 0);
+    } else {
+      double n[3];
+      if (track_direction(o, cx0 + a2, b, c, n)) add(n, 0);
+    }
+  }
+  for (int dir = -1; dir <= 1; dir += 2) {          // y neighbours: the next cell column across the track
+    const int b2 = b + dir;
+    if (b2 < 0 || b2 >= o.ncy || mm_grain_of(o, cx0 + a, b2) != g) continue;
+    add(&X[3 * mm_idx(o, a, b2, c)], 1);
+  }
+  for (int dir = -1; dir <= 1; dir += 2) {          // z neighbours: same column, same grain
+    const int c2 = c + dir;
+    if (c2 < 0 || c2 >= o.ncz) continue;
+    add(&X[3 * mm_idx(o, a, b, c2)], 2);
+  }
+  const double* e = &o.axis[3 * g];
+  const double ca = 2.0 * o.mm_K0[g] * M.me[q] * M.me[q] / o.mm_Ms0 * (m[0] * e[0] + m[1] * e[1] + m[2] * e[2]);
+  for (int t = 0; t < 3; ++t) B[t] += ca * e[t];
+  B[0] += o.scale * M.Bx[q]; B[1] += o.scale * M.By[q]; B[2] += o.scale * M.Bz[q];
+}
+
+// dm/dt of every cell of one mesh: Eq. (1) without the stochastic field, damping alpha(T), LL form as llg_rhs.
+void mm_rhs(const Oracle& o, int side, const std::vector<double>& X, std::vector<double>& f) {
+  const Oracle::MicroMesh& M = o.mesh[side];
+  f.assign(X.size(), 0.0);
+  for (int a = 0; a < M.mcx; ++a)
+    for (int b = 0; b < o.ncy; ++b)
+      for (int c = 0; c < o.ncz; ++c) {
+        const size_t q = mm_idx(o, a, b, c);
+        double B[3];
+        mm_field(o, side, X, a, b, c, B);
+        const double* S = &X[3 * q];
+        const double a0 = S[1] * B[2] - S[2] * B[1], a1 = S[2] * B[0] - S[0] * B[2], a2 = S[0] * B[1] - S[1] * B[0];
+        const double b0 = S[1] * a2 - S[2] * a1, b1 = S[2] * a0 - S[0] * a2, b2 = S[0] * a1 - S[1] * a0;
+        const double al = M.alpha[q], cf = -o.gamma / (1.0 + al * al);
+        f[3 * q] = cf * (a0 + al * b0); f[3 * q + 1] = cf * (a1 + al * b1); f[3 * q + 2] = cf * (a2 + al * b2);
+      }
+}
+
+// M7: one classical RK4 step of length h on both meshes, boundary data held; |m| = 1 restored after the step.
+void mm_rk4_step(Oracle& o, double h) {
+  for (int side = 0; side < 2; ++side) {
+    std::vector<double>& m = o.mesh[side].m;
+    std::vector<double> k1, k2, k3, k4, y(m.size());
+    mm_rhs(o, side, m, k1);
+    for (size_t t = 0; t < m.size(); ++t) y[t] = m[t] + 0.5 * h * k1[t];
+    mm_rhs(o, side, y, k2);
+    for (size_t t = 0; t < m.size(); ++t) y[t] = m[t] + 0.5 * h * k2[t];
+    mm_rhs(o, side, y, k3);
+    for (size_t t = 0; t < m.size(); ++t) y[t] = m[t] + h * k3[t];
+    mm_rhs(o, side, y, k4);
+    for (size_t q = 0; q < m.size() / 3; ++q) {
+      double v[3];
+      for (int t = 0; t < 3; ++t)
+        v[t] = m[3 * q + t] + h / 6.0 * (k1[3 * q + t] + 2.0 * k2[3 * q + t] + 2.0 * k3[3 * q + t] + k4[3 * q + t]);
+      const double n = std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+      for (int t = 0; t < 3; ++t) m[3 * q + t] = n > 0.0 ? v[t] / n : 0.0;
+    }
+  }
+}
+
+// M9: called at the top of every Heun step.  Every mm_every-th step the meshes trade boundary data with the atomistic
+// mesh (both directions, from the configurations at that instant) and advance by one RK4 step of mm_every * dt; the
+// atomistic mesh then takes its mm_every Heun steps against the held mesh directions.
+void mm_before_heun_step(Oracle& o) {
+  if (!o.mm) return;
+  if (o.mm_age % o.mm_every == 0) {
+    mm_exchange(o);
+    mm_refresh_params(o);
+    mm_rk4_step(o, o.mm_every * o.dt);
+  }
+  o.mm_age += 1;
+}
+
+// number of magnetic sites of track cell (cx, b, c)
+int64_t cell_site_count(const Oracle& o, int64_t cx, int b, int c) {
+  int64_t n = 0;
+  for (int64_t gx = cx * o.macro[0]; gx < std::min<int64_t>((cx + 1) * o.macro[0], o.track_nx); ++gx)
+    for (int j = b * o.macro[1]; j < std::min((b + 1) * o.macro[1], o.ny); ++j)
+      if (o.grain_map[(size_t)(gx * o.ny + j)] >= 0) n += std::min((c + 1) * o.macro[2], o.nz) - c * o.macro[2];
+  return n;
+}
+
+// M10: the window moves by pc whole cells ("in steps set by the track discretization cellsize").
+//   trailing mesh -> track (as M / M_S^0 = m_e m on the cell's magnetic sites);  outgoing atomistic planes -> the
+//   trailing mesh by Eq. (6) ("averaging", Fig. 1);  incoming atomistic planes <- the leading mesh by the cone
+//   thermalisation about m with magnitude m_e ("thermalization", Fig. 1);  leading mesh <- the track ahead.
+void seed_plane_from(Oracle& o, int i, int64_t gx, const Oracle::MicroMesh* from, int a_from);
+int mm_shift(Oracle& o, int p) {
+  const int mx = o.macro[0];
+  if (p % mx != 0) return 1;
+  const int pc = p / mx;
+  Oracle::MicroMesh &L = o.mesh[0], &R = o.mesh[1];
+  if (pc > L.mcx || pc > R.mcx) return 1;
+  if (mm_cx0(o, 1) + R.mcx + pc > o.ncx) return 1;
+  const int64_t cxL = mm_cx0(o, 0), cxA = o.x0 / mx, cxR = mm_cx0(o, 1);
+  // 1. trailing mesh columns a < pc -> track
+  for (int a = 0; a < pc; ++a)
+    for (int b = 0; b < o.ncy; ++b)
+      for (int c = 0; c < o.ncz; ++c) {
+        if (mm_grain_of(o, cxL + a, b) < 0) continue;
+        const size_t q = mm_idx(o, a, b, c);
+        const size_t t = (size_t)(((cxL + a) * o.ncy + b) * o.ncz + c);
+        const int64_t n = cell_site_count(o, cxL + a, b, c);
+        for (int u = 0; u < 3; ++u) o.out_sum[3 * t + u] += L.me[q] * L.m[3 * q + u] * (double)n;
+        o.out_cnt[t] += n;
+      }
+  // 2. trailing mesh moves; its new columns are the Eq. (6) averages of the outgoing atomistic cells (direction)
+  std::vector<double> newL((size_t)pc * o.ncy * o.ncz * 3, 0.0);
+  for (int a = 0; a < pc; ++a)
+    for (int b = 0; b < o.ncy; ++b)
+      for (int c = 0; c < o.ncz; ++c) {
+        if (mm_grain_of(o, cxA + a, b) < 0) continue;
+        double s[3] = {0, 0, 0};
+        for (int i = a * mx; i < (a + 1) * mx; ++i)
+          for (int k = c * o.macro[2]; k < std::min((c + 1) * o.macro[2], o.nz); ++k)
+            for (int j = b * o.macro[1]; j < std::min((b + 1) * o.macro[1], o.ny); ++j) {
+              if (o.grain_of(i, j) < 0) continue;
+              const int64_t l = o.site(i, k, j);
+              s[0] += o.sx[l]; s[1] += o.sy[l]; s[2] += o.sz[l];
+            }
+        const double n = std::sqrt(s[0] * s[0] + s[1] * s[1] + s[2] * s[2]);
+        double* d = &newL[3 * mm_idx(o, a, b, c)];
+        if (n > 0.0) { d[0] = s[0] / n; d[1] = s[1] / n; d[2] = s[2] / n; } else { d[2] = 1.0; }
+      }
+  const size_t col = (size_t)o.ncy * o.ncz * 3;
+  for (int a = 0; a + pc < L.mcx; ++a) std::memcpy(&L.m[a * col], &L.m[(a + pc) * col], sizeof(double) * col);
+  for (int a = 0; a < pc; ++a) std::memcpy(&L.m[(L.mcx - pc + a) * col], &newL[a * col], sizeof(double) * col);
+  // 3. atomistic planes move; the incoming ones are generated from the leading mesh's first pc columns
+  for (int i = 0; i + p < o.nx; ++i)
+    for (int k = 0; k < o.nz; ++k)
+      for (int j = 0; j < o.ny; ++j) {
+        const int64_t l = o.site(i, k, j), s = o.site(i + p, k, j);
+        o.sx[l] = o.sx[s]; o.sy[l] = o.sy[s]; o.sz[l] = o.sz[s];
+      }
+  for (int i = o.nx - p; i < o.nx; ++i) seed_plane_from(o, i, o.x0 + p + i, &R, (i - (o.nx - p)) / mx);
+  // 4. leading mesh moves; its new columns are the track ahead (direction)
+  for (int a = 0; a + pc < R.mcx; ++a) std::memcpy(&R.m[a * col], &R.m[(a + pc) * col], sizeof(double) * col);
+  for (int a = 0; a < pc; ++a)
+    for (int b = 0; b < o.ncy; ++b)
+      for (int c = 0; c < o.ncz; ++c) {
+        double* d = &R.m[3 * mm_idx(o, R.mcx - pc + a, b, c)];
+        d[0] = d[1] = d[2] = 0.0;
+        const int64_t cx = cxR + R.mcx + a;
+        if (mm_grain_of(o, cx, b) < 0) continue;
+        const double* v = &o.init_mean[3 * (size_t)((cx * o.ncy + b) * o.ncz + c)];
+        const double n = std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+        if (n > 0.0) { d[0] = v[0] / n; d[1] = v[1] / n; d[2] = v[2] / n; } else { d[2] = 1.0; }
+      }
+  o.x0 += p; o.shift += 1;
+  o.mm_age = 0; o.demag_age = 0;
+  return 0;
+}
+
+// Window plane i becomes global plane gx, generated from mesh cell column a_from of `from` (v = m_e m).
+void seed_plane_from(Oracle& o, int i, int64_t gx, const Oracle::MicroMesh* from, int a_from) {
+  for (int k = 0; k < o.nz; ++k)
+    for (int j = 0; j < o.ny; ++j) {
+      const int64_t l = o.site(i, k, j);
+      if (o.grain_map[(size_t)(gx * o.ny + j)] < 0) { o.sx[l] = o.sy[l] = o.sz[l] = 0.0; continue; }
+      const size_t q = mm_idx(o, a_from, j / o.macro[1], k / o.macro[2]);
+      const double v[3] = {from->me[q] * from->m[3 * q], from->me[q] * from->m[3 * q + 1], from->me[q] * from->m[3 * q + 2]};
+      double S[3];
+      seed_site_about(o, gx, k, j, v, S);
+      o.sx[l] = S[0]; o.sy[l] = S[1]; o.sz[l] = S[2];
+    }
 }
 
 // Window plane i becomes global plane gx of the track: vacant columns 0, magnetic sites seeded (S3).
@@ -616,6 +936,7 @@ void orc_step_heun(void* h, int64_t n) {
 // Deterministic field (no noise) or field with the noise of the current step counter, Tesla.
 void orc_field(void* h, int with_noise, double* bx, double* by, double* bz) {
   Oracle& o = *static_cast<Oracle*>(h);
+  if (o.mm) mm_exchange(o);
   std::vector<double> Bd;
   if (o.demag) demag_cells(o, o.sx.data(), o.sy.data(), o.sz.data(), Bd);
   for (int i = 0; i < o.nx; ++i)
@@ -690,6 +1011,7 @@ int orc_shift_window(void* h, int32_t p) {
   if (p < 1 || p > o.nx) return 1;
   if (o.ell_width > 0) return 5;                       // general ELL cannot follow the window
   if (o.x0 + p + o.nx > o.track_nx) return 1;          // grain map must cover the new window
+  if (o.mm) return mm_shift(o, p);                     // multiscale window: whole cells, through the meshes (M10)
   o.demag_age = 0;                                     // a held demagnetising field belongs to the old window
   const int nx = o.nx, ny = o.ny, nz = o.nz;
   // S2 outgoing: planes i < p, magnetic sites only, ascending l.
@@ -725,7 +1047,7 @@ int orc_shift_window(void* h, int32_t p) {
 //    The written store is kept (orc_track_get / orc_track_read_scan read it).
 int orc_track_end_pass(void* h) {
   Oracle& o = *static_cast<Oracle*>(h);
-  if (o.ell_width > 0) return 5;
+  if (o.ell_width > 0 || o.mm) return 5;
   for (int i = 0; i < o.nx; ++i)
     for (int k = 0; k < o.nz; ++k)
       for (int j = 0; j < o.ny; ++j) {
@@ -748,7 +1070,7 @@ int orc_track_end_pass(void* h) {
 //    The step and shift counters run on.
 int orc_track_begin_pass(void* h, int64_t x0_new) {
   Oracle& o = *static_cast<Oracle*>(h);
-  if (o.ell_width > 0) return 5;
+  if (o.ell_width > 0 || o.mm) return 5;
   if (x0_new < 0 || x0_new + o.nx > o.track_nx) return 1;
   const size_t nc = (size_t)(o.ncx * o.ncy * o.ncz);
   for (size_t c = 0; c < nc; ++c) { o.out_cnt[c] = 0; o.out_sum[3 * c] = o.out_sum[3 * c + 1] = o.out_sum[3 * c + 2] = 0.0; }
@@ -821,6 +1143,111 @@ void orc_set_counters(void* h, int64_t step, int64_t shift, int64_t pass) {
   Oracle& o = *static_cast<Oracle*>(h);
   o.step = step; o.shift = shift; o.pass = pass;
 }
+
+// ---- multiscale window (S:8(f) item 3) ----
+struct orc_mm_desc {
+  int32_t mcx[2];             // cells along x of the trailing / leading mesh
+  int32_t every;              // Heun steps per RK4 step
+  double Ms0, A0[3];          // A/m; J/m along x, y, z
+  const double* K0;           // [n_grains] J/m^3
+  const double* Tc;           // [n_grains] K
+  const int32_t* cell_grain;  // [ncx*ncy] grain id per track cell column, -1 = empty
+  double spacing[3];          // lattice constants, metres (cell = macro * spacing)
+};
+// 0 ok; 1 bad geometry (M1: x0 and nx whole cells; meshes inside the track); 5 unsupported lattice options
+int orc_mm_enable(void* h, const orc_mm_desc* d) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  if (o.ell_width > 0 || o.pbc[0] || o.pbc[1] || o.pbc[2]) return 5;
+  const int mx = o.macro[0];
+  if (o.x0 % mx != 0 || o.nx % mx != 0 || d->mcx[0] < 1 || d->mcx[1] < 1 || d->every < 1) return 1;
+  if (o.x0 / mx - d->mcx[0] < 0 || (o.x0 + o.nx) / mx + d->mcx[1] > o.ncx) return 1;
+  o.mm_Ms0 = d->Ms0; for (int a = 0; a < 3; ++a) o.mm_A0[a] = d->A0[a]; o.mm_every = d->every; o.mm_age = 0;
+  o.mm_K0.assign(d->K0, d->K0 + o.n_grains); o.mm_Tc.assign(d->Tc, d->Tc + o.n_grains);
+  o.mm_grain.assign(d->cell_grain, d->cell_grain + (size_t)(o.ncx * o.ncy));
+  for (int a = 0; a < 3; ++a) o.mm_cell[a] = o.macro[a] * d->spacing[a];
+  for (int side = 0; side < 2; ++side) {
+    Oracle::MicroMesh& M = o.mesh[side];
+    M.mcx = d->mcx[side];
+    const size_t n = (size_t)M.mcx * o.ncy * o.ncz;
+    M.m.assign(3 * n, 0.0); M.T.assign(n, 0.0); M.Bx.assign(n, 0.0); M.By.assign(n, 0.0); M.Bz.assign(n, 0.0);
+    M.me.assign(n, 0.0); M.alpha.assign(n, 0.0);
+    o.mm_ghost[side].assign((size_t)o.ncy * o.ncz * 3, 0.0);
+    o.mm_avg[side].assign((size_t)o.ncy * o.ncz * 3, 0.0);
+  }
+  o.mm = true;
+  // initial state: the direction of the track the meshes lie over (empty cells 0)
+  for (int side = 0; side < 2; ++side) {
+    Oracle::MicroMesh& M = o.mesh[side];
+    const int64_t cx0 = mm_cx0(o, side);
+    for (int a = 0; a < M.mcx; ++a)
+      for (int b = 0; b < o.ncy; ++b)
+        for (int c = 0; c < o.ncz; ++c) {
+          if (mm_grain_of(o, cx0 + a, b) < 0) continue;
+          double n[3] = {0.0, 0.0, 1.0};
+          track_direction(o, cx0 + a, b, c, n);
+          for (int u = 0; u < 3; ++u) M.m[3 * mm_idx(o, a, b, c) + u] = n[u];
+        }
+  }
+  mm_refresh_params(o);
+  return 0;
+}
+int64_t orc_mm_cells(void* h, int side) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  return (int64_t)o.mesh[side].mcx * o.ncy * o.ncz;
+}
+// per cell (a slowest, then b, then c): T [K] and B [Tesla]; NULL keeps the previous array
+void orc_mm_set_fields(void* h, int side, const double* T, const double* Bx, const double* By, const double* Bz) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  Oracle::MicroMesh& M = o.mesh[side];
+  for (size_t q = 0; q < M.T.size(); ++q) {
+    if (T) M.T[q] = T[q];
+    if (Bx) M.Bx[q] = Bx[q];
+    if (By) M.By[q] = By[q];
+    if (Bz) M.Bz[q] = Bz[q];
+  }
+  mm_refresh_params(o);
+}
+// m [cells*3]; set: empty cells stay 0, others are stored as given (unit vectors expected)
+void orc_mm_set_m(void* h, int side, const double* m) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  Oracle::MicroMesh& M = o.mesh[side];
+  const int64_t cx0 = mm_cx0(o, side);
+  for (int a = 0; a < M.mcx; ++a)
+    for (int b = 0; b < o.ncy; ++b)
+      for (int c = 0; c < o.ncz; ++c) {
+        const size_t q = mm_idx(o, a, b, c);
+        const bool full = mm_grain_of(o, cx0 + a, b) >= 0;
+        for (int u = 0; u < 3; ++u) M.m[3 * q + u] = full ? m[3 * q + u] : 0.0;
+      }
+  o.mm_age = 0;
+}
+void orc_mm_get_m(void* h, int side, double* m) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  std::memcpy(m, o.mesh[side].m.data(), sizeof(double) * o.mesh[side].m.size());
+}
+void orc_mm_get_params(void* h, int side, double* me, double* alpha) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  mm_refresh_params(o);
+  std::memcpy(me, o.mesh[side].me.data(), sizeof(double) * o.mesh[side].me.size());
+  std::memcpy(alpha, o.mesh[side].alpha.data(), sizeof(double) * o.mesh[side].alpha.size());
+}
+// effective field of every cell of one mesh for the current configurations (boundary data exchanged now), Tesla
+void orc_mm_field(void* h, int side, double* B) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  mm_exchange(o);
+  mm_refresh_params(o);
+  const Oracle::MicroMesh& M = o.mesh[side];
+  for (int a = 0; a < M.mcx; ++a)
+    for (int b = 0; b < o.ncy; ++b)
+      for (int c = 0; c < o.ncz; ++c) mm_field(o, side, M.m, a, b, c, &B[3 * mm_idx(o, a, b, c)]);
+}
+// n RK4 steps of length h on the meshes alone (boundary data exchanged before each): for the pins
+void orc_mm_step(void* h, int64_t n, double step) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  for (int64_t t = 0; t < n; ++t) { mm_exchange(o); mm_refresh_params(o); mm_rk4_step(o, step); }
+}
+double orc_mm_me(double T, double Tc, double mu_s_Bext) { return m_e_of(T, Tc, mu_s_Bext); }
+double orc_langevin(double x) { return langevin(x); }
 
 // ---- building blocks exposed for the pins ----
 void orc_philox4x32_10(const uint32_t key[2], const uint32_t ctr[4], uint32_t out[4]) { philox4x32_10(key, ctr, out); }

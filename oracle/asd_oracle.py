@@ -53,6 +53,16 @@ class _Desc(C.Structure):
     ]
 
 
+class _MmDesc(C.Structure):
+    _fields_ = [
+        ("mcx", C.c_int32 * 2), ("every", C.c_int32),
+        ("Ms0", C.c_double), ("A0", C.c_double * 3),
+        ("K0", C.POINTER(C.c_double)), ("Tc", C.POINTER(C.c_double)),
+        ("cell_grain", C.POINTER(C.c_int32)),
+        ("spacing", C.c_double * 3),
+    ]
+
+
 _lib = None
 
 
@@ -91,6 +101,20 @@ def lib():
         L.orc_track_read_scan.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double,
                                           C.c_int64, dp]
         L.orc_get_counters.argtypes = [C.c_void_p, ip64, ip64, ip64, ip64]
+        L.orc_mm_enable.restype = C.c_int
+        L.orc_mm_enable.argtypes = [C.c_void_p, C.POINTER(_MmDesc)]
+        L.orc_mm_cells.restype = C.c_int64
+        L.orc_mm_cells.argtypes = [C.c_void_p, C.c_int]
+        L.orc_mm_set_fields.argtypes = [C.c_void_p, C.c_int, dp, dp, dp, dp]
+        L.orc_mm_set_m.argtypes = [C.c_void_p, C.c_int, dp]
+        L.orc_mm_get_m.argtypes = [C.c_void_p, C.c_int, dp]
+        L.orc_mm_get_params.argtypes = [C.c_void_p, C.c_int, dp, dp]
+        L.orc_mm_field.argtypes = [C.c_void_p, C.c_int, dp]
+        L.orc_mm_step.argtypes = [C.c_void_p, C.c_int64, C.c_double]
+        L.orc_mm_me.restype = C.c_double
+        L.orc_mm_me.argtypes = [C.c_double, C.c_double, C.c_double]
+        L.orc_langevin.restype = C.c_double
+        L.orc_langevin.argtypes = [C.c_double]
         L.orc_set_counters.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_int64]
         u32p = C.POINTER(C.c_uint32)
         L.orc_philox4x32_10.argtypes = [u32p, u32p, u32p]
@@ -161,6 +185,15 @@ def newell_tensor(cell, R) -> np.ndarray:
 
 def theta_max(m: float) -> float:
     return float(lib().orc_theta_max(C.c_double(m)))
+
+
+def mm_me(T: float, Tc: float, mu_s_Bext: float = 0.0) -> float:
+    """m_e(T): largest root of m = B(3 T_C m / T + mu_s B_ext / k_B T)."""
+    return float(lib().orc_mm_me(C.c_double(T), C.c_double(Tc), C.c_double(mu_s_Bext)))
+
+
+def langevin(x: float) -> float:
+    return float(lib().orc_langevin(C.c_double(x)))
 
 
 def max_threads() -> int:
@@ -338,6 +371,65 @@ class Oracle:
         lib().orc_track_read_scan(self._h, C.c_double(y_r), C.c_double(sigma_x), C.c_double(sigma_y),
                                   C.c_double(x_first), C.c_double(x_step), C.c_int64(count), _ptr(out, C.c_double))
         return out
+
+    # ---- multiscale window: micromagnetic meshes either side of the atomistic mesh (SURVEY 8(f) item 3) ----
+    def mm_enable(self, mcx, every, Ms0, A0, K0, Tc, cell_grain, spacing_m) -> int:
+        d = _MmDesc()
+        d.mcx = (C.c_int32 * 2)(int(mcx[0]), int(mcx[1]))
+        d.every = int(every)
+        d.Ms0 = float(Ms0)
+        A0 = np.broadcast_to(np.asarray(A0, dtype=np.float64), (3,))
+        d.A0 = (C.c_double * 3)(*[float(x) for x in A0])
+        self._mmK = np.ascontiguousarray(K0, dtype=np.float64).reshape(-1)
+        self._mmT = np.ascontiguousarray(Tc, dtype=np.float64).reshape(-1)
+        self._mmG = np.ascontiguousarray(cell_grain, dtype=np.int32).reshape(-1)
+        assert self._mmK.size == self.n_grains and self._mmT.size == self.n_grains
+        ncx, ncy, _ = self.track_dims()
+        assert self._mmG.size == ncx * ncy
+        d.K0, d.Tc, d.cell_grain = _ptr(self._mmK, C.c_double), _ptr(self._mmT, C.c_double), _ptr(self._mmG, C.c_int32)
+        d.spacing = (C.c_double * 3)(*[float(x) for x in spacing_m])
+        st = int(lib().orc_mm_enable(self._h, C.byref(d)))
+        if st == 0:
+            self.mm_mcx = (int(mcx[0]), int(mcx[1]))
+        return st
+
+    def mm_shape(self, side: int):
+        _, ncy, ncz = self.track_dims()
+        return (self.mm_mcx[side], ncy, ncz)
+
+    def mm_set_fields(self, side: int, T=None, Bx=None, By=None, Bz=None):
+        n = int(np.prod(self.mm_shape(side)))
+        arrs = [None if a is None else np.ascontiguousarray(a, dtype=np.float64).reshape(-1) for a in (T, Bx, By, Bz)]
+        for a in arrs:
+            assert a is None or a.size == n
+        lib().orc_mm_set_fields(self._h, int(side), *[_ptr(a, C.c_double) for a in arrs])
+
+    def mm_set_m(self, side: int, m):
+        a = np.ascontiguousarray(m, dtype=np.float64).reshape(-1)
+        assert a.size == 3 * int(np.prod(self.mm_shape(side)))
+        lib().orc_mm_set_m(self._h, int(side), _ptr(a, C.c_double))
+
+    def mm_get_m(self, side: int) -> np.ndarray:
+        """[mcx, ncy, ncz, 3]"""
+        out = np.zeros(self.mm_shape(side) + (3,))
+        lib().orc_mm_get_m(self._h, int(side), _ptr(out, C.c_double))
+        return out
+
+    def mm_params(self, side: int):
+        """(m_e, alpha), each [mcx, ncy, ncz]"""
+        me, al = np.zeros(self.mm_shape(side)), np.zeros(self.mm_shape(side))
+        lib().orc_mm_get_params(self._h, int(side), _ptr(me, C.c_double), _ptr(al, C.c_double))
+        return me, al
+
+    def mm_field(self, side: int) -> np.ndarray:
+        """Effective field per cell, Tesla, [mcx, ncy, ncz, 3] (boundary data exchanged now)."""
+        out = np.zeros(self.mm_shape(side) + (3,))
+        lib().orc_mm_field(self._h, int(side), _ptr(out, C.c_double))
+        return out
+
+    def mm_step(self, n: int, h: float):
+        """n RK4 steps of length h [s] on the meshes alone."""
+        lib().orc_mm_step(self._h, C.c_int64(n), C.c_double(h))
 
     def counters(self):
         a, b, c, d = C.c_int64(0), C.c_int64(0), C.c_int64(0), C.c_int64(0)
