@@ -217,6 +217,50 @@ ASD_API asd_status asd_track_begin_pass(asd_ctx *ctx, int64_t x0_new);
 ASD_API asd_status asd_track_read_scan(asd_ctx *ctx, double y_r, double sigma_x, double sigma_y, double x_first,
                                        double x_step, int64_t count, double *out);
 
+/* ---- Multiscale window: micromagnetic LLG meshes either side of the atomistic mesh (Fig. 1, P:29-33, P:38, P:54-62,
+ * P:118, readings M1-M10) --------------------------------------------------------------------------
+ * The window becomes [trailing mesh | atomistic mesh | leading mesh]; the mesh cells are the track macrocells, so the
+ * window origin x0 and nx must be whole cells (multiples of macro[0]) and the meshes must lie inside the track.
+ *   state      one unit direction m per cell (0 = empty cell), fp32
+ *   field      B = (2 A_0 m_e / M_S^0) lap(m) + (2 K_0 m_e^2 / M_S^0)(m.e)e + s B_app     (Eq. (4), (5) with A = A_0 m_e^2,
+ *              K = K_0 m_e^3, M_S = M_S^0 m_e; 6-neighbour stencil; none between different grains);
+ *              m_e(T) = largest root of m = B(3 T_C m / T + mu_s |s B_app| / k_B T), B(x) = coth x - 1/x
+ *   dynamics   Eq. (1) without the stochastic field, damping lambda (1 - T / 3 T_C) (held at its T_C value above
+ *              T_C), classical RK4: one step of every * dt per `every` Heun steps
+ *   coupling   across each mesh boundary, both ways: the atomistic sites of the first / last plane take the
+ *              mesh direction in place of their missing neighbour spins in Eq. (2); the mesh cells take the direction
+ *              of the average atomistic spin of the adjacent stencil cell in the Laplacian; the far mesh ends take the
+ *              frozen track.  Boundary data is exchanged when the meshes step and held in between.
+ *   shift      asd_shift_window then moves by whole cells (p a multiple of macro[0], at most the shorter mesh):
+ *              trailing mesh -> track store (as m_e m per magnetic site), outgoing atoms -> trailing mesh by Eq. (6),
+ *              leading mesh -> incoming atoms by the cone sampling of P:68 about m with magnitude m_e, track ahead ->
+ *              leading mesh; ASD_EINVAL otherwise.
+ * HOST pointers of the description are read during asd_mm_enable only.  The caller owns the workspace (DEVICE, 256-byte
+ * aligned) for the life of the context.  Not available with general ELL tables, periodic boundaries, ASD_KERNEL_TMA,
+ * CUDA-graph replay, asd_track_end_pass / asd_track_begin_pass (ASD_EUNSUPPORTED). */
+typedef struct {
+  int32_t mcx[2];            /* cells along x of the trailing / leading mesh, each >= 1                          */
+  int32_t every;             /* Heun steps per RK4 step, >= 1                                                    */
+  double Ms0;                /* M_S^0, A/m                                                                       */
+  double A0[3];              /* A_0 along x, y, z, J/m (one value three times = the paper's scalar A)            */
+  const double *K0;          /* HOST [n_grains] K_0, J/m^3 (easy axes = grain_axis of the lattice)               */
+  const double *Tc;          /* HOST [n_grains] T_C, K                                                           */
+  const int32_t *cell_grain; /* HOST [ncx*ncy] grain id of track cell column (cx, cy) at cx*ncy + cy; -1 = empty */
+  double spacing_m[3];       /* lattice constants, metres (cell edge = macro * spacing)                          */
+} asd_mm_desc;
+ASD_API size_t asd_mm_workspace_bytes(const asd_ctx *ctx, const asd_mm_desc *desc);
+/* Initial mesh state: the direction of the track the meshes lie over; T = 0, B = 0. */
+ASD_API asd_status asd_mm_enable(asd_ctx *ctx, const asd_mm_desc *desc, void *d_workspace, size_t bytes);
+/* dims = (mcx[side], ncy, ncz); cell (a, b, c) of a mesh is element (a*ncy + b)*ncz + c of the arrays below. */
+ASD_API asd_status asd_mm_dims(const asd_ctx *ctx, int32_t side, int64_t dims[3]);
+/* Per-cell temperature [K] and applied field [Tesla] of one mesh, HOST [cells]; window-fixed profiles like the
+ * atomistic ones; NULL = keep.  Synchronises. */
+ASD_API asd_status asd_mm_set_fields_host(asd_ctx *ctx, int32_t side, const float *T, const float *Bx, const float *By,
+                                          const float *Bz);
+/* Cell directions of one mesh, HOST [cells*3] (component fastest).  set: empty cells stay 0.  Both synchronise. */
+ASD_API asd_status asd_mm_set_m_host(asd_ctx *ctx, int32_t side, const float *m);
+ASD_API asd_status asd_mm_get_m_host(asd_ctx *ctx, int32_t side, float *m);
+
 /* Counters for bit-exact checkpoint / resume (Philox is counter based: there is no RNG state). */
 ASD_API asd_status asd_get_counters(const asd_ctx *ctx, int64_t *step, int64_t *shift, int64_t *x0, int64_t *pass);
 ASD_API asd_status asd_set_counters(asd_ctx *ctx, int64_t step, int64_t shift, int64_t pass);

@@ -24,7 +24,9 @@ EXPORTED_SYMBOLS = [
     "asd_demag_field", "asd_set_demag_every", "asd_staging_bytes", "asd_set_staging", "asd_stage_fields_host",
     "asd_commit_fields", "asd_shift_window", "asd_magnetisation", "asd_grain_magnetisation",
     "asd_track_dims", "asd_track_set_init", "asd_track_get",
-    "asd_track_end_pass", "asd_track_begin_pass", "asd_track_read_scan", "asd_get_counters", "asd_set_counters",
+    "asd_track_end_pass", "asd_track_begin_pass", "asd_track_read_scan",
+    "asd_mm_workspace_bytes", "asd_mm_enable", "asd_mm_dims", "asd_mm_set_fields_host", "asd_mm_set_m_host",
+    "asd_mm_get_m_host", "asd_get_counters", "asd_set_counters",
     "asd_launch_count", "asd_last_error", "asd_version",
 ]
 
@@ -51,6 +53,16 @@ class _Desc(C.Structure):
         ("ell_J", C.POINTER(C.c_float)),
         ("ell_width", C.c_int32),
         ("seed", C.c_uint64),
+    ]
+
+
+class _MmDesc(C.Structure):
+    _fields_ = [
+        ("mcx", C.c_int32 * 2), ("every", C.c_int32),
+        ("Ms0", C.c_double), ("A0", C.c_double * 3),
+        ("K0", C.POINTER(C.c_double)), ("Tc", C.POINTER(C.c_double)),
+        ("cell_grain", C.POINTER(C.c_int32)),
+        ("spacing_m", C.c_double * 3),
     ]
 
 
@@ -110,6 +122,13 @@ def load_library(build_if_missing: bool = True):
     L.asd_track_begin_pass.argtypes = [C.c_void_p, C.c_int64]
     L.asd_track_read_scan.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double,
                                       C.c_int64, dp]
+    L.asd_mm_workspace_bytes.restype = C.c_size_t
+    L.asd_mm_workspace_bytes.argtypes = [C.c_void_p, C.POINTER(_MmDesc)]
+    L.asd_mm_enable.argtypes = [C.c_void_p, C.POINTER(_MmDesc), C.c_void_p, C.c_size_t]
+    L.asd_mm_dims.argtypes = [C.c_void_p, C.c_int32, ip64]
+    L.asd_mm_set_fields_host.argtypes = [C.c_void_p, C.c_int32, fp, fp, fp, fp]
+    L.asd_mm_set_m_host.argtypes = [C.c_void_p, C.c_int32, fp]
+    L.asd_mm_get_m_host.argtypes = [C.c_void_p, C.c_int32, fp]
     L.asd_get_counters.argtypes = [C.c_void_p, ip64, ip64, ip64, ip64]
     L.asd_set_counters.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_int64]
     L.asd_launch_count.restype = C.c_int64
@@ -375,6 +394,51 @@ class Context:
         self._ck(self._L.asd_track_read_scan(self._h, C.c_double(y_r), C.c_double(sigma_x), C.c_double(sigma_y),
                                              C.c_double(x_first), C.c_double(x_step), C.c_int64(count),
                                              out.ctypes.data_as(C.POINTER(C.c_double))))
+        return out
+
+    # ---- multiscale window ----
+    def mm_enable(self, mcx, every, Ms0, A0, K0, Tc, cell_grain, spacing_m):
+        """asd_mm_enable (allocates the mesh workspace)."""
+        import torch
+        d = _MmDesc()
+        d.mcx = (C.c_int32 * 2)(int(mcx[0]), int(mcx[1]))
+        d.every = int(every)
+        d.Ms0 = float(Ms0)
+        d.A0 = (C.c_double * 3)(*[float(x) for x in np.broadcast_to(np.asarray(A0, dtype=np.float64), (3,))])
+        K0 = np.ascontiguousarray(K0, dtype=np.float64).reshape(-1)
+        Tc = np.ascontiguousarray(Tc, dtype=np.float64).reshape(-1)
+        cg = np.ascontiguousarray(cell_grain, dtype=np.int32).reshape(-1)
+        ncx, ncy, _ = self.track_dims()
+        if K0.size != self.n_grains or Tc.size != self.n_grains or cg.size != ncx * ncy:
+            raise AsdError(1, "mm_enable: K0 / Tc need one entry per grain, cell_grain one per track cell column")
+        d.K0 = K0.ctypes.data_as(C.POINTER(C.c_double))
+        d.Tc = Tc.ctypes.data_as(C.POINTER(C.c_double))
+        d.cell_grain = cg.ctypes.data_as(C.POINTER(C.c_int32))
+        d.spacing_m = (C.c_double * 3)(*[float(x) for x in spacing_m])
+        nbytes = int(self._L.asd_mm_workspace_bytes(self._h, C.byref(d)))
+        if nbytes == 0:
+            raise AsdError(1, "asd_mm_workspace_bytes rejected the description")
+        self._mm_ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        ptr = (self._mm_ws.data_ptr() + 255) & ~255
+        self._ck(self._L.asd_mm_enable(self._h, C.byref(d), C.c_void_p(ptr), C.c_size_t(nbytes)))
+
+    def mm_shape(self, side: int):
+        d = (C.c_int64 * 3)()
+        self._ck(self._L.asd_mm_dims(self._h, C.c_int32(side), d))
+        return tuple(int(x) for x in d)
+
+    def mm_set_fields(self, side: int, T=None, Bx=None, By=None, Bz=None):
+        keep = []
+        self._ck(self._L.asd_mm_set_fields_host(self._h, C.c_int32(side), _host_ptr(T, keep), _host_ptr(Bx, keep),
+                                                _host_ptr(By, keep), _host_ptr(Bz, keep)))
+
+    def mm_set_m(self, side: int, m):
+        keep = []
+        self._ck(self._L.asd_mm_set_m_host(self._h, C.c_int32(side), _host_ptr(m, keep)))
+
+    def mm_get_m(self, side: int) -> np.ndarray:
+        out = np.zeros(self.mm_shape(side) + (3,), dtype=np.float32)
+        self._ck(self._L.asd_mm_get_m_host(self._h, C.c_int32(side), C.c_void_p(out.ctypes.data)))
         return out
 
     # ---- counters ----

@@ -230,6 +230,7 @@ asd_status asd_destroy(asd_ctx* ctx) {
   asd::graphs_free(ctx->c);
   if (ctx->c.copy_stream) { cudaStreamDestroy(ctx->c.copy_stream); cudaEventDestroy(ctx->c.staged_ev); cudaEventDestroy(ctx->c.consumed_ev); }
   asd::demag_free(ctx->c);
+  asd::mm_free(ctx->c);
   delete ctx;
   return ASD_OK;
 }
@@ -239,6 +240,7 @@ asd_status asd_destroy(asd_ctx* ctx) {
 static asd_status set_spins_impl(Ctx& c, const float* sx, const float* sy, const float* sz, bool host) {
   if (!sx || !sy || !sz) return fail(c, ASD_EINVAL, "asd_set_spins: NULL pointer");
   c.demag_age = 0;                             // a held demagnetising field belongs to the old spins
+  mm_restart_cadence(c);                       // ... and so do the held mesh boundary data
   if (host) {
     const float* src[3] = {sx, sy, sz};
     for (int a = 0; a < 3; ++a)
@@ -387,6 +389,7 @@ asd_status asd_set_kernel(asd_ctx* ctx, int32_t variant) {
     return fail(c, ASD_EINVAL, "asd_set_kernel: unknown variant");
   if (variant == ASD_KERNEL_FUSED && (!heun_fused_supported(c) || c.demag || !fused_plan(c)))
     return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: the fused step needs what the film kernel needs, no demagnetising field, and a strip plan that fits in shared memory");
+  if (variant == ASD_KERNEL_TMA && c.mm) return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: the staged film kernel does not take a multiscale window");
   if (variant == ASD_KERNEL_TMA && (!heun_tma_supported(c) || !tma_plan(c)))
     return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: the staged film kernel needs what the film kernel needs and a strip plan that fits in shared memory");
   if (variant == ASD_KERNEL_FAST && !heun_fast_supported(c))
@@ -443,6 +446,15 @@ asd_status asd_shift_window(asd_ctx* ctx, int32_t p) {
   if (c.x0 + p + c.d.nx > c.d.track_nx) return fail(c, ASD_ESTATE, "asd_shift_window: past the end of the track");
   graphs_invalidate(c);                        // window origin and buffer roles are frozen in recorded graphs
   c.demag_age = 0;                             // a held demagnetising field belongs to the old window position
+  if (c.mm) {                                  // multiscale window: whole cells, through the meshes (M10)
+    int64_t dl[3], dr[3];
+    mm_dims(c, 0, dl); mm_dims(c, 1, dr);
+    const int mx = c.d.macro[0];
+    if (p % mx != 0 || p / mx > dl[0] || p / mx > dr[0])
+      return fail(c, ASD_EINVAL, "asd_shift_window: a multiscale window moves by whole macrocells, at most the shorter mesh");
+    if ((c.x0 + c.d.nx) / mx + dr[0] + p / mx > c.ncx) return fail(c, ASD_ESTATE, "asd_shift_window: leading mesh past the end of the track");
+    return launch_shift_mm(c, p);
+  }
   return launch_shift(c, p);
 }
 
@@ -495,6 +507,7 @@ asd_status asd_track_get(asd_ctx* ctx, double* sum, int64_t* count) {
 asd_status asd_track_end_pass(asd_ctx* ctx) {
   CTX_OR_RETURN(ctx);
   if (c.d.ell_width > 0) return fail(c, ASD_EUNSUPPORTED, "asd_track_end_pass: a general ELL table has no track");
+  if (c.mm) return fail(c, ASD_EUNSUPPORTED, "asd_track_end_pass: not defined for a multiscale window");
   return launch_track_end_pass(c);
 }
 
@@ -502,6 +515,7 @@ asd_status asd_track_begin_pass(asd_ctx* ctx, int64_t x0_new) {
   CTX_OR_RETURN(ctx);
   if (c.d.ell_width > 0) return fail(c, ASD_EUNSUPPORTED, "asd_track_begin_pass: a general ELL table cannot follow the window");
   if (c.d.pbc[0]) return fail(c, ASD_EUNSUPPORTED, "asd_track_begin_pass: window is periodic in x");
+  if (c.mm) return fail(c, ASD_EUNSUPPORTED, "asd_track_begin_pass: not defined for a multiscale window");
   if (x0_new < 0 || x0_new + c.d.nx > c.d.track_nx) return fail(c, ASD_EINVAL, "asd_track_begin_pass: window must lie inside the track");
   graphs_invalidate(c);
   c.demag_age = 0;
@@ -516,6 +530,71 @@ asd_status asd_track_read_scan(asd_ctx* ctx, double y_r, double sigma_x, double 
       !std::isfinite(x_first) || !std::isfinite(x_step))
     return fail(c, ASD_EINVAL, "asd_track_read_scan: footprint widths must be > 0 and positions finite");
   return launch_track_read_scan(c, y_r, sigma_x, sigma_y, x_first, x_step, count, out);
+}
+
+static const char* mm_check(const Ctx& c, const asd_mm_desc* d) {
+  if (!d || !d->K0 || !d->Tc || !d->cell_grain) return "asd_mm: NULL description or array";
+  if (d->mcx[0] < 1 || d->mcx[1] < 1 || d->every < 1) return "asd_mm: mcx[] and every must be >= 1";
+  if (!(d->Ms0 > 0.0) || !std::isfinite(d->Ms0)) return "asd_mm: Ms0 must be > 0";
+  for (int a = 0; a < 3; ++a) {
+    if (!(d->A0[a] >= 0.0) || !std::isfinite(d->A0[a])) return "asd_mm: A0[] must be >= 0";
+    if (!(d->spacing_m[a] > 0.0)) return "asd_mm: lattice constants must be > 0";
+  }
+  const int mx = c.d.macro[0];
+  if (c.x0 % mx != 0 || c.d.nx % mx != 0) return "asd_mm: window origin and length must be whole macrocells";
+  if (c.x0 / mx - d->mcx[0] < 0 || (c.x0 + c.d.nx) / mx + d->mcx[1] > c.ncx) return "asd_mm: meshes must lie inside the track";
+  for (int g = 0; g < c.d.n_grains; ++g)
+    if (!(d->Tc[g] > 0.0) || !std::isfinite(d->K0[g])) return "asd_mm: Tc[] must be > 0 and K0[] finite";
+  for (int64_t t = 0; t < c.ncx * c.ncy; ++t)
+    if (d->cell_grain[t] < -1 || d->cell_grain[t] >= c.d.n_grains) return "asd_mm: cell grain id out of range";
+  return nullptr;
+}
+
+size_t asd_mm_workspace_bytes(const asd_ctx* ctx, const asd_mm_desc* desc) {
+  if (!ctx || !desc || desc->mcx[0] < 1 || desc->mcx[1] < 1) return 0;
+  return mm_workspace_bytes(ctx->c, desc->mcx);
+}
+
+asd_status asd_mm_enable(asd_ctx* ctx, const asd_mm_desc* desc, void* d_workspace, size_t bytes) {
+  CTX_OR_RETURN(ctx);
+  if (c.d.ell_width > 0 || c.d.pbc[0] || c.d.pbc[1] || c.d.pbc[2])
+    return fail(c, ASD_EUNSUPPORTED, "asd_mm_enable: open-boundary lattices with built-in shells only");
+  if (c.kernel_variant == ASD_KERNEL_TMA) return fail(c, ASD_EUNSUPPORTED, "asd_mm_enable: not with ASD_KERNEL_TMA");
+  if (const char* why = mm_check(c, desc)) return fail(c, ASD_EINVAL, why);
+  if (!d_workspace || ((uintptr_t)d_workspace & 255u)) return fail(c, ASD_EINVAL, "asd_mm_enable: workspace NULL or not 256-byte aligned");
+  graphs_invalidate(c);
+  return mm_enable(c, *desc, d_workspace, bytes);
+}
+
+asd_status asd_mm_dims(const asd_ctx* ctx, int32_t side, int64_t dims[3]) {
+  if (!ctx || !dims || (side != 0 && side != 1)) return ASD_EINVAL;
+  if (!ctx->c.mm) return ASD_ESTATE;
+  mm_dims(ctx->c, side, dims);
+  return ASD_OK;
+}
+
+#define MM_OR_RETURN(name)                                                                         \
+  if (side != 0 && side != 1) return fail(c, ASD_EINVAL, name ": side must be 0 or 1");            \
+  if (!c.mm) return fail(c, ASD_ESTATE, name ": asd_mm_enable has not been called");
+
+asd_status asd_mm_set_fields_host(asd_ctx* ctx, int32_t side, const float* T, const float* Bx, const float* By, const float* Bz) {
+  CTX_OR_RETURN(ctx);
+  MM_OR_RETURN("asd_mm_set_fields_host");
+  return mm_set_fields_host(c, side, T, Bx, By, Bz);
+}
+
+asd_status asd_mm_set_m_host(asd_ctx* ctx, int32_t side, const float* m) {
+  CTX_OR_RETURN(ctx);
+  MM_OR_RETURN("asd_mm_set_m_host");
+  if (!m) return fail(c, ASD_EINVAL, "asd_mm_set_m_host: m is NULL");
+  return mm_set_m_host(c, side, m);
+}
+
+asd_status asd_mm_get_m_host(asd_ctx* ctx, int32_t side, float* m) {
+  CTX_OR_RETURN(ctx);
+  MM_OR_RETURN("asd_mm_get_m_host");
+  if (!m) return fail(c, ASD_EINVAL, "asd_mm_get_m_host: m is NULL");
+  return mm_get_m_host(c, side, m);
 }
 
 asd_status asd_get_counters(const asd_ctx* ctx, int64_t* step, int64_t* shift, int64_t* x0, int64_t* pass) {

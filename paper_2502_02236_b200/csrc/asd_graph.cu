@@ -90,7 +90,7 @@ void graphs_free(Ctx& c) {
 
 asd_status launch_heun(Ctx& c, int64_t n) {
   c.launch_stream = c.stream;
-  const bool use = !c.demag &&                  // the demag pipeline is launched plainly
+  const bool use = !c.demag && !c.mm &&         // the demag pipeline and the mesh steps are launched plainly
                    c.kernel_variant != ASD_KERNEL_FUSED &&   // the fused step swaps the spin buffers every step
                    (c.graph_mode == ASD_GRAPH_ON || (c.graph_mode == ASD_GRAPH_AUTO && c.N <= kAutoMaxSites));
   while (use && n >= 2) {

@@ -176,6 +176,20 @@ __global__ void __launch_bounds__(256) heun_stage_general(const StageParams p) {
       }
     }
 
+    if (p.edgeB && LAT != LAT_ELL) {                 // multiscale window: the held mesh directions beyond the x edges
+#pragma unroll
+      for (int side = 0; side < 2; ++side) {
+        if (i != (side == 0 ? 0 : p.nx - 1)) continue;
+        const float* eb = p.edgeB + (size_t)side * 3u * (size_t)planep + (size_t)k * p.nyp + j0;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          float ev[VEC];
+          VecIO<VEC>::ld(eb + (size_t)c * (size_t)planep, ev);
+#pragma unroll
+          for (int v = 0; v < VEC; ++v) Bex[c][v] += ev[v];
+        }
+      }
+    }
     float sg[VEC], Ba[3][VEC], Ain[3][VEC];
     VecIO<VEC>::ld(p.arrays + (size_t)AR_SIGMA * p.as + e0, sg);
 #pragma unroll
@@ -266,6 +280,7 @@ void fill_stage_params(const Ctx& c, StageParams& p) {
   p.scale = c.scale;
   p.g0 = (uint64_t)c.x0 * (uint64_t)c.plane;
   demag_fill_params(c, p);
+  p.edgeB = mm_edge_field(c);
   uint32_t k0 = (uint32_t)(c.d.seed & 0xFFFFFFFFull), k1 = (uint32_t)(c.d.seed >> 32);
   for (int r = 0; r < 10; ++r) {
     p.key.k0[r] = k0; p.key.k1[r] = k1;
@@ -282,11 +297,13 @@ asd_status launch_heun_direct(Ctx& c, int64_t n, const DynState* dyn) {
   p.dyn = dyn;
   const bool vec4 = (c.d.ny % 4 == 0);
   // with the demagnetising field on, the film kernel assumes its 4 sites span at most two macrocells (my >= 3)
-  const bool fast = c.kernel_variant != ASD_KERNEL_GENERAL && heun_fast_supported(c) && !(c.demag && c.d.macro[1] < 3);
+  const bool fast = c.kernel_variant != ASD_KERNEL_GENERAL && heun_fast_supported(c) && !(c.demag && c.d.macro[1] < 3) &&
+                    !(c.demag && c.mm);
   if (c.kernel_variant == ASD_KERNEL_FAST && !fast) return ASD_EUNSUPPORTED;
   const bool staged = c.kernel_variant == ASD_KERNEL_TMA;
   if (staged && !(heun_tma_supported(c) && tma_plan(c))) return ASD_EUNSUPPORTED;
   if (c.demag && (staged || c.d.ell_width > 0)) return ASD_EUNSUPPORTED;   // demag: film and general kernels only
+  if (c.mm && (staged || dyn)) return ASD_EUNSUPPORTED;                    // multiscale: film, fused and general kernels, plain launches
   // one kernel per step: asked for, or AUTO on a film large enough to fill the machine with strip x chunk CTAs.
   // Not inside a recorded graph (the spin buffers swap roles every step) and not with the demagnetising field.
   const bool fused = !dyn && !c.demag && heun_fused_supported(c) &&
@@ -297,6 +314,7 @@ asd_status launch_heun_direct(Ctx& c, int64_t n, const DynState* dyn) {
     const uint64_t idx = dyn ? (uint64_t)s : (uint64_t)c.step;
     p.n_lo = (uint32_t)(idx & 0xFFFFFFFFull);
     p.n_hi = (uint32_t)(idx >> 32);
+    if (c.mm) { const asd_status sm = mm_before_step(c); if (sm != ASD_OK) return sm; }
     if (c.demag) {
       c.demag_refresh = c.demag_every <= 0 ? 3 : (c.demag_age % c.demag_every == 0 ? 1 : 0);
       c.demag_age += 1;

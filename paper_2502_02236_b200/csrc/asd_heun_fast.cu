@@ -39,6 +39,7 @@ struct FastParams {
   const DynState* dyn;
   DemagGeom dm;                    // demagnetising field per macrocell; used by the DEMAG instances
   uint32_t dm_my;                  // macrocell edge in y (sites)
+  const float* edgeB;              // multiscale window: mesh exchange field on planes 0 / nx-1 (MM instances)
   uint64_t g0;
   PhiloxKey key;
 };
@@ -62,7 +63,7 @@ constexpr uint32_t kPrefetchAhead = 148;
 
 // CTA shape: 128 threads x 5 CTAs per SM (96 registers per thread).  Measured on cfg4: 57.9 us per stage, against
 // 59.9 (256 x 3, 80 registers), 58.3 (128 x 4), 58.8 (128 x 6), 60.8 (256 x 2), 69.5 (512 x 1).
-template <int LAT, int STAGE, int NT = 128, int MINB = 5, bool DEMAG = false>
+template <int LAT, int STAGE, int NT = 128, int MINB = 5, bool DEMAG = false, bool MM = false>
 __global__ void __launch_bounds__(NT, MINB) heun_stage_fast(const FastParams p) {
   // ---- L2 prefetch: one bulk-prefetch instruction per streamed array brings the sites of the CTA that will run
   // kPrefetchAhead blocks later from HBM into L2.  It holds no registers and nobody waits for it; when that CTA's
@@ -134,6 +135,21 @@ __global__ void __launch_bounds__(NT, MINB) heun_stage_fast(const FastParams p) 
         const float s1 = xs[v + 1] + (own[c][v] + own[c][v + 2]);
         const float s3 = xs[v] + xs[v + 2];
         Bex[c][v] = fmaf(p.j3, s3, fmaf(p.j2, zs[v], p.j1 * s1));
+      }
+    }
+  }
+
+  if (MM) {
+    // multiscale window: the x neighbours beyond the first / last plane are held mesh directions; their share of
+    // Eq. (2) was summed per site at the last exchange (asd_mm.cu) and is added here
+#pragma unroll
+    for (int side = 0; side < 2; ++side) {
+      if (i != (side == 0 ? 0u : p.nx - 1u)) continue;
+      const float* eb = p.edgeB + ((uint32_t)side * 3u * p.planep + k * p.nyp + j0);
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        const float4 ev = __ldg(reinterpret_cast<const float4*>(eb + (uint32_t)c * p.planep));
+        Bex[c][0] += ev.x; Bex[c][1] += ev.y; Bex[c][2] += ev.z; Bex[c][3] += ev.w;
       }
     }
   }
@@ -215,18 +231,18 @@ __global__ void __launch_bounds__(NT, MINB) heun_stage_fast(const FastParams p) 
 }
 
 
-template <int LAT, bool DEMAG, int NT = 128, int MINB = 5>
+template <int LAT, bool DEMAG, bool MM = false, int NT = 128, int MINB = 5>
 asd_status launch_pair_fast(Ctx& c, FastParams& f) {
   const unsigned blocks = (f.nthreads + NT - 1u) / NT;
   f.pf_elems = ((uint32_t)NT * 4u / f.ny + 2u) * f.nyp;
   const uint32_t as = f.as;
   f.oX = (uint32_t)c.aS * as; f.oOut = (uint32_t)c.aSt * as; f.oOutA = AR_A * as; f.oA = AR_A * as;
   if (DEMAG && (c.demag_refresh & 1)) { const asd_status st = launch_demag(c, c.aS); if (st != ASD_OK) return st; }
-  launch_pdl(heun_stage_fast<LAT, 0, NT, MINB, DEMAG>, blocks, NT, c.launch_stream, f, c.launch_stream == c.stream);
+  launch_pdl(heun_stage_fast<LAT, 0, NT, MINB, DEMAG, MM>, blocks, NT, c.launch_stream, f, c.launch_stream == c.stream);
   ASD_LAUNCH_CHECK(c, "heun predictor (fast)");
   f.oX = (uint32_t)c.aSt * as; f.oOut = (uint32_t)c.aS * as;
   if (DEMAG && (c.demag_refresh & 2)) { const asd_status st = launch_demag(c, c.aSt); if (st != ASD_OK) return st; }
-  launch_pdl(heun_stage_fast<LAT, 1, NT, MINB, DEMAG>, blocks, NT, c.launch_stream, f, c.launch_stream == c.stream);
+  launch_pdl(heun_stage_fast<LAT, 1, NT, MINB, DEMAG, MM>, blocks, NT, c.launch_stream, f, c.launch_stream == c.stream);
   ASD_LAUNCH_CHECK(c, "heun corrector (fast)");
   return ASD_OK;
 }
@@ -253,6 +269,11 @@ asd_status launch_heun_fast(Ctx& c, StageParams& p) {
   f.gdt = p.gdt; f.lambda = p.lambda; f.scale = p.scale;
   f.n_lo = p.n_lo; f.n_hi = p.n_hi; f.dyn = p.dyn; f.g0 = p.g0; f.key = p.key;
   f.dm = p.dm; f.dm_my = (uint32_t)c.d.macro[1];
+  f.edgeB = p.edgeB;
+  if (p.edgeB) {
+    if (p.dm.B) return ASD_EUNSUPPORTED;             // multiscale + demagnetising field: general kernel only
+    return c.d.lattice == ASD_SC ? launch_pair_fast<LAT_SC, false, true>(c, f) : launch_pair_fast<LAT_L10, false, true>(c, f);
+  }
   if (p.dm.B) return c.d.lattice == ASD_SC ? launch_pair_fast<LAT_SC, true>(c, f) : launch_pair_fast<LAT_L10, true>(c, f);
   return c.d.lattice == ASD_SC ? launch_pair_fast<LAT_SC, false>(c, f) : launch_pair_fast<LAT_L10, false>(c, f);
 }

@@ -56,6 +56,7 @@ struct FusedParams {
   uint32_t n_lo, n_hi;
   const DynState* dyn;
   uint64_t g0;
+  const float* edgeB;              // multiscale window: mesh exchange field on planes 0 / nx-1 ([side][comp][nz*nyp]); nullptr: off
   PhiloxKey key;
 };
 
@@ -341,6 +342,22 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
             Bn[2][v] = fmaf(sgs, xi[v][2], sscale * bz[v]);
           }
         }
+        if (p.edgeB) {
+          // multiscale window: the held mesh directions beyond the first / last plane enter Eq. (2) of BOTH stages as a
+          // constant field, so they ride with the stage-independent part (asd_mm.cu)
+          const int q = i0 - 1 + m;
+#pragma unroll 1
+          for (int side = 0; side < 2; ++side) {
+            if (!active || q != (side == 0 ? 0 : p.nx - 1)) continue;
+            const float* eb = p.edgeB + ((uint32_t)side * 3u * planep + (uint32_t)(k * p.nyp + j));
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+              const float4 ev = __ldg(reinterpret_cast<const float4*>(eb + (uint32_t)c * planep));
+              Bn[c][0] = fmaf(p.ngdt, ev.x, Bn[c][0]); Bn[c][1] = fmaf(p.ngdt, ev.y, Bn[c][1]);
+              Bn[c][2] = fmaf(p.ngdt, ev.z, Bn[c][2]); Bn[c][3] = fmaf(p.ngdt, ev.w, Bn[c][3]);
+            }
+          }
+        }
         // the field box is refilled as soon as the last main warp has its values in registers (mid-predictor): the copy
         // has the rest of the march step to land.  That warp issues it.
         if (warp_count_last(cnt_fld, (uint32_t)p.n_main / 32u) && m + 1 <= L + 1) {
@@ -537,6 +554,15 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
               Bex[c] = fmaf(p.j3s, s3, fmaf(p.j2s, zs[c], p.j1s * (xs + ys)));
             }
           }
+          if (p.edgeB) {
+#pragma unroll 1
+            for (int side = 0; side < 2; ++side) {
+              if (q != (side == 0 ? 0 : p.nx - 1)) continue;
+              const float* eb = p.edgeB + ((uint32_t)side * 3u * planep + (uint32_t)(k * p.nyp + jh[s]));
+#pragma unroll
+              for (int c = 0; c < 3; ++c) Bex[c] = fmaf(p.ngdt, __ldg(eb + (uint32_t)c * planep), Bex[c]);
+            }
+          }
           const float4 gp = lds4(gpring + ((uint32_t)m & (kGpRing - 1u)) * gp_pitch + 16u * (uint32_t)(G + s));
           const float ca = gp.w * fmaf(Xs[0], gp.x, fmaf(Xs[1], gp.y, Xs[2] * gp.z));
           const float sgs = p.ngdt * sg[s];
@@ -724,6 +750,7 @@ asd_status launch_heun_fused(Ctx& c, StageParams& p) {
   f.j1s = f.ngdt * p.jx[0]; f.j2s = f.ngdt * p.jx[1]; f.j3s = f.ngdt * p.jx[2];
   f.lambda = p.lambda; f.scale = p.scale;
   f.n_lo = p.n_lo; f.n_hi = p.n_hi; f.dyn = p.dyn; f.g0 = p.g0; f.key = p.key;
+  f.edgeB = p.edgeB;
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)(pl->nstrips * pl->nchunks)); cfg.blockDim = dim3((unsigned)pl->threads);
   cfg.dynamicSmemBytes = pl->smem_bytes; cfg.stream = c.launch_stream;

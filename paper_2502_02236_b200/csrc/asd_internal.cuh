@@ -116,6 +116,8 @@ struct StageParams {
   uint32_t n_lo, n_hi;         // step index before the step (with dyn: offset of this step inside the graph)
   const DynState* dyn;         // nullptr outside graph replays
   DemagGeom dm;                // demagnetising field per macrocell (asd_demag.cu); dm.B == nullptr: off
+  const float* edgeB;          // multiscale window (asd_mm.cu): exchange field of the held mesh directions on the sites of
+                               // plane 0 (side 0) and nx-1 (side 1), [side][component][nz*nyp] padded rows; nullptr: off
   uint64_t g0;                 // x0 * ny * nz: global id of window site 0
   PhiloxKey key;
 };
@@ -124,6 +126,7 @@ struct StageParams {
 struct DemagPlan;           // asd_demag.cu: plans, transformed tensor and buffers of the demagnetising field
 struct TmaPlan;             // asd_heun_tma.cu: tensor maps + strip / chunk plan of the staged film kernel
 struct FusedPlan;           // asd_heun_fused.cu: tensor map + strip / chunk plan of the one-kernel Heun step
+struct MmPlan;              // asd_mm.cu: the micromagnetic meshes of the multiscale window
 
 struct Ctx {
   asd_lattice_desc d;          // host pointers inside are NOT valid after create
@@ -177,6 +180,7 @@ struct Ctx {
   int32_t demag_every = 0;          // 0: field recomputed in every stage; P >= 1: from S at every P-th Heun step, held in between
   int64_t demag_age = 0;            // Heun steps since the held field was last invalidated (enable, shift, set_spins)
   int32_t demag_refresh = 3;        // this step: bit 0 = recompute before the predictor, bit 1 = before the corrector
+  MmPlan* mm = nullptr;             // non-null once asd_mm_enable succeeded
   TmaPlan* tma_plan = nullptr;      // built lazily by the first staged launch (host memory, freed by asd_destroy)
   bool tma_plan_tried = false;
   FusedPlan* fused_plan = nullptr;  // likewise for the fused one-kernel step
@@ -241,6 +245,21 @@ bool heun_fused_preferred(Ctx& c);                            // what ASD_KERNEL
 FusedPlan* fused_plan(Ctx& c);
 void fused_plan_free(Ctx& c);
 void fill_stage_params(const Ctx& c, StageParams& p);
+// multiscale window (asd_mm.cu)
+size_t mm_workspace_bytes(const Ctx& c, const int32_t mcx[2]);
+asd_status mm_enable(Ctx& c, const asd_mm_desc& d, void* ws, size_t bytes);
+void mm_free(Ctx& c);
+asd_status mm_before_step(Ctx& c);                            // exchange + RK4 step when the cadence says so
+void mm_restart_cadence(Ctx& c);
+const float* mm_edge_field(const Ctx& c);
+asd_status mm_set_fields_host(Ctx& c, int side, const float* T, const float* Bx, const float* By, const float* Bz);
+asd_status mm_set_m_host(Ctx& c, int side, const float* m);
+asd_status mm_get_m_host(Ctx& c, int side, float* m);
+void mm_dims(const Ctx& c, int side, int64_t dims[3]);
+asd_status mm_shift_prepare(Ctx& c, int pc);
+const float* mm_shift_frames(const Ctx& c);
+asd_status mm_shift_finish(Ctx& c, int pc);
+asd_status launch_shift_mm(Ctx& c, int32_t p);                // asd_shift.cu: whole-cell shift of a multiscale window
 asd_status launch_shift(Ctx& c, int32_t p);
 asd_status launch_cell_frames(Ctx& c);
 asd_status launch_track_end_pass(Ctx& c);

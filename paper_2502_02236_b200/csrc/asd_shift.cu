@@ -76,7 +76,7 @@ __global__ void move_planes_v4(const float4* __restrict__ sx, const float4* __re
 // One thread per site of the incoming planes (window planes nx-p .. nx-1 AFTER the move).
 __global__ void seed_incoming(float* __restrict__ dx, float* __restrict__ dy, float* __restrict__ dz,
                               const uint32_t* __restrict__ col_track, const float* __restrict__ cell_frame,
-                              ShiftGeom g, PhiloxKey key, uint32_t pass_lo, uint32_t pass_hi) {
+                              ShiftGeom g, PhiloxKey key, uint32_t pass_lo, uint32_t pass_hi, int64_t cx_sub = 0) {
   const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= (int64_t)g.p * g.plane) return;
   const int di = (int)(t / g.plane);
@@ -86,7 +86,8 @@ __global__ void seed_incoming(float* __restrict__ dx, float* __restrict__ dy, fl
   const int64_t gx = g.x0 + g.p + i;                   // its global plane
   const int64_t l = g.lead + ((int64_t)i * g.nz + k) * g.nyp + j;
   if ((col_track[gx * g.ny + j] & 0xFFFFu) == 0u) { dx[l] = 0.0f; dy[l] = 0.0f; dz[l] = 0.0f; return; }
-  const int64_t c = ((gx / g.mx) * g.ncy + (j / g.my)) * g.ncz + (k / g.mz);
+  // cell_frame is indexed by track macrocell, or (cx_sub != 0) by the cells of the mesh columns the planes come from
+  const int64_t c = ((gx / g.mx - cx_sub) * g.ncy + (j / g.my)) * g.ncz + (k / g.mz);
   const float* f = cell_frame + 12 * c;
   const float theta_max = f[0];
   uint32_t r[4];
@@ -258,6 +259,33 @@ asd_status launch_track_read_scan(Ctx& c, double y_r, double sigma_x, double sig
 asd_status launch_cell_frames(Ctx& c) {
   cell_frames_kernel<<<nblocks(c.ncell, 128), 128, 0, c.stream>>>(c.init_mean, c.cell_frame, c.ncell);
   ASD_LAUNCH_CHECK(c, "cell_frames");
+  return ASD_OK;
+}
+
+// Shift of a multiscale window by p = pc * mx planes (reading M10; Fig. 1 of the paper): trailing mesh
+// -> track, outgoing atoms -> trailing mesh (Eq. (6)), atoms move, leading mesh -> incoming atoms (cone about m with
+// magnitude m_e), both meshes move, track ahead -> leading mesh.
+asd_status launch_shift_mm(Ctx& c, int32_t p) {
+  const int pc = p / c.d.macro[0];
+  { const asd_status st = mm_shift_prepare(c, pc); if (st != ASD_OK) return st; }
+  const ShiftGeom g = shift_geom(c, p);
+  const Vec3Ptr S = c.S(), St = c.St();
+  const int64_t planep = (int64_t)c.d.nz * c.nyp;
+  const int64_t off = (int64_t)p * planep, n_keep = c.nrows * c.nyp - off;
+  if (n_keep > 0) {
+    move_planes_v4<<<nblocks(n_keep / 4, 256), 256, 0, c.stream>>>(
+        (const float4*)(S.x + c.lead), (const float4*)(S.y + c.lead), (const float4*)(S.z + c.lead),
+        (float4*)(St.x + c.lead), (float4*)(St.y + c.lead), (float4*)(St.z + c.lead), off / 4, n_keep / 4);
+    ASD_LAUNCH_CHECK(c, "move_planes");
+  }
+  seed_incoming<<<nblocks((int64_t)p * c.plane, 256), 256, 0, c.stream>>>(
+      St.x, St.y, St.z, c.col, mm_shift_frames(c), g, expand_key(c.d.seed), (uint32_t)((uint64_t)c.pass & 0xFFFFFFFFull),
+      (uint32_t)((uint64_t)c.pass >> 32), (c.x0 + c.d.nx) / c.d.macro[0]);
+  ASD_LAUNCH_CHECK(c, "seed_incoming(from the leading mesh)");
+  { const asd_status st = mm_shift_finish(c, pc); if (st != ASD_OK) return st; }   // still at the old window origin
+  { const int t = c.aS; c.aS = c.aSt; c.aSt = t; }
+  c.x0 += p;
+  c.shift += 1;
   return ASD_OK;
 }
 
