@@ -250,9 +250,13 @@ class Run:
         hps, N, w = self.hps, self.N, self.w
         heun_steps = hps * t["steps"]
         per_step = t["heun_launches"] / max(1, heun_steps)            # kernels per Heun step: 1 fused, 2 stage kernels
-        fused = per_step < 1.5 and self.ell_w == 0
+        persistent = per_step < 0.5                                     # all Heun steps of a batch in one cluster launch
+        fused = per_step < 1.5 and self.ell_w == 0 and not persistent
         avg_launch_s = t["heun_ms"] * 1e-3 / max(1, t["heun_launches"])
-        if fused:
+        if persistent:
+            name = "heun_persistent (%d Heun steps per launch, lattice resident in distributed shared memory)" % hps
+            alg, cap = 40.0 * N, "heun_persistent"                      # HBM bytes per LAUNCH: in and out once
+        elif fused:
             name, alg = "heun_fused (one kernel per Heun step, 40 B/site)", FUSED_BYTES_PER_SITE_STEP * N
             cap = "heun_fused"
         elif self.ell_w:

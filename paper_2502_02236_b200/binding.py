@@ -13,7 +13,7 @@ from typing import Optional, Sequence
 import numpy as np
 
 ASD_SC, ASD_L10_FE = 0, 1
-KERNEL_AUTO, KERNEL_GENERAL, KERNEL_FAST, KERNEL_TMA, KERNEL_FUSED = 0, 1, 2, 3, 4
+KERNEL_AUTO, KERNEL_GENERAL, KERNEL_FAST, KERNEL_TMA, KERNEL_FUSED, KERNEL_PERSISTENT = 0, 1, 2, 3, 4, 5
 GRAPH_AUTO, GRAPH_OFF, GRAPH_ON = 0, 1, 2
 _STATUS = {0: "ASD_OK", 1: "ASD_EINVAL", 2: "ASD_ENOMEM", 3: "ASD_ECUDA", 4: "ASD_ESTATE", 5: "ASD_EUNSUPPORTED"}
 

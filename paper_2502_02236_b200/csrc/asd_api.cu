@@ -385,8 +385,10 @@ asd_status asd_step_heun(asd_ctx* ctx, int64_t n) {
 asd_status asd_set_kernel(asd_ctx* ctx, int32_t variant) {
   CTX_OR_RETURN(ctx);
   if (variant != ASD_KERNEL_AUTO && variant != ASD_KERNEL_GENERAL && variant != ASD_KERNEL_FAST &&
-      variant != ASD_KERNEL_TMA && variant != ASD_KERNEL_FUSED)
+      variant != ASD_KERNEL_TMA && variant != ASD_KERNEL_FUSED && variant != ASD_KERNEL_PERSISTENT)
     return fail(c, ASD_EINVAL, "asd_set_kernel: unknown variant");
+  if (variant == ASD_KERNEL_PERSISTENT && !heun_persist_supported(c))
+    return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: the persistent cluster needs built-in shells, ny % 4 == 0, grains that do not touch, no demagnetising field or meshes, and x-slabs that fit a CTA");
   if (variant == ASD_KERNEL_FUSED && (!heun_fused_supported(c) || c.demag || !fused_plan(c)))
     return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: the fused step needs what the film kernel needs, no demagnetising field, and a strip plan that fits in shared memory");
   if (variant == ASD_KERNEL_TMA && c.mm) return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: the staged film kernel does not take a multiscale window");

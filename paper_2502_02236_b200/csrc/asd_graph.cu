@@ -92,6 +92,8 @@ asd_status launch_heun(Ctx& c, int64_t n) {
   c.launch_stream = c.stream;
   const bool use = !c.demag && !c.mm &&         // the demag pipeline and the mesh steps are launched plainly
                    c.kernel_variant != ASD_KERNEL_FUSED &&   // the fused step swaps the spin buffers every step
+                   c.kernel_variant != ASD_KERNEL_PERSISTENT &&
+                   !(c.kernel_variant == ASD_KERNEL_AUTO && c.N <= (1 << 14) && heun_persist_supported(c)) &&   // one launch already
                    (c.graph_mode == ASD_GRAPH_ON || (c.graph_mode == ASD_GRAPH_AUTO && c.N <= kAutoMaxSites));
   while (use && n >= 2) {
     const int64_t k = n < kBatch ? n : kBatch;

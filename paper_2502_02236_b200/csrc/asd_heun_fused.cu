@@ -117,7 +117,7 @@ constexpr uint32_t kGpRing = 8;   // planes of per-group anisotropy parameters k
 
 // NZ_T / BY_T != 0: film thickness and strip width are compile-time constants (every shared-memory offset becomes an
 // immediate of its LDS / STS); 0: taken from the parameter block.
-template <int LAT, int NT, int MINB, int NZ_T, int BY_T>
+template <int LAT, int NT, int MINB, int NZ_T, int BY_T, bool MM = false>
 __global__ void __launch_bounds__(NT, MINB)
 heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUtensorMap mapF, const FusedParams p) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -342,7 +342,7 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
             Bn[2][v] = fmaf(sgs, xi[v][2], sscale * bz[v]);
           }
         }
-        if (p.edgeB) {
+        if (MM) {
           // multiscale window: the held mesh directions beyond the first / last plane enter Eq. (2) of BOTH stages as a
           // constant field, so they ride with the stage-independent part (asd_mm.cu)
           const int q = i0 - 1 + m;
@@ -554,7 +554,7 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
               Bex[c] = fmaf(p.j3s, s3, fmaf(p.j2s, zs[c], p.j1s * (xs + ys)));
             }
           }
-          if (p.edgeB) {
+          if (MM) {
 #pragma unroll 1
             for (int side = 0; side < 2; ++side) {
               if (q != (side == 0 ? 0 : p.nx - 1)) continue;
@@ -606,7 +606,13 @@ constexpr int kNumShapes = 2;
 
 // Film thickness 27 planes with 32-site strips (BASELINE configs 1, 3, 4) has its own instance with compile-time shared-
 // memory offsets; everything else takes the generic one.
-FusedKernel kernel_for(int lattice, int shape, int nz, int by) {
+FusedKernel kernel_for(int lattice, int shape, int nz, int by, bool mm = false) {
+  if (mm) {                                             // multiscale window: the 256 x 2 shape only
+    if (shape != 0) return nullptr;
+    if (nz == 27 && by == 32)
+      return lattice == ASD_SC ? heun_fused<LAT_SC, 256, 2, 27, 32, true> : heun_fused<LAT_L10, 256, 2, 27, 32, true>;
+    return lattice == ASD_SC ? heun_fused<LAT_SC, 256, 2, 0, 0, true> : heun_fused<LAT_L10, 256, 2, 0, 0, true>;
+  }
   if (shape == 0 && nz == 27 && by == 32)
     return lattice == ASD_SC ? heun_fused<LAT_SC, 256, 2, 27, 32> : heun_fused<LAT_L10, 256, 2, 27, 32>;
   if (lattice == ASD_SC) return shape == 0 ? heun_fused<LAT_SC, 256, 2, 0, 0> : heun_fused<LAT_SC, 512, 1, 0, 0>;
@@ -626,6 +632,7 @@ uint32_t plan_smem(int nz, int by, uint32_t& slot_pitch) {
 struct FusedPlan {
   CUtensorMap mapS, mapF;
   FusedKernel kern = nullptr;
+  FusedKernel kern_mm = nullptr;   // the instance that adds the mesh exchange field on planes 0 / nx-1 (asd_mm.cu); may be null
   int32_t BY = 0, G = 0, nstrips = 0, CX = 0, nchunks = 0, threads = 0, n_main = 0, ctas_per_sm = 0;
   uint32_t slot_pitch = 0, smem_bytes = 0;
 };
@@ -685,6 +692,12 @@ bool build_plan(Ctx& c, FusedPlan& pl) {
   pl.threads = pl.n_main + round_up32(nz);
   pl.smem_bytes = plan_smem(nz, pl.BY, pl.slot_pitch);
   pl.kern = kernel_for(c.d.lattice, best.shape, nz, pl.BY);
+  pl.kern_mm = kernel_for(c.d.lattice, best.shape, nz, pl.BY, true);
+  if (pl.kern_mm && cudaFuncSetAttribute((const void*)pl.kern_mm, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)pl.smem_bytes) != cudaSuccess) {
+    cudaGetLastError();
+    pl.kern_mm = nullptr;
+  }
   int bps = 0;
   if (cudaFuncSetAttribute((const void*)pl.kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes) != cudaSuccess ||
       cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, (const void*)pl.kern, pl.threads, pl.smem_bytes) != cudaSuccess ||
@@ -718,6 +731,8 @@ bool build_plan(Ctx& c, FusedPlan& pl) {
 }
 
 }  // namespace
+
+bool heun_fused_takes_mm(Ctx& c) { const FusedPlan* pl = fused_plan(c); return pl && pl->kern_mm; }
 
 FusedPlan* fused_plan(Ctx& c) {
   if (!c.fused_plan_tried) {
@@ -758,7 +773,8 @@ asd_status launch_heun_fused(Ctx& c, StageParams& p) {
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr; cfg.numAttrs = 1;
-  cudaLaunchKernelEx(&cfg, pl->kern, pl->mapS, pl->mapF, f);
+  if (f.edgeB && !pl->kern_mm) return ASD_EUNSUPPORTED;
+  cudaLaunchKernelEx(&cfg, f.edgeB ? pl->kern_mm : pl->kern, pl->mapS, pl->mapF, f);
   ASD_LAUNCH_CHECK(c, "heun step (fused)");
   const int t = c.aS; c.aS = c.aSt; c.aSt = t;
   return ASD_OK;

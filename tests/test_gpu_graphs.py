@@ -39,7 +39,11 @@ def test_graph_replay_is_bit_identical_to_plain_launches(lattice, kernel):
 
 def test_cfg0_1000_steps_through_graphs_matches_oracle():
     """cfg0 (4096 spins) is launch-bound: ASD_GRAPH_AUTO replays graphs there.  Same tolerance as the plain path."""
+    import paper_2502_02236_b200 as asd
     w = ai.make_config(0, uniform_T=0.0)
     o, g = oracle_from_workload(w), gpu_from_workload(w)
+    g.set_kernel(asd.KERNEL_GENERAL)         # AUTO would take the persistent cluster (one launch, no graph) on 4096 sites
+    n0 = g.launch_count()
     o.step_heun(1000); g.step_heun(1000)
+    assert g.launch_count() - n0 >= 2000     # 2000 kernel nodes replayed (+ one set_dyn per replay)
     assert max_abs_diff(g, o) <= 1e-4
