@@ -184,7 +184,7 @@ def _captured(workload: str, kernel_prefix: str):
 class Run:
     """One context on one workload: warm-up, device-timed bench steps (Heun batches + the schedule's shifts)."""
 
-    def __init__(self, asd, torch, w, device, hps, kernel="auto", ell=False, demag=False, demag_every=0):
+    def __init__(self, asd, torch, w, device, hps, kernel="auto", ell=False, demag=False, demag_every=0, multiscale=None):
         self.asd, self.torch, self.w, self.hps = asd, torch, w, hps
         self.N = w.n_sites
         table = None
@@ -198,9 +198,11 @@ class Run:
         if demag:
             self.ctx.enable_demag([a * 1e-9 for a in w.spacing_nm])
             self.ctx.set_demag_every(demag_every)
+        if multiscale is not None:                   # micromagnetic meshes either side
+            ai.apply_multiscale(self.ctx, multiscale)
         if kernel != "auto":
             self.ctx.set_kernel({"general": asd.KERNEL_GENERAL, "fast": asd.KERNEL_FAST, "tma": asd.KERNEL_TMA,
-                                 "fused": asd.KERNEL_FUSED}[kernel])
+                                 "fused": asd.KERNEL_FUSED, "persistent": asd.KERNEL_PERSISTENT}[kernel])
         pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory()
         self.hT, self.hBx, self.hBy, self.hBz = pin(w.T), pin(w.Bx), pin(w.By), pin(w.Bz)
         self.ctx.set_spins_host(pin(w.sx), pin(w.sy), pin(w.sz))
@@ -419,6 +421,10 @@ def secondary(asd, torch, device, args, peak, peak_src):
                 w4 = w4 or _workload(4)
                 import copy
                 w = copy.copy(w4)
+            elif cfg == "multiscale":
+                # [48-cell mesh | 336 x 200 x 27 SC atoms | 48-cell mesh]: the paper's three equal parts on cfg3's film
+                kw["multiscale"] = ai.multiscale_film(ai.SC, every=kw.pop("every", 20))
+                w = kw["multiscale"].w
             else:
                 w = _workload(cfg)
             run = Run(asd, torch, w, device, hps, **kw)
@@ -430,7 +436,10 @@ def secondary(asd, torch, device, args, peak, peak_src):
                    "unit": UNIT, "us_per_heun_step": t["heun_ms"] * 1e3 / heun_steps, "kernel": r["kernel"],
                    "avg_launch_us": r["avg_launch_us"], "frac": r["frac"], "frac_survey_floor": r["frac_survey_floor"],
                    "shifts_in_timed_region": t["shifts"]}
-            if kw.get("demag"):
+            if kw.get("multiscale") is not None:
+                rec.update(kernel="Heun kernels + mesh kernels (exchange, edge field, m_e, 4 RK4 stages per mesh step)",
+                           avg_launch_us=None, frac=None)
+            elif kw.get("demag"):
                 # the launches of a step include the demagnetising-field pipeline: no single-kernel fraction to quote
                 rec.update(kernel="stage kernels + demagnetising-field pipeline", avg_launch_us=None, frac=None)
             elif w.n_sites < (1 << 18):
@@ -447,7 +456,11 @@ def secondary(asd, torch, device, args, peak, peak_src):
     one("cfg4 as a general ELL table, W = 10, per-pair J (no shifts)", 4, ell=True)
     one("cfg4 with the demagnetising field recomputed in every stage", 4, demag=True, demag_every=0)
     one("cfg3 SC 400x200x27", 3)
-    one("cfg0 SC 16^3 periodic (launch-bound: us per Heun step is the figure)", 0, hps=1000, steps=3)
+    one("cfg0 SC 16^3 periodic on the persistent cluster (us per Heun step is the figure)", 0, hps=1000, steps=3)
+    one("cfg0 through CUDA-graph replay of the stage kernels (round 1's path)", 0, hps=1000, steps=3, kernel="general")
+    one("multiscale window: 48-cell LLG mesh | SC 336x200x27 atoms | 48-cell mesh, mesh RK4 step every 20 Heun steps",
+        "multiscale", every=20)
+    one("multiscale window, meshes in lock-step (every Heun step)", "multiscale", every=1)
     return out
 
 
@@ -545,7 +558,7 @@ def main():
                     help="switch the demagnetising field on (Eq. (6)-(7): coarse-graining + FFT convolution per stage)")
     ap.add_argument("--demag-every", type=int, default=0,
                     help="0: demag field recomputed in every Heun stage; P >= 1: every P-th step, held in between")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "general", "fast", "tma", "fused"],
+    ap.add_argument("--kernel", default="auto", choices=["auto", "general", "fast", "tma", "fused", "persistent"],
                     help="stage-kernel variant (asd_set_kernel); auto = the library's choice")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

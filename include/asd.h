@@ -264,6 +264,27 @@ ASD_API asd_status asd_mm_set_fields_host(asd_ctx *ctx, int32_t side, const floa
 ASD_API asd_status asd_mm_set_m_host(asd_ctx *ctx, int32_t side, const float *m);
 ASD_API asd_status asd_mm_get_m_host(asd_ctx *ctx, int32_t side, float *m);
 
+/* ---- Slab decomposition across devices ("implemented for ... multiple GPUs"; DESIGN.md
+ * sec. 9) --------------------------------------------------------------------------------------------------------------
+ * A window cut along x into slabs is just one ordinary context per slab whose window holds the slab's own planes plus
+ * H >= 2 ghost planes towards each neighbour: one Heun step spoils two more ghost planes from the outside in (the
+ * predictor of a plane needs its x neighbours, the corrector the predictor of its x neighbours), so H ghost planes last
+ * H / 2 steps, and the own planes stay exact -- the noise is keyed by GLOBAL site, so a slab computes for a ghost atom
+ * what its owner computes.  Between steps the owners' planes are copied over the ghosts; these two calls are what that
+ * copy needs, and nothing else in the library knows about slabs (paper_2502_02236_b200/slab.py drives it: device-to-
+ * device copies between contexts of one process, or NCCL send/recv between ranks).
+ *   asd_planes_view            DEVICE pointer to the storage of planes i0 .. i0+n-1 of component comp (0, 1, 2) of the
+ *                              CURRENT spins: *count = n * nz * row_stride floats, contiguous, rows of ny sites at the
+ *                              library's padded row stride (the pad floats are zero and must stay zero; two contexts
+ *                              with equal ny and nz have equal strides, so planes are copied verbatim).  The pointer is
+ *                              valid until the next asd_step_heun / asd_shift_window / asd_set_spins on this context
+ *                              (the spins change buffers): ask again after each.  Writing through it is the caller's
+ *                              responsibility: vacant sites must receive zeros (a peer's copy of the same planes does).
+ *   asd_magnetisation_planes   sum of S over the magnetic sites of planes i0 .. i0+n-1 and their number (fp64, same
+ *                              deterministic reduction as asd_magnetisation); synchronises. */
+ASD_API asd_status asd_planes_view(asd_ctx *ctx, int32_t comp, int32_t i0, int32_t n, float **d_ptr, size_t *count);
+ASD_API asd_status asd_magnetisation_planes(asd_ctx *ctx, int32_t i0, int32_t n, double sum[3], double *n_magnetic);
+
 /* Counters for bit-exact checkpoint / resume (Philox is counter based: there is no RNG state). */
 ASD_API asd_status asd_get_counters(const asd_ctx *ctx, int64_t *step, int64_t *shift, int64_t *x0, int64_t *pass);
 ASD_API asd_status asd_set_counters(asd_ctx *ctx, int64_t step, int64_t shift, int64_t pass);

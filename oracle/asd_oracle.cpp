@@ -877,6 +877,19 @@ void orc_set_spins(void* h, const float* sx, const float* sy, const float* sz) {
       }
 }
 
+// fp64 spins as they are (vacant -> 0): for harnesses that move planes between oracles (slab decomposition tests).
+void orc_set_spins_f64(void* h, const double* sx, const double* sy, const double* sz) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  o.demag_age = 0; o.mm_age = 0;
+  for (int i = 0; i < o.nx; ++i)
+    for (int k = 0; k < o.nz; ++k)
+      for (int j = 0; j < o.ny; ++j) {
+        const int64_t l = o.site(i, k, j);
+        const bool mag = o.grain_of(i, j) >= 0;
+        o.sx[l] = mag ? sx[l] : 0.0; o.sy[l] = mag ? sy[l] : 0.0; o.sz[l] = mag ? sz[l] : 0.0;
+      }
+}
+
 void orc_get_spins(void* h, double* sx, double* sy, double* sz) {
   Oracle& o = *static_cast<Oracle*>(h);
   std::memcpy(sx, o.sx.data(), sizeof(double) * (size_t)o.N);

@@ -80,6 +80,7 @@ def lib():
         ip64 = C.POINTER(C.c_int64)
         L.orc_set_spins.argtypes = [C.c_void_p, fp, fp, fp]
         L.orc_get_spins.argtypes = [C.c_void_p, dp, dp, dp]
+        L.orc_set_spins_f64.argtypes = [C.c_void_p, dp, dp, dp]
         L.orc_set_fields.argtypes = [C.c_void_p, fp, fp, fp, fp]
         L.orc_set_field_scale.argtypes = [C.c_void_p, C.c_float]
         L.orc_step_heun.argtypes = [C.c_void_p, C.c_int64]
@@ -280,6 +281,11 @@ class Oracle:
         sx, sy, sz = _f32(sx).reshape(-1), _f32(sy).reshape(-1), _f32(sz).reshape(-1)
         assert sx.size == self.N and sy.size == self.N and sz.size == self.N
         lib().orc_set_spins(self._h, _ptr(sx, C.c_float), _ptr(sy, C.c_float), _ptr(sz, C.c_float))
+
+    def set_spins_f64(self, S):
+        """S: [3, N] float64, stored as given (vacant sites 0)."""
+        S = np.ascontiguousarray(S, dtype=np.float64).reshape(3, self.N)
+        lib().orc_set_spins_f64(self._h, _ptr(S[0], C.c_double), _ptr(S[1], C.c_double), _ptr(S[2], C.c_double))
 
     def get_spins(self) -> np.ndarray:
         """Returns [3, N] float64."""

@@ -26,7 +26,7 @@ EXPORTED_SYMBOLS = [
     "asd_track_dims", "asd_track_set_init", "asd_track_get",
     "asd_track_end_pass", "asd_track_begin_pass", "asd_track_read_scan",
     "asd_mm_workspace_bytes", "asd_mm_enable", "asd_mm_dims", "asd_mm_set_fields_host", "asd_mm_set_m_host",
-    "asd_mm_get_m_host", "asd_get_counters", "asd_set_counters",
+    "asd_mm_get_m_host", "asd_planes_view", "asd_magnetisation_planes", "asd_get_counters", "asd_set_counters",
     "asd_launch_count", "asd_last_error", "asd_version",
 ]
 
@@ -129,6 +129,8 @@ def load_library(build_if_missing: bool = True):
     L.asd_mm_set_fields_host.argtypes = [C.c_void_p, C.c_int32, fp, fp, fp, fp]
     L.asd_mm_set_m_host.argtypes = [C.c_void_p, C.c_int32, fp]
     L.asd_mm_get_m_host.argtypes = [C.c_void_p, C.c_int32, fp]
+    L.asd_planes_view.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_void_p), C.POINTER(C.c_size_t)]
+    L.asd_magnetisation_planes.argtypes = [C.c_void_p, C.c_int32, C.c_int32, dp, dp]
     L.asd_get_counters.argtypes = [C.c_void_p, ip64, ip64, ip64, ip64]
     L.asd_set_counters.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_int64]
     L.asd_launch_count.restype = C.c_int64
@@ -395,6 +397,22 @@ class Context:
                                              C.c_double(x_first), C.c_double(x_step), C.c_int64(count),
                                              out.ctypes.data_as(C.POINTER(C.c_double))))
         return out
+
+    # ---- slab decomposition ----
+    def planes_view(self, comp: int, i0: int, n: int):
+        """asd_planes_view as a torch tensor over the context's own workspace (no copy): [n * nz * row_stride] fp32."""
+        import torch
+        ptr, cnt = C.c_void_p(), C.c_size_t()
+        self._ck(self._L.asd_planes_view(self._h, C.c_int32(comp), C.c_int32(i0), C.c_int32(n), C.byref(ptr), C.byref(cnt)))
+        off = ptr.value - self.workspace.data_ptr()
+        return self.workspace[off:off + 4 * cnt.value].view(torch.float32)
+
+    def magnetisation_planes(self, i0: int, n: int):
+        s = np.zeros(3)
+        cnt = C.c_double(0)
+        self._ck(self._L.asd_magnetisation_planes(self._h, C.c_int32(i0), C.c_int32(n),
+                                                  s.ctypes.data_as(C.POINTER(C.c_double)), C.byref(cnt)))
+        return s, cnt.value
 
     # ---- multiscale window ----
     def mm_enable(self, mcx, every, Ms0, A0, K0, Tc, cell_grain, spacing_m):

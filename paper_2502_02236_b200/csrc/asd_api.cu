@@ -472,6 +472,31 @@ asd_status asd_magnetisation(asd_ctx* ctx, double m[3], double* n_magnetic) {
   return ASD_OK;
 }
 
+asd_status asd_magnetisation_planes(asd_ctx* ctx, int32_t i0, int32_t n, double sum[3], double* n_magnetic) {
+  CTX_OR_RETURN(ctx);
+  if (!sum) return fail(c, ASD_EINVAL, "asd_magnetisation_planes: sum is NULL");
+  if (i0 < 0 || n < 1 || (int64_t)i0 + n > c.d.nx) return fail(c, ASD_EINVAL, "asd_magnetisation_planes: planes outside the window");
+  double o[4];
+  const asd_status s = launch_magnetisation(c, o, i0, n);
+  if (s != ASD_OK) return s;
+  sum[0] = o[0]; sum[1] = o[1]; sum[2] = o[2];
+  if (n_magnetic) *n_magnetic = o[3];
+  return ASD_OK;
+}
+
+asd_status asd_planes_view(asd_ctx* ctx, int32_t comp, int32_t i0, int32_t n, float** d_ptr, size_t* count) {
+  CTX_OR_RETURN(ctx);
+  if (!d_ptr || !count) return fail(c, ASD_EINVAL, "asd_planes_view: NULL output pointer");
+  if (comp < 0 || comp > 2 || i0 < 0 || n < 1 || (int64_t)i0 + n > c.d.nx)
+    return fail(c, ASD_EINVAL, "asd_planes_view: component must be 0..2 and the planes inside the window");
+  const size_t planep = (size_t)c.d.nz * (size_t)c.nyp;
+  *d_ptr = c.arr(c.aS + comp) + c.lead + (size_t)i0 * planep;
+  *count = (size_t)n * planep;
+  c.demag_age = 0;                             // the caller is about to change spins behind the library's back
+  mm_restart_cadence(c);
+  return ASD_OK;
+}
+
 asd_status asd_grain_magnetisation(asd_ctx* ctx, double* m) {
   CTX_OR_RETURN(ctx);
   if (!m) return fail(c, ASD_EINVAL, "asd_grain_magnetisation: m is NULL");

@@ -269,7 +269,7 @@ asd_status launch_track_end_pass(Ctx& c);
 asd_status launch_track_begin_pass(Ctx& c, int64_t x0_new);
 asd_status launch_track_read_scan(Ctx& c, double y_r, double sigma_x, double sigma_y, double x_first, double x_step,
                                   int64_t count, double* out_host);
-asd_status launch_magnetisation(Ctx& c, double out4[4]);
+asd_status launch_magnetisation(Ctx& c, double out4[4], int32_t i0 = -1, int32_t n = 0);   // i0 < 0: the whole window
 asd_status launch_grain_magnetisation(Ctx& c, double* m_host);
 asd_status launch_ell_transpose(Ctx& c, const int32_t* idx_site_major, const float* J_site_major);
 

@@ -70,12 +70,17 @@ __global__ void grain_accumulate(const float* __restrict__ sx, const float* __re
 
 }  // namespace
 
-asd_status launch_magnetisation(Ctx& c, double out4[4]) {
-  const int nb = (int)min((int64_t)kMaxPartialBlocks - 1, max((int64_t)1, c.N / 4096));
+asd_status launch_magnetisation(Ctx& c, double out4[4], int32_t i0, int32_t n) {
+  const int64_t planep = (int64_t)c.d.nz * c.nyp;
+  const int64_t first = i0 < 0 ? 0 : (int64_t)c.lead + (int64_t)i0 * planep;       // i0 < 0: the whole padded array
+  const int64_t count = i0 < 0 ? c.Np : (int64_t)n * planep;
+  const int64_t ncol = i0 < 0 ? (int64_t)c.d.nx * c.d.ny : (int64_t)n * c.d.ny;
+  const uint32_t* col = c.col_win() + (i0 < 0 ? 0 : (int64_t)i0 * c.d.ny);
+  const int nb = (int)min((int64_t)kMaxPartialBlocks - 1, max((int64_t)1, count / 4096));
   double* final_slot = c.partials + 4 * (int64_t)(kMaxPartialBlocks - 1);
   // the padded arrays are summed whole: pads and vacant sites hold exact zeros
   const Vec3Ptr S = c.S();
-  mag_partial<<<nb, 256, 0, c.stream>>>(S.x, S.y, S.z, c.col_win(), c.Np, (int64_t)c.d.nx * c.d.ny, c.partials);
+  mag_partial<<<nb, 256, 0, c.stream>>>(S.x + first, S.y + first, S.z + first, col, count, ncol, c.partials);
   ASD_LAUNCH_CHECK(c, "mag_partial");
   mag_final<<<1, 128, 0, c.stream>>>(c.partials, nb, final_slot);
   ASD_LAUNCH_CHECK(c, "mag_final");

@@ -47,3 +47,18 @@ def test_cfg0_1000_steps_through_graphs_matches_oracle():
     o.step_heun(1000); g.step_heun(1000)
     assert g.launch_count() - n0 >= 2000     # 2000 kernel nodes replayed (+ one set_dyn per replay)
     assert max_abs_diff(g, o) <= 1e-4
+
+
+@pytest.mark.parametrize("kernel", ["general", "fast"])
+def test_dependent_launches_match_serialised_graph_edges_over_many_steps(kernel):
+    """The stage kernels are launched with programmatic dependent launch and read what the previous grid wrote through
+    the read-only data path after their griddepcontrol.wait.  On a lattice this small three grids
+    are co-resident.  Recorded graphs keep plain (fully serialising) edges: 3000 steps of both must agree bit for bit."""
+    import paper_2502_02236_b200 as asd
+    k = {"general": asd.KERNEL_GENERAL, "fast": asd.KERNEL_FAST}[kernel]
+    w = ai.small_film(ai.L10, 16, 32, 6, tilt_deg=20.0)
+    a, b = gpu_from_workload(w), gpu_from_workload(w)
+    for g, mode in ((a, asd.GRAPH_OFF), (b, asd.GRAPH_ON)):
+        g.set_kernel(k); g.set_graph_mode(mode)
+        g.step_heun(3000)
+    assert np.array_equal(a.get_spins_host(), b.get_spins_host())
