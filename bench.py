@@ -314,10 +314,18 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     device = f"cuda:{local}"
-    w = _workload(args.config, seed_offset=rank)
+    msw = None
+    if args.multiscale:
+        # [48-cell LLG mesh | atomistic mesh | 48-cell mesh] on the film of config 3 (SC) or 4 (L1_0); no shifts (a
+        # multiscale window moves by whole 2 nm cells, not by the 1 nm of the configs' schedule)
+        msw = ai.multiscale_film(ai.L10 if args.config == 4 else ai.SC, every=args.mm_every, seed=1 + rank)
+        w = msw.w
+    else:
+        w = _workload(args.config, seed_offset=rank)
     N = w.n_sites
     hps = args.heun_per_step
-    run = Run(asd, torch, w, device, hps, kernel=args.kernel, ell=args.ell, demag=args.demag, demag_every=args.demag_every)
+    run = Run(asd, torch, w, device, hps, kernel=args.kernel, ell=args.ell, demag=args.demag, demag_every=args.demag_every,
+              multiscale=msw)
     ctx, dev = run.ctx, run.ctx.device
     run.start(args.warmup, args.steps)
     barrier()
@@ -370,7 +378,7 @@ def run_ours(args):
         "config": {"workload": w.name, "sites": N, "heun_steps_per_step": hps, "shifts_in_timed_region": t["shifts"],
                    "shift_every_heun_steps": w.shift_every, "dt": w.dt, "parallelism": f"replicas x{world}",
                    "ell_width": run.ell_w, "demag": bool(args.demag), "demag_every": args.demag_every if args.demag else None,
-                   "kernel": args.kernel,
+                   "kernel": args.kernel, "multiscale": ({"mesh_cells": list(msw.mcx), "every": msw.every} if msw else None),
                    "l2": "working set (13 fp32 arrays/site = %.0f MB) exceeds the 126 MB L2" % (13 * 4 * N / 1e6)},
         "clocks": clocks, "gpu_launches": int(t["launches"]),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 16 * N, "d2h_bytes_per_step": 32,
@@ -558,6 +566,9 @@ def main():
                     help="switch the demagnetising field on (Eq. (6)-(7): coarse-graining + FFT convolution per stage)")
     ap.add_argument("--demag-every", type=int, default=0,
                     help="0: demag field recomputed in every Heun stage; P >= 1: every P-th step, held in between")
+    ap.add_argument("--multiscale", action="store_true",
+                    help="the multiscale window: a micromagnetic LLG mesh either side of the atomistic mesh (DESIGN.md sec. 14)")
+    ap.add_argument("--mm-every", type=int, default=20, help="Heun steps per RK4 step of the meshes")
     ap.add_argument("--kernel", default="auto", choices=["auto", "general", "fast", "tma", "fused", "persistent"],
                     help="stage-kernel variant (asd_set_kernel); auto = the library's choice")
     args = ap.parse_args()

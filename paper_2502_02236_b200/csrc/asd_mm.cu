@@ -50,6 +50,10 @@ struct MmPlan {
   float* frames = nullptr;    // [maxpc*ncol*12] cone frames of the leading mesh's outgoing columns
   float* stage = nullptr;     // host uploads land here: [4][max(n0, n1)]
   int32_t maxpc = 0;
+  // m_e and alpha depend on T, B_app, the field scale and the grain under each cell: recomputed (fp64 bisection, the
+  // costliest mesh kernel) only when one of those has changed since the last time
+  bool params_dirty = true;
+  float params_scale = 0.f;
 };
 
 namespace {
@@ -472,6 +476,7 @@ asd_status launch_params(Ctx& c) {
   mm_params_kernel<<<nblocks(P.ntot, 128), 128, 0, c.stream>>>(geom(c), P.T, P.B, P.cell_grain, P.Tc, c.scale,
                                                              c.d.mu_s, c.d.lambda, P.me, P.alpha);
   ASD_LAUNCH_CHECK(c, "mm_params");
+  P.params_dirty = false; P.params_scale = c.scale;
   return ASD_OK;
 }
 
@@ -520,7 +525,7 @@ asd_status mm_before_step(Ctx& c) {
   MmPlan& P = *c.mm;
   if (P.age % P.every == 0) {
     asd_status st = launch_exchange(c);
-    if (st == ASD_OK) st = launch_params(c);
+    if (st == ASD_OK && (P.params_dirty || P.params_scale != c.scale)) st = launch_params(c);
     if (st == ASD_OK) st = launch_rk4(c, (double)P.every * c.d.dt);
     if (st != ASD_OK) return st;
   }
@@ -627,6 +632,7 @@ asd_status mm_shift_finish(Ctx& c, int pc) {
   ASD_LAUNCH_CHECK(c, "mm_move");
   ASD_CUDA_TRY(c, cudaMemcpyAsync(P.m, P.ya, 12 * (size_t)P.ntot, cudaMemcpyDeviceToDevice, c.stream));
   P.age = 0;
+  P.params_dirty = true;                                 // other grains now lie under the window-fixed profiles
   return ASD_OK;
 }
 
