@@ -160,19 +160,27 @@ __global__ void __launch_bounds__(NT, 1) heun_persistent(const PersistParams p) 
     }
   };
 
-  for (int s = 0; s < p.nsteps; ++s) {
-    const uint64_t n = p.step0 + (uint64_t)s;
+  // The noise of a step depends on nothing but its counters: it is drawn between the ARRIVAL at the barrier that closes
+  // the previous step and the WAIT for it, so that the barrier's latency hides behind Philox and Box-Muller.
+  float xi[VEC][3];
+  auto draw = [&](uint64_t n) {
     const uint32_t n_lo = (uint32_t)n, n_hi = (uint32_t)(n >> 32);
-    float A[3][VEC], xi[VEC][3];
+#pragma unroll
+    for (int v = 0; v < VEC; ++v) {
+      uint32_t rnd[4];
+      philox_site(p.key, n_lo, n_hi, gsite + (uint64_t)v, 0u, rnd);
+      normals3(rnd, xi[v]);
+    }
+  };
+  draw(p.step0);
+  for (int s = 0; s < p.nsteps; ++s) {
+    float A[3][VEC];
     // ---- predictor: S~ = normalise(S + dt k1), A = S + dt/2 k1 ----
     if (active) {
       float X[3][VEC], Bex[3][VEC];
       exchange(0, X, Bex);
 #pragma unroll
       for (int v = 0; v < VEC; ++v) {
-        uint32_t rnd[4];
-        philox_site(p.key, n_lo, n_hi, gsite + (uint64_t)v, 0u, rnd);
-        normals3(rnd, xi[v]);
         const float Xs[3] = {X[0][v], X[1][v], X[2][v]};
         const float Be[3] = {Bex[0][v], Bex[1][v], Bex[2][v]};
         const float Ba[3] = {Bap[0][v], Bap[1][v], Bap[2][v]};
@@ -202,7 +210,9 @@ __global__ void __launch_bounds__(NT, 1) heun_persistent(const PersistParams p) 
 #pragma unroll
       for (int c = 0; c < 3; ++c) PV<VEC>::st(smem + c * slab + own, X[c]);
     }
-    cluster.sync();                                  // S complete everywhere; nobody reads S~ any more
+    cluster.barrier_arrive();                        // this CTA's share of S is written ...
+    if (s + 1 < p.nsteps) draw(p.step0 + (uint64_t)(s + 1));
+    cluster.barrier_wait();                          // ... S complete everywhere; nobody reads S~ any more
   }
 
   if (active) {
