@@ -449,7 +449,8 @@ def secondary(asd, torch, device, args, peak, peak_src):
                            avg_launch_us=None, frac=None)
             elif kw.get("demag"):
                 # the launches of a step include the demagnetising-field pipeline: no single-kernel fraction to quote
-                rec.update(kernel="stage kernels + demagnetising-field pipeline", avg_launch_us=None, frac=None)
+                rec.update(kernel=("fused Heun step" if kw.get("demag_every") else "stage kernels") +
+                           " + demagnetising-field pipeline", avg_launch_us=None, frac=None)
             elif w.n_sites < (1 << 18):
                 rec.update(frac=None, frac_survey_floor=None, note="launch-bound: no roofline fraction")
             elif 13 * 4 * w.n_sites < 126e6:
@@ -463,6 +464,8 @@ def secondary(asd, torch, device, args, peak, peak_src):
     one("cfg4, two-kernel film kernel (asd_set_kernel FAST)", 4, kernel="fast")
     one("cfg4 as a general ELL table, W = 10, per-pair J (no shifts)", 4, ell=True)
     one("cfg4 with the demagnetising field recomputed in every stage", 4, demag=True, demag_every=0)
+    one("cfg4 with the demagnetising field recomputed once per Heun step and held for both stages (fused step)", 4,
+        demag=True, demag_every=1)
     one("cfg3 SC 400x200x27", 3)
     one("cfg0 SC 16^3 periodic on the persistent cluster (us per Heun step is the figure)", 0, hps=1000, steps=3)
     one("cfg0 through CUDA-graph replay of the stage kernels (round 1's path)", 0, hps=1000, steps=3, kernel="general")

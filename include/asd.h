@@ -162,7 +162,8 @@ ASD_API asd_status asd_set_graph_mode(asd_ctx *ctx, int32_t mode);
  *   B_c = -mu_0 sum_c' N(r_c' - r_c) M_c',  M_c = (mu_s / V) sum_{j in c} S_j   (V = macro[0..2] * spacing, full cell),
  * N = demagnetising tensor of two equal cuboids (Newell et al., the paper's ref. [28]), summed over the macrocells that
  * overlap the window (open boundaries).  Open-boundary lattices with the built-in shells; ASD_KERNEL_TMA and CUDA graphs
- * are not used while it is on.  The caller owns the workspace (DEVICE, 256-byte aligned) for the life of the context.
+ * are not used while it is on; ASD_KERNEL_FUSED (and AUTO's choice of it) needs the held-field scheme of
+ * asd_set_demag_every (every >= 1).  The caller owns the workspace (DEVICE, 256-byte aligned) for the life of the context.
  * The convolution is the library's own (direct sum over the film's macrocell layers, DFT across the film, shared-memory
  * FFT along the track; no FFT library): ASD_EUNSUPPORTED if 3 * (layers of macrocells) fields of the padded track length
  * do not fit in one CTA's shared memory (about 300 macrocell layers x cells along x / 256).

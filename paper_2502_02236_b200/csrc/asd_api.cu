@@ -389,8 +389,8 @@ asd_status asd_set_kernel(asd_ctx* ctx, int32_t variant) {
     return fail(c, ASD_EINVAL, "asd_set_kernel: unknown variant");
   if (variant == ASD_KERNEL_PERSISTENT && !heun_persist_supported(c))
     return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: the persistent cluster needs built-in shells, ny % 4 == 0, grains that do not touch, no demagnetising field or meshes, and x-slabs that fit a CTA");
-  if (variant == ASD_KERNEL_FUSED && (!heun_fused_supported(c) || c.demag || !fused_plan(c)))
-    return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: the fused step needs what the film kernel needs, no demagnetising field, and a strip plan that fits in shared memory");
+  if (variant == ASD_KERNEL_FUSED && (!heun_fused_supported(c) || (c.demag && c.demag_every < 1) || !fused_plan(c)))
+    return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: the fused step needs what the film kernel needs, a strip plan that fits in shared memory, and -- with the demagnetising field on -- the held-field scheme (asd_set_demag_every >= 1)");
   if (variant == ASD_KERNEL_TMA && c.mm) return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: the staged film kernel does not take a multiscale window");
   if (variant == ASD_KERNEL_TMA && (!heun_tma_supported(c) || !tma_plan(c)))
     return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: the staged film kernel needs what the film kernel needs and a strip plan that fits in shared memory");

@@ -32,6 +32,8 @@
 #include <complex>
 #include <vector>
 
+#include <cstdlib>
+
 #include "asd_internal.cuh"
 
 namespace asd {
@@ -171,7 +173,7 @@ __device__ __forceinline__ void row_ydft(const float* cells, const float2* tws, 
 // sweep of ny floats per component; the unrolled row loop keeps several rows in flight); the partial column sums meet in
 // shared memory, where thread b adds the row lanes and the my columns of macrocell (a, b, c) in a fixed order.
 // Deterministic.  The dcy cell values of each component are then transformed along y (row_ydft).
-constexpr int kMaxRowLanes = 8;
+constexpr int kMaxRowLanes = 4;   // measured on cfg4 (B200): 3-4 lanes 141.6-142.0 us per held-field Heun step, 8 lanes 146.3, 1 lane 155.6
 template <int VEC>
 __global__ void coarse_grain_ydft(const float* __restrict__ X, uint32_t as, int nx, int ny, int nz, int nyp, int lead,
                                   int mx, int my, int mz, long long x0, int dcx, int dcy, int dcz, int PY, int NKY,
@@ -595,6 +597,7 @@ asd_status launch_demag(Ctx& c, int aX) {
     const int vec = (c.d.ny % 4 == 0) ? 4 : 1, groups = c.d.ny / vec;
     int lanes = 1024 / groups;
     if (lanes > kMaxRowLanes) lanes = kMaxRowLanes;
+    if (const char* ev = std::getenv("ASD_CG_LANES")) { const int v = std::atoi(ev); if (v >= 1 && v <= lanes) lanes = v; }   // tuning override
     if (lanes < 1) lanes = 1;                                   // groups <= 1024 is checked at enable time
     const int threads = (int)align_up((size_t)(groups * lanes), 32);
     const size_t smem = cg_smem_bytes(lanes, c.d.ny, pl);

@@ -308,7 +308,10 @@ asd_status launch_heun_direct(Ctx& c, int64_t n, const DynState* dyn) {
   if (c.mm && (staged || dyn)) return ASD_EUNSUPPORTED;                    // multiscale: film, fused and general kernels, plain launches
   // one kernel per step: asked for, or AUTO on a film large enough to fill the machine with strip x chunk CTAs.
   // Not inside a recorded graph (the spin buffers swap roles every step) and not with the demagnetising field.
-  const bool fused = !dyn && !c.demag && heun_fused_supported(c) &&
+  // With the demagnetising field: only in the held-field scheme (asd_set_demag_every >= 1; the per-stage scheme needs the
+  // field of S~, a global quantity, between the two stages), macrocells of >= 3 sites across, no meshes.
+  const bool fused_dm_ok = !c.demag || (c.demag_every >= 1 && c.d.macro[1] >= 3 && !c.mm && heun_fused_takes_demag(c));
+  const bool fused = !dyn && fused_dm_ok && heun_fused_supported(c) &&
                      (c.kernel_variant == ASD_KERNEL_FUSED || (c.kernel_variant == ASD_KERNEL_AUTO && heun_fused_preferred(c))) &&
                      fused_plan(c) && (!c.mm || heun_fused_takes_mm(c));
   if (c.kernel_variant == ASD_KERNEL_FUSED && !fused) return ASD_EUNSUPPORTED;

@@ -57,6 +57,8 @@ struct FusedParams {
   const DynState* dyn;
   uint64_t g0;
   const float* edgeB;              // multiscale window: mesh exchange field on planes 0 / nx-1 ([side][comp][nz*nyp]); nullptr: off
+  DemagGeom dm;                    // held demagnetising field per macrocell (DEMAG instances; asd_set_demag_every >= 1)
+  uint32_t dm_my;                  // macrocell edge in y (sites)
   PhiloxKey key;
 };
 
@@ -117,7 +119,7 @@ constexpr uint32_t kGpRing = 8;   // planes of per-group anisotropy parameters k
 
 // NZ_T / BY_T != 0: film thickness and strip width are compile-time constants (every shared-memory offset becomes an
 // immediate of its LDS / STS); 0: taken from the parameter block.
-template <int LAT, int NT, int MINB, int NZ_T, int BY_T, bool MM = false>
+template <int LAT, int NT, int MINB, int NZ_T, int BY_T, bool MM = false, bool DEMAG = false>
 __global__ void __launch_bounds__(NT, MINB)
 heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUtensorMap mapF, const FusedParams p) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -264,6 +266,15 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
 #pragma unroll
     for (int c = 0; c < 3; ++c) { sP[c][0] = sP[c][1] = sC[c][0] = sC[c][1] = tP[c][0] = tP[c][1] = tC[c][0] = tC[c][1] = 0.0f; }
 
+    // held demagnetising field (DEMAG): the thread's two macrocells across the film and through its thickness are fixed
+    uint32_t dm_yz_lo = 0u, dm_yz_hi = 0u;
+    int dm_nlo = 4;                                    // own sites v < dm_nlo lie in the lower-y cell
+    if (DEMAG && active) {
+      const uint32_t cj_lo = div_u31((uint32_t)j, p.dm.my_m, p.dm.my_s), cj_hi = div_u31((uint32_t)j + 3u, p.dm.my_m, p.dm.my_s);
+      const uint32_t ck = div_u31((uint32_t)k, p.dm.mz_m, p.dm.mz_s);
+      dm_yz_lo = cj_lo * p.dm.sy + ck; dm_yz_hi = cj_hi * p.dm.sy + ck;
+      dm_nlo = (cj_lo == cj_hi) ? 4 : (int)(cj_hi * p.dm_my) - j;
+    }
     mbar_wait_long(bar_full + 0u, 0u);
     mbar_wait_long(bar_full + 8u, 0u);
     asm volatile("bar.sync 1;" ::: "memory");          // the parameter ring's first planes are in place
@@ -340,6 +351,25 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
             Bn[0][v] = fmaf(sgs, xi[v][0], sscale * bx[v]);
             Bn[1][v] = fmaf(sgs, xi[v][1], sscale * by[v]);
             Bn[2][v] = fmaf(sgs, xi[v][2], sscale * bz[v]);
+          }
+        }
+        if (DEMAG) {
+          // Eq. (7), held-field scheme (D3, asd_set_demag_every >= 1): the field of the site's macrocell was
+          // computed from S before this step and serves both stages, so it rides with the stage-independent part.  The
+          // 4 sites lie in at most two macrocells (my >= 3).
+          // Only the x index of the cell changes along the march; the two cells' y-z offsets are per-thread constants.
+          // The six values are loaded here, at their point of use (a few-KB table: L1 hits), so that nothing extra is
+          // live across the Philox / Box-Muller chains above.
+          const int q = i0 - 1 + m;
+          if (active && q >= 0 && q < p.nx) {
+            const uint32_t cb = (div_u31(p.dm.x0 + (uint32_t)q, p.dm.mx_m, p.dm.mx_s) - p.dm.c0) * p.dm.sx;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+              const float lo = p.ngdt * __ldg(p.dm.B + ((uint32_t)c * p.dm.comp_stride + cb + dm_yz_lo));
+              const float hi = p.ngdt * __ldg(p.dm.B + ((uint32_t)c * p.dm.comp_stride + cb + dm_yz_hi));
+#pragma unroll
+              for (int v = 0; v < 4; ++v) Bn[c][v] += (v < dm_nlo) ? lo : hi;
+            }
           }
         }
         if (MM) {
@@ -498,6 +528,8 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
           rC[s][c][d] = lds1(sring + slot_pitch + off);
         }
     uint32_t t3 = 0u;
+    uint32_t hd_ci[2] = {0xFFFFFFFFu, 0xFFFFFFFFu};     // DEMAG: cell x index whose field hd[] holds, per side
+    float hd[2][3] = {{0.0f, 0.0f, 0.0f}, {0.0f, 0.0f, 0.0f}};
 
     for (int m = 0; m <= L + 1; ++m) {
       const int q = i0 - 1 + m;
@@ -554,6 +586,18 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
               Bex[c] = fmaf(p.j3s, s3, fmaf(p.j2s, zs[c], p.j1s * (xs + ys)));
             }
           }
+          if (DEMAG) {
+            const uint32_t ci = div_u31(p.dm.x0 + (uint32_t)q, p.dm.mx_m, p.dm.mx_s) - p.dm.c0;
+            if (ci != hd_ci[s]) {
+              hd_ci[s] = ci;
+              const uint32_t cq = ci * p.dm.sx + div_u31((uint32_t)jh[s], p.dm.my_m, p.dm.my_s) * p.dm.sy +
+                                  div_u31((uint32_t)k, p.dm.mz_m, p.dm.mz_s);
+#pragma unroll
+              for (int c = 0; c < 3; ++c) hd[s][c] = p.ngdt * __ldg(p.dm.B + ((uint32_t)c * p.dm.comp_stride + cq));
+            }
+#pragma unroll
+            for (int c = 0; c < 3; ++c) Bex[c] += hd[s][c];
+          }
           if (MM) {
 #pragma unroll 1
             for (int side = 0; side < 2; ++side) {
@@ -606,7 +650,13 @@ constexpr int kNumShapes = 2;
 
 // Film thickness 27 planes with 32-site strips (BASELINE configs 1, 3, 4) has its own instance with compile-time shared-
 // memory offsets; everything else takes the generic one.
-FusedKernel kernel_for(int lattice, int shape, int nz, int by, bool mm = false) {
+FusedKernel kernel_for(int lattice, int shape, int nz, int by, bool mm = false, bool demag = false) {
+  if (demag) {                                          // held demagnetising field: the 256 x 2 shape only, no meshes
+    if (shape != 0 || mm) return nullptr;
+    if (nz == 27 && by == 32)
+      return lattice == ASD_SC ? heun_fused<LAT_SC, 256, 2, 27, 32, false, true> : heun_fused<LAT_L10, 256, 2, 27, 32, false, true>;
+    return lattice == ASD_SC ? heun_fused<LAT_SC, 256, 2, 0, 0, false, true> : heun_fused<LAT_L10, 256, 2, 0, 0, false, true>;
+  }
   if (mm) {                                             // multiscale window: the 256 x 2 shape only
     if (shape != 0) return nullptr;
     if (nz == 27 && by == 32)
@@ -633,6 +683,7 @@ struct FusedPlan {
   CUtensorMap mapS, mapF;
   FusedKernel kern = nullptr;
   FusedKernel kern_mm = nullptr;   // the instance that adds the mesh exchange field on planes 0 / nx-1 (asd_mm.cu); may be null
+  FusedKernel kern_dm = nullptr;   // the instance that adds a held demagnetising field per macrocell; may be null
   int32_t BY = 0, G = 0, nstrips = 0, CX = 0, nchunks = 0, threads = 0, n_main = 0, ctas_per_sm = 0;
   uint32_t slot_pitch = 0, smem_bytes = 0;
 };
@@ -698,6 +749,12 @@ bool build_plan(Ctx& c, FusedPlan& pl) {
     cudaGetLastError();
     pl.kern_mm = nullptr;
   }
+  pl.kern_dm = kernel_for(c.d.lattice, best.shape, nz, pl.BY, false, true);
+  if (pl.kern_dm && cudaFuncSetAttribute((const void*)pl.kern_dm, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)pl.smem_bytes) != cudaSuccess) {
+    cudaGetLastError();
+    pl.kern_dm = nullptr;
+  }
   int bps = 0;
   if (cudaFuncSetAttribute((const void*)pl.kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes) != cudaSuccess ||
       cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, (const void*)pl.kern, pl.threads, pl.smem_bytes) != cudaSuccess ||
@@ -733,6 +790,7 @@ bool build_plan(Ctx& c, FusedPlan& pl) {
 }  // namespace
 
 bool heun_fused_takes_mm(Ctx& c) { const FusedPlan* pl = fused_plan(c); return pl && pl->kern_mm; }
+bool heun_fused_takes_demag(Ctx& c) { const FusedPlan* pl = fused_plan(c); return pl && pl->kern_dm; }
 
 FusedPlan* fused_plan(Ctx& c) {
   if (!c.fused_plan_tried) {
@@ -773,8 +831,12 @@ asd_status launch_heun_fused(Ctx& c, StageParams& p) {
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr; cfg.numAttrs = 1;
+  f.dm = p.dm; f.dm_my = (uint32_t)c.d.macro[1];
   if (f.edgeB && !pl->kern_mm) return ASD_EUNSUPPORTED;
-  cudaLaunchKernelEx(&cfg, f.edgeB ? pl->kern_mm : pl->kern, pl->mapS, pl->mapF, f);
+  if (f.dm.B && (!pl->kern_dm || f.edgeB || c.demag_every < 1)) return ASD_EUNSUPPORTED;
+  // held-field scheme: the field of S is refreshed before the step when the cadence says so, then serves both stages
+  if (f.dm.B && (c.demag_refresh & 1)) { const asd_status st = launch_demag(c, c.aS); if (st != ASD_OK) return st; }
+  cudaLaunchKernelEx(&cfg, f.dm.B ? pl->kern_dm : (f.edgeB ? pl->kern_mm : pl->kern), pl->mapS, pl->mapF, f);
   ASD_LAUNCH_CHECK(c, "heun step (fused)");
   const int t = c.aS; c.aS = c.aSt; c.aSt = t;
   return ASD_OK;

@@ -57,6 +57,32 @@ def test_heun_steps_with_demag(lattice, kernel):
     assert max_abs_diff(g, o) <= 1e-4
 
 
+@pytest.mark.parametrize("lattice", [ai.SC, ai.L10])
+@pytest.mark.parametrize("every", [1, 3])
+def test_fused_step_with_the_held_field(lattice, every):
+    """The one-kernel Heun step takes the demagnetising field in the held-field scheme (the field of S serves both
+    stages): same tolerances as the stage kernels; the per-stage scheme is refused."""
+    import paper_2502_02236_b200 as asd
+    w = _film(lattice, 24, 40, 6, (4, 5, 2), 1, 25.0, dt=1e-16)
+    o, g = _pair(w)
+    with pytest.raises(asd.AsdError):
+        g.set_kernel(asd.KERNEL_FUSED)                               # per-stage scheme: the field of S~ is a global quantity
+    o.set_demag_every(every); g.set_demag_every(every)
+    g.set_kernel(asd.KERNEL_FUSED)
+    o.step_heun(1); g.step_heun(1)
+    assert max_abs_diff(g, o) <= 1e-5
+    o.step_heun(4); g.step_heun(4)
+    assert max_abs_diff(g, o) <= 5e-5
+    o.shift_window(3); g.shift_window(3)
+    o.step_heun(2); g.step_heun(2)
+    assert max_abs_diff(g, o) <= 1e-4
+    # and it is the stage kernels' held-field result up to rounding
+    h = gpu_from_workload(w)
+    h.enable_demag([a * 1e-9 for a in w.spacing_nm]); h.set_demag_every(every); h.set_kernel(asd.KERNEL_FAST)
+    h.step_heun(5); h.shift_window(3); h.step_heun(2)
+    assert np.abs(h.get_spins_host() - g.get_spins_host()).max() <= 2e-5
+
+
 @pytest.mark.parametrize("every", [1, 3])
 def test_held_field_update_period(every):
     """asd_set_demag_every(P): field from S at every P-th step, held for both stages in between; a shift re-arms it."""
