@@ -17,4 +17,6 @@ from .workloads import (  # noqa: F401
 )
 from .two_track import TwoTrack, two_track_film, drive_pass, read_tracks  # noqa: F401
 from . import multiscale  # noqa: F401
-from .multiscale import Multiscale, multiscale_film, apply_multiscale, cell_grain_map  # noqa: F401
+from .multiscale import (  # noqa: F401
+    Multiscale, multiscale_film, apply_multiscale, cell_grain_map, MultiscaleWrite, multiscale_write, drive_multiscale_write,
+)

@@ -151,3 +151,86 @@ def apply_multiscale(sim, ms: Multiscale):
     for side in (0, 1):
         B = ms.B_mesh[side]
         sim.mm_set_fields(side, ms.T_mesh[side], B[..., 0], B[..., 1], B[..., 2])
+
+
+# ----------------------------------------------------------------------------------------------------------------------
+# Writing a bit sequence with a multiscale window (the paper's Fig. 3 experiment in miniature): the window
+# [mesh | atoms | mesh] moves along the track one cell at a time while the head polarity follows a seeded bit pattern.
+# ----------------------------------------------------------------------------------------------------------------------
+@dataclass
+class MultiscaleWrite:
+    ms: Multiscale
+    bits: np.ndarray               # NRZ polarity (+1 / -1) per bit
+    bit_cells: int                 # cells per written bit
+    steps_per_cell: int            # Heun steps between shifts of one cell (same velocity as 5000 steps per nm)
+    batch: int
+    spot_plane: float              # global plane under the spot centre when the pass starts
+    write_offset: float            # planes from the spot centre back to where the grains freeze (edge of T > T_C)
+    reader_sigma: Tuple[float, float]
+    track_y: float
+
+    @property
+    def bit_origin(self) -> float:
+        """Global plane where bit 0 starts: where the freezing point stands when the pass starts."""
+        return self.spot_plane - self.write_offset
+
+    def bit_at(self, gx: float) -> float:
+        """Polarity the head writes while the spot centre is over global plane gx."""
+        bp = self.bit_cells * self.ms.w.macro[0]
+        b = min(max(int((gx - self.write_offset - self.bit_origin) // bp), 0), len(self.bits) - 1)
+        return float(self.bits[b])
+
+    def cells_per_pass(self) -> int:
+        m = self.ms
+        return m.track_cells()[0] - (m.w.x0 + m.w.nx) // m.w.macro[0] - m.mcx[1]
+
+    def swept_bits(self, cells: Optional[int] = None) -> np.ndarray:
+        cells = self.cells_per_pass() if cells is None else cells
+        bp = self.bit_cells * self.ms.w.macro[0]
+        b = np.arange(len(self.bits))
+        return b[(b + 1) * bp <= cells * self.ms.w.macro[0]]
+
+    def bit_centres(self) -> np.ndarray:
+        return self.bit_origin + (np.arange(len(self.bits)) + 0.5) * self.bit_cells * self.ms.w.macro[0]
+
+
+def multiscale_write(lattice: int = wl.SC, atom_cells: int = 57, mesh_cells: Tuple[int, int] = (24, 24), n_bits: int = 8,
+                     bit_cells: int = 10, width_nm: float = 60.0, nz: int = 27, every: int = 20, fwhm_nm: float = 60.0,
+                     steps_per_nm: int = 5000, batch: int = 100, bit_seed: int = 3, meshes: bool = True,
+                     **kw) -> MultiscaleWrite:
+    """meshes = False: the same atomistic mesh, track, schedule and bit pattern without the micromagnetic meshes (the
+    fully atomistic window the paper compares with); the recipe still carries the mesh description, unused."""
+    macro = kw.pop("macro", None) or ((7, 7, 7) if lattice == wl.SC else (7, 7, 5))
+    total_bits_cells = n_bits * bit_cells
+    ms = multiscale_film(lattice, atom_cells=atom_cells, mesh_cells=mesh_cells, width_nm=width_nm, nz=nz,
+                         extra_cells=total_bits_cells, every=every, macro=macro, fwhm_nm=fwhm_nm, **kw)
+    sp = ms.w.spacing_nm
+    # diameter of the spot above 710 K for T = 300 + 500 exp(-4 ln2 r^2 / FWHM^2): 0.535 FWHM (two_track.py)
+    r_hot_nm = 0.5 * 0.535 * fwhm_nm
+    return MultiscaleWrite(ms=ms, bits=wl.nrz_bits(n_bits, bit_seed), bit_cells=bit_cells,
+                           steps_per_cell=int(round(steps_per_nm * macro[0] * sp[0])), batch=batch,
+                           spot_plane=ms.w.x0 + 0.5 * ms.w.nx, write_offset=r_hot_nm / sp[0],
+                           reader_sigma=(0.25 * bit_cells * macro[0], 0.25 * width_nm / sp[1]),
+                           track_y=0.5 * ms.w.ny)
+
+
+def drive_multiscale_write(sim, mw: MultiscaleWrite, cells: Optional[int] = None, with_meshes: bool = True) -> int:
+    """One pass: per shift period the head polarity of the bit under the freezing point, steps_per_cell Heun steps, a
+    shift by one cell; then asd_track_end_pass.  `sim`: the oracle or the CUDA context.  Returns the Heun steps taken."""
+    if with_meshes:
+        apply_multiscale(sim, mw.ms)
+    cells = mw.cells_per_pass() if cells is None else cells
+    mx = mw.ms.w.macro[0]
+    gx, steps = mw.spot_plane, 0
+    for _ in range(cells):
+        sim.set_field_scale(mw.bit_at(gx))
+        left = mw.steps_per_cell
+        while left > 0:
+            n = min(mw.batch, left)
+            sim.step_heun(n)
+            left -= n
+            steps += n
+        sim.shift_window(mx)
+        gx += mx
+    sim.track_end_pass()
+    return steps

@@ -241,7 +241,10 @@ ASD_API asd_status asd_track_read_scan(asd_ctx *ctx, double y_r, double sigma_x,
  *              leading mesh; ASD_EINVAL otherwise.
  * HOST pointers of the description are read during asd_mm_enable only.  The caller owns the workspace (DEVICE, 256-byte
  * aligned) for the life of the context.  Not available with general ELL tables, periodic boundaries, ASD_KERNEL_TMA,
- * CUDA-graph replay, asd_track_end_pass / asd_track_begin_pass (ASD_EUNSUPPORTED). */
+ * CUDA-graph replay (ASD_EUNSUPPORTED).
+ *   passes     asd_track_end_pass also transfers every cell of both meshes to the track store (as m_e m on the cell's
+ *              magnetic sites); asd_track_begin_pass(x0_new) needs x0_new on a whole macrocell with both meshes inside
+ *              the track, and restarts the meshes along the track they then lie over. */
 typedef struct {
   int32_t mcx[2];            /* cells along x of the trailing / leading mesh, each >= 1                          */
   int32_t every;             /* Heun steps per RK4 step, >= 1                                                    */

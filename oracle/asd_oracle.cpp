@@ -692,6 +692,40 @@ int64_t cell_site_count(const Oracle& o, int64_t cx, int b, int c) {
   return n;
 }
 
+// The first `count` cell columns of a mesh go to the track store: M / M_S^0 = m_e m on the magnetic sites of each cell.
+void mm_columns_to_track(Oracle& o, int side, int count) {
+  const Oracle::MicroMesh& M = o.mesh[side];
+  const int64_t cx0 = mm_cx0(o, side);
+  for (int a = 0; a < count; ++a)
+    for (int b = 0; b < o.ncy; ++b)
+      for (int c = 0; c < o.ncz; ++c) {
+        if (mm_grain_of(o, cx0 + a, b) < 0) continue;
+        const size_t q = mm_idx(o, a, b, c);
+        const size_t t = (size_t)(((cx0 + a) * o.ncy + b) * o.ncz + c);
+        const int64_t n = cell_site_count(o, cx0 + a, b, c);
+        for (int u = 0; u < 3; ++u) o.out_sum[3 * t + u] += M.me[q] * M.m[3 * q + u] * (double)n;
+        o.out_cnt[t] += n;
+      }
+}
+
+// Mesh state = the direction of the track the meshes lie over (empty cells 0): at enable time and at the start of a pass.
+void mm_init_from_track(Oracle& o) {
+  for (int side = 0; side < 2; ++side) {
+    Oracle::MicroMesh& M = o.mesh[side];
+    const int64_t cx0 = mm_cx0(o, side);
+    for (int a = 0; a < M.mcx; ++a)
+      for (int b = 0; b < o.ncy; ++b)
+        for (int c = 0; c < o.ncz; ++c) {
+          double n[3] = {0.0, 0.0, 0.0};
+          if (mm_grain_of(o, cx0 + a, b) >= 0) {
+            n[2] = 1.0;
+            track_direction(o, cx0 + a, b, c, n);
+          }
+          for (int u = 0; u < 3; ++u) M.m[3 * mm_idx(o, a, b, c) + u] = n[u];
+        }
+  }
+}
+
 // M10: the window moves by pc whole cells ("in steps set by the track discretization cellsize").
 //   trailing mesh -> track (as M / M_S^0 = m_e m on the cell's magnetic sites);  outgoing atomistic planes -> the
 //   trailing mesh by Eq. (6) ("averaging", Fig. 1);  incoming atomistic planes <- the leading mesh by the cone
@@ -706,16 +740,7 @@ int mm_shift(Oracle& o, int p) {
   if (mm_cx0(o, 1) + R.mcx + pc > o.ncx) return 1;
   const int64_t cxL = mm_cx0(o, 0), cxA = o.x0 / mx, cxR = mm_cx0(o, 1);
   // 1. trailing mesh columns a < pc -> track
-  for (int a = 0; a < pc; ++a)
-    for (int b = 0; b < o.ncy; ++b)
-      for (int c = 0; c < o.ncz; ++c) {
-        if (mm_grain_of(o, cxL + a, b) < 0) continue;
-        const size_t q = mm_idx(o, a, b, c);
-        const size_t t = (size_t)(((cxL + a) * o.ncy + b) * o.ncz + c);
-        const int64_t n = cell_site_count(o, cxL + a, b, c);
-        for (int u = 0; u < 3; ++u) o.out_sum[3 * t + u] += L.me[q] * L.m[3 * q + u] * (double)n;
-        o.out_cnt[t] += n;
-      }
+  mm_columns_to_track(o, 0, pc);
   // 2. trailing mesh moves; its new columns are the Eq. (6) averages of the outgoing atomistic cells (direction)
   std::vector<double> newL((size_t)pc * o.ncy * o.ncz * 3, 0.0);
   for (int a = 0; a < pc; ++a)
@@ -1058,9 +1083,12 @@ int orc_shift_window(void* h, int32_t p) {
 //    planes are (S2), and every macrocell the pass has written (count > 0) becomes what lies ahead of the next pass:
 //    init_mean[c] = out_sum[c] / out_cnt[c]  (mean spin = M / M_S^0 of the cell).  Cells never written keep their value.
 //    The written store is kept (orc_track_get / orc_track_read_scan read it).
+//    Multiscale window (reading T1'): the cells of both meshes go to the track as well, as m_e m on their magnetic
+//    sites -- exactly what a shift does with the trailing mesh's outgoing columns (M10).
 int orc_track_end_pass(void* h) {
   Oracle& o = *static_cast<Oracle*>(h);
-  if (o.ell_width > 0 || o.mm) return 5;
+  if (o.ell_width > 0) return 5;
+  if (o.mm) { mm_columns_to_track(o, 0, o.mesh[0].mcx); mm_columns_to_track(o, 1, o.mesh[1].mcx); }
   for (int i = 0; i < o.nx; ++i)
     for (int k = 0; k < o.nz; ++k)
       for (int j = 0; j < o.ny; ++j) {
@@ -1081,16 +1109,21 @@ int orc_track_end_pass(void* h) {
 // T2 start of the next pass: the written store is cleared, pass += 1, the window returns to global plane x0_new and
 //    ALL its planes are generated from the track by the cone thermalisation of P:68 (S3), Philox counter n := pass.
 //    The step and shift counters run on.
+//    Multiscale window (reading T2'): x0_new must be a whole number of cells with both meshes inside the track; the
+//    meshes restart from the direction of the track they now lie over, as at enable time.
 int orc_track_begin_pass(void* h, int64_t x0_new) {
   Oracle& o = *static_cast<Oracle*>(h);
-  if (o.ell_width > 0 || o.mm) return 5;
+  if (o.ell_width > 0) return 5;
   if (x0_new < 0 || x0_new + o.nx > o.track_nx) return 1;
+  if (o.mm && (x0_new % o.macro[0] != 0 || x0_new / o.macro[0] - o.mesh[0].mcx < 0 ||
+               (x0_new + o.nx) / o.macro[0] + o.mesh[1].mcx > o.ncx)) return 1;
   const size_t nc = (size_t)(o.ncx * o.ncy * o.ncz);
   for (size_t c = 0; c < nc; ++c) { o.out_cnt[c] = 0; o.out_sum[3 * c] = o.out_sum[3 * c + 1] = o.out_sum[3 * c + 2] = 0.0; }
   o.pass += 1;
   o.x0 = x0_new;
   o.demag_age = 0;
   for (int i = 0; i < o.nx; ++i) seed_plane(o, i, o.x0 + i);
+  if (o.mm) { mm_init_from_track(o); o.mm_age = 0; mm_refresh_params(o); }
   return 0;
 }
 
@@ -1188,19 +1221,7 @@ int orc_mm_enable(void* h, const orc_mm_desc* d) {
     o.mm_avg[side].assign((size_t)o.ncy * o.ncz * 3, 0.0);
   }
   o.mm = true;
-  // initial state: the direction of the track the meshes lie over (empty cells 0)
-  for (int side = 0; side < 2; ++side) {
-    Oracle::MicroMesh& M = o.mesh[side];
-    const int64_t cx0 = mm_cx0(o, side);
-    for (int a = 0; a < M.mcx; ++a)
-      for (int b = 0; b < o.ncy; ++b)
-        for (int c = 0; c < o.ncz; ++c) {
-          if (mm_grain_of(o, cx0 + a, b) < 0) continue;
-          double n[3] = {0.0, 0.0, 1.0};
-          track_direction(o, cx0 + a, b, c, n);
-          for (int u = 0; u < 3; ++u) M.m[3 * mm_idx(o, a, b, c) + u] = n[u];
-        }
-  }
+  mm_init_from_track(o);                                  // initial state: the direction of the track under the meshes
   mm_refresh_params(o);
   return 0;
 }

@@ -534,7 +534,6 @@ asd_status asd_track_get(asd_ctx* ctx, double* sum, int64_t* count) {
 asd_status asd_track_end_pass(asd_ctx* ctx) {
   CTX_OR_RETURN(ctx);
   if (c.d.ell_width > 0) return fail(c, ASD_EUNSUPPORTED, "asd_track_end_pass: a general ELL table has no track");
-  if (c.mm) return fail(c, ASD_EUNSUPPORTED, "asd_track_end_pass: not defined for a multiscale window");
   return launch_track_end_pass(c);
 }
 
@@ -542,8 +541,14 @@ asd_status asd_track_begin_pass(asd_ctx* ctx, int64_t x0_new) {
   CTX_OR_RETURN(ctx);
   if (c.d.ell_width > 0) return fail(c, ASD_EUNSUPPORTED, "asd_track_begin_pass: a general ELL table cannot follow the window");
   if (c.d.pbc[0]) return fail(c, ASD_EUNSUPPORTED, "asd_track_begin_pass: window is periodic in x");
-  if (c.mm) return fail(c, ASD_EUNSUPPORTED, "asd_track_begin_pass: not defined for a multiscale window");
   if (x0_new < 0 || x0_new + c.d.nx > c.d.track_nx) return fail(c, ASD_EINVAL, "asd_track_begin_pass: window must lie inside the track");
+  if (c.mm) {
+    int64_t dl[3], dr[3];
+    mm_dims(c, 0, dl); mm_dims(c, 1, dr);
+    const int mx = c.d.macro[0];
+    if (x0_new % mx != 0 || x0_new / mx - dl[0] < 0 || (x0_new + c.d.nx) / mx + dr[0] > c.ncx)
+      return fail(c, ASD_EINVAL, "asd_track_begin_pass: a multiscale window starts on a whole macrocell with both meshes inside the track");
+  }
   graphs_invalidate(c);
   c.demag_age = 0;
   return launch_track_begin_pass(c, x0_new);

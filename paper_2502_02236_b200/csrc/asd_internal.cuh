@@ -263,6 +263,8 @@ void mm_dims(const Ctx& c, int side, int64_t dims[3]);
 asd_status mm_shift_prepare(Ctx& c, int pc);
 const float* mm_shift_frames(const Ctx& c);
 asd_status mm_shift_finish(Ctx& c, int pc);
+asd_status mm_flush_to_track(Ctx& c);                         // end of a pass: every mesh cell -> track store
+asd_status mm_restart_from_track(Ctx& c);                     // start of a pass: meshes along the track under them
 asd_status launch_shift_mm(Ctx& c, int32_t p);                // asd_shift.cu: whole-cell shift of a multiscale window
 asd_status launch_shift(Ctx& c, int32_t p);
 asd_status launch_cell_frames(Ctx& c);

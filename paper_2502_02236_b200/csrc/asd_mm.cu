@@ -311,13 +311,15 @@ __global__ void mm_init_kernel(MmGeom g, const int32_t* __restrict__ cell_grain,
 
 // ---- shift by pc whole cells (reading M10) ----
 // 1. trailing mesh columns a < pc -> track: M / M_S^0 = m_e m on the magnetic sites of the cell.
-__global__ void mm_out_to_track_kernel(MmGeom g, int pc, const float* __restrict__ m, const float* __restrict__ me,
+// (side 0, pc columns at a shift; all columns of either mesh at the end of a pass)
+__global__ void mm_out_to_track_kernel(MmGeom g, int side, int pc, const float* __restrict__ m, const float* __restrict__ me,
                                        const int32_t* __restrict__ cell_grain, const uint32_t* __restrict__ col_track,
                                        int64_t track_nx, double* __restrict__ out_sum, long long* __restrict__ out_cnt) {
-  const int q = blockIdx.x * blockDim.x + threadIdx.x;
-  if (q >= pc * g.ncol) return;
-  const int a = q / g.ncol, t = q - a * g.ncol, b = t / g.ncz, c = t - b * g.ncz;
-  const int64_t cx = g.cx0[0] + a;
+  const int r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= pc * g.ncol) return;
+  const int a = r / g.ncol, t = r - a * g.ncol, b = t / g.ncz, c = t - b * g.ncz;
+  const int q = (side ? g.n0 : 0) + r;
+  const int64_t cx = g.cx0[side] + a;
   if (grain_at(g, cell_grain, cx, b) < 0) return;
   long long n = 0;
   const int kext = min((c + 1) * g.mz, g.nz) - c * g.mz;
@@ -614,7 +616,7 @@ asd_status mm_shift_prepare(Ctx& c, int pc) {
   MmPlan& P = *c.mm;
   const MmGeom g = geom(c);
   const Vec3Ptr S = c.S();
-  mm_out_to_track_kernel<<<nblocks((int64_t)pc * P.ncol, 128), 128, 0, c.stream>>>(g, pc, P.m, P.me, P.cell_grain, c.col,
+  mm_out_to_track_kernel<<<nblocks((int64_t)pc * P.ncol, 128), 128, 0, c.stream>>>(g, 0, pc, P.m, P.me, P.cell_grain, c.col,
                                                                                  c.d.track_nx, c.out_sum, c.out_cnt);
   ASD_LAUNCH_CHECK(c, "mm_out_to_track");
   mm_new_trailing_kernel<<<nblocks((int64_t)pc * P.ncol * 32, 128), 128, 0, c.stream>>>(g, pc, S.x, S.y, S.z, P.cell_grain,
@@ -625,6 +627,26 @@ asd_status mm_shift_prepare(Ctx& c, int pc) {
   return ASD_OK;
 }
 const float* mm_shift_frames(const Ctx& c) { return c.mm->frames; }
+
+// End of a pass (reading T1'): every cell of both meshes goes to the track store.
+asd_status mm_flush_to_track(Ctx& c) {
+  MmPlan& P = *c.mm;
+  const MmGeom g = geom(c);
+  for (int side = 0; side < 2; ++side) {
+    mm_out_to_track_kernel<<<nblocks(P.n[side], 128), 128, 0, c.stream>>>(g, side, P.mcx[side], P.m, P.me, P.cell_grain, c.col,
+                                                                        c.d.track_nx, c.out_sum, c.out_cnt);
+    ASD_LAUNCH_CHECK(c, "mm_out_to_track(all columns)");
+  }
+  return ASD_OK;
+}
+// Start of a pass (reading T2'): the meshes restart along the track they lie over at the context's (new) window origin.
+asd_status mm_restart_from_track(Ctx& c) {
+  MmPlan& P = *c.mm;
+  mm_init_kernel<<<nblocks(P.ntot, 128), 128, 0, c.stream>>>(geom(c), P.cell_grain, c.out_sum, c.out_cnt, c.init_mean, P.m);
+  ASD_LAUNCH_CHECK(c, "mm_init");
+  P.age = 0;
+  return launch_params(c);
+}
 // ... and AFTER: both meshes move by pc columns (geometry still that of the old window origin).
 asd_status mm_shift_finish(Ctx& c, int pc) {
   MmPlan& P = *c.mm;

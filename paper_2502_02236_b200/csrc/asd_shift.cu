@@ -216,6 +216,7 @@ asd_status launch_coarse_grain(Ctx& c, const ShiftGeom& g) {
 
 // asd_track_end_pass: all nx planes of the window -> track (Eq. (6)); written cells -> init_mean; frames rebuilt.
 asd_status launch_track_end_pass(Ctx& c) {
+  if (c.mm) { const asd_status sm = mm_flush_to_track(c); if (sm != ASD_OK) return sm; }
   const asd_status st = launch_coarse_grain(c, shift_geom(c, c.d.nx));
   if (st != ASD_OK) return st;
   track_commit_kernel<<<nblocks(c.ncell, 128), 128, 0, c.stream>>>(c.out_sum, c.out_cnt, c.init_mean, c.ncell);
@@ -236,6 +237,7 @@ asd_status launch_track_begin_pass(Ctx& c, int64_t x0_new) {
       S.x, S.y, S.z, c.col, c.cell_frame, g, expand_key(c.d.seed), (uint32_t)((uint64_t)c.pass & 0xFFFFFFFFull),
       (uint32_t)((uint64_t)c.pass >> 32));
   ASD_LAUNCH_CHECK(c, "seed_incoming(all planes)");
+  if (c.mm) return mm_restart_from_track(c);
   return ASD_OK;
 }
 

@@ -119,9 +119,36 @@ def test_error_paths():
         g.set_kernel(asd.KERNEL_TMA)
     assert e.value.status == 5
     with pytest.raises(asd.AsdError) as e:
-        g.track_end_pass()
-    assert e.value.status == 5
+        g.track_begin_pass(10)                                        # not on a whole cell
+    assert e.value.status == 1
     g.shift_window(6)
     with pytest.raises(asd.AsdError) as e:
         g.shift_window(3)                                             # leading mesh would leave the track
     assert e.value.status == 4
+
+
+@pytest.mark.parametrize("lattice", [ai.SC, ai.L10])
+def test_passes_over_the_track_with_the_meshes(lattice):
+    """asd_track_end_pass / asd_track_begin_pass on a multiscale window (readings T1', T2'): meshes and atoms to the track,
+    then the next pass's window (atoms regenerated, meshes along the track) one cell further along."""
+    ms, o, g = _pair(lattice, every=2, t_peak=450.0)
+    w = ms.w
+    o.step_heun(2); g.step_heun(2)
+    assert o.shift_window(w.macro[0]) == 0
+    g.shift_window(w.macro[0])
+    o.step_heun(2); g.step_heun(2)
+    assert o.track_end_pass() == 0
+    g.track_end_pass()
+    _, cnt_o, sum_o = o.track_get()
+    sum_g, cnt_g = g.track_get()
+    assert np.array_equal(cnt_o, cnt_g)
+    assert np.abs(sum_o - sum_g).max() <= 1e-4 * max(1, cnt_o.max())
+    x1 = w.x0 + 2 * w.macro[0]
+    assert o.track_begin_pass(x1) == 0
+    g.track_begin_pass(x1)
+    assert g.counters() == o.counters()
+    assert _mesh_diff(o, g) <= 2e-6
+    assert np.abs(o.get_spins() - g.get_spins_host()).max() <= 3e-5
+    o.step_heun(3); g.step_heun(3)
+    assert np.abs(o.get_spins() - g.get_spins_host()).max() <= 6e-5
+    assert _mesh_diff(o, g) <= 2e-5

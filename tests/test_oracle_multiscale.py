@@ -372,8 +372,6 @@ def test_p19_shift_by_whole_cells_moves_everything_exactly():
                 else:
                     v = init[cxR + 3 + a, b, cz].astype(np.float64)
                     assert np.allclose(got, v / np.linalg.norm(v), atol=1e-14)
-    # passes over the track are not defined for a multiscale window
-    assert o.track_end_pass() == 5 and o.track_begin_pass(0) == 5
 
 
 def test_mm_enable_rejects_misaligned_windows_and_recipe_is_consistent():
@@ -398,3 +396,72 @@ def test_mm_enable_rejects_misaligned_windows_and_recipe_is_consistent():
     assert abs(A[0] - 3.0 * J / (2.0 * 0.371e-9)) < 1e-20                      # Eq. (10) with a -> the plane spacing
     cgm = ai.multiscale.cell_grain_map(np.array([[0, 0, -1, 1], [0, -1, -1, 1], [2, 2, 2, -1], [2, 2, -1, -1]]), (2, 2, 1))
     assert cgm.tolist() == [[0, -1], [2, -1]] or cgm.tolist() == [[0, 1], [2, -1]]
+
+
+def test_passes_over_the_track_with_a_multiscale_window():
+    """Readings T1' / T2': at the end of a pass the cells of both meshes go to the track as m_e m on
+    their magnetic sites, next to the atoms' Eq. (6) sums; the next pass starts with the meshes along the track they lie
+    over and the atoms regenerated from it.  Integer-valued atoms, T = 0 (m_e = 1): exact."""
+    ms = ai.multiscale_film(ai.SC, atom_cells=3, mesh_cells=(2, 3), width_nm=7.2, nz=5, extra_cells=3,
+                            macro=(3, 4, 2), pitch_nm=3.0, boundary_nm=0.6, t_peak=0.0, t_ambient=0.0)
+    w = ms.w
+    mx, my, mz = w.macro
+    gidx = np.arange(w.n_sites, dtype=np.int64)
+    mag = w.magnetic_mask().reshape(-1)
+    w.sx = ((gidx % 61) * mag).astype(np.float32)
+    w.sy = ((gidx // 61 % 7) * mag).astype(np.float32)
+    w.sz = ((gidx % 13 + 1) * mag).astype(np.float32)
+    o = orc.from_workload(w)
+    ai.apply_multiscale(o, ms)
+    rng = np.random.default_rng(17)
+    mesh = []
+    for side in (0, 1):
+        v = rng.standard_normal(o.mm_shape(side) + (3,)); v /= np.linalg.norm(v, axis=-1, keepdims=True)
+        o.mm_set_m(side, v)
+        mesh.append(o.mm_get_m(side))
+    ncx, ncy, ncz = o.track_dims()
+    S = o.get_spins().reshape(3, w.nx, w.nz, w.ny)
+    assert o.track_end_pass() == 0
+    mean, cnt, sm = o.track_get()
+    cnt, sm = cnt.reshape(ncx, ncy, ncz), sm.reshape(ncx, ncy, ncz, 3)
+    gm = w.grain_map
+    cxA = w.x0 // mx
+    for side, cx0 in ((0, cxA - 2), (1, cxA + 3)):
+        for a in range(ms.mcx[side]):
+            for b in range(ncy):
+                for cz in range(ncz):
+                    cols = (gm[(cx0 + a) * mx:(cx0 + a + 1) * mx, b * my:(b + 1) * my] >= 0).sum()
+                    n = cols * (min((cz + 1) * mz, w.nz) - cz * mz) if ms.cell_grain[cx0 + a, b] >= 0 else 0
+                    assert cnt[cx0 + a, b, cz] == n
+                    assert np.allclose(sm[cx0 + a, b, cz], mesh[side][a, b, cz] * n, atol=1e-12)
+    for a in range(3):                                     # the atoms' cells: Eq. (6) sums, exact
+        for b in range(ncy):
+            for cz in range(ncz):
+                blk = S[:, a * mx:(a + 1) * mx, cz * mz:(cz + 1) * mz, b * my:(b + 1) * my].reshape(3, -1).sum(axis=1)
+                assert np.array_equal(sm[cxA + a, b, cz], blk)
+    assert cnt[cxA + 6:].sum() == 0 and cnt[:cxA - 2].sum() == 0
+    # next pass, one cell further along: the meshes lie along the committed track (or what lay ahead where nothing was written)
+    x1 = w.x0 + mx
+    assert o.track_begin_pass(x1 + 1) == 1                 # whole cells only
+    assert o.track_begin_pass(x1) == 0
+    c = o.counters()
+    assert c["pass"] == 1 and c["x0"] == x1
+    _, cnt2, _ = o.track_get()
+    assert not cnt2.any()
+    mean = mean.reshape(ncx, ncy, ncz, 3)
+    for side, cx0 in ((0, x1 // mx - 2), (1, (x1 + w.nx) // mx)):
+        m = o.mm_get_m(side)
+        for a in range(ms.mcx[side]):
+            for b in range(ncy):
+                for cz in range(ncz):
+                    if ms.cell_grain[cx0 + a, b] < 0:
+                        assert not m[a, b, cz].any()
+                    elif cnt[cx0 + a, b, cz] > 0:
+                        v = mean[cx0 + a, b, cz]
+                        assert np.allclose(m[a, b, cz], v / np.linalg.norm(v), atol=1e-6)   # init_mean is fp64 here; exact up to the division
+                    else:
+                        assert np.array_equal(m[a, b, cz], [0.0, 0.0, 1.0])                 # the default track ahead: +z
+    R = o.get_spins().reshape(3, w.nx, w.nz, w.ny)
+    assert np.allclose(np.linalg.norm(R, axis=0)[np.broadcast_to((gm[x1:x1 + w.nx] >= 0)[:, None, :], R.shape[1:])], 1.0, atol=1e-14)
+    # the dynamics go on
+    o.step_heun(2)
