@@ -409,9 +409,13 @@ def sustained(run, seconds, ms_per_step, gpu_index, peak, peak_src):
     t = run.timed(steps)
     clocks = sampler.stop()
     r = run.roofline(t, peak, peak_src)
-    return {"value": float(steps) * run.hps * run.N / (t["ms"] * 1e-3), "unit": UNIT, "steps": steps,
+    value = float(steps) * run.hps * run.N / (t["ms"] * 1e-3)
+    # energy per site update from the median board power over the run (20 samples in 2 s): under a power cap this, not
+    # bytes or instructions, is what binds
+    nj = (clocks["power_w"] / value * 1e9) if clocks.get("power_w") else None
+    return {"value": value, "unit": UNIT, "steps": steps,
             "seconds": t["ms"] * 1e-3, "ms_per_step": t["ms"] / steps, "shifts_in_timed_region": t["shifts"],
-            "clocks": clocks, "avg_launch_us": r["avg_launch_us"], "frac": r["frac"],
+            "clocks": clocks, "nj_per_spin_update": nj, "avg_launch_us": r["avg_launch_us"], "frac": r["frac"],
             "frac_survey_floor": r["frac_survey_floor"]}
 
 
