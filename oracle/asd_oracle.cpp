@@ -20,6 +20,7 @@
 //   * multiscale window: micromagnetic LLG meshes either side of the atomistic mesh, Eq. (4)-(5), temperature scalings
 //     m_e(T), A = A0 m_e^2, K = K0 m_e^3, alpha = lambda (1 - T/3T_C), RK4, two-way exchange coupling
 //     across the mesh boundaries, transfers on a shift (Fig. 1) -> the "Multiscale window" section (S:8(f) item 3)
+//   * stray field of the frozen track on the window -> stray_cells()  (reading D4)
 //   * passes over the track (two parallel tracks) -> orc_track_end_pass(), orc_track_begin_pass();
 //     Gaussian-footprint read-back standing in for the TMR head -> orc_track_read_scan()  (S:8(f) item 4)
 //
@@ -154,6 +155,11 @@ struct Oracle {
   int demag_every = 0;             // 0: recomputed in every stage; P >= 1: from S at every P-th step, held in between (D3)
   int64_t demag_age = 0;           // steps since the held field was invalidated (enable, set_every, shift, set_spins)
   std::vector<double> demag_hold;  // the held per-macrocell field
+  // stray field of the frozen track on the window's macrocells (reading D4); off unless enabled
+  bool stray = false;
+  int stray_range = 0;             // source cells taken up to this many cells from a target cell along x; 0 = the whole track
+  bool stray_dirty = true;         // window origin or track state changed since stray_B was computed
+  std::vector<double> stray_B;     // [dcx*dcy*dcz*3] Tesla
   // multiscale window (S:8(f) item 3): micromagnetic LLG meshes either side of the atomistic
   // mesh; off unless orc_mm_enable was called.  Mesh cells ARE track macrocells; side 0 = trailing (lower x), 1 = leading.
   bool mm = false;
@@ -352,6 +358,57 @@ inline const double* demag_of_site(const Oracle& o, const std::vector<double>& B
   return &Bd[3 * c];
 }
 
+// Stray field of the frozen track on the window's macrocells (reading D4; "the stray field generated by [the
+// frozen track] is fully computed when the simulation window is shifted, and included in the simulation window at each
+// iteration").  Sources: every track macrocell's sites that are NOT inside the window -- what has left it (out_sum,
+// the actual frozen moments) and what the window has never held (init mean spin times the number of such magnetic sites):
+//   mom_c' = out_sum_c' + init_mean_c' (n_behind_c' - out_cnt_c' + n_ahead_c'),   M_c' = (mu_s / V) mom_c'
+//   B_c = -mu_0 sum_c' N(r_c' - r_c) M_c'      (Eq. (7) with the same cuboid tensor; a cell the window edge cuts is a
+//                                               source with its outside sites and a demag cell with its inside sites)
+void stray_cells(const Oracle& o, std::vector<double>& Bs) {
+  const double mu0 = 4.0e-7 * 3.14159265358979323846;
+  const int mx = o.macro[0], my = o.macro[1], mz = o.macro[2];
+  const int64_t c0 = o.x0 / mx;
+  const int ncxw = (int)((o.x0 + o.nx - 1) / mx - c0) + 1;
+  const double V = o.cell_m[0] * o.cell_m[1] * o.cell_m[2];
+  Bs.assign((size_t)o.dcx * o.dcy * o.dcz * 3, 0.0);
+  for (int64_t cx = 0; cx < o.ncx; ++cx)
+    for (int b2 = 0; b2 < o.ncy; ++b2)
+      for (int c2 = 0; c2 < o.ncz; ++c2) {
+        const size_t t = (size_t)((cx * o.ncy + b2) * o.ncz + c2);
+        int64_t n_out = 0;                                   // magnetic sites of the cell outside the window
+        const int kext = std::min((c2 + 1) * mz, o.nz) - c2 * mz;
+        for (int64_t gx = cx * mx; gx < std::min<int64_t>((cx + 1) * mx, o.track_nx); ++gx) {
+          if (gx >= o.x0 && gx < o.x0 + o.nx) continue;
+          for (int j = b2 * my; j < std::min((b2 + 1) * my, o.ny); ++j)
+            if (o.grain_map[(size_t)(gx * o.ny + j)] >= 0) n_out += kext;
+        }
+        const double fresh = (double)(n_out - o.out_cnt[t]);  // sites the window has never held
+        double M[3];
+        for (int u = 0; u < 3; ++u) M[u] = o.mu_s / V * (o.out_sum[3 * t + u] + o.init_mean[3 * t + u] * fresh);
+        if (M[0] == 0.0 && M[1] == 0.0 && M[2] == 0.0) continue;
+        for (int a = 0; a < ncxw; ++a) {
+          if (o.stray_range > 0 && std::llabs(cx - (c0 + a)) > o.stray_range) continue;
+          for (int b = 0; b < o.dcy; ++b)
+            for (int c = 0; c < o.dcz; ++c) {
+              const double R[3] = {(double)(cx - (c0 + a)) * o.cell_m[0], (double)(b2 - b) * o.cell_m[1], (double)(c2 - c) * o.cell_m[2]};
+              double N[6];
+              newell_tensor(o.cell_m, R, N);
+              double* B = &Bs[3 * (((size_t)a * o.dcy + b) * o.dcz + c)];
+              B[0] -= mu0 * (N[0] * M[0] + N[3] * M[1] + N[4] * M[2]);
+              B[1] -= mu0 * (N[3] * M[0] + N[1] * M[1] + N[5] * M[2]);
+              B[2] -= mu0 * (N[4] * M[0] + N[5] * M[1] + N[2] * M[2]);
+            }
+        }
+      }
+}
+// cell field every site sees in a stage: the window's demagnetising field (Bd, already computed) + the track's stray field
+void add_stray(Oracle& o, std::vector<double>& Bd) {
+  if (!o.stray) return;
+  if (o.stray_dirty) { stray_cells(o, o.stray_B); o.stray_dirty = false; }
+  for (size_t t = 0; t < Bd.size(); ++t) Bd[t] += o.stray_B[t];
+}
+
 // Effective field in Tesla at a magnetic site (S:O3):
 // B_i(X) = (1/mu_s) sum_j J_ij X_j + (2 k_u,g/mu_s)(X_i.e_g) e_g + s*B_app,i + sigma_i xi_i.
 void field_at(const Oracle& o, const double* X0, const double* X1, const double* X2,
@@ -417,8 +474,10 @@ void heun_step(Oracle& o) {
     if (o.demag_age % o.demag_every == 0) demag_cells(o, o.sx.data(), o.sy.data(), o.sz.data(), o.demag_hold);
     Bd = o.demag_hold;
     o.demag_age += 1;
+    add_stray(o, Bd);
   } else if (o.demag) {
     demag_cells(o, o.sx.data(), o.sy.data(), o.sz.data(), Bd);
+    add_stray(o, Bd);
   }
 #pragma omp parallel for collapse(2) schedule(static) num_threads(nt)
   for (int i = 0; i < nx; ++i)
@@ -439,7 +498,7 @@ void heun_step(Oracle& o) {
         tx[l] = p0 / nrm; ty[l] = p1 / nrm; tz[l] = p2 / nrm;
       }
   std::vector<double> n0((size_t)N, 0.0), n1((size_t)N, 0.0), n2((size_t)N, 0.0);
-  if (o.demag && !held) demag_cells(o, tx.data(), ty.data(), tz.data(), Bd);   // B(S~) includes the demagnetising field of S~
+  if (o.demag && !held) { demag_cells(o, tx.data(), ty.data(), tz.data(), Bd); add_stray(o, Bd); }   // B(S~): demagnetising field of S~ (+ the track's)
 #pragma omp parallel for collapse(2) schedule(static) num_threads(nt)
   for (int i = 0; i < nx; ++i)
     for (int k = 0; k < nz; ++k)
@@ -784,7 +843,7 @@ int mm_shift(Oracle& o, int p) {
         if (n > 0.0) { d[0] = v[0] / n; d[1] = v[1] / n; d[2] = v[2] / n; } else { d[2] = 1.0; }
       }
   o.x0 += p; o.shift += 1;
-  o.mm_age = 0; o.demag_age = 0;
+  o.mm_age = 0; o.demag_age = 0; o.stray_dirty = true;
   return 0;
 }
 
@@ -948,7 +1007,7 @@ void orc_enable_demag(void* h, const double spacing[3]) {
         newell_tensor(o.cell_m, R, &o.demag_N[(((size_t)a * sy + b) * sz + c) * 6]);
       }
   o.demag = true;
-  o.demag_age = 0;
+  o.demag_age = 0; o.stray_dirty = true;
 }
 void orc_set_demag_every(void* h, int every) {
   Oracle& o = *static_cast<Oracle*>(h);
@@ -964,6 +1023,22 @@ void orc_demag_cells(void* h, double* out, int64_t dims[3]) {
   if (out) for (size_t t = 0; t < Bd.size(); ++t) out[t] = Bd[t];
 }
 
+// Stray field of the frozen track (reading D4) on / off; range_cells = 0: every track cell is a source.  Needs the
+// demagnetising field (its cell geometry).  Returns 0, or 4 if orc_enable_demag has not been called.
+int orc_enable_track_stray(void* h, int on, int range_cells) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  if (!o.demag) return 4;
+  o.stray = on != 0; o.stray_range = range_cells > 0 ? range_cells : 0; o.stray_dirty = true; o.demag_age = 0;
+  return 0;
+}
+// The track's stray field per window macrocell for the current window origin and track state, Tesla: out[dcx*dcy*dcz*3].
+void orc_stray_cells(void* h, double* out) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  std::vector<double> Bs;
+  stray_cells(o, Bs);
+  for (size_t t = 0; t < Bs.size(); ++t) out[t] = Bs[t];
+}
+
 void orc_set_field_scale(void* h, float s) { static_cast<Oracle*>(h)->scale = (double)s; }
 
 void orc_step_heun(void* h, int64_t n) {
@@ -976,7 +1051,7 @@ void orc_field(void* h, int with_noise, double* bx, double* by, double* bz) {
   Oracle& o = *static_cast<Oracle*>(h);
   if (o.mm) mm_exchange(o);
   std::vector<double> Bd;
-  if (o.demag) demag_cells(o, o.sx.data(), o.sy.data(), o.sz.data(), Bd);
+  if (o.demag) { demag_cells(o, o.sx.data(), o.sy.data(), o.sz.data(), Bd); add_stray(o, Bd); }
   for (int i = 0; i < o.nx; ++i)
     for (int k = 0; k < o.nz; ++k)
       for (int j = 0; j < o.ny; ++j) {
@@ -1072,6 +1147,7 @@ int orc_shift_window(void* h, int32_t p) {
   // S3 incoming: planes i >= nx-p; new global plane gx = x0 + p + i.
   for (int i = nx - p; i < nx; ++i) seed_plane(o, i, o.x0 + p + i);
   o.x0 += p; o.shift += 1;                              // S4: T and B are NOT moved
+  o.stray_dirty = true;
   return 0;
 }
 
@@ -1103,6 +1179,7 @@ int orc_track_end_pass(void* h) {
     if (o.out_cnt[c] == 0) continue;
     for (int a = 0; a < 3; ++a) o.init_mean[3 * c + a] = o.out_sum[3 * c + a] / (double)o.out_cnt[c];
   }
+  o.stray_dirty = true; o.demag_age = 0;
   return 0;
 }
 
@@ -1121,7 +1198,7 @@ int orc_track_begin_pass(void* h, int64_t x0_new) {
   for (size_t c = 0; c < nc; ++c) { o.out_cnt[c] = 0; o.out_sum[3 * c] = o.out_sum[3 * c + 1] = o.out_sum[3 * c + 2] = 0.0; }
   o.pass += 1;
   o.x0 = x0_new;
-  o.demag_age = 0;
+  o.demag_age = 0; o.stray_dirty = true;
   for (int i = 0; i < o.nx; ++i) seed_plane(o, i, o.x0 + i);
   if (o.mm) { mm_init_from_track(o); o.mm_age = 0; mm_refresh_params(o); }
   return 0;
@@ -1155,6 +1232,7 @@ void orc_track_read_scan(void* h, double y_r, double sigma_x, double sigma_y, do
 
 void orc_track_set_init(void* h, const float* mean_spin /* [ncell*3] or null */, float m0) {
   Oracle& o = *static_cast<Oracle*>(h);
+  o.stray_dirty = true; o.demag_age = 0;
   const size_t nc = (size_t)(o.ncx * o.ncy * o.ncz);
   for (size_t c = 0; c < nc; ++c)
     for (int a = 0; a < 3; ++a)

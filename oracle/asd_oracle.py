@@ -132,6 +132,9 @@ def lib():
         L.orc_set_demag_every.argtypes = [C.c_void_p, C.c_int]
         L.orc_newell_tensor.argtypes = [dp, dp, dp]
         L.orc_demag_cells.argtypes = [C.c_void_p, dp, ip64]
+        L.orc_enable_track_stray.restype = C.c_int
+        L.orc_enable_track_stray.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        L.orc_stray_cells.argtypes = [C.c_void_p, dp]
         _lib = L
     return _lib
 
@@ -314,6 +317,18 @@ class Oracle:
         lib().orc_demag_cells(self._h, None, _ptr(dims, C.c_int64))
         out = np.zeros((int(dims[0]), int(dims[1]), int(dims[2]), 3))
         lib().orc_demag_cells(self._h, _ptr(out, C.c_double), _ptr(dims, C.c_int64))
+        return out
+
+    def enable_track_stray(self, on: bool = True, range_cells: int = 0) -> int:
+        """Stray field of the frozen track on the window's macrocells (needs enable_demag); 0 = every track cell."""
+        return int(lib().orc_enable_track_stray(self._h, int(bool(on)), int(range_cells)))
+
+    def stray_cells(self) -> np.ndarray:
+        """The track's stray field per window macrocell, Tesla: [dcx, dcy, dcz, 3]."""
+        dims = np.zeros(3, dtype=np.int64)
+        lib().orc_demag_cells(self._h, None, _ptr(dims, C.c_int64))
+        out = np.zeros((int(dims[0]), int(dims[1]), int(dims[2]), 3))
+        lib().orc_stray_cells(self._h, _ptr(out, C.c_double))
         return out
 
     def set_field_scale(self, s: float):

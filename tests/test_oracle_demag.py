@@ -11,6 +11,9 @@ checked against things that are not the oracle's formula:
   * the thin-film limit: an extended film magnetised along its normal has B_d -> -mu_0 M at its centre, and -> 0 in plane.
 """
 import numpy as np
+import pytest
+
+import asd_inputs as ai
 
 from oracle import asd_oracle as orc
 from tests.helpers import single_grain_spec
@@ -120,3 +123,95 @@ def test_p12_field_enters_the_effective_field_and_the_step():
     assert np.abs(cells).max() > 1e-3                          # it is not nothing: ~0.1 T scale
     o0.step_heun(1); o1.step_heun(1)
     assert np.abs(o1.get_spins() - o0.get_spins()).max() > 1e-9
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Stray field of the frozen track (reading D4): pinned to the window demagnetising field above
+# (itself pinned by P12) through the identity  "a window's own field + the field of everything outside it = the field
+# of the whole track", with the whole track held by a second oracle whose window IS the track.
+# ---------------------------------------------------------------------------------------------------------------
+def _cellwise_track(track_nx, ny, nz, macro, seed):
+    """A granular track whose spins are uniform inside every macrocell (one random direction per cell), so that a cell's
+    mean spin describes any part of it exactly."""
+    w = ai.small_film(ai.SC, track_nx, ny, nz, extra_track=0, macro=macro, pitch_nm=3.0, boundary_nm=0.6)
+    rng = np.random.default_rng(seed)
+    mx, my, mz = macro
+    ncx, ncy, ncz = -(-track_nx // mx), -(-ny // my), -(-nz // mz)
+    d = rng.standard_normal((ncx, ncy, ncz, 3)); d /= np.linalg.norm(d, axis=-1, keepdims=True)
+    d = d.astype(np.float32).astype(np.float64)
+    i, k, j = np.meshgrid(np.arange(track_nx), np.arange(nz), np.arange(ny), indexing="ij")
+    S = np.moveaxis(d[i // mx, j // my, k // mz], -1, 0) * w.magnetic_mask()[None]
+    return w, d, S                                            # S: [3, track_nx, nz, ny]
+
+
+@pytest.mark.parametrize("start,shifts", [(0, (4, 6)), (4, (3, 5, 2)), (8, ())])
+def test_d4_track_stray_field_completes_the_window_field_to_the_whole_track_field(start, shifts):
+    track_nx, ny, nz, macro, nx = 40, 8, 4, (4, 4, 2), 12
+    wt, d, S = _cellwise_track(track_nx, ny, nz, macro, seed=5)
+    sp = [a * 1e-9 for a in wt.spacing_nm]
+    whole = orc.from_workload(wt)
+    whole.set_spins_f64(S.reshape(3, -1))
+    whole.enable_demag(sp)
+    B_full = whole.demag_cells()                              # [10, 2, 2, 3]
+    # the window: the same track, 12 planes long, walked from `start` by the given shifts; after every shift its spins are
+    # put back to the track's (a shift seeds the incoming planes at random), so what has left it is exactly the track
+    import copy
+    ww = copy.copy(wt)
+    ww.nx, ww.x0 = nx, start
+    plane = ny * nz
+    for name in ("T", "Bx", "By", "Bz", "sx", "sy", "sz"):
+        setattr(ww, name, getattr(wt, name)[:nx * plane].copy())
+    o = orc.from_workload(ww)
+    o.track_set_init(d.reshape(-1, 3).astype(np.float32))     # what lies ahead (and behind, where the window never was)
+    x0 = start
+    o.set_spins_f64(S[:, x0:x0 + nx].reshape(3, -1))
+    for p in shifts:
+        assert o.shift_window(p) == 0
+        x0 += p
+        o.set_spins_f64(S[:, x0:x0 + nx].reshape(3, -1))
+    o.enable_demag(sp)
+    assert o.enable_track_stray(True, 0) == 0
+    own, stray = o.demag_cells(), o.stray_cells()
+    c0 = x0 // macro[0]
+    ncw = (x0 + nx - 1) // macro[0] - c0 + 1
+    total = own[:ncw] + stray[:ncw]
+    assert np.abs(stray[:ncw]).max() > 1e-3                   # tens of millitesla: not a small correction
+    assert np.abs(total - B_full[c0:c0 + ncw]).max() < 1e-9 * max(1.0, np.abs(B_full).max()) + 1e-10
+    assert not stray[ncw:].any()
+    # a range that covers the track changes nothing; a short range drops the far cells (a smaller field, same sign structure)
+    assert o.enable_track_stray(True, 10) == 0
+    assert np.array_equal(o.stray_cells(), stray)
+    assert o.enable_track_stray(True, 1) == 0
+    near = o.stray_cells()
+    assert 0.0 < np.abs(near - stray).max() < np.abs(stray).max()
+
+
+def test_d4_stray_field_enters_the_effective_field_and_follows_the_window():
+    track_nx, ny, nz, macro, nx = 40, 8, 4, (4, 4, 2), 12
+    wt, d, S = _cellwise_track(track_nx, ny, nz, macro, seed=6)
+    import copy
+    ww = copy.copy(wt)
+    ww.nx, ww.x0 = nx, 8
+    plane = ny * nz
+    for name in ("T", "Bx", "By", "Bz", "sx", "sy", "sz"):
+        setattr(ww, name, getattr(wt, name)[:nx * plane].copy())
+    sp = [a * 1e-9 for a in wt.spacing_nm]
+    a, b = orc.from_workload(ww), orc.from_workload(ww)
+    for o in (a, b):
+        o.track_set_init(d.reshape(-1, 3).astype(np.float32))
+        o.set_spins_f64(S[:, 8:20].reshape(3, -1))
+        o.enable_demag(sp)
+    assert orc.from_workload(ww).enable_track_stray(True, 0) == 4          # needs the demagnetising field's cells
+    b.enable_track_stray(True, 0)
+    # every site sees its cell's stray field on top of the rest of the effective field
+    diff = (b.field() - a.field()).reshape(3, nx, nz, ny)
+    st = b.stray_cells()
+    i, k, j = np.meshgrid(np.arange(nx), np.arange(nz), np.arange(ny), indexing="ij")
+    want = np.moveaxis(st[(8 + i) // macro[0] - 2, j // macro[1], k // macro[2]], -1, 0) * ww.magnetic_mask()[None]
+    assert np.abs(diff - want).max() < 1e-12
+    # ... in both Heun stages, and it is recomputed when the window moves
+    a.step_heun(1); b.step_heun(1)
+    assert np.abs(a.get_spins() - b.get_spins()).max() > 1e-9
+    before = b.stray_cells().copy()
+    b.shift_window(4)
+    assert np.abs(b.stray_cells() - before).max() > 1e-6
