@@ -184,7 +184,8 @@ def _captured(workload: str, kernel_prefix: str):
 class Run:
     """One context on one workload: warm-up, device-timed bench steps (Heun batches + the schedule's shifts)."""
 
-    def __init__(self, asd, torch, w, device, hps, kernel="auto", ell=False, demag=False, demag_every=0, multiscale=None):
+    def __init__(self, asd, torch, w, device, hps, kernel="auto", ell=False, demag=False, demag_every=0, multiscale=None,
+                 track_stray=False):
         self.asd, self.torch, self.w, self.hps = asd, torch, w, hps
         self.N = w.n_sites
         table = None
@@ -198,6 +199,8 @@ class Run:
         if demag:
             self.ctx.enable_demag([a * 1e-9 for a in w.spacing_nm])
             self.ctx.set_demag_every(demag_every)
+            if track_stray:                              # + the frozen track's stray field, recomputed at every shift
+                self.ctx.enable_track_stray(True, 0)
         if multiscale is not None:                   # micromagnetic meshes either side
             ai.apply_multiscale(self.ctx, multiscale)
         if kernel != "auto":
@@ -325,7 +328,7 @@ def run_ours(args):
     N = w.n_sites
     hps = args.heun_per_step
     run = Run(asd, torch, w, device, hps, kernel=args.kernel, ell=args.ell, demag=args.demag, demag_every=args.demag_every,
-              multiscale=msw)
+              multiscale=msw, track_stray=args.track_stray)
     ctx, dev = run.ctx, run.ctx.device
     run.start(args.warmup, args.steps)
     barrier()
@@ -378,6 +381,7 @@ def run_ours(args):
         "config": {"workload": w.name, "sites": N, "heun_steps_per_step": hps, "shifts_in_timed_region": t["shifts"],
                    "shift_every_heun_steps": w.shift_every, "dt": w.dt, "parallelism": f"replicas x{world}",
                    "ell_width": run.ell_w, "demag": bool(args.demag), "demag_every": args.demag_every if args.demag else None,
+                   "track_stray": bool(args.demag and args.track_stray),
                    "kernel": args.kernel, "multiscale": ({"mesh_cells": list(msw.mcx), "every": msw.every} if msw else None),
                    "l2": "working set (13 fp32 arrays/site = %.0f MB) exceeds the 126 MB L2" % (13 * 4 * N / 1e6)},
         "clocks": clocks, "gpu_launches": int(t["launches"]),
@@ -573,6 +577,8 @@ def main():
                     help="switch the demagnetising field on (Eq. (6)-(7): coarse-graining + FFT convolution per stage)")
     ap.add_argument("--demag-every", type=int, default=0,
                     help="0: demag field recomputed in every Heun stage; P >= 1: every P-th step, held in between")
+    ap.add_argument("--track-stray", action="store_true",
+                    help="with --demag: also the stray field of the frozen track (DESIGN.md sec. 12, reading D4)")
     ap.add_argument("--multiscale", action="store_true",
                     help="the multiscale window: a micromagnetic LLG mesh either side of the atomistic mesh (DESIGN.md sec. 14)")
     ap.add_argument("--mm-every", type=int, default=20, help="Heun steps per RK4 step of the meshes")

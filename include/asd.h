@@ -178,6 +178,24 @@ ASD_API asd_status asd_demag_field(asd_ctx *ctx, float *cells, int64_t dims[3]);
  * enable / this call / window shift / asd_set_spins) and held for both stages in between (reading D3). */
 ASD_API asd_status asd_set_demag_every(asd_ctx *ctx, int32_t every);
 
+/* Stray field of the frozen track on the window ("the stray field generated by [the frozen track] is fully
+ * computed when the simulation window is shifted, and included in the simulation window at each iteration"; P:76;
+ * DESIGN.md sec. 12, reading D4).  Needs asd_enable_demag (it shares the macrocell geometry and rides on the cell field
+ * the Heun kernels already add).  Sources: of every track macrocell, the sites that are NOT inside the window --
+ *   mom_c' = out_sum_c' (what has left the window: the frozen spins themselves)
+ *          + init_mean_c' * (magnetic sites of the cell the window has never held),     M_c' = (mu_s / V) mom_c',
+ *   B_c = -mu_0 sum_c' N(r_c' - r_c) M_c'   over the track cells within range_cells of the target cell along x
+ *                                           (range_cells <= 0: the whole track),
+ * with the cuboid tensor of asd_enable_demag; a cell the window edge cuts is a source with its outside sites.  The field
+ * is recomputed (two small kernels, direct sum) at enable time and whenever the window origin or the track store
+ * changes: asd_shift_window, asd_track_set_init, asd_track_end_pass, asd_track_begin_pass.  Caller-owned DEVICE
+ * workspace (256-byte aligned) for the life of the context; on == 0 switches it off.  asd_track_stray_field copies the
+ * field per window macrocell to HOST cells[dims[0]*dims[1]*dims[2]*3] (layout of asd_demag_field) and synchronises.
+ * ASD_ESTATE without asd_enable_demag. */
+ASD_API size_t asd_track_stray_workspace_bytes(asd_ctx *ctx, int32_t range_cells);
+ASD_API asd_status asd_enable_track_stray(asd_ctx *ctx, int32_t on, int32_t range_cells, void *d_workspace, size_t bytes);
+ASD_API asd_status asd_track_stray_field(asd_ctx *ctx, float *cells);
+
 /* Window moves +x by p planes, 1 <= p <= nx (S:O5): outgoing planes -> macrocell sums and counts (Eq. 6);
  * spins move by p planes; incoming planes seeded by cone sampling (D:S3); x0 += p; shift counter += 1.
  * ASD_ESTATE if x0 + p + nx > track_nx; ASD_EUNSUPPORTED with a general ELL table or pbc[0]. */

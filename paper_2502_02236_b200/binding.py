@@ -26,7 +26,8 @@ EXPORTED_SYMBOLS = [
     "asd_track_dims", "asd_track_set_init", "asd_track_get",
     "asd_track_end_pass", "asd_track_begin_pass", "asd_track_read_scan",
     "asd_mm_workspace_bytes", "asd_mm_enable", "asd_mm_dims", "asd_mm_set_fields_host", "asd_mm_set_m_host",
-    "asd_mm_get_m_host", "asd_planes_view", "asd_magnetisation_planes", "asd_get_counters", "asd_set_counters",
+    "asd_mm_get_m_host", "asd_planes_view", "asd_magnetisation_planes",
+    "asd_track_stray_workspace_bytes", "asd_enable_track_stray", "asd_track_stray_field", "asd_get_counters", "asd_set_counters",
     "asd_launch_count", "asd_last_error", "asd_version",
 ]
 
@@ -112,6 +113,10 @@ def load_library(build_if_missing: bool = True):
     L.asd_enable_demag.argtypes = [C.c_void_p, dp, C.c_void_p, C.c_size_t]
     L.asd_demag_field.argtypes = [C.c_void_p, fp, C.POINTER(C.c_int64)]
     L.asd_set_demag_every.argtypes = [C.c_void_p, C.c_int32]
+    L.asd_track_stray_workspace_bytes.restype = C.c_size_t
+    L.asd_track_stray_workspace_bytes.argtypes = [C.c_void_p, C.c_int32]
+    L.asd_enable_track_stray.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_size_t]
+    L.asd_track_stray_field.argtypes = [C.c_void_p, fp]
     L.asd_shift_window.argtypes = [C.c_void_p, C.c_int32]
     L.asd_magnetisation.argtypes = [C.c_void_p, dp, dp]
     L.asd_grain_magnetisation.argtypes = [C.c_void_p, dp]
@@ -336,6 +341,27 @@ class Context:
         ptr = (self._demag_ws.data_ptr() + 255) & ~255
         a = (C.c_double * 3)(*[float(x) for x in spacing_m])
         self._ck(self._L.asd_enable_demag(self._h, a, C.c_void_p(ptr), C.c_size_t(nbytes)))
+
+    def enable_track_stray(self, on: bool = True, range_cells: int = 0):
+        """asd_enable_track_stray (allocates its workspace): the frozen track's stray field on the window's macrocells."""
+        import torch
+        if not on:
+            self._ck(self._L.asd_enable_track_stray(self._h, C.c_int32(0), C.c_int32(0), None, C.c_size_t(0)))
+            return
+        nbytes = int(self._L.asd_track_stray_workspace_bytes(self._h, C.c_int32(range_cells)))
+        if nbytes == 0:
+            raise AsdError(4, "asd_track_stray_workspace_bytes: asd_enable_demag has not been called")
+        self._stray_ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        ptr = (self._stray_ws.data_ptr() + 255) & ~255
+        self._ck(self._L.asd_enable_track_stray(self._h, C.c_int32(1), C.c_int32(range_cells), C.c_void_p(ptr), C.c_size_t(nbytes)))
+
+    def stray_cells(self) -> np.ndarray:
+        """asd_track_stray_field: [dcx, dcy, dcz, 3] Tesla."""
+        dims = (C.c_int64 * 3)()
+        self._ck(self._L.asd_demag_field(self._h, None, dims))
+        out = np.zeros((dims[0], dims[1], dims[2], 3), dtype=np.float32)
+        self._ck(self._L.asd_track_stray_field(self._h, C.c_void_p(out.ctypes.data)))
+        return out
 
     def set_demag_every(self, every: int):
         self._ck(self._L.asd_set_demag_every(self._h, C.c_int32(every)))

@@ -440,6 +440,29 @@ asd_status asd_demag_field(asd_ctx* ctx, float* cells, int64_t dims[3]) {
   return demag_field_host(c, cells, dims);
 }
 
+size_t asd_track_stray_workspace_bytes(asd_ctx* ctx, int32_t range_cells) {
+  if (!ctx) return 0;
+  return demag_stray_workspace_bytes(ctx->c, range_cells);
+}
+
+asd_status asd_enable_track_stray(asd_ctx* ctx, int32_t on, int32_t range_cells, void* d_workspace, size_t bytes) {
+  CTX_OR_RETURN(ctx);
+  if (!c.demag) return fail(c, ASD_ESTATE, "asd_enable_track_stray: asd_enable_demag has not been called");
+  if (on && (!d_workspace || ((uintptr_t)d_workspace & 255u)))
+    return fail(c, ASD_EINVAL, "asd_enable_track_stray: workspace NULL or not 256-byte aligned");
+  return demag_stray_enable(c, on, range_cells, d_workspace, bytes);
+}
+
+asd_status asd_track_stray_field(asd_ctx* ctx, float* cells) {
+  CTX_OR_RETURN(ctx);
+  if (!cells) return fail(c, ASD_EINVAL, "asd_track_stray_field: cells is NULL");
+  if (!demag_stray_on(c)) return fail(c, ASD_ESTATE, "asd_track_stray_field: asd_enable_track_stray has not been called");
+  return demag_stray_field_host(c, cells);
+}
+
+// the track's stray field belongs to one window origin and one track state
+static asd_status then_refresh_stray(Ctx& c, asd_status st) { return st == ASD_OK ? demag_stray_refresh(c) : st; }
+
 asd_status asd_shift_window(asd_ctx* ctx, int32_t p) {
   CTX_OR_RETURN(ctx);
   if (p < 1 || p > c.d.nx) return fail(c, ASD_EINVAL, "asd_shift_window: p must be in 1..nx");
@@ -455,9 +478,9 @@ asd_status asd_shift_window(asd_ctx* ctx, int32_t p) {
     if (p % mx != 0 || p / mx > dl[0] || p / mx > dr[0])
       return fail(c, ASD_EINVAL, "asd_shift_window: a multiscale window moves by whole macrocells, at most the shorter mesh");
     if ((c.x0 + c.d.nx) / mx + dr[0] + p / mx > c.ncx) return fail(c, ASD_ESTATE, "asd_shift_window: leading mesh past the end of the track");
-    return launch_shift_mm(c, p);
+    return then_refresh_stray(c, launch_shift_mm(c, p));
   }
-  return launch_shift(c, p);
+  return then_refresh_stray(c, launch_shift(c, p));
 }
 
 asd_status asd_magnetisation(asd_ctx* ctx, double m[3], double* n_magnetic) {
@@ -520,7 +543,7 @@ asd_status asd_track_set_init(asd_ctx* ctx, const float* mean_spin, float m0) {
   if (e == cudaSuccess) e = cudaStreamSynchronize(c.stream);
   cudaFreeHost(im);
   if (e != cudaSuccess) return fail_cuda(c, e, "asd_track_set_init copy");
-  return launch_cell_frames(c);
+  return then_refresh_stray(c, launch_cell_frames(c));
 }
 
 asd_status asd_track_get(asd_ctx* ctx, double* sum, int64_t* count) {
@@ -534,7 +557,7 @@ asd_status asd_track_get(asd_ctx* ctx, double* sum, int64_t* count) {
 asd_status asd_track_end_pass(asd_ctx* ctx) {
   CTX_OR_RETURN(ctx);
   if (c.d.ell_width > 0) return fail(c, ASD_EUNSUPPORTED, "asd_track_end_pass: a general ELL table has no track");
-  return launch_track_end_pass(c);
+  return then_refresh_stray(c, launch_track_end_pass(c));
 }
 
 asd_status asd_track_begin_pass(asd_ctx* ctx, int64_t x0_new) {
@@ -551,7 +574,7 @@ asd_status asd_track_begin_pass(asd_ctx* ctx, int64_t x0_new) {
   }
   graphs_invalidate(c);
   c.demag_age = 0;
-  return launch_track_begin_pass(c, x0_new);
+  return then_refresh_stray(c, launch_track_begin_pass(c, x0_new));
 }
 
 asd_status asd_track_read_scan(asd_ctx* ctx, double y_r, double sigma_x, double sigma_y, double x_first, double x_step,

@@ -52,6 +52,12 @@ struct DemagPlan {
   float2* twy = nullptr;              // [PY]   exp(+2 pi i n / PY)
   unsigned xconv_threads = 0;
   size_t xconv_smem = 0;
+  // stray field of the frozen track on the window's macrocells (reading D4); own workspace
+  bool stray = false;
+  int XR = 0;                         // largest |x offset| in cells between a source and a target cell
+  float* Nt = nullptr;                // [2 XR + 1][2 dcy - 1][2 dcz - 1][6] cuboid tensor times -mu_0 mu_s / V
+  float* mom = nullptr;               // [track cells][3] sum of the frozen spins of a cell that lie outside the window
+  float* Bt = nullptr;                // [3][dcx][dcy][dcz] the track's stray field, Tesla (added by demag_yinv)
 };
 
 namespace {
@@ -421,7 +427,7 @@ demag_xconv(const float2* __restrict__ Y, float2* __restrict__ Z, const float* _
 // thread and pass.
 constexpr int kYinvCols = 8;
 __global__ void demag_yinv(const float2* __restrict__ Z, const float2* __restrict__ twy, float* __restrict__ B,
-                           int dcx, int dcy, int dcz, int PY, int NKY) {
+                           int dcx, int dcy, int dcz, int PY, int NKY, const float* __restrict__ Bt) {
   extern __shared__ __align__(16) float2 zs[];                   // [NKY][8] | tws[PY]
   float2* tws = zs + NKY * kYinvCols;
   const int F = 3 * dcz, f = blockIdx.y, a0 = blockIdx.x * kYinvCols;
@@ -453,7 +459,74 @@ __global__ void demag_yinv(const float2* __restrict__ Z, const float2* __restric
       const float2 z0 = zs[ky * kYinvCols + da];
       acc0 = fmaf(z0.x, w0.x, fmaf(-z0.y, w0.y, acc0));
     }
-    B[(((size_t)comp * dcx + (a0 + da)) * dcy + b) * dcz + c] = acc0 + acc1;
+    const size_t o = (((size_t)comp * dcx + (a0 + da)) * dcy + b) * dcz + c;
+    B[o] = acc0 + acc1 + (Bt ? Bt[o] : 0.0f);            // + the frozen track's stray field (static between shifts)
+  }
+}
+
+// ---- stray field of the frozen track (reading D4) ----
+// Outside moment of every track cell in columns [cx_lo, cx_hi]: what has left the window (out_sum: the frozen spins
+// themselves) plus the init mean spin times the number of magnetic sites the window has never held.
+__global__ void stray_moments_kernel(const uint32_t* __restrict__ col_track, const double* __restrict__ out_sum,
+                                     const long long* __restrict__ out_cnt, const float* __restrict__ init_mean,
+                                     float* __restrict__ mom, long long cx_lo, long long cx_hi, int ncy, int ncz, int mx,
+                                     int my, int mz, int ny, int nz, long long track_nx, long long x0, int nx) {
+  const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long n = (cx_hi - cx_lo + 1) * ncy * ncz;
+  if (r >= n) return;
+  const int c2 = (int)(r % ncz), b2 = (int)((r / ncz) % ncy);
+  const long long cx = cx_lo + r / ((long long)ncz * ncy);
+  const int kext = min((c2 + 1) * mz, nz) - c2 * mz;
+  long long n_out = 0;
+  for (long long gx = cx * mx; gx < min((cx + 1) * (long long)mx, track_nx); ++gx) {
+    if (gx >= x0 && gx < x0 + nx) continue;
+    for (int j = b2 * my; j < min((b2 + 1) * my, ny); ++j)
+      if ((col_track[gx * ny + j] & 0xFFFFu) != 0u) n_out += kext;
+  }
+  const long long t = (cx * ncy + b2) * ncz + c2;
+  const double fresh = (double)(n_out - out_cnt[t]);
+  for (int u = 0; u < 3; ++u) mom[3 * t + u] = (float)(out_sum[3 * t + u] + (double)init_mean[3 * t + u] * fresh);
+}
+
+// B_c = sum_c' Nt(r_c' - r_c) mom_c' for the window cells of one x column (blockIdx.x = a); thread = (b, c).  Source
+// columns are taken one at a time through shared memory, in ascending order (deterministic); all-zero columns (the
+// window's interior) are skipped.
+__global__ void stray_sum_kernel(const float* __restrict__ Nt, const float* __restrict__ mom, float* __restrict__ Bt,
+                                 long long c0, long long cx_lo, long long cx_hi, int XR, int dcx, int dcy, int dcz,
+                                 int ncy, int ncz) {
+  extern __shared__ float sm_mom[];                              // [ncy*ncz][3]
+  const int a = blockIdx.x, ncol = ncy * ncz;
+  const int sy = 2 * dcy - 1, sz = 2 * dcz - 1;
+  for (int tgt0 = 0; tgt0 < dcy * dcz; tgt0 += blockDim.x) {
+    const int tgt = tgt0 + threadIdx.x;
+    const bool on = tgt < dcy * dcz;
+    const int b = on ? tgt / dcz : 0, c = on ? tgt - b * dcz : 0;
+    float acc[3] = {0.f, 0.f, 0.f};
+    for (long long cx = cx_lo; cx <= cx_hi; ++cx) {
+      const long long dx = cx - (c0 + a);
+      if (dx > XR || dx < -XR) continue;                          // uniform over the block
+      int nz_any = 0;
+      __syncthreads();
+      for (int t = threadIdx.x; t < 3 * ncol; t += blockDim.x) {
+        const float v = mom[3 * cx * ncol + t];
+        sm_mom[t] = v;
+        nz_any |= (v != 0.0f);
+      }
+      if (!__syncthreads_or(nz_any)) continue;
+      if (on) {
+        const float* Nx = Nt + (size_t)(dx + XR) * sy * sz * 6;
+        for (int b2 = 0; b2 < ncy; ++b2)
+          for (int c2 = 0; c2 < ncz; ++c2) {
+            const float* N = Nx + ((size_t)(b2 - b + dcy - 1) * sz + (c2 - c + dcz - 1)) * 6;
+            const float m0 = sm_mom[3 * (b2 * ncz + c2)], m1 = sm_mom[3 * (b2 * ncz + c2) + 1], m2 = sm_mom[3 * (b2 * ncz + c2) + 2];
+            acc[0] = fmaf(N[0], m0, fmaf(N[3], m1, fmaf(N[4], m2, acc[0])));
+            acc[1] = fmaf(N[3], m0, fmaf(N[1], m1, fmaf(N[5], m2, acc[1])));
+            acc[2] = fmaf(N[4], m0, fmaf(N[5], m1, fmaf(N[2], m2, acc[2])));
+          }
+      }
+    }
+    if (on)
+      for (int u = 0; u < 3; ++u) Bt[(((size_t)u * dcx + a) * dcy + b) * dcz + c] = acc[u];
   }
 }
 
@@ -577,6 +650,96 @@ asd_status demag_enable(Ctx& c, const double spacing[3], void* ws, size_t bytes)
   return ASD_OK;
 }
 
+// ---- stray field of the frozen track: workspace, enable, refresh ----
+static int stray_xr(const Ctx& c, int range_cells) {
+  const int far = (int)c.ncx - 1;
+  return (range_cells > 0 && range_cells < far) ? range_cells : (far > 0 ? far : 0);
+}
+struct StrayCarve { size_t Nt, mom, Bt, total; };
+static void stray_carve(const Ctx& c, const DemagPlan& pl, int XR, StrayCarve& cv) {
+  size_t off = 0;
+  auto take = [&](size_t bytes) { const size_t o = off; off = align_up(off + bytes, 256); return o; };
+  cv.Nt = take((size_t)(2 * XR + 1) * (2 * pl.dcy - 1) * (2 * pl.dcz - 1) * 6 * sizeof(float));
+  cv.mom = take((size_t)c.ncell * 3 * sizeof(float));
+  cv.Bt = take((size_t)3 * pl.dcx * pl.dcy * pl.dcz * sizeof(float));
+  cv.total = off;
+}
+size_t demag_stray_workspace_bytes(Ctx& c, int range_cells) {
+  if (!c.demag) return 0;
+  StrayCarve cv;
+  stray_carve(c, *c.demag, stray_xr(c, range_cells), cv);
+  return cv.total;
+}
+
+// The field the frozen track adds to every window macrocell, for the current window origin and track state.
+asd_status demag_stray_refresh(Ctx& c) {
+  if (!c.demag || !c.demag->stray) return ASD_OK;
+  DemagPlan& pl = *c.demag;
+  const int mx = c.d.macro[0];
+  const long long c0 = c.x0 / mx, c_last = (c.x0 + c.d.nx - 1) / mx;
+  const long long cx_lo = std::max<long long>(0, c0 - pl.XR), cx_hi = std::min<long long>(c.ncx - 1, c_last + pl.XR);
+  const long long n = (cx_hi - cx_lo + 1) * c.ncy * c.ncz;
+  stray_moments_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c.stream>>>(
+      c.col, c.out_sum, c.out_cnt, c.init_mean, pl.mom, cx_lo, cx_hi, (int)c.ncy, (int)c.ncz, mx, c.d.macro[1], c.d.macro[2],
+      c.d.ny, c.d.nz, (long long)c.d.track_nx, (long long)c.x0, c.d.nx);
+  ASD_LAUNCH_CHECK(c, "stray_moments");
+  ASD_CUDA_TRY(c, cudaMemsetAsync(pl.Bt, 0, (size_t)3 * pl.dcx * pl.dcy * pl.dcz * sizeof(float), c.stream));
+  const int ncw = (int)(c_last - c0 + 1);
+  const int threads = std::min(1024, (int)align_up((size_t)(pl.dcy * pl.dcz), 32));
+  stray_sum_kernel<<<(unsigned)ncw, threads, (size_t)c.ncy * c.ncz * 3 * sizeof(float), c.stream>>>(
+      pl.Nt, pl.mom, pl.Bt, c0, cx_lo, cx_hi, pl.XR, pl.dcx, pl.dcy, pl.dcz, (int)c.ncy, (int)c.ncz);
+  ASD_LAUNCH_CHECK(c, "stray_sum");
+  c.demag_age = 0;                                              // a held cell field was made with the old stray field
+  return ASD_OK;
+}
+
+asd_status demag_stray_enable(Ctx& c, int on, int range_cells, void* ws, size_t bytes) {
+  DemagPlan& pl = *c.demag;
+  if (!on) { pl.stray = false; c.demag_age = 0; return ASD_OK; }
+  const int XR = stray_xr(c, range_cells);
+  StrayCarve cv;
+  stray_carve(c, pl, XR, cv);
+  if (bytes < cv.total) { std::snprintf(c.err, sizeof(c.err), "asd_enable_track_stray: workspace too small"); return ASD_ENOMEM; }
+  if ((size_t)c.ncy * c.ncz * 3 * sizeof(float) > 48 * 1024) {
+    std::snprintf(c.err, sizeof(c.err), "asd_enable_track_stray: more than 4096 macrocells per track cross-section");
+    return ASD_EUNSUPPORTED;
+  }
+  char* base = (char*)ws;
+  pl.Nt = (float*)(base + cv.Nt); pl.mom = (float*)(base + cv.mom); pl.Bt = (float*)(base + cv.Bt);
+  pl.XR = XR;
+  // cuboid tensor for every source-target offset (fp64 on the host, as for the window's own field), times -mu_0 mu_s / V
+  const int sy = 2 * pl.dcy - 1, sz = 2 * pl.dcz - 1;
+  const double V = pl.cell[0] * pl.cell[1] * pl.cell[2], scale = -4.0e-7 * kPi * c.d.mu_s / V;
+  std::vector<float> Nt((size_t)(2 * XR + 1) * sy * sz * 6);
+  for (int a = -XR; a <= XR; ++a)
+    for (int b = -(pl.dcy - 1); b <= pl.dcy - 1; ++b)
+      for (int g = -(pl.dcz - 1); g <= pl.dcz - 1; ++g) {
+        const double R[3] = {a * pl.cell[0], b * pl.cell[1], g * pl.cell[2]};
+        double N[6];
+        cuboid_tensor(pl.cell, R, N);
+        float* dst = Nt.data() + (((size_t)(a + XR) * sy + (b + pl.dcy - 1)) * sz + (g + pl.dcz - 1)) * 6;
+        for (int comp = 0; comp < 6; ++comp) dst[comp] = (float)(N[comp] * scale);
+      }
+  ASD_CUDA_TRY(c, cudaMemcpyAsync(pl.Nt, Nt.data(), Nt.size() * sizeof(float), cudaMemcpyHostToDevice, c.stream));
+  ASD_CUDA_TRY(c, cudaMemsetAsync(pl.mom, 0, (size_t)c.ncell * 3 * sizeof(float), c.stream));
+  ASD_CUDA_TRY(c, cudaStreamSynchronize(c.stream));
+  pl.stray = true;
+  return demag_stray_refresh(c);
+}
+
+// Host copy of the track's stray field per window macrocell (tests, diagnostics); synchronises.
+asd_status demag_stray_field_host(Ctx& c, float* out) {
+  DemagPlan& pl = *c.demag;
+  const size_t cells = (size_t)pl.dcx * pl.dcy * pl.dcz;
+  std::vector<float> h(3 * cells);
+  ASD_CUDA_TRY(c, cudaMemcpyAsync(h.data(), pl.Bt, 3 * cells * sizeof(float), cudaMemcpyDeviceToHost, c.stream));
+  ASD_CUDA_TRY(c, cudaStreamSynchronize(c.stream));
+  for (size_t q = 0; q < cells; ++q)
+    for (int comp = 0; comp < 3; ++comp) out[3 * q + comp] = h[comp * cells + q];
+  return ASD_OK;
+}
+bool demag_stray_on(const Ctx& c) { return c.demag && c.demag->stray; }
+
 namespace {
 template <typename... Args>
 void launch_chain(void (*kern)(Args...), dim3 grid, unsigned threads, size_t smem, cudaStream_t stream, Args... args) {
@@ -617,7 +780,8 @@ asd_status launch_demag(Ctx& c, int aX) {
   ASD_LAUNCH_CHECK(c, "demag_xconv");
   launch_chain(demag_yinv, dim3((unsigned)((pl.dcx + kYinvCols - 1) / kYinvCols), (unsigned)pl.F), 256u,
                ((size_t)pl.NKY * kYinvCols + pl.PY) * sizeof(float2), c.launch_stream,
-               (const float2*)pl.Z, (const float2*)pl.twy, pl.B, pl.dcx, pl.dcy, pl.dcz, pl.PY, pl.NKY);
+               (const float2*)pl.Z, (const float2*)pl.twy, pl.B, pl.dcx, pl.dcy, pl.dcz, pl.PY, pl.NKY,
+               (const float*)(pl.stray ? pl.Bt : nullptr));
   ASD_LAUNCH_CHECK(c, "demag_yinv");
   return ASD_OK;
 }

@@ -231,6 +231,11 @@ void demag_free(Ctx& c);
 asd_status launch_demag(Ctx& c, int aX);                      // field of the configuration in arrays aX..aX+2
 void demag_fill_params(const Ctx& c, StageParams& p);
 asd_status demag_field_host(Ctx& c, float* out, int64_t dims[3]);
+size_t demag_stray_workspace_bytes(Ctx& c, int range_cells);     // stray field of the frozen track (reading D4)
+asd_status demag_stray_enable(Ctx& c, int on, int range_cells, void* ws, size_t bytes);
+asd_status demag_stray_refresh(Ctx& c);                          // after the window origin or the track store changed
+asd_status demag_stray_field_host(Ctx& c, float* out);
+bool demag_stray_on(const Ctx& c);
 asd_status launch_heun_fast(Ctx& c, StageParams& p);          // one Heun step (2 kernels), fast path
 bool heun_fast_supported(const Ctx& c);
 asd_status launch_heun_ell(Ctx& c, StageParams& p);           // one Heun step (2 kernels), general ELL table

@@ -111,3 +111,73 @@ def test_demag_changes_the_dynamics_and_tma_is_refused():
     b.set_kernel(asd.KERNEL_TMA)
     with pytest.raises(asd.AsdError):
         b.step_heun(1)
+
+
+# ---- stray field of the frozen track (reading D4) ----
+def _stray_pair(lattice, x0=3, **kw):
+    """A window in the middle of a longer track with a non-trivial track state on both sides: what lies ahead is a random
+    mean spin per cell, what lies behind has been written by two shifts."""
+    w = ai.small_film(lattice, 21, 40, 6, extra_track=30, macro=(4, 5, 2), tilt_deg=30.0, dt=1e-16, **kw)
+    w.x0 = x0
+    sx, sy, sz = ai.tilted_spins(w.n_sites, 30.0, seed=23)
+    mag = w.magnetic_mask().reshape(-1)
+    w.sx, w.sy, w.sz = (sx * mag).astype(np.float32), (sy * mag).astype(np.float32), (sz * mag).astype(np.float32)
+    o, g = _pair(w)
+    rng = np.random.default_rng(31)
+    ncell = int(np.prod(o.track_dims()))
+    v = rng.standard_normal((ncell, 3)); v *= rng.uniform(0.5, 1.0, (ncell, 1)) / np.linalg.norm(v, axis=1, keepdims=True)
+    v = v.astype(np.float32)
+    o.track_set_init(v); g.track_set_init(v)
+    for p in (3, 4):
+        assert o.shift_window(p) == 0
+        g.shift_window(p)
+    return w, o, g
+
+
+@pytest.mark.parametrize("lattice", [ai.SC, ai.L10])
+@pytest.mark.parametrize("rng_cells", [0, 3])
+def test_track_stray_field_matches_oracle(lattice, rng_cells):
+    w, o, g = _stray_pair(lattice)
+    assert o.enable_track_stray(True, rng_cells) == 0
+    g.enable_track_stray(True, rng_cells)
+    Bo, Bg = o.stray_cells(), g.stray_cells()
+    scale = np.abs(Bo).max()
+    assert scale > 1e-3
+    assert np.abs(Bg - Bo).max() <= 3e-6 * max(scale, 1.0) + 1e-7
+    # the total cell field the kernels add = own demagnetising field + the track's
+    tot = g.demag_field()
+    assert np.abs(tot - (o.demag_cells() + Bo)).max() <= 5e-6 * max(scale, 1.0) + 2e-7
+    # recomputed when the window moves and when the track state changes
+    assert o.shift_window(2) == 0
+    g.shift_window(2)
+    assert np.abs(g.stray_cells() - o.stray_cells()).max() <= 3e-6 * max(scale, 1.0) + 1e-7
+    o.track_set_init(None, 0.7); g.track_set_init(None, 0.7)
+    Bo2 = o.stray_cells()
+    assert np.abs(Bo2 - Bo).max() > 1e-4
+    assert np.abs(g.stray_cells() - Bo2).max() <= 3e-6 * max(scale, 1.0) + 1e-7
+
+
+@pytest.mark.parametrize("lattice", [ai.SC, ai.L10])
+@pytest.mark.parametrize("kernel,every", [("general", 0), ("fast", 0), ("fast", 2), ("fused", 1)])
+def test_heun_steps_with_the_track_stray_field(lattice, kernel, every):
+    import paper_2502_02236_b200 as asd
+    w, o, g = _stray_pair(lattice)
+    o.enable_track_stray(True, 0); g.enable_track_stray(True, 0)
+    o.set_demag_every(every); g.set_demag_every(every)
+    g.set_kernel({"general": asd.KERNEL_GENERAL, "fast": asd.KERNEL_FAST, "fused": asd.KERNEL_FUSED}[kernel])
+    o.step_heun(1); g.step_heun(1)
+    assert max_abs_diff(g, o) <= 1e-5
+    o.step_heun(3); g.step_heun(3)
+    assert max_abs_diff(g, o) <= 5e-5
+    o.shift_window(3); g.shift_window(3)
+    o.step_heun(2); g.step_heun(2)
+    assert max_abs_diff(g, o) <= 1e-4
+
+
+def test_track_stray_needs_demag():
+    import paper_2502_02236_b200 as asd
+    w = ai.small_film(ai.SC, 12, 16, 4, extra_track=8)
+    g = gpu_from_workload(w)
+    with pytest.raises(asd.AsdError) as e:
+        g.enable_track_stray(True, 0)
+    assert e.value.status == 4
