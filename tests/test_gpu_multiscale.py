@@ -152,3 +152,25 @@ def test_passes_over_the_track_with_the_meshes(lattice):
     o.step_heun(3); g.step_heun(3)
     assert np.abs(o.get_spins() - g.get_spins_host()).max() <= 6e-5
     assert _mesh_diff(o, g) <= 2e-5
+
+
+def test_full_size_multiscale_window_one_coupled_step():
+    """The bench's multiscale workload at full size ([48-cell mesh | SC 336 x 200 x 27 atoms | 48-cell mesh], 1.81 M sites,
+    11 136 cells; the stage kernels' edge-field instances, as ASD_KERNEL_AUTO runs them): every site and every cell
+    against the oracle after one coupled step, then after a whole-cell shift and one more step."""
+    ms = ai.multiscale_film(ai.SC, every=1)
+    o, g = oracle_from_workload(ms.w), gpu_from_workload(ms.w)
+    ai.apply_multiscale(o, ms); ai.apply_multiscale(g, ms)
+    rng = np.random.default_rng(3)
+    for side in (0, 1):
+        v = np.array([0.0, 0.0, 1.0]) + 0.3 * rng.standard_normal(o.mm_shape(side) + (3,))
+        v = (v / np.linalg.norm(v, axis=-1, keepdims=True)).astype(np.float32)
+        o.mm_set_m(side, v); g.mm_set_m(side, v)
+    o.step_heun(1); g.step_heun(1)
+    assert np.abs(o.get_spins() - g.get_spins_host()).max() <= 1e-5
+    assert _mesh_diff(o, g) <= 1e-5
+    assert o.shift_window(7) == 0
+    g.shift_window(7)
+    o.step_heun(1); g.step_heun(1)
+    assert np.abs(o.get_spins() - g.get_spins_host()).max() <= 3e-5
+    assert _mesh_diff(o, g) <= 2e-5

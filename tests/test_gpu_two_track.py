@@ -110,3 +110,26 @@ def test_two_track_workload_two_passes(lattice):
         ro, rg = ai.read_tracks(o, tt), ai.read_tracks(g, tt)
         assert ro.shape == (2, 2) and np.abs(ro - rg).max() < 1e-4
     assert o.counters()["pass"] == 1
+
+
+def test_full_size_two_track_window_flush_and_scan():
+    """The two-track window at the demo's size (SC 400 x 268 x 27, 2.89 M sites; macrocells (7, 7, 7)): a shift, the flush
+    of the whole window, the committed track and the read-back scan against the oracle -- store bit-exact on
+    integer-valued spins, scan to 1e-12, regenerated window to 3e-6."""
+    tt = ai.two_track_film(ai.SC, n_bits=2)
+    w = _integer_valued(tt.w)
+    o, g = oracle_from_workload(w), gpu_from_workload(w)
+    o.shift_window(3); g.shift_window(3)
+    assert o.track_end_pass() == 0
+    g.track_end_pass()
+    _, cnt_o, sum_o = o.track_get()
+    sum_g, cnt_g = g.track_get()
+    assert np.array_equal(cnt_o, cnt_g) and np.array_equal(sum_o, sum_g)
+    c = tt.bit_centres()
+    for y in tt.track_y:
+        a = o.track_read_scan(y, tt.reader_sigma[0], tt.reader_sigma[1], float(c[0]), 5.0, 40)
+        b = g.track_read_scan(y, tt.reader_sigma[0], tt.reader_sigma[1], float(c[0]), 5.0, 40)
+        assert np.abs(a - b).max() <= 1e-12 * np.abs(a).max()
+    assert o.track_begin_pass(0) == 0
+    g.track_begin_pass(0)
+    assert np.abs(o.get_spins() - g.get_spins_host()).max() <= 3e-6
