@@ -31,12 +31,18 @@
 //
 // Units: B = mu_0 H in Tesla, energies in Joule, mu_s in J/T, gamma in rad s^-1 T^-1.
 //
-// Pins (tests/test_oracle_*.py): Philox vs ATen host engine; single-spin damped
+// Pins (tests/test_oracle_*.py; table in DESIGN.md sec. 3): Philox vs ATen host engine; single-spin damped
 // precession closed form; Langevin function; monotone energy; brute-force energy
 // gradient; |S|=1; spin-wave dispersion (fixes exchange normalisation and the L1_0
 // shell geometry); simple-cubic T_C = 1.44 J/k_B;
-// shift index exactness; seeded-slab magnetisation magnitude (P:68 purpose clause).
-// "parity unpinned": bit-pattern outcomes / read-head scans -- not computed here.
+// shift index exactness; seeded-slab magnetisation magnitude (P:68 purpose clause);
+// cuboid demagnetising tensor vs direct quadrature and sum rules (P12); track stray field vs the
+// whole-track field (D4); ELL branch, magnetisation divisors, held-field composition (round 2);
+// track passes and read-back scan (T1-T3); m_e(T), macrospin with alpha(T), RK4 order, mesh spin
+// waves, both directions of the mesh coupling, whole-cell shift (P13-P19).
+// "parity unpinned": the OUTCOME of a recording run (which grains end up reversed) and
+// the paper's TMR read-head signal (its solver is not part of the method; orc_track_read_scan
+// is a stated stand-in and is pinned as such).
 // ============================================================================
 #include <cmath>
 #include <cstdint>
