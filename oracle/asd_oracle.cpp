@@ -162,6 +162,7 @@ struct Oracle {
   int64_t demag_age = 0;           // steps since the held field was invalidated (enable, set_every, shift, set_spins)
   std::vector<double> demag_hold;  // the held per-macrocell field
   // stray field of the frozen track on the window's macrocells (reading D4); off unless enabled
+  bool track_exch = false;         // window ends exchange coupled to the frozen track (reading E1); off unless enabled
   bool stray = false;
   int stray_range = 0;             // source cells taken up to this many cells from a target cell along x; 0 = the whole track
   bool stray_dirty = true;         // window origin or track state changed since stray_B was computed
@@ -213,6 +214,8 @@ inline bool wrap(int& c, int n, int periodic) {
   return true;
 }
 
+bool track_direction(const Oracle& o, int64_t cx, int b, int c, double n[3]);   // defined with the multiscale window
+
 // Exchange sum  sum_j J_ij X_j  (Joule), Eq. (2) numerator, for site (i,k,j) in configuration X.
 // A bond is kept only if the neighbour exists, both ends are magnetic and in the same grain
 // (exchange-decoupled grains).
@@ -234,6 +237,20 @@ void exchange_sum(const Oracle& o, const double* X0, const double* X1, const dou
   const int noff = (o.lattice == 0) ? 6 : 10;
   for (int s = 0; s < noff; ++s) {
     int ii = i + offs[s].dx, jj = j + offs[s].dy, kk = k + offs[s].dz;
+    if (!o.mm && o.track_exch && !o.pbc[0] && (ii == -1 || ii == o.nx)) {
+      // Reading E1 ("the ends of the simulation window are exchange coupled to the track"): the neighbour spin beyond
+      // the window's first / last plane is the DIRECTION of the frozen track in the macrocell that holds the neighbour
+      // position (what the window has written there, else what lies ahead) -- as for a micromagnetic neighbour.
+      const int64_t gxn = o.x0 + ii;
+      if (gxn < 0 || gxn >= o.track_nx || jj < 0 || jj >= o.ny || kk < 0 || kk >= o.nz) continue;
+      const int32_t gn = o.grain_map[(size_t)(gxn * o.ny + jj)];
+      if (gn < 0 || gn != g) continue;                        // exchange-decoupled grains
+      double nd[3];
+      if (!track_direction(o, gxn / o.macro[0], jj / o.macro[1], kk / o.macro[2], nd)) continue;
+      const double Jij = o.J[offs[s].shell];
+      e[0] += Jij * nd[0]; e[1] += Jij * nd[1]; e[2] += Jij * nd[2];
+      continue;
+    }
     if (o.mm && (ii == -1 || ii == o.nx)) {
       // Across the mesh boundary: "For the contribution from the micromagnetic region the respective
       // magnetization direction is used directly" -- the neighbour spin of Eq. (2) is the direction m of the
@@ -1044,6 +1061,9 @@ void orc_stray_cells(void* h, double* out) {
   stray_cells(o, Bs);
   for (size_t t = 0; t < Bs.size(); ++t) out[t] = Bs[t];
 }
+
+// Window ends exchange coupled to the frozen track (reading E1); superseded by the meshes of a multiscale window.
+void orc_enable_track_exchange(void* h, int on) { static_cast<Oracle*>(h)->track_exch = on != 0; }
 
 void orc_set_field_scale(void* h, float s) { static_cast<Oracle*>(h)->scale = (double)s; }
 

@@ -135,6 +135,7 @@ def lib():
         L.orc_enable_track_stray.restype = C.c_int
         L.orc_enable_track_stray.argtypes = [C.c_void_p, C.c_int, C.c_int]
         L.orc_stray_cells.argtypes = [C.c_void_p, dp]
+        L.orc_enable_track_exchange.argtypes = [C.c_void_p, C.c_int]
         _lib = L
     return _lib
 
@@ -322,6 +323,10 @@ class Oracle:
     def enable_track_stray(self, on: bool = True, range_cells: int = 0) -> int:
         """Stray field of the frozen track on the window's macrocells (needs enable_demag); 0 = every track cell."""
         return int(lib().orc_enable_track_stray(self._h, int(bool(on)), int(range_cells)))
+
+    def enable_track_exchange(self, on: bool = True):
+        """The window's first / last plane exchange coupled to the frozen track's direction (reading E1)."""
+        lib().orc_enable_track_exchange(self._h, int(bool(on)))
 
     def stray_cells(self) -> np.ndarray:
         """The track's stray field per window macrocell, Tesla: [dcx, dcy, dcz, 3]."""
