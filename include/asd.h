@@ -178,6 +178,17 @@ ASD_API asd_status asd_demag_field(asd_ctx *ctx, float *cells, int64_t dims[3]);
  * enable / this call / window shift / asd_set_spins) and held for both stages in between (reading D3). */
 ASD_API asd_status asd_set_demag_every(asd_ctx *ctx, int32_t every);
 
+/* Window ends exchange coupled to the frozen track ("the ends of the simulation window are exchange coupled to the
+ * track"; reading E1), for a purely atomistic window (the meshes of asd_mm_enable take the ends over).  The
+ * neighbour spins beyond the first / last plane in Eq. (2) -- x-1 of plane 0, x+1 of plane nx-1, for L1_0 their two
+ * in-plane diagonals as well -- are the DIRECTION of the frozen track in the macrocell that holds the neighbour position
+ * (what the window has written there, else what lies ahead; as for a micromagnetic neighbour), subject to the
+ * same-grain rule.  Off by default (the ends are then open boundaries).  Recomputed whenever the window origin or the
+ * track store changes.  Caller-owned DEVICE workspace (256-byte aligned) for the life of the context.  Not with general
+ * ELL tables, pbc[0], ASD_KERNEL_TMA, ASD_KERNEL_PERSISTENT, CUDA-graph replay. */
+ASD_API size_t asd_track_exchange_workspace_bytes(const asd_ctx *ctx);
+ASD_API asd_status asd_enable_track_exchange(asd_ctx *ctx, int32_t on, void *d_workspace, size_t bytes);
+
 /* Stray field of the frozen track on the window ("the stray field generated by [the frozen track] is fully
  * computed when the simulation window is shifted, and included in the simulation window at each iteration"; P:76;
  * DESIGN.md sec. 12, reading D4).  Needs asd_enable_demag (it shares the macrocell geometry and rides on the cell field

@@ -27,7 +27,8 @@ EXPORTED_SYMBOLS = [
     "asd_track_end_pass", "asd_track_begin_pass", "asd_track_read_scan",
     "asd_mm_workspace_bytes", "asd_mm_enable", "asd_mm_dims", "asd_mm_set_fields_host", "asd_mm_set_m_host",
     "asd_mm_get_m_host", "asd_planes_view", "asd_magnetisation_planes",
-    "asd_track_stray_workspace_bytes", "asd_enable_track_stray", "asd_track_stray_field", "asd_get_counters", "asd_set_counters",
+    "asd_track_stray_workspace_bytes", "asd_enable_track_stray", "asd_track_stray_field",
+    "asd_track_exchange_workspace_bytes", "asd_enable_track_exchange", "asd_get_counters", "asd_set_counters",
     "asd_launch_count", "asd_last_error", "asd_version",
 ]
 
@@ -117,6 +118,9 @@ def load_library(build_if_missing: bool = True):
     L.asd_track_stray_workspace_bytes.argtypes = [C.c_void_p, C.c_int32]
     L.asd_enable_track_stray.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_size_t]
     L.asd_track_stray_field.argtypes = [C.c_void_p, fp]
+    L.asd_track_exchange_workspace_bytes.restype = C.c_size_t
+    L.asd_track_exchange_workspace_bytes.argtypes = [C.c_void_p]
+    L.asd_enable_track_exchange.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_size_t]
     L.asd_shift_window.argtypes = [C.c_void_p, C.c_int32]
     L.asd_magnetisation.argtypes = [C.c_void_p, dp, dp]
     L.asd_grain_magnetisation.argtypes = [C.c_void_p, dp]
@@ -354,6 +358,17 @@ class Context:
         self._stray_ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
         ptr = (self._stray_ws.data_ptr() + 255) & ~255
         self._ck(self._L.asd_enable_track_stray(self._h, C.c_int32(1), C.c_int32(range_cells), C.c_void_p(ptr), C.c_size_t(nbytes)))
+
+    def enable_track_exchange(self, on: bool = True):
+        """asd_enable_track_exchange (allocates its workspace): the window's ends exchange coupled to the frozen track."""
+        import torch
+        if not on:
+            self._ck(self._L.asd_enable_track_exchange(self._h, C.c_int32(0), None, C.c_size_t(0)))
+            return
+        nbytes = int(self._L.asd_track_exchange_workspace_bytes(self._h))
+        self._tex_ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        ptr = (self._tex_ws.data_ptr() + 255) & ~255
+        self._ck(self._L.asd_enable_track_exchange(self._h, C.c_int32(1), C.c_void_p(ptr), C.c_size_t(nbytes)))
 
     def stray_cells(self) -> np.ndarray:
         """asd_track_stray_field: [dcx, dcy, dcz, 3] Tesla."""

@@ -391,7 +391,7 @@ asd_status asd_set_kernel(asd_ctx* ctx, int32_t variant) {
     return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: the persistent cluster needs built-in shells, ny % 4 == 0, grains that do not touch, no demagnetising field or meshes, and x-slabs that fit a CTA");
   if (variant == ASD_KERNEL_FUSED && (!heun_fused_supported(c) || (c.demag && c.demag_every < 1) || !fused_plan(c)))
     return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: the fused step needs what the film kernel needs, a strip plan that fits in shared memory, and -- with the demagnetising field on -- the held-field scheme (asd_set_demag_every >= 1)");
-  if (variant == ASD_KERNEL_TMA && c.mm) return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: the staged film kernel does not take a multiscale window");
+  if (variant == ASD_KERNEL_TMA && edge_field_on(c)) return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: the staged film kernel takes neither a multiscale window nor track-coupled ends");
   if (variant == ASD_KERNEL_TMA && (!heun_tma_supported(c) || !tma_plan(c)))
     return fail(c, ASD_EUNSUPPORTED, "asd_set_kernel: the staged film kernel needs what the film kernel needs and a strip plan that fits in shared memory");
   if (variant == ASD_KERNEL_FAST && !heun_fast_supported(c))
@@ -440,6 +440,18 @@ asd_status asd_demag_field(asd_ctx* ctx, float* cells, int64_t dims[3]) {
   return demag_field_host(c, cells, dims);
 }
 
+size_t asd_track_exchange_workspace_bytes(const asd_ctx* ctx) { return ctx ? track_exchange_workspace_bytes(ctx->c) : 0; }
+
+asd_status asd_enable_track_exchange(asd_ctx* ctx, int32_t on, void* d_workspace, size_t bytes) {
+  CTX_OR_RETURN(ctx);
+  if (c.d.ell_width > 0 || c.d.pbc[0]) return fail(c, ASD_EUNSUPPORTED, "asd_enable_track_exchange: built-in shells, open in x");
+  if (c.kernel_variant == ASD_KERNEL_TMA) return fail(c, ASD_EUNSUPPORTED, "asd_enable_track_exchange: not with ASD_KERNEL_TMA");
+  if (on && (!d_workspace || ((uintptr_t)d_workspace & 255u)))
+    return fail(c, ASD_EINVAL, "asd_enable_track_exchange: workspace NULL or not 256-byte aligned");
+  graphs_invalidate(c);
+  return track_exchange_enable(c, on, d_workspace, bytes);
+}
+
 size_t asd_track_stray_workspace_bytes(asd_ctx* ctx, int32_t range_cells) {
   if (!ctx) return 0;
   return demag_stray_workspace_bytes(ctx->c, range_cells);
@@ -461,7 +473,11 @@ asd_status asd_track_stray_field(asd_ctx* ctx, float* cells) {
 }
 
 // the track's stray field belongs to one window origin and one track state
-static asd_status then_refresh_stray(Ctx& c, asd_status st) { return st == ASD_OK ? demag_stray_refresh(c) : st; }
+static asd_status then_refresh_stray(Ctx& c, asd_status st) {
+  if (st == ASD_OK) st = demag_stray_refresh(c);
+  if (st == ASD_OK) st = track_exchange_refresh(c);
+  return st;
+}
 
 asd_status asd_shift_window(asd_ctx* ctx, int32_t p) {
   CTX_OR_RETURN(ctx);

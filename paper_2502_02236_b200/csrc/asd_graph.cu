@@ -90,7 +90,7 @@ void graphs_free(Ctx& c) {
 
 asd_status launch_heun(Ctx& c, int64_t n) {
   c.launch_stream = c.stream;
-  const bool use = !c.demag && !c.mm &&         // the demag pipeline and the mesh steps are launched plainly
+  const bool use = !c.demag && !edge_field_on(c) &&         // the demag pipeline and the mesh steps are launched plainly
                    c.kernel_variant != ASD_KERNEL_FUSED &&   // the fused step swaps the spin buffers every step
                    c.kernel_variant != ASD_KERNEL_PERSISTENT &&
                    !(c.kernel_variant == ASD_KERNEL_AUTO && c.N <= (1 << 14) && heun_persist_supported(c)) &&   // one launch already

@@ -261,7 +261,7 @@ bool persist_shape(const Ctx& c, PersistShape& sh) {
 // per-stage global quantity (demagnetising field, mesh coupling), and a lattice that fits one cluster.
 bool heun_persist_supported(const Ctx& c) {
   PersistShape sh;
-  return c.d.ell_width == 0 && !c.grains_touch && !c.demag && !c.mm && (int64_t)AR_COUNT * c.as < (1ll << 31) &&
+  return c.d.ell_width == 0 && !c.grains_touch && !c.demag && !edge_field_on(c) && (int64_t)AR_COUNT * c.as < (1ll << 31) &&
          persist_shape(c, sh);
 }
 

@@ -181,6 +181,11 @@ struct Ctx {
   int64_t demag_age = 0;            // Heun steps since the held field was last invalidated (enable, shift, set_spins)
   int32_t demag_refresh = 3;        // this step: bit 0 = recompute before the predictor, bit 1 = before the corrector
   MmPlan* mm = nullptr;             // non-null once asd_mm_enable succeeded
+  // window ends exchange coupled to the frozen track (asd_enable_track_exchange; reading E1): the track's
+  // directions beyond the two ends and the edge field they make on planes 0 / nx-1 (caller's workspace)
+  bool tex_on = false;
+  float* tex_ghost = nullptr;       // [2][3][ncy*ncz]
+  float* tex_edgeB = nullptr;       // [2][3][nz*nyp]
   TmaPlan* tma_plan = nullptr;      // built lazily by the first staged launch (host memory, freed by asd_destroy)
   bool tma_plan_tried = false;
   FusedPlan* fused_plan = nullptr;  // likewise for the fused one-kernel step
@@ -260,7 +265,11 @@ asd_status mm_enable(Ctx& c, const asd_mm_desc& d, void* ws, size_t bytes);
 void mm_free(Ctx& c);
 asd_status mm_before_step(Ctx& c);                            // exchange + RK4 step when the cadence says so
 void mm_restart_cadence(Ctx& c);
-const float* mm_edge_field(const Ctx& c);
+const float* mm_edge_field(const Ctx& c);                       // the meshes' edge field, else the track's, else nullptr
+inline bool edge_field_on(const Ctx& c) { return c.mm != nullptr || c.tex_on; }
+size_t track_exchange_workspace_bytes(const Ctx& c);
+asd_status track_exchange_enable(Ctx& c, int on, void* ws, size_t bytes);
+asd_status track_exchange_refresh(Ctx& c);                      // after the window origin or the track store changed
 asd_status mm_set_fields_host(Ctx& c, int side, const float* T, const float* Bx, const float* By, const float* Bz);
 asd_status mm_set_m_host(Ctx& c, int side, const float* m);
 asd_status mm_get_m_host(Ctx& c, int side, float* m);

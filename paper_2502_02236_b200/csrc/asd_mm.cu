@@ -519,7 +519,56 @@ asd_status launch_rk4(Ctx& c, double h) {
 
 }  // namespace
 
-const float* mm_edge_field(const Ctx& c) { return c.mm ? c.mm->edgeB : nullptr; }
+const float* mm_edge_field(const Ctx& c) { return c.mm ? c.mm->edgeB : (c.tex_on ? c.tex_edgeB : nullptr); }
+
+// ---- window ends exchange coupled to the frozen track (reading E1), for a purely atomistic window ----
+namespace {
+// ghost[side][u][b*ncz + c] = direction of the frozen track in the macrocell that holds the plane just beyond the window
+// end (side 0: plane x0 - 1; side 1: plane x0 + nx); 0 where there is no track or no direction.
+__global__ void track_ghost_kernel(int ncy, int ncz, long long ncx, long long cxg0, long long cxg1,
+                                   const double* __restrict__ out_sum, const long long* __restrict__ out_cnt,
+                                   const float* __restrict__ init_mean, float* __restrict__ ghost) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x, ncol = ncy * ncz;
+  if (t >= 2 * ncol) return;
+  const int side = t / ncol, r = t - side * ncol;
+  const long long cx = side ? cxg1 : cxg0;
+  float n[3] = {0.f, 0.f, 0.f}, d[3];
+  if (cx >= 0 && cx < ncx && track_dir(out_sum, out_cnt, init_mean, cx * ncol + r, d)) { n[0] = d[0]; n[1] = d[1]; n[2] = d[2]; }
+  for (int u = 0; u < 3; ++u) ghost[(side * 3 + u) * ncol + r] = n[u];
+}
+}  // namespace
+
+size_t track_exchange_workspace_bytes(const Ctx& c) {
+  return align_up(sizeof(float) * 6 * (size_t)(c.ncy * c.ncz), 256) + align_up(sizeof(float) * 6 * (size_t)c.d.nz * (size_t)c.nyp, 256);
+}
+
+asd_status track_exchange_refresh(Ctx& c) {
+  if (!c.tex_on || c.mm) return ASD_OK;                   // the meshes of a multiscale window take over the ends
+  const int mx = c.d.macro[0], ncol = (int)(c.ncy * c.ncz);
+  const long long cxg0 = c.x0 > 0 ? (c.x0 - 1) / mx : -1, cxg1 = (c.x0 + c.d.nx < c.d.track_nx) ? (c.x0 + c.d.nx) / mx : -1;
+  track_ghost_kernel<<<nblocks(2 * ncol, 128), 128, 0, c.stream>>>((int)c.ncy, (int)c.ncz, (long long)c.ncx, cxg0, cxg1,
+                                                                  c.out_sum, c.out_cnt, c.init_mean, c.tex_ghost);
+  ASD_LAUNCH_CHECK(c, "track_ghost");
+  MmGeom g = {};
+  g.ncy = (int32_t)c.ncy; g.ncz = (int32_t)c.ncz; g.ncol = ncol;
+  g.nx = c.d.nx; g.ny = c.d.ny; g.nz = c.d.nz; g.nyp = c.nyp; g.lead = c.lead;
+  g.mx = mx; g.my = c.d.macro[1]; g.mz = c.d.macro[2];
+  const float j1 = (float)(c.d.J[0] / c.d.mu_s), j3 = (float)(c.d.J[2] / c.d.mu_s);
+  const int n = 2 * c.d.nz * c.nyp;
+  if (c.d.lattice == ASD_SC) mm_edge_kernel<0><<<nblocks(n, 128), 128, 0, c.stream>>>(g, c.col_win(), c.tex_ghost, j1, j3, c.tex_edgeB);
+  else mm_edge_kernel<1><<<nblocks(n, 128), 128, 0, c.stream>>>(g, c.col_win(), c.tex_ghost, j1, j3, c.tex_edgeB);
+  ASD_LAUNCH_CHECK(c, "track_edge");
+  return ASD_OK;
+}
+
+asd_status track_exchange_enable(Ctx& c, int on, void* ws, size_t bytes) {
+  if (!on) { c.tex_on = false; return ASD_OK; }
+  if (bytes < track_exchange_workspace_bytes(c)) { std::snprintf(c.err, sizeof(c.err), "asd_enable_track_exchange: workspace too small"); return ASD_ENOMEM; }
+  c.tex_ghost = (float*)ws;
+  c.tex_edgeB = (float*)((char*)ws + align_up(sizeof(float) * 6 * (size_t)(c.ncy * c.ncz), 256));
+  c.tex_on = true;
+  return track_exchange_refresh(c);
+}
 
 // Called before every Heun step (reading M9): every `every`-th step the meshes and the atoms trade boundary data (from
 // the configurations at that instant) and the meshes advance by one RK4 step of every * dt.
