@@ -220,13 +220,13 @@ __global__ void coarse_grain_ydft(const float* __restrict__ X, uint32_t as, int 
       for (int v = 0; v < VEC; ++v) col[((size_t)rl * 3 + comp) * ny + g * VEC + v] = s[comp][v];
   }
   __syncthreads();
-  for (int b = threadIdx.x; b < dcy; b += blockDim.x) {
-    float t[3] = {0.0f, 0.0f, 0.0f};
+  for (int t = threadIdx.x; t < 3 * dcy; t += blockDim.x) {      // one thread per (component, macrocell): fixed order
+    const int comp = t / dcy, b = t - comp * dcy;
+    float acc = 0.0f;
     const int j1 = min((b + 1) * my, ny);
     for (int j = b * my; j < j1; ++j)
-      for (int l = 0; l < lanes; ++l)
-        for (int comp = 0; comp < 3; ++comp) t[comp] += col[((size_t)l * 3 + comp) * ny + j];
-    cells[b] = t[0] * mu_over_V; cells[dcy + b] = t[1] * mu_over_V; cells[2 * dcy + b] = t[2] * mu_over_V;
+      for (int l = 0; l < lanes; ++l) acc += col[((size_t)l * 3 + comp) * ny + j];
+    cells[t] = acc * mu_over_V;
   }
   __syncthreads();
   row_ydft(cells, tws, dcy, dcz, dcx, PY, NKY, a, c, Y);
