@@ -233,7 +233,9 @@ ASD_API asd_status asd_track_get(asd_ctx *ctx, double *sum, int64_t *count);
  * asd_track_end_pass    the nx planes still inside the window are transferred to the track by Eq. (6) exactly
  *                       as outgoing planes are; then every macrocell the pass has written (count > 0) becomes what lies
  *                       ahead of the next pass: init mean spin = sum / count (cells never written keep theirs).  The
- *                       written store stays readable (asd_track_get, asd_track_read_scan).  Asynchronous.
+ *                       written store stays readable (asd_track_get, asd_track_read_scan).  Asynchronous.  The window's
+ *                       spins now belong to the track as well: start the next pass (or load new spins) before stepping
+ *                       on with the demagnetising / stray field, which would otherwise count them twice.
  * asd_track_begin_pass  the written store is cleared, pass counter += 1, the window returns to global plane x0_new
  *                       (0 <= x0_new <= track_nx - nx) and ALL its planes are generated from the track by the cone
  *                       sampling of P:68 (D:S3) with Philox counter n := pass; step and shift counters run on.  T and B
