@@ -3,7 +3,8 @@
 //
 // A 4096-site lattice finishes a stage kernel in ~2 us, less than it costs to launch it ("cfg 0 is
 // launch/latency-bound ... one persistent CTA"); graphs and dependent launches bring a Heun step to 8 us.  Here the
-// window is cut along x into as many slabs as the cluster has CTAs (8: the portable maximum); every CTA keeps its slab of
+// window is cut along x into as many slabs as the cluster has CTAs (16 where the device schedules it, else 8, the
+// portable maximum); every CTA keeps its slab of
 // S and S~ in its own shared memory, one thread owning VEC (1, 2 or 4) consecutive y-sites with A = S + dt/2 k1, the
 // noise xi and the site's constants in registers (VEC is chosen so that a CTA has as many warps as fit: a slab of a few
 // hundred sites is latency-bound, and warps are what hides latency).  The x+-1 planes of a slab's first / last plane live in
@@ -14,6 +15,7 @@
 // xi in both stages.  Periodic wraps and open edges by index arithmetic; vacant sites hold 0, so a vacant neighbour drops
 // out of Eq. (2) by itself -- which needs grains that do not touch (or one grain), checked by the dispatcher.
 #include <cooperative_groups.h>
+#include <cstdlib>
 
 #include "asd_internal.cuh"
 #include "asd_site.cuh"
@@ -241,7 +243,10 @@ bool persist_shape(const Ctx& c, PersistShape& sh) {
   if (c.d.ny % 4 != 0) return false;
   int smem_cta = 0;
   cudaDeviceGetAttribute(&smem_cta, cudaDevAttrMaxSharedMemoryPerBlockOptin, c.device);
-  for (int ncta = 8; ncta >= 1; ncta >>= 1) {
+  // 16 CTAs per cluster is beyond the portable size: taken when the device can schedule it (asked once per shape below)
+  int max_ncta = 16;                                      // measured on cfg0: 16 CTAs 1.32 us per Heun step, 8: 1.46, 4: 2.27
+  if (const char* ev = std::getenv("ASD_PERSIST_CLUSTER")) max_ncta = std::atoi(ev);       // tuning override: 1, 2, 4, 8, 16
+  for (int ncta = max_ncta; ncta >= 1; ncta >>= 1) {
     if (c.d.nx % ncta != 0) continue;
     const int ppc = c.d.nx / ncta;
     const int64_t sites = (int64_t)ppc * c.d.nz * c.d.ny;
@@ -250,6 +255,21 @@ bool persist_shape(const Ctx& c, PersistShape& sh) {
     const int vec = sites <= 512 ? 1 : (sites / 2 <= 512 ? 2 : 4);
     sh.ncta = ncta; sh.ppc = ppc; sh.vec = vec; sh.threads = (int)((sites / vec + 31) / 32 * 32); sh.smem = smem;
     sh.kern = c.d.lattice == ASD_SC ? persist_kernel<LAT_SC>(vec, sh.threads) : persist_kernel<LAT_L10>(vec, sh.threads);
+    if (ncta > 8) {                                       // non-portable cluster size: opt in, and ask whether it can run
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3((unsigned)ncta); cfg.blockDim = dim3((unsigned)sh.threads); cfg.dynamicSmemBytes = smem;
+      cudaLaunchAttribute attr[1];
+      attr[0].id = cudaLaunchAttributeClusterDimension;
+      attr[0].val.clusterDim.x = (unsigned)ncta; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+      cfg.attrs = attr; cfg.numAttrs = 1;
+      int nclusters = 0;
+      if (cudaFuncSetAttribute((const void*)sh.kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess ||
+          cudaFuncSetAttribute((const void*)sh.kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
+          cudaOccupancyMaxActiveClusters(&nclusters, (const void*)sh.kern, &cfg) != cudaSuccess || nclusters < 1) {
+        cudaGetLastError();
+        continue;
+      }
+    }
     return true;
   }
   return false;
