@@ -437,6 +437,9 @@ def secondary(asd, torch, device, args, peak, peak_src):
                 w4 = w4 or _workload(4)
                 import copy
                 w = copy.copy(w4)
+            elif cfg == "two_track":
+                # the 80 nm wide two-track window: SC 400 x 268 x 27, spot on the bottom track
+                w = ai.two_track_film(ai.SC, n_bits=4).w
             elif cfg == "multiscale":
                 # [48-cell mesh | 336 x 200 x 27 SC atoms | 48-cell mesh]: the paper's three equal parts on cfg3's film
                 kw["multiscale"] = ai.multiscale_film(ai.SC, every=kw.pop("every", 20))
@@ -480,6 +483,7 @@ def secondary(asd, torch, device, args, peak, peak_src):
     one("multiscale window: 48-cell LLG mesh | SC 336x200x27 atoms | 48-cell mesh, mesh RK4 step every 20 Heun steps",
         "multiscale", every=20)
     one("multiscale window, meshes in lock-step (every Heun step)", "multiscale", every=1)
+    one("two-track window SC 400x268x27 (pass 0 of the two-track write; profiles/r2_two_track.md has both passes)", "two_track")
     return out
 
 
