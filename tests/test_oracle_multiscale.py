@@ -465,3 +465,48 @@ def test_passes_over_the_track_with_a_multiscale_window():
     assert np.allclose(np.linalg.norm(R, axis=0)[np.broadcast_to((gm[x1:x1 + w.nx] >= 0)[:, None, :], R.shape[1:])], 1.0, atol=1e-14)
     # the dynamics go on
     o.step_heun(2)
+
+
+# ---------------------------------------------------------------------------------------------- M9 (who steps when)
+def test_m9_mesh_takes_one_step_of_every_dt_per_every_heun_steps():
+    """Cadence and step length from a closed form: a decoupled, uniformly magnetised mesh in a field is a macrospin
+    (P14); after n Heun steps with `every` = P it has precessed by gamma B / (1 + alpha^2) x ceil(n / P) P dt."""
+    lam, T, Tc, B, dt = 0.1, 300.0, 700.0, 5.0, 1e-15
+    for every, n in ((1, 7), (4, 9), (5, 10), (20, 1)):
+        o = _window(decouple=True, lam=lam, Tc=Tc, every=every, dt=dt)
+        th0 = 0.5
+        for side in (0, 1):
+            _uniform(o, side, [math.sin(th0), 0.0, math.cos(th0)])
+            sh = o.mm_shape(side)
+            o.mm_set_fields(side, np.full(sh, T), np.zeros(sh), np.zeros(sh), np.full(sh, B))
+        o.step_heun(n)
+        alpha = lam * (1.0 - T / (3.0 * Tc))
+        t = -(-n // every) * every * dt
+        m = o.mm_get_m(0)[1, 0, 0]
+        assert abs(math.atan2(m[1], m[0]) - G * B * t / (1.0 + alpha ** 2)) < 1e-9, (every, n)
+        th = 2.0 * math.atan(math.tan(th0 / 2.0) * math.exp(-alpha * G * B * t / (1.0 + alpha ** 2)))
+        assert abs(math.acos(m[2]) - th) < 1e-9
+
+
+def test_m9_atoms_see_the_mesh_directions_of_the_exchange_instant():
+    """The boundary data go both ways from the configurations at the exchange instant, BEFORE the meshes step: during the
+    following Heun steps the atoms see m(t_n), not m(t_n + every dt).  A window whose meshes rotate a lot in one step
+    (30 T on the cells only) and a twin whose meshes cannot move (no field there) leave the atoms identical."""
+    def make(mesh_field):
+        o = _window(lattice=ai.SC, mcx=(2, 2), atom_cells=2, ny=4, nz=2, macro=(2, 2, 2), every=3, K0=0.0, A0=0.0)
+        for side in (0, 1):
+            _uniform(o, side, [0.5, 0.2, 0.84])
+            sh = o.mm_shape(side)
+            o.mm_set_fields(side, np.zeros(sh), np.zeros(sh), np.full(sh, mesh_field), np.zeros(sh))
+        rng = np.random.default_rng(2)
+        v = rng.standard_normal((o.N, 3)); v /= np.linalg.norm(v, axis=1, keepdims=True)
+        o.set_spins(v[:, 0], v[:, 1], v[:, 2])
+        return o
+    a, b = make(30.0), make(0.0)
+    m0 = b.mm_get_m(0).copy()
+    a.step_heun(3); b.step_heun(3)                                             # one exchange, one mesh step, three Heun steps
+XX
+    assert np.array_equal(b.mm_get_m(0), m0)
+    assert np.array_equal(a.get_spins(), b.get_spins())                        # ... and its atoms never saw it
+    a.step_heun(1); b.step_heun(1)                                             # next exchange: now they do
+    assert np.abs(a.get_spins() - b.get_spins()).max() > 1e-6
