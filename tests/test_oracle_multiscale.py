@@ -505,7 +505,7 @@ def test_m9_atoms_see_the_mesh_directions_of_the_exchange_instant():
     a, b = make(30.0), make(0.0)
     m0 = b.mm_get_m(0).copy()
     a.step_heun(3); b.step_heun(3)                                             # one exchange, one mesh step, three Heun steps
-XX
+    assert np.abs(a.mm_get_m(0) - m0).max() > 5e-3                             # a's meshes did turn ...
     assert np.array_equal(b.mm_get_m(0), m0)
     assert np.array_equal(a.get_spins(), b.get_spins())                        # ... and its atoms never saw it
     a.step_heun(1); b.step_heun(1)                                             # next exchange: now they do
