@@ -690,12 +690,13 @@ struct FusedPlan {
 
 bool heun_fused_supported(const Ctx& c) { return heun_fast_supported(c) && c.d.nz + 2 <= 256; }
 
-// ASD_KERNEL_AUTO takes the fused step for windows that stream from HBM (more than 2^21 sites) and give every CTA a march
-// of at least 8 planes (a chunk recomputes the predictor of 2 extra planes).  Smaller films are L2-resident or launch-
-// bound; there the two stage kernels (or their graph replay) stay in charge.  Measured (B200, G updates/s, two-kernel ->
-// fused): cfg4 46.0 -> 55.3, cfg3 42.9 -> 46.6, cfg2 46.6 -> 32.3, cfg1 48.9 -> 41.3.
+// ASD_KERNEL_AUTO takes the fused step for windows of more than 1.5 M sites that give every CTA a march of at least 8
+// planes (a chunk recomputes the predictor of 2 extra planes).  Smaller films are L2-resident or launch-bound; there the
+// two stage kernels (or their graph replay) stay in charge.  Measured (B200, G updates/s, two-kernel -> fused): cfg4
+// 46.0 -> 55.3, cfg3 42.9 -> 46.6, the 336 x 200 x 27 multiscale window (1.81 M sites, 8-plane marches) 39.0 -> 43.8;
+// cfg2 46.6 -> 32.3 and cfg1 48.9 -> 41.3 (1 M sites, marches of 5-6 planes).
 bool heun_fused_preferred(Ctx& c) {
-  if (c.N <= (1ll << 21)) return false;
+  if (c.N <= 1500000) return false;
   const FusedPlan* pl = fused_plan(c);
   return pl && pl->CX >= 8;
 }

@@ -156,7 +156,7 @@ def test_passes_over_the_track_with_the_meshes(lattice):
 
 def test_full_size_multiscale_window_one_coupled_step():
     """The bench's multiscale workload at full size ([48-cell mesh | SC 336 x 200 x 27 atoms | 48-cell mesh], 1.81 M sites,
-    11 136 cells; the stage kernels' edge-field instances, as ASD_KERNEL_AUTO runs them): every site and every cell
+    11 136 cells; the fused step's edge-field instance, as ASD_KERNEL_AUTO runs it): every site and every cell
     against the oracle after one coupled step, then after a whole-cell shift and one more step."""
     ms = ai.multiscale_film(ai.SC, every=1)
     o, g = oracle_from_workload(ms.w), gpu_from_workload(ms.w)
