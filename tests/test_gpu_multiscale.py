@@ -174,3 +174,19 @@ def test_full_size_multiscale_window_one_coupled_step():
     o.step_heun(1); g.step_heun(1)
     assert np.abs(o.get_spins() - g.get_spins_host()).max() <= 3e-5
     assert _mesh_diff(o, g) <= 2e-5
+
+
+@pytest.mark.parametrize("lattice", [ai.SC, ai.L10])
+def test_multiscale_window_with_the_demagnetising_field(lattice):
+    """Meshes and the window's demagnetising field together (the general kernel carries both): coupled steps against the
+    oracle, per-stage and held-field schemes."""
+    for every_dm in (0, 2):
+        ms, o, g = _pair(lattice, every=2)
+        sp = [a * 1e-9 for a in ms.w.spacing_nm]
+        o.enable_demag(sp); g.enable_demag(sp)
+        o.set_demag_every(every_dm); g.set_demag_every(every_dm)
+        o.step_heun(1); g.step_heun(1)
+        assert np.abs(o.get_spins() - g.get_spins_host()).max() <= 1e-5
+        o.step_heun(3); g.step_heun(3)
+        assert np.abs(o.get_spins() - g.get_spins_host()).max() <= 4e-5
+        assert _mesh_diff(o, g) <= 2e-5
