@@ -205,8 +205,11 @@ def multiscale_write(lattice: int = wl.SC, atom_cells: int = 57, mesh_cells: Tup
     ms = multiscale_film(lattice, atom_cells=atom_cells, mesh_cells=mesh_cells, width_nm=width_nm, nz=nz,
                          extra_cells=total_bits_cells, every=every, macro=macro, fwhm_nm=fwhm_nm, **kw)
     sp = ms.w.spacing_nm
-    # diameter of the spot above 710 K for T = 300 + 500 exp(-4 ln2 r^2 / FWHM^2): 0.535 FWHM (two_track.py)
-    r_hot_nm = 0.5 * 0.535 * fwhm_nm
+    # the grains freeze where the trailing flank of the spot crosses T_C: T = T_amb + dT exp(-4 ln2 r^2 / FWHM^2) = T_C,
+    # with the recipe's mean T_C (Eq. (8): 700 K for the SC exchange, 512 K for the L1_0 shells) and its 300 / 800 K spot
+    t_amb, t_peak = float(kw.get("t_ambient", 300.0)), float(kw.get("t_peak", 800.0))
+    t_c = min(float(np.mean(ms.Tc)), t_peak - 1.0)
+    r_hot_nm = fwhm_nm * math.sqrt(math.log((t_peak - t_amb) / (t_c - t_amb)) / (4.0 * math.log(2.0)))
     return MultiscaleWrite(ms=ms, bits=wl.nrz_bits(n_bits, bit_seed), bit_cells=bit_cells,
                            steps_per_cell=int(round(steps_per_nm * macro[0] * sp[0])), batch=batch,
                            spot_plane=ms.w.x0 + 0.5 * ms.w.nx, write_offset=r_hot_nm / sp[0],
