@@ -8,8 +8,9 @@ Geometry: the film is `width_nm` wide; the two track centres
 (width + pitch)/2 with pitch = bit width + separation = 25 + 15 = 40 nm ("the bits are approximately 25 nm wide
 as before, with the separation between tracks being 15 nm, for a total simulation window with 80 nm width").  Pass p
 centres the laser spot on track p ("achieved by positioning the laser spot in the centre of the bottom track").
-The spot FWHM is chosen so that its diameter above T_C = 710 K is the 25 nm of P:86:
-T = 300 + 500 exp(-4 ln2 r^2 / FWHM^2) > 710 K  <=>  r < 0.2675 FWHM  =>  FWHM = 46.7 nm.
+The spot FWHM is chosen so that its diameter above T_C is the 25 nm of P:86; for the paper's 710 K (simple cubic):
+T = 300 + 500 exp(-4 ln2 r^2 / FWHM^2) > 710 K  <=>  r < 0.2675 FWHM  =>  FWHM = 46.7 nm; for the L1_0 shells of
+BASELINE.json (mean-field T_C = 512 K) the same rule gives 22.5 nm.
 """
 from __future__ import annotations
 
@@ -69,7 +70,8 @@ def two_track_film(lattice: int = wl.SC, length_nm: float = 120.0, width_nm: flo
                    pitch_nm: float = 8.0, boundary_nm: float = 1.0, fwhm_nm: Optional[float] = None,
                    t_peak: float = 800.0, bz: float = 0.8, lam: float = 0.1, dt: float = 1e-15,
                    shift_every: int = 5000, batch: int = 100, macro: Optional[Sequence[int]] = None,
-                   grain_seed: int = 2, seed: int = 1, bit_seeds: Tuple[int, int] = (3, 4)) -> TwoTrack:
+                   grain_seed: int = 2, seed: int = 1, bit_seeds: Tuple[int, int] = (3, 4),
+                   t_c: Optional[float] = None) -> TwoTrack:
     """The two-track window at any size: defaults are the paper's geometry on the cfg3 / cfg4 lattices; the parity tests
     shrink every length."""
     spacing = wl.A_SC if lattice == wl.SC else wl.A_L10
@@ -80,8 +82,13 @@ def two_track_film(lattice: int = wl.SC, length_nm: float = 120.0, width_nm: flo
     ny = int(round(width_nm / spacing[1] / 4.0)) * 4
     bit_planes = int(round(bit_nm / spacing[0]))
     track_nx = nx + n_bits * bit_planes
+    if t_c is None:
+        # the temperature the bits are written at: the paper's 710 K for its simple-cubic exchange; for the L1_0 shells
+        # of BASELINE.json the mean-field estimate of Eq. (8), eps (4 J1 + 2 J2 + 4 J3) / 3 k_B = 512 K
+        t_c = 710.0 if lattice == wl.SC else 0.78 * (4 * J[0] + 2 * J[1] + 4 * J[2]) / (3.0 * wl.K_B)
     if fwhm_nm is None:
-        fwhm_nm = bit_width_nm / (2.0 * math.sqrt(math.log(500.0 / 410.0) / (4.0 * math.log(2.0))))
+        # spot width such that its diameter above t_c is the bit width: T = 300 + (t_peak - 300) exp(-4 ln2 r^2 / FWHM^2)
+        fwhm_nm = bit_width_nm / (2.0 * math.sqrt(math.log((t_peak - 300.0) / (t_c - 300.0)) / (4.0 * math.log(2.0))))
     gm, ku, axis = wl.voronoi_grain_map(track_nx, ny, spacing[0], spacing[1], pitch_nm=pitch_nm,
                                         boundary_nm=boundary_nm, seed=grain_seed)
     N = nx * ny * nz
