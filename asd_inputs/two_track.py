@@ -88,7 +88,10 @@ def two_track_film(lattice: int = wl.SC, length_nm: float = 120.0, width_nm: flo
         t_c = 710.0 if lattice == wl.SC else 0.78 * (4 * J[0] + 2 * J[1] + 4 * J[2]) / (3.0 * wl.K_B)
     if fwhm_nm is None:
         # spot width such that its diameter above t_c is the bit width: T = 300 + (t_peak - 300) exp(-4 ln2 r^2 / FWHM^2)
-        fwhm_nm = bit_width_nm / (2.0 * math.sqrt(math.log((t_peak - 300.0) / (t_c - 300.0)) / (4.0 * math.log(2.0))))
+        frac = (t_c - 300.0) / (t_peak - 300.0)
+        if not 0.0 < frac < 1.0:                 # a spot that never reaches t_c (the cool parity tests): the paper's proportions
+            frac = 410.0 / 500.0
+        fwhm_nm = bit_width_nm / (2.0 * math.sqrt(math.log(1.0 / frac) / (4.0 * math.log(2.0))))
     gm, ku, axis = wl.voronoi_grain_map(track_nx, ny, spacing[0], spacing[1], pitch_nm=pitch_nm,
                                         boundary_nm=boundary_nm, seed=grain_seed)
     N = nx * ny * nz
