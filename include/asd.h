@@ -69,7 +69,7 @@ enum { ASD_SC = 0, ASD_L10_FE = 1 };
  * kernel per stage; PERSISTENT: all n steps of an asd_step_heun(n) call in one launch of one thread-block cluster that
  * keeps the lattice in (distributed) shared memory -- 16 CTAs where the device schedules that cluster size, else 8; x-slabs
  * of at most 1024 four-site groups that fit a CTA's shared memory, built-in shells, grains that do not touch; what AUTO
- * runs on lattices of <= 2^14 sites. */
+ * runs where it measured faster than graph replay (slabs of up to 1024-3072 sites per CTA, by lattice). */
 enum { ASD_KERNEL_AUTO = 0, ASD_KERNEL_GENERAL = 1, ASD_KERNEL_FAST = 2, ASD_KERNEL_TMA = 3, ASD_KERNEL_FUSED = 4,
        ASD_KERNEL_PERSISTENT = 5 };
 

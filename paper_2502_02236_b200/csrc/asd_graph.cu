@@ -93,7 +93,7 @@ asd_status launch_heun(Ctx& c, int64_t n) {
   const bool use = !c.demag && !edge_field_on(c) &&         // the demag pipeline and the mesh steps are launched plainly
                    c.kernel_variant != ASD_KERNEL_FUSED &&   // the fused step swaps the spin buffers every step
                    c.kernel_variant != ASD_KERNEL_PERSISTENT &&
-                   !(c.kernel_variant == ASD_KERNEL_AUTO && c.N <= (1 << 14) && heun_persist_supported(c)) &&   // one launch already
+                   !(c.kernel_variant == ASD_KERNEL_AUTO && heun_persist_preferred(c)) &&   // one launch already
                    (c.graph_mode == ASD_GRAPH_ON || (c.graph_mode == ASD_GRAPH_AUTO && c.N <= kAutoMaxSites));
   while (use && n >= 2) {
     const int64_t k = n < kBatch ? n : kBatch;

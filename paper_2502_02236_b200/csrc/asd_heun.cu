@@ -291,8 +291,6 @@ void fill_stage_params(const Ctx& c, StageParams& p) {
 // n Heun steps as 2n plain launches on c.launch_stream.  dyn == nullptr: step indices come from c.step, which advances.
 // dyn != nullptr (graph capture): step s of the batch carries the offset s and reads the base from *dyn; c.step is
 // left to the caller.
-constexpr int64_t kPersistAutoMaxSites = 1 << 14;   // ASD_KERNEL_AUTO: lattices this small run as one persistent cluster
-
 asd_status launch_heun_direct(Ctx& c, int64_t n, const DynState* dyn) {
   StageParams p;
   fill_stage_params(c, p);
@@ -317,7 +315,7 @@ asd_status launch_heun_direct(Ctx& c, int64_t n, const DynState* dyn) {
   if (c.kernel_variant == ASD_KERNEL_FUSED && !fused) return ASD_EUNSUPPORTED;
   // a lattice that fits one thread-block cluster's shared memory: all n steps in one launch (asd_heun_persist.cu)
   const bool persist = !dyn && heun_persist_supported(c) &&
-                       (c.kernel_variant == ASD_KERNEL_PERSISTENT || (c.kernel_variant == ASD_KERNEL_AUTO && c.N <= kPersistAutoMaxSites));
+                       (c.kernel_variant == ASD_KERNEL_PERSISTENT || (c.kernel_variant == ASD_KERNEL_AUTO && heun_persist_preferred(c)));
   if (c.kernel_variant == ASD_KERNEL_PERSISTENT && !persist) return ASD_EUNSUPPORTED;
   if (persist) return n > 0 ? launch_heun_persist(c, p, n) : ASD_OK;
   for (int64_t s = 0; s < n; ++s) {

@@ -234,7 +234,7 @@ template <int LAT>
 PersistKernel persist_kernel(int vec, int threads) {
   if (vec == 1) return heun_persistent<LAT, 1, 512>;
   if (vec == 2) return heun_persistent<LAT, 2, 512>;
-  return threads <= 256 ? heun_persistent<LAT, 4, 256> : heun_persistent<LAT, 4, 1024>;
+  return threads <= 256 ? heun_persistent<LAT, 4, 256> : (threads <= 512 ? heun_persistent<LAT, 4, 512> : heun_persistent<LAT, 4, 1024>);
 }
 
 // Largest cluster (8, 4, 2, 1 CTAs) whose slabs are whole planes and fit a CTA's shared memory; then as few sites per
@@ -283,6 +283,19 @@ bool heun_persist_supported(const Ctx& c) {
   PersistShape sh;
   return c.d.ell_width == 0 && !c.grains_touch && !c.demag && !edge_field_on(c) && (int64_t)AR_COUNT * c.as < (1ll << 31) &&
          persist_shape(c, sh);
+}
+
+// What ASD_KERNEL_AUTO asks: is the persistent cluster the fastest path for this lattice?  Measured on B200, us per Heun step,
+// persistent against CUDA-graph replay of the stage kernels (film kernel 4.9-5.6, general kernel 8.0-9.4 whatever the size
+// below 2^16 sites): simple cubic 1024 / 1536 / 2048 / 3072 sites per CTA: 2.3 / 3.5 / 3.7 / 8.1; L1_0 1024 / 1536 / 2048 /
+// 3072: 3.3 / 6.2 / 5.8 / 11.9 (from 1024 sites per CTA on a thread owns 4 sites; from 2048 the 64-register instance spills).
+bool heun_persist_preferred(const Ctx& c) {
+  PersistShape sh;
+  if (!heun_persist_supported(c) || !persist_shape(c, sh)) return false;
+  const int64_t per_cta = (int64_t)sh.ppc * c.d.nz * c.d.ny;
+  const bool film_kernel = heun_fast_supported(c);          // else the replayed kernel is the general one, twice as slow
+  const int64_t limit = c.d.lattice == ASD_SC ? (film_kernel ? 2048 : 3072) : (film_kernel ? 1024 : 2048);
+  return per_cta <= limit;
 }
 
 // n Heun steps in one launch; advances c.step.

@@ -257,6 +257,7 @@ bool heun_fused_takes_mm(Ctx& c);                             // the plan's CTA 
 bool heun_fused_takes_demag(Ctx& c);                          // ... a held-demagnetising-field instance
 asd_status launch_heun_persist(Ctx& c, StageParams& p, int64_t n);   // n Heun steps in one cluster launch (asd_heun_persist.cu)
 bool heun_persist_supported(const Ctx& c);
+bool heun_persist_preferred(const Ctx& c);                    // what ASD_KERNEL_AUTO asks (measured crossover vs graph replay)
 void fused_plan_free(Ctx& c);
 void fill_stage_params(const Ctx& c, StageParams& p);
 // multiscale window (asd_mm.cu)

@@ -49,10 +49,11 @@ def test_one_launch_of_n_steps_is_bit_identical_to_n_launches():
 
 @pytest.mark.parametrize("lattice", [ai.SC, ai.L10])
 @pytest.mark.parametrize("dims,pbc", [((16, 8, 4), (0, 0, 0)), ((8, 16, 6), (0, 0, 0)), ((24, 12, 5), (0, 0, 0)),
-                                      ((6, 8, 5), (0, 0, 0)), ((5, 4, 3), (0, 0, 0)), ((32, 32, 8), (0, 0, 0))])
+                                      ((6, 8, 5), (0, 0, 0)), ((5, 4, 3), (0, 0, 0)), ((32, 32, 8), (0, 0, 0)),
+                                      ((32, 64, 12), (0, 0, 0)), ((64, 64, 12), (0, 0, 0))])
 def test_open_films_with_grains(lattice, dims, pbc):
     """Granular films (vacant boundaries, several grains, Gaussian spot, head field): clusters of 8, 4, 2 and 1 CTAs,
-    one to several planes per CTA, a 1024-thread slab."""
+    one to several planes per CTA, 256-, 512- and 1024-thread slabs, one and four sites per thread."""
     nx, ny, nz = dims
     w = ai.small_film(lattice, nx, ny, nz, tilt_deg=25.0, dt=1e-16)
     o, g = oracle_from_workload(w), gpu_from_workload(w)
@@ -96,6 +97,21 @@ def test_periodic_wraps(lattice, pbc):
         assert np.abs(o.get_spins() - g.get_spins_host()).max() <= 1e-5
         o.step_heun(3); g.step_heun(3)
         assert np.abs(o.get_spins() - g.get_spins_host()).max() <= 4e-5
+
+
+def test_auto_takes_the_cluster_where_it_measured_faster():
+    """ASD_KERNEL_AUTO (heun_persist_preferred): simple-cubic film slabs up to 2048 sites per CTA, L1_0 up to 1024; beyond
+    that the replayed stage kernels.  Same arithmetic per path, so the comparison is bit for bit."""
+    for lattice, dims, expect in ((ai.SC, (32, 64, 12), "persistent"), (ai.SC, (64, 64, 12), "fast"),
+                                  (ai.L10, (64, 32, 8), "persistent"), (ai.L10, (32, 64, 12), "fast")):
+        w = ai.small_film(lattice, *dims, tilt_deg=25.0, dt=1e-16)
+        a, b = gpu_from_workload(w), gpu_from_workload(w)
+        b.set_kernel(asd.KERNEL_PERSISTENT if expect == "persistent" else asd.KERNEL_FAST)
+        n0 = a.launch_count()
+        a.step_heun(6); b.step_heun(6)
+        n1 = a.launch_count()                                   # before the read-back launches its unpack kernel
+        assert np.array_equal(a.get_spins_host(), b.get_spins_host())
+        assert (n1 - n0 == 1) == (expect == "persistent")
 
 
 def test_refused_where_it_does_not_apply():
