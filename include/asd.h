@@ -178,6 +178,11 @@ ASD_API asd_status asd_demag_field(asd_ctx *ctx, float *cells, int64_t dims[3]);
  * field).  every = P >= 1: it is recomputed from S at the predictor of every P-th Heun step (counted from the last
  * enable / this call / window shift / asd_set_spins) and held for both stages in between (reading D3). */
 ASD_API asd_status asd_set_demag_every(asd_ctx *ctx, int32_t every);
+/* The cell field as the last Heun stage used it (nothing is recomputed): in the held-field scheme, the field of the
+ * spins at the last refresh.  Same HOST layout, dims and errors as asd_demag_field; synchronises.  With the one-kernel
+ * step (ASD_KERNEL_FUSED / AUTO) the macrocell sums of Eq. (6) behind a refresh are accumulated by the corrector of the
+ * step before it (64-bit fixed point, order-independent), not by a pass of their own over the spins. */
+ASD_API asd_status asd_demag_held_field(asd_ctx *ctx, float *cells, int64_t dims[3]);
 
 /* Window ends exchange coupled to the frozen track ("the ends of the simulation window are exchange coupled to the
  * track"; reading E1), for a purely atomistic window (the meshes of asd_mm_enable take the ends over).  The

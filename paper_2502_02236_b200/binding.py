@@ -21,7 +21,7 @@ EXPORTED_SYMBOLS = [
     "asd_workspace_bytes", "asd_create_lattice", "asd_destroy", "asd_set_spins", "asd_get_spins",
     "asd_set_spins_host", "asd_get_spins_host", "asd_set_fields", "asd_set_fields_host", "asd_set_field_scale",
     "asd_step_heun", "asd_set_kernel", "asd_set_graph_mode", "asd_demag_workspace_bytes", "asd_enable_demag",
-    "asd_demag_field", "asd_set_demag_every", "asd_staging_bytes", "asd_set_staging", "asd_stage_fields_host",
+    "asd_demag_field", "asd_demag_held_field", "asd_set_demag_every", "asd_staging_bytes", "asd_set_staging", "asd_stage_fields_host",
     "asd_commit_fields", "asd_shift_window", "asd_magnetisation", "asd_grain_magnetisation",
     "asd_track_dims", "asd_track_set_init", "asd_track_get",
     "asd_track_end_pass", "asd_track_begin_pass", "asd_track_read_scan",
@@ -113,6 +113,7 @@ def load_library(build_if_missing: bool = True):
     L.asd_demag_workspace_bytes.argtypes = [C.c_void_p]
     L.asd_enable_demag.argtypes = [C.c_void_p, dp, C.c_void_p, C.c_size_t]
     L.asd_demag_field.argtypes = [C.c_void_p, fp, C.POINTER(C.c_int64)]
+    L.asd_demag_held_field.argtypes = [C.c_void_p, fp, C.POINTER(C.c_int64)]
     L.asd_set_demag_every.argtypes = [C.c_void_p, C.c_int32]
     L.asd_track_stray_workspace_bytes.restype = C.c_size_t
     L.asd_track_stray_workspace_bytes.argtypes = [C.c_void_p, C.c_int32]
@@ -387,6 +388,14 @@ class Context:
         self._ck(self._L.asd_demag_field(self._h, None, dims))
         out = np.zeros((dims[0], dims[1], dims[2], 3), dtype=np.float32)
         self._ck(self._L.asd_demag_field(self._h, out.ctypes.data_as(C.POINTER(C.c_float)), dims))
+        return out
+
+    def demag_held_field(self) -> np.ndarray:
+        """asd_demag_held_field: the cell field as the last Heun stage used it (nothing recomputed), [dcx, dcy, dcz, 3]."""
+        dims = (C.c_int64 * 3)()
+        self._ck(self._L.asd_demag_held_field(self._h, None, dims))
+        out = np.zeros((dims[0], dims[1], dims[2], 3), dtype=np.float32)
+        self._ck(self._L.asd_demag_held_field(self._h, out.ctypes.data_as(C.POINTER(C.c_float)), dims))
         return out
 
     def set_graph_mode(self, mode: int):

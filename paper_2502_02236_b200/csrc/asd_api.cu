@@ -239,7 +239,7 @@ asd_status asd_destroy(asd_ctx* ctx) {
 // corrector, and nothing reads A's padding), then packed into the padded-row layout by a kernel.
 static asd_status set_spins_impl(Ctx& c, const float* sx, const float* sy, const float* sz, bool host) {
   if (!sx || !sy || !sz) return fail(c, ASD_EINVAL, "asd_set_spins: NULL pointer");
-  c.demag_age = 0;                             // a held demagnetising field belongs to the old spins
+  demag_held_invalidate(c);                             // a held demagnetising field belongs to the old spins
   mm_restart_cadence(c);                       // ... and so do the held mesh boundary data
   if (host) {
     const float* src[3] = {sx, sy, sz};
@@ -440,6 +440,13 @@ asd_status asd_demag_field(asd_ctx* ctx, float* cells, int64_t dims[3]) {
   return demag_field_host(c, cells, dims);
 }
 
+asd_status asd_demag_held_field(asd_ctx* ctx, float* cells, int64_t dims[3]) {
+  CTX_OR_RETURN(ctx);
+  if (!dims) return fail(c, ASD_EINVAL, "asd_demag_held_field: dims is NULL");
+  if (!c.demag) return fail(c, ASD_ESTATE, "asd_demag_held_field: asd_enable_demag has not been called");
+  return demag_field_host(c, cells, dims, true);
+}
+
 size_t asd_track_exchange_workspace_bytes(const asd_ctx* ctx) { return ctx ? track_exchange_workspace_bytes(ctx->c) : 0; }
 
 asd_status asd_enable_track_exchange(asd_ctx* ctx, int32_t on, void* d_workspace, size_t bytes) {
@@ -486,7 +493,7 @@ asd_status asd_shift_window(asd_ctx* ctx, int32_t p) {
   if (c.d.pbc[0]) return fail(c, ASD_EUNSUPPORTED, "asd_shift_window: window is periodic in x");
   if (c.x0 + p + c.d.nx > c.d.track_nx) return fail(c, ASD_ESTATE, "asd_shift_window: past the end of the track");
   graphs_invalidate(c);                        // window origin and buffer roles are frozen in recorded graphs
-  c.demag_age = 0;                             // a held demagnetising field belongs to the old window position
+  demag_held_invalidate(c);                             // a held demagnetising field belongs to the old window position
   if (c.mm) {                                  // multiscale window: whole cells, through the meshes (M10)
     int64_t dl[3], dr[3];
     mm_dims(c, 0, dl); mm_dims(c, 1, dr);
@@ -531,7 +538,7 @@ asd_status asd_planes_view(asd_ctx* ctx, int32_t comp, int32_t i0, int32_t n, fl
   const size_t planep = (size_t)c.d.nz * (size_t)c.nyp;
   *d_ptr = c.arr(c.aS + comp) + c.lead + (size_t)i0 * planep;
   *count = (size_t)n * planep;
-  c.demag_age = 0;                             // the caller is about to change spins behind the library's back
+  demag_held_invalidate(c);                             // the caller is about to change spins behind the library's back
   mm_restart_cadence(c);
   return ASD_OK;
 }
@@ -589,7 +596,7 @@ asd_status asd_track_begin_pass(asd_ctx* ctx, int64_t x0_new) {
       return fail(c, ASD_EINVAL, "asd_track_begin_pass: a multiscale window starts on a whole macrocell with both meshes inside the track");
   }
   graphs_invalidate(c);
-  c.demag_age = 0;
+  demag_held_invalidate(c);
   return then_refresh_stray(c, launch_track_begin_pass(c, x0_new));
 }
 

@@ -52,6 +52,10 @@ struct DemagPlan {
   float2* twy = nullptr;              // [PY]   exp(+2 pi i n / PY)
   unsigned xconv_threads = 0;
   size_t xconv_smem = 0;
+  // Eq. (6) folded into the fused step (asd_heun_fused.cu): macrocell sums of the spins the last fused step wrote
+  long long* acc = nullptr;           // [3][dcx][dcy][dcz], units of 1 / acc_fx
+  float acc_fx = 0.0f;                // a power of two; a whole cell's sum stays below 2^31
+  enum AccState { ACC_CLEAN, ACC_VALID, ACC_STALE } acc_state = ACC_CLEAN;   // zeros / sums of the current S / leftovers
   // stray field of the frozen track on the window's macrocells (reading D4); own workspace
   bool stray = false;
   int XR = 0;                         // largest |x offset| in cells between a source and a target cell
@@ -191,7 +195,9 @@ __global__ void coarse_grain_ydft(const float* __restrict__ X, uint32_t as, int 
   const int i0 = (int)((x0 / mx + a) * (long long)mx - x0);      // first window plane of the cell (may be < 0)
   const int rows = mx * mz, groups = ny / VEC;
   const int rl = threadIdx.x / groups, g = threadIdx.x - rl * groups;
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   for (int t = threadIdx.x; t < PY; t += blockDim.x) tws[t] = __ldg(twy + t);
+  asm volatile("griddepcontrol.wait;" ::: "memory");            // the kernel that wrote X has completed
   if (rl < lanes) {
     float s[3][VEC];
 #pragma unroll
@@ -227,6 +233,27 @@ __global__ void coarse_grain_ydft(const float* __restrict__ X, uint32_t as, int 
     for (int j = b * my; j < j1; ++j)
       for (int l = 0; l < lanes; ++l) acc += col[((size_t)l * 3 + comp) * ny + j];
     cells[t] = acc * mu_over_V;
+  }
+  __syncthreads();
+  row_ydft(cells, tws, dcy, dcz, dcx, PY, NKY, a, c, Y);
+}
+
+// The same from the cell sums the fused step's corrector accumulated (64-bit fixed point, 1 / fx units): one CTA per
+// (cell-x a, cell-z c).  The sums are cleared for the next accumulation by demag_xconv, which follows: scattered 8-byte
+// stores from here kept every CTA waiting at its exit (measured: 10.1 us with them, 6.3 without).
+__global__ void cells_ydft(const long long* __restrict__ acc, double scale, int dcx, int dcy, int dcz, int PY, int NKY,
+                           const float2* __restrict__ twy, float2* __restrict__ Y) {
+  extern __shared__ __align__(16) float col[];                   // cells [3][dcy] | tws [PY]
+  float* cells = col;
+  float2* tws = reinterpret_cast<float2*>(cells + ((3 * dcy + 1) & ~1));
+  const int a = blockIdx.x / dcz, c = blockIdx.x - a * dcz;
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  for (int t = threadIdx.x; t < PY; t += blockDim.x) tws[t] = __ldg(twy + t);
+  asm volatile("griddepcontrol.wait;" ::: "memory");            // the step that accumulated the sums has completed
+  for (int t = threadIdx.x; t < 3 * dcy; t += blockDim.x) {
+    const int comp = t / dcy, b = t - comp * dcy;
+    const size_t q = (((size_t)comp * dcx + a) * dcy + b) * dcz + c;
+    cells[t] = (float)((double)acc[q] * scale);
   }
   __syncthreads();
   row_ydft(cells, tws, dcy, dcz, dcx, PY, NKY, a, c, Y);
@@ -345,7 +372,8 @@ __device__ __forceinline__ void chunk8(float2* x, int f_count, int logPX, int PX
 // over layers, inverse x-FFT of the dcz output fields of component oc.
 __global__ void __launch_bounds__(1024, 1)
 demag_xconv(const float2* __restrict__ Y, float2* __restrict__ Z, const float* __restrict__ Kh,
-            const float2* __restrict__ twx, int dcx, int dcz, int PX, int logPX, int NKY) {
+            const float2* __restrict__ twx, int dcx, int dcz, int PX, int logPX, int NKY,
+            long long* __restrict__ acc_clear, int acc_n) {
   extern __shared__ __align__(16) float2 xs[];                   // X[F][PXP] | O[dcz][PXP] | tw[PX/2] | Ks[3][NDZ][PX]
   const int F = 3 * dcz, NDZ = 2 * dcz - 1, H = PX >> 1, PXP = PX + (PX >> 3);
   float2* X = xs;
@@ -368,6 +396,11 @@ demag_xconv(const float2* __restrict__ Y, float2* __restrict__ Z, const float* _
   }
   asm volatile("cp.async.commit_group;" ::: "memory");
   asm volatile("griddepcontrol.wait;" ::: "memory");
+  if (acc_clear) {
+    // cells_ydft has read the fused step's cell sums: cleared here (coalesced, long before this kernel ends)
+    const int gt = (blockIdx.y * gridDim.x + blockIdx.x) * nt + tid, gn = gridDim.x * gridDim.y * nt;
+    for (int t = gt; t < acc_n; t += gn) acc_clear[t] = 0;
+  }
   __syncthreads();
   // Load with the first forward stage folded in: the upper half of the padded input is zero (dcx <= PX/2), so that
   // stage is X[p] = x[p], X[p + PX/2] = x[p] w^p.
@@ -550,7 +583,7 @@ size_t cg_smem_bytes(int lanes, int ny, const DemagPlan& pl) {
 }
 
 struct Carve {
-  size_t Y, Z, Kh, B, twx, twy, total;
+  size_t Y, Z, Kh, B, twx, twy, acc, total;
 };
 void carve(const DemagPlan& pl, Carve& cv) {
   const size_t spec = (size_t)pl.NKY * pl.F * pl.dcx;
@@ -562,6 +595,7 @@ void carve(const DemagPlan& pl, Carve& cv) {
   cv.B = take((size_t)3 * pl.dcx * pl.dcy * pl.dcz * sizeof(float));
   cv.twx = take((size_t)(pl.PX / 2) * sizeof(float2));
   cv.twy = take((size_t)pl.PY * sizeof(float2));
+  cv.acc = take((size_t)3 * pl.dcx * pl.dcy * pl.dcz * sizeof(long long));
   cv.total = off;
 }
 
@@ -600,6 +634,13 @@ asd_status demag_enable(Ctx& c, const double spacing[3], void* ws, size_t bytes)
   char* base = (char*)ws;
   pl->Y = (float2*)(base + cv.Y); pl->Z = (float2*)(base + cv.Z); pl->Kh = (float*)(base + cv.Kh);
   pl->B = (float*)(base + cv.B); pl->twx = (float2*)(base + cv.twx); pl->twy = (float2*)(base + cv.twy);
+  pl->acc = (long long*)(base + cv.acc);
+  {
+    const long long sites = (long long)c.d.macro[0] * c.d.macro[1] * c.d.macro[2];
+    int bits = 30;
+    while (bits > 0 && (sites << bits) >= (1ll << 31)) --bits;
+    pl->acc_fx = (float)(1ll << bits);
+  }
   for (int a = 0; a < 3; ++a) pl->cell[a] = c.d.macro[a] * spacing[a];
   pl->mu_over_V = (float)(c.d.mu_s / (pl->cell[0] * pl->cell[1] * pl->cell[2]));
   ASD_CUDA_TRY(c, cudaFuncSetAttribute((const void*)demag_xconv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->xconv_smem));
@@ -645,6 +686,8 @@ asd_status demag_enable(Ctx& c, const double spacing[3], void* ws, size_t bytes)
   ASD_CUDA_TRY(c, cudaMemcpyAsync(pl->twx, twx.data(), twx.size() * sizeof(float2), cudaMemcpyHostToDevice, c.stream));
   ASD_CUDA_TRY(c, cudaMemcpyAsync(pl->twy, twy.data(), twy.size() * sizeof(float2), cudaMemcpyHostToDevice, c.stream));
   ASD_CUDA_TRY(c, cudaMemsetAsync(pl->B, 0, (size_t)3 * pl->dcx * pl->dcy * pl->dcz * sizeof(float), c.stream));
+  ASD_CUDA_TRY(c, cudaMemsetAsync(pl->acc, 0, (size_t)3 * pl->dcx * pl->dcy * pl->dcz * sizeof(long long), c.stream));
+  pl->acc_state = DemagPlan::ACC_CLEAN;
   ASD_CUDA_TRY(c, cudaStreamSynchronize(c.stream));             // the host vectors are about to go out of scope
   graphs_invalidate(c);
   return ASD_OK;
@@ -754,9 +797,21 @@ void launch_chain(void (*kern)(Args...), dim3 grid, unsigned threads, size_t sme
 }  // namespace
 
 // Demagnetising field of the configuration in array block aX (S or S~) into demag->B, on c.launch_stream.
-asd_status launch_demag(Ctx& c, int aX) {
+asd_status launch_demag(Ctx& c, int aX, bool may_use_acc) {
   DemagPlan& pl = *c.demag;
-  {
+  long long* acc_used = nullptr;
+  if (may_use_acc && pl.acc_state == DemagPlan::ACC_VALID && aX == c.aS) {
+    // Eq. (6) was done by the corrector of the fused step that wrote these spins
+    // latency-bound (one dependent load, one barrier, a 3 NKY x dcy transform): small CTAs so that all of them are
+    // resident at once (two passes of row_ydft each)
+    const unsigned threads = (unsigned)std::min<size_t>(1024, align_up((size_t)6 * pl.NKY, 32));
+    launch_chain(cells_ydft, dim3((unsigned)(pl.dcx * pl.dcz)), threads, cg_smem_bytes(0, c.d.ny, pl), c.launch_stream,
+                 (const long long*)pl.acc, (double)pl.mu_over_V / (double)pl.acc_fx, pl.dcx, pl.dcy, pl.dcz, pl.PY, pl.NKY,
+                 (const float2*)pl.twy, pl.Y);
+    ASD_LAUNCH_CHECK(c, "cells_ydft");
+    acc_used = pl.acc;
+    pl.acc_state = DemagPlan::ACC_CLEAN;
+  } else {
     const int vec = (c.d.ny % 4 == 0) ? 4 : 1, groups = c.d.ny / vec;
     int lanes = 1024 / groups;
     if (lanes > kMaxRowLanes) lanes = kMaxRowLanes;
@@ -765,18 +820,15 @@ asd_status launch_demag(Ctx& c, int aX) {
     const int threads = (int)align_up((size_t)(groups * lanes), 32);
     const size_t smem = cg_smem_bytes(lanes, c.d.ny, pl);
     const unsigned blocks = (unsigned)(pl.dcx * pl.dcz);
-    if (vec == 4)
-      coarse_grain_ydft<4><<<blocks, threads, smem, c.launch_stream>>>(
-          c.arr(aX), (uint32_t)c.as, c.d.nx, c.d.ny, c.d.nz, c.nyp, c.lead, c.d.macro[0], c.d.macro[1], c.d.macro[2],
-          (long long)c.x0, pl.dcx, pl.dcy, pl.dcz, pl.PY, pl.NKY, pl.mu_over_V, lanes, pl.twy, pl.Y);
-    else
-      coarse_grain_ydft<1><<<blocks, threads, smem, c.launch_stream>>>(
-          c.arr(aX), (uint32_t)c.as, c.d.nx, c.d.ny, c.d.nz, c.nyp, c.lead, c.d.macro[0], c.d.macro[1], c.d.macro[2],
-          (long long)c.x0, pl.dcx, pl.dcy, pl.dcz, pl.PY, pl.NKY, pl.mu_over_V, lanes, pl.twy, pl.Y);
+    launch_chain(vec == 4 ? coarse_grain_ydft<4> : coarse_grain_ydft<1>, dim3(blocks), (unsigned)threads, smem, c.launch_stream,
+                 (const float*)c.arr(aX), (uint32_t)c.as, c.d.nx, c.d.ny, c.d.nz, c.nyp, c.lead, c.d.macro[0], c.d.macro[1],
+                 c.d.macro[2], (long long)c.x0, pl.dcx, pl.dcy, pl.dcz, pl.PY, pl.NKY, pl.mu_over_V, lanes,
+                 (const float2*)pl.twy, pl.Y);
+    ASD_LAUNCH_CHECK(c, "coarse_grain_ydft");
   }
-  ASD_LAUNCH_CHECK(c, "coarse_grain_ydft");
   launch_chain(demag_xconv, dim3((unsigned)pl.NKY, 3u), pl.xconv_threads, pl.xconv_smem, c.launch_stream,
-               (const float2*)pl.Y, pl.Z, (const float*)pl.Kh, (const float2*)pl.twx, pl.dcx, pl.dcz, pl.PX, pl.logPX, pl.NKY);
+               (const float2*)pl.Y, pl.Z, (const float*)pl.Kh, (const float2*)pl.twx, pl.dcx, pl.dcz, pl.PX, pl.logPX, pl.NKY,
+               acc_used, 3 * pl.dcx * pl.dcy * pl.dcz);
   ASD_LAUNCH_CHECK(c, "demag_xconv");
   launch_chain(demag_yinv, dim3((unsigned)((pl.dcx + kYinvCols - 1) / kYinvCols), (unsigned)pl.F), 256u,
                ((size_t)pl.NKY * kYinvCols + pl.PY) * sizeof(float2), c.launch_stream,
@@ -784,6 +836,29 @@ asd_status launch_demag(Ctx& c, int aX) {
                (const float*)(pl.stray ? pl.Bt : nullptr));
   ASD_LAUNCH_CHECK(c, "demag_yinv");
   return ASD_OK;
+}
+
+long long* demag_acc_arm(Ctx& c, float& fx) {
+  if (!c.demag) return nullptr;
+  static const bool off = [] { const char* e = std::getenv("ASD_DEMAG_EPILOGUE"); return e && std::atoi(e) == 0; }();   // tuning override
+  if (off) return nullptr;
+  DemagPlan& pl = *c.demag;
+  if (pl.acc_state != DemagPlan::ACC_CLEAN) {
+    if (cudaMemsetAsync(pl.acc, 0, (size_t)3 * pl.dcx * pl.dcy * pl.dcz * sizeof(long long), c.launch_stream) != cudaSuccess) {
+      cudaGetLastError();
+      return nullptr;
+    }
+  }
+  pl.acc_state = DemagPlan::ACC_VALID;
+  fx = pl.acc_fx;
+  return pl.acc;
+}
+void demag_acc_drop(Ctx& c) {
+  if (c.demag && c.demag->acc_state == DemagPlan::ACC_VALID) c.demag->acc_state = DemagPlan::ACC_STALE;
+}
+void demag_held_invalidate(Ctx& c) {
+  c.demag_age = 0;
+  demag_acc_drop(c);
 }
 
 void demag_fill_params(const Ctx& c, StageParams& p) {
@@ -800,13 +875,15 @@ void demag_fill_params(const Ctx& c, StageParams& p) {
 }
 
 // Host copy of the cell field of the CURRENT spins (tests, diagnostics); synchronises.
-asd_status demag_field_host(Ctx& c, float* out, int64_t dims[3]) {
+asd_status demag_field_host(Ctx& c, float* out, int64_t dims[3], bool held) {
   DemagPlan& pl = *c.demag;
   dims[0] = pl.dcx; dims[1] = pl.dcy; dims[2] = pl.dcz;
   if (!out) return ASD_OK;
   c.launch_stream = c.stream;
-  const asd_status st = launch_demag(c, c.aS);
-  if (st != ASD_OK) return st;
+  if (!held) {
+    const asd_status st = launch_demag(c, c.aS);
+    if (st != ASD_OK) return st;
+  }
   const size_t cells = (size_t)pl.dcx * pl.dcy * pl.dcz;
   std::vector<float> h(3 * cells);
   ASD_CUDA_TRY(c, cudaMemcpyAsync(h.data(), pl.B, 3 * cells * sizeof(float), cudaMemcpyDeviceToHost, c.stream));

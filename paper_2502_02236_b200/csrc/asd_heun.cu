@@ -327,6 +327,7 @@ asd_status launch_heun_direct(Ctx& c, int64_t n, const DynState* dyn) {
       c.demag_refresh = c.demag_every <= 0 ? 3 : (c.demag_age % c.demag_every == 0 ? 1 : 0);
       c.demag_age += 1;
     }
+    if (c.demag && !fused) demag_acc_drop(c);           // cell sums a fused step left behind: of spins about to change
     asd_status st;
     if (fused) st = launch_heun_fused(c, p);
     else if (staged) st = launch_heun_tma(c, p);

@@ -59,6 +59,11 @@ struct FusedParams {
   const float* edgeB;              // multiscale window: mesh exchange field on planes 0 / nx-1 ([side][comp][nz*nyp]); nullptr: off
   DemagGeom dm;                    // held demagnetising field per macrocell (DEMAG instances; asd_set_demag_every >= 1)
   uint32_t dm_my;                  // macrocell edge in y (sites)
+  // Eq. (6) folded into the corrector (DEMAG instances, dm_acc != nullptr): the new spins' macrocell sums, in units of
+  // 1 / dm_fx, are added to dm_acc[comp * comp_stride + cell] -- the layout of dm.B -- for the next refresh of the held field
+  long long* dm_acc;
+  uint32_t dm_mx, dm_ncyl;         // macrocell edge in x (sites); y-cells a strip can overlap
+  float dm_fx;                     // fixed-point scale (a power of two; a whole cell's sum stays below 2^31)
   PhiloxKey key;
 };
 
@@ -115,6 +120,10 @@ __device__ __forceinline__ bool warp_count_last(uint32_t cnt, uint32_t nwarps) {
   return last;
 }
 
+__device__ __forceinline__ void red_shared_add(uint32_t a, int v) {
+  asm volatile("red.shared.add.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
+}
+
 constexpr uint32_t kGpRing = 8;   // planes of per-group anisotropy parameters kept in shared memory
 
 // NZ_T / BY_T != 0: film thickness and strip width are compile-time constants (every shared-memory offset becomes an
@@ -139,6 +148,10 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
   const uint32_t sring = gpring + ((kGpRing * gp_pitch + 127u) & ~127u);
   const uint32_t tring = sring + kRingS * slot_pitch;
   const uint32_t fbox = tring + kRingT * slot_pitch;
+  // DEMAG with dm_acc: cell sums of the new spins, [2 x-cell parities][3][dm_ncyl][dcz] int32, behind the field box
+  const uint32_t sacc = fbox + ((fbytes + 127u) & ~127u);
+  const uint32_t acc_comp = DEMAG ? p.dm_ncyl * p.dm.sy * 4u : 0u, acc_buf = 3u * acc_comp;
+  const bool acc_on = DEMAG && p.dm_acc != nullptr;
 
   const int tid = (int)threadIdx.x;
   const int strip = (int)blockIdx.x % p.nstrips, chunk = (int)blockIdx.x / p.nstrips;
@@ -184,6 +197,8 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
   // is discarded, but a stray "two grains" flag would send it to the column table)
   for (uint32_t o = (uint32_t)tid * 16u; o < kGpRing * gp_pitch; o += (uint32_t)blockDim.x * 16u)
     sts4(gpring + o, 0.0f, 0.0f, 0.0f, 0.0f);
+  if (acc_on)
+    for (uint32_t o = (uint32_t)tid * 4u; o < 2u * acc_buf; o += (uint32_t)blockDim.x * 4u) sts1(sacc + o, 0.0f);
   asm volatile("bar.sync 0;" ::: "memory");
   if (tid == 0) {
     for (int s = 0; s < 4; ++s) {
@@ -238,6 +253,22 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
   auto arrive_done = [&](int m) { warp_arrive(done_bar(m)); };
   auto phase = [](int m) { return (uint32_t)(m >> 2) & 1u; };
 
+  // DEMAG with dm_acc, halo warp(s): the shared sums of the cells with x index ca (absolute) -> global, slots cleared
+  auto acc_flush = [&](uint32_t ca) {
+    const uint32_t nent = p.dm_ncyl * p.dm.sy, cy0 = div_u31((uint32_t)j0, p.dm.my_m, p.dm.my_s), dcy = p.dm.sx / p.dm.sy;
+    const uint32_t sb = sacc + (ca & 1u) * acc_buf;
+    for (uint32_t t = (uint32_t)(tid - p.n_main); t < 3u * nent; t += blockDim.x - (uint32_t)p.n_main) {
+      const uint32_t comp = t / nent, r = t - comp * nent, cyl = r / p.dm.sy, ck = r - cyl * p.dm.sy;
+      const int v = __float_as_int(lds1(sb + t * 4u));
+      if (v != 0 && cy0 + cyl < dcy) {
+        atomicAdd(reinterpret_cast<unsigned long long*>(p.dm_acc) +
+                      (comp * p.dm.comp_stride + (ca - p.dm.c0) * p.dm.sx + (cy0 + cyl) * p.dm.sy + ck),
+                  (unsigned long long)(long long)v);
+        sts1(sb + t * 4u, 0.0f);
+      }
+    }
+  };
+
   if (is_main) {
     // ================= main threads: 4 consecutive y-sites of one z-row, predictor and corrector =================
     const int k = tid / G, g = tid - k * G;
@@ -269,11 +300,13 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
     // held demagnetising field (DEMAG): the thread's two macrocells across the film and through its thickness are fixed
     uint32_t dm_yz_lo = 0u, dm_yz_hi = 0u;
     int dm_nlo = 4;                                    // own sites v < dm_nlo lie in the lower-y cell
+    uint32_t sacc_own = sacc;                          // the lower-y cell's slot in the shared cell sums (parity 0, component 0)
     if (DEMAG && active) {
       const uint32_t cj_lo = div_u31((uint32_t)j, p.dm.my_m, p.dm.my_s), cj_hi = div_u31((uint32_t)j + 3u, p.dm.my_m, p.dm.my_s);
       const uint32_t ck = div_u31((uint32_t)k, p.dm.mz_m, p.dm.mz_s);
       dm_yz_lo = cj_lo * p.dm.sy + ck; dm_yz_hi = cj_hi * p.dm.sy + ck;
       dm_nlo = (cj_lo == cj_hi) ? 4 : (int)(cj_hi * p.dm_my) - j;
+      sacc_own = sacc + ((cj_lo - div_u31((uint32_t)j0, p.dm.my_m, p.dm.my_s)) * p.dm.sy + ck) * 4u;
     }
     mbar_wait_long(bar_full + 0u, 0u);
     mbar_wait_long(bar_full + 8u, 0u);
@@ -485,6 +518,20 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
           for (int c = 0; c < 3; ++c)
             *reinterpret_cast<float4*>(p.arrays_w + (p.oOut + (uint32_t)c * p.as + eo)) =
                 make_float4(So[c][0], So[c][1], So[c][2], So[c][3]);
+          if (acc_on) {
+            // Eq. (6) for the next refresh of the held field: this plane's share of the thread's one or two macrocells,
+            // as integers (the sum is then independent of the order in which the threads arrive)
+            const uint32_t cpar = div_u31(p.dm.x0 + (uint32_t)(i0 + m - 2), p.dm.mx_m, p.dm.mx_s) & 1u;
+            const uint32_t sb = sacc_own + cpar * acc_buf;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+              float lo = 0.0f, hi = 0.0f;
+#pragma unroll
+              for (int v = 0; v < 4; ++v) { if (v < dm_nlo) lo += So[c][v]; else hi += So[c][v]; }
+              red_shared_add(sb + (uint32_t)c * acc_comp, __float2int_rn(lo * p.dm_fx));
+              if (dm_nlo < 4) red_shared_add(sb + (uint32_t)c * acc_comp + p.dm.sy * 4u, __float2int_rn(hi * p.dm_fx));
+            }
+          }
         }
       }
 #pragma unroll
@@ -494,6 +541,7 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
       e += planep; ec += (uint32_t)p.ny; gsite += gplane;
       t3 = (t3 == 2u) ? 0u : t3 + 1u;
     }
+    if (acc_on) arrive_done(L + 2);                   // the last planes' cell sums are in shared memory
   } else {
     // ================= halo warp(s): the two sites (y = j0 - 1, y = j0 + BY) of one z-row, predictor only; =================
     // ================= and the per-group anisotropy parameters two planes ahead                              =================
@@ -621,6 +669,13 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
       // the edges of their x+1 plane) or m - 2 (SC: as the edges of their own plane), i.e. before they arrived for
       // step m - 1.
       if (m >= 1) mbar_wait_long(done_bar(m - 1), phase(m - 1));
+      if (acc_on && m >= 4) {
+        // every main warp has arrived for step m - 1, i.e. has added plane i0 + m - 4 (corrected in step m - 2) to the cell
+        // sums: if that plane closes its macrocell, the cell's sums go to global memory and its slots are cleared (the
+        // slots of this parity are next written for the cell after the next, behind this warp's arrival for step m)
+        const uint32_t xg = p.dm.x0 + (uint32_t)(i0 + m - 4), ca = div_u31(xg, p.dm.mx_m, p.dm.mx_s);
+        if (xg + 1u == (ca + 1u) * p.dm_mx) acc_flush(ca);
+      }
 #pragma unroll
       for (int s = 0; s < 2; ++s)
         if (act[s]) {
@@ -636,6 +691,14 @@ heun_fused(const __grid_constant__ CUtensorMap mapS, const __grid_constant__ CUt
           for (int d = 0; d < 3; ++d) { rP[s][c][d] = rC[s][c][d]; rC[s][c][d] = rN[s][c][d]; }
       e += planep; ec += (uint32_t)p.ny; gsite += gplane;
       t3 = (t3 == 2u) ? 0u : t3 + 1u;
+    }
+    if (acc_on) {
+      // what is left: the (at most two) cells that the chunk's last two planes belong to
+      arrive_done(L + 2);
+      mbar_wait_long(done_bar(L + 2), phase(L + 2));
+      const uint32_t ca = div_u31(p.dm.x0 + (uint32_t)(i0 + L - 1), p.dm.mx_m, p.dm.mx_s);
+      acc_flush(ca);
+      if (ca > p.dm.c0) acc_flush(ca - 1u);
     }
   }
 }
@@ -686,6 +749,8 @@ struct FusedPlan {
   FusedKernel kern_dm = nullptr;   // the instance that adds a held demagnetising field per macrocell; may be null
   int32_t BY = 0, G = 0, nstrips = 0, CX = 0, nchunks = 0, threads = 0, n_main = 0, ctas_per_sm = 0;
   uint32_t slot_pitch = 0, smem_bytes = 0;
+  uint32_t smem_bytes_dm = 0;      // kern_dm: + the shared cell sums of the Eq. (6) epilogue (0: they do not fit; no epilogue)
+  uint32_t dm_ncyl = 0;
 };
 
 bool heun_fused_supported(const Ctx& c) { return heun_fast_supported(c) && c.d.nz + 2 <= 256; }
@@ -751,8 +816,18 @@ bool build_plan(Ctx& c, FusedPlan& pl) {
     pl.kern_mm = nullptr;
   }
   pl.kern_dm = kernel_for(c.d.lattice, best.shape, nz, pl.BY, false, true);
+  {
+    // Eq. (6) epilogue: [2][3][y-cells a strip can overlap][cell layers] int32 behind the field box, if that keeps the
+    // CTAs per SM (else the cell sums come from coarse_grain_ydft as before)
+    const int my = c.d.macro[1] > 0 ? c.d.macro[1] : 1, mz = c.d.macro[2] > 0 ? c.d.macro[2] : 1;
+    pl.dm_ncyl = (uint32_t)((pl.BY - 1) / my + 2);
+    const uint32_t acc_bytes = (uint32_t)align_up((size_t)2 * 3 * pl.dm_ncyl * ((nz + mz - 1) / mz) * 4, 128);
+    const uint32_t with_acc = pl.smem_bytes + acc_bytes;
+    pl.smem_bytes_dm = ((int)with_acc <= smem_cta && smem_sm / (int)(with_acc + 1024) >= std::min(best.ctas, smem_sm / (int)(pl.smem_bytes + 1024)))
+                           ? with_acc : 0u;
+  }
   if (pl.kern_dm && cudaFuncSetAttribute((const void*)pl.kern_dm, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)pl.smem_bytes) != cudaSuccess) {
+                                         (int)std::max(pl.smem_bytes, pl.smem_bytes_dm)) != cudaSuccess) {
     cudaGetLastError();
     pl.kern_dm = nullptr;
   }
@@ -836,7 +911,14 @@ asd_status launch_heun_fused(Ctx& c, StageParams& p) {
   if (f.edgeB && !pl->kern_mm) return ASD_EUNSUPPORTED;
   if (f.dm.B && (!pl->kern_dm || f.edgeB || c.demag_every < 1)) return ASD_EUNSUPPORTED;
   // held-field scheme: the field of S is refreshed before the step when the cadence says so, then serves both stages
-  if (f.dm.B && (c.demag_refresh & 1)) { const asd_status st = launch_demag(c, c.aS); if (st != ASD_OK) return st; }
+  // (from the cell sums the previous fused step left behind, when it did: demag_acc_arm below)
+  if (f.dm.B && (c.demag_refresh & 1)) { const asd_status st = launch_demag(c, c.aS, true); if (st != ASD_OK) return st; }
+  f.dm_acc = nullptr; f.dm_mx = (uint32_t)c.d.macro[0]; f.dm_ncyl = pl->dm_ncyl; f.dm_fx = 0.0f;
+  if (f.dm.B && pl->smem_bytes_dm && c.demag_age % c.demag_every == 0) {
+    // the NEXT step refreshes the held field from the spins this step writes: Eq. (6) rides with the corrector
+    f.dm_acc = demag_acc_arm(c, f.dm_fx);
+    if (f.dm_acc) cfg.dynamicSmemBytes = pl->smem_bytes_dm;
+  }
   cudaLaunchKernelEx(&cfg, f.dm.B ? pl->kern_dm : (f.edgeB ? pl->kern_mm : pl->kern), pl->mapS, pl->mapF, f);
   ASD_LAUNCH_CHECK(c, "heun step (fused)");
   const int t = c.aS; c.aS = c.aSt; c.aSt = t;

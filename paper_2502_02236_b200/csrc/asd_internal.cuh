@@ -233,9 +233,13 @@ DynState* dyn_state(const Ctx& c);
 size_t demag_workspace_bytes(Ctx& c);
 asd_status demag_enable(Ctx& c, const double spacing[3], void* ws, size_t bytes);
 void demag_free(Ctx& c);
-asd_status launch_demag(Ctx& c, int aX);                      // field of the configuration in arrays aX..aX+2
+asd_status launch_demag(Ctx& c, int aX, bool may_use_acc = false);   // field of the configuration in arrays aX..aX+2
+// Eq. (6) folded into the fused step's corrector: the macrocell sums of the spins a step writes, as 64-bit fixed point
+long long* demag_acc_arm(Ctx& c, float& fx);                  // zeroed buffer for the step about to be launched (or nullptr), its scale
+void demag_acc_drop(Ctx& c);                                  // the spins changed by other means: the sums are stale
+void demag_held_invalidate(Ctx& c);                           // ... and so is the held field (age 0)
 void demag_fill_params(const Ctx& c, StageParams& p);
-asd_status demag_field_host(Ctx& c, float* out, int64_t dims[3]);
+asd_status demag_field_host(Ctx& c, float* out, int64_t dims[3], bool held = false);   // held: the stored field, nothing recomputed
 size_t demag_stray_workspace_bytes(Ctx& c, int range_cells);     // stray field of the frozen track (reading D4)
 asd_status demag_stray_enable(Ctx& c, int on, int range_cells, void* ws, size_t bytes);
 asd_status demag_stray_refresh(Ctx& c);                          // after the window origin or the track store changed

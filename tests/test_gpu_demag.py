@@ -83,6 +83,41 @@ def test_fused_step_with_the_held_field(lattice, every):
     assert np.abs(h.get_spins_host() - g.get_spins_host()).max() <= 2e-5
 
 
+@pytest.mark.parametrize("lattice", [ai.SC, ai.L10])
+@pytest.mark.parametrize("dims,macro,x0,every", [((24, 40, 6), (4, 5, 2), 1, 1), ((40, 132, 9), (7, 7, 5), 5, 1),
+                                                 ((21, 40, 7), (4, 5, 2), 2, 2), ((36, 64, 8), (1, 3, 1), 0, 1),
+                                                 ((30, 36, 5), (9, 4, 5), 4, 3)])
+def test_cell_sums_from_the_fused_corrector(lattice, dims, macro, x0, every):
+    """Eq. (6) behind a refresh of the held field is accumulated by the corrector of the fused step before it (integer
+    cell sums): the field the next step holds is the oracle's field of those spins, and the film kernel's (whose cell
+    sums come from a pass of their own), before and after a shift that leaves stale sums behind."""
+    import paper_2502_02236_b200 as asd
+    nx, ny, nz = dims
+    w = _film(lattice, nx, ny, nz, macro, x0, 30.0, dt=1e-16)
+    o, g = _pair(w)
+    h = gpu_from_workload(w); h.enable_demag([a * 1e-9 for a in w.spacing_nm])
+    for c in (o, g, h):
+        c.set_demag_every(every)
+    g.set_kernel(asd.KERNEL_FUSED); h.set_kernel(asd.KERNEL_FAST)
+    n = 2 * every + 1                                               # steps 1, every + 1, 2 every + 1 refresh
+    for leg in range(2):
+        o.step_heun(n - 1)
+        Bo = o.demag_cells()                                        # field of the spins step n starts from
+        o.step_heun(1)
+        g.step_heun(n); h.step_heun(n)
+        Bg, Bh = g.demag_held_field(), h.demag_held_field()
+        scale = np.abs(Bo).max()
+        assert scale > 1e-3
+        assert np.abs(Bg - Bo).max() <= 1e-4 * scale                # spins differ by <= 5e-5 by then
+        assert np.abs(Bg - Bh).max() <= 3e-5 * scale
+        assert max_abs_diff(g, o) <= 1e-4
+        if leg == 0:
+            if every > 1:                                           # end on a step that armed the sums
+                g.step_heun(every - 1); h.step_heun(every - 1); o.step_heun(every - 1)
+            assert o.shift_window(3) == 0
+            g.shift_window(3); h.shift_window(3)
+
+
 @pytest.mark.parametrize("every", [1, 3])
 def test_held_field_update_period(every):
     """asd_set_demag_every(P): field from S at every P-th step, held for both stages in between; a shift re-arms it."""
