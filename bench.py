@@ -188,6 +188,7 @@ class Run:
                  track_stray=False):
         self.asd, self.torch, self.w, self.hps = asd, torch, w, hps
         self.N = w.n_sites
+        self.demag, self.demag_every, self.multiscale = demag, demag_every, multiscale is not None
         table = None
         if ell:
             # the same exchange bonds handed over as a general ELL table (per-pair J); such a table cannot follow the
@@ -281,6 +282,21 @@ class Run:
              "frac_survey_floor": SURVEY_FLOOR_BYTES[w.lattice] * N / step_s / 1e9 / peak if not self.ell_w else None,
              # DRAM bytes the committed ncu capture counted for this kernel / this run's launch time
              "frac_dram": (traffic / avg_launch_s / 1e9 / peak) if traffic else None}
+        if self.demag or self.multiscale:
+            # the launches of a Heun step include the field pipeline's (mesh kernels'): the events around a batch cannot
+            # time the Heun kernel alone, so the record is the WHOLE step at the Heun kernels' algorithmic bytes -- a lower
+            # bound on their own fraction; per-kernel times: profiles/r2_demag.md, r2_multiscale.md
+            refreshes = (2.0 if self.demag_every < 1 else 1.0 / self.demag_every) if self.demag else 0.0   # 3 launches each
+            one_kernel = (per_step - 3.0 * refreshes) < (1.9 if self.multiscale else 1.5)
+            alg = (FUSED_BYTES_PER_SITE_STEP if one_kernel else 2 * BYTES_PER_SITE_PER_STAGE) * N
+            extra = "demagnetising-field pipeline" if self.demag else "mesh kernels"
+            r.update(kernel=("heun_fused, one kernel per Heun step (40 B/site)" if one_kernel else
+                             "stage kernels (predictor + corrector, 52 B/site each)") + " + " + extra +
+                            " (%.2f launches per Heun step)" % per_step,
+                     achieved=alg / step_s / 1e9, frac=alg / step_s / 1e9 / peak, avg_launch_us=None,
+                     algorithmic_bytes_per_launch=alg, traffic=None, frac_dram=None,
+                     note="whole Heun step incl. the %s, at the Heun kernels' algorithmic bytes per step" % extra)
+            return r
         if fused:
             issue_peak = SM_COUNT * SCHEDULERS_PER_SM * LANES * _sm_max_hz()
             alg_inst = ALG_INST_PER_SITE_STEP[w.lattice] * N
@@ -455,13 +471,8 @@ def secondary(asd, torch, device, args, peak, peak_src):
                    "unit": UNIT, "us_per_heun_step": t["heun_ms"] * 1e3 / heun_steps, "kernel": r["kernel"],
                    "avg_launch_us": r["avg_launch_us"], "frac": r["frac"], "frac_survey_floor": r["frac_survey_floor"],
                    "shifts_in_timed_region": t["shifts"]}
-            if kw.get("multiscale") is not None:
-                rec.update(kernel="Heun kernels + mesh kernels (exchange, edge field, m_e, 4 RK4 stages per mesh step)",
-                           avg_launch_us=None, frac=None)
-            elif kw.get("demag"):
-                # the launches of a step include the demagnetising-field pipeline: no single-kernel fraction to quote
-                rec.update(kernel=("fused Heun step" if kw.get("demag_every") else "stage kernels") +
-                           " + demagnetising-field pipeline", avg_launch_us=None, frac=None)
+            if kw.get("multiscale") is not None or kw.get("demag"):
+                rec.update(frac=None)      # the step includes other kernels: no single-kernel fraction to quote
             elif w.n_sites < (1 << 18):
                 rec.update(frac=None, frac_survey_floor=None, note="launch-bound: no roofline fraction")
             elif 13 * 4 * w.n_sites < 126e6:
