@@ -185,10 +185,10 @@ class Run:
     """One context on one workload: warm-up, device-timed bench steps (Heun batches + the schedule's shifts)."""
 
     def __init__(self, asd, torch, w, device, hps, kernel="auto", ell=False, demag=False, demag_every=0, multiscale=None,
-                 track_stray=False):
+                 track_stray=False, track_exchange=False):
         self.asd, self.torch, self.w, self.hps = asd, torch, w, hps
         self.N = w.n_sites
-        self.demag, self.demag_every, self.multiscale = demag, demag_every, multiscale is not None
+        self.demag, self.demag_every, self.multiscale = demag, demag_every, (multiscale is not None)
         table = None
         if ell:
             # the same exchange bonds handed over as a general ELL table (per-pair J); such a table cannot follow the
@@ -202,6 +202,8 @@ class Run:
             self.ctx.set_demag_every(demag_every)
             if track_stray:                              # + the frozen track's stray field, recomputed at every shift
                 self.ctx.enable_track_stray(True, 0)
+        if track_exchange:                           # window ends exchange coupled to the frozen track (reading E1)
+            self.ctx.enable_track_exchange(True)
         if multiscale is not None:                   # micromagnetic meshes either side
             ai.apply_multiscale(self.ctx, multiscale)
         if kernel != "auto":
@@ -344,7 +346,7 @@ def run_ours(args):
     N = w.n_sites
     hps = args.heun_per_step
     run = Run(asd, torch, w, device, hps, kernel=args.kernel, ell=args.ell, demag=args.demag, demag_every=args.demag_every,
-              multiscale=msw, track_stray=args.track_stray)
+              multiscale=msw, track_stray=args.track_stray, track_exchange=args.track_exchange)
     ctx, dev = run.ctx, run.ctx.device
     run.start(args.warmup, args.steps)
     barrier()
@@ -397,7 +399,7 @@ def run_ours(args):
         "config": {"workload": w.name, "sites": N, "heun_steps_per_step": hps, "shifts_in_timed_region": t["shifts"],
                    "shift_every_heun_steps": w.shift_every, "dt": w.dt, "parallelism": f"replicas x{world}",
                    "ell_width": run.ell_w, "demag": bool(args.demag), "demag_every": args.demag_every if args.demag else None,
-                   "track_stray": bool(args.demag and args.track_stray),
+                   "track_stray": bool(args.demag and args.track_stray), "track_exchange": bool(args.track_exchange),
                    "kernel": args.kernel, "multiscale": ({"mesh_cells": list(msw.mcx), "every": msw.every} if msw else None),
                    "l2": "working set (13 fp32 arrays/site = %.0f MB) exceeds the 126 MB L2" % (13 * 4 * N / 1e6)},
         "clocks": clocks, "gpu_launches": int(t["launches"]),
@@ -488,6 +490,9 @@ def secondary(asd, torch, device, args, peak, peak_src):
     one("cfg4 with the demagnetising field recomputed in every stage", 4, demag=True, demag_every=0)
     one("cfg4 with the demagnetising field recomputed once per Heun step and held for both stages (fused step)", 4,
         demag=True, demag_every=1)
+    one("cfg4 with everything P:33 puts on the window: ends exchange coupled to the frozen track, demagnetising field "
+        "once per Heun step, the track's stray field at every shift (fused step)", 4, demag=True, demag_every=1,
+        track_stray=True, track_exchange=True)
     one("cfg3 SC 400x200x27", 3)
     one("cfg0 SC 16^3 periodic on the persistent cluster (us per Heun step is the figure)", 0, hps=1000, steps=3)
     one("cfg0 through CUDA-graph replay of the stage kernels (round 1's path)", 0, hps=1000, steps=3, kernel="general")
@@ -594,6 +599,8 @@ def main():
                     help="0: demag field recomputed in every Heun stage; P >= 1: every P-th step, held in between")
     ap.add_argument("--track-stray", action="store_true",
                     help="with --demag: also the stray field of the frozen track (DESIGN.md sec. 12, reading D4)")
+    ap.add_argument("--track-exchange", action="store_true",
+                    help="window ends exchange coupled to the frozen track (DESIGN.md sec. 10, reading E1)")
     ap.add_argument("--multiscale", action="store_true",
                     help="the multiscale window: a micromagnetic LLG mesh either side of the atomistic mesh (DESIGN.md sec. 14)")
     ap.add_argument("--mm-every", type=int, default=20, help="Heun steps per RK4 step of the meshes")

@@ -297,8 +297,7 @@ asd_status launch_heun_direct(Ctx& c, int64_t n, const DynState* dyn) {
   p.dyn = dyn;
   const bool vec4 = (c.d.ny % 4 == 0);
   // with the demagnetising field on, the film kernel assumes its 4 sites span at most two macrocells (my >= 3)
-  const bool fast = c.kernel_variant != ASD_KERNEL_GENERAL && heun_fast_supported(c) && !(c.demag && c.d.macro[1] < 3) &&
-                    !(c.demag && edge_field_on(c));
+  const bool fast = c.kernel_variant != ASD_KERNEL_GENERAL && heun_fast_supported(c) && !(c.demag && c.d.macro[1] < 3);
   if (c.kernel_variant == ASD_KERNEL_FAST && !fast) return ASD_EUNSUPPORTED;
   const bool staged = c.kernel_variant == ASD_KERNEL_TMA;
   if (staged && !(heun_tma_supported(c) && tma_plan(c))) return ASD_EUNSUPPORTED;
@@ -307,8 +306,8 @@ asd_status launch_heun_direct(Ctx& c, int64_t n, const DynState* dyn) {
   // one kernel per step: asked for, or AUTO on a film large enough to fill the machine with strip x chunk CTAs.
   // Not inside a recorded graph (the spin buffers swap roles every step) and not with the demagnetising field.
   // With the demagnetising field: only in the held-field scheme (asd_set_demag_every >= 1; the per-stage scheme needs the
-  // field of S~, a global quantity, between the two stages), macrocells of >= 3 sites across, no meshes.
-  const bool fused_dm_ok = !c.demag || (c.demag_every >= 1 && c.d.macro[1] >= 3 && !edge_field_on(c) && heun_fused_takes_demag(c));
+  // field of S~, a global quantity, between the two stages), macrocells of >= 3 sites across.
+  const bool fused_dm_ok = !c.demag || (c.demag_every >= 1 && c.d.macro[1] >= 3 && heun_fused_takes_demag(c, edge_field_on(c)));
   const bool fused = !dyn && fused_dm_ok && heun_fused_supported(c) &&
                      (c.kernel_variant == ASD_KERNEL_FUSED || (c.kernel_variant == ASD_KERNEL_AUTO && heun_fused_preferred(c))) &&
                      fused_plan(c) && (!edge_field_on(c) || heun_fused_takes_mm(c));

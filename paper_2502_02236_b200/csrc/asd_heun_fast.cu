@@ -271,7 +271,7 @@ asd_status launch_heun_fast(Ctx& c, StageParams& p) {
   f.dm = p.dm; f.dm_my = (uint32_t)c.d.macro[1];
   f.edgeB = p.edgeB;
   if (p.edgeB) {
-    if (p.dm.B) return ASD_EUNSUPPORTED;             // multiscale + demagnetising field: general kernel only
+    if (p.dm.B) return c.d.lattice == ASD_SC ? launch_pair_fast<LAT_SC, true, true>(c, f) : launch_pair_fast<LAT_L10, true, true>(c, f);
     return c.d.lattice == ASD_SC ? launch_pair_fast<LAT_SC, false, true>(c, f) : launch_pair_fast<LAT_L10, false, true>(c, f);
   }
   if (p.dm.B) return c.d.lattice == ASD_SC ? launch_pair_fast<LAT_SC, true>(c, f) : launch_pair_fast<LAT_L10, true>(c, f);

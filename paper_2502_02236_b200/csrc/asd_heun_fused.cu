@@ -714,8 +714,13 @@ constexpr int kNumShapes = 2;
 // Film thickness 27 planes with 32-site strips (BASELINE configs 1, 3, 4) has its own instance with compile-time shared-
 // memory offsets; everything else takes the generic one.
 FusedKernel kernel_for(int lattice, int shape, int nz, int by, bool mm = false, bool demag = false) {
-  if (demag) {                                          // held demagnetising field: the 256 x 2 shape only, no meshes
-    if (shape != 0 || mm) return nullptr;
+  if (demag) {                                          // held demagnetising field: the 256 x 2 shape only
+    if (shape != 0) return nullptr;
+    if (mm) {                                           // ... with meshes / track-coupled ends as well
+      if (nz == 27 && by == 32)
+        return lattice == ASD_SC ? heun_fused<LAT_SC, 256, 2, 27, 32, true, true> : heun_fused<LAT_L10, 256, 2, 27, 32, true, true>;
+      return lattice == ASD_SC ? heun_fused<LAT_SC, 256, 2, 0, 0, true, true> : heun_fused<LAT_L10, 256, 2, 0, 0, true, true>;
+    }
     if (nz == 27 && by == 32)
       return lattice == ASD_SC ? heun_fused<LAT_SC, 256, 2, 27, 32, false, true> : heun_fused<LAT_L10, 256, 2, 27, 32, false, true>;
     return lattice == ASD_SC ? heun_fused<LAT_SC, 256, 2, 0, 0, false, true> : heun_fused<LAT_L10, 256, 2, 0, 0, false, true>;
@@ -747,6 +752,7 @@ struct FusedPlan {
   FusedKernel kern = nullptr;
   FusedKernel kern_mm = nullptr;   // the instance that adds the mesh exchange field on planes 0 / nx-1 (asd_mm.cu); may be null
   FusedKernel kern_dm = nullptr;   // the instance that adds a held demagnetising field per macrocell; may be null
+  FusedKernel kern_dm_mm = nullptr;   // ... and the edge field as well; may be null
   int32_t BY = 0, G = 0, nstrips = 0, CX = 0, nchunks = 0, threads = 0, n_main = 0, ctas_per_sm = 0;
   uint32_t slot_pitch = 0, smem_bytes = 0;
   uint32_t smem_bytes_dm = 0;      // kern_dm: + the shared cell sums of the Eq. (6) epilogue (0: they do not fit; no epilogue)
@@ -831,6 +837,12 @@ bool build_plan(Ctx& c, FusedPlan& pl) {
     cudaGetLastError();
     pl.kern_dm = nullptr;
   }
+  pl.kern_dm_mm = kernel_for(c.d.lattice, best.shape, nz, pl.BY, true, true);
+  if (pl.kern_dm_mm && cudaFuncSetAttribute((const void*)pl.kern_dm_mm, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                            (int)std::max(pl.smem_bytes, pl.smem_bytes_dm)) != cudaSuccess) {
+    cudaGetLastError();
+    pl.kern_dm_mm = nullptr;
+  }
   int bps = 0;
   if (cudaFuncSetAttribute((const void*)pl.kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem_bytes) != cudaSuccess ||
       cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, (const void*)pl.kern, pl.threads, pl.smem_bytes) != cudaSuccess ||
@@ -866,7 +878,10 @@ bool build_plan(Ctx& c, FusedPlan& pl) {
 }  // namespace
 
 bool heun_fused_takes_mm(Ctx& c) { const FusedPlan* pl = fused_plan(c); return pl && pl->kern_mm; }
-bool heun_fused_takes_demag(Ctx& c) { const FusedPlan* pl = fused_plan(c); return pl && pl->kern_dm; }
+bool heun_fused_takes_demag(Ctx& c, bool with_edge_field) {
+  const FusedPlan* pl = fused_plan(c);
+  return pl && (with_edge_field ? pl->kern_dm_mm : pl->kern_dm);
+}
 
 FusedPlan* fused_plan(Ctx& c) {
   if (!c.fused_plan_tried) {
@@ -908,8 +923,8 @@ asd_status launch_heun_fused(Ctx& c, StageParams& p) {
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr; cfg.numAttrs = 1;
   f.dm = p.dm; f.dm_my = (uint32_t)c.d.macro[1];
-  if (f.edgeB && !pl->kern_mm) return ASD_EUNSUPPORTED;
-  if (f.dm.B && (!pl->kern_dm || f.edgeB || c.demag_every < 1)) return ASD_EUNSUPPORTED;
+  const FusedKernel kern = f.dm.B ? (f.edgeB ? pl->kern_dm_mm : pl->kern_dm) : (f.edgeB ? pl->kern_mm : pl->kern);
+  if (!kern || (f.dm.B && c.demag_every < 1)) return ASD_EUNSUPPORTED;
   // held-field scheme: the field of S is refreshed before the step when the cadence says so, then serves both stages
   // (from the cell sums the previous fused step left behind, when it did: demag_acc_arm below)
   if (f.dm.B && (c.demag_refresh & 1)) { const asd_status st = launch_demag(c, c.aS, true); if (st != ASD_OK) return st; }
@@ -919,7 +934,7 @@ asd_status launch_heun_fused(Ctx& c, StageParams& p) {
     f.dm_acc = demag_acc_arm(c, f.dm_fx);
     if (f.dm_acc) cfg.dynamicSmemBytes = pl->smem_bytes_dm;
   }
-  cudaLaunchKernelEx(&cfg, f.dm.B ? pl->kern_dm : (f.edgeB ? pl->kern_mm : pl->kern), pl->mapS, pl->mapF, f);
+  cudaLaunchKernelEx(&cfg, kern, pl->mapS, pl->mapF, f);
   ASD_LAUNCH_CHECK(c, "heun step (fused)");
   const int t = c.aS; c.aS = c.aSt; c.aSt = t;
   return ASD_OK;

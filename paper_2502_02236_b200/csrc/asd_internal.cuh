@@ -258,7 +258,7 @@ bool heun_fused_supported(const Ctx& c);
 bool heun_fused_preferred(Ctx& c);                            // what ASD_KERNEL_AUTO asks (builds the plan)
 FusedPlan* fused_plan(Ctx& c);
 bool heun_fused_takes_mm(Ctx& c);                             // the plan's CTA shape has a multiscale instance
-bool heun_fused_takes_demag(Ctx& c);                          // ... a held-demagnetising-field instance
+bool heun_fused_takes_demag(Ctx& c, bool with_edge_field = false);                          // ... a held-demagnetising-field instance
 asd_status launch_heun_persist(Ctx& c, StageParams& p, int64_t n);   // n Heun steps in one cluster launch (asd_heun_persist.cu)
 bool heun_persist_supported(const Ctx& c);
 bool heun_persist_preferred(const Ctx& c);                    // what ASD_KERNEL_AUTO asks (measured crossover vs graph replay)

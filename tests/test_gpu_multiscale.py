@@ -177,14 +177,19 @@ def test_full_size_multiscale_window_one_coupled_step():
 
 
 @pytest.mark.parametrize("lattice", [ai.SC, ai.L10])
-def test_multiscale_window_with_the_demagnetising_field(lattice):
-    """Meshes and the window's demagnetising field together (the general kernel carries both): coupled steps against the
-    oracle, per-stage and held-field schemes."""
-    for every_dm in (0, 2):
+@pytest.mark.parametrize("kernel", ["general", "fast", "fused", "auto"])
+def test_multiscale_window_with_the_demagnetising_field(lattice, kernel):
+    """Meshes and the window's demagnetising field together (general, film and -- held-field scheme -- fused kernels carry
+    both): coupled steps against the oracle, per-stage and held-field schemes."""
+    for every_dm in (0, 2, 1):
+        if kernel == "fused" and every_dm == 0:
+            continue                                                # the one-kernel step takes the held field only
         ms, o, g = _pair(lattice, every=2)
         sp = [a * 1e-9 for a in ms.w.spacing_nm]
         o.enable_demag(sp); g.enable_demag(sp)
         o.set_demag_every(every_dm); g.set_demag_every(every_dm)
+        if kernel != "auto":
+            g.set_kernel({"general": asd.KERNEL_GENERAL, "fast": asd.KERNEL_FAST, "fused": asd.KERNEL_FUSED}[kernel])
         o.step_heun(1); g.step_heun(1)
         assert np.abs(o.get_spins() - g.get_spins_host()).max() <= 1e-5
         o.step_heun(3); g.step_heun(3)

@@ -43,6 +43,31 @@ def test_coupled_ends_match_the_oracle(lattice, kernel):
     assert d[:, 0].max() > 1e-4 and d[:, -1].max() > 1e-4 and d[:, 1].max() < 1e-4 and not d[:, 2:-2].any()
 
 
+@pytest.mark.parametrize("lattice", [ai.SC, ai.L10])
+@pytest.mark.parametrize("kernel,every", [("general", 0), ("fast", 0), ("fast", 2), ("fused", 1), ("auto", 1)])
+def test_the_whole_window_of_p33(lattice, kernel, every):
+    """Everything P:33 puts on the window at once: ends exchange coupled to the frozen track, the window's own
+    demagnetising field and the track's stray field -- film and fused kernels carry the edge field and the cell field
+    together."""
+    w = ai.small_film(lattice, 20, 40, 6, extra_track=24, macro=(4, 5, 2), tilt_deg=25.0, dt=1e-16)
+    o, g = oracle_from_workload(w), gpu_from_workload(w)
+    rng = np.random.default_rng(5)
+    v = rng.standard_normal((int(np.prod(o.track_dims())), 3)).astype(np.float32)
+    o.track_set_init(v); g.track_set_init(v)
+    o.shift_window(3); g.shift_window(3)
+    sp = [a * 1e-9 for a in w.spacing_nm]
+    for c in (o, g):
+        c.enable_demag(sp); c.set_demag_every(every); c.enable_track_stray(True, 0); c.enable_track_exchange(True)
+    g.set_kernel(KERNELS[kernel])
+    o.step_heun(1); g.step_heun(1)
+    assert max_abs_diff(g, o) <= 1e-5
+    o.step_heun(4); g.step_heun(4)
+    assert max_abs_diff(g, o) <= 6e-5
+    o.shift_window(4); g.shift_window(4)
+    o.step_heun(3); g.step_heun(3)
+    assert max_abs_diff(g, o) <= 1.2e-4
+
+
 def test_refusals_and_switching_off():
     w = ai.small_film(ai.L10, 16, 24, 4, extra_track=16, macro=(4, 4, 2))
     g = gpu_from_workload(w)
