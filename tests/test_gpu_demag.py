@@ -214,5 +214,8 @@ def test_track_stray_needs_demag():
     w = ai.small_film(ai.SC, 12, 16, 4, extra_track=8)
     g = gpu_from_workload(w)
     with pytest.raises(asd.AsdError) as e:
+        g.demag_held_field()
+    assert e.value.status == 4
+    with pytest.raises(asd.AsdError) as e:
         g.enable_track_stray(True, 0)
     assert e.value.status == 4
