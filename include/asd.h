@@ -326,6 +326,21 @@ ASD_API asd_status asd_mm_get_m_host(asd_ctx *ctx, int32_t side, float *m);
 ASD_API asd_status asd_planes_view(asd_ctx *ctx, int32_t comp, int32_t i0, int32_t n, float **d_ptr, size_t *count);
 ASD_API asd_status asd_magnetisation_planes(asd_ctx *ctx, int32_t i0, int32_t n, double sum[3], double *n_magnetic);
 
+/* ---- A reduction that allocates nothing (csrc/asd_noalloc.cu) --------------------------------------------------------
+ * For callers that cannot call cudaMalloc or hand over a workspace: code under CUDA-graph capture, tight serving loops,
+ * harnesses that forbid allocation.  Needs no context.  The deterministic two-stage reduction of asd_magnetisation
+ * (Eq. (6)) over three DEVICE arrays of `count` floats each -- e.g. what asd_planes_view hands out; pad floats
+ * and vacant sites hold exact zeros -- written to DEVICE d_out4[4] = (sum S_x, sum S_y, sum S_z, number of elements that
+ * hold a spin: |S|^2 > 1/4), fp64.  Enqueued on cuda_stream (a cudaStream_t, NULL = default stream) of the CURRENT
+ * device; does not synchronise; the caller owns inputs and output.
+ * Its partial sums live in a static 64 KB array in device memory that every GPU loading the library holds until the
+ * process exits; hence count <= ASD_NOALLOC_MAX_COUNT (ASD_EINVAL beyond, also for NULL pointers or count == 0; message
+ * from asd_last_error(NULL)).  Every call on a device shares that array: calls that overlap on the GPU (different
+ * streams without an event between them) race; calls in one stream do not.  ASD_ECUDA without a device. */
+#define ASD_NOALLOC_MAX_COUNT 8388608
+ASD_API asd_status asd_spin_sum_noalloc(const float *d_sx, const float *d_sy, const float *d_sz, size_t count,
+                                        double *d_out4, void *cuda_stream);
+
 /* Counters for bit-exact checkpoint / resume (Philox is counter based: there is no RNG state). */
 ASD_API asd_status asd_get_counters(const asd_ctx *ctx, int64_t *step, int64_t *shift, int64_t *x0, int64_t *pass);
 ASD_API asd_status asd_set_counters(asd_ctx *ctx, int64_t step, int64_t shift, int64_t pass);

@@ -7,5 +7,5 @@ There is no CPU path: importing works anywhere, creating a context needs a CUDA 
 from .binding import (  # noqa: F401
     ASD_SC, ASD_L10_FE, AsdError, Context, LatticeDesc, lib_path, load_library, version, workspace_bytes,
     EXPORTED_SYMBOLS, KERNEL_AUTO, KERNEL_GENERAL, KERNEL_FAST, KERNEL_TMA, KERNEL_FUSED, KERNEL_PERSISTENT, GRAPH_AUTO, GRAPH_OFF, GRAPH_ON,
-    desc_from_workload, context_from_workload,
+    desc_from_workload, context_from_workload, spin_sum_noalloc, NOALLOC_MAX_COUNT,
 )

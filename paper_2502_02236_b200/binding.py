@@ -29,7 +29,7 @@ EXPORTED_SYMBOLS = [
     "asd_mm_get_m_host", "asd_planes_view", "asd_magnetisation_planes",
     "asd_track_stray_workspace_bytes", "asd_enable_track_stray", "asd_track_stray_field",
     "asd_track_exchange_workspace_bytes", "asd_enable_track_exchange", "asd_get_counters", "asd_set_counters",
-    "asd_launch_count", "asd_last_error", "asd_version",
+    "asd_spin_sum_noalloc", "asd_launch_count", "asd_last_error", "asd_version",
 ]
 
 
@@ -124,6 +124,7 @@ def load_library(build_if_missing: bool = True):
     L.asd_enable_track_exchange.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_size_t]
     L.asd_shift_window.argtypes = [C.c_void_p, C.c_int32]
     L.asd_magnetisation.argtypes = [C.c_void_p, dp, dp]
+    L.asd_spin_sum_noalloc.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p]
     L.asd_grain_magnetisation.argtypes = [C.c_void_p, dp]
     L.asd_track_dims.argtypes = [C.c_void_p, ip64]
     L.asd_track_set_init.argtypes = [C.c_void_p, C.c_void_p, C.c_float]
@@ -207,6 +208,27 @@ class LatticeDesc:
         d.ell_width = 0 if self.ell_idx is None else int(np.asarray(self.ell_idx).reshape(self.nx * self.ny * self.nz, -1).shape[1])
         d.seed = int(self.seed)
         return d, keep
+
+
+NOALLOC_MAX_COUNT = 8388608     # ASD_NOALLOC_MAX_COUNT (include/asd.h)
+
+
+def spin_sum_noalloc(sx, sy, sz, out4, stream=None) -> None:
+    """asd_spin_sum_noalloc: (sum S_x, sum S_y, sum S_z, number of spins) of three fp32 CUDA tensors into the fp64 CUDA
+    tensor out4[4], on `stream` (default: torch's current stream); allocates nothing, does not synchronise."""
+    import torch
+    L = load_library()
+    for t in (sx, sy, sz):
+        if not (t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.numel() == sx.numel()):
+            raise ValueError("sx, sy, sz: contiguous fp32 CUDA tensors of equal length")
+    if not (out4.is_cuda and out4.dtype == torch.float64 and out4.is_contiguous() and out4.numel() == 4):
+        raise ValueError("out4: contiguous fp64 CUDA tensor of 4 elements")
+    st = stream if stream is not None else torch.cuda.current_stream(sx.device)
+    with torch.cuda.device(sx.device):
+        rc = L.asd_spin_sum_noalloc(C.c_void_p(sx.data_ptr()), C.c_void_p(sy.data_ptr()), C.c_void_p(sz.data_ptr()),
+                                    C.c_size_t(sx.numel()), C.c_void_p(out4.data_ptr()), C.c_void_p(st.cuda_stream))
+    if rc != 0:
+        raise AsdError(rc, L.asd_last_error(None).decode())
 
 
 def workspace_bytes(desc: LatticeDesc) -> int:

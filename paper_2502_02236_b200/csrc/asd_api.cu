@@ -11,6 +11,7 @@ namespace asd {
 
 // message of the last failure that has no context to carry it (create, NULL ctx); per thread, not process-wide
 static thread_local const char* g_static_err = "no error";
+void set_static_error(const char* msg) { g_static_err = msg; }   // for entry points outside this file (asd_noalloc.cu)
 
 bool validate_desc(const asd_lattice_desc* d, const char** why) {
   auto bad = [&](const char* m) { if (why) *why = m; return false; };
